@@ -1,0 +1,133 @@
+/* ringx.h -- C ABI of libringx: the single-GPU hot path of RingX sequence-parallel attention
+ * (arXiv 2507.16697, "Pixel-Resolved Long-Context Learning for Turbulence at Exascale"),
+ * hand-written for NVIDIA B200 (sm_100a: TMA + tcgen05.mma + TMEM).
+ *
+ * What the path computes (citations are /root/reference/PAPER.md lines):
+ *   - exact, non-causal softmax attention  A^s = sum_i Softmax(Q_s . K_i^T) V_i   (Eq. 1, l.89),
+ *     evaluated through the log-sum-exp  LSE_s = log sum_i exp(e_i^s), e_i^s = Q_s . K_i^T
+ *     (Eq. 3-4, l.124-126);
+ *   - split over key/value chunks S_i whose partial results (loc_out_i, loc_lse_i) are combined by
+ *       num = sum_i loc_out_i exp(loc_lse_i - lse_max),  den = sum_i exp(loc_lse_i - lse_max),
+ *       A = num/den                                              (Eq. 5, l.130-133; l.137, l.143);
+ *     on one GPU the "ring" over devices is a loop over KV-chunk passes (RingX_b with the
+ *     all-gather replaced by "K,V already resident", l.145);
+ *   - the backward pass: dK,dV complete per KV chunk, dQ "accumulated ... over N steps" (l.143).
+ *
+ * Conventions that hold for every entry point
+ *   Layout     All tensors are contiguous [B,H,N,d], d fastest (the head-split layout
+ *              (b*a, S, h/a) of Table II, l.188).  lse is [B,H,N] float.
+ *   Pointers   Unless a parameter says HOST, every pointer is a DEVICE pointer, 16-byte aligned.
+ *   Ownership  The caller owns every buffer.  The library never allocates or frees device
+ *              memory and keeps no pointer after a call returns.  Scratch space is the
+ *              caller-provided `workspace`, sized by the *_workspace_bytes queries.
+ *   Streams    All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy
+ *              default stream).  Calls return after enqueue; there is no host synchronisation
+ *              (ringx_attn_fwd_host is the exception: it synchronises `stream` before returning).
+ *   Errors     Return value is a ringx_status (0 = RINGX_OK).  Arguments are validated before the
+ *              first launch: an error other than RINGX_ERR_CUDA means nothing was enqueued and no
+ *              output was touched.  No abort, no printf, no exceptions cross this boundary.
+ *   Domain     d in {64, 128}; N % 128 == 0; kv_chunk % 128 == 0; 0 < kv_chunk <= N;
+ *              N % kv_chunk == 0 (every device holds an equal chunk S/N, l.128).  bf16 kernels also
+ *              need N % 256 == 0 (one CTA owns two 128-row query tiles).  Anything else returns
+ *              RINGX_ERR_BAD_SHAPE -- never a silently wrong answer.  A device that is not
+ *              compute capability 10.x returns RINGX_ERR_UNSUPPORTED_ARCH.
+ *   Semantics  Non-causal, no mask, no dropout, no bias.  `scale` multiplies Q.K^T before the
+ *              softmax (Eq. 1/4 print no 1/sqrt(d); it is explicit here); it must be finite and
+ *              > 0 (anything else: RINGX_ERR_BAD_SHAPE).  lse is the natural-log
+ *              LSE of the *scaled* scores.  bf16 outputs are rounded to nearest even once, at the
+ *              end; partial results between chunk passes are fp32.
+ *   Threads    Functions are re-entrant.
+ */
+#ifndef RINGX_H_
+#define RINGX_H_
+
+#include <stddef.h>
+
+#if defined(__GNUC__)
+#define RINGX_API __attribute__((visibility("default")))
+#else
+#define RINGX_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  RINGX_OK = 0,
+  RINGX_ERR_NULL_PTR = 1,
+  RINGX_ERR_BAD_SHAPE = 2,
+  RINGX_ERR_BAD_DTYPE = 3,
+  RINGX_ERR_MISALIGNED = 4,
+  RINGX_ERR_WORKSPACE_TOO_SMALL = 5,
+  RINGX_ERR_UNSUPPORTED_ARCH = 6,
+  RINGX_ERR_CUDA = 7
+} ringx_status;
+
+typedef enum { RINGX_F32 = 0, RINGX_BF16 = 1 } ringx_dtype;
+
+/* Forward (Eq. 1 via Eq. 5).  For c = 0 .. N/kv_chunk-1: one chunk pass computes
+ * (loc_out_c, loc_lse_c) of every query row against keys [c*kv_chunk, (c+1)*kv_chunk); partials
+ * are folded left to right with the two-operand Eq. 5 (ringx_lse_merge) in fp32.
+ *   q,k,v  [B,H,N,d] of `dtype` (in).   o [B,H,N,d] of `dtype` (out).   lse [B,H,N] float (out).
+ *   dtype  RINGX_BF16: tcgen05 tensor-core path, fp32 accumulation (mixed fp32/bf16, l.286).
+ *          RINGX_F32 : plain FFMA path (max abs error ~1e-6; tf32 would not meet 1e-5).
+ *   workspace  >= ringx_attn_fwd_workspace_bytes(...) bytes, 256-byte aligned; may be NULL when
+ *              that query returns 0 (kv_chunk == N with bf16).  Contents are scratch. */
+RINGX_API int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* lse,
+                   int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
+                   void* workspace, size_t workspace_bytes, void* stream);
+
+/* Backward of L = sum dO.O (derivative of Eq. 1; data-flow of l.143).  bf16 only, d = 64 or 128.
+ * P is recomputed from the saved *global* lse; each KV-chunk pass writes that chunk's dK,dV once
+ * (atomic-free: a CTA owns a 128-key tile) and adds its contribution to dQ in an fp32 accumulator
+ * ("accumulated ... over N steps"); dQ summation order is not deterministic.
+ *   q,k,v,o,dO [B,H,N,d] bf16 (in), lse [B,H,N] float (in, as written by ringx_attn_fwd).
+ *   dq,dk,dv   [B,H,N,d] bf16 (out); must not alias any input.
+ *   workspace  >= ringx_attn_bwd_workspace_bytes(...) bytes, 256-byte aligned. */
+RINGX_API int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                   const void* dO, void* dq, void* dk, void* dv,
+                   int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
+                   void* workspace, size_t workspace_bytes, void* stream);
+
+/* Two-operand Eq. 5, row by row:  m = max(lse_a,lse_b); w_a = exp(lse_a-m); w_b = exp(lse_b-m);
+ * o_out = (w_a o_a + w_b o_b)/(w_a+w_b);  lse_out = m + log(w_a+w_b).
+ * An operand with lse = -inf has weight 0; both -inf gives o_out = 0, lse_out = -inf; NaN propagates.
+ *   o_a,o_b [rows,d] of o_in_dtype; o_out [rows,d] of o_out_dtype; lse_* [rows] float.
+ *   o_out may alias o_a (same dtype) and lse_out may alias lse_a: the merge runs in place.
+ *   d % 8 == 0, 8 <= d <= 1024; rows >= 0 (rows == 0 is a no-op). */
+RINGX_API int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b,
+                    void* o_out, float* lse_out, long long rows, int d,
+                    int o_in_dtype, int o_out_dtype, void* stream);
+
+/* One KV-chunk pass on its own: (loc_out, loc_lse) of `Nq` query rows per head against `Nk` keys
+ * (l.135) -- the per-device step of RingX_a/RingX_b with Nq != Nk allowed.
+ *   q [B,H,Nq,d], k,v [B,H,Nk,d] of `dtype`; loc_out [B,H,Nq,d] FLOAT; loc_lse [B,H,Nq] float.
+ *   Nq % 256 == 0 (bf16) or % 128 (f32), Nk % 128 == 0, d in {64,128}.  No workspace. */
+RINGX_API int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse,
+                         int B, int H, int Nq, int Nk, int d, float scale, int dtype, void* stream);
+
+/* ringx_attn_fwd with HOST buffers (the end-to-end entry): copies q,k,v host->device into the
+ * workspace, runs ringx_attn_fwd, copies o and lse back, and synchronises `stream`.
+ *   q_host,k_host,v_host,o_host,lse_host  HOST pointers (pinned memory recommended).
+ *   workspace  DEVICE, >= ringx_attn_fwd_host_workspace_bytes(...) bytes. */
+RINGX_API int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_host,
+                        void* o_host, float* lse_host,
+                        int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
+                        void* workspace, size_t workspace_bytes, void* stream);
+
+RINGX_API size_t ringx_attn_fwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
+RINGX_API size_t ringx_attn_bwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
+RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
+
+/* Number of kernel launches the last successful call on this thread enqueued (bench.py's
+ * `gpu_launches` claim is counted here, not guessed). */
+RINGX_API int ringx_last_launch_count(void);
+
+RINGX_API const char* ringx_status_string(int status);
+RINGX_API int ringx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RINGX_H_ */

@@ -1,0 +1,350 @@
+// api.cu -- the C-ABI layer of libringx (include/ringx.h): argument validation, workspace carving,
+// TMA tensor-map creation and the KV-chunk pass loop.  No arithmetic of the method lives here; every
+// step of the path runs in the kernels this file launches.
+#include <mutex>
+
+#include "kernels.cuh"
+
+namespace ringx {
+
+namespace {
+
+thread_local int tl_launches = 0;
+thread_local int tl_last_launches = 0;
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                              const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                              CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeFn encode_fn() {
+  static EncodeFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+        qr == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeFn>(p);
+  });
+  return fn;
+}
+
+// RINGX_OK when the current device is compute capability 10.x.
+int check_arch() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return RINGX_ERR_CUDA;
+  }
+  static std::mutex mu;
+  static int cached[64];   // 0 = unknown, 1 = ok, 2 = unsupported
+  std::lock_guard<std::mutex> g(mu);
+  if (dev >= 0 && dev < 64 && cached[dev]) return cached[dev] == 1 ? RINGX_OK : RINGX_ERR_UNSUPPORTED_ARCH;
+  int major = 0;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return RINGX_ERR_CUDA;
+  }
+  if (dev >= 0 && dev < 64) cached[dev] = (major == 10) ? 1 : 2;
+  return major == 10 ? RINGX_OK : RINGX_ERR_UNSUPPORTED_ARCH;
+}
+
+int check_shape(int B, int H, int N, int d, int kv_chunk, float scale, int dtype, bool backward) {
+  if (dtype != RINGX_F32 && dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (backward && dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (B <= 0 || H <= 0 || N <= 0 || kv_chunk <= 0) return RINGX_ERR_BAD_SHAPE;
+  if (d != 64 && d != 128) return RINGX_ERR_BAD_SHAPE;
+  if (N % 128 || kv_chunk % 128 || kv_chunk > N || N % kv_chunk) return RINGX_ERR_BAD_SHAPE;
+  if (dtype == RINGX_BF16 && !backward && N % 256) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * H > 65535) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * H * N > 0x7FFFFFFFLL) return RINGX_ERR_BAD_SHAPE;   // TMA row coordinate is int32
+  if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
+  return RINGX_OK;
+}
+
+struct FwdWorkspace {
+  float* o_acc = nullptr;      // running (merged) output, fp32 [R,d]   (bf16 only; f32 uses `o` itself)
+  float* lse_acc = nullptr;    // running LSE [R]                        (bf16 only; f32 uses `lse`)
+  float* o_part = nullptr;     // loc_out of the current pass, fp32 [R,d]
+  float* lse_part = nullptr;   // loc_lse of the current pass [R]
+  size_t bytes = 0;
+};
+
+FwdWorkspace carve_fwd(void* ws, int B, int H, int N, int d, int kv_chunk, int dtype) {
+  FwdWorkspace w;
+  if (kv_chunk == N) return w;   // single pass: the chunk kernel writes (o, lse) directly
+  const size_t R = (size_t)B * H * N;
+  char* p = static_cast<char*>(ws);
+  size_t off = 0;
+  auto take = [&](size_t n) {
+    char* r = p ? p + off : nullptr;
+    off += align_up(n);
+    return r;
+  };
+  if (dtype == RINGX_BF16) {
+    w.o_acc = reinterpret_cast<float*>(take(R * d * sizeof(float)));
+    w.lse_acc = reinterpret_cast<float*>(take(R * sizeof(float)));
+  }
+  w.o_part = reinterpret_cast<float*>(take(R * d * sizeof(float)));
+  w.lse_part = reinterpret_cast<float*>(take(R * sizeof(float)));
+  w.bytes = off;
+  return w;
+}
+
+struct BwdWorkspace {
+  float* D = nullptr;        // D_i = dO_i . O_i, [R]
+  float* dq_acc = nullptr;   // fp32 dQ accumulator [R,d]
+  size_t bytes = 0;
+};
+
+BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
+  BwdWorkspace w;
+  const size_t R = (size_t)B * H * N;
+  char* p = static_cast<char*>(ws);
+  w.D = reinterpret_cast<float*>(p);
+  size_t off = align_up(R * sizeof(float));
+  w.dq_acc = reinterpret_cast<float*>(p ? p + off : nullptr);
+  off += align_up(R * d * sizeof(float));
+  w.bytes = off;
+  return w;
+}
+
+int cuda_status(cudaError_t e) {
+  if (e == cudaSuccess) return RINGX_OK;
+  cudaGetLastError();
+  return RINGX_ERR_CUDA;
+}
+
+}  // namespace
+
+void count_launch(int n) { tl_launches += n; }
+
+bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t rows,
+                  uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz) {
+  EncodeFn enc = encode_fn();
+  if (!enc) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols * (uint64_t)elem_bytes};
+  cuuint32_t box[2] = {box_cols, box_rows};
+  cuuint32_t es[2] = {1, 1};
+  CUresult r = enc(out, dt, 2, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   swz == kSwizzle128B ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+// One KV-chunk pass, either dtype.  o_out: fp32 partial, or the final dtype when `final_out`.
+static cudaError_t chunk_pass(const void* q, const void* k, const void* v, void* o_out, float* lse_out, int BH, int Nq,
+                              int nk_stride, int k_off, int nk, int d, float scale, int dtype, bool final_out,
+                              cudaStream_t stream) {
+  if (dtype == RINGX_F32)
+    return launch_attn_chunk_f32(static_cast<const float*>(q), static_cast<const float*>(k),
+                                 static_cast<const float*>(v), static_cast<float*>(o_out), lse_out, BH, Nq, nk_stride,
+                                 k_off, nk, d, scale, stream);
+  return launch_attn_chunk_fwd_sm100(q, k, v, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, d, scale,
+                                     final_out ? 1 : 0, stream);
+}
+
+}  // namespace ringx
+
+using namespace ringx;
+
+extern "C" {
+
+size_t ringx_attn_fwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false) != RINGX_OK) return 0;
+  return carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype).bytes;
+}
+
+size_t ringx_attn_bwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, true) != RINGX_OK) return 0;
+  return carve_bwd(nullptr, B, H, N, d).bytes;
+}
+
+size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false) != RINGX_OK) return 0;
+  const size_t e = dtype == RINGX_F32 ? 4 : 2;
+  const size_t R = (size_t)B * H * N;
+  return 4 * align_up(R * d * e) + align_up(R * sizeof(float)) + carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype).bytes;
+}
+
+int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* lse, int B, int H, int N, int d,
+                   int kv_chunk, float scale, int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o || !lse) return RINGX_ERR_NULL_PTR;
+  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false);
+  if (st != RINGX_OK) return st;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse)) return RINGX_ERR_MISALIGNED;
+  const FwdWorkspace need = carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype);
+  if (need.bytes) {
+    if (!workspace) return RINGX_ERR_NULL_PTR;
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+    if (workspace_bytes < need.bytes) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  }
+  if ((st = check_arch()) != RINGX_OK) return st;
+
+  tl_launches = 0;
+  const int BH = B * H;
+  const long long R = (long long)BH * N;
+  const int n_chunks = N / kv_chunk;
+  if (n_chunks == 1) {
+    cudaError_t e = chunk_pass(q, k, v, o, lse, BH, N, N, 0, N, d, scale, dtype, true, stream);
+    if (e != cudaSuccess) return cuda_status(e);
+    tl_last_launches = tl_launches;
+    return RINGX_OK;
+  }
+  const FwdWorkspace w = carve_fwd(workspace, B, H, N, d, kv_chunk, dtype);
+  // running accumulator: fp32 for both dtypes (f32 accumulates straight into the caller's o/lse)
+  float* o_acc = dtype == RINGX_F32 ? static_cast<float*>(o) : w.o_acc;
+  float* lse_acc = dtype == RINGX_F32 ? lse : w.lse_acc;
+  for (int c = 0; c < n_chunks; ++c) {
+    const bool first = c == 0, last = c == n_chunks - 1;
+    cudaError_t e = chunk_pass(q, k, v, first ? o_acc : w.o_part, first ? lse_acc : w.lse_part, BH, N, N,
+                               c * kv_chunk, kv_chunk, d, scale, dtype, false, stream);
+    if (e != cudaSuccess) return cuda_status(e);
+    if (first) continue;
+    // Eq. 5, two operands, folded left to right; the last fold writes the caller's dtype
+    const bool to_out = last && dtype == RINGX_BF16;
+    e = launch_lse_merge(o_acc, lse_acc, w.o_part, w.lse_part, to_out ? o : o_acc, to_out ? lse : lse_acc, R, d,
+                         RINGX_F32, to_out ? RINGX_BF16 : RINGX_F32, stream);
+    count_launch();
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse, int B, int H,
+                         int Nq, int Nk, int d, float scale, int dtype, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !loc_out || !loc_lse) return RINGX_ERR_NULL_PTR;
+  if (dtype != RINGX_F32 && dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
+  if (Nk % 128 || Nq % (dtype == RINGX_BF16 ? 256 : 128)) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
+    return RINGX_ERR_BAD_SHAPE;
+  if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(loc_out) || !aligned16(loc_lse))
+    return RINGX_ERR_MISALIGNED;
+  int st = check_arch();
+  if (st != RINGX_OK) return st;
+  tl_launches = 0;
+  cudaError_t e = chunk_pass(q, k, v, loc_out, loc_lse, B * H, Nq, Nk, 0, Nk, d, scale, dtype, false, stream);
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b, void* o_out,
+                    float* lse_out, long long rows, int d, int o_in_dtype, int o_out_dtype, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (rows < 0 || d < 8 || d > 1024 || d % 8) return RINGX_ERR_BAD_SHAPE;
+  if ((o_in_dtype != RINGX_F32 && o_in_dtype != RINGX_BF16) || (o_out_dtype != RINGX_F32 && o_out_dtype != RINGX_BF16))
+    return RINGX_ERR_BAD_DTYPE;
+  if (rows == 0) {
+    tl_last_launches = 0;
+    return RINGX_OK;
+  }
+  if (!o_a || !lse_a || !o_b || !lse_b || !o_out || !lse_out) return RINGX_ERR_NULL_PTR;
+  if (!aligned16(o_a) || !aligned16(o_b) || !aligned16(o_out)) return RINGX_ERR_MISALIGNED;
+  if ((reinterpret_cast<uintptr_t>(lse_a) | reinterpret_cast<uintptr_t>(lse_b) |
+       reinterpret_cast<uintptr_t>(lse_out)) & 3u)
+    return RINGX_ERR_MISALIGNED;
+  tl_launches = 0;
+  cudaError_t e = launch_lse_merge(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, o_in_dtype, o_out_dtype, stream);
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
+                   void* dq, void* dk, void* dv, int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
+                   void* workspace, size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o || !lse || !dO || !dq || !dk || !dv) return RINGX_ERR_NULL_PTR;
+  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, true);
+  if (st != RINGX_OK) return st;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse) || !aligned16(dO) ||
+      !aligned16(dq) || !aligned16(dk) || !aligned16(dv))
+    return RINGX_ERR_MISALIGNED;
+  const BwdWorkspace need = carve_bwd(nullptr, B, H, N, d);
+  if (!workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < need.bytes) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  if ((st = check_arch()) != RINGX_OK) return st;
+
+  tl_launches = 0;
+  const int BH = B * H;
+  const long long R = (long long)BH * N;
+  const BwdWorkspace w = carve_bwd(workspace, B, H, N, d);
+  cudaError_t e = launch_bwd_preprocess(o, dO, w.D, w.dq_acc, R, d, stream);
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  for (int c = 0; c < N / kv_chunk; ++c) {
+    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse, w.D, w.dq_acc, dk, dv, BH, N, c * kv_chunk, kv_chunk, d, scale,
+                                    stream);
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  e = launch_dq_convert(w.dq_acc, dq, R * d, scale, stream);
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_host, void* o_host, float* lse_host,
+                        int B, int H, int N, int d, int kv_chunk, float scale, int dtype, void* workspace,
+                        size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q_host || !k_host || !v_host || !o_host || !lse_host) return RINGX_ERR_NULL_PTR;
+  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false);
+  if (st != RINGX_OK) return st;
+  const size_t need = ringx_attn_fwd_host_workspace_bytes(B, H, N, d, kv_chunk, dtype);
+  if (!workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < need) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  const size_t e = dtype == RINGX_F32 ? 4 : 2;
+  const size_t R = (size_t)B * H * N;
+  const size_t tb = R * d * e, tba = align_up(tb);
+  char* p = static_cast<char*>(workspace);
+  void *dq = p, *dk = p + tba, *dv = p + 2 * tba, *dob = p + 3 * tba;
+  float* dlse = reinterpret_cast<float*>(p + 4 * tba);
+  char* inner = p + 4 * tba + align_up(R * sizeof(float));
+  const size_t inner_bytes = workspace_bytes - (size_t)(inner - p);
+  cudaError_t ce;
+  if ((ce = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaMemcpyAsync(dk, k_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaMemcpyAsync(dv, v_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+  st = ringx_attn_fwd(dq, dk, dv, dob, dlse, B, H, N, d, kv_chunk, scale, dtype, inner, inner_bytes, stream_);
+  if (st != RINGX_OK) return st;
+  if ((ce = cudaMemcpyAsync(o_host, dob, tb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaMemcpyAsync(lse_host, dlse, R * sizeof(float), cudaMemcpyDeviceToHost, stream)) != cudaSuccess)
+    return cuda_status(ce);
+  if ((ce = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_status(ce);
+  return RINGX_OK;
+}
+
+int ringx_last_launch_count(void) { return tl_last_launches; }
+
+const char* ringx_status_string(int status) {
+  switch (status) {
+    case RINGX_OK: return "ok";
+    case RINGX_ERR_NULL_PTR: return "null pointer";
+    case RINGX_ERR_BAD_SHAPE: return "unsupported shape or scale (see include/ringx.h, Domain)";
+    case RINGX_ERR_BAD_DTYPE: return "unsupported dtype";
+    case RINGX_ERR_MISALIGNED: return "pointer not sufficiently aligned";
+    case RINGX_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case RINGX_ERR_UNSUPPORTED_ARCH: return "device is not compute capability 10.x (sm_100a)";
+    case RINGX_ERR_CUDA: return "CUDA runtime error";
+    default: return "unknown status";
+  }
+}
+
+int ringx_version(void) { return 100; }
+
+}  // extern "C"

@@ -1,0 +1,314 @@
+// attn_fwd_sm100.cu -- one KV-chunk pass of the forward on tcgen05 tensor cores.
+//
+// For every query row of a [128 x 2]-row CTA tile and the keys [k_off, k_off + nk) of its head:
+//   loc_out = softmax(scale q K_c^T) V_c,  loc_lse = log sum_j exp(scale q.k_j)      (Eq. 1/3/4)
+// bf16 operands, fp32 accumulation ("mixed float32-bfloat16").
+//
+// Structure (one CTA per SM, 320 threads):
+//   warps 0-3   softmax warpgroup of query tile 0 (thread = one query row; owns TMEM lane = row)
+//   warps 4-7   softmax warpgroup of query tile 1
+//   warp  8     TMA producer: Q tiles once, then the K/V ring (K_0, V_0, K_1, V_1, ...)
+//   warp  9     MMA issuer (one elected lane): S_t = Q_t K_j^T (SS), O_t += P_t V_j (P from TMEM)
+// TMEM columns: S_0 [0,128) S_1 [128,256) O_0 [256,256+d) O_1 [256+d,256+2d); P_t (bf16) overwrites
+// the first 64 columns of S_t.  The two query tiles ping-pong: while warpgroup t turns S_t into P_t the
+// tensor core works on tile 1-t.  The MMA pipe executes in issue order, so S_t(j+1) -- issued right after
+// O_t += P_t(j) V_j -- cannot overwrite P_t(j) early, and the commit that signals S_t(j+1) also proves
+// O_t(j) complete: the softmax warps may rescale O_t in place without a further barrier.
+// Online softmax in the exp2 domain with a lazy running max (O, l are only rescaled when the row max
+// grew by more than 2^8), so the rescale is off the common path.
+#include "kernels.cuh"
+
+namespace ringx {
+namespace {
+
+using namespace ptx;
+
+constexpr int kBlockM = 128;          // query rows per tile (= TMEM lanes)
+constexpr int kBlockN = 128;          // keys per KV tile
+constexpr int kFwdThreads = 320;
+constexpr float kRescaleThreshold = 8.0f;   // log2 units
+
+template <int kD>
+struct FwdCfg {
+  static constexpr int kPanels = kD / 64;                    // 64 bf16 = one 128-byte swizzle row
+  static constexpr int kPanelBytes = 128 * 128;              // 128 rows x 128 B
+  static constexpr int kTileBytes = kPanels * kPanelBytes;   // Q, K or V tile
+  static constexpr int kStages = kD == 128 ? 5 : 8;          // K/V ring slots
+  static constexpr int kBarBytes = 256;
+  static constexpr int kSmemBytes = 1024 + 2 * kTileBytes + kStages * kTileBytes + kBarBytes;
+};
+
+template <int kD, bool kOutBf16>
+__global__ void __launch_bounds__(kFwdThreads, 1)
+attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
+                      const __grid_constant__ CUtensorMap map_v, void* __restrict__ o_out,
+                      float* __restrict__ lse_out, int Nq, int nk_stride, int k_off, int n_kv, float scale_log2) {
+  using Cfg = FwdCfg<kD>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* sQ = smem;
+  uint8_t* sKV = smem + 2 * Cfg::kTileBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + Cfg::kStages * Cfg::kTileBytes);
+  uint64_t* q_full = bars;                  // [2]  TMA -> MMA
+  uint64_t* s_full = bars + 2;              // [2]  MMA -> softmax: S_t(j) in TMEM
+  uint64_t* p_full = bars + 4;              // [2]  softmax -> MMA: P_t(j) in TMEM (O_t rescaled if needed)
+  uint64_t* o_full = bars + 6;              // [2]  MMA -> softmax: last O_t complete
+  uint64_t* kv_full = bars + 8;             // [kStages]
+  uint64_t* kv_empty = bars + 8 + Cfg::kStages;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 8 + 2 * Cfg::kStages);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int bh = blockIdx.y;
+  const int q_row0 = bh * Nq + blockIdx.x * (2 * kBlockM);     // row in the [BH*Nq, d] view
+  const int k_row0 = bh * nk_stride + k_off;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&q_full[i], 1);
+      mbar_init(&s_full[i], 1);
+      mbar_init(&p_full[i], kBlockM);
+      mbar_init(&o_full[i], 1);
+    }
+    for (int i = 0; i < Cfg::kStages; ++i) {
+      mbar_init(&kv_full[i], 1);
+      mbar_init(&kv_empty[i], 1);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 8) {
+    if (lane == 0) {
+      prefetch_tmap(&map_q);
+      prefetch_tmap(&map_k);
+      prefetch_tmap(&map_v);
+    }
+    tmem_alloc<512>(tmem_slot);
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+
+  if (warp == 8) {
+    // ------------------------------------------------------------------ TMA producer
+    if (lane == 0) {
+      const uint64_t pol_q = policy_evict_first();
+      const uint64_t pol_kv = policy_evict_last();
+      auto load_tile = [&](uint8_t* dst, const CUtensorMap* map, uint64_t* bar, int row, uint64_t pol) {
+        mbar_arrive_expect_tx(bar, Cfg::kTileBytes);
+#pragma unroll
+        for (int p = 0; p < Cfg::kPanels; ++p) tma_load_2d(dst + p * Cfg::kPanelBytes, map, bar, p * 64, row, pol);
+      };
+      load_tile(sQ, &map_q, &q_full[0], q_row0, pol_q);
+      int stage = 0, phase = 0;
+      for (int i = 0; i < 2 * n_kv; ++i) {      // ring order K_0, V_0, K_1, V_1, ...
+        mbar_wait(&kv_empty[stage], phase ^ 1);
+        load_tile(sKV + stage * Cfg::kTileBytes, (i & 1) ? &map_v : &map_k, &kv_full[stage],
+                  k_row0 + (i >> 1) * kBlockN, pol_kv);
+        if (i == 0) load_tile(sQ + Cfg::kTileBytes, &map_q, &q_full[1], q_row0 + kBlockM, pol_q);
+        if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
+      }
+    }
+  } else if (warp == 9) {
+    // ------------------------------------------------------------------ MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc_s = make_idesc_bf16(kBlockM, kBlockN, 0, 0);    // Q (K-major) x K^T (K-major)
+      constexpr uint32_t idesc_o = make_idesc_bf16(kBlockM, kD, 0, 1);         // P (TMEM) x V (MN-major)
+      const uint32_t q_addr = smem_u32(sQ), kv_addr = smem_u32(sKV);
+      int stage = 0, phase = 0;
+      auto advance = [&]() { if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; } };
+      // S_t = Q_t K^T from the K tile in ring slot `st`
+      auto issue_s = [&](int t, int st) {
+        const uint32_t a0 = q_addr + t * Cfg::kTileBytes, b0 = kv_addr + st * Cfg::kTileBytes;
+#pragma unroll
+        for (int k = 0; k < kD / 16; ++k) {
+          const uint32_t off = (k >> 2) * Cfg::kPanelBytes + (k & 3) * 32;
+          mma_ss(tmem + t * kBlockN, make_smem_desc_sw128(a0 + off, 16, 1024), make_smem_desc_sw128(b0 + off, 16, 1024),
+                 idesc_s, k > 0);
+        }
+        mma_commit(&s_full[t]);
+      };
+      // O_t (+)= P_t V from the V tile in ring slot `st`
+      auto issue_o = [&](int t, int st, bool accumulate) {
+        const uint32_t b0 = kv_addr + st * Cfg::kTileBytes;
+#pragma unroll
+        for (int k = 0; k < kBlockN / 16; ++k)
+          mma_ts(tmem + 256 + t * kD, tmem + t * kBlockN + k * 8,
+                 make_smem_desc_sw128(b0 + k * 2048, Cfg::kPanelBytes, 1024), idesc_o, accumulate || k > 0);
+      };
+      // prologue: S_0(0), S_1(0)
+      mbar_wait(&kv_full[stage], phase);
+      mbar_wait(&q_full[0], 0);
+      tc_fence_after();
+      issue_s(0, stage);
+      mbar_wait(&q_full[1], 0);
+      tc_fence_after();
+      issue_s(1, stage);
+      mma_commit(&kv_empty[stage]);
+      advance();
+      for (int j = 0; j < n_kv; ++j) {
+        const int v_stage = stage, v_phase = phase;
+        advance();
+        const int k_stage = stage, k_phase = phase;
+        const bool more = j + 1 < n_kv;
+        if (more) advance();
+        mbar_wait(&kv_full[v_stage], v_phase);
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          mbar_wait(&p_full[t], j & 1);
+          tc_fence_after();
+          issue_o(t, v_stage, j > 0);
+          if (t == 1) mma_commit(&kv_empty[v_stage]);
+          if (more) {
+            if (t == 0) {
+              mbar_wait(&kv_full[k_stage], k_phase);
+              tc_fence_after();
+            }
+            issue_s(t, k_stage);
+            if (t == 1) mma_commit(&kv_empty[k_stage]);
+          } else {
+            mma_commit(&o_full[t]);
+          }
+        }
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------ softmax warpgroups
+    const int t = warp >> 2;
+    const uint32_t lane_off = static_cast<uint32_t>((warp & 3) * 32) << 16;
+    const uint32_t tS = tmem + t * kBlockN + lane_off;
+    const uint32_t tO = tmem + 256 + t * kD + lane_off;
+    float m_raw = -CUDART_INF_F;   // running (lazy) row max of the unscaled scores
+    float m_sc = -CUDART_INF_F;    // m_raw * scale_log2
+    float l = 0.f;                 // running row sum of exp2(s*scale_log2 - m_sc)
+    for (int j = 0; j < n_kv; ++j) {
+      mbar_wait(&s_full[t], j & 1);
+      tc_fence_after();
+      uint32_t s[kBlockN];
+#pragma unroll
+      for (int c = 0; c < kBlockN / 32; ++c) tmem_ld_x32(tS + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
+      tmem_wait_ld();
+      float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]),
+            mx3 = __uint_as_float(s[3]);
+#pragma unroll
+      for (int i = 4; i < kBlockN; i += 4) {
+        mx0 = fmaxf(mx0, __uint_as_float(s[i]));
+        mx1 = fmaxf(mx1, __uint_as_float(s[i + 1]));
+        mx2 = fmaxf(mx2, __uint_as_float(s[i + 2]));
+        mx3 = fmaxf(mx3, __uint_as_float(s[i + 3]));
+      }
+      const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+      const bool grow = (mx - m_raw) * scale_log2 > kRescaleThreshold;
+      if (__any_sync(0xffffffffu, grow)) {
+        const float m_new = fmaxf(m_raw, mx);
+        const float alpha = ex2((m_raw - m_new) * scale_log2);   // 0 on the first tile (m_raw = -inf)
+        l *= alpha;
+        if (j > 0) {
+#pragma unroll
+          for (int c = 0; c < kD / 32; ++c) {
+            uint32_t o[32];
+            tmem_ld_x32(tO + c * 32, o);
+            tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st_x32(tO + c * 32, o);
+          }
+        }
+        m_raw = m_new;
+        m_sc = m_new * scale_log2;
+      }
+      float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+#pragma unroll
+      for (int c = 0; c < kBlockN / 32; ++c) {
+        uint32_t pk[16];
+#pragma unroll
+        for (int i = 0; i < 32; i += 4) {
+          const float p0 = ex2(fmaf(__uint_as_float(s[c * 32 + i]), scale_log2, -m_sc));
+          const float p1 = ex2(fmaf(__uint_as_float(s[c * 32 + i + 1]), scale_log2, -m_sc));
+          const float p2 = ex2(fmaf(__uint_as_float(s[c * 32 + i + 2]), scale_log2, -m_sc));
+          const float p3 = ex2(fmaf(__uint_as_float(s[c * 32 + i + 3]), scale_log2, -m_sc));
+          l0 += p0; l1 += p1; l2 += p2; l3 += p3;
+          pk[i / 2] = pack_bf16x2(p0, p1);
+          pk[i / 2 + 1] = pack_bf16x2(p2, p3);
+        }
+        tmem_st_x16(tS + c * 16, pk);
+      }
+      l += (l0 + l1) + (l2 + l3);
+      tmem_wait_st();
+      tc_fence_before();
+      mbar_arrive(&p_full[t]);
+    }
+    // ---- chunk epilogue: loc_out = O / l, loc_lse = m*scale + ln l  (natural log of the scaled scores)
+    mbar_wait(&o_full[t], 0);
+    tc_fence_after();
+    const float inv = 1.0f / l;
+    const size_t row = static_cast<size_t>(q_row0) + t * kBlockM + (warp & 3) * 32 + lane;
+#pragma unroll
+    for (int c = 0; c < kD / 32; ++c) {
+      uint32_t o[32];
+      tmem_ld_x32(tO + c * 32, o);
+      tmem_wait_ld();
+      if (kOutBf16) {
+        uint4* dst = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(o_out) + row * kD + c * 32);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          uint4 u;
+          u.x = pack_bf16x2(__uint_as_float(o[i * 8 + 0]) * inv, __uint_as_float(o[i * 8 + 1]) * inv);
+          u.y = pack_bf16x2(__uint_as_float(o[i * 8 + 2]) * inv, __uint_as_float(o[i * 8 + 3]) * inv);
+          u.z = pack_bf16x2(__uint_as_float(o[i * 8 + 4]) * inv, __uint_as_float(o[i * 8 + 5]) * inv);
+          u.w = pack_bf16x2(__uint_as_float(o[i * 8 + 6]) * inv, __uint_as_float(o[i * 8 + 7]) * inv);
+          dst[i] = u;
+        }
+      } else {
+        float4* dst = reinterpret_cast<float4*>(static_cast<float*>(o_out) + row * kD + c * 32);
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          dst[i] = make_float4(__uint_as_float(o[i * 4]) * inv, __uint_as_float(o[i * 4 + 1]) * inv,
+                               __uint_as_float(o[i * 4 + 2]) * inv, __uint_as_float(o[i * 4 + 3]) * inv);
+      }
+    }
+    lse_out[row] = (m_sc + lg2(l)) * 0.6931471805599453f;
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 8) tmem_dealloc<512>(tmem);
+}
+
+template <int kD, bool kOutBf16>
+cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, void* o_out, float* lse_out,
+                     int BH, int Nq, int nk_stride, int k_off, int nk, float scale, cudaStream_t stream) {
+  using Cfg = FwdCfg<kD>;
+  auto kern = attn_chunk_fwd_kernel<kD, kOutBf16>;
+  static bool configured = false;   // benign race: the attribute is idempotent
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  dim3 grid(Nq / (2 * kBlockM), BH);
+  kern<<<grid, kFwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, Nq, nk_stride, k_off,
+                                                       nk / kBlockN, scale * 1.4426950408889634f);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
+                                        int BH, int Nq, int nk_stride, int k_off, int nk, int d, float scale,
+                                        int out_bf16, cudaStream_t stream) {
+  CUtensorMap mq, mk, mv;
+  const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+  if (!make_tmap_2d(&mq, q, dt, 2, (uint64_t)BH * Nq, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mk, k, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mv, v, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B))
+    return cudaErrorInvalidValue;
+  if (d == 64)
+    return out_bf16 ? launch_t<64, true>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream)
+                    : launch_t<64, false>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream);
+  return out_bf16 ? launch_t<128, true>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream)
+                  : launch_t<128, false>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream);
+}
+
+}  // namespace ringx

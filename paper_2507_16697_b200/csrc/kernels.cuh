@@ -1,0 +1,47 @@
+// kernels.cuh -- internal launch interface between the C-ABI layer (api.cu) and the kernels.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "../../include/ringx.h"
+#include "ptx.cuh"
+
+namespace ringx {
+
+// ---- merge.cu (HBM-bound helpers)
+cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b, void* o_out,
+                             float* lse_out, long long rows, int d, int in_dtype, int out_dtype, cudaStream_t stream);
+cudaError_t launch_bwd_preprocess(const void* o, const void* dO, float* D, float* dq_acc, long long rows, int d,
+                                  cudaStream_t stream);
+cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
+
+// ---- attn_f32.cu (plain FFMA path, config C1)
+// One KV-chunk pass, fp32: q [BH,Nq,d], k/v [BH,nk_stride,d] rows [k_off, k_off+nk) -> o_out fp32, lse_out.
+cudaError_t launch_attn_chunk_f32(const float* q, const float* k, const float* v, float* o_out, float* lse_out, int BH,
+                                  int Nq, int nk_stride, int k_off, int nk, int d, float scale, cudaStream_t stream);
+
+// ---- attn_fwd_sm100.cu (tcgen05 path)
+// One KV-chunk pass, bf16 in / fp32 accumulate.  out_bf16 = 0: o_out is float [BH,Nq,d] (a partial,
+// loc_out); out_bf16 = 1: o_out is bf16 (single-pass final result).
+cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
+                                        int BH, int Nq, int nk_stride, int k_off, int nk, int d, float scale,
+                                        int out_bf16, cudaStream_t stream);
+
+// ---- attn_bwd_sm100.cu (tcgen05 path)
+// One KV-chunk pass of the backward: writes dk,dv rows [k_off, k_off+nk) of every head (bf16),
+// reduce-adds this chunk's contribution into dq_acc (fp32 [BH,N,d], unscaled by `scale`).
+cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse,
+                                        const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
+                                        int nk, int d, float scale, cudaStream_t stream);
+
+// ---- tensor maps (api.cu): 2-D row-major [rows, cols] view, box = {box_cols, box_rows}
+enum TmapSwizzle { kSwizzleNone = 0, kSwizzle128B = 1 };
+bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t rows,
+                  uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz);
+
+void count_launch(int n = 1);
+
+}  // namespace ringx

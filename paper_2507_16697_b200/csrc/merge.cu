@@ -1,0 +1,239 @@
+// merge.cu -- HBM-bound helper kernels of the RingX hot path:
+//   lse_merge_kernel   two-operand Eq. (5): SURVEY.md §8(a) row a5/a6
+//   bwd_preprocess     D_i = sum_c dO_ic O_ic and zeroing of the fp32 dQ accumulator: row a7
+//   dq_convert         dq = bf16(scale * dq_acc): row a9
+// Roofline: HBM bandwidth.  Algorithmic bytes per row: merge 2*(d*e_in+4) read + (d*e_out+4)
+// written; preprocess 2*d*2 read + 4 written (+ d*4 zeroed); convert d*4 read + d*2 written.
+#include "kernels.cuh"
+
+namespace ringx {
+
+namespace {
+
+constexpr int kMergeThreads = 256;
+constexpr int kRowUnroll = 4;
+
+template <typename T>
+struct Vec4;  // 4 consecutive elements of a row
+template <>
+struct Vec4<float> {
+  static __device__ __forceinline__ float4 load(const void* p, size_t i4) {
+    return __ldcs(reinterpret_cast<const float4*>(p) + i4);
+  }
+  static __device__ __forceinline__ void store(void* p, size_t i4, float4 v) {
+    __stcs(reinterpret_cast<float4*>(p) + i4, v);
+  }
+};
+template <>
+struct Vec4<__nv_bfloat16> {
+  static __device__ __forceinline__ float4 load(const void* p, size_t i4) {
+    uint2 u = __ldcs(reinterpret_cast<const uint2*>(p) + i4);
+    float4 v;
+    v.x = __uint_as_float(u.x << 16);
+    v.y = __uint_as_float(u.x & 0xFFFF0000u);
+    v.z = __uint_as_float(u.y << 16);
+    v.w = __uint_as_float(u.y & 0xFFFF0000u);
+    return v;
+  }
+  static __device__ __forceinline__ void store(void* p, size_t i4, float4 v) {
+    uint2 u;
+    u.x = ptx::pack_bf16x2(v.x, v.y);
+    u.y = ptx::pack_bf16x2(v.z, v.w);
+    __stcs(reinterpret_cast<uint2*>(p) + i4, u);
+  }
+};
+
+// Weights of the two-operand Eq. (5).  -inf operands get weight 0 (reading g12).
+__device__ __forceinline__ void merge_weights(float la, float lb, float& wa, float& wb, float& lse) {
+  const float m = fmaxf(la, lb);
+  if (m == -INFINITY) {
+    wa = 0.f; wb = 0.f; lse = -INFINITY;
+    return;
+  }
+  const float ea = expf(la - m), eb = expf(lb - m);   // exp(-inf) = 0; NaN propagates
+  const float den = ea + eb;
+  const float inv = 1.0f / den;
+  wa = ea * inv;
+  wb = eb * inv;
+  lse = m + logf(den);
+}
+
+// One group of kLanes lanes owns a row (d/4 = kLanes * iters vectors).  A warp owns 32/kLanes rows
+// per step and kRowUnroll steps are in flight, so the lse read, the two o reads and the write of a
+// row all come from one warp: running in place on operand a is race-free.
+template <typename TIn, typename TOut, int kLanes>
+__global__ void __launch_bounds__(kMergeThreads)
+lse_merge_kernel(const void* __restrict__ o_a, const float* lse_a, const void* __restrict__ o_b,
+                 const float* __restrict__ lse_b, void* o_out, float* lse_out, long long rows, int d) {
+  constexpr int kRowsPerWarp = 32 / kLanes;
+  const int lane = threadIdx.x & 31;
+  const int sub = lane / kLanes, l = lane % kLanes;
+  const int vecs = d >> 2;
+  const long long warp_global = (long long)blockIdx.x * (kMergeThreads / 32) + (threadIdx.x >> 5);
+  const long long warp_count = (long long)gridDim.x * (kMergeThreads / 32);
+  const long long rows_per_iter = (long long)kRowsPerWarp * kRowUnroll;
+  for (long long base = warp_global * rows_per_iter; base < rows; base += warp_count * rows_per_iter) {
+    float wa[kRowUnroll], wb[kRowUnroll], lse[kRowUnroll];
+    long long row[kRowUnroll];
+#pragma unroll
+    for (int u = 0; u < kRowUnroll; ++u) {
+      row[u] = base + u * kRowsPerWarp + sub;
+      float la = -INFINITY, lb = -INFINITY;
+      if (row[u] < rows) {
+        la = lse_a[row[u]];
+        lb = lse_b[row[u]];
+      }
+      merge_weights(la, lb, wa[u], wb[u], lse[u]);
+    }
+    for (int v0 = 0; v0 < vecs; v0 += kLanes) {
+      const int v = v0 + l;
+      float4 a[kRowUnroll], b[kRowUnroll];
+#pragma unroll
+      for (int u = 0; u < kRowUnroll; ++u)
+        if (row[u] < rows && v < vecs) {
+          a[u] = Vec4<TIn>::load(o_a, (size_t)row[u] * vecs + v);
+          b[u] = Vec4<TIn>::load(o_b, (size_t)row[u] * vecs + v);
+        }
+#pragma unroll
+      for (int u = 0; u < kRowUnroll; ++u)
+        if (row[u] < rows && v < vecs) {
+          float4 r;
+          // weight-0 operands are skipped so that garbage (even NaN) behind an empty chunk is ignored
+          r.x = (wa[u] != 0.f ? wa[u] * a[u].x : 0.f) + (wb[u] != 0.f ? wb[u] * b[u].x : 0.f);
+          r.y = (wa[u] != 0.f ? wa[u] * a[u].y : 0.f) + (wb[u] != 0.f ? wb[u] * b[u].y : 0.f);
+          r.z = (wa[u] != 0.f ? wa[u] * a[u].z : 0.f) + (wb[u] != 0.f ? wb[u] * b[u].z : 0.f);
+          r.w = (wa[u] != 0.f ? wa[u] * a[u].w : 0.f) + (wb[u] != 0.f ? wb[u] * b[u].w : 0.f);
+          Vec4<TOut>::store(o_out, (size_t)row[u] * vecs + v, r);
+        }
+    }
+    __syncwarp();   // every lane has read lse_a of its rows before lane 0 of the group overwrites it
+#pragma unroll
+    for (int u = 0; u < kRowUnroll; ++u)
+      if (row[u] < rows && l == 0) lse_out[row[u]] = lse[u];
+  }
+}
+
+template <typename TIn, typename TOut>
+cudaError_t launch_merge_t(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b, void* o_out,
+                           float* lse_out, long long rows, int d, cudaStream_t stream) {
+  const int vecs = d / 4;
+  int lanes = 32;
+  if (vecs < 32 && (vecs & (vecs - 1)) == 0) lanes = vecs;
+  const long long rows_per_block = (long long)(kMergeThreads / 32) * (32 / lanes) * kRowUnroll;
+  long long blocks = (rows + rows_per_block - 1) / rows_per_block;
+  const long long max_blocks = 148LL * 8 * 4;   // 8 CTAs of 256 threads per SM, 4 waves
+  if (blocks > max_blocks) blocks = max_blocks;
+  if (blocks < 1) blocks = 1;
+#define RINGX_MERGE_CASE(L)                                                                                     \
+  case L:                                                                                                       \
+    lse_merge_kernel<TIn, TOut, L><<<(unsigned)blocks, kMergeThreads, 0, stream>>>(o_a, lse_a, o_b, lse_b, o_out, \
+                                                                                   lse_out, rows, d);           \
+    break;
+  switch (lanes) {
+    RINGX_MERGE_CASE(2)
+    RINGX_MERGE_CASE(4)
+    RINGX_MERGE_CASE(8)
+    RINGX_MERGE_CASE(16)
+    default:
+      lse_merge_kernel<TIn, TOut, 32><<<(unsigned)blocks, kMergeThreads, 0, stream>>>(o_a, lse_a, o_b, lse_b, o_out,
+                                                                                      lse_out, rows, d);
+  }
+#undef RINGX_MERGE_CASE
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------- backward helpers
+// D_i = sum_c dO_ic * O_ic (fp32), one 16-lane (d=64: 8 B/lane... ) group per row: each lane takes
+// 8 bf16 (16 B) of dO and of O; d/8 lanes per row.  Also zeroes the row of the fp32 dQ accumulator.
+template <int kLanes>
+__global__ void __launch_bounds__(256)
+bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO, float* __restrict__ D,
+                      float4* __restrict__ dq_acc, long long rows) {
+  constexpr int kRowsPerWarp = 32 / kLanes;
+  const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
+  const long long warp_global = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const long long warp_count = (long long)gridDim.x * 8;
+  for (long long base = warp_global * kRowsPerWarp * 4; base < rows; base += warp_count * kRowsPerWarp * 4) {
+    uint4 a[4], b[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const long long r = base + u * kRowsPerWarp + sub;
+      if (r < rows) {
+        a[u] = __ldg(o + r * kLanes + l);
+        b[u] = __ldg(dO + r * kLanes + l);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const long long r = base + u * kRowsPerWarp + sub;
+      float s = 0.f;
+      if (r < rows) {
+        const uint32_t* pa = reinterpret_cast<const uint32_t*>(&a[u]);
+        const uint32_t* pb = reinterpret_cast<const uint32_t*>(&b[u]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          s = fmaf(__uint_as_float(pa[i] << 16), __uint_as_float(pb[i] << 16), s);
+          s = fmaf(__uint_as_float(pa[i] & 0xFFFF0000u), __uint_as_float(pb[i] & 0xFFFF0000u), s);
+        }
+        const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+        dq_acc[(r * kLanes + l) * 2] = z;
+        dq_acc[(r * kLanes + l) * 2 + 1] = z;
+      }
+#pragma unroll
+      for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+      if (r < rows && l == 0) D[r] = s;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256)
+dq_convert_kernel(const float4* __restrict__ dq_acc, uint2* __restrict__ dq, long long n4, float scale) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+    const float4 v = __ldcs(dq_acc + i);
+    uint2 u;
+    u.x = ptx::pack_bf16x2(v.x * scale, v.y * scale);
+    u.y = ptx::pack_bf16x2(v.z * scale, v.w * scale);
+    dq[i] = u;
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b, void* o_out,
+                             float* lse_out, long long rows, int d, int in_dtype, int out_dtype,
+                             cudaStream_t stream) {
+  if (rows == 0) return cudaSuccess;
+  if (in_dtype == RINGX_F32 && out_dtype == RINGX_F32)
+    return launch_merge_t<float, float>(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, stream);
+  if (in_dtype == RINGX_F32 && out_dtype == RINGX_BF16)
+    return launch_merge_t<float, __nv_bfloat16>(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, stream);
+  if (in_dtype == RINGX_BF16 && out_dtype == RINGX_F32)
+    return launch_merge_t<__nv_bfloat16, float>(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, stream);
+  return launch_merge_t<__nv_bfloat16, __nv_bfloat16>(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, stream);
+}
+
+cudaError_t launch_bwd_preprocess(const void* o, const void* dO, float* D, float* dq_acc, long long rows, int d,
+                                  cudaStream_t stream) {
+  const int lanes = d / 8;   // 8 or 16
+  const long long rows_per_block = 8LL * (32 / lanes) * 4;
+  long long blocks = (rows + rows_per_block - 1) / rows_per_block;
+  if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
+  if (lanes == 8)
+    bwd_preprocess_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, D,
+                                                                   (float4*)dq_acc, rows);
+  else
+    bwd_preprocess_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, D,
+                                                                    (float4*)dq_acc, rows);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream) {
+  const long long n4 = n / 4;
+  long long blocks = (n4 + 255) / 256;
+  if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
+  dq_convert_kernel<<<(unsigned)blocks, 256, 0, stream>>>((const float4*)dq_acc, (uint2*)dq, n4, scale);
+  return cudaGetLastError();
+}
+
+}  // namespace ringx

@@ -1,0 +1,190 @@
+"""Thin ctypes binding over libringx.so -- same names as include/ringx.h, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; this file allocates outputs/workspace with
+torch (device memory and streams are what PyTorch is used for here) and passes raw pointers.  There
+is no CPU fallback: a missing library or a non-CUDA tensor raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from .build import LIB_PATH
+
+RINGX_F32, RINGX_BF16 = 0, 1
+_DTYPES = {torch.float32: RINGX_F32, torch.bfloat16: RINGX_BF16}
+_lib = None
+
+
+class RingxError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().ringx_status_string(status).decode()
+        super().__init__(f"{where}: {msg} (ringx_status {status})")
+
+
+def lib() -> ctypes.CDLL:
+    """Load libringx.so (built in-tree by `python -m paper_2507_16697_b200.build`).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2507_16697_b200.build` "
+            "(there is no CPU or PyTorch fallback for the RingX hot path)")
+    L = ctypes.CDLL(LIB_PATH)
+    c_p, c_i, c_f, c_sz, c_ll = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t, ctypes.c_longlong
+    L.ringx_attn_fwd.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_fwd.restype = c_i
+    L.ringx_attn_fwd_host.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_fwd_host.restype = c_i
+    L.ringx_attn_bwd.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_bwd.restype = c_i
+    L.ringx_lse_merge.argtypes = [c_p] * 6 + [c_ll, c_i, c_i, c_i, c_p]
+    L.ringx_lse_merge.restype = c_i
+    L.ringx_attn_chunk_fwd.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p]
+    L.ringx_attn_chunk_fwd.restype = c_i
+    for name in ("ringx_attn_fwd_workspace_bytes", "ringx_attn_bwd_workspace_bytes",
+                 "ringx_attn_fwd_host_workspace_bytes"):
+        getattr(L, name).argtypes = [c_i] * 6
+        getattr(L, name).restype = c_sz
+    L.ringx_last_launch_count.argtypes = []
+    L.ringx_last_launch_count.restype = c_i
+    L.ringx_status_string.argtypes = [c_i]
+    L.ringx_status_string.restype = ctypes.c_char_p
+    L.ringx_version.argtypes = []
+    L.ringx_version.restype = c_i
+    _lib = L
+    return L
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise RingxError(status, where)
+
+
+def _dev(t: torch.Tensor, name: str) -> int:
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous [B,H,N,d]")
+    return t.data_ptr()
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _workspace(nbytes: int, device) -> torch.Tensor | None:
+    return torch.empty(nbytes, dtype=torch.uint8, device=device) if nbytes else None
+
+
+def ringx_attn_fwd_workspace_bytes(B, H, N, d, kv_chunk, dtype) -> int:
+    return lib().ringx_attn_fwd_workspace_bytes(B, H, N, d, kv_chunk, _DTYPES[dtype])
+
+
+def ringx_attn_bwd_workspace_bytes(B, H, N, d, kv_chunk, dtype) -> int:
+    return lib().ringx_attn_bwd_workspace_bytes(B, H, N, d, kv_chunk, _DTYPES[dtype])
+
+
+def ringx_attn_fwd_host_workspace_bytes(B, H, N, d, kv_chunk, dtype) -> int:
+    return lib().ringx_attn_fwd_host_workspace_bytes(B, H, N, d, kv_chunk, _DTYPES[dtype])
+
+
+def ringx_attn_fwd(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, workspace=None):
+    """O, LSE = chunked attention of q,k,v [B,H,N,d] (include/ringx.h: ringx_attn_fwd)."""
+    B, H, N, d = q.shape
+    dt = _DTYPES[q.dtype]
+    if o is None:
+        o = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    need = lib().ringx_attn_fwd_workspace_bytes(B, H, N, d, kv_chunk, dt)
+    if workspace is None:
+        workspace = _workspace(need, q.device)
+    ws_ptr = workspace.data_ptr() if workspace is not None else None
+    ws_len = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    st = lib().ringx_attn_fwd(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                              B, H, N, d, kv_chunk, scale, dt, ws_ptr, ws_len, _stream())
+    _check(st, "ringx_attn_fwd")
+    return o, lse
+
+
+def ringx_attn_chunk_fwd(q, k, v, scale: float):
+    """(loc_out fp32, loc_lse) of q [B,H,Nq,d] against the keys k,v [B,H,Nk,d] (one chunk pass)."""
+    B, H, Nq, d = q.shape
+    Nk = k.shape[2]
+    loc_out = torch.empty((B, H, Nq, d), dtype=torch.float32, device=q.device)
+    loc_lse = torch.empty((B, H, Nq), dtype=torch.float32, device=q.device)
+    st = lib().ringx_attn_chunk_fwd(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(loc_out, "loc_out"),
+                                    _dev(loc_lse, "loc_lse"), B, H, Nq, Nk, d, scale, _DTYPES[q.dtype], _stream())
+    _check(st, "ringx_attn_chunk_fwd")
+    return loc_out, loc_lse
+
+
+def ringx_lse_merge(o_a, lse_a, o_b, lse_b, out_dtype=None, inplace: bool = False):
+    """Two-operand Eq. 5 on [..., d] partials (include/ringx.h: ringx_lse_merge)."""
+    d = o_a.shape[-1]
+    rows = o_a.numel() // d if d else 0
+    out_dtype = o_a.dtype if out_dtype is None else out_dtype
+    if inplace:
+        if out_dtype != o_a.dtype:
+            raise ValueError("in-place merge keeps the dtype of operand a")
+        o_out, lse_out = o_a, lse_a
+    else:
+        o_out = torch.empty(o_a.shape, dtype=out_dtype, device=o_a.device)
+        lse_out = torch.empty_like(lse_a)
+    st = lib().ringx_lse_merge(_dev(o_a, "o_a"), _dev(lse_a, "lse_a"), _dev(o_b, "o_b"), _dev(lse_b, "lse_b"),
+                               _dev(o_out, "o_out"), _dev(lse_out, "lse_out"), rows, d, _DTYPES[o_a.dtype],
+                               _DTYPES[out_dtype], _stream())
+    _check(st, "ringx_lse_merge")
+    return o_out, lse_out
+
+
+def ringx_attn_bwd(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspace=None):
+    """dQ, dK, dV (bf16) from the saved (o, lse) of ringx_attn_fwd (include/ringx.h: ringx_attn_bwd)."""
+    B, H, N, d = q.shape
+    dt = _DTYPES[q.dtype]
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    need = lib().ringx_attn_bwd_workspace_bytes(B, H, N, d, kv_chunk, dt)
+    if workspace is None:
+        workspace = _workspace(max(need, 256), q.device)
+    st = lib().ringx_attn_bwd(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                              _dev(dO, "dO"), _dev(dq, "dq"), _dev(dk, "dk"), _dev(dv, "dv"),
+                              B, H, N, d, kv_chunk, scale, dt, workspace.data_ptr(),
+                              workspace.numel() * workspace.element_size(), _stream())
+    _check(st, "ringx_attn_bwd")
+    return dq, dk, dv
+
+
+def ringx_attn_fwd_host(q_host, k_host, v_host, kv_chunk: int, scale: float, o_host=None, lse_host=None,
+                        workspace=None, device="cuda"):
+    """End-to-end entry with HOST tensors (pinned recommended): H2D, forward, D2H, synchronise."""
+    B, H, N, d = q_host.shape
+    dt = _DTYPES[q_host.dtype]
+    for t in (q_host, k_host, v_host):
+        if t.is_cuda or not t.is_contiguous():
+            raise ValueError("ringx_attn_fwd_host takes contiguous HOST tensors")
+    if o_host is None:
+        o_host = torch.empty_like(q_host).pin_memory()
+    if lse_host is None:
+        lse_host = torch.empty((B, H, N), dtype=torch.float32).pin_memory()
+    need = lib().ringx_attn_fwd_host_workspace_bytes(B, H, N, d, kv_chunk, dt)
+    if workspace is None:
+        workspace = _workspace(need, device)
+    with torch.cuda.device(workspace.device):
+        st = lib().ringx_attn_fwd_host(q_host.data_ptr(), k_host.data_ptr(), v_host.data_ptr(), o_host.data_ptr(),
+                                       lse_host.data_ptr(), B, H, N, d, kv_chunk, scale, dt, workspace.data_ptr(),
+                                       workspace.numel(), _stream())
+    _check(st, "ringx_attn_fwd_host")
+    return o_host, lse_host
+
+
+def ringx_last_launch_count() -> int:
+    return lib().ringx_last_launch_count()
+
+
+def ringx_version() -> int:
+    return lib().ringx_version()
