@@ -124,6 +124,18 @@ RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d,
  * `gpu_launches` claim is counted here, not guessed). */
 RINGX_API int ringx_last_launch_count(void);
 
+/* Optional live per-kernel timing on the calling thread (bench.py's roofline figure).  While enabled,
+ * every kernel launch the library makes is bracketed by two CUDA events on the caller's stream (the
+ * events are host objects created lazily and reused; no device memory is allocated).
+ * ringx_profile_read synchronises on the recorded events, adds the elapsed milliseconds and launch
+ * counts per kind into ms[RINGX_PROFILE_KINDS] / launches[RINGX_PROFILE_KINDS] (HOST arrays), and
+ * forgets the records.  Kinds: attention forward chunk kernel, Eq. 5 merge kernel, attention
+ * backward chunk kernel, backward helpers (D_i preprocess and dQ convert). */
+enum { RINGX_PROFILE_ATTN_FWD = 0, RINGX_PROFILE_MERGE = 1, RINGX_PROFILE_ATTN_BWD = 2, RINGX_PROFILE_BWD_AUX = 3,
+       RINGX_PROFILE_KINDS = 4 };
+RINGX_API int ringx_profile_enable(int on);
+RINGX_API int ringx_profile_read(double* ms, int* launches);
+
 RINGX_API const char* ringx_status_string(int status);
 RINGX_API int ringx_version(void);
 

@@ -2,6 +2,7 @@
 // TMA tensor-map creation and the KV-chunk pass loop.  No arithmetic of the method lives here; every
 // step of the path runs in the kernels this file launches.
 #include <mutex>
+#include <vector>
 
 #include "kernels.cuh"
 
@@ -113,6 +114,33 @@ BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
   return w;
 }
 
+// ---- optional live per-kernel timing (ringx_profile_*): CUDA events around each launch, per thread
+struct Profile {
+  bool on = false;
+  std::vector<cudaEvent_t> pool;     // start/stop pairs, reused across reads
+  std::vector<int> kinds;            // kind of pair i (events pool[2i], pool[2i+1])
+};
+thread_local Profile tl_prof;
+
+struct Timed {   // RAII: brackets the launches made during its lifetime
+  cudaStream_t stream;
+  cudaEvent_t stop = nullptr;
+  Timed(int kind, cudaStream_t s) : stream(s) {
+    Profile& p = tl_prof;
+    if (!p.on) return;
+    const size_t i = p.kinds.size();
+    while (p.pool.size() < 2 * (i + 1)) {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return; }
+      p.pool.push_back(e);
+    }
+    p.kinds.push_back(kind);
+    cudaEventRecord(p.pool[2 * i], stream);
+    stop = p.pool[2 * i + 1];
+  }
+  ~Timed() { if (stop) cudaEventRecord(stop, stream); }
+};
+
 int cuda_status(cudaError_t e) {
   if (e == cudaSuccess) return RINGX_OK;
   cudaGetLastError();
@@ -141,6 +169,7 @@ bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, in
 static cudaError_t chunk_pass(const void* q, const void* k, const void* v, void* o_out, float* lse_out, int BH, int Nq,
                               int nk_stride, int k_off, int nk, int d, float scale, int dtype, bool final_out,
                               cudaStream_t stream) {
+  Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
   if (dtype == RINGX_F32)
     return launch_attn_chunk_f32(static_cast<const float*>(q), static_cast<const float*>(k),
                                  static_cast<const float*>(v), static_cast<float*>(o_out), lse_out, BH, Nq, nk_stride,
@@ -209,6 +238,7 @@ int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* 
     if (first) continue;
     // Eq. 5, two operands, folded left to right; the last fold writes the caller's dtype
     const bool to_out = last && dtype == RINGX_BF16;
+    Timed timed(RINGX_PROFILE_MERGE, stream);
     e = launch_lse_merge(o_acc, lse_acc, w.o_part, w.lse_part, to_out ? o : o_acc, to_out ? lse : lse_acc, R, d,
                          RINGX_F32, to_out ? RINGX_BF16 : RINGX_F32, stream);
     count_launch();
@@ -255,7 +285,11 @@ int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const 
        reinterpret_cast<uintptr_t>(lse_out)) & 3u)
     return RINGX_ERR_MISALIGNED;
   tl_launches = 0;
-  cudaError_t e = launch_lse_merge(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, o_in_dtype, o_out_dtype, stream);
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_MERGE, stream);
+    e = launch_lse_merge(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, o_in_dtype, o_out_dtype, stream);
+  }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
   tl_last_launches = tl_launches;
@@ -282,15 +316,23 @@ int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, c
   const int BH = B * H;
   const long long R = (long long)BH * N;
   const BwdWorkspace w = carve_bwd(workspace, B, H, N, d);
-  cudaError_t e = launch_bwd_preprocess(o, dO, w.D, w.dq_acc, R, d, stream);
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = launch_bwd_preprocess(o, dO, w.D, w.dq_acc, R, d, stream);
+  }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
   for (int c = 0; c < N / kv_chunk; ++c) {
+    Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
     e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse, w.D, w.dq_acc, dk, dv, BH, N, c * kv_chunk, kv_chunk, d, scale,
                                     stream);
     if (e != cudaSuccess) return cuda_status(e);
   }
-  e = launch_dq_convert(w.dq_acc, dq, R * d, scale, stream);
+  {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = launch_dq_convert(w.dq_acc, dq, R * d, scale, stream);
+  }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
   tl_last_launches = tl_launches;
@@ -330,6 +372,32 @@ int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_ho
 }
 
 int ringx_last_launch_count(void) { return tl_last_launches; }
+
+int ringx_profile_enable(int on) {
+  tl_prof.on = on != 0;
+  tl_prof.kinds.clear();
+  return RINGX_OK;
+}
+
+int ringx_profile_read(double* ms, int* launches) {
+  if (!ms || !launches) return RINGX_ERR_NULL_PTR;
+  for (int i = 0; i < RINGX_PROFILE_KINDS; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  Profile& p = tl_prof;
+  int st = RINGX_OK;
+  for (size_t i = 0; i < p.kinds.size(); ++i) {
+    float t = 0.f;
+    if (cudaEventSynchronize(p.pool[2 * i + 1]) != cudaSuccess ||
+        cudaEventElapsedTime(&t, p.pool[2 * i], p.pool[2 * i + 1]) != cudaSuccess) {
+      cudaGetLastError();
+      st = RINGX_ERR_CUDA;
+      continue;
+    }
+    ms[p.kinds[i]] += t;
+    launches[p.kinds[i]] += 1;
+  }
+  p.kinds.clear();
+  return st;
+}
 
 const char* ringx_status_string(int status) {
   switch (status) {

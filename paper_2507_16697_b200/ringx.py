@@ -52,6 +52,10 @@ def lib() -> ctypes.CDLL:
         getattr(L, name).restype = c_sz
     L.ringx_last_launch_count.argtypes = []
     L.ringx_last_launch_count.restype = c_i
+    L.ringx_profile_enable.argtypes = [c_i]
+    L.ringx_profile_enable.restype = c_i
+    L.ringx_profile_read.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(c_i)]
+    L.ringx_profile_read.restype = c_i
     L.ringx_status_string.argtypes = [c_i]
     L.ringx_status_string.restype = ctypes.c_char_p
     L.ringx_version.argtypes = []
@@ -184,6 +188,21 @@ def ringx_attn_fwd_host(q_host, k_host, v_host, kv_chunk: int, scale: float, o_h
 
 def ringx_last_launch_count() -> int:
     return lib().ringx_last_launch_count()
+
+
+PROFILE_KINDS = ("attn_fwd", "merge", "attn_bwd", "bwd_aux")
+
+
+def ringx_profile_enable(on: bool) -> None:
+    _check(lib().ringx_profile_enable(1 if on else 0), "ringx_profile_enable")
+
+
+def ringx_profile_read() -> dict:
+    """{kind: (total_ms, launches)} of the launches recorded since the last read (synchronises)."""
+    ms = (ctypes.c_double * len(PROFILE_KINDS))()
+    n = (ctypes.c_int * len(PROFILE_KINDS))()
+    _check(lib().ringx_profile_read(ms, n), "ringx_profile_read")
+    return {k: (ms[i], n[i]) for i, k in enumerate(PROFILE_KINDS)}
 
 
 def ringx_version() -> int:

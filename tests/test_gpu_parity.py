@@ -1,0 +1,310 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the fp64 oracle on the
+same seeded inputs, element by element.  Tolerances are BASELINE.json's (north_star):
+  fp32 path  max|O - O_ref| <= 1e-5;   bf16  max|O - O_ref| <= 1e-2 * max|V|;   LSE <= 1e-3 abs;
+  gradients  <= 2e-2 relative Frobenius error.
+Because |O| is far below 1e-2*max|V| on the diffuse configs (an all-zero O would pass), every
+bf16 check also imposes a scale-free bound: relative Frobenius error of O <= 1e-2 (expected ~2.3e-3: P and
+the output are each rounded to bf16 once, unit roundoff 2^-8)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import attention as orc
+from paper_2507_16697_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_F32_O = 1e-5
+TOL_BF16_O_REL_V = 1e-2
+TOL_LSE = 1e-3
+TOL_GRAD = 2e-2
+TOL_BF16_O_RELF = 1e-2     # self-imposed, scale-free
+
+
+@pytest.fixture(scope="module")
+def rx():
+    from paper_2507_16697_b200 import ringx
+    from paper_2507_16697_b200.build import build_library
+    build_library()
+    assert torch.cuda.is_available(), "GPU tests need a B200"
+    ringx.lib()
+    return ringx
+
+
+def f64(t):
+    return wl.to_f64_numpy(t)
+
+
+def check_fwd(o, lse, o_ref, lse_ref, v64, dtype):
+    og = o.float().cpu().double().numpy()
+    lg = lse.cpu().double().numpy()
+    err_o = np.abs(og - o_ref).max()
+    err_l = np.abs(lg - lse_ref).max()
+    assert np.isfinite(og).all() and np.isfinite(lg).all()
+    if dtype == "f32":
+        assert err_o <= TOL_F32_O, err_o
+        assert err_l <= 1e-5, err_l
+    else:
+        assert err_o <= TOL_BF16_O_REL_V * np.abs(v64).max(), err_o
+        relf = np.linalg.norm(og - o_ref) / np.linalg.norm(o_ref)
+        assert relf <= TOL_BF16_O_RELF, relf
+        assert err_l <= TOL_LSE, err_l
+        assert err_l <= 5e-5, err_l          # fp32 row sums: far tighter than the stated bar
+
+
+# ------------------------------------------------------------------------------------------------
+# ringx_lse_merge (Eq. 5, two operands)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("rows,d", [(1, 8), (7, 64), (1000, 64), (4099, 128), (333, 24), (65, 1024), (5000, 256)])
+@pytest.mark.parametrize("in_dt,out_dt", [("f32", "f32"), ("f32", "bf16"), ("bf16", "bf16"), ("bf16", "f32")])
+def test_merge_matches_oracle(rx, rows, d, in_dt, out_dt):
+    tdt = {"f32": torch.float32, "bf16": torch.bfloat16}
+    g = torch.Generator().manual_seed(rows * 131 + d)
+    o_a = torch.randn(rows, d, generator=g).to(tdt[in_dt])
+    o_b = torch.randn(rows, d, generator=g).to(tdt[in_dt])
+    lse_a = torch.randn(rows, generator=g) * 5
+    lse_b = torch.randn(rows, generator=g) * 5
+    o, lse = rx.ringx_lse_merge(o_a.cuda(), lse_a.cuda(), o_b.cuda(), lse_b.cuda(), out_dtype=tdt[out_dt])
+    o_ref, lse_ref = orc.lse_merge(f64(o_a), f64(lse_a), f64(o_b), f64(lse_b))
+    tol = 2e-6 * max(1.0, np.abs(o_ref).max()) if out_dt == "f32" else 2 ** -8 * np.abs(o_ref).max()
+    assert np.abs(o.float().cpu().double().numpy() - o_ref).max() <= tol
+    assert np.abs(lse.cpu().double().numpy() - lse_ref).max() <= 2e-6 * max(1.0, np.abs(lse_ref).max())
+
+
+def test_merge_degenerate_operands(rx):
+    """-inf operands get weight 0 even if the o behind them is garbage; both -inf -> (0, -inf); rows=0 no-op;
+    merge with itself adds ln 2 (SURVEY.md §8c pins; reading g12)."""
+    rows, d = 64, 64
+    g = torch.Generator().manual_seed(5)
+    o_a = torch.randn(rows, d, generator=g)
+    o_b = torch.randn(rows, d, generator=g)
+    lse_a = torch.randn(rows, generator=g)
+    lse_b = torch.randn(rows, generator=g)
+    lse_b[:16] = -math.inf
+    o_b[:8] = float("nan")               # garbage behind an empty chunk must be ignored
+    lse_a[16:32] = -math.inf
+    lse_a[60:] = -math.inf
+    lse_b[60:] = -math.inf
+    o, lse = rx.ringx_lse_merge(o_a.cuda(), lse_a.cuda(), o_b.cuda(), lse_b.cuda())
+    o, lse = o.cpu(), lse.cpu()
+    assert torch.equal(o[:16], o_a[:16]) and torch.equal(lse[:16], lse_a[:16])
+    assert torch.equal(o[16:32], o_b[16:32]) and torch.equal(lse[16:32], lse_b[16:32])
+    assert torch.all(o[60:] == 0) and torch.all(lse[60:] == -math.inf)
+    o_ref, lse_ref = orc.lse_merge(f64(o_a[32:60]), f64(lse_a[32:60]), f64(o_b[32:60]), f64(lse_b[32:60]))
+    assert np.abs(o[32:60].double().numpy() - o_ref).max() <= 1e-5
+    # self-merge: (o, lse + ln 2)
+    o2, lse2 = rx.ringx_lse_merge(o_a.cuda(), lse_a.cuda(), o_a.cuda(), lse_a.cuda())
+    fin = torch.isfinite(lse_a)
+    assert torch.allclose(o2.cpu()[fin], o_a[fin], atol=1e-6)
+    assert torch.allclose(lse2.cpu()[fin], lse_a[fin] + math.log(2.0), atol=1e-6)
+    # rows == 0
+    e = torch.empty(0, d, device="cuda")
+    el = torch.empty(0, device="cuda")
+    o0, _ = rx.ringx_lse_merge(e, el, e, el)
+    assert o0.numel() == 0 and rx.ringx_last_launch_count() == 0
+    # NaN propagates
+    lse_n = lse_a.clone()
+    lse_n[40] = float("nan")
+    _, lse3 = rx.ringx_lse_merge(o_a.cuda(), lse_n.cuda(), o_b.cuda(), lse_b.cuda())
+    assert math.isnan(lse3[40].item())
+
+
+def test_merge_in_place_and_any_fold_order(rx):
+    """Running left fold in place on operand a == one Eq. 5 over all chunks (associativity)."""
+    rows, d, n = 777, 128, 5
+    g = torch.Generator().manual_seed(9)
+    outs = [torch.randn(rows, d, generator=g) for _ in range(n)]
+    lses = [torch.randn(rows, generator=g) * 3 for _ in range(n)]
+    o_ref, lse_ref = orc.merge_partials([f64(o) for o in outs], [f64(l) for l in lses])
+    acc_o, acc_l = outs[0].cuda().clone(), lses[0].cuda().clone()
+    for ob, lb in zip(outs[1:], lses[1:]):
+        r_o, r_l = rx.ringx_lse_merge(acc_o, acc_l, ob.cuda(), lb.cuda(), inplace=True)
+        assert r_o.data_ptr() == acc_o.data_ptr()
+    assert np.abs(acc_o.cpu().double().numpy() - o_ref).max() <= 1e-5
+    assert np.abs(acc_l.cpu().double().numpy() - lse_ref).max() <= 1e-5
+    # reverse order
+    acc_o, acc_l = outs[-1].cuda().clone(), lses[-1].cuda().clone()
+    for ob, lb in zip(outs[-2::-1], lses[-2::-1]):
+        rx.ringx_lse_merge(acc_o, acc_l, ob.cuda(), lb.cuda(), inplace=True)
+    assert np.abs(acc_o.cpu().double().numpy() - o_ref).max() <= 1e-5
+
+
+# ------------------------------------------------------------------------------------------------
+# forward: fp32 path (config C1) and bf16 tcgen05 path at oracle-sized shapes
+# ------------------------------------------------------------------------------------------------
+def test_fwd_C1_fp32(rx):
+    """BASELINE.json configs[0]: B=1,H=1,N=1024,d=64, 4 chunks of 256 merged by LSE; max abs err <= 1e-5."""
+    cfg = wl.CONFIGS["C1"]
+    q, k, v = wl.make_qkv(cfg)
+    o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), cfg.kv_chunk, cfg.scale)
+    assert rx.ringx_last_launch_count() == 4 + 3
+    o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), cfg.scale)
+    check_fwd(o, lse, o_ref, lse_ref, f64(v), "f32")
+
+
+@pytest.mark.parametrize("B,H,N,d,chunk", [(1, 2, 512, 128, 128), (2, 1, 384, 64, 128), (1, 1, 128, 64, 128)])
+def test_fwd_fp32_shapes(rx, B, H, N, d, chunk):
+    q, k, v = wl.make_qkv((B, H, N, d), seed=3, dtype="f32")
+    scale = 1.0 / math.sqrt(d)
+    o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), chunk, scale)
+    o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+    check_fwd(o, lse, o_ref, lse_ref, f64(v), "f32")
+
+
+BF16_SHAPES = [
+    # B, H, N, d, kv_chunk, qk_gain        (several 256-row CTA tiles, ragged KV-tile counts, 1..16 passes)
+    (1, 1, 256, 64, 256, 1.0),             # minimum size, single pass, one KV... two KV tiles
+    (1, 1, 256, 128, 128, 1.0),            # two passes of one KV tile each
+    (2, 3, 1280, 64, 256, 1.0),            # 5 passes, 5 CTAs per head
+    (1, 2, 2304, 128, 768, 1.0),           # 3 passes of 6 KV tiles (ring wraps: 5 slots)
+    (1, 2, 2048, 64, 2048, 1.0),           # single pass, 16 KV tiles (ring wraps: 8 slots)
+    (1, 2, 2048, 128, 128, 3.0),           # 16 passes, peaked softmax (C5-like gain on Q and K)
+    (1, 1, 4096, 128, 1024, 3.0),
+    (1, 4, 1024, 64, 512, 0.05),           # nearly uniform softmax
+]
+
+
+@pytest.mark.parametrize("B,H,N,d,chunk,gain", BF16_SHAPES)
+def test_fwd_bf16_matches_oracle(rx, B, H, N, d, chunk, gain):
+    q, k, v = (wl.make_tensor((B, H, N, d), w, seed=17, dtype="bf16", gain=(gain if w != "v" else 1.0)) for w in "qkv")
+    scale = 1.0 / math.sqrt(d)
+    o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), chunk, scale)
+    n_c = N // chunk
+    assert rx.ringx_last_launch_count() == n_c + (n_c - 1)
+    o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+    check_fwd(o, lse, o_ref, lse_ref, f64(v), "bf16")
+
+
+def test_fwd_bf16_chunk_partials_and_merge_are_the_papers_quantities(rx):
+    """ringx_attn_chunk_fwd returns (loc_out_i, loc_lse_i) of PAPER.md:135 with Nq != Nk; merging them with
+    ringx_lse_merge reproduces the oracle's Eq. 5 result."""
+    B, H, Nq, Nk, d = 1, 2, 512, 768, 128
+    q = wl.make_tensor((B, H, Nq, d), "q", seed=23)
+    k = wl.make_tensor((B, H, Nk, d), "k", seed=23)
+    v = wl.make_tensor((B, H, Nk, d), "v", seed=23)
+    scale = 0.1
+    bounds = [0, 256, 768]
+    parts = []
+    for lo, hi in zip(bounds[:-1], bounds[1:]):
+        lo_o, lo_l = rx.ringx_attn_chunk_fwd(q.cuda(), k[:, :, lo:hi].contiguous().cuda(),
+                                             v[:, :, lo:hi].contiguous().cuda(), scale)
+        parts.append((lo_o, lo_l))
+        for h in range(H):
+            outs, lses = orc.chunk_partials(f64(q[0, h]), f64(k[0, h]), f64(v[0, h]), scale, bounds)
+            i = len(parts) - 1
+            assert np.abs(lo_l[0, h].cpu().double().numpy() - lses[i]).max() <= 5e-5
+            rel = np.linalg.norm(lo_o[0, h].cpu().double().numpy() - outs[i]) / np.linalg.norm(outs[i])
+            assert rel <= 5e-3, rel
+    o, lse = rx.ringx_lse_merge(parts[0][0], parts[0][1], parts[1][0], parts[1][1], out_dtype=torch.bfloat16)
+    o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+    check_fwd(o, lse, o_ref, lse_ref, f64(v), "bf16")
+
+
+def test_fwd_bf16_result_is_independent_of_kv_chunk(rx):
+    """Several results are correct up to rounding (reading g5): every chunking agrees to bf16 rounding."""
+    B, H, N, d = 1, 2, 2048, 128
+    q, k, v = wl.make_qkv((B, H, N, d), seed=29)
+    qd, kd, vd = q.cuda(), k.cuda(), v.cuda()
+    scale = 1.0 / math.sqrt(d)
+    o_ref, lse_ref = rx.ringx_attn_fwd(qd, kd, vd, N, scale)
+    for chunk in (128, 256, 512, 1024):
+        o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
+        assert (lse - lse_ref).abs().max().item() <= 2e-5
+        rel = ((o.float() - o_ref.float()).norm() / o_ref.float().norm()).item()
+        assert rel <= 4e-3, (chunk, rel)
+
+
+def test_fwd_bf16_one_hot_v_reads_P(rx):
+    """V = identity block over d chosen keys => O[:, c] = P[:, key(c)]: checks individual probabilities,
+    which localises any tile-layout / swizzle / transposition error."""
+    B, H, N, d = 1, 1, 512, 64
+    q, k, _ = wl.make_qkv((B, H, N, d), seed=31)
+    keys = np.array([0, 1, 63, 64, 127, 128, 129, 255, 256, 300, 383, 384, 450, 500, 510, 511] * 4)[:d]
+    keys = (keys + np.arange(d) // 16 * 3) % N
+    keys = np.unique(keys)
+    v = torch.zeros(B, H, N, d, dtype=torch.bfloat16)
+    for c, j in enumerate(keys):
+        v[0, 0, j, c] = 1.0
+    scale = 0.35
+    o, _ = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), 256, scale)
+    P = orc.softmax_probs(f64(q[0, 0]), f64(k[0, 0]), scale)
+    og = o[0, 0].float().cpu().double().numpy()
+    for c, j in enumerate(keys):
+        assert np.abs(og[:, c] - P[:, j]).max() <= 2 ** -7 * max(P[:, j].max(), 1e-3) + 1e-6, (c, j)   # two bf16 roundings
+    assert np.abs(og[:, len(keys):]).max() == 0.0
+
+
+def test_fwd_closed_forms(rx):
+    """Identical keys => O = mean(V), LSE = s + ln N;  Q = 0 => same with s = 0."""
+    B, H, N, d = 1, 1, 512, 64
+    q, _, v = wl.make_qkv((B, H, N, d), seed=37)
+    k1 = wl.make_tensor((1, 1, 1, d), "k", seed=37)
+    k = k1.expand(B, H, N, d).contiguous()
+    scale = 0.125
+    o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), 128, scale)
+    mean_v = f64(v)[0, 0].mean(axis=0)
+    s = scale * f64(q)[0, 0] @ f64(k1)[0, 0, 0]
+    assert np.abs(o[0, 0].float().cpu().double().numpy() - mean_v[None, :]).max() <= 2 ** -8 * np.abs(mean_v).max() + 1e-4
+    assert np.abs(lse[0, 0].cpu().double().numpy() - (s + math.log(N))).max() <= 1e-4
+    q0 = torch.zeros_like(q)
+    o, lse = rx.ringx_attn_fwd(q0.cuda(), wl.make_tensor((B, H, N, d), "k", seed=38).cuda(), v.cuda(), 256, scale)
+    assert np.abs(o[0, 0].float().cpu().double().numpy() - mean_v[None, :]).max() <= 2 ** -8 * np.abs(mean_v).max() + 1e-4
+    assert np.abs(lse.cpu().double().numpy() - math.log(N)).max() <= 1e-5
+
+
+def test_fwd_large_magnitude_scores_do_not_overflow(rx):
+    """Row maxima that keep growing across KV tiles exercise the lazy-rescale branch on every tile."""
+    B, H, N, d = 1, 1, 1024, 64
+    q, k, v = wl.make_qkv((B, H, N, d), seed=41)
+    ramp = torch.linspace(0.2, 6.0, N).view(1, 1, N, 1)
+    k = (k.float() * ramp).to(torch.bfloat16)         # later keys have larger norms
+    scale = 1.0
+    o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), 512, scale)
+    o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+    og = o.float().cpu().double().numpy()
+    assert np.isfinite(og).all()
+    assert np.abs(og - o_ref).max() <= TOL_BF16_O_REL_V * np.abs(f64(v)).max()
+    assert np.abs(lse.cpu().double().numpy() - lse_ref).max() <= TOL_LSE
+
+
+def test_fwd_permutation_invariances(rx):
+    """Jointly permuting (K,V) rows leaves (O,LSE) unchanged, and permuting Q rows permutes the outputs, both up
+    to rounding (the lazy running max is decided per warp of 32 rows, so a row's rounding depends on its
+    neighbours) -- the voxel flatten order is metadata only (reading g15)."""
+    B, H, N, d = 1, 1, 1024, 128
+    q, k, v = wl.make_qkv((B, H, N, d), seed=43)
+    scale = 1.0 / math.sqrt(d)
+    o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), 256, scale)
+    g = torch.Generator().manual_seed(1)
+    pq = torch.randperm(N, generator=g)
+    o2, lse2 = rx.ringx_attn_fwd(q[:, :, pq].contiguous().cuda(), k.cuda(), v.cuda(), 256, scale)
+    assert (lse2.cpu() - lse.cpu()[:, :, pq]).abs().max().item() <= 2e-5
+    assert ((o2.cpu().float() - o.cpu().float()[:, :, pq]).norm() / o.float().norm()).item() <= 4e-3
+    pk = torch.randperm(N, generator=g)
+    o3, lse3 = rx.ringx_attn_fwd(q.cuda(), k[:, :, pk].contiguous().cuda(), v[:, :, pk].contiguous().cuda(), 256, scale)
+    assert (lse3 - lse).abs().max().item() <= 2e-5
+    assert ((o3.float() - o.float()).norm() / o.float().norm()).item() <= 4e-3
+
+
+def test_fwd_host_entry_matches_device_entry(rx):
+    B, H, N, d, chunk = 1, 2, 1024, 64, 256
+    q, k, v = wl.make_qkv((B, H, N, d), seed=47)
+    scale = 0.125
+    o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), chunk, scale)
+    oh, lh = rx.ringx_attn_fwd_host(q.pin_memory(), k.pin_memory(), v.pin_memory(), chunk, scale)
+    assert torch.equal(oh, o.cpu()) and torch.equal(lh, lse.cpu())
+
+
+def test_errors_on_the_gpu_box(rx):
+    q = torch.zeros(1, 1, 512, 64, dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(rx.RingxError) as e:
+        rx.ringx_attn_fwd(q, q, q, 384, 0.125)
+    assert e.value.status == 2
+    with pytest.raises(rx.RingxError) as e:
+        rx.ringx_attn_fwd(q, q, q, 256, 0.125, workspace=torch.empty(256, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == 5
+    with pytest.raises(rx.RingxError) as e:
+        rx.ringx_attn_fwd(q, q, q, 256, -1.0)
+    assert e.value.status == 2
