@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py -- the RingX hot path on B200: attention TFLOP/s of the chunked forward (and backward), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C3]
+
+A "step" is one pass of the hot path over one batch of synthetic input of the named BASELINE.json config
+(default C3: bf16, B=1, H=8, N=262144, d=128, kv_chunk=32768 -- the configuration the north_star's target
+"bf16 forward at N >= 262,144" is quoted on): `ringx_attn_fwd` = 8 KV-chunk passes of the tcgen05 kernel +
+7 Eq. 5 merges; configs with `backward` add `ringx_attn_bwd`.  FLOPs: forward 4*B*H*N^2*d,
+backward 10*B*H*N^2*d.  Inputs are seeded synthetic (paper_2507_16697_b200/workloads.py), resident in HBM for
+`value`; `e2e` times the same metric through the C ABI with HOST buffers (H2D + D2H inside the timed region).
+Multi-GPU (--gpus N under torchrun): the path has no exchange step on one node (batch x heads
+are independent) -> every rank runs the workload on its own seeded batch, no data-path collective, "weak".
+`--impl reference` times the fp64 CPU oracle (oracle/), as it stands, on a bounded sample of the workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+import torch  # noqa: E402
+
+METRIC = "attention TFLOPS fwd at 1 B200 (4*B*H*N^2*d; fraction of dense bf16 tensor peak in roofline.frac)"
+UNIT = "TFLOP/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return {k: float(d[k]) for k in FALLBACK_PEAKS if k in d} | {"source": "measured"}
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS) | {"source": "fallback"}
+
+
+def load_traffic(key):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (or None)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(key)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return None
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, val in zip(self.NAMES, f[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return None
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def oracle_sample(cfg, k64, v64, q_rows64, block=256):
+    """The oracle as it stands on a bounded sample: `attention_fwd` of the sampled query rows of one head
+    against ALL keys of that head.  Returns (seconds, flops)."""
+    from oracle import attention as orc
+    t0 = time.perf_counter()
+    for r0 in range(0, q_rows64.shape[0], block):
+        orc.attention_fwd(q_rows64[r0:r0 + block], k64, v64, cfg.scale)
+    dt = time.perf_counter() - t0
+    return dt, 4.0 * q_rows64.shape[0] * cfg.N * cfg.d
+
+
+def run_reference(args, cfg, rank):
+    """--impl reference: the fp64 numpy oracle on this box's host cores, each step a bounded sample."""
+    from paper_2507_16697_b200 import workloads as wl
+    if rank != 0:
+        return
+    rows_per_step = args.ref_rows
+    # one head of the workload, generated on the host by the same counter-based recipe (first rows of head 0)
+    head = wl.Config(cfg.name, cfg.dtype, 1, 1, cfg.N, cfg.d, cfg.kv_chunk, cfg.qk_gain, False, cfg.seed)
+    q, k, v = wl.make_qkv(head)
+    k64, v64 = wl.to_f64_numpy(k[0, 0]), wl.to_f64_numpy(v[0, 0])
+    q64 = wl.to_f64_numpy(q[0, 0])
+    rng = np.random.default_rng(0)
+    for _ in range(args.warmup):
+        oracle_sample(cfg, k64, v64, q64[rng.integers(0, cfg.N, 64)])
+    t_total, f_total = 0.0, 0.0
+    for _ in range(args.steps):
+        rows = rng.integers(0, cfg.N, rows_per_step)
+        dt, fl = oracle_sample(cfg, k64, v64, q64[rows])
+        t_total += dt
+        f_total += fl
+    value = f_total / t_total / 1e12
+    sample = (f"{rows_per_step} query rows of head 0 against all {cfg.N} keys per step "
+              f"({rows_per_step * cfg.N:.3g} of the config's {cfg.B * cfg.H * cfg.N * cfg.N:.3g} query-key pairs)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, "fwd"),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": host_cores(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, what):
+    return {"workload": f"{cfg.name}: {cfg.dtype} {what}, non-causal, B={cfg.B} H={cfg.H} N={cfg.N} d={cfg.d} "
+                        f"kv_chunk={cfg.kv_chunk} ({cfg.N // cfg.kv_chunk} ring passes)",
+            "B": cfg.B, "H": cfg.H, "N": cfg.N, "d": cfg.d, "kv_chunk": cfg.kv_chunk, "qk_gain": cfg.qk_gain,
+            "pass": what, "seed": cfg.seed, "l2": "inputs larger than L2 (no flush needed)"
+            if 3 * cfg.B * cfg.H * cfg.N * cfg.d * 2 > 126e6 else "L2 flushed between steps"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C3", choices=["C2", "C3", "C4", "C5"])
+    ap.add_argument("--ref-rows", type=int, default=512, help="query rows per step of the reference arm")
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
+    ap.add_argument("--no-extra", action="store_true", help="skip the short C2/C4 side measurements")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    from paper_2507_16697_b200 import workloads as wl
+    cfg = wl.CONFIGS[args.config]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    from paper_2507_16697_b200 import ringx
+    from paper_2507_16697_b200.build import build_library
+    if rank == 0:
+        build_library()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+        dist.barrier()
+    ringx.lib()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    # ---------------------------------------------------------------- inputs (seeded, per-rank batch)
+    rcfg = wl.Config(cfg.name, cfg.dtype, cfg.B, cfg.H, cfg.N, cfg.d, cfg.kv_chunk, cfg.qk_gain, cfg.backward,
+                     cfg.seed + 1000 * rank)
+    tensors = wl.make_qkv(rcfg, with_do=cfg.backward, device=dev)
+    q, k, v = tensors[:3]
+    dO = tensors[3] if cfg.backward else None
+    B, H, N, d = q.shape
+    o = torch.empty_like(q)
+    lse = torch.empty((B, H, N), dtype=torch.float32, device=dev)
+    ws_f = torch.empty(max(256, ringx.ringx_attn_fwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
+                       dtype=torch.uint8, device=dev)
+    ws_b = None
+    if cfg.backward:
+        ws_b = torch.empty(max(256, ringx.ringx_attn_bwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
+                           dtype=torch.uint8, device=dev)
+    flops_step = cfg.fwd_flops + (cfg.bwd_flops if cfg.backward else 0.0)
+    launches = [0]
+
+    def step():
+        ringx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale, o=o, lse=lse, workspace=ws_f)
+        n = ringx.ringx_last_launch_count()
+        if cfg.backward:
+            ringx.ringx_attn_bwd(q, k, v, o, lse, dO, cfg.kv_chunk, cfg.scale, workspace=ws_b)
+            n += ringx.ringx_last_launch_count()
+        launches[0] += n
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+
+    # ---------------------------------------------------------------- timed region
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    launches[0] = 0
+    ringx.ringx_profile_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    prof = ringx.ringx_profile_read()
+    ringx.ringx_profile_enable(False)
+    ms_total = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = t.item()
+    ms_step = ms_total / args.steps
+    value = world * flops_step / (ms_step * 1e-3) / 1e12
+    gpu_launches = launches[0]
+
+    # ---------------------------------------------------------------- roofline of the dominant kernel
+    peaks = load_peaks()
+    dom = "attn_bwd" if (cfg.backward and prof["attn_bwd"][0] > prof["attn_fwd"][0]) else "attn_fwd"
+    dom_ms, dom_n = prof[dom]
+    per_launch = (10.0 if dom == "attn_bwd" else 4.0) * B * H * N * cfg.kv_chunk * d
+    achieved = per_launch / (dom_ms / max(dom_n, 1) * 1e-3) / 1e12 if dom_n else None
+    roofline = {
+        "bound": "tensor", "kernel": "attn_chunk_fwd_kernel" if dom == "attn_fwd" else "attn_chunk_bwd_kernel",
+        "achieved": achieved, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+        "frac": achieved / peaks["bf16_tflops_sustained"] if achieved else None,
+        "peak_kind": f"bf16 dense, sustained (kernel timed inside a long step), {peaks['source']}",
+        "peak_burst": peaks["bf16_tflops"], "frac_of_burst": achieved / peaks["bf16_tflops"] if achieved else None,
+        "frac_of_nominal_2250": achieved / 2250.0 if achieved else None,
+        "flops_per_launch": per_launch, "launches_timed": dom_n, "avg_launch_ms": dom_ms / max(dom_n, 1),
+        "share_of_step": dom_ms / ms_total if world == 1 else None,
+        "traffic": load_traffic(f"{cfg.name}_{dom}"),
+    }
+    merge_ms, merge_n = prof["merge"]
+    merge_info = None
+    if merge_n:
+        mbytes = 3.0 * B * H * N * (d * 4 + 4) - (B * H * N * d * 2 / merge_n)   # last merge writes bf16
+        merge_info = {"avg_launch_ms": merge_ms / merge_n, "launches_timed": merge_n,
+                      "achieved_gbs": mbytes / (merge_ms / merge_n * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
+                      "frac": mbytes / (merge_ms / merge_n * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+
+    # ---------------------------------------------------------------- e2e: HOST buffers through the C ABI
+    e2e = None
+    if not cfg.backward:
+        qh, kh, vh = (t.cpu().pin_memory() for t in (q, k, v))
+        oh = torch.empty_like(qh).pin_memory()
+        lh = torch.empty((B, H, N), dtype=torch.float32).pin_memory()
+        ws_h = torch.empty(ringx.ringx_attn_fwd_host_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype),
+                           dtype=torch.uint8, device=dev)
+        n_e2e = max(1, min(args.steps, 3))
+        ringx.ringx_attn_fwd_host(qh, kh, vh, cfg.kv_chunk, cfg.scale, o_host=oh, lse_host=lh, workspace=ws_h)
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            ringx.ringx_attn_fwd_host(qh, kh, vh, cfg.kv_chunk, cfg.scale, o_host=oh, lse_host=lh, workspace=ws_h)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / n_e2e
+        if dist is not None:
+            t = torch.tensor([dt], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = t.item()
+        e2e = {"value": world * cfg.fwd_flops / dt / 1e12, "unit": UNIT, "ms_per_step": dt * 1e3, "steps": n_e2e,
+               "h2d_bytes_per_step": 3 * q.numel() * q.element_size(),
+               "d2h_bytes_per_step": q.numel() * q.element_size() + lse.numel() * 4,
+               "entry": "ringx_attn_fwd_host (pinned host q,k,v -> device, forward, o+lse -> host, synchronised)"}
+        del ws_h, qh, kh, vh, oh, lh
+
+    # ---------------------------------------------------------------- short side measurements (not the metric)
+    extra = {}
+    if rank == 0 and not args.no_extra:
+        for name in ("C2", "C4"):
+            if name == cfg.name:
+                continue
+            extra[name] = side_measure(ringx, wl, wl.CONFIGS[name], dev)
+
+    # ---------------------------------------------------------------- CPU baseline: the oracle, bounded sample
+    cpu_baseline = None
+    if rank == 0 and world == 1:
+        k64, v64 = wl.to_f64_numpy(k[0, 0]), wl.to_f64_numpy(v[0, 0])
+        q64 = wl.to_f64_numpy(q[0, 0, :8192])
+        dt0, _ = oracle_sample(cfg, k64, v64, q64[:128])
+        n_rows = int(min(q64.shape[0], max(128, args.cpu_baseline_seconds / (dt0 / 128.0) // 128 * 128)))
+        dt, fl = oracle_sample(cfg, k64, v64, q64[:n_rows])
+        cpu_baseline = {"value": fl / dt / 1e12, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
+                        "seconds": dt,
+                        "sample": f"first {n_rows} query rows of head (0,0) against all {N} keys "
+                                  f"(oracle.attention_fwd, fp64 numpy, blocks of 256 rows)"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": workload_config(cfg, "fwd+bwd" if cfg.backward else "fwd"),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": gpu_launches,
+            "roofline": roofline, "merge_kernel": merge_info, "cpu_baseline": cpu_baseline, "extra": extra,
+            "frac_of_bf16_peak": {"sustained": value / world / peaks["bf16_tflops_sustained"],
+                                  "burst": value / world / peaks["bf16_tflops"], "nominal_2250": value / world / 2250.0,
+                                  "source": peaks["source"]},
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def side_measure(ringx, wl, cfg, dev, reps=3):
+    """A short forward (and backward) timing of another BASELINE.json config; context, not the metric."""
+    tensors = wl.make_qkv(cfg, with_do=cfg.backward, device=dev)
+    q, k, v = tensors[:3]
+    B, H, N, d = q.shape
+    o = torch.empty_like(q)
+    lse = torch.empty((B, H, N), dtype=torch.float32, device=dev)
+    ws = torch.empty(max(256, ringx.ringx_attn_fwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
+                     dtype=torch.uint8, device=dev)
+    out = {}
+
+    def timeit(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    ms = timeit(lambda: ringx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale, o=o, lse=lse, workspace=ws))
+    out["fwd_ms"] = ms
+    out["fwd_tflops"] = cfg.fwd_flops / ms / 1e9
+    if cfg.backward:
+        wsb = torch.empty(max(256, ringx.ringx_attn_bwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
+                          dtype=torch.uint8, device=dev)
+        try:
+            ms = timeit(lambda: ringx.ringx_attn_bwd(q, k, v, o, lse, tensors[3], cfg.kv_chunk, cfg.scale,
+                                                     workspace=wsb))
+            out["bwd_ms"] = ms
+            out["bwd_tflops"] = cfg.bwd_flops / ms / 1e9
+        except ringx.RingxError as e:
+            out["bwd"] = f"unavailable: {e}"
+    return out
+
+
+if __name__ == "__main__":
+    main()

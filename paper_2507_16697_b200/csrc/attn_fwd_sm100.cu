@@ -19,6 +19,12 @@
 #include "kernels.cuh"
 
 namespace ringx {
+#ifdef RINGX_FWD_CLOCKS
+__device__ long long g_fwd_clocks[16];
+#define CLK() clock64()
+#else
+#define CLK() 0ll
+#endif
 namespace {
 
 using namespace ptx;
@@ -57,7 +63,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   uint64_t* kv_empty = bars + 8 + Cfg::kStages;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 8 + 2 * Cfg::kStages);
 
-  const int warp = threadIdx.x >> 5;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // provably warp-uniform: keeps MMA/TMA operands in uniform registers
   const int lane = threadIdx.x & 31;
   const int bh = blockIdx.y;
   const int q_row0 = bh * Nq + blockIdx.x * (2 * kBlockM);     // row in the [BH*Nq, d] view
@@ -91,13 +97,18 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 
   if (warp == 8) {
     // ------------------------------------------------------------------ TMA producer
-    if (lane == 0) {
+    // (the whole warp runs the loop so that every operand is warp-uniform; one elected lane issues)
+    {
+      const bool leader = elect_one();
       const uint64_t pol_q = policy_evict_first();
       const uint64_t pol_kv = policy_evict_last();
       auto load_tile = [&](uint8_t* dst, const CUtensorMap* map, uint64_t* bar, int row, uint64_t pol) {
-        mbar_arrive_expect_tx(bar, Cfg::kTileBytes);
+        if (leader) {
+          mbar_arrive_expect_tx(bar, Cfg::kTileBytes);
 #pragma unroll
-        for (int p = 0; p < Cfg::kPanels; ++p) tma_load_2d(dst + p * Cfg::kPanelBytes, map, bar, p * 64, row, pol);
+          for (int p = 0; p < Cfg::kPanels; ++p) tma_load_2d(dst + p * Cfg::kPanelBytes, map, bar, p * 64, row, pol);
+        }
+        __syncwarp();
       };
       load_tile(sQ, &map_q, &q_full[0], q_row0, pol_q);
       int stage = 0, phase = 0;
@@ -111,7 +122,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     }
   } else if (warp == 9) {
     // ------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
+    {
+      const bool leader = elect_one();
       constexpr uint32_t idesc_s = make_idesc_bf16(kBlockM, kBlockN, 0, 0);    // Q (K-major) x K^T (K-major)
       constexpr uint32_t idesc_o = make_idesc_bf16(kBlockM, kD, 0, 1);         // P (TMEM) x V (MN-major)
       const uint32_t q_addr = smem_u32(sQ), kv_addr = smem_u32(sKV);
@@ -120,21 +132,31 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       // S_t = Q_t K^T from the K tile in ring slot `st`
       auto issue_s = [&](int t, int st) {
         const uint32_t a0 = q_addr + t * Cfg::kTileBytes, b0 = kv_addr + st * Cfg::kTileBytes;
+        if (leader) {
 #pragma unroll
-        for (int k = 0; k < kD / 16; ++k) {
-          const uint32_t off = (k >> 2) * Cfg::kPanelBytes + (k & 3) * 32;
-          mma_ss(tmem + t * kBlockN, make_smem_desc_sw128(a0 + off, 16, 1024), make_smem_desc_sw128(b0 + off, 16, 1024),
-                 idesc_s, k > 0);
+          for (int k = 0; k < kD / 16; ++k) {
+            const uint32_t off = (k >> 2) * Cfg::kPanelBytes + (k & 3) * 32;
+            mma_ss(tmem + t * kBlockN, make_smem_desc_sw128(a0 + off, 16, 1024),
+                   make_smem_desc_sw128(b0 + off, 16, 1024), idesc_s, k > 0);
+          }
+          mma_commit(&s_full[t]);
         }
-        mma_commit(&s_full[t]);
+        __syncwarp();
       };
       // O_t (+)= P_t V from the V tile in ring slot `st`
       auto issue_o = [&](int t, int st, bool accumulate) {
         const uint32_t b0 = kv_addr + st * Cfg::kTileBytes;
+        if (leader) {
 #pragma unroll
-        for (int k = 0; k < kBlockN / 16; ++k)
-          mma_ts(tmem + 256 + t * kD, tmem + t * kBlockN + k * 8,
-                 make_smem_desc_sw128(b0 + k * 2048, Cfg::kPanelBytes, 1024), idesc_o, accumulate || k > 0);
+          for (int k = 0; k < kBlockN / 16; ++k)
+            mma_ts(tmem + 256 + t * kD, tmem + t * kBlockN + k * 8,
+                   make_smem_desc_sw128(b0 + k * 2048, Cfg::kPanelBytes, 1024), idesc_o, accumulate || k > 0);
+        }
+        __syncwarp();
+      };
+      auto commit = [&](uint64_t* bar) {
+        if (leader) mma_commit(bar);
+        __syncwarp();
       };
       // prologue: S_0(0), S_1(0)
       mbar_wait(&kv_full[stage], phase);
@@ -144,7 +166,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(&q_full[1], 0);
       tc_fence_after();
       issue_s(1, stage);
-      mma_commit(&kv_empty[stage]);
+      commit(&kv_empty[stage]);
       advance();
       for (int j = 0; j < n_kv; ++j) {
         const int v_stage = stage, v_phase = phase;
@@ -155,19 +177,23 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         mbar_wait(&kv_full[v_stage], v_phase);
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
+          const long long m0 = CLK();
           mbar_wait(&p_full[t], j & 1);
           tc_fence_after();
+#ifdef RINGX_FWD_CLOCKS
+          if (blockIdx.x == 0 && blockIdx.y == 0 && leader && j >= 8) atomicAdd((unsigned long long*)&g_fwd_clocks[8 + t], (unsigned long long)(CLK() - m0));
+#endif
           issue_o(t, v_stage, j > 0);
-          if (t == 1) mma_commit(&kv_empty[v_stage]);
+          if (t == 1) commit(&kv_empty[v_stage]);
           if (more) {
             if (t == 0) {
               mbar_wait(&kv_full[k_stage], k_phase);
               tc_fence_after();
             }
             issue_s(t, k_stage);
-            if (t == 1) mma_commit(&kv_empty[k_stage]);
+            if (t == 1) commit(&kv_empty[k_stage]);
           } else {
-            mma_commit(&o_full[t]);
+            commit(&o_full[t]);
           }
         }
       }
@@ -182,8 +208,10 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     float m_sc = -CUDART_INF_F;    // m_raw * scale_log2
     float l = 0.f;                 // running row sum of exp2(s*scale_log2 - m_sc)
     for (int j = 0; j < n_kv; ++j) {
+      const long long c0 = CLK();
       mbar_wait(&s_full[t], j & 1);
       tc_fence_after();
+      const long long c1 = CLK();
       uint32_t s[kBlockN];
 #pragma unroll
       for (int c = 0; c < kBlockN / 32; ++c) tmem_ld_x32(tS + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
@@ -237,6 +265,13 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       tmem_wait_st();
       tc_fence_before();
       mbar_arrive(&p_full[t]);
+#ifdef RINGX_FWD_CLOCKS
+      if (blockIdx.x == 0 && blockIdx.y == 0 && (threadIdx.x & 127) == 0 && j >= 8) {
+        atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 0], (unsigned long long)(c1 - c0));   // wait S
+        atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 1], (unsigned long long)(CLK() - c1));  // softmax
+        atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 2], 1ull);
+      }
+#endif
     }
     // ---- chunk epilogue: loc_out = O / l, loc_lse = m*scale + ln l  (natural log of the scaled scores)
     mbar_wait(&o_full[t], 0);
@@ -312,3 +347,13 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
 }
 
 }  // namespace ringx
+
+#ifdef RINGX_FWD_CLOCKS
+extern "C" __attribute__((visibility("default"))) int ringx_debug_clocks(long long* out) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, ringx::g_fwd_clocks, sizeof(long long) * 16);
+  long long z[16] = {0};
+  cudaMemcpyToSymbol(ringx::g_fwd_clocks, z, sizeof(z));
+  return 0;
+}
+#endif
