@@ -98,6 +98,7 @@ FwdWorkspace carve_fwd(void* ws, int B, int H, int N, int d, int kv_chunk, int d
 
 struct BwdWorkspace {
   float* D = nullptr;        // D_i = dO_i . O_i, [R]
+  float* lse2 = nullptr;     // LSE_i * log2(e), [R]
   float* dq_acc = nullptr;   // fp32 dQ accumulator [R,d]
   size_t bytes = 0;
 };
@@ -108,6 +109,8 @@ BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
   char* p = static_cast<char*>(ws);
   w.D = reinterpret_cast<float*>(p);
   size_t off = align_up(R * sizeof(float));
+  w.lse2 = reinterpret_cast<float*>(p ? p + off : nullptr);
+  off += align_up(R * sizeof(float));
   w.dq_acc = reinterpret_cast<float*>(p ? p + off : nullptr);
   off += align_up(R * d * sizeof(float));
   w.bytes = off;
@@ -319,13 +322,13 @@ int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, c
   cudaError_t e;
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-    e = launch_bwd_preprocess(o, dO, w.D, w.dq_acc, R, d, stream);
+    e = launch_bwd_preprocess(o, dO, lse, w.D, w.lse2, w.dq_acc, R, d, stream);
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
   for (int c = 0; c < N / kv_chunk; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
-    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse, w.D, w.dq_acc, dk, dv, BH, N, c * kv_chunk, kv_chunk, d, scale,
+    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, w.lse2, w.D, w.dq_acc, dk, dv, BH, N, c * kv_chunk, kv_chunk, d, scale,
                                     stream);
     if (e != cudaSuccess) return cuda_status(e);
   }

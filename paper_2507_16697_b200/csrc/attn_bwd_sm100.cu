@@ -1,8 +1,393 @@
-// attn_bwd_sm100.cu -- placeholder until the tcgen05 backward lands (reports "not supported").
+// attn_bwd_sm100.cu -- one KV-chunk pass of the backward on tcgen05 tensor cores.
+//
+// A CTA owns one 128-key tile (K_j, V_j) of one head and loops over all 128-row query tiles i of that head:
+//   S^T  = K_j Q_i^T                      P^T  = exp2(scale*log2e * S^T - lse2_i)   (P recomputed from the saved
+//   dP^T = V_j dO_i^T                     dS^T = P^T o (dP^T - D_i)                  *global* LSE; reading g8)
+//   dV_j += P^T dO_i      dK_j += dS^T Q_i      dQ_i += dS K_j                       (all unscaled; scale is applied
+// when dK is written here and when dQ is converted).  dK_j, dV_j live in TMEM for the whole loop and are written once
+// (atomic-free: the CTA owns the tile); dQ_i is reduce-added into the fp32 accumulator with red.global.add.v4.f32 --
+// the single-GPU image of "the gradient for Q is accumulated ... over N steps".
+//
+// Roles (448 threads):  warps 0-7  compute (thread = key row = TMEM lane; warps 0-3 take query columns 0-63 of the
+//                                  tile, warps 4-7 columns 64-127)
+//                       warps 8-11 dQ drain (thread = query row): TMEM -> registers -> red.global.add
+//                       warp  12   TMA producer (K_j,V_j once; then the Q_i/dO_i/lse2_i/D_i ring)
+//                       warp  13   MMA issuer
+// TMEM columns: S^T [0,128) (P^T, bf16, overwrites the first 32 columns of each 64-column half), dP^T [128,256),
+// dV [256,256+d), dK [256+d,256+2d), dQ [384,448) for d = 64; for d = 128 dQ overlays dP^T (drained before the next
+// dP^T is issued).  dS^T goes to shared memory as a [keys][queries] bf16 tile that serves as the K-major A operand of
+// dK += dS^T Q and as the MN-major A operand of dQ = dS K.
+// Pipeline: the compute warps alternate phase A (S^T -> P^T) and phase B (dP^T -> dS^T) while the tensor core runs
+// {dV(i), S^T(i+1)} behind phase A and {dK(i), dQ(i), dP^T(i+1)} behind phase B; in-order MMA execution makes the
+// P^T / S^T overlay safe.
 #include "kernels.cuh"
+
 namespace ringx {
-cudaError_t launch_attn_chunk_bwd_sm100(const void*, const void*, const void*, const void*, const float*, const float*,
-                                        float*, void*, void*, int, int, int, int, int, float, cudaStream_t) {
-  return cudaErrorNotSupported;
+namespace {
+
+using namespace ptx;
+
+constexpr int kTile = 128;
+constexpr int kBwdThreads = 448;
+
+template <int kD>
+struct BwdCfg {
+  static constexpr int kPanels = kD / 64;
+  static constexpr int kPanelBytes = 128 * 128;
+  static constexpr int kTileBytes = kPanels * kPanelBytes;     // one [128, d] bf16 tile
+  static constexpr int kStages = kD == 64 ? 3 : 2;             // Q_i / dO_i ring
+  static constexpr int kStageBytes = 2 * kTileBytes + 1024;    // Q, dO, lse2[128], D[128]
+  static constexpr int kDsBytes = 2 * kPanelBytes;             // dS^T [128 keys][128 queries] bf16
+  static constexpr int kAlignSlack = kD == 64 ? 1024 : 0;      // d = 128 uses every byte: base must be 1 KB aligned
+  static constexpr int kSmemBytes = kAlignSlack + 2 * kTileBytes + kStages * kStageBytes + kDsBytes + 256;
+  static constexpr uint32_t tS = 0, tDP = 128, tDV = 256, tDK = 256 + kD, tDQ = kD == 64 ? 384 : 128;
+  static constexpr bool kDqOverlaysDp = kD != 64;
+};
+
+template <int kD>
+__global__ void __launch_bounds__(kBwdThreads, 1)
+attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
+                      const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_do,
+                      const float* __restrict__ lse2, const float* __restrict__ Dvec, float* __restrict__ dq_acc,
+                      __nv_bfloat16* __restrict__ dk, __nv_bfloat16* __restrict__ dv, int N, int k_off,
+                      float scale_log2, float scale) {
+  using Cfg = BwdCfg<kD>;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  if (Cfg::kAlignSlack == 0 && smem != smem_raw) __trap();
+  uint8_t* sK = smem;
+  uint8_t* sV = smem + Cfg::kTileBytes;
+  uint8_t* sStage = smem + 2 * Cfg::kTileBytes;
+  uint8_t* sDs = sStage + Cfg::kStages * Cfg::kStageBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sDs + Cfg::kDsBytes);
+  uint64_t* kv_full = bars;          // TMA -> MMA: K_j, V_j
+  uint64_t* s_full = bars + 1;       // MMA -> compute: S^T(i)
+  uint64_t* dp_full = bars + 2;      // MMA -> compute: dP^T(i)
+  uint64_t* p_full = bars + 3;       // compute -> MMA: P^T(i) in TMEM, S^T(i) consumed            (256 arrivals)
+  uint64_t* ds_full = bars + 4;      // compute -> MMA: dS^T(i) in smem, dP^T(i) consumed          (256 arrivals)
+  uint64_t* ds_empty = bars + 5;     // MMA -> compute: dK(i), dQ(i) have read dS^T(i)
+  uint64_t* dq_full = bars + 6;      // MMA -> drain: dQ(i) in TMEM
+  uint64_t* dq_empty = bars + 7;     // drain -> MMA: dQ(i) in registers                            (128 arrivals)
+  uint64_t* dkv_full = bars + 8;     // MMA -> compute: dK_j, dV_j complete
+  uint64_t* q_full = bars + 9;       // [kStages] TMA -> MMA, compute
+  uint64_t* q_empty = q_full + Cfg::kStages;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(q_empty + Cfg::kStages);
+
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+  const int lane = threadIdx.x & 31;
+  const int bh = blockIdx.y;
+  const int n_q = N / kTile;
+  const int q_row0 = bh * N;                                  // rows of this head in the [BH*N, d] views
+  const int k_row0 = bh * N + k_off + blockIdx.x * kTile;
+
+  if (threadIdx.x == 0) {
+    mbar_init(kv_full, 1);
+    mbar_init(s_full, 1);
+    mbar_init(dp_full, 1);
+    mbar_init(p_full, 256);
+    mbar_init(ds_full, 256);
+    mbar_init(ds_empty, 1);
+    mbar_init(dq_full, 1);
+    mbar_init(dq_empty, 128);
+    mbar_init(dkv_full, 1);
+    for (int i = 0; i < Cfg::kStages; ++i) {
+      mbar_init(&q_full[i], 1);
+      mbar_init(&q_empty[i], 1);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 12) {
+    if (lane == 0) {
+      prefetch_tmap(&map_q);
+      prefetch_tmap(&map_k);
+      prefetch_tmap(&map_v);
+      prefetch_tmap(&map_do);
+    }
+    tmem_alloc<512>(tmem_slot);
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+
+  if (warp == 12) {
+    // ------------------------------------------------------------------ TMA producer
+    const bool leader = elect_one();
+    const uint64_t pol_kv = policy_evict_first();
+    const uint64_t pol_q = policy_evict_last();      // Q/dO tiles are re-read by every CTA of the head
+    if (leader) {
+      mbar_arrive_expect_tx(kv_full, 2 * Cfg::kTileBytes);
+#pragma unroll
+      for (int p = 0; p < Cfg::kPanels; ++p) {
+        tma_load_2d(sK + p * Cfg::kPanelBytes, &map_k, kv_full, p * 64, k_row0, pol_kv);
+        tma_load_2d(sV + p * Cfg::kPanelBytes, &map_v, kv_full, p * 64, k_row0, pol_kv);
+      }
+    }
+    __syncwarp();
+    int stage = 0, phase = 0;
+    for (int i = 0; i < n_q; ++i) {
+      mbar_wait(&q_empty[stage], phase ^ 1);
+      if (leader) {
+        uint8_t* st = sStage + stage * Cfg::kStageBytes;
+        const int row = q_row0 + i * kTile;
+        mbar_arrive_expect_tx(&q_full[stage], Cfg::kStageBytes);
+#pragma unroll
+        for (int p = 0; p < Cfg::kPanels; ++p) {
+          tma_load_2d(st + p * Cfg::kPanelBytes, &map_q, &q_full[stage], p * 64, row, pol_q);
+          tma_load_2d(st + Cfg::kTileBytes + p * Cfg::kPanelBytes, &map_do, &q_full[stage], p * 64, row, pol_q);
+        }
+        bulk_load_1d(st + 2 * Cfg::kTileBytes, lse2 + row, 512, &q_full[stage]);
+        bulk_load_1d(st + 2 * Cfg::kTileBytes + 512, Dvec + row, 512, &q_full[stage]);
+      }
+      __syncwarp();
+      if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
+    }
+  } else if (warp == 13) {
+    // ------------------------------------------------------------------ MMA issuer
+    const bool leader = elect_one();
+    constexpr uint32_t idesc_st = make_idesc_bf16(kTile, kTile, 0, 0);   // K_j (K-major) x Q_i^T (K-major)
+    constexpr uint32_t idesc_kn = make_idesc_bf16(kTile, kD, 0, 1);      // A K-major/TMEM x B MN-major -> [128, d]
+    constexpr uint32_t idesc_mn = make_idesc_bf16(kTile, kD, 1, 1);      // A MN-major (dS from dS^T) x B MN-major
+    const uint32_t k_addr = smem_u32(sK), v_addr = smem_u32(sV), ds_addr = smem_u32(sDs);
+    const uint32_t stage_addr = smem_u32(sStage);
+    auto kmajor = [](uint32_t base, int k) {   // K-step k of a K-major [128 rows][d or 128] tile (64-element panels)
+      return make_smem_desc_sw128(base + (k >> 2) * Cfg::kPanelBytes + (k & 3) * 32, 16, 1024);
+    };
+    auto mnmajor = [](uint32_t base, int k) {  // K-step k (16 rows) of a [K rows][MN contiguous] tile
+      return make_smem_desc_sw128(base + k * 2048, Cfg::kPanelBytes, 1024);
+    };
+    auto commit = [&](uint64_t* bar) {
+      if (leader) mma_commit(bar);
+      __syncwarp();
+    };
+    // S^T(i) = K_j Q_i^T ; dP^T(i) = V_j dO_i^T
+    auto issue_st = [&](uint32_t q_addr) {
+      if (leader) {
+#pragma unroll
+        for (int k = 0; k < kD / 16; ++k) mma_ss(tmem + Cfg::tS, kmajor(k_addr, k), kmajor(q_addr, k), idesc_st, k > 0);
+        mma_commit(s_full);
+      }
+      __syncwarp();
+    };
+    auto issue_dpt = [&](uint32_t do_addr) {
+      if (leader) {
+#pragma unroll
+        for (int k = 0; k < kD / 16; ++k) mma_ss(tmem + Cfg::tDP, kmajor(v_addr, k), kmajor(do_addr, k), idesc_st, k > 0);
+        mma_commit(dp_full);
+      }
+      __syncwarp();
+    };
+    mbar_wait(kv_full, 0);
+    mbar_wait(&q_full[0], 0);
+    tc_fence_after();
+    issue_st(stage_addr);
+    issue_dpt(stage_addr + Cfg::kTileBytes);
+    int stage = 0, phase = 0;
+    for (int i = 0; i < n_q; ++i) {
+      const uint32_t q_addr = stage_addr + stage * Cfg::kStageBytes, do_addr = q_addr + Cfg::kTileBytes;
+      const int cur_stage = stage;
+      if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
+      const uint32_t nq_addr = stage_addr + stage * Cfg::kStageBytes;
+      const bool more = i + 1 < n_q;
+      // ---- behind phase A: dV += P^T(i) dO_i, then S^T(i+1)
+      mbar_wait(p_full, i & 1);
+      tc_fence_after();
+      if (leader) {
+#pragma unroll
+        for (int k = 0; k < kTile / 16; ++k)
+          mma_ts(tmem + Cfg::tDV, tmem + Cfg::tS + (k >> 2) * 64 + (k & 3) * 8, mnmajor(do_addr, k), idesc_kn,
+                 i > 0 || k > 0);
+      }
+      __syncwarp();
+      if (more) {
+        mbar_wait(&q_full[stage], phase);
+        tc_fence_after();
+        issue_st(nq_addr);
+      }
+      // ---- behind phase B: dK += dS^T(i) Q_i, dQ(i) = dS(i) K_j, then dP^T(i+1)
+      mbar_wait(ds_full, i & 1);
+      if (!Cfg::kDqOverlaysDp && i > 0) mbar_wait(dq_empty, (i - 1) & 1);
+      tc_fence_after();
+      if (leader) {
+#pragma unroll
+        for (int k = 0; k < kTile / 16; ++k)
+          mma_ss(tmem + Cfg::tDK, kmajor(ds_addr, k), mnmajor(q_addr, k), idesc_kn, i > 0 || k > 0);
+#pragma unroll
+        for (int k = 0; k < kTile / 16; ++k)
+          mma_ss(tmem + Cfg::tDQ, mnmajor(ds_addr, k), mnmajor(k_addr, k), idesc_mn, k > 0);
+        mma_commit(dq_full);
+        mma_commit(ds_empty);
+        mma_commit(&q_empty[cur_stage]);
+      }
+      __syncwarp();
+      if (more) {
+        if (Cfg::kDqOverlaysDp) {
+          mbar_wait(dq_empty, i & 1);      // dQ(i) sits in the dP^T columns until the drain warps took it
+          tc_fence_after();
+        }
+        issue_dpt(nq_addr + Cfg::kTileBytes);
+      }
+    }
+    commit(dkv_full);
+  } else if (warp < 8) {
+    // ------------------------------------------------------------------ compute warps
+    const int half = warp >> 2;                                  // which 64 query columns of the tile
+    const int row = (warp & 3) * 32 + lane;                      // key row of the tile = TMEM lane
+    const uint32_t lane_off = static_cast<uint32_t>((warp & 3) * 32) << 16;
+    const uint32_t tS = tmem + Cfg::tS + lane_off + half * 64;   // my S^T columns; P^T goes to the first 32 of them
+    const uint32_t tDP = tmem + Cfg::tDP + lane_off + half * 64;
+    uint8_t* ds_row = sDs + half * Cfg::kPanelBytes + row * 128;
+    int stage = 0, phase = 0;
+    for (int i = 0; i < n_q; ++i) {
+      const float4* stats = reinterpret_cast<const float4*>(sStage + stage * Cfg::kStageBytes + 2 * Cfg::kTileBytes);
+      const float4* lse4 = stats + half * 16;                    // lse2 of my 64 query columns
+      const float4* d4 = stats + 32 + half * 16;                 // D of my 64 query columns
+      mbar_wait(&q_full[stage], phase);
+      if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
+      // ---- phase A: P^T = exp2(scale_log2 * S^T - lse2)
+      mbar_wait(s_full, i & 1);
+      tc_fence_after();
+      float p[64];
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        uint32_t s[32];
+        tmem_ld_x32(tS + c * 32, s);
+        tmem_wait_ld();
+        uint32_t pk[16];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          const float4 l = lse4[c * 8 + g];
+          const float p0 = ex2(fmaf(__uint_as_float(s[g * 4 + 0]), scale_log2, -l.x));
+          const float p1 = ex2(fmaf(__uint_as_float(s[g * 4 + 1]), scale_log2, -l.y));
+          const float p2 = ex2(fmaf(__uint_as_float(s[g * 4 + 2]), scale_log2, -l.z));
+          const float p3 = ex2(fmaf(__uint_as_float(s[g * 4 + 3]), scale_log2, -l.w));
+          p[c * 32 + g * 4 + 0] = p0; p[c * 32 + g * 4 + 1] = p1;
+          p[c * 32 + g * 4 + 2] = p2; p[c * 32 + g * 4 + 3] = p3;
+          pk[g * 2] = pack_bf16x2(p0, p1);
+          pk[g * 2 + 1] = pack_bf16x2(p2, p3);
+        }
+        tmem_st_x16(tS + c * 16, pk);      // overlays only S^T columns this thread has already loaded
+      }
+      tmem_wait_st();
+      tc_fence_before();
+      mbar_arrive(p_full);
+      // ---- phase B: dS^T = P^T o (dP^T - D), bf16, to shared memory [keys][queries] (128B-swizzled rows)
+      mbar_wait(dp_full, i & 1);
+      if (i > 0) mbar_wait(ds_empty, (i - 1) & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        uint32_t dp[32];
+        tmem_ld_x32(tDP + c * 32, dp);
+        tmem_wait_ld();
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {     // 8 queries = one 16-byte chunk of the row
+          const float4 da = d4[c * 8 + g * 2], db = d4[c * 8 + g * 2 + 1];
+          const int e = c * 32 + g * 8;
+          const uint32_t w0 = pack_bf16x2(p[e + 0] * (__uint_as_float(dp[g * 8 + 0]) - da.x),
+                                          p[e + 1] * (__uint_as_float(dp[g * 8 + 1]) - da.y));
+          const uint32_t w1 = pack_bf16x2(p[e + 2] * (__uint_as_float(dp[g * 8 + 2]) - da.z),
+                                          p[e + 3] * (__uint_as_float(dp[g * 8 + 3]) - da.w));
+          const uint32_t w2 = pack_bf16x2(p[e + 4] * (__uint_as_float(dp[g * 8 + 4]) - db.x),
+                                          p[e + 5] * (__uint_as_float(dp[g * 8 + 5]) - db.y));
+          const uint32_t w3 = pack_bf16x2(p[e + 6] * (__uint_as_float(dp[g * 8 + 6]) - db.z),
+                                          p[e + 7] * (__uint_as_float(dp[g * 8 + 7]) - db.w));
+          const int chunk = c * 4 + g;
+          st_shared_v4(ds_row + ((chunk ^ (row & 7)) << 4), w0, w1, w2, w3);
+        }
+      }
+      fence_proxy_async_smem();
+      tc_fence_before();
+      mbar_arrive(ds_full);
+    }
+    // ---- epilogue: dV_j (warps 0-3) and scale * dK_j (warps 4-7), bf16, written once
+    mbar_wait(dkv_full, 0);
+    tc_fence_after();
+    const uint32_t tSrc = tmem + (half == 0 ? Cfg::tDV : Cfg::tDK) + lane_off;
+    const float mul = half == 0 ? 1.0f : scale;
+    __nv_bfloat16* dst_base = (half == 0 ? dv : dk) + (static_cast<size_t>(k_row0) + row) * kD;
+#pragma unroll
+    for (int c = 0; c < kD / 32; ++c) {
+      uint32_t r[32];
+      tmem_ld_x32(tSrc + c * 32, r);
+      tmem_wait_ld();
+      uint4* dst = reinterpret_cast<uint4*>(dst_base + c * 32);
+#pragma unroll
+      for (int g = 0; g < 4; ++g) {
+        uint4 u;
+        u.x = pack_bf16x2(__uint_as_float(r[g * 8 + 0]) * mul, __uint_as_float(r[g * 8 + 1]) * mul);
+        u.y = pack_bf16x2(__uint_as_float(r[g * 8 + 2]) * mul, __uint_as_float(r[g * 8 + 3]) * mul);
+        u.z = pack_bf16x2(__uint_as_float(r[g * 8 + 4]) * mul, __uint_as_float(r[g * 8 + 5]) * mul);
+        u.w = pack_bf16x2(__uint_as_float(r[g * 8 + 6]) * mul, __uint_as_float(r[g * 8 + 7]) * mul);
+        dst[g] = u;
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------ dQ drain warps (8-11)
+    const int row = (warp & 3) * 32 + lane;                      // query row of the tile = TMEM lane
+    const uint32_t tDQ = tmem + Cfg::tDQ + (static_cast<uint32_t>((warp & 3) * 32) << 16);
+    float* dst_row = dq_acc + (static_cast<size_t>(q_row0) + row) * kD;
+    for (int i = 0; i < n_q; ++i) {
+      mbar_wait(dq_full, i & 1);
+      tc_fence_after();
+      float* dst = dst_row + static_cast<size_t>(i) * kTile * kD;
+#pragma unroll
+      for (int c = 0; c < kD / 32; ++c) {
+        uint32_t r[32];
+        tmem_ld_x32(tDQ + c * 32, r);
+        tmem_wait_ld();
+        if (c == kD / 32 - 1) {          // the whole dQ(i) row is in registers: hand the columns back
+          tc_fence_before();
+          mbar_arrive(dq_empty);
+        }
+#pragma unroll
+        for (int e = 0; e < 32; e += 4)
+          red_add_v4(dst + c * 32 + e, __uint_as_float(r[e]), __uint_as_float(r[e + 1]), __uint_as_float(r[e + 2]),
+                     __uint_as_float(r[e + 3]));
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 12) tmem_dealloc<512>(tmem);
 }
+
+template <int kD>
+cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
+                     const float* lse2, const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
+                     int nk, float scale, cudaStream_t stream) {
+  using Cfg = BwdCfg<kD>;
+  auto kern = attn_chunk_bwd_kernel<kD>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  dim3 grid(nk / kTile, BH);
+  kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, lse2, D, dq_acc,
+                                                       static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv),
+                                                       N, k_off, scale * 1.4426950408889634f, scale);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
+                                        const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
+                                        int nk, int d, float scale, cudaStream_t stream) {
+  CUtensorMap mq, mk, mv, mdo;
+  const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+  const uint64_t rows = (uint64_t)BH * N;
+  if (!make_tmap_2d(&mq, q, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mk, k, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mv, v, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B))
+    return cudaErrorInvalidValue;
+  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, lse2, D, dq_acc, dk, dv, BH, N, k_off, nk, scale, stream);
+  return launch_t<128>(mq, mk, mv, mdo, lse2, D, dq_acc, dk, dv, BH, N, k_off, nk, scale, stream);
+}
+
 }  // namespace ringx

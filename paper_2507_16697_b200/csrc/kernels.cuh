@@ -14,8 +14,8 @@ namespace ringx {
 // ---- merge.cu (HBM-bound helpers)
 cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b, void* o_out,
                              float* lse_out, long long rows, int d, int in_dtype, int out_dtype, cudaStream_t stream);
-cudaError_t launch_bwd_preprocess(const void* o, const void* dO, float* D, float* dq_acc, long long rows, int d,
-                                  cudaStream_t stream);
+cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* lse, float* D, float* lse2,
+                                  float* dq_acc, long long rows, int d, cudaStream_t stream);
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
 
 // ---- attn_f32.cu (plain FFMA path, config C1)
@@ -33,7 +33,8 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
 // ---- attn_bwd_sm100.cu (tcgen05 path)
 // One KV-chunk pass of the backward: writes dk,dv rows [k_off, k_off+nk) of every head (bf16),
 // reduce-adds this chunk's contribution into dq_acc (fp32 [BH,N,d], unscaled by `scale`).
-cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse,
+// lse2 = LSE * log2(e) and D = rowsum(dO*O) come from launch_bwd_preprocess.
+cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
                                         int nk, int d, float scale, cudaStream_t stream);
 

@@ -1,6 +1,6 @@
 // merge.cu -- HBM-bound helper kernels of the RingX hot path:
 //   lse_merge_kernel   two-operand Eq. (5): SURVEY.md §8(a) row a5/a6
-//   bwd_preprocess     D_i = sum_c dO_ic O_ic and zeroing of the fp32 dQ accumulator: row a7
+//   bwd_preprocess     D_i = sum_c dO_ic O_ic, lse2_i = LSE_i log2(e), zeroing of the fp32 dQ accumulator: row a7
 //   dq_convert         dq = bf16(scale * dq_acc): row a9
 // Roofline: HBM bandwidth.  Algorithmic bytes per row: merge 2*(d*e_in+4) read + (d*e_out+4)
 // written; preprocess 2*d*2 read + 4 written (+ d*4 zeroed); convert d*4 read + d*2 written.
@@ -147,8 +147,8 @@ cudaError_t launch_merge_t(const void* o_a, const float* lse_a, const void* o_b,
 // 8 bf16 (16 B) of dO and of O; d/8 lanes per row.  Also zeroes the row of the fp32 dQ accumulator.
 template <int kLanes>
 __global__ void __launch_bounds__(256)
-bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO, float* __restrict__ D,
-                      float4* __restrict__ dq_acc, long long rows) {
+bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO, const float* __restrict__ lse,
+                      float* __restrict__ D, float* __restrict__ lse2, float4* __restrict__ dq_acc, long long rows) {
   constexpr int kRowsPerWarp = 32 / kLanes;
   const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
   const long long warp_global = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -181,7 +181,10 @@ bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO,
       }
 #pragma unroll
       for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
-      if (r < rows && l == 0) D[r] = s;
+      if (r < rows && l == 0) {
+        D[r] = s;
+        lse2[r] = lse[r] * 1.4426950408889634f;   // the backward kernel works in the exp2 domain
+      }
     }
   }
 }
@@ -213,17 +216,17 @@ cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_
   return launch_merge_t<__nv_bfloat16, __nv_bfloat16>(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, stream);
 }
 
-cudaError_t launch_bwd_preprocess(const void* o, const void* dO, float* D, float* dq_acc, long long rows, int d,
-                                  cudaStream_t stream) {
+cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* lse, float* D, float* lse2,
+                                  float* dq_acc, long long rows, int d, cudaStream_t stream) {
   const int lanes = d / 8;   // 8 or 16
   const long long rows_per_block = 8LL * (32 / lanes) * 4;
   long long blocks = (rows + rows_per_block - 1) / rows_per_block;
   if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
   if (lanes == 8)
-    bwd_preprocess_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, D,
+    bwd_preprocess_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, lse, D, lse2,
                                                                    (float4*)dq_acc, rows);
   else
-    bwd_preprocess_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, D,
+    bwd_preprocess_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, lse, D, lse2,
                                                                     (float4*)dq_acc, rows);
   return cudaGetLastError();
 }
