@@ -101,3 +101,68 @@ def test_voxel_order_is_metadata(rx):
                                  cfg.kv_chunk, cfg.scale)
     assert (lse2 - lse[:, :, idx]).abs().max().item() <= 5e-5
     assert ((o2.float() - o.float()[:, :, idx]).norm() / o.float().norm()).item() <= 4e-3
+
+
+def test_C4_full_size_forward_and_backward(rx):
+    """BASELINE.json configs[3]: B=2,H=16,N=65536,d=64, kv_chunk=8192, fwd + bwd.  Oracle on sampled query rows
+    (O, LSE, dQ -- exact per row) and on sampled key columns of one head (dK, dV -- needs LSE_i and D_i of ALL
+    65536 rows of that head: one full 4*N^2*d fp64 pass), plus O(N d) invariants on the full GPU output."""
+    cfg = wl.CONFIGS["C4"]
+    q, k, v, do = wl.make_qkv(cfg, with_do=True, device="cuda")
+    o, lse = rx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale)
+    dq, dk, dv = rx.ringx_attn_bwd(q, k, v, o, lse, do, cfg.kv_chunk, cfg.scale)
+    torch.cuda.synchronize()
+    assert rx.ringx_last_launch_count() == cfg.N // cfg.kv_chunk + 2
+    for t in (dq, dk, dv):
+        assert torch.isfinite(t.float()).all()
+    # ---- sampled rows: forward and dQ
+    for (b, h) in [(0, 0), (1, 9)]:
+        rows = sample_rows(cfg.N, 64, seed=cfg.seed + 100 * b + h)
+        k64, v64 = wl.to_f64_numpy(k[b, h]), wl.to_f64_numpy(v[b, h])
+        q64, do64 = wl.to_f64_numpy(q[b, h][rows]), wl.to_f64_numpy(do[b, h][rows])
+        o_ref, lse_ref = orc.attention_fwd(q64, k64, v64, cfg.scale)
+        dq_ref, _, _ = orc.attention_bwd(q64, k64, v64, do64, cfg.scale)
+        og = o[b, h][rows].float().cpu().double().numpy()
+        assert np.abs(og - o_ref).max() <= 1e-2 * np.abs(v64).max()
+        assert np.linalg.norm(og - o_ref) / np.linalg.norm(o_ref) <= 1e-2
+        assert np.abs(lse[b, h][rows].cpu().double().numpy() - lse_ref).max() <= 1e-3
+        dqg = dq[b, h][rows].float().cpu().double().numpy()
+        assert np.linalg.norm(dqg - dq_ref) / np.linalg.norm(dq_ref) <= 2e-2
+    # ---- sampled key columns of one head: dK, dV (tile / chunk boundaries + random)
+    b, h = 1, 3
+    q64, k64, v64, do64 = (wl.to_f64_numpy(t[b, h]) for t in (q, k, v, do))
+    lse_all = np.empty(cfg.N)
+    D_all = np.empty(cfg.N)
+    for r0 in range(0, cfg.N, 2048):
+        lse_all[r0:r0 + 2048], D_all[r0:r0 + 2048] = orc.row_stats(q64[r0:r0 + 2048], k64, v64, do64[r0:r0 + 2048],
+                                                                   cfg.scale)
+    assert np.abs(lse[b, h].cpu().double().numpy() - lse_all).max() <= 1e-3       # every row of the head
+    C = cfg.kv_chunk
+    cols = sorted(set([0, 127, 128, C - 1, C, C + 127, 3 * C - 1, 3 * C, cfg.N - 128, cfg.N - 1])
+                  | set(np.random.default_rng(cfg.seed).integers(0, cfg.N, 54).tolist()))
+    cols = np.array(cols)
+    dk_ref, dv_ref = orc.attention_bwd_cols(q64, k64[cols], v64[cols], do64, lse_all, D_all, cfg.scale)
+    dkg = dk[b, h][cols].float().cpu().double().numpy()
+    dvg = dv[b, h][cols].float().cpu().double().numpy()
+    assert np.linalg.norm(dkg - dk_ref) / np.linalg.norm(dk_ref) <= 2e-2
+    assert np.linalg.norm(dvg - dv_ref) / np.linalg.norm(dv_ref) <= 2e-2
+    # ---- invariants on the full output (every head)
+    sum_dv, sum_do = dv.float().sum(dim=2), do.float().sum(dim=2)
+    assert ((sum_dv - sum_do).norm() / sum_do.norm()).item() <= 1e-2
+    assert (dk.float().sum(dim=2).norm() / dk.float().abs().sum(dim=2).norm()).item() <= 1e-2
+
+
+def test_C3_shape_backward_d128_sampled(rx):
+    """d = 128 backward at a long sequence (one head of the C3 shape family, N = 65536): dQ rows vs the oracle."""
+    B, H, N, d, chunk = 1, 2, 65536, 128, 16384
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=71, device="cuda")
+    scale = 1.0 / math.sqrt(d)
+    o, lse = rx.ringx_attn_fwd(q, k, v, chunk, scale)
+    dq, dk, dv = rx.ringx_attn_bwd(q, k, v, o, lse, do, chunk, scale)
+    rows = sample_rows(N, 48, seed=5)
+    k64, v64 = wl.to_f64_numpy(k[0, 1]), wl.to_f64_numpy(v[0, 1])
+    dq_ref, _, _ = orc.attention_bwd(wl.to_f64_numpy(q[0, 1][rows]), k64, v64, wl.to_f64_numpy(do[0, 1][rows]), scale)
+    assert np.linalg.norm(dq[0, 1][rows].float().cpu().double().numpy() - dq_ref) / np.linalg.norm(dq_ref) <= 2e-2
+    sum_dv, sum_do = dv.float().sum(dim=2), do.float().sum(dim=2)
+    assert ((sum_dv - sum_do).norm() / sum_do.norm()).item() <= 1e-2
+    assert (dk.float().sum(dim=2).norm() / dk.float().abs().sum(dim=2).norm()).item() <= 1e-2

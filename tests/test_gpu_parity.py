@@ -308,3 +308,93 @@ def test_errors_on_the_gpu_box(rx):
     with pytest.raises(rx.RingxError) as e:
         rx.ringx_attn_fwd(q, q, q, 256, -1.0)
     assert e.value.status == 2
+
+
+# ------------------------------------------------------------------------------------------------
+# backward: dQ, dK, dV against the oracle's derivative of the definition (reading g8)
+# ------------------------------------------------------------------------------------------------
+def rel_f(g, ref):
+    return np.linalg.norm(g.float().cpu().double().numpy() - ref) / np.linalg.norm(ref)
+
+
+BWD_SHAPES = [
+    # B, H, N, d, kv_chunk, qk_gain
+    (1, 1, 128, 64, 128, 1.0),             # one tile pair: minimum size (backward needs N % 128 only)
+    (1, 1, 256, 128, 256, 1.0),
+    (2, 2, 1152, 64, 384, 1.0),            # 9 query tiles (ring of 3 wraps), 3 passes of 3 key tiles
+    (1, 2, 1280, 128, 256, 1.0),           # d = 128: dQ overlays dP^T in TMEM, ring of 2
+    (1, 1, 2048, 64, 2048, 3.0),           # peaked softmax, single pass
+    (1, 2, 1024, 128, 128, 3.0),           # 8 passes
+    (1, 1, 1024, 64, 512, 0.05),           # nearly uniform softmax
+]
+
+
+@pytest.mark.parametrize("B,H,N,d,chunk,gain", BWD_SHAPES)
+def test_bwd_bf16_matches_oracle(rx, B, H, N, d, chunk, gain):
+    q, k, v, do = (wl.make_tensor((B, H, N, d), w, seed=53, dtype="bf16", gain=(gain if w in "qk" else 1.0))
+                   for w in ("q", "k", "v", "do"))
+    scale = 1.0 / math.sqrt(d)
+    qd, kd, vd, dod = q.cuda(), k.cuda(), v.cuda(), do.cuda()
+    if N % 256 == 0:
+        o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
+    else:   # the bf16 forward needs N % 256 == 0: take (o, lse) of this shape from the oracle instead
+        o64, lse64 = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+        o, lse = torch.from_numpy(o64).to(torch.bfloat16).cuda(), torch.from_numpy(lse64).float().cuda()
+    dq, dk, dv = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale)
+    assert rx.ringx_last_launch_count() == N // chunk + 2
+    dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(f64(q), f64(k), f64(v), f64(do), scale)
+    for name, g, r in (("dq", dq, dq_ref), ("dk", dk, dk_ref), ("dv", dv, dv_ref)):
+        assert torch.isfinite(g.float()).all()
+        e = rel_f(g, r)
+        assert e <= TOL_GRAD, (name, e)
+        assert e <= 8e-3, (name, e)        # expected ~2.4e-3 (bf16 P, dS and outputs); 5e-3 when peaked
+
+
+def test_bwd_is_independent_of_kv_chunk_and_repeatable_within_rounding(rx):
+    """dK/dV of a key tile are written once by one CTA -> bit-identical across chunkings; dQ is an fp32
+    reduce-add in arbitrary order -> equal up to fp32 rounding before the final bf16 cast."""
+    B, H, N, d = 1, 2, 1024, 64
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=59)
+    qd, kd, vd, dod = q.cuda(), k.cuda(), v.cuda(), do.cuda()
+    scale = 0.125
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, N, scale)
+    ref = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, N, scale)
+    for chunk in (128, 256, 512):
+        dq, dk, dv = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale)
+        assert torch.equal(dk, ref[1]) and torch.equal(dv, ref[2])
+        assert ((dq.float() - ref[0].float()).norm() / ref[0].float().norm()).item() <= 2e-3
+
+
+def test_bwd_invariants_and_degenerate_dO(rx):
+    """sum_j dV_j = sum_i dO_i; sum_j dK_j = 0; dO = 0 => all gradients 0; linear in dO."""
+    B, H, N, d = 1, 2, 1024, 64
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=61)
+    qd, kd, vd, dod = q.cuda(), k.cuda(), v.cuda(), do.cuda()
+    scale = 0.125
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, 256, scale)
+    dq, dk, dv = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, 256, scale)
+    sum_dv = dv.float().sum(dim=2)
+    sum_do = dod.float().sum(dim=2)
+    assert ((sum_dv - sum_do).norm() / sum_do.norm()).item() <= 1e-2
+    assert (dk.float().sum(dim=2).norm() / dk.float().abs().sum(dim=2).norm()).item() <= 1e-2
+    z = torch.zeros_like(dod)
+    dq0, dk0, dv0 = rx.ringx_attn_bwd(qd, kd, vd, o, lse, z, 256, scale)
+    assert not dq0.float().any() and not dk0.float().any() and not dv0.float().any()
+    dq2, dk2, dv2 = rx.ringx_attn_bwd(qd, kd, vd, o, lse, (dod.float() * 2).to(torch.bfloat16), 256, scale)
+    for a, b_ in ((dq2, dq), (dk2, dk), (dv2, dv)):
+        assert ((a.float() - 2 * b_.float()).norm() / (2 * b_.float()).norm()).item() <= 5e-3
+
+
+def test_bwd_errors(rx):
+    q = torch.zeros(1, 1, 256, 64, dtype=torch.float32, device="cuda")
+    lse = torch.zeros(1, 1, 256, device="cuda")
+    with pytest.raises(KeyError):
+        rx.ringx_attn_bwd(q.half(), q.half(), q.half(), q.half(), lse, q.half(), 256, 0.125)   # fp16 unsupported
+    with pytest.raises(rx.RingxError) as e:
+        rx.ringx_attn_bwd(q, q, q, q, lse, q, 256, 0.125)                                      # f32 backward
+    assert e.value.status == 3
+    qb = q.to(torch.bfloat16)
+    with pytest.raises(rx.RingxError) as e:
+        rx.ringx_attn_bwd(qb, qb, qb, qb, lse, qb, 256, 0.125,
+                          workspace=torch.empty(512, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == 5
