@@ -3,11 +3,13 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C3]
 
-A "step" is one pass of the hot path over one batch of synthetic input of the named BASELINE.json config
-(default C3: bf16, B=1, H=8, N=262144, d=128, kv_chunk=32768 -- the configuration the north_star's target
-"bf16 forward at N >= 262,144" is quoted on): `ringx_attn_fwd` = 8 KV-chunk passes of the tcgen05 kernel +
-7 Eq. 5 merges; configs with `backward` add `ringx_attn_bwd`.  FLOPs: forward 4*B*H*N^2*d,
-backward 10*B*H*N^2*d.  Inputs are seeded synthetic (paper_2507_16697_b200/workloads.py), resident in HBM for
+A "step" is one pass of the WHOLE hot path over one batch of synthetic input of
+the named BASELINE.json config (default C3: bf16, B=1, H=8, N=262144, d=128, kv_chunk=32768 -- the configuration
+the north_star's target "bf16 forward at N >= 262,144" is quoted on): `ringx_attn_fwd` (8 KV-chunk passes of the
+tcgen05 kernel + 7 Eq. 5 merges) followed by `ringx_attn_bwd` (D_i preprocess, 8 backward chunk passes, dQ
+convert).  `--pass fwd` times the forward alone.  FLOPs: forward 4*B*H*N^2*d, backward
+10*B*H*N^2*d; `value` is their sum over the step time, and the line also carries forward-only and backward-only
+TFLOP/s from the live per-kernel CUDA-event timing.  Inputs are seeded synthetic (paper_2507_16697_b200/workloads.py), resident in HBM for
 `value`; `e2e` times the same metric through the C ABI with HOST buffers (H2D + D2H inside the timed region).
 Multi-GPU (--gpus N under torchrun): the path has no exchange step on one node (batch x heads
 are independent) -> every rank runs the workload on its own seeded batch, no data-path collective, "weak".
@@ -31,7 +33,8 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 import torch  # noqa: E402
 
-METRIC = "attention TFLOPS fwd at 1 B200 (4*B*H*N^2*d; fraction of dense bf16 tensor peak in roofline.frac)"
+METRIC = ("attention TFLOPS fwd+bwd at 1 B200 (fwd 4*B*H*N^2*d + bwd 10*B*H*N^2*d per step; fwd-only and bwd-only in "
+          "`fwd`/`bwd`; fraction of dense bf16 tensor peak in roofline.frac)")
 UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 
@@ -118,15 +121,17 @@ def host_cores() -> int:
         return os.cpu_count() or 1
 
 
-def oracle_sample(cfg, k64, v64, q_rows64, block=256):
-    """The oracle as it stands on a bounded sample: `attention_fwd` of the sampled query rows of one head
-    against ALL keys of that head.  Returns (seconds, flops)."""
+def oracle_sample(cfg, k64, v64, q_rows64, do_rows64=None, block=256):
+    """The oracle as it stands on a bounded sample: `attention_fwd` (and `attention_bwd` when dO rows are given) of
+    the sampled query rows of one head against ALL keys of that head.  Returns (seconds, flops)."""
     from oracle import attention as orc
     t0 = time.perf_counter()
     for r0 in range(0, q_rows64.shape[0], block):
         orc.attention_fwd(q_rows64[r0:r0 + block], k64, v64, cfg.scale)
+        if do_rows64 is not None:
+            orc.attention_bwd(q_rows64[r0:r0 + block], k64, v64, do_rows64[r0:r0 + block], cfg.scale)
     dt = time.perf_counter() - t0
-    return dt, 4.0 * q_rows64.shape[0] * cfg.N * cfg.d
+    return dt, (4.0 if do_rows64 is None else 14.0) * q_rows64.shape[0] * cfg.N * cfg.d
 
 
 def run_reference(args, cfg, rank):
@@ -137,16 +142,18 @@ def run_reference(args, cfg, rank):
     rows_per_step = args.ref_rows
     # one head of the workload, generated on the host by the same counter-based recipe (first rows of head 0)
     head = wl.Config(cfg.name, cfg.dtype, 1, 1, cfg.N, cfg.d, cfg.kv_chunk, cfg.qk_gain, False, cfg.seed)
-    q, k, v = wl.make_qkv(head)
+    bwd = args.passes == "fwd+bwd"
+    q, k, v, do = wl.make_qkv(head, with_do=True)
     k64, v64 = wl.to_f64_numpy(k[0, 0]), wl.to_f64_numpy(v[0, 0])
-    q64 = wl.to_f64_numpy(q[0, 0])
+    q64, do64 = wl.to_f64_numpy(q[0, 0]), wl.to_f64_numpy(do[0, 0])
     rng = np.random.default_rng(0)
     for _ in range(args.warmup):
-        oracle_sample(cfg, k64, v64, q64[rng.integers(0, cfg.N, 64)])
+        rows = rng.integers(0, cfg.N, 64)
+        oracle_sample(cfg, k64, v64, q64[rows], do64[rows] if bwd else None)
     t_total, f_total = 0.0, 0.0
     for _ in range(args.steps):
         rows = rng.integers(0, cfg.N, rows_per_step)
-        dt, fl = oracle_sample(cfg, k64, v64, q64[rows])
+        dt, fl = oracle_sample(cfg, k64, v64, q64[rows], do64[rows] if bwd else None)
         t_total += dt
         f_total += fl
     value = f_total / t_total / 1e12
@@ -156,7 +163,7 @@ def run_reference(args, cfg, rank):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(cfg, "fwd"),
+        "config": workload_config(cfg, args.passes),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": host_cores(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -179,7 +186,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3", choices=["C2", "C3", "C4", "C5"])
-    ap.add_argument("--ref-rows", type=int, default=512, help="query rows per step of the reference arm")
+    ap.add_argument("--pass", dest="passes", default="fwd+bwd", choices=["fwd", "fwd+bwd"])
+    ap.add_argument("--ref-rows", type=int, default=256, help="query rows per step of the reference arm")
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--no-extra", action="store_true", help="skip the short C2/C4 side measurements")
     args = ap.parse_args()
@@ -217,25 +225,26 @@ def main():
     # ---------------------------------------------------------------- inputs (seeded, per-rank batch)
     rcfg = wl.Config(cfg.name, cfg.dtype, cfg.B, cfg.H, cfg.N, cfg.d, cfg.kv_chunk, cfg.qk_gain, cfg.backward,
                      cfg.seed + 1000 * rank)
-    tensors = wl.make_qkv(rcfg, with_do=cfg.backward, device=dev)
+    do_bwd = args.passes == "fwd+bwd"
+    tensors = wl.make_qkv(rcfg, with_do=do_bwd, device=dev)
     q, k, v = tensors[:3]
-    dO = tensors[3] if cfg.backward else None
+    dO = tensors[3] if do_bwd else None
     B, H, N, d = q.shape
     o = torch.empty_like(q)
     lse = torch.empty((B, H, N), dtype=torch.float32, device=dev)
     ws_f = torch.empty(max(256, ringx.ringx_attn_fwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
                        dtype=torch.uint8, device=dev)
     ws_b = None
-    if cfg.backward:
+    if do_bwd:
         ws_b = torch.empty(max(256, ringx.ringx_attn_bwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
                            dtype=torch.uint8, device=dev)
-    flops_step = cfg.fwd_flops + (cfg.bwd_flops if cfg.backward else 0.0)
+    flops_step = cfg.fwd_flops + (cfg.bwd_flops if do_bwd else 0.0)
     launches = [0]
 
     def step():
         ringx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale, o=o, lse=lse, workspace=ws_f)
         n = ringx.ringx_last_launch_count()
-        if cfg.backward:
+        if do_bwd:
             ringx.ringx_attn_bwd(q, k, v, o, lse, dO, cfg.kv_chunk, cfg.scale, workspace=ws_b)
             n += ringx.ringx_last_launch_count()
         launches[0] += n
@@ -271,57 +280,83 @@ def main():
     value = world * flops_step / (ms_step * 1e-3) / 1e12
     gpu_launches = launches[0]
 
-    # ---------------------------------------------------------------- roofline of the dominant kernel
+    # ---------------------------------------------------------------- roofline of the dominant kernel(s)
     peaks = load_peaks()
-    dom = "attn_bwd" if (cfg.backward and prof["attn_bwd"][0] > prof["attn_fwd"][0]) else "attn_fwd"
-    dom_ms, dom_n = prof[dom]
-    per_launch = (10.0 if dom == "attn_bwd" else 4.0) * B * H * N * cfg.kv_chunk * d
-    achieved = per_launch / (dom_ms / max(dom_n, 1) * 1e-3) / 1e12 if dom_n else None
-    roofline = {
-        "bound": "tensor", "kernel": "attn_chunk_fwd_kernel" if dom == "attn_fwd" else "attn_chunk_bwd_kernel",
-        "achieved": achieved, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
-        "frac": achieved / peaks["bf16_tflops_sustained"] if achieved else None,
-        "peak_kind": f"bf16 dense, sustained (kernel timed inside a long step), {peaks['source']}",
-        "peak_burst": peaks["bf16_tflops"], "frac_of_burst": achieved / peaks["bf16_tflops"] if achieved else None,
-        "frac_of_nominal_2250": achieved / 2250.0 if achieved else None,
-        "flops_per_launch": per_launch, "launches_timed": dom_n, "avg_launch_ms": dom_ms / max(dom_n, 1),
-        "share_of_step": dom_ms / ms_total if world == 1 else None,
-        "traffic": load_traffic(f"{cfg.name}_{dom}"),
-    }
+
+    def roofline_of(kind):
+        ms, n = prof[kind]
+        if not n:
+            return None
+        per_launch = (10.0 if kind == "attn_bwd" else 4.0) * B * H * N * cfg.kv_chunk * d
+        ach = per_launch / (ms / n * 1e-3) / 1e12
+        return {
+            "bound": "tensor", "kernel": "attn_chunk_fwd_kernel" if kind == "attn_fwd" else "attn_chunk_bwd_kernel",
+            "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+            "frac": ach / peaks["bf16_tflops_sustained"],
+            "peak_kind": f"bf16 dense, sustained (kernel timed inside a long step), {peaks['source']}",
+            "peak_burst": peaks["bf16_tflops"], "frac_of_burst": ach / peaks["bf16_tflops"],
+            "frac_of_nominal_2250": ach / 2250.0, "flops_per_launch": per_launch, "launches_timed": n,
+            "avg_launch_ms": ms / n, "share_of_step": ms / ms_total if world == 1 else None,
+            "traffic": load_traffic(f"{cfg.name}_{kind}"),
+        }
+
+    dom = "attn_bwd" if prof["attn_bwd"][0] > prof["attn_fwd"][0] else "attn_fwd"
+    roofline = roofline_of(dom)
+    roofline_other = roofline_of("attn_fwd" if dom == "attn_bwd" else "attn_bwd")
+    fwd_ms = (prof["attn_fwd"][0] + prof["merge"][0]) / args.steps
+    bwd_ms = (prof["attn_bwd"][0] + prof["bwd_aux"][0]) / args.steps
+    fwd_info = {"ms_per_step": fwd_ms, "tflops": cfg.fwd_flops / fwd_ms / 1e9,
+                "frac_of_sustained_peak": cfg.fwd_flops / fwd_ms / 1e9 / peaks["bf16_tflops_sustained"],
+                "frac_of_burst_peak": cfg.fwd_flops / fwd_ms / 1e9 / peaks["bf16_tflops"]} if fwd_ms > 0 else None
+    bwd_info = {"ms_per_step": bwd_ms, "tflops": cfg.bwd_flops / bwd_ms / 1e9,
+                "frac_of_sustained_peak": cfg.bwd_flops / bwd_ms / 1e9 / peaks["bf16_tflops_sustained"],
+                "frac_of_burst_peak": cfg.bwd_flops / bwd_ms / 1e9 / peaks["bf16_tflops"]} if bwd_ms > 0 else None
     merge_ms, merge_n = prof["merge"]
     merge_info = None
     if merge_n:
-        mbytes = 3.0 * B * H * N * (d * 4 + 4) - (B * H * N * d * 2 / merge_n)   # last merge writes bf16
-        merge_info = {"avg_launch_ms": merge_ms / merge_n, "launches_timed": merge_n,
-                      "achieved_gbs": mbytes / (merge_ms / merge_n * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
+        mbytes = 3.0 * B * H * N * (d * 4 + 4) - (B * H * N * d * 2 * args.steps / merge_n)   # last merge writes bf16
+        merge_info = {"bound": "hbm", "avg_launch_ms": merge_ms / merge_n, "launches_timed": merge_n,
+                      "achieved": mbytes / (merge_ms / merge_n * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                       "frac": mbytes / (merge_ms / merge_n * 1e-3) / 1e9 / peaks["hbm_gbs"]}
 
     # ---------------------------------------------------------------- e2e: HOST buffers through the C ABI
-    e2e = None
-    if not cfg.backward:
-        qh, kh, vh = (t.cpu().pin_memory() for t in (q, k, v))
-        oh = torch.empty_like(qh).pin_memory()
+    n_e2e = max(1, min(args.steps, 3))
+    tb = q.numel() * q.element_size()
+    if do_bwd:
+        host_in = [t.cpu().pin_memory() for t in (q, k, v, dO)]
+        outs = (torch.empty_like(host_in[0]).pin_memory(), torch.empty((B, H, N), dtype=torch.float32).pin_memory(),
+                torch.empty_like(host_in[0]).pin_memory(), torch.empty_like(host_in[0]).pin_memory(),
+                torch.empty_like(host_in[0]).pin_memory())
+        ws_h = torch.empty(ringx.ringx_attn_fwd_bwd_host_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype),
+                           dtype=torch.uint8, device=dev)
+        call = lambda: ringx.ringx_attn_fwd_bwd_host(*host_in, cfg.kv_chunk, cfg.scale, outs=outs, workspace=ws_h)
+        h2d, d2h = 4 * tb, 4 * tb + lse.numel() * 4
+        entry = "ringx_attn_fwd_bwd_host (pinned host q,k,v,dO -> device, fwd+bwd, o,lse,dq,dk,dv -> host, synchronised)"
+    else:
+        host_in = [t.cpu().pin_memory() for t in (q, k, v)]
+        oh = torch.empty_like(host_in[0]).pin_memory()
         lh = torch.empty((B, H, N), dtype=torch.float32).pin_memory()
         ws_h = torch.empty(ringx.ringx_attn_fwd_host_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype),
                            dtype=torch.uint8, device=dev)
-        n_e2e = max(1, min(args.steps, 3))
-        ringx.ringx_attn_fwd_host(qh, kh, vh, cfg.kv_chunk, cfg.scale, o_host=oh, lse_host=lh, workspace=ws_h)
-        barrier()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            ringx.ringx_attn_fwd_host(qh, kh, vh, cfg.kv_chunk, cfg.scale, o_host=oh, lse_host=lh, workspace=ws_h)
-        torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) / n_e2e
-        if dist is not None:
-            t = torch.tensor([dt], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = t.item()
-        e2e = {"value": world * cfg.fwd_flops / dt / 1e12, "unit": UNIT, "ms_per_step": dt * 1e3, "steps": n_e2e,
-               "h2d_bytes_per_step": 3 * q.numel() * q.element_size(),
-               "d2h_bytes_per_step": q.numel() * q.element_size() + lse.numel() * 4,
-               "entry": "ringx_attn_fwd_host (pinned host q,k,v -> device, forward, o+lse -> host, synchronised)"}
-        del ws_h, qh, kh, vh, oh, lh
+        call = lambda: ringx.ringx_attn_fwd_host(*host_in, cfg.kv_chunk, cfg.scale, o_host=oh, lse_host=lh,
+                                                 workspace=ws_h)
+        h2d, d2h = 3 * tb, tb + lse.numel() * 4
+        entry = "ringx_attn_fwd_host (pinned host q,k,v -> device, forward, o+lse -> host, synchronised)"
+    call()
+    barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        call()
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / n_e2e
+    if dist is not None:
+        t = torch.tensor([dt], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = t.item()
+    e2e = {"value": world * flops_step / dt / 1e12, "unit": UNIT, "ms_per_step": dt * 1e3, "steps": n_e2e,
+           "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "entry": entry}
+    del ws_h, host_in
 
     # ---------------------------------------------------------------- short side measurements (not the metric)
     extra = {}
@@ -336,22 +371,25 @@ def main():
     if rank == 0 and world == 1:
         k64, v64 = wl.to_f64_numpy(k[0, 0]), wl.to_f64_numpy(v[0, 0])
         q64 = wl.to_f64_numpy(q[0, 0, :8192])
-        dt0, _ = oracle_sample(cfg, k64, v64, q64[:128])
+        do64 = wl.to_f64_numpy(dO[0, 0, :8192]) if do_bwd else None
+        dt0, _ = oracle_sample(cfg, k64, v64, q64[:128], do64[:128] if do_bwd else None)
         n_rows = int(min(q64.shape[0], max(128, args.cpu_baseline_seconds / (dt0 / 128.0) // 128 * 128)))
-        dt, fl = oracle_sample(cfg, k64, v64, q64[:n_rows])
+        dt, fl = oracle_sample(cfg, k64, v64, q64[:n_rows], do64[:n_rows] if do_bwd else None)
         cpu_baseline = {"value": fl / dt / 1e12, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
                         "seconds": dt,
                         "sample": f"first {n_rows} query rows of head (0,0) against all {N} keys "
-                                  f"(oracle.attention_fwd, fp64 numpy, blocks of 256 rows)"}
+                                  f"(oracle.attention_fwd" + (" + attention_bwd" if do_bwd else "") +
+                                  ", fp64 numpy, blocks of 256 rows)"}
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": workload_config(cfg, "fwd+bwd" if cfg.backward else "fwd"),
+            "config": workload_config(cfg, args.passes),
             "clocks": clocks, "e2e": e2e, "gpu_launches": gpu_launches,
-            "roofline": roofline, "merge_kernel": merge_info, "cpu_baseline": cpu_baseline, "extra": extra,
+            "roofline": roofline, "roofline_other_kernel": roofline_other, "merge_kernel": merge_info,
+            "fwd": fwd_info, "bwd": bwd_info, "cpu_baseline": cpu_baseline, "extra": extra,
             "frac_of_bf16_peak": {"sustained": value / world / peaks["bf16_tflops_sustained"],
                                   "burst": value / world / peaks["bf16_tflops"], "nominal_2250": value / world / 2250.0,
                                   "source": peaks["source"]},

@@ -116,6 +116,17 @@ RINGX_API int ringx_attn_fwd_host(const void* q_host, const void* k_host, const 
                         int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
                         void* workspace, size_t workspace_bytes, void* stream);
 
+/* Forward + backward with HOST buffers (the end-to-end training-step entry): copies q,k,v,dO host->device
+ * into the workspace, runs ringx_attn_fwd then ringx_attn_bwd, copies o, lse, dq, dk, dv back and
+ * synchronises `stream`.  bf16 only.  All *_host pointers are HOST pointers (pinned recommended).
+ *   workspace  DEVICE, >= ringx_attn_fwd_bwd_host_workspace_bytes(...) bytes. */
+RINGX_API int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* v_host,
+                            const void* dO_host, void* o_host, float* lse_host,
+                            void* dq_host, void* dk_host, void* dv_host,
+                            int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
+                            void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_fwd_bwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
+
 RINGX_API size_t ringx_attn_fwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
 RINGX_API size_t ringx_attn_bwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
 RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);

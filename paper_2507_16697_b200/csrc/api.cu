@@ -374,6 +374,58 @@ int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_ho
   return RINGX_OK;
 }
 
+size_t ringx_attn_fwd_bwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, true) != RINGX_OK ||
+      check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false) != RINGX_OK)
+    return 0;
+  const size_t R = (size_t)B * H * N;
+  const size_t fw = carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype).bytes, bw = carve_bwd(nullptr, B, H, N, d).bytes;
+  return 8 * align_up(R * d * 2) + align_up(R * sizeof(float)) + (fw > bw ? fw : bw);
+}
+
+int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* v_host, const void* dO_host,
+                            void* o_host, float* lse_host, void* dq_host, void* dk_host, void* dv_host, int B, int H,
+                            int N, int d, int kv_chunk, float scale, int dtype, void* workspace,
+                            size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q_host || !k_host || !v_host || !dO_host || !o_host || !lse_host || !dq_host || !dk_host || !dv_host)
+    return RINGX_ERR_NULL_PTR;
+  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, true);
+  if (st == RINGX_OK) st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false);
+  if (st != RINGX_OK) return st;
+  const size_t need = ringx_attn_fwd_bwd_host_workspace_bytes(B, H, N, d, kv_chunk, dtype);
+  if (!workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < need) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  const size_t R = (size_t)B * H * N;
+  const size_t tb = R * d * 2, tba = align_up(tb);
+  char* p = static_cast<char*>(workspace);
+  void* t[8];   // q k v dO | o dq dk dv
+  for (int i = 0; i < 8; ++i) t[i] = p + i * tba;
+  float* dlse = reinterpret_cast<float*>(p + 8 * tba);
+  char* inner = p + 8 * tba + align_up(R * sizeof(float));
+  const size_t inner_bytes = workspace_bytes - (size_t)(inner - p);
+  const void* src[4] = {q_host, k_host, v_host, dO_host};
+  cudaError_t ce;
+  for (int i = 0; i < 4; ++i)
+    if ((ce = cudaMemcpyAsync(t[i], src[i], tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+  st = ringx_attn_fwd(t[0], t[1], t[2], t[4], dlse, B, H, N, d, kv_chunk, scale, dtype, inner, inner_bytes, stream_);
+  if (st != RINGX_OK) return st;
+  const int fwd_launches = tl_last_launches;
+  st = ringx_attn_bwd(t[0], t[1], t[2], t[4], dlse, t[3], t[5], t[6], t[7], B, H, N, d, kv_chunk, scale, dtype, inner,
+                      inner_bytes, stream_);
+  if (st != RINGX_OK) return st;
+  tl_last_launches += fwd_launches;
+  void* dst[4] = {o_host, dq_host, dk_host, dv_host};
+  for (int i = 0; i < 4; ++i)
+    if ((ce = cudaMemcpyAsync(dst[i], t[4 + i], tb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess)
+      return cuda_status(ce);
+  if ((ce = cudaMemcpyAsync(lse_host, dlse, R * sizeof(float), cudaMemcpyDeviceToHost, stream)) != cudaSuccess)
+    return cuda_status(ce);
+  if ((ce = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_status(ce);
+  return RINGX_OK;
+}
+
 int ringx_last_launch_count(void) { return tl_last_launches; }
 
 int ringx_profile_enable(int on) {

@@ -46,8 +46,10 @@ def lib() -> ctypes.CDLL:
     L.ringx_lse_merge.restype = c_i
     L.ringx_attn_chunk_fwd.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p]
     L.ringx_attn_chunk_fwd.restype = c_i
+    L.ringx_attn_fwd_bwd_host.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_fwd_bwd_host.restype = c_i
     for name in ("ringx_attn_fwd_workspace_bytes", "ringx_attn_bwd_workspace_bytes",
-                 "ringx_attn_fwd_host_workspace_bytes"):
+                 "ringx_attn_fwd_host_workspace_bytes", "ringx_attn_fwd_bwd_host_workspace_bytes"):
         getattr(L, name).argtypes = [c_i] * 6
         getattr(L, name).restype = c_sz
     L.ringx_last_launch_count.argtypes = []
@@ -184,6 +186,35 @@ def ringx_attn_fwd_host(q_host, k_host, v_host, kv_chunk: int, scale: float, o_h
                                        workspace.numel(), _stream())
     _check(st, "ringx_attn_fwd_host")
     return o_host, lse_host
+
+
+def ringx_attn_fwd_bwd_host_workspace_bytes(B, H, N, d, kv_chunk, dtype) -> int:
+    return lib().ringx_attn_fwd_bwd_host_workspace_bytes(B, H, N, d, kv_chunk, _DTYPES[dtype])
+
+
+def ringx_attn_fwd_bwd_host(q_host, k_host, v_host, dO_host, kv_chunk: int, scale: float, outs=None, workspace=None,
+                            device="cuda"):
+    """End-to-end forward+backward with HOST tensors: returns (o, lse, dq, dk, dv) host tensors."""
+    B, H, N, d = q_host.shape
+    dt = _DTYPES[q_host.dtype]
+    for t in (q_host, k_host, v_host, dO_host):
+        if t.is_cuda or not t.is_contiguous():
+            raise ValueError("ringx_attn_fwd_bwd_host takes contiguous HOST tensors")
+    if outs is None:
+        outs = (torch.empty_like(q_host).pin_memory(), torch.empty((B, H, N), dtype=torch.float32).pin_memory(),
+                torch.empty_like(q_host).pin_memory(), torch.empty_like(q_host).pin_memory(),
+                torch.empty_like(q_host).pin_memory())
+    o_host, lse_host, dq_host, dk_host, dv_host = outs
+    need = lib().ringx_attn_fwd_bwd_host_workspace_bytes(B, H, N, d, kv_chunk, dt)
+    if workspace is None:
+        workspace = _workspace(need, device)
+    with torch.cuda.device(workspace.device):
+        st = lib().ringx_attn_fwd_bwd_host(q_host.data_ptr(), k_host.data_ptr(), v_host.data_ptr(), dO_host.data_ptr(),
+                                           o_host.data_ptr(), lse_host.data_ptr(), dq_host.data_ptr(),
+                                           dk_host.data_ptr(), dv_host.data_ptr(), B, H, N, d, kv_chunk, scale, dt,
+                                           workspace.data_ptr(), workspace.numel(), _stream())
+    _check(st, "ringx_attn_fwd_bwd_host")
+    return outs
 
 
 def ringx_last_launch_count() -> int:

@@ -398,3 +398,18 @@ def test_bwd_errors(rx):
         rx.ringx_attn_bwd(qb, qb, qb, qb, lse, qb, 256, 0.125,
                           workspace=torch.empty(512, dtype=torch.uint8, device="cuda"))
     assert e.value.status == 5
+
+
+def test_fwd_bwd_host_entry_matches_device_entries(rx):
+    B, H, N, d, chunk = 1, 2, 1024, 64, 256
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=67)
+    scale = 0.125
+    qd, kd, vd, dod = q.cuda(), k.cuda(), v.cuda(), do.cuda()
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
+    dq, dk, dv = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale)
+    oh, lh, dqh, dkh, dvh = rx.ringx_attn_fwd_bwd_host(q.pin_memory(), k.pin_memory(), v.pin_memory(),
+                                                       do.pin_memory(), chunk, scale)
+    assert rx.ringx_last_launch_count() == (2 * (N // chunk) - 1) + (N // chunk + 2)
+    assert torch.equal(oh, o.cpu()) and torch.equal(lh, lse.cpu())
+    assert torch.equal(dkh, dk.cpu()) and torch.equal(dvh, dv.cpu())
+    assert ((dqh.float() - dq.cpu().float()).norm() / dq.float().norm()).item() <= 2e-3   # fp32 red order
