@@ -203,7 +203,7 @@ def main():
         run_reference(args, cfg, rank)
         return
 
-    from paper_2507_16697_b200 import ringx
+    from paper_2507_16697_b200 import multirank, ringx
     from paper_2507_16697_b200.build import build_library
     if rank == 0:
         build_library()
@@ -223,8 +223,7 @@ def main():
             dist.barrier()
 
     # ---------------------------------------------------------------- inputs (seeded, per-rank batch)
-    rcfg = wl.Config(cfg.name, cfg.dtype, cfg.B, cfg.H, cfg.N, cfg.d, cfg.kv_chunk, cfg.qk_gain, cfg.backward,
-                     cfg.seed + 1000 * rank)
+    rcfg = multirank.rank_config(cfg, rank)
     do_bwd = args.passes == "fwd+bwd"
     tensors = wl.make_qkv(rcfg, with_do=do_bwd, device=dev)
     q, k, v = tensors[:3]
@@ -271,13 +270,9 @@ def main():
     clocks = sampler.stop() if sampler else None
     prof = ringx.ringx_profile_read()
     ringx.ringx_profile_enable(False)
-    ms_total = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = t.item()
+    ms_total = multirank.max_over_ranks(e0.elapsed_time(e1), dist, dev)
     ms_step = ms_total / args.steps
-    value = world * flops_step / (ms_step * 1e-3) / 1e12
+    value = multirank.aggregate_tflops(world, flops_step, ms_step)
     gpu_launches = launches[0]
 
     # ---------------------------------------------------------------- roofline of the dominant kernel(s)
@@ -349,12 +344,8 @@ def main():
     for _ in range(n_e2e):
         call()
     torch.cuda.synchronize()
-    dt = (time.perf_counter() - t0) / n_e2e
-    if dist is not None:
-        t = torch.tensor([dt], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt = t.item()
-    e2e = {"value": world * flops_step / dt / 1e12, "unit": UNIT, "ms_per_step": dt * 1e3, "steps": n_e2e,
+    dt = multirank.max_over_ranks((time.perf_counter() - t0) / n_e2e, dist, dev)
+    e2e = {"value": multirank.aggregate_tflops(world, flops_step, dt * 1e3), "unit": UNIT, "ms_per_step": dt * 1e3, "steps": n_e2e,
            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "entry": entry}
     del ws_h, host_in
 
