@@ -23,6 +23,14 @@
 #include "kernels.cuh"
 
 namespace ringx {
+#ifdef RINGX_BWD_CLOCKS
+__device__ long long g_bwd_clocks[16];
+#define BCLK() clock64()
+#define BADD(i, v) do { if (blockIdx.x == 0 && blockIdx.y == 0 && i_ >= 8) atomicAdd((unsigned long long*)&g_bwd_clocks[i], (unsigned long long)(v)); } while (0)
+#else
+#define BCLK() 0ll
+#define BADD(i, v) do { } while (0)
+#endif
 namespace {
 
 using namespace ptx;
@@ -35,11 +43,14 @@ struct BwdCfg {
   static constexpr int kPanels = kD / 64;
   static constexpr int kPanelBytes = 128 * 128;
   static constexpr int kTileBytes = kPanels * kPanelBytes;     // one [128, d] bf16 tile
-  static constexpr int kStages = kD == 64 ? 3 : 2;             // Q_i / dO_i ring
-  static constexpr int kStageBytes = 2 * kTileBytes + 1024;    // Q, dO, lse2[128], D[128]
+  static constexpr int kQStages = kD == 64 ? 3 : 2;            // Q_i (+ lse2_i, D_i) ring: live from S^T(i) to dK(i)
+  static constexpr int kDoStages = kD == 64 ? 3 : 1;           // dO_i ring: live from dP^T(i) to dV(i)
+  static constexpr int kQStageBytes = kTileBytes + 1024;       // Q, lse2[128], D[128]
   static constexpr int kDsBytes = 2 * kPanelBytes;             // dS^T [128 keys][128 queries] bf16
+  static constexpr int kDqPanelBytes = 128 * 128;              // dQ staging: [128 rows][32 fp32], 128B-swizzled
   static constexpr int kAlignSlack = kD == 64 ? 1024 : 0;      // d = 128 uses every byte: base must be 1 KB aligned
-  static constexpr int kSmemBytes = kAlignSlack + 2 * kTileBytes + kStages * kStageBytes + kDsBytes + 256;
+  static constexpr int kSmemBytes = kAlignSlack + 2 * kTileBytes + kQStages * kQStageBytes + kDoStages * kTileBytes +
+                                    kDsBytes + 2 * kDqPanelBytes + 256;
   static constexpr uint32_t tS = 0, tDP = 128, tDV = 256, tDK = 256 + kD, tDQ = kD == 64 ? 384 : 128;
   static constexpr bool kDqOverlaysDp = kD != 64;
 };
@@ -48,7 +59,8 @@ template <int kD>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                       const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_do,
-                      const float* __restrict__ lse2, const float* __restrict__ Dvec, float* __restrict__ dq_acc,
+                      const __grid_constant__ CUtensorMap map_dq, const float* __restrict__ lse2,
+                      const float* __restrict__ Dvec,
                       __nv_bfloat16* __restrict__ dk, __nv_bfloat16* __restrict__ dv, int N, int k_off,
                       float scale_log2, float scale) {
   using Cfg = BwdCfg<kD>;
@@ -57,9 +69,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   if (Cfg::kAlignSlack == 0 && smem != smem_raw) __trap();
   uint8_t* sK = smem;
   uint8_t* sV = smem + Cfg::kTileBytes;
-  uint8_t* sStage = smem + 2 * Cfg::kTileBytes;
-  uint8_t* sDs = sStage + Cfg::kStages * Cfg::kStageBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sDs + Cfg::kDsBytes);
+  uint8_t* sQ = smem + 2 * Cfg::kTileBytes;                    // [kQStages] Q_i | lse2_i | D_i
+  uint8_t* sDo = sQ + Cfg::kQStages * Cfg::kQStageBytes;       // [kDoStages] dO_i
+  uint8_t* sDs = sDo + Cfg::kDoStages * Cfg::kTileBytes;
+  uint8_t* sDq = sDs + Cfg::kDsBytes;                          // 2 staging panels for the dQ reduce-add
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sDq + 2 * Cfg::kDqPanelBytes);
   uint64_t* kv_full = bars;          // TMA -> MMA: K_j, V_j
   uint64_t* s_full = bars + 1;       // MMA -> compute: S^T(i)
   uint64_t* dp_full = bars + 2;      // MMA -> compute: dP^T(i)
@@ -69,9 +83,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   uint64_t* dq_full = bars + 6;      // MMA -> drain: dQ(i) in TMEM
   uint64_t* dq_empty = bars + 7;     // drain -> MMA: dQ(i) in registers                            (128 arrivals)
   uint64_t* dkv_full = bars + 8;     // MMA -> compute: dK_j, dV_j complete
-  uint64_t* q_full = bars + 9;       // [kStages] TMA -> MMA, compute
-  uint64_t* q_empty = q_full + Cfg::kStages;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(q_empty + Cfg::kStages);
+  uint64_t* q_full = bars + 9;       // [kQStages] TMA -> MMA, compute
+  uint64_t* q_empty = q_full + Cfg::kQStages;
+  uint64_t* do_full = q_empty + Cfg::kQStages;     // [kDoStages]
+  uint64_t* do_empty = do_full + Cfg::kDoStages;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(do_empty + Cfg::kDoStages);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   const int lane = threadIdx.x & 31;
@@ -90,9 +106,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     mbar_init(dq_full, 1);
     mbar_init(dq_empty, 128);
     mbar_init(dkv_full, 1);
-    for (int i = 0; i < Cfg::kStages; ++i) {
+    for (int i = 0; i < Cfg::kQStages; ++i) {
       mbar_init(&q_full[i], 1);
       mbar_init(&q_empty[i], 1);
+    }
+    for (int i = 0; i < Cfg::kDoStages; ++i) {
+      mbar_init(&do_full[i], 1);
+      mbar_init(&do_empty[i], 1);
     }
     fence_mbar_init();
   }
@@ -102,6 +122,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       prefetch_tmap(&map_k);
       prefetch_tmap(&map_v);
       prefetch_tmap(&map_do);
+      prefetch_tmap(&map_dq);
     }
     tmem_alloc<512>(tmem_slot);
   }
@@ -124,23 +145,39 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       }
     }
     __syncwarp();
-    int stage = 0, phase = 0;
-    for (int i = 0; i < n_q; ++i) {
-      mbar_wait(&q_empty[stage], phase ^ 1);
+    auto load_q = [&](int i, int st) {
       if (leader) {
-        uint8_t* st = sStage + stage * Cfg::kStageBytes;
+        uint8_t* dst = sQ + st * Cfg::kQStageBytes;
         const int row = q_row0 + i * kTile;
-        mbar_arrive_expect_tx(&q_full[stage], Cfg::kStageBytes);
+        mbar_arrive_expect_tx(&q_full[st], Cfg::kQStageBytes);
 #pragma unroll
-        for (int p = 0; p < Cfg::kPanels; ++p) {
-          tma_load_2d(st + p * Cfg::kPanelBytes, &map_q, &q_full[stage], p * 64, row, pol_q);
-          tma_load_2d(st + Cfg::kTileBytes + p * Cfg::kPanelBytes, &map_do, &q_full[stage], p * 64, row, pol_q);
-        }
-        bulk_load_1d(st + 2 * Cfg::kTileBytes, lse2 + row, 512, &q_full[stage]);
-        bulk_load_1d(st + 2 * Cfg::kTileBytes + 512, Dvec + row, 512, &q_full[stage]);
+        for (int p = 0; p < Cfg::kPanels; ++p)
+          tma_load_2d(dst + p * Cfg::kPanelBytes, &map_q, &q_full[st], p * 64, row, pol_q);
+        bulk_load_1d(dst + Cfg::kTileBytes, lse2 + row, 512, &q_full[st]);
+        bulk_load_1d(dst + Cfg::kTileBytes + 512, Dvec + row, 512, &q_full[st]);
       }
       __syncwarp();
-      if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
+    };
+    load_q(0, 0);
+    int qs = Cfg::kQStages > 1 ? 1 : 0, qph = Cfg::kQStages > 1 ? 0 : 1, ds = 0, dph = 0;
+    for (int i = 0; i < n_q; ++i) {
+      // dO_i: its slot is free once dV(i - kDoStages) has read it
+      mbar_wait(&do_empty[ds], dph ^ 1);
+      if (leader) {
+        mbar_arrive_expect_tx(&do_full[ds], Cfg::kTileBytes);
+#pragma unroll
+        for (int p = 0; p < Cfg::kPanels; ++p)
+          tma_load_2d(sDo + ds * Cfg::kTileBytes + p * Cfg::kPanelBytes, &map_do, &do_full[ds], p * 64,
+                      q_row0 + i * kTile, pol_q);
+      }
+      __syncwarp();
+      if (++ds == Cfg::kDoStages) { ds = 0; dph ^= 1; }
+      // Q_{i+1}: its slot is free once dK(i + 1 - kQStages) has read it
+      if (i + 1 < n_q) {
+        mbar_wait(&q_empty[qs], qph ^ 1);
+        load_q(i + 1, qs);
+        if (++qs == Cfg::kQStages) { qs = 0; qph ^= 1; }
+      }
     }
   } else if (warp == 13) {
     // ------------------------------------------------------------------ MMA issuer
@@ -149,7 +186,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     constexpr uint32_t idesc_kn = make_idesc_bf16(kTile, kD, 0, 1);      // A K-major/TMEM x B MN-major -> [128, d]
     constexpr uint32_t idesc_mn = make_idesc_bf16(kTile, kD, 1, 1);      // A MN-major (dS from dS^T) x B MN-major
     const uint32_t k_addr = smem_u32(sK), v_addr = smem_u32(sV), ds_addr = smem_u32(sDs);
-    const uint32_t stage_addr = smem_u32(sStage);
+    const uint32_t q_base = smem_u32(sQ), do_base = smem_u32(sDo);
     auto kmajor = [](uint32_t base, int k) {   // K-step k of a K-major [128 rows][d or 128] tile (64-element panels)
       return make_smem_desc_sw128(base + (k >> 2) * Cfg::kPanelBytes + (k & 3) * 32, 16, 1024);
     };
@@ -180,14 +217,16 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     mbar_wait(kv_full, 0);
     mbar_wait(&q_full[0], 0);
     tc_fence_after();
-    issue_st(stage_addr);
-    issue_dpt(stage_addr + Cfg::kTileBytes);
-    int stage = 0, phase = 0;
+    issue_st(q_base);
+    mbar_wait(&do_full[0], 0);
+    tc_fence_after();
+    issue_dpt(do_base);
+    int qs = 0, qph = 0, ds = 0, dph = 0;
     for (int i = 0; i < n_q; ++i) {
-      const uint32_t q_addr = stage_addr + stage * Cfg::kStageBytes, do_addr = q_addr + Cfg::kTileBytes;
-      const int cur_stage = stage;
-      if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
-      const uint32_t nq_addr = stage_addr + stage * Cfg::kStageBytes;
+      const uint32_t q_addr = q_base + qs * Cfg::kQStageBytes, do_addr = do_base + ds * Cfg::kTileBytes;
+      const int cur_qs = qs, cur_ds = ds;
+      if (++qs == Cfg::kQStages) { qs = 0; qph ^= 1; }
+      if (++ds == Cfg::kDoStages) { ds = 0; dph ^= 1; }
       const bool more = i + 1 < n_q;
       // ---- behind phase A: dV += P^T(i) dO_i, then S^T(i+1)
       mbar_wait(p_full, i & 1);
@@ -197,12 +236,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         for (int k = 0; k < kTile / 16; ++k)
           mma_ts(tmem + Cfg::tDV, tmem + Cfg::tS + (k >> 2) * 64 + (k & 3) * 8, mnmajor(do_addr, k), idesc_kn,
                  i > 0 || k > 0);
+        mma_commit(&do_empty[cur_ds]);
       }
       __syncwarp();
       if (more) {
-        mbar_wait(&q_full[stage], phase);
+        mbar_wait(&q_full[qs], qph);
         tc_fence_after();
-        issue_st(nq_addr);
+        issue_st(q_base + qs * Cfg::kQStageBytes);
       }
       // ---- behind phase B: dK += dS^T(i) Q_i, dQ(i) = dS(i) K_j, then dP^T(i+1)
       mbar_wait(ds_full, i & 1);
@@ -217,15 +257,14 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           mma_ss(tmem + Cfg::tDQ, mnmajor(ds_addr, k), mnmajor(k_addr, k), idesc_mn, k > 0);
         mma_commit(dq_full);
         mma_commit(ds_empty);
-        mma_commit(&q_empty[cur_stage]);
+        mma_commit(&q_empty[cur_qs]);
       }
       __syncwarp();
       if (more) {
-        if (Cfg::kDqOverlaysDp) {
-          mbar_wait(dq_empty, i & 1);      // dQ(i) sits in the dP^T columns until the drain warps took it
-          tc_fence_after();
-        }
-        issue_dpt(nq_addr + Cfg::kTileBytes);
+        mbar_wait(&do_full[ds], dph);
+        if (Cfg::kDqOverlaysDp) mbar_wait(dq_empty, i & 1);   // dQ(i) sits in the dP^T columns until drained
+        tc_fence_after();
+        issue_dpt(do_base + ds * Cfg::kTileBytes);
       }
     }
     commit(dkv_full);
@@ -239,14 +278,17 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     uint8_t* ds_row = sDs + half * Cfg::kPanelBytes + row * 128;
     int stage = 0, phase = 0;
     for (int i = 0; i < n_q; ++i) {
-      const float4* stats = reinterpret_cast<const float4*>(sStage + stage * Cfg::kStageBytes + 2 * Cfg::kTileBytes);
+      const float4* stats = reinterpret_cast<const float4*>(sQ + stage * Cfg::kQStageBytes + Cfg::kTileBytes);
       const float4* lse4 = stats + half * 16;                    // lse2 of my 64 query columns
       const float4* d4 = stats + 32 + half * 16;                 // D of my 64 query columns
       mbar_wait(&q_full[stage], phase);
-      if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
+      if (++stage == Cfg::kQStages) { stage = 0; phase ^= 1; }
       // ---- phase A: P^T = exp2(scale_log2 * S^T - lse2)
+      const int i_ = i;
+      const long long b0 = BCLK();
       mbar_wait(s_full, i & 1);
       tc_fence_after();
+      const long long b1 = BCLK();
       float p[64];
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
@@ -271,10 +313,12 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       tmem_wait_st();
       tc_fence_before();
       mbar_arrive(p_full);
+      const long long b2 = BCLK();
       // ---- phase B: dS^T = P^T o (dP^T - D), bf16, to shared memory [keys][queries] (128B-swizzled rows)
       mbar_wait(dp_full, i & 1);
       if (i > 0) mbar_wait(ds_empty, (i - 1) & 1);
       tc_fence_after();
+      const long long b3 = BCLK();
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
         uint32_t dp[32];
@@ -299,6 +343,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       fence_proxy_async_smem();
       tc_fence_before();
       mbar_arrive(ds_full);
+      if (threadIdx.x == 0) { BADD(0, b1 - b0); BADD(1, b2 - b1); BADD(2, b3 - b2); BADD(3, BCLK() - b3); BADD(4, 1); }
     }
     // ---- epilogue: dV_j (warps 0-3) and scale * dK_j (warps 4-7), bf16, written once
     mbar_wait(dkv_full, 0);
@@ -324,28 +369,45 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     }
   } else {
     // ------------------------------------------------------------------ dQ drain warps (8-11)
+    // TMEM -> registers -> 128B-swizzled fp32 staging panel [128 rows][32 cols] -> one TMA reduce-add per panel
+    // (cp.reduce.async.bulk.tensor ... .add): full-line L2 atomics issued by the TMA engine, nothing on the LSU
+    // but conflict-free 16-byte shared stores.
     const int row = (warp & 3) * 32 + lane;                      // query row of the tile = TMEM lane
     const uint32_t tDQ = tmem + Cfg::tDQ + (static_cast<uint32_t>((warp & 3) * 32) << 16);
-    float* dst_row = dq_acc + (static_cast<size_t>(q_row0) + row) * kD;
+    const bool leader = warp == 8 && elect_one();
+    int buf = 0;
     for (int i = 0; i < n_q; ++i) {
+      const int i_ = i;
+      const long long d0 = BCLK();
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
-      float* dst = dst_row + static_cast<size_t>(i) * kTile * kD;
+      const long long d1 = BCLK();
 #pragma unroll
       for (int c = 0; c < kD / 32; ++c) {
         uint32_t r[32];
         tmem_ld_x32(tDQ + c * 32, r);
+        if (leader) tma_wait_group_read<1>();      // the reduce that last read this panel has finished reading
+        named_bar_sync(1, 128);
         tmem_wait_ld();
-        if (c == kD / 32 - 1) {          // the whole dQ(i) row is in registers: hand the columns back
+        if (c == kD / 32 - 1) {          // the whole dQ(i) row has left TMEM: hand the columns back
           tc_fence_before();
           mbar_arrive(dq_empty);
         }
+        uint8_t* prow = sDq + buf * Cfg::kDqPanelBytes + row * 128;
 #pragma unroll
-        for (int e = 0; e < 32; e += 4)
-          red_add_v4(dst + c * 32 + e, __uint_as_float(r[e]), __uint_as_float(r[e + 1]), __uint_as_float(r[e + 2]),
-                     __uint_as_float(r[e + 3]));
+        for (int g = 0; g < 8; ++g) st_shared_v4(prow + ((g ^ (row & 7)) << 4), r[g * 4], r[g * 4 + 1], r[g * 4 + 2], r[g * 4 + 3]);
+        fence_proxy_async_smem();
+        named_bar_sync(2, 128);
+        if (leader) {
+          tma_reduce_add_2d(&map_dq, sDq + buf * Cfg::kDqPanelBytes, c * 32, q_row0 + i * kTile);
+          tma_commit_group();
+        }
+        buf ^= 1;
       }
+      if (threadIdx.x == 256) { BADD(5, d1 - d0); BADD(6, BCLK() - d1); }
     }
+    if (leader) tma_wait_group<0>();
+    __syncwarp();
   }
 
   tc_fence_before();
@@ -355,8 +417,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 
 template <int kD>
 cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
-                     const float* lse2, const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
-                     int nk, float scale, cudaStream_t stream) {
+                     const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int BH, int N,
+                     int k_off, int nk, float scale, cudaStream_t stream) {
   using Cfg = BwdCfg<kD>;
   auto kern = attn_chunk_bwd_kernel<kD>;
   static bool configured = false;
@@ -366,7 +428,7 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
     configured = true;
   }
   dim3 grid(nk / kTile, BH);
-  kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, lse2, D, dq_acc,
+  kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D,
                                                        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv),
                                                        N, k_off, scale * 1.4426950408889634f, scale);
   count_launch();
@@ -378,16 +440,27 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
                                         int nk, int d, float scale, cudaStream_t stream) {
-  CUtensorMap mq, mk, mv, mdo;
+  CUtensorMap mq, mk, mv, mdo, mdq;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   const uint64_t rows = (uint64_t)BH * N;
   if (!make_tmap_2d(&mq, q, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mk, k, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mv, v, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B))
+      !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mdq, dq_acc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, rows, d, 128, 32, kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, lse2, D, dq_acc, dk, dv, BH, N, k_off, nk, scale, stream);
-  return launch_t<128>(mq, mk, mv, mdo, lse2, D, dq_acc, dk, dv, BH, N, k_off, nk, scale, stream);
+  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, k_off, nk, scale, stream);
+  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, k_off, nk, scale, stream);
 }
 
 }  // namespace ringx
+
+#ifdef RINGX_BWD_CLOCKS
+extern "C" __attribute__((visibility("default"))) int ringx_debug_bwd_clocks(long long* out) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, ringx::g_bwd_clocks, sizeof(long long) * 16);
+  long long z[16] = {0};
+  cudaMemcpyToSymbol(ringx::g_bwd_clocks, z, sizeof(z));
+  return 0;
+}
+#endif
