@@ -4,18 +4,22 @@
 //   loc_out = softmax(scale q K_c^T) V_c,  loc_lse = log sum_j exp(scale q.k_j)      (Eq. 1/3/4)
 // bf16 operands, fp32 accumulation ("mixed float32-bfloat16").
 //
-// Structure (one CTA per SM, 320 threads):
-//   warps 0-3   softmax warpgroup of query tile 0 (thread = one query row; owns TMEM lane = row)
-//   warps 4-7   softmax warpgroup of query tile 1
-//   warp  8     TMA producer: Q tiles once, then the K/V ring (K_0, V_0, K_1, V_1, ...)
-//   warp  9     MMA issuer (one elected lane): S_t = Q_t K_j^T (SS), O_t += P_t V_j (P from TMEM)
+// Structure (one CTA per SM, 384 threads = 3 warpgroups; registers re-split with setmaxnreg):
+//   warps 0-3   softmax warpgroup of query tile 0 (thread = one query row; owns TMEM lane = row)   224 regs
+//   warps 4-7   softmax warpgroup of query tile 1                                                  224 regs
+//   warp  8     TMA producer: Q tiles once, then the K/V ring (K_0, V_0, K_1, V_1, ...)              56 regs
+//   warp  9     MMA issuer (one elected lane): S_t = Q_t K_j^T (SS), O_t += P_t V_j (P from TMEM)    56 regs
+//   warps 10-11 idle (they only complete the third warpgroup so that setmaxnreg can be used)
 // TMEM columns: S_0 [0,128) S_1 [128,256) O_0 [256,256+d) O_1 [256+d,256+2d); P_t (bf16) overwrites
 // the first 64 columns of S_t.  The two query tiles ping-pong: while warpgroup t turns S_t into P_t the
 // tensor core works on tile 1-t.  The MMA pipe executes in issue order, so S_t(j+1) -- issued right after
 // O_t += P_t(j) V_j -- cannot overwrite P_t(j) early, and the commit that signals S_t(j+1) also proves
 // O_t(j) complete: the softmax warps may rescale O_t in place without a further barrier.
 // Online softmax in the exp2 domain with a lazy running max (O, l are only rescaled when the row max
-// grew by more than 2^8), so the rescale is off the common path.
+// grew by more than 2^8), so the rescale is off the common path.  The softmax streams S out of TMEM in
+// 32-column pieces (the row max of piece c is taken while piece c+1 is in flight), uses the packed
+// FFMA2/FADD2 and three-input FMNMX3 forms, and hands P to the tensor core in two 64-key halves so that
+// the first half of O += P V starts while the second half of P is still being exponentiated.
 #include "kernels.cuh"
 
 namespace ringx {
@@ -31,7 +35,8 @@ using namespace ptx;
 
 constexpr int kBlockM = 128;          // query rows per tile (= TMEM lanes)
 constexpr int kBlockN = 128;          // keys per KV tile
-constexpr int kFwdThreads = 320;
+constexpr int kFwdThreads = 384;
+constexpr int kSoftmaxRegs = 224, kAuxRegs = 56;   // 256*224 + 128*56 = 64512 <= 65536
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
 
 template <int kD>
@@ -57,11 +62,11 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + Cfg::kStages * Cfg::kTileBytes);
   uint64_t* q_full = bars;                  // [2]  TMA -> MMA
   uint64_t* s_full = bars + 2;              // [2]  MMA -> softmax: S_t(j) in TMEM
-  uint64_t* p_full = bars + 4;              // [2]  softmax -> MMA: P_t(j) in TMEM (O_t rescaled if needed)
-  uint64_t* o_full = bars + 6;              // [2]  MMA -> softmax: last O_t complete
-  uint64_t* kv_full = bars + 8;             // [kStages]
-  uint64_t* kv_empty = bars + 8 + Cfg::kStages;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 8 + 2 * Cfg::kStages);
+  uint64_t* p_full = bars + 4;              // [2][2] softmax -> MMA: half h (64 keys) of P_t(j) in TMEM (O_t rescaled if needed)
+  uint64_t* o_full = bars + 8;              // [2]  MMA -> softmax: last O_t complete
+  uint64_t* kv_full = bars + 10;            // [kStages]
+  uint64_t* kv_empty = bars + 10 + Cfg::kStages;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 10 + 2 * Cfg::kStages);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // provably warp-uniform: keeps MMA/TMA operands in uniform registers
   const int lane = threadIdx.x & 31;
@@ -73,7 +78,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     for (int i = 0; i < 2; ++i) {
       mbar_init(&q_full[i], 1);
       mbar_init(&s_full[i], 1);
-      mbar_init(&p_full[i], kBlockM);
+      mbar_init(&p_full[2 * i], kBlockM);
+      mbar_init(&p_full[2 * i + 1], kBlockM);
       mbar_init(&o_full[i], 1);
     }
     for (int i = 0; i < Cfg::kStages; ++i) {
@@ -96,6 +102,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   const uint32_t tmem = *tmem_slot;
 
   if (warp == 8) {
+    setmaxnreg_dec<kAuxRegs>();
     // ------------------------------------------------------------------ TMA producer
     // (the whole warp runs the loop so that every operand is warp-uniform; one elected lane issues)
     {
@@ -122,6 +129,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     }
   } else if (warp == 9) {
     // ------------------------------------------------------------------ MMA issuer
+    setmaxnreg_dec<kAuxRegs>();
     {
       const bool leader = elect_one();
       constexpr uint32_t idesc_s = make_idesc_bf16(kBlockM, kBlockN, 0, 0);    // Q (K-major) x K^T (K-major)
@@ -144,11 +152,11 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         __syncwarp();
       };
       // O_t (+)= P_t V from the V tile in ring slot `st`
-      auto issue_o = [&](int t, int st, bool accumulate) {
+      auto issue_o = [&](int t, int st, int half, bool accumulate) {   // keys [64*half, 64*half + 64) of the tile
         const uint32_t b0 = kv_addr + st * Cfg::kTileBytes;
         if (leader) {
 #pragma unroll
-          for (int k = 0; k < kBlockN / 16; ++k)
+          for (int k = half * 4; k < half * 4 + 4; ++k)
             mma_ts(tmem + 256 + t * kD, tmem + t * kBlockN + k * 8,
                    make_smem_desc_sw128(b0 + k * 2048, Cfg::kPanelBytes, 1024), idesc_o, accumulate || k > 0);
         }
@@ -178,12 +186,15 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
           const long long m0 = CLK();
-          mbar_wait(&p_full[t], j & 1);
+          mbar_wait(&p_full[2 * t], j & 1);
           tc_fence_after();
 #ifdef RINGX_FWD_CLOCKS
           if (blockIdx.x == 0 && blockIdx.y == 0 && leader && j >= 8) atomicAdd((unsigned long long*)&g_fwd_clocks[8 + t], (unsigned long long)(CLK() - m0));
 #endif
-          issue_o(t, v_stage, j > 0);
+          issue_o(t, v_stage, 0, j > 0);
+          mbar_wait(&p_full[2 * t + 1], j & 1);
+          tc_fence_after();
+          issue_o(t, v_stage, 1, true);
           if (t == 1) commit(&kv_empty[v_stage]);
           if (more) {
             if (t == 0) {
@@ -198,8 +209,9 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         }
       }
     }
-  } else {
+  } else if (warp < 8) {
     // ------------------------------------------------------------------ softmax warpgroups
+    setmaxnreg_inc<kSoftmaxRegs>();
     const int t = warp >> 2;
     const uint32_t lane_off = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tS = tmem + t * kBlockN + lane_off;
@@ -207,24 +219,35 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     float m_raw = -CUDART_INF_F;   // running (lazy) row max of the unscaled scores
     float m_sc = -CUDART_INF_F;    // m_raw * scale_log2
     float l = 0.f;                 // running row sum of exp2(s*scale_log2 - m_sc)
+    const float2 sc2 = make_float2(scale_log2, scale_log2);
     for (int j = 0; j < n_kv; ++j) {
       const long long c0 = CLK();
       mbar_wait(&s_full[t], j & 1);
       tc_fence_after();
       const long long c1 = CLK();
+      // ---- pass 1: stream S_t(j) out of TMEM; the row max of piece c is taken while piece c+1 is in flight
       uint32_t s[kBlockN];
+      auto piece = [&](int c) -> uint32_t(&)[32] { return *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]); };
+      auto piece_max = [&](int c, float& a, float& b) {
 #pragma unroll
-      for (int c = 0; c < kBlockN / 32; ++c) tmem_ld_x32(tS + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
-      tmem_wait_ld();
-      float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]),
-            mx3 = __uint_as_float(s[3]);
-#pragma unroll
-      for (int i = 4; i < kBlockN; i += 4) {
-        mx0 = fmaxf(mx0, __uint_as_float(s[i]));
-        mx1 = fmaxf(mx1, __uint_as_float(s[i + 1]));
-        mx2 = fmaxf(mx2, __uint_as_float(s[i + 2]));
-        mx3 = fmaxf(mx3, __uint_as_float(s[i + 3]));
-      }
+        for (int i = 0; i < 32; i += 4) {
+          a = fmax3(a, __uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1]));
+          b = fmax3(b, __uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3]));
+        }
+      };
+      float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F, mx2 = -CUDART_INF_F, mx3 = -CUDART_INF_F;
+      tmem_ld_x32(tS, piece(0));
+      tmem_wait_ld_x32(piece(0));
+      tmem_ld_x32(tS + 32, piece(1));
+      piece_max(0, mx0, mx1);
+      tmem_wait_ld_x32(piece(1));
+      tmem_ld_x32(tS + 64, piece(2));
+      piece_max(1, mx2, mx3);
+      tmem_wait_ld_x32(piece(2));
+      tmem_ld_x32(tS + 96, piece(3));
+      piece_max(2, mx0, mx1);
+      tmem_wait_ld_x32(piece(3));
+      piece_max(3, mx2, mx3);
       const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
       const bool grow = (mx - m_raw) * scale_log2 > kRescaleThreshold;
       if (__any_sync(0xffffffffu, grow)) {
@@ -236,7 +259,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           for (int c = 0; c < kD / 32; ++c) {
             uint32_t o[32];
             tmem_ld_x32(tO + c * 32, o);
-            tmem_wait_ld();
+            tmem_wait_ld_x32(o);
 #pragma unroll
             for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
             tmem_st_x32(tO + c * 32, o);
@@ -245,26 +268,31 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         m_raw = m_new;
         m_sc = m_new * scale_log2;
       }
-      float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+      // ---- pass 2: P = exp2(s * scale_log2 - m_sc), bf16, into the first 64 columns of S_t; row sum in fp32
+      const float2 nm2 = make_float2(-m_sc, -m_sc);
+      float2 la = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
 #pragma unroll
       for (int c = 0; c < kBlockN / 32; ++c) {
         uint32_t pk[16];
 #pragma unroll
         for (int i = 0; i < 32; i += 4) {
-          const float p0 = ex2(fmaf(__uint_as_float(s[c * 32 + i]), scale_log2, -m_sc));
-          const float p1 = ex2(fmaf(__uint_as_float(s[c * 32 + i + 1]), scale_log2, -m_sc));
-          const float p2 = ex2(fmaf(__uint_as_float(s[c * 32 + i + 2]), scale_log2, -m_sc));
-          const float p3 = ex2(fmaf(__uint_as_float(s[c * 32 + i + 3]), scale_log2, -m_sc));
-          l0 += p0; l1 += p1; l2 += p2; l3 += p3;
-          pk[i / 2] = pack_bf16x2(p0, p1);
-          pk[i / 2 + 1] = pack_bf16x2(p2, p3);
+          const float2 x0 = ffma2(make_float2(__uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1])), sc2, nm2);
+          const float2 x1 = ffma2(make_float2(__uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3])), sc2, nm2);
+          const float2 p0 = make_float2(ex2(x0.x), ex2(x0.y));
+          const float2 p1 = make_float2(ex2(x1.x), ex2(x1.y));
+          la = fadd2(la, p0);
+          lb = fadd2(lb, p1);
+          pk[i / 2] = pack_bf16x2(p0.x, p0.y);
+          pk[i / 2 + 1] = pack_bf16x2(p1.x, p1.y);
         }
         tmem_st_x16(tS + c * 16, pk);
+        if (c & 1) {                       // 64 keys of P are in TMEM: let the tensor core start on them
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(&p_full[2 * t + (c >> 1)]);
+        }
       }
-      l += (l0 + l1) + (l2 + l3);
-      tmem_wait_st();
-      tc_fence_before();
-      mbar_arrive(&p_full[t]);
+      l += (la.x + la.y) + (lb.x + lb.y);
 #ifdef RINGX_FWD_CLOCKS
       if (blockIdx.x == 0 && blockIdx.y == 0 && (threadIdx.x & 127) == 0 && j >= 8) {
         atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 0], (unsigned long long)(c1 - c0));   // wait S
@@ -303,6 +331,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       }
     }
     lse_out[row] = (m_sc + lg2(l)) * 0.6931471805599453f;
+  } else {
+    setmaxnreg_dec<kAuxRegs>();   // warps 10-11: nothing to do but release their registers
   }
 
   tc_fence_before();
