@@ -5,21 +5,23 @@
 //   dP^T = V_j dO_i^T                     dS^T = P^T o (dP^T - D_i)                  *global* LSE; reading g8)
 //   dV_j += P^T dO_i      dK_j += dS^T Q_i      dQ_i += dS K_j                       (all unscaled; scale is applied
 // when dK is written here and when dQ is converted).  dK_j, dV_j live in TMEM for the whole loop and are written once
-// (atomic-free: the CTA owns the tile); dQ_i is reduce-added into the fp32 accumulator with red.global.add.v4.f32 --
+// (atomic-free: the CTA owns the tile); dQ_i is reduce-added into the fp32 accumulator by TMA (cp.reduce.async.bulk) --
 // the single-GPU image of "the gradient for Q is accumulated ... over N steps".
 //
-// Roles (448 threads):  warps 0-7  compute (thread = key row = TMEM lane; warps 0-3 take query columns 0-63 of the
+// Roles (512 threads):  warps 0-7  compute (thread = key row = TMEM lane; warps 0-3 take query columns 0-63 of the
 //                                  tile, warps 4-7 columns 64-127)
-//                       warps 8-11 dQ drain (thread = query row): TMEM -> registers -> red.global.add
-//                       warp  12   TMA producer (K_j,V_j once; then the Q_i/dO_i/lse2_i/D_i ring)
+//                       warps 8-11 dQ drain (thread = query row): TMEM -> registers (TMEM columns released at once)
+//                                  -> swizzled fp32 staging panels -> TMA reduce-add into dq_acc
+//                       warp  12   TMA producer (K_j,V_j once; then the Q_i/lse2_i/D_i and dO_i rings)
 //                       warp  13   MMA issuer
+//                       warps 14-15 idle (complete the fourth warpgroup for setmaxnreg)
 // TMEM columns: S^T [0,128) (P^T, bf16, overwrites the first 32 columns of each 64-column half), dP^T [128,256),
 // dV [256,256+d), dK [256+d,256+2d), dQ [384,448) for d = 64; for d = 128 dQ overlays dP^T (drained before the next
 // dP^T is issued).  dS^T goes to shared memory as a [keys][queries] bf16 tile that serves as the K-major A operand of
 // dK += dS^T Q and as the MN-major A operand of dQ = dS K.
 // Pipeline: the compute warps alternate phase A (S^T -> P^T) and phase B (dP^T -> dS^T) while the tensor core runs
-// {dV(i), S^T(i+1)} behind phase A and {dK(i), dQ(i), dP^T(i+1)} behind phase B; in-order MMA execution makes the
-// P^T / S^T overlay safe.
+// {dV(i), S^T(i+1)} behind phase A and {dQ(i), dK(i), dP^T(i+1)} behind phase B (dQ first, so that its drain runs
+// under the dK MMA); in-order MMA execution makes the P^T / S^T overlay safe.
 #include "kernels.cuh"
 
 namespace ringx {
@@ -36,7 +38,8 @@ namespace {
 using namespace ptx;
 
 constexpr int kTile = 128;
-constexpr int kBwdThreads = 448;
+constexpr int kBwdThreads = 512;                 // 4 warpgroups; registers re-split with setmaxnreg
+constexpr int kBwdComputeRegs = 152, kBwdDrainRegs = 152, kBwdAuxRegs = 40;   // 256*152 + 128*152 + 128*40 = 63488
 
 template <int kD>
 struct BwdCfg {
@@ -133,6 +136,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 
   if (warp == 12) {
     // ------------------------------------------------------------------ TMA producer
+    setmaxnreg_dec<kBwdAuxRegs>();
     const bool leader = elect_one();
     const uint64_t pol_kv = policy_evict_first();
     const uint64_t pol_q = policy_evict_last();      // Q/dO tiles are re-read by every CTA of the head
@@ -181,6 +185,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     }
   } else if (warp == 13) {
     // ------------------------------------------------------------------ MMA issuer
+    setmaxnreg_dec<kBwdAuxRegs>();
     const bool leader = elect_one();
     constexpr uint32_t idesc_st = make_idesc_bf16(kTile, kTile, 0, 0);   // K_j (K-major) x Q_i^T (K-major)
     constexpr uint32_t idesc_kn = make_idesc_bf16(kTile, kD, 0, 1);      // A K-major/TMEM x B MN-major -> [128, d]
@@ -244,18 +249,18 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         tc_fence_after();
         issue_st(q_base + qs * Cfg::kQStageBytes);
       }
-      // ---- behind phase B: dK += dS^T(i) Q_i, dQ(i) = dS(i) K_j, then dP^T(i+1)
+      // ---- behind phase B: dQ(i) = dS(i) K_j (drained under the next MMA), dK += dS^T(i) Q_i, then dP^T(i+1)
       mbar_wait(ds_full, i & 1);
       if (!Cfg::kDqOverlaysDp && i > 0) mbar_wait(dq_empty, (i - 1) & 1);
       tc_fence_after();
       if (leader) {
 #pragma unroll
         for (int k = 0; k < kTile / 16; ++k)
-          mma_ss(tmem + Cfg::tDK, kmajor(ds_addr, k), mnmajor(q_addr, k), idesc_kn, i > 0 || k > 0);
-#pragma unroll
-        for (int k = 0; k < kTile / 16; ++k)
           mma_ss(tmem + Cfg::tDQ, mnmajor(ds_addr, k), mnmajor(k_addr, k), idesc_mn, k > 0);
         mma_commit(dq_full);
+#pragma unroll
+        for (int k = 0; k < kTile / 16; ++k)
+          mma_ss(tmem + Cfg::tDK, kmajor(ds_addr, k), mnmajor(q_addr, k), idesc_kn, i > 0 || k > 0);
         mma_commit(ds_empty);
         mma_commit(&q_empty[cur_qs]);
       }
@@ -270,12 +275,14 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     commit(dkv_full);
   } else if (warp < 8) {
     // ------------------------------------------------------------------ compute warps
+    setmaxnreg_inc<kBwdComputeRegs>();
     const int half = warp >> 2;                                  // which 64 query columns of the tile
     const int row = (warp & 3) * 32 + lane;                      // key row of the tile = TMEM lane
     const uint32_t lane_off = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tS = tmem + Cfg::tS + lane_off + half * 64;   // my S^T columns; P^T goes to the first 32 of them
     const uint32_t tDP = tmem + Cfg::tDP + lane_off + half * 64;
     uint8_t* ds_row = sDs + half * Cfg::kPanelBytes + row * 128;
+    const float2 sc2 = make_float2(scale_log2, scale_log2);
     int stage = 0, phase = 0;
     for (int i = 0; i < n_q; ++i) {
       const float4* stats = reinterpret_cast<const float4*>(sQ + stage * Cfg::kQStageBytes + Cfg::kTileBytes);
@@ -289,26 +296,33 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(s_full, i & 1);
       tc_fence_after();
       const long long b1 = BCLK();
-      float p[64];
+      float2 p[32];
+      {
+        uint32_t s0[32], s1[32];
+        tmem_ld_x32(tS, s0);
+        tmem_ld_x32(tS + 32, s1);
+        auto half_a = [&](const uint32_t (&s)[32], int c) {
+          uint32_t pk[16];
 #pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        uint32_t s[32];
-        tmem_ld_x32(tS + c * 32, s);
-        tmem_wait_ld();
-        uint32_t pk[16];
-#pragma unroll
-        for (int g = 0; g < 8; ++g) {
-          const float4 l = lse4[c * 8 + g];
-          const float p0 = ex2(fmaf(__uint_as_float(s[g * 4 + 0]), scale_log2, -l.x));
-          const float p1 = ex2(fmaf(__uint_as_float(s[g * 4 + 1]), scale_log2, -l.y));
-          const float p2 = ex2(fmaf(__uint_as_float(s[g * 4 + 2]), scale_log2, -l.z));
-          const float p3 = ex2(fmaf(__uint_as_float(s[g * 4 + 3]), scale_log2, -l.w));
-          p[c * 32 + g * 4 + 0] = p0; p[c * 32 + g * 4 + 1] = p1;
-          p[c * 32 + g * 4 + 2] = p2; p[c * 32 + g * 4 + 3] = p3;
-          pk[g * 2] = pack_bf16x2(p0, p1);
-          pk[g * 2 + 1] = pack_bf16x2(p2, p3);
-        }
-        tmem_st_x16(tS + c * 16, pk);      // overlays only S^T columns this thread has already loaded
+          for (int g = 0; g < 8; ++g) {
+            const float4 l = ld_shared_v4(lse4 + c * 8 + g);
+            const float2 x0 = ffma2(make_float2(__uint_as_float(s[g * 4 + 0]), __uint_as_float(s[g * 4 + 1])), sc2,
+                                    make_float2(-l.x, -l.y));
+            const float2 x1 = ffma2(make_float2(__uint_as_float(s[g * 4 + 2]), __uint_as_float(s[g * 4 + 3])), sc2,
+                                    make_float2(-l.z, -l.w));
+            const float2 p0 = make_float2(ex2(x0.x), ex2(x0.y));
+            const float2 p1 = make_float2(ex2(x1.x), ex2(x1.y));
+            p[c * 16 + g * 2] = p0;
+            p[c * 16 + g * 2 + 1] = p1;
+            pk[g * 2] = pack_bf16x2(p0.x, p0.y);
+            pk[g * 2 + 1] = pack_bf16x2(p1.x, p1.y);
+          }
+          tmem_st_x16(tS + c * 16, pk);      // overlays only S^T columns this thread has already loaded
+        };
+        tmem_wait_ld_x32(s0);
+        tmem_wait_ld_x32(s1);
+        half_a(s0, 0);
+        half_a(s1, 1);
       }
       tmem_wait_st();
       tc_fence_before();
@@ -319,26 +333,28 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       if (i > 0) mbar_wait(ds_empty, (i - 1) & 1);
       tc_fence_after();
       const long long b3 = BCLK();
+      {
+        uint32_t dp0[32], dp1[32];
+        tmem_ld_x32(tDP, dp0);
+        tmem_ld_x32(tDP + 32, dp1);
+        auto half_b = [&](const uint32_t (&dp)[32], int c) {
 #pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        uint32_t dp[32];
-        tmem_ld_x32(tDP + c * 32, dp);
-        tmem_wait_ld();
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {     // 8 queries = one 16-byte chunk of the row
-          const float4 da = d4[c * 8 + g * 2], db = d4[c * 8 + g * 2 + 1];
-          const int e = c * 32 + g * 8;
-          const uint32_t w0 = pack_bf16x2(p[e + 0] * (__uint_as_float(dp[g * 8 + 0]) - da.x),
-                                          p[e + 1] * (__uint_as_float(dp[g * 8 + 1]) - da.y));
-          const uint32_t w1 = pack_bf16x2(p[e + 2] * (__uint_as_float(dp[g * 8 + 2]) - da.z),
-                                          p[e + 3] * (__uint_as_float(dp[g * 8 + 3]) - da.w));
-          const uint32_t w2 = pack_bf16x2(p[e + 4] * (__uint_as_float(dp[g * 8 + 4]) - db.x),
-                                          p[e + 5] * (__uint_as_float(dp[g * 8 + 5]) - db.y));
-          const uint32_t w3 = pack_bf16x2(p[e + 6] * (__uint_as_float(dp[g * 8 + 6]) - db.z),
-                                          p[e + 7] * (__uint_as_float(dp[g * 8 + 7]) - db.w));
-          const int chunk = c * 4 + g;
-          st_shared_v4(ds_row + ((chunk ^ (row & 7)) << 4), w0, w1, w2, w3);
-        }
+          for (int g = 0; g < 4; ++g) {     // 8 queries = one 16-byte chunk of the row
+            const float4 da = ld_shared_v4(d4 + c * 8 + g * 2), db = ld_shared_v4(d4 + c * 8 + g * 2 + 1);
+            const int e = c * 16 + g * 4;
+            const float2 t0 = fmul2(p[e + 0], fadd2(make_float2(__uint_as_float(dp[g * 8 + 0]), __uint_as_float(dp[g * 8 + 1])), make_float2(-da.x, -da.y)));
+            const float2 t1 = fmul2(p[e + 1], fadd2(make_float2(__uint_as_float(dp[g * 8 + 2]), __uint_as_float(dp[g * 8 + 3])), make_float2(-da.z, -da.w)));
+            const float2 t2 = fmul2(p[e + 2], fadd2(make_float2(__uint_as_float(dp[g * 8 + 4]), __uint_as_float(dp[g * 8 + 5])), make_float2(-db.x, -db.y)));
+            const float2 t3 = fmul2(p[e + 3], fadd2(make_float2(__uint_as_float(dp[g * 8 + 6]), __uint_as_float(dp[g * 8 + 7])), make_float2(-db.z, -db.w)));
+            const int chunk = c * 4 + g;
+            st_shared_v4(ds_row + ((chunk ^ (row & 7)) << 4), pack_bf16x2(t0.x, t0.y), pack_bf16x2(t1.x, t1.y),
+                         pack_bf16x2(t2.x, t2.y), pack_bf16x2(t3.x, t3.y));
+          }
+        };
+        tmem_wait_ld_x32(dp0);
+        tmem_wait_ld_x32(dp1);
+        half_b(dp0, 0);
+        half_b(dp1, 1);
       }
       fence_proxy_async_smem();
       tc_fence_before();
@@ -367,11 +383,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         dst[g] = u;
       }
     }
-  } else {
+  } else if (warp < 12) {
     // ------------------------------------------------------------------ dQ drain warps (8-11)
-    // TMEM -> registers -> 128B-swizzled fp32 staging panel [128 rows][32 cols] -> one TMA reduce-add per panel
+    // TMEM -> registers (all d columns at once, so the TMEM columns go back to the MMA warp immediately)
+    // -> 128B-swizzled fp32 staging panel [128 rows][32 cols] -> one TMA reduce-add per panel
     // (cp.reduce.async.bulk.tensor ... .add): full-line L2 atomics issued by the TMA engine, nothing on the LSU
     // but conflict-free 16-byte shared stores.
+    setmaxnreg_inc<kBwdDrainRegs>();
     const int row = (warp & 3) * 32 + lane;                      // query row of the tile = TMEM lane
     const uint32_t tDQ = tmem + Cfg::tDQ + (static_cast<uint32_t>((warp & 3) * 32) << 16);
     const bool leader = warp == 8 && elect_one();
@@ -382,20 +400,21 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
       const long long d1 = BCLK();
+      uint32_t r[kD / 32][32];
+#pragma unroll
+      for (int c = 0; c < kD / 32; ++c) tmem_ld_x32(tDQ + c * 32, r[c]);
+#pragma unroll
+      for (int c = 0; c < kD / 32; ++c) tmem_wait_ld_x32(r[c]);
+      tc_fence_before();
+      mbar_arrive(dq_empty);               // the whole dQ(i) row has left TMEM: hand the columns back
 #pragma unroll
       for (int c = 0; c < kD / 32; ++c) {
-        uint32_t r[32];
-        tmem_ld_x32(tDQ + c * 32, r);
         if (leader) tma_wait_group_read<1>();      // the reduce that last read this panel has finished reading
         named_bar_sync(1, 128);
-        tmem_wait_ld();
-        if (c == kD / 32 - 1) {          // the whole dQ(i) row has left TMEM: hand the columns back
-          tc_fence_before();
-          mbar_arrive(dq_empty);
-        }
         uint8_t* prow = sDq + buf * Cfg::kDqPanelBytes + row * 128;
 #pragma unroll
-        for (int g = 0; g < 8; ++g) st_shared_v4(prow + ((g ^ (row & 7)) << 4), r[g * 4], r[g * 4 + 1], r[g * 4 + 2], r[g * 4 + 3]);
+        for (int g = 0; g < 8; ++g)
+          st_shared_v4(prow + ((g ^ (row & 7)) << 4), r[c][g * 4], r[c][g * 4 + 1], r[c][g * 4 + 2], r[c][g * 4 + 3]);
         fence_proxy_async_smem();
         named_bar_sync(2, 128);
         if (leader) {
@@ -408,6 +427,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     }
     if (leader) tma_wait_group<0>();
     __syncwarp();
+  } else {
+    setmaxnreg_dec<kBwdAuxRegs>();   // warps 14-15: release their registers
   }
 
   tc_fence_before();

@@ -287,6 +287,14 @@ __device__ __forceinline__ void red_add_v4(float* gptr, float a, float b, float 
   asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(gptr), "f"(a), "f"(b), "f"(c), "f"(d)
                : "memory");
 }
+// explicit shared-space 16-byte load (a generic-pointer dereference would compile to LD.E, not LDS)
+__device__ __forceinline__ float4 ld_shared_v4(const void* smem_src) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+               : "r"(smem_u32(smem_src)));
+  return v;
+}
 __device__ __forceinline__ void st_shared_v4(void* smem_dst, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(smem_u32(smem_dst)), "r"(a), "r"(b), "r"(c), "r"(d)
                : "memory");
