@@ -166,7 +166,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     int qs = Cfg::kQStages > 1 ? 1 : 0, qph = Cfg::kQStages > 1 ? 0 : 1, ds = 0, dph = 0;
     for (int i = 0; i < n_q; ++i) {
       // dO_i: its slot is free once dV(i - kDoStages) has read it
-      mbar_wait(&do_empty[ds], dph ^ 1);
+      mbar_wait_relaxed(&do_empty[ds], dph ^ 1);
       if (leader) {
         mbar_arrive_expect_tx(&do_full[ds], Cfg::kTileBytes);
 #pragma unroll
@@ -178,7 +178,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       if (++ds == Cfg::kDoStages) { ds = 0; dph ^= 1; }
       // Q_{i+1}: its slot is free once dK(i + 1 - kQStages) has read it
       if (i + 1 < n_q) {
-        mbar_wait(&q_empty[qs], qph ^ 1);
+        mbar_wait_relaxed(&q_empty[qs], qph ^ 1);
         load_q(i + 1, qs);
         if (++qs == Cfg::kQStages) { qs = 0; qph ^= 1; }
       }

@@ -120,7 +120,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       load_tile(sQ, &map_q, &q_full[0], q_row0, pol_q);
       int stage = 0, phase = 0;
       for (int i = 0; i < 2 * n_kv; ++i) {      // ring order K_0, V_0, K_1, V_1, ...
-        mbar_wait(&kv_empty[stage], phase ^ 1);
+        mbar_wait_relaxed(&kv_empty[stage], phase ^ 1);
         load_tile(sKV + stage * Cfg::kTileBytes, (i & 1) ? &map_v : &map_k, &kv_full[stage],
                   k_row0 + (i >> 1) * kBlockN, pol_kv);
         if (i == 0) load_tile(sQ + Cfg::kTileBytes, &map_q, &q_full[1], q_row0 + kBlockM, pol_q);
