@@ -39,7 +39,7 @@ using namespace ptx;
 
 constexpr int kTile = 128;
 constexpr int kBwdThreads = 512;                 // 4 warpgroups; registers re-split with setmaxnreg
-constexpr int kBwdComputeRegs = 152, kBwdDrainRegs = 152, kBwdAuxRegs = 40;   // 256*152 + 128*152 + 128*40 = 63488
+constexpr int kBwdComputeRegs = 176, kBwdDrainRegs = 96, kBwdAuxRegs = 40;   // 256*176 + 128*96 + 128*40 = 62464
 
 template <int kD>
 struct BwdCfg {
@@ -291,8 +291,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(&q_full[stage], phase);
       if (++stage == Cfg::kQStages) { stage = 0; phase ^= 1; }
       // ---- phase A: P^T = exp2(scale_log2 * S^T - lse2)
+      // (lse2 / D are read from shared memory eight 16-byte loads at a time, ahead of the arithmetic that uses
+      // them, so that their latency is paid once per half and mostly behind the mbarrier wait)
       const int i_ = i;
       const long long b0 = BCLK();
+      float4 aux[8];
+#pragma unroll
+      for (int g = 0; g < 8; ++g) aux[g] = ld_shared_v4(lse4 + g);
       mbar_wait(s_full, i & 1);
       tc_fence_after();
       const long long b1 = BCLK();
@@ -302,20 +307,27 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         tmem_ld_x32(tS, s0);
         tmem_ld_x32(tS + 32, s1);
         auto half_a = [&](const uint32_t (&s)[32], int c) {
-          uint32_t pk[16];
+          float2 x[16];
 #pragma unroll
           for (int g = 0; g < 8; ++g) {
-            const float4 l = ld_shared_v4(lse4 + c * 8 + g);
-            const float2 x0 = ffma2(make_float2(__uint_as_float(s[g * 4 + 0]), __uint_as_float(s[g * 4 + 1])), sc2,
-                                    make_float2(-l.x, -l.y));
-            const float2 x1 = ffma2(make_float2(__uint_as_float(s[g * 4 + 2]), __uint_as_float(s[g * 4 + 3])), sc2,
-                                    make_float2(-l.z, -l.w));
-            const float2 p0 = make_float2(ex2(x0.x), ex2(x0.y));
-            const float2 p1 = make_float2(ex2(x1.x), ex2(x1.y));
-            p[c * 16 + g * 2] = p0;
-            p[c * 16 + g * 2 + 1] = p1;
-            pk[g * 2] = pack_bf16x2(p0.x, p0.y);
-            pk[g * 2 + 1] = pack_bf16x2(p1.x, p1.y);
+            x[g * 2] = ffma2(make_float2(__uint_as_float(s[g * 4 + 0]), __uint_as_float(s[g * 4 + 1])), sc2,
+                             make_float2(-aux[g].x, -aux[g].y));
+            x[g * 2 + 1] = ffma2(make_float2(__uint_as_float(s[g * 4 + 2]), __uint_as_float(s[g * 4 + 3])), sc2,
+                                 make_float2(-aux[g].z, -aux[g].w));
+          }
+          if (c == 0) {
+#pragma unroll
+            for (int g = 0; g < 8; ++g) aux[g] = ld_shared_v4(lse4 + 8 + g);     // second half's lse2
+          } else {
+#pragma unroll
+            for (int g = 0; g < 8; ++g) aux[g] = ld_shared_v4(d4 + g);           // phase B's first half of D
+          }
+          uint32_t pk[16];
+#pragma unroll
+          for (int e = 0; e < 16; ++e) {
+            const float2 pe = make_float2(ex2(x[e].x), ex2(x[e].y));
+            p[c * 16 + e] = pe;
+            pk[e] = pack_bf16x2(pe.x, pe.y);
           }
           tmem_st_x16(tS + c * 16, pk);      // overlays only S^T columns this thread has already loaded
         };
@@ -338,17 +350,26 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         tmem_ld_x32(tDP, dp0);
         tmem_ld_x32(tDP + 32, dp1);
         auto half_b = [&](const uint32_t (&dp)[32], int c) {
+          float2 t[16];
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            t[g * 2] = fadd2(make_float2(__uint_as_float(dp[g * 4 + 0]), __uint_as_float(dp[g * 4 + 1])),
+                             make_float2(-aux[g].x, -aux[g].y));
+            t[g * 2 + 1] = fadd2(make_float2(__uint_as_float(dp[g * 4 + 2]), __uint_as_float(dp[g * 4 + 3])),
+                                 make_float2(-aux[g].z, -aux[g].w));
+          }
+          if (c == 0) {
+#pragma unroll
+            for (int g = 0; g < 8; ++g) aux[g] = ld_shared_v4(d4 + 8 + g);       // second half of D
+          }
 #pragma unroll
           for (int g = 0; g < 4; ++g) {     // 8 queries = one 16-byte chunk of the row
-            const float4 da = ld_shared_v4(d4 + c * 8 + g * 2), db = ld_shared_v4(d4 + c * 8 + g * 2 + 1);
-            const int e = c * 16 + g * 4;
-            const float2 t0 = fmul2(p[e + 0], fadd2(make_float2(__uint_as_float(dp[g * 8 + 0]), __uint_as_float(dp[g * 8 + 1])), make_float2(-da.x, -da.y)));
-            const float2 t1 = fmul2(p[e + 1], fadd2(make_float2(__uint_as_float(dp[g * 8 + 2]), __uint_as_float(dp[g * 8 + 3])), make_float2(-da.z, -da.w)));
-            const float2 t2 = fmul2(p[e + 2], fadd2(make_float2(__uint_as_float(dp[g * 8 + 4]), __uint_as_float(dp[g * 8 + 5])), make_float2(-db.x, -db.y)));
-            const float2 t3 = fmul2(p[e + 3], fadd2(make_float2(__uint_as_float(dp[g * 8 + 6]), __uint_as_float(dp[g * 8 + 7])), make_float2(-db.z, -db.w)));
+            const int e = g * 4;
+            const float2 w0 = fmul2(p[c * 16 + e + 0], t[e + 0]), w1 = fmul2(p[c * 16 + e + 1], t[e + 1]);
+            const float2 w2 = fmul2(p[c * 16 + e + 2], t[e + 2]), w3 = fmul2(p[c * 16 + e + 3], t[e + 3]);
             const int chunk = c * 4 + g;
-            st_shared_v4(ds_row + ((chunk ^ (row & 7)) << 4), pack_bf16x2(t0.x, t0.y), pack_bf16x2(t1.x, t1.y),
-                         pack_bf16x2(t2.x, t2.y), pack_bf16x2(t3.x, t3.y));
+            st_shared_v4(ds_row + ((chunk ^ (row & 7)) << 4), pack_bf16x2(w0.x, w0.y), pack_bf16x2(w1.x, w1.y),
+                         pack_bf16x2(w2.x, w2.y), pack_bf16x2(w3.x, w3.y));
           }
         };
         tmem_wait_ld_x32(dp0);
@@ -389,7 +410,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     // -> 128B-swizzled fp32 staging panel [128 rows][32 cols] -> one TMA reduce-add per panel
     // (cp.reduce.async.bulk.tensor ... .add): full-line L2 atomics issued by the TMA engine, nothing on the LSU
     // but conflict-free 16-byte shared stores.
-    setmaxnreg_inc<kBwdDrainRegs>();
+    setmaxnreg_dec<kBwdDrainRegs>();
     const int row = (warp & 3) * 32 + lane;                      // query row of the tile = TMEM lane
     const uint32_t tDQ = tmem + Cfg::tDQ + (static_cast<uint32_t>((warp & 3) * 32) << 16);
     const bool leader = warp == 8 && elect_one();
@@ -400,28 +421,33 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
       const long long d1 = BCLK();
-      uint32_t r[kD / 32][32];
 #pragma unroll
-      for (int c = 0; c < kD / 32; ++c) tmem_ld_x32(tDQ + c * 32, r[c]);
+      for (int rd = 0; rd < kD / 64; ++rd) {     // 64 columns per round keep the drain warps under 100 registers
+        uint32_t r[2][32];
 #pragma unroll
-      for (int c = 0; c < kD / 32; ++c) tmem_wait_ld_x32(r[c]);
-      tc_fence_before();
-      mbar_arrive(dq_empty);               // the whole dQ(i) row has left TMEM: hand the columns back
+        for (int c = 0; c < 2; ++c) tmem_ld_x32(tDQ + rd * 64 + c * 32, r[c]);
 #pragma unroll
-      for (int c = 0; c < kD / 32; ++c) {
-        if (leader) tma_wait_group_read<1>();      // the reduce that last read this panel has finished reading
-        named_bar_sync(1, 128);
-        uint8_t* prow = sDq + buf * Cfg::kDqPanelBytes + row * 128;
-#pragma unroll
-        for (int g = 0; g < 8; ++g)
-          st_shared_v4(prow + ((g ^ (row & 7)) << 4), r[c][g * 4], r[c][g * 4 + 1], r[c][g * 4 + 2], r[c][g * 4 + 3]);
-        fence_proxy_async_smem();
-        named_bar_sync(2, 128);
-        if (leader) {
-          tma_reduce_add_2d(&map_dq, sDq + buf * Cfg::kDqPanelBytes, c * 32, q_row0 + i * kTile);
-          tma_commit_group();
+        for (int c = 0; c < 2; ++c) tmem_wait_ld_x32(r[c]);
+        if (rd == kD / 64 - 1) {
+          tc_fence_before();
+          mbar_arrive(dq_empty);             // the whole dQ(i) row has left TMEM: hand the columns back
         }
-        buf ^= 1;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          if (leader) tma_wait_group_read<1>();      // the reduce that last read this panel has finished reading
+          named_bar_sync(1, 128);
+          uint8_t* prow = sDq + buf * Cfg::kDqPanelBytes + row * 128;
+#pragma unroll
+          for (int g = 0; g < 8; ++g)
+            st_shared_v4(prow + ((g ^ (row & 7)) << 4), r[c][g * 4], r[c][g * 4 + 1], r[c][g * 4 + 2], r[c][g * 4 + 3]);
+          fence_proxy_async_smem();
+          named_bar_sync(2, 128);
+          if (leader) {
+            tma_reduce_add_2d(&map_dq, sDq + buf * Cfg::kDqPanelBytes, rd * 64 + c * 32, q_row0 + i * kTile);
+            tma_commit_group();
+          }
+          buf ^= 1;
+        }
       }
       if (threadIdx.x == 256) { BADD(5, d1 - d0); BADD(6, BCLK() - d1); }
     }
