@@ -33,6 +33,13 @@ __device__ long long g_bwd_clocks[16];
 #define BCLK() 0ll
 #define BADD(i, v) do { } while (0)
 #endif
+#ifdef RINGX_BWD_TRACE
+// debug timeline: clock64 of event `ev` of step i (16 <= i < 24) of CTA (0,0), one writer thread per event
+__device__ long long g_bwd_trace[8 * 16];
+#define BTRACE(ev, step) do { if (blockIdx.x == 0 && blockIdx.y == 0 && (step) >= 16 && (step) < 24) g_bwd_trace[((step) - 16) * 16 + (ev)] = clock64(); } while (0)
+#else
+#define BTRACE(ev, step) do { } while (0)
+#endif
 namespace {
 
 using namespace ptx;
@@ -40,6 +47,16 @@ using namespace ptx;
 constexpr int kTile = 128;
 constexpr int kBwdThreads = 512;                 // 4 warpgroups; registers re-split with setmaxnreg
 constexpr int kBwdComputeRegs = 176, kBwdDrainRegs = 96, kBwdAuxRegs = 40;   // 256*176 + 128*96 + 128*40 = 62464
+// Which of the 16 element pairs per 32-column half of phase A take 2^x from the FMA-pipe polynomial (ptx::ex2_poly2)
+// instead of MUFU.EX2.  At d = 64 phase A's 16 ex2 per clock are the co-limiter (5 MMAs of half the length per
+// exponential): every fourth pair on the FMA pipe measured +4 % (C4 backward 897 -> 935 TFLOP/s); at d = 128 the
+// tensor chain hides phase A and any share measured -1 %, so it stays on the MUFU.
+#ifndef RINGX_BWD_POLY_MASK_D64
+#define RINGX_BWD_POLY_MASK_D64 0x8888
+#endif
+#ifndef RINGX_BWD_POLY_MASK_D128
+#define RINGX_BWD_POLY_MASK_D128 0x0000
+#endif
 
 template <int kD>
 struct BwdCfg {
@@ -56,6 +73,7 @@ struct BwdCfg {
                                     kDsBytes + 2 * kDqPanelBytes + 256;
   static constexpr uint32_t tS = 0, tDP = 128, tDV = 256, tDK = 256 + kD, tDQ = kD == 64 ? 384 : 128;
   static constexpr bool kDqOverlaysDp = kD != 64;
+  static constexpr unsigned kPolyMask = kD == 64 ? RINGX_BWD_POLY_MASK_D64 : RINGX_BWD_POLY_MASK_D128;
 };
 
 template <int kD>
@@ -236,6 +254,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       // ---- behind phase A: dV += P^T(i) dO_i, then S^T(i+1)
       mbar_wait(p_full, i & 1);
       tc_fence_after();
+      if (leader) BTRACE(8, i);      // MMA warp saw p_full(i)
       if (leader) {
 #pragma unroll
         for (int k = 0; k < kTile / 16; ++k)
@@ -247,12 +266,14 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       if (more) {
         mbar_wait(&q_full[qs], qph);
         tc_fence_after();
+        if (leader) BTRACE(9, i);    // Q(i+1) there, S^T(i+1) issued
         issue_st(q_base + qs * Cfg::kQStageBytes);
       }
       // ---- behind phase B: dQ(i) = dS(i) K_j (drained under the next MMA), dK += dS^T(i) Q_i, then dP^T(i+1)
       mbar_wait(ds_full, i & 1);
       if (!Cfg::kDqOverlaysDp && i > 0) mbar_wait(dq_empty, (i - 1) & 1);
       tc_fence_after();
+      if (leader) BTRACE(10, i);     // MMA warp saw ds_full(i)
       if (leader) {
 #pragma unroll
         for (int k = 0; k < kTile / 16; ++k)
@@ -267,8 +288,10 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       __syncwarp();
       if (more) {
         mbar_wait(&do_full[ds], dph);
+        if (leader) BTRACE(11, i);   // dO(i+1) there
         if (Cfg::kDqOverlaysDp) mbar_wait(dq_empty, i & 1);   // dQ(i) sits in the dP^T columns until drained
         tc_fence_after();
+        if (leader) BTRACE(12, i);   // dq_empty(i) seen, dP^T(i+1) issued
         issue_dpt(do_base + ds * Cfg::kTileBytes);
       }
     }
@@ -301,6 +324,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(s_full, i & 1);
       tc_fence_after();
       const long long b1 = BCLK();
+      if (threadIdx.x == 0) BTRACE(0, i);   // s_full(i) seen
       float2 p[32];
       {
         uint32_t s0[32], s1[32];
@@ -325,7 +349,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           uint32_t pk[16];
 #pragma unroll
           for (int e = 0; e < 16; ++e) {
-            const float2 pe = make_float2(ex2(x[e].x), ex2(x[e].y));
+            const float2 pe = ((Cfg::kPolyMask >> e) & 1) ? ex2_poly2(x[e]) : make_float2(ex2(x[e].x), ex2(x[e].y));
             p[c * 16 + e] = pe;
             pk[e] = pack_bf16x2(pe.x, pe.y);
           }
@@ -340,11 +364,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       tc_fence_before();
       mbar_arrive(p_full);
       const long long b2 = BCLK();
+      if (threadIdx.x == 0) BTRACE(1, i);   // p_full(i) arrived
       // ---- phase B: dS^T = P^T o (dP^T - D), bf16, to shared memory [keys][queries] (128B-swizzled rows)
       mbar_wait(dp_full, i & 1);
       if (i > 0) mbar_wait(ds_empty, (i - 1) & 1);
       tc_fence_after();
       const long long b3 = BCLK();
+      if (threadIdx.x == 0) BTRACE(2, i);   // dp_full(i) (and ds_empty(i-1)) seen
       {
         uint32_t dp0[32], dp1[32];
         tmem_ld_x32(tDP, dp0);
@@ -380,6 +406,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       fence_proxy_async_smem();
       tc_fence_before();
       mbar_arrive(ds_full);
+      if (threadIdx.x == 0) BTRACE(3, i);   // ds_full(i) arrived
       if (threadIdx.x == 0) { BADD(0, b1 - b0); BADD(1, b2 - b1); BADD(2, b3 - b2); BADD(3, BCLK() - b3); BADD(4, 1); }
     }
     // ---- epilogue: dV_j (warps 0-3) and scale * dK_j (warps 4-7), bf16, written once
@@ -421,6 +448,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
       const long long d1 = BCLK();
+      if (threadIdx.x == 256) BTRACE(4, i);   // dq_full(i) seen
 #pragma unroll
       for (int rd = 0; rd < kD / 64; ++rd) {     // 64 columns per round keep the drain warps under 100 registers
         uint32_t r[2][32];
@@ -431,6 +459,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         if (rd == kD / 64 - 1) {
           tc_fence_before();
           mbar_arrive(dq_empty);             // the whole dQ(i) row has left TMEM: hand the columns back
+          if (threadIdx.x == 256) BTRACE(5, i);
         }
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
@@ -502,6 +531,13 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
 
 }  // namespace ringx
 
+#ifdef RINGX_BWD_TRACE
+extern "C" __attribute__((visibility("default"))) int ringx_debug_bwd_trace(long long* out) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, ringx::g_bwd_trace, sizeof(long long) * 128);
+  return 0;
+}
+#endif
 #ifdef RINGX_BWD_CLOCKS
 extern "C" __attribute__((visibility("default"))) int ringx_debug_bwd_clocks(long long* out) {
   cudaDeviceSynchronize();

@@ -10,11 +10,16 @@
 //   warp  8     TMA producer: Q tiles once, then the K/V ring (K_0, V_0, K_1, V_1, ...)              56 regs
 //   warp  9     MMA issuer (one elected lane): S_t = Q_t K_j^T (SS), O_t += P_t V_j (P from TMEM)    56 regs
 //   warps 10-11 idle (they only complete the third warpgroup so that setmaxnreg can be used)
-// TMEM columns: S_0 [0,128) S_1 [128,256) O_0 [256,256+d) O_1 [256+d,256+2d); P_t (bf16) overwrites
+// TMEM columns (d = 128): S_0 [0,128) S_1 [128,256) O_0 [256,384) O_1 [384,512); P_t (bf16) overwrites
 // the first 64 columns of S_t.  The two query tiles ping-pong: while warpgroup t turns S_t into P_t the
 // tensor core works on tile 1-t.  The MMA pipe executes in issue order, so S_t(j+1) -- issued right after
 // O_t += P_t(j) V_j -- cannot overwrite P_t(j) early, and the commit that signals S_t(j+1) also proves
 // O_t(j) complete: the softmax warps may rescale O_t in place without a further barrier.
+// d = 64 has 128 TMEM columns to spare and uses them for a third score buffer: S number n = 2j + t goes to
+// buffer n % 3 [0,384), O_0 [384,448), O_1 [448,512), and is issued behind PV number n - 3, i.e. one tile
+// ahead, so a softmax warpgroup finds its next scores waiting (ring order K_0 K_1 V_0 K_2 V_1 ...).  Running
+// ahead of PV_t(j-1) costs two waits on pv_done[t]: before the (rare) in-place rescale of O_t, and before P_t(j)
+// is signalled (so that p_full cannot complete twice before the MMA warp has seen it once).
 // Online softmax in the exp2 domain with a lazy running max (O, l are only rescaled when the row max
 // grew by more than 2^8), so the rescale is off the common path.  The softmax streams S out of TMEM in
 // 32-column pieces (the row max of piece c is taken while piece c+1 is in flight), uses the packed
@@ -38,6 +43,17 @@ constexpr int kBlockN = 128;          // keys per KV tile
 constexpr int kFwdThreads = 384;
 constexpr int kSoftmaxRegs = 224, kAuxRegs = 56;   // 256*224 + 128*56 = 64512 <= 65536
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
+// d = 64 is bound by the softmax warps (one exponential per 4*64 tensor FLOPs: 2048 clk of MUFU.EX2 against 1024 clk
+// of MMA per 128-key iteration).  Of the 16 element pairs of every 32-key piece, those in this mask take 2^x from the
+// FMA-pipe polynomial ptx::ex2_poly2 (degree 4, relative error 2.7e-6: P also feeds the fp32 row sum behind LSE).
+// Measured on C4 forward with three score buffers: 0 -> 781, 1/8 -> 796, 1/4 -> 791 TFLOP/s (the warps are close to
+// issue-bound as well).  d = 128 is balanced and power-capped: it stays on the MUFU.
+#ifndef RINGX_FWD_POLY_MASK_D64
+#define RINGX_FWD_POLY_MASK_D64 0x8080
+#endif
+#ifndef RINGX_FWD_POLY_DEGREE
+#define RINGX_FWD_POLY_DEGREE 4
+#endif
 
 template <int kD>
 struct FwdCfg {
@@ -45,6 +61,12 @@ struct FwdCfg {
   static constexpr int kPanelBytes = 128 * 128;              // 128 rows x 128 B
   static constexpr int kTileBytes = kPanels * kPanelBytes;   // Q, K or V tile
   static constexpr int kStages = kD == 128 ? 5 : 8;          // K/V ring slots
+  static constexpr unsigned kPolyMask = kD == 64 ? RINGX_FWD_POLY_MASK_D64 : 0u;
+  // Score buffers in TMEM.  d = 128: one per query tile (2 x 128 + 2 x 128 O columns = 512).  d = 64 leaves 128
+  // columns, enough for a third buffer: the score MMAs then run one tile ahead (S number n = 2j + t goes to buffer
+  // n % 3 and is issued behind PV number n - 3), so a softmax warpgroup never waits for its next scores.
+  static constexpr int kSBufs = kD == 128 ? 2 : 3;
+  static constexpr uint32_t kOBase = kSBufs * 128;           // O_t at kOBase + t * kD
   static constexpr int kBarBytes = 256;
   static constexpr int kSmemBytes = 1024 + 2 * kTileBytes + kStages * kTileBytes + kBarBytes;
 };
@@ -61,12 +83,13 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   uint8_t* sKV = smem + 2 * Cfg::kTileBytes;
   uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + Cfg::kStages * Cfg::kTileBytes);
   uint64_t* q_full = bars;                  // [2]  TMA -> MMA
-  uint64_t* s_full = bars + 2;              // [2]  MMA -> softmax: S_t(j) in TMEM
-  uint64_t* p_full = bars + 4;              // [2][2] softmax -> MMA: half h (64 keys) of P_t(j) in TMEM (O_t rescaled if needed)
-  uint64_t* o_full = bars + 8;              // [2]  MMA -> softmax: last O_t complete
-  uint64_t* kv_full = bars + 10;            // [kStages]
-  uint64_t* kv_empty = bars + 10 + Cfg::kStages;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 10 + 2 * Cfg::kStages);
+  uint64_t* s_full = bars + 2;              // [kSBufs] MMA -> softmax: score buffer b holds S number n (n % kSBufs == b)
+  uint64_t* p_full = bars + 5;              // [2][2] softmax -> MMA: half h (64 keys) of P_t(j) in TMEM (O_t rescaled if needed)
+  uint64_t* o_full = bars + 9;              // [2]  MMA -> softmax: last O_t complete
+  uint64_t* pv_done = bars + 11;            // [2]  MMA -> softmax: O_t += P_t(j) V_j complete (used when kSBufs > 2)
+  uint64_t* kv_full = bars + 13;            // [kStages]
+  uint64_t* kv_empty = bars + 13 + Cfg::kStages;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 13 + 2 * Cfg::kStages);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // provably warp-uniform: keeps MMA/TMA operands in uniform registers
   const int lane = threadIdx.x & 31;
@@ -77,11 +100,12 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
       mbar_init(&q_full[i], 1);
-      mbar_init(&s_full[i], 1);
       mbar_init(&p_full[2 * i], kBlockM);
       mbar_init(&p_full[2 * i + 1], kBlockM);
       mbar_init(&o_full[i], 1);
+      mbar_init(&pv_done[i], 1);
     }
+    for (int i = 0; i < Cfg::kSBufs; ++i) mbar_init(&s_full[i], 1);
     for (int i = 0; i < Cfg::kStages; ++i) {
       mbar_init(&kv_full[i], 1);
       mbar_init(&kv_empty[i], 1);
@@ -118,13 +142,22 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         __syncwarp();
       };
       load_tile(sQ, &map_q, &q_full[0], q_row0, pol_q);
-      int stage = 0, phase = 0;
-      for (int i = 0; i < 2 * n_kv; ++i) {      // ring order K_0, V_0, K_1, V_1, ...
+      // ring order = the order in which the MMA warp first touches the tiles: the K tiles of the kSBufs score MMAs
+      // of the prologue, then per PV number n its V tile (n even) and the K tile of S number n + kSBufs (if even)
+      //   kSBufs = 2: K_0 V_0 K_1 V_1 ...        kSBufs = 3: K_0 K_1 V_0 K_2 V_1 K_3 ...
+      int stage = 0, phase = 0, loaded = 0;
+      auto push = [&](const CUtensorMap* map, int j) {
         mbar_wait_relaxed(&kv_empty[stage], phase ^ 1);
-        load_tile(sKV + stage * Cfg::kTileBytes, (i & 1) ? &map_v : &map_k, &kv_full[stage],
-                  k_row0 + (i >> 1) * kBlockN, pol_kv);
-        if (i == 0) load_tile(sQ + Cfg::kTileBytes, &map_q, &q_full[1], q_row0 + kBlockM, pol_q);
+        load_tile(sKV + stage * Cfg::kTileBytes, map, &kv_full[stage], k_row0 + j * kBlockN, pol_kv);
+        if (loaded++ == 0) load_tile(sQ + Cfg::kTileBytes, &map_q, &q_full[1], q_row0 + kBlockM, pol_q);
         if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
+      };
+      const int n_s = 2 * n_kv;                  // score / PV MMAs are numbered n = 2 j + t
+      for (int m = 0; m < Cfg::kSBufs && m < n_s; m += 2) push(&map_k, m >> 1);
+      for (int n = 0; n < n_s; n += 2) {
+        push(&map_v, n >> 1);
+        const int m = n + Cfg::kSBufs + (Cfg::kSBufs & 1);     // the even S number among n + kSBufs, n + 1 + kSBufs
+        if (m < n_s) push(&map_k, m >> 1);
       }
     }
   } else if (warp == 9) {
@@ -137,27 +170,29 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       const uint32_t q_addr = smem_u32(sQ), kv_addr = smem_u32(sKV);
       int stage = 0, phase = 0;
       auto advance = [&]() { if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; } };
-      // S_t = Q_t K^T from the K tile in ring slot `st`
-      auto issue_s = [&](int t, int st) {
+      // S number n (tile t = n & 1) = Q_t K^T from the K tile in ring slot `st`, into score buffer n % kSBufs
+      auto issue_s = [&](int n, int t, int st) {
+        const int buf = Cfg::kSBufs == 2 ? t : n % Cfg::kSBufs;
         const uint32_t a0 = q_addr + t * Cfg::kTileBytes, b0 = kv_addr + st * Cfg::kTileBytes;
         if (leader) {
 #pragma unroll
           for (int k = 0; k < kD / 16; ++k) {
             const uint32_t off = (k >> 2) * Cfg::kPanelBytes + (k & 3) * 32;
-            mma_ss(tmem + t * kBlockN, make_smem_desc_sw128(a0 + off, 16, 1024),
+            mma_ss(tmem + buf * kBlockN, make_smem_desc_sw128(a0 + off, 16, 1024),
                    make_smem_desc_sw128(b0 + off, 16, 1024), idesc_s, k > 0);
           }
-          mma_commit(&s_full[t]);
+          mma_commit(&s_full[buf]);
         }
         __syncwarp();
       };
-      // O_t (+)= P_t V from the V tile in ring slot `st`
-      auto issue_o = [&](int t, int st, int half, bool accumulate) {   // keys [64*half, 64*half + 64) of the tile
+      // O_t (+)= P V: keys [64*half, 64*half + 64) of PV number n (P sits in score buffer n % kSBufs)
+      auto issue_o = [&](int n, int t, int st, int half, bool accumulate) {
+        const int buf = Cfg::kSBufs == 2 ? t : n % Cfg::kSBufs;
         const uint32_t b0 = kv_addr + st * Cfg::kTileBytes;
         if (leader) {
 #pragma unroll
           for (int k = half * 4; k < half * 4 + 4; ++k)
-            mma_ts(tmem + 256 + t * kD, tmem + t * kBlockN + k * 8,
+            mma_ts(tmem + Cfg::kOBase + t * kD, tmem + buf * kBlockN + k * 8,
                    make_smem_desc_sw128(b0 + k * 2048, Cfg::kPanelBytes, 1024), idesc_o, accumulate || k > 0);
         }
         __syncwarp();
@@ -166,46 +201,47 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         if (leader) mma_commit(bar);
         __syncwarp();
       };
-      // prologue: S_0(0), S_1(0)
-      mbar_wait(&kv_full[stage], phase);
-      mbar_wait(&q_full[0], 0);
-      tc_fence_after();
-      issue_s(0, stage);
-      mbar_wait(&q_full[1], 0);
-      tc_fence_after();
-      issue_s(1, stage);
-      commit(&kv_empty[stage]);
-      advance();
-      for (int j = 0; j < n_kv; ++j) {
-        const int v_stage = stage, v_phase = phase;
+      // ring slots are taken in the producer's order; a K tile serves S numbers 2j, 2j+1, a V tile PV numbers 2j, 2j+1
+      int k_slot = 0, v_slot = 0;
+      auto acquire = [&]() {
+        const int st = stage;
+        mbar_wait(&kv_full[stage], phase);
+        tc_fence_after();
         advance();
-        const int k_stage = stage, k_phase = phase;
-        const bool more = j + 1 < n_kv;
-        if (more) advance();
-        mbar_wait(&kv_full[v_stage], v_phase);
+        return st;
+      };
+      auto score = [&](int m, int t) {   // issue S number m (tile t = m & 1); the odd one releases the K tile
+        if (t == 0) k_slot = acquire();
+        if (m < 2) {
+          mbar_wait(&q_full[t], 0);
+          tc_fence_after();
+        }
+        issue_s(m, t, k_slot);
+        if (t == 1) commit(&kv_empty[k_slot]);
+      };
+      const int n_s = 2 * n_kv;
+#pragma unroll
+      for (int m = 0; m < Cfg::kSBufs; ++m)                            // prologue: the first kSBufs score tiles
+        if (m < n_s) score(m, m & 1);
+      for (int j = 0; j < n_kv; ++j) {
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
+          const int n = 2 * j + t;
+          if (t == 0) v_slot = acquire();
           const long long m0 = CLK();
           mbar_wait(&p_full[2 * t], j & 1);
           tc_fence_after();
 #ifdef RINGX_FWD_CLOCKS
           if (blockIdx.x == 0 && blockIdx.y == 0 && leader && j >= 8) atomicAdd((unsigned long long*)&g_fwd_clocks[8 + t], (unsigned long long)(CLK() - m0));
 #endif
-          issue_o(t, v_stage, 0, j > 0);
+          issue_o(n, t, v_slot, 0, j > 0);
           mbar_wait(&p_full[2 * t + 1], j & 1);
           tc_fence_after();
-          issue_o(t, v_stage, 1, true);
-          if (t == 1) commit(&kv_empty[v_stage]);
-          if (more) {
-            if (t == 0) {
-              mbar_wait(&kv_full[k_stage], k_phase);
-              tc_fence_after();
-            }
-            issue_s(t, k_stage);
-            if (t == 1) commit(&kv_empty[k_stage]);
-          } else {
-            commit(&o_full[t]);
-          }
+          issue_o(n, t, v_slot, 1, true);
+          if (Cfg::kSBufs > 2) commit(&pv_done[t]);
+          if (t == 1) commit(&kv_empty[v_slot]);
+          if (j + 1 == n_kv) commit(&o_full[t]);                              // last PV of tile t
+          if (n + Cfg::kSBufs < n_s) score(n + Cfg::kSBufs, (t + Cfg::kSBufs) & 1);   // refill the buffer PV number n freed
         }
       }
     }
@@ -214,15 +250,16 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     setmaxnreg_inc<kSoftmaxRegs>();
     const int t = warp >> 2;
     const uint32_t lane_off = static_cast<uint32_t>((warp & 3) * 32) << 16;
-    const uint32_t tS = tmem + t * kBlockN + lane_off;
-    const uint32_t tO = tmem + 256 + t * kD + lane_off;
+    const uint32_t tO = tmem + Cfg::kOBase + t * kD + lane_off;
     float m_raw = -CUDART_INF_F;   // running (lazy) row max of the unscaled scores
     float m_sc = -CUDART_INF_F;    // m_raw * scale_log2
     float l = 0.f;                 // running row sum of exp2(s*scale_log2 - m_sc)
     const float2 sc2 = make_float2(scale_log2, scale_log2);
     for (int j = 0; j < n_kv; ++j) {
       const long long c0 = CLK();
-      mbar_wait(&s_full[t], j & 1);
+      const int n = 2 * j + t, buf = Cfg::kSBufs == 2 ? t : n % Cfg::kSBufs;     // this tile's scores are S number n
+      const uint32_t tS = tmem + buf * kBlockN + lane_off;
+      mbar_wait(&s_full[buf], (Cfg::kSBufs == 2 ? j : n / Cfg::kSBufs) & 1);
       tc_fence_after();
       const long long c1 = CLK();
       // ---- pass 1: stream S_t(j) out of TMEM; the row max of piece c is taken while piece c+1 is in flight
@@ -255,6 +292,10 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         const float alpha = ex2((m_raw - m_new) * scale_log2);   // 0 on the first tile (m_raw = -inf)
         l *= alpha;
         if (j > 0) {
+          if (Cfg::kSBufs > 2) {     // the scores ran ahead of O_t += P_t(j-1) V: wait for it before touching O_t
+            mbar_wait(&pv_done[t], (j - 1) & 1);
+            tc_fence_after();
+          }
 #pragma unroll
           for (int c = 0; c < kD / 32; ++c) {
             uint32_t o[32];
@@ -278,8 +319,10 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         for (int i = 0; i < 32; i += 4) {
           const float2 x0 = ffma2(make_float2(__uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1])), sc2, nm2);
           const float2 x1 = ffma2(make_float2(__uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3])), sc2, nm2);
-          const float2 p0 = make_float2(ex2(x0.x), ex2(x0.y));
-          const float2 p1 = make_float2(ex2(x1.x), ex2(x1.y));
+          const float2 p0 = ((Cfg::kPolyMask >> (i / 2)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x0)
+                                                              : make_float2(ex2(x0.x), ex2(x0.y));
+          const float2 p1 = ((Cfg::kPolyMask >> (i / 2 + 1)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x1)
+                                                                  : make_float2(ex2(x1.x), ex2(x1.y));
           la = fadd2(la, p0);
           lb = fadd2(lb, p1);
           pk[i / 2] = pack_bf16x2(p0.x, p0.y);
@@ -289,6 +332,9 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         if (c & 1) {                       // 64 keys of P are in TMEM: let the tensor core start on them
           tmem_wait_st();
           tc_fence_before();
+          // (with the scores running ahead, P_t(j) could otherwise complete p_full a second time before the MMA warp
+          // has seen P_t(j-1): PV_t(j-1) complete proves it has)
+          if (Cfg::kSBufs > 2 && c == 1 && j > 0) mbar_wait(&pv_done[t], (j - 1) & 1);
           mbar_arrive(&p_full[2 * t + (c >> 1)]);
         }
       }

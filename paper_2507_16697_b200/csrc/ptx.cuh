@@ -282,6 +282,34 @@ __device__ __forceinline__ float2 fmul2(float2 a, float2 b) {
       : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
   return d;
 }
+// 2^x for a pair, x <= ~0, on the FMA/ALU pipes only (no MUFU): Cody-Waite split x = n + f with the
+// 1.5*2^23 rounding constant (n lands in the low mantissa bits of x + magic), a degree-3 minimax
+// polynomial for 2^f on [-0.5, 0.5] (max relative error 7.5e-5 -- 50x below the bf16 rounding P gets
+// next; degree 4: 2.7e-6), and n added straight into the exponent field.  Inputs below -125 are clamped (result ~2^-125).
+template <int kDegree = 3>
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  const float2 magic = make_float2(12582912.f, 12582912.f);
+  x.x = fmaxf(x.x, -125.f);
+  x.y = fmaxf(x.y, -125.f);
+  const float2 xr = fadd2(x, magic);
+  const float2 n = fadd2(xr, make_float2(-12582912.f, -12582912.f));
+  const float2 f = ffma2(n, make_float2(-1.f, -1.f), x);
+  float2 p;
+  if (kDegree == 3) {
+    p = ffma2(f, make_float2(0x1.c3f75ep-5f, 0x1.c3f75ep-5f), make_float2(0x1.f0de1ap-3f, 0x1.f0de1ap-3f));
+    p = ffma2(p, f, make_float2(0x1.62f31ap-1f, 0x1.62f31ap-1f));
+    p = ffma2(p, f, make_float2(0x1.fff692p-1f, 0x1.fff692p-1f));
+  } else {   // degree 4: max relative error 2.7e-6 (where the result also feeds an fp32 row sum / LSE)
+    p = ffma2(f, make_float2(0x1.3997d4p-7f, 0x1.3997d4p-7f), make_float2(0x1.ca1440p-5f, 0x1.ca1440p-5f));
+    p = ffma2(p, f, make_float2(0x1.ec06dap-3f, 0x1.ec06dap-3f));
+    p = ffma2(p, f, make_float2(0x1.62e0dcp-1f, 0x1.62e0dcp-1f));
+    p = ffma2(p, f, make_float2(0x1.ffffe8p-1f, 0x1.ffffe8p-1f));
+  }
+  float2 r;
+  r.x = __uint_as_float(__float_as_uint(p.x) + (__float_as_uint(xr.x) << 23));
+  r.y = __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(xr.y) << 23));
+  return r;
+}
 // three-input max (FMNMX3)
 __device__ __forceinline__ float fmax3(float a, float b, float c) {
   float d;
