@@ -107,6 +107,41 @@ RINGX_API int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o
 RINGX_API int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse,
                          int B, int H, int Nq, int Nk, int d, float scale, int dtype, void* stream);
 
+/* Per-device backward step of RingX_a / RingX_b (l.143, l.145): the gradient contributions that `Nq` query
+ * rows and `Nk` keys of every head exchange, with P recomputed from the *global* lse of those rows (the
+ * LSE over ALL keys of the sequence, not only the Nk given here; reading g8 of DESIGN.md).
+ *   q, o, dO [B,H,Nq,d] bf16 (in); lse [B,H,Nq] float (in); k, v [B,H,Nk,d] bf16 (in).
+ *   dq_acc [B,H,Nq,d] FLOAT, in/out: += sum over the Nk keys of dS_ij K_j (scale included) -- "the gradient
+ *          for Q is accumulated ... over N steps"; the caller zeroes it before the first step and casts it
+ *          with ringx_dq_finalize after the last.  Summation order is not deterministic.
+ *   dk, dv [B,H,Nk,d] bf16 (out): the sums over the Nq query rows given (complete when the caller holds
+ *          every query of the head, otherwise one device's share to be reduced across devices).
+ *   Nq % 128 == 0, Nk % 128 == 0, d in {64,128}; dtype must be RINGX_BF16.
+ *   workspace  >= ringx_attn_bwd_partial_workspace_bytes(B,H,Nq,d) bytes, 256-byte aligned. */
+RINGX_API int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                           const void* dO, float* dq_acc, void* dk, void* dv,
+                           int B, int H, int Nq, int Nk, int d, float scale, int dtype,
+                           void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d);
+
+/* dq = bf16(dq_acc), n elements (n % 4 == 0), round to nearest even: closes the accumulation over steps. */
+RINGX_API int ringx_dq_finalize(const float* dq_acc, void* dq, long long n, void* stream);
+
+/* Eq. 5 in its N-operand form, as RingX_a uses it across devices (l.130-133, l.137, l.143):
+ *   ringx_eq5_scale     one operand's share: w = exp(loc_lse - lse_max); num = w * loc_out; den = w, where
+ *                       lse_max is the element-wise max of loc_lse over all operands (the all-reduce(max));
+ *                       an operand with loc_lse = -inf has weight 0 and its loc_out is ignored.
+ *   ringx_eq5_finalize  after num and den were summed over the operands (the reduce): o = num / den,
+ *                       lse = lse_max + log(den); den = 0 gives o = 0, lse = -inf.
+ *   loc_out, num [rows,d] float; loc_lse, lse_max, den, lse_out [rows] float; o_out [rows,d] of o_out_dtype.
+ *   num may alias loc_out; o_out may alias num when float; lse_out may alias lse_max.  den must not alias
+ *   loc_lse or lse_max, and lse_out must not alias den (other threads of the row still read them).
+ *   d % 8 == 0, 8 <= d <= 1024; rows >= 0. */
+RINGX_API int ringx_eq5_scale(const float* loc_out, const float* loc_lse, const float* lse_max,
+                    float* num, float* den, long long rows, int d, void* stream);
+RINGX_API int ringx_eq5_finalize(const float* num, const float* den, const float* lse_max,
+                       void* o_out, float* lse_out, long long rows, int d, int o_out_dtype, void* stream);
+
 /* ringx_attn_fwd with HOST buffers (the end-to-end entry): copies q,k,v host->device into the
  * workspace, runs ringx_attn_fwd, copies o and lse back, and synchronises `stream`.
  *   q_host,k_host,v_host,o_host,lse_host  HOST pointers (pinned memory recommended).

@@ -148,6 +148,16 @@ def attention_bwd_cols(q, k_cols, v_cols, dO, lse, D, scale):
     return dk, dv
 
 
+def attention_bwd_partial(q, k_cols, v_cols, dO, lse, D, scale):
+    """One device's step of the RingX backward (reading g8): with the *global* LSE_i and D_i
+    of the given query rows, the key subset (k_cols, v_cols) yields its complete share of those rows' dQ,
+    dQ_i += scale sum_{j in cols} dS_ij k_j, and these rows' share of dK_j, dV_j for j in cols.
+    Summing the dQ shares over a partition of the keys gives `attention_bwd`'s dQ."""
+    p = np.exp(scores(q, k_cols, scale) - lse[:, None])       # [Nq, ncols]
+    ds = p * (dO @ v_cols.T - D[:, None])
+    return scale * (ds @ k_cols), scale * (ds.T @ q), p.T @ dO
+
+
 # --------------------------------------------------------------------------------------------
 # [B,H,N,d] conveniences (loops over heads; block_rows bounds the [rows, N] score matrix)
 # --------------------------------------------------------------------------------------------

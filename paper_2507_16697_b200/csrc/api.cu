@@ -299,6 +299,34 @@ int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const 
   return RINGX_OK;
 }
 
+// Shared backward driver: D/lse2 preprocess, one kernel pass per KV chunk of the nk keys, optional bf16 cast of dQ.
+// q,o,dO,lse: Nq rows per head; k,v,dk,dv: Nk rows per head.  dq_acc fp32 [BH,Nq,d] (zeroed first when zero_dq).
+static int bwd_core(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
+                    float* D, float* lse2, float* dq_acc, bool zero_dq, void* dq_bf16, void* dk, void* dv, int BH,
+                    int Nq, int Nk, int d, int kv_chunk, float scale, cudaStream_t stream) {
+  const long long R = (long long)BH * Nq;
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = launch_bwd_preprocess(o, dO, lse, D, lse2, dq_acc, R, d, scale, zero_dq, stream);
+  }
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  for (int c = 0; c < Nk / kv_chunk; ++c) {
+    Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
+    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, dq_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, kv_chunk, d, scale,
+                                    stream);
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  if (dq_bf16) {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = launch_dq_convert(dq_acc, dq_bf16, R * d, 1.0f, stream);
+    count_launch();
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  return RINGX_OK;
+}
+
 int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
                    void* dq, void* dk, void* dv, int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
                    void* workspace, size_t workspace_bytes, void* stream_) {
@@ -316,25 +344,104 @@ int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, c
   if ((st = check_arch()) != RINGX_OK) return st;
 
   tl_launches = 0;
-  const int BH = B * H;
-  const long long R = (long long)BH * N;
   const BwdWorkspace w = carve_bwd(workspace, B, H, N, d);
+  st = bwd_core(q, k, v, o, lse, dO, w.D, w.lse2, w.dq_acc, true, dq, dk, dv, B * H, N, N, d, kv_chunk, scale, stream);
+  if (st != RINGX_OK) return st;
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d) {
+  if (B <= 0 || H <= 0 || Nq <= 0 || (d != 64 && d != 128)) return 0;
+  return 2 * align_up((size_t)B * H * Nq * sizeof(float));
+}
+
+int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                           const void* dO, float* dq_acc, void* dk, void* dv, int B, int H, int Nq, int Nk, int d,
+                           float scale, int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o || !lse || !dO || !dq_acc || !dk || !dv) return RINGX_ERR_NULL_PTR;
+  if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
+  if (Nq % 128 || Nk % 128) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
+    return RINGX_ERR_BAD_SHAPE;
+  if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse) || !aligned16(dO) ||
+      !aligned16(dq_acc) || !aligned16(dk) || !aligned16(dv))
+    return RINGX_ERR_MISALIGNED;
+  const size_t need = ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d);
+  if (!workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < need) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  int st = check_arch();
+  if (st != RINGX_OK) return st;
+  tl_launches = 0;
+  float* D = static_cast<float*>(workspace);
+  float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + need / 2);
+  st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, stream);
+  if (st != RINGX_OK) return st;
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_dq_finalize(const float* dq_acc, void* dq, long long n, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (n < 0 || n % 4) return RINGX_ERR_BAD_SHAPE;
+  if (n == 0) { tl_last_launches = 0; return RINGX_OK; }
+  if (!dq_acc || !dq) return RINGX_ERR_NULL_PTR;
+  if (!aligned16(dq_acc) || (reinterpret_cast<uintptr_t>(dq) & 7u)) return RINGX_ERR_MISALIGNED;
+  tl_launches = 0;
   cudaError_t e;
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-    e = launch_bwd_preprocess(o, dO, lse, w.D, w.lse2, w.dq_acc, R, d, stream);
+    e = launch_dq_convert(dq_acc, dq, n, 1.0f, stream);
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
-  for (int c = 0; c < N / kv_chunk; ++c) {
-    Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
-    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, w.lse2, w.D, w.dq_acc, dk, dv, BH, N, c * kv_chunk, kv_chunk, d, scale,
-                                    stream);
-    if (e != cudaSuccess) return cuda_status(e);
-  }
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+static int check_eq5(const void* a, const void* b, const void* c, const void* d_, const void* e, long long rows, int d) {
+  if (rows < 0 || d < 8 || d > 1024 || d % 8) return RINGX_ERR_BAD_SHAPE;
+  if (rows == 0) return RINGX_OK;
+  if (!a || !b || !c || !d_ || !e) return RINGX_ERR_NULL_PTR;
+  return RINGX_OK;
+}
+
+int ringx_eq5_scale(const float* loc_out, const float* loc_lse, const float* lse_max, float* num, float* den,
+                    long long rows, int d, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int st = check_eq5(loc_out, loc_lse, lse_max, num, den, rows, d);
+  if (st != RINGX_OK) return st;
+  if (rows == 0) { tl_last_launches = 0; return RINGX_OK; }
+  if (!aligned16(loc_out) || !aligned16(num)) return RINGX_ERR_MISALIGNED;
+  tl_launches = 0;
+  cudaError_t e;
   {
-    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-    e = launch_dq_convert(w.dq_acc, dq, R * d, scale, stream);
+    Timed timed(RINGX_PROFILE_MERGE, stream);
+    e = launch_eq5_scale(loc_out, loc_lse, lse_max, num, den, rows, d, stream);
+  }
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_eq5_finalize(const float* num, const float* den, const float* lse_max, void* o_out, float* lse_out,
+                       long long rows, int d, int o_out_dtype, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (o_out_dtype != RINGX_F32 && o_out_dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  int st = check_eq5(num, den, lse_max, o_out, lse_out, rows, d);
+  if (st != RINGX_OK) return st;
+  if (rows == 0) { tl_last_launches = 0; return RINGX_OK; }
+  if (!aligned16(num) || !aligned16(o_out)) return RINGX_ERR_MISALIGNED;
+  tl_launches = 0;
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_MERGE, stream);
+    e = launch_eq5_finalize(num, den, lse_max, o_out, lse_out, rows, d, o_out_dtype, stream);
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
@@ -468,6 +575,6 @@ const char* ringx_status_string(int status) {
   }
 }
 
-int ringx_version(void) { return 100; }
+int ringx_version(void) { return 110; }
 
 }  // extern "C"

@@ -3,8 +3,8 @@
 // A CTA owns one 128-key tile (K_j, V_j) of one head and loops over all 128-row query tiles i of that head:
 //   S^T  = K_j Q_i^T                      P^T  = exp2(scale*log2e * S^T - lse2_i)   (P recomputed from the saved
 //   dP^T = V_j dO_i^T                     dS^T = P^T o (dP^T - D_i)                  *global* LSE; reading g8)
-//   dV_j += P^T dO_i      dK_j += dS^T Q_i      dQ_i += dS K_j                       (all unscaled; scale is applied
-// when dK is written here and when dQ is converted).  dK_j, dV_j live in TMEM for the whole loop and are written once
+//   dV_j += P^T dO_i      dK_j += dS^T Q_i      dQ_i += dS K_j                       (dS carries `scale`: phase B forms
+// scale*dP - scale*D_i with one FFMA2).  dK_j, dV_j live in TMEM for the whole loop and are written once
 // (atomic-free: the CTA owns the tile); dQ_i is reduce-added into the fp32 accumulator by TMA (cp.reduce.async.bulk) --
 // the single-GPU image of "the gradient for Q is accumulated ... over N steps".
 //
@@ -82,7 +82,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
                       const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_do,
                       const __grid_constant__ CUtensorMap map_dq, const float* __restrict__ lse2,
                       const float* __restrict__ Dvec,
-                      __nv_bfloat16* __restrict__ dk, __nv_bfloat16* __restrict__ dv, int N, int k_off,
+                      __nv_bfloat16* __restrict__ dk, __nv_bfloat16* __restrict__ dv, int N, int nk_stride, int k_off,
                       float scale_log2, float scale) {
   using Cfg = BwdCfg<kD>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -115,7 +115,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   const int bh = blockIdx.y;
   const int n_q = N / kTile;
   const int q_row0 = bh * N;                                  // rows of this head in the [BH*N, d] views
-  const int k_row0 = bh * N + k_off + blockIdx.x * kTile;
+  const int k_row0 = bh * nk_stride + k_off + blockIdx.x * kTile;   // rows in the [BH*nk_stride, d] views of K, V, dK, dV
 
   if (threadIdx.x == 0) {
     mbar_init(kv_full, 1);
@@ -306,6 +306,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     const uint32_t tDP = tmem + Cfg::tDP + lane_off + half * 64;
     uint8_t* ds_row = sDs + half * Cfg::kPanelBytes + row * 128;
     const float2 sc2 = make_float2(scale_log2, scale_log2);
+    const float2 scl2 = make_float2(scale, scale);               // dS^T carries `scale` (Dvec holds scale * D_i)
     int stage = 0, phase = 0;
     for (int i = 0; i < n_q; ++i) {
       const float4* stats = reinterpret_cast<const float4*>(sQ + stage * Cfg::kQStageBytes + Cfg::kTileBytes);
@@ -379,9 +380,9 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           float2 t[16];
 #pragma unroll
           for (int g = 0; g < 8; ++g) {
-            t[g * 2] = fadd2(make_float2(__uint_as_float(dp[g * 4 + 0]), __uint_as_float(dp[g * 4 + 1])),
+            t[g * 2] = ffma2(make_float2(__uint_as_float(dp[g * 4 + 0]), __uint_as_float(dp[g * 4 + 1])), scl2,
                              make_float2(-aux[g].x, -aux[g].y));
-            t[g * 2 + 1] = fadd2(make_float2(__uint_as_float(dp[g * 4 + 2]), __uint_as_float(dp[g * 4 + 3])),
+            t[g * 2 + 1] = ffma2(make_float2(__uint_as_float(dp[g * 4 + 2]), __uint_as_float(dp[g * 4 + 3])), scl2,
                                  make_float2(-aux[g].z, -aux[g].w));
           }
           if (c == 0) {
@@ -409,11 +410,10 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       if (threadIdx.x == 0) BTRACE(3, i);   // ds_full(i) arrived
       if (threadIdx.x == 0) { BADD(0, b1 - b0); BADD(1, b2 - b1); BADD(2, b3 - b2); BADD(3, BCLK() - b3); BADD(4, 1); }
     }
-    // ---- epilogue: dV_j (warps 0-3) and scale * dK_j (warps 4-7), bf16, written once
+    // ---- epilogue: dV_j (warps 0-3) and dK_j (warps 4-7), bf16, written once
     mbar_wait(dkv_full, 0);
     tc_fence_after();
     const uint32_t tSrc = tmem + (half == 0 ? Cfg::tDV : Cfg::tDK) + lane_off;
-    const float mul = half == 0 ? 1.0f : scale;
     __nv_bfloat16* dst_base = (half == 0 ? dv : dk) + (static_cast<size_t>(k_row0) + row) * kD;
 #pragma unroll
     for (int c = 0; c < kD / 32; ++c) {
@@ -424,10 +424,10 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 #pragma unroll
       for (int g = 0; g < 4; ++g) {
         uint4 u;
-        u.x = pack_bf16x2(__uint_as_float(r[g * 8 + 0]) * mul, __uint_as_float(r[g * 8 + 1]) * mul);
-        u.y = pack_bf16x2(__uint_as_float(r[g * 8 + 2]) * mul, __uint_as_float(r[g * 8 + 3]) * mul);
-        u.z = pack_bf16x2(__uint_as_float(r[g * 8 + 4]) * mul, __uint_as_float(r[g * 8 + 5]) * mul);
-        u.w = pack_bf16x2(__uint_as_float(r[g * 8 + 6]) * mul, __uint_as_float(r[g * 8 + 7]) * mul);
+        u.x = pack_bf16x2(__uint_as_float(r[g * 8 + 0]), __uint_as_float(r[g * 8 + 1]));
+        u.y = pack_bf16x2(__uint_as_float(r[g * 8 + 2]), __uint_as_float(r[g * 8 + 3]));
+        u.z = pack_bf16x2(__uint_as_float(r[g * 8 + 4]), __uint_as_float(r[g * 8 + 5]));
+        u.w = pack_bf16x2(__uint_as_float(r[g * 8 + 6]), __uint_as_float(r[g * 8 + 7]));
         dst[g] = u;
       }
     }
@@ -494,7 +494,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 template <int kD>
 cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
                      const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int BH, int N,
-                     int k_off, int nk, float scale, cudaStream_t stream) {
+                     int nk_stride, int k_off, int nk, float scale, cudaStream_t stream) {
   using Cfg = BwdCfg<kD>;
   auto kern = attn_chunk_bwd_kernel<kD>;
   static bool configured = false;
@@ -506,7 +506,7 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
   dim3 grid(nk / kTile, BH);
   kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D,
                                                        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv),
-                                                       N, k_off, scale * 1.4426950408889634f, scale);
+                                                       N, nk_stride, k_off, scale * 1.4426950408889634f, scale);
   count_launch();
   return cudaGetLastError();
 }
@@ -514,19 +514,19 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
 }  // namespace
 
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
-                                        const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
-                                        int nk, int d, float scale, cudaStream_t stream) {
+                                        const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
+                                        int nk_stride, int k_off, int nk, int d, float scale, cudaStream_t stream) {
   CUtensorMap mq, mk, mv, mdo, mdq;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
-  const uint64_t rows = (uint64_t)BH * N;
+  const uint64_t rows = (uint64_t)BH * N, krows = (uint64_t)BH * nk_stride;
   if (!make_tmap_2d(&mq, q, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mk, k, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mv, v, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mk, k, dt, 2, krows, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_2d(&mv, v, dt, 2, krows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mdq, dq_acc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, rows, d, 128, 32, kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, k_off, nk, scale, stream);
-  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, k_off, nk, scale, stream);
+  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, stream);
+  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, stream);
 }
 
 }  // namespace ringx

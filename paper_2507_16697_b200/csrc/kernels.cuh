@@ -14,8 +14,16 @@ namespace ringx {
 // ---- merge.cu (HBM-bound helpers)
 cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b, void* o_out,
                              float* lse_out, long long rows, int d, int in_dtype, int out_dtype, cudaStream_t stream);
+// Eq. 5 in its N-operand form: num = loc_out * exp(loc_lse - lse_max), den = exp(loc_lse -
+// lse_max) for one operand; o = num/den, lse = lse_max + ln(den) after the sums.  fp32 [rows,d] / [rows].
+cudaError_t launch_eq5_scale(const float* loc_out, const float* loc_lse, const float* lse_max, float* num, float* den,
+                             long long rows, int d, cudaStream_t stream);
+cudaError_t launch_eq5_finalize(const float* num, const float* den, const float* lse_max, void* o_out, float* lse_out,
+                                long long rows, int d, int out_dtype, cudaStream_t stream);
+// D = scale * rowsum(dO*O), lse2 = lse * log2(e); zeroes dq_acc when zero_dq.
 cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* lse, float* D, float* lse2,
-                                  float* dq_acc, long long rows, int d, cudaStream_t stream);
+                                  float* dq_acc, long long rows, int d, float scale, bool zero_dq,
+                                  cudaStream_t stream);
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
 
 // ---- attn_f32.cu (plain FFMA path, config C1)
@@ -31,12 +39,13 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
                                         int out_bf16, cudaStream_t stream);
 
 // ---- attn_bwd_sm100.cu (tcgen05 path)
-// One KV-chunk pass of the backward: writes dk,dv rows [k_off, k_off+nk) of every head (bf16),
-// reduce-adds this chunk's contribution into dq_acc (fp32 [BH,N,d], unscaled by `scale`).
-// lse2 = LSE * log2(e) and D = rowsum(dO*O) come from launch_bwd_preprocess.
+// One KV-chunk pass of the backward: q,dO [BH,N,d], k,v,dk,dv [BH,nk_stride,d]; writes dk,dv rows
+// [k_off, k_off+nk) of every head (bf16, the sum over the N query rows given), reduce-adds these keys'
+// contribution to dQ into dq_acc (fp32 [BH,N,d]).
+// lse2 = LSE * log2(e) and D = scale * rowsum(dO*O) come from launch_bwd_preprocess.
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
-                                        const float* D, float* dq_acc, void* dk, void* dv, int BH, int N, int k_off,
-                                        int nk, int d, float scale, cudaStream_t stream);
+                                        const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
+                                        int nk_stride, int k_off, int nk, int d, float scale, cudaStream_t stream);
 
 // ---- tensor maps (api.cu): 2-D row-major [rows, cols] view, box = {box_cols, box_rows}
 enum TmapSwizzle { kSwizzleNone = 0, kSwizzle128B = 1 };

@@ -2,6 +2,8 @@
 //   lse_merge_kernel   two-operand Eq. (5): SURVEY.md §8(a) row a5/a6
 //   bwd_preprocess     D_i = sum_c dO_ic O_ic, lse2_i = LSE_i log2(e), zeroing of the fp32 dQ accumulator: row a7
 //   dq_convert         dq = bf16(scale * dq_acc): row a9
+//   eq5_scale / eq5_finalize   Eq. (5) in its N-operand form (num, den before / after the cross-device sums;
+//                      PAPER.md:137-143): the RingX_a merge, SURVEY.md §8(f) NEXT-1
 // Roofline: HBM bandwidth.  Algorithmic bytes per row: merge 2*(d*e_in+4) read + (d*e_out+4)
 // written; preprocess 2*d*2 read + 4 written (+ d*4 zeroed); convert d*4 read + d*2 written.
 #include "kernels.cuh"
@@ -142,13 +144,58 @@ cudaError_t launch_merge_t(const void* o_a, const float* lse_a, const void* o_b,
   return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------- Eq. 5, N-operand form (RingX_a: PAPER.md:137-143)
+// One operand's share before the cross-device sums: w = exp(loc_lse - lse_max), num = w * loc_out, den = w.
+// lse_max is the all-reduce(max) of loc_lse over the devices; an operand with loc_lse = -inf (or a row whose
+// lse_max is -inf) contributes 0 and its loc_out is not read into the result.  One thread per float4.
+__global__ void __launch_bounds__(256)
+eq5_scale_kernel(const float4* __restrict__ loc_out, const float* __restrict__ loc_lse,
+                 const float* __restrict__ lse_max, float4* __restrict__ num, float* __restrict__ den, long long rows,
+                 int vecs) {
+  const long long total = rows * vecs, stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
+    const long long r = i / vecs;
+    const float l = loc_lse[r], m = lse_max[r];
+    const float w = (l == -INFINITY || m == -INFINITY) ? 0.f : expf(l - m);
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (w != 0.f) {
+      v = __ldcs(loc_out + i);
+      v.x *= w; v.y *= w; v.z *= w; v.w *= w;
+    }
+    __stcs(num + i, v);
+    if (i - r * vecs == 0) den[r] = w;
+  }
+}
+
+// After the sums: o = num / den, lse = lse_max + ln(den); den = 0 (every operand empty) gives o = 0, lse = -inf.
+template <typename TOut>
+__global__ void __launch_bounds__(256)
+eq5_finalize_kernel(const float4* __restrict__ num, const float* __restrict__ den, const float* __restrict__ lse_max,
+                    void* __restrict__ o_out, float* __restrict__ lse_out, long long rows, int vecs) {
+  const long long total = rows * vecs, stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
+    const long long r = i / vecs;
+    const float dn = den[r];
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (dn != 0.f) {
+      const float inv = 1.0f / dn;
+      v = __ldcs(num + i);
+      v.x *= inv; v.y *= inv; v.z *= inv; v.w *= inv;
+    }
+    Vec4<TOut>::store(o_out, (size_t)i, v);
+    if (i - r * vecs == 0) lse_out[r] = dn != 0.f ? lse_max[r] + logf(dn) : -INFINITY;   // NaN den propagates
+  }
+}
+
 // ---------------------------------------------------------------- backward helpers
 // D_i = sum_c dO_ic * O_ic (fp32), one 16-lane (d=64: 8 B/lane... ) group per row: each lane takes
-// 8 bf16 (16 B) of dO and of O; d/8 lanes per row.  Also zeroes the row of the fp32 dQ accumulator.
+// 8 bf16 (16 B) of dO and of O; d/8 lanes per row.  Stores scale * D_i; zeroes the row of the fp32 dQ accumulator
+// when zero_dq.
 template <int kLanes>
 __global__ void __launch_bounds__(256)
 bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO, const float* __restrict__ lse,
-                      float* __restrict__ D, float* __restrict__ lse2, float4* __restrict__ dq_acc, long long rows) {
+                      float* __restrict__ D, float* __restrict__ lse2, float4* __restrict__ dq_acc, long long rows,
+                      float scale, bool zero_dq) {
   constexpr int kRowsPerWarp = 32 / kLanes;
   const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
   const long long warp_global = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -175,14 +222,16 @@ bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO,
           s = fmaf(__uint_as_float(pa[i] << 16), __uint_as_float(pb[i] << 16), s);
           s = fmaf(__uint_as_float(pa[i] & 0xFFFF0000u), __uint_as_float(pb[i] & 0xFFFF0000u), s);
         }
-        const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-        dq_acc[(r * kLanes + l) * 2] = z;
-        dq_acc[(r * kLanes + l) * 2 + 1] = z;
+        if (zero_dq) {
+          const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+          dq_acc[(r * kLanes + l) * 2] = z;
+          dq_acc[(r * kLanes + l) * 2 + 1] = z;
+        }
       }
 #pragma unroll
       for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
       if (r < rows && l == 0) {
-        D[r] = s;
+        D[r] = s * scale;                          // phase B of the backward forms scale*dP - scale*D
         lse2[r] = lse[r] * 1.4426950408889634f;   // the backward kernel works in the exp2 domain
       }
     }
@@ -216,18 +265,45 @@ cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_
   return launch_merge_t<__nv_bfloat16, __nv_bfloat16>(o_a, lse_a, o_b, lse_b, o_out, lse_out, rows, d, stream);
 }
 
+static unsigned eq5_blocks(long long total) {
+  long long blocks = (total + 255) / 256;
+  if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
+  return (unsigned)(blocks < 1 ? 1 : blocks);
+}
+
+cudaError_t launch_eq5_scale(const float* loc_out, const float* loc_lse, const float* lse_max, float* num, float* den,
+                             long long rows, int d, cudaStream_t stream) {
+  if (rows == 0) return cudaSuccess;
+  eq5_scale_kernel<<<eq5_blocks(rows * (d / 4)), 256, 0, stream>>>((const float4*)loc_out, loc_lse, lse_max,
+                                                                  (float4*)num, den, rows, d / 4);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_eq5_finalize(const float* num, const float* den, const float* lse_max, void* o_out, float* lse_out,
+                                long long rows, int d, int out_dtype, cudaStream_t stream) {
+  if (rows == 0) return cudaSuccess;
+  if (out_dtype == RINGX_BF16)
+    eq5_finalize_kernel<__nv_bfloat16><<<eq5_blocks(rows * (d / 4)), 256, 0, stream>>>(
+        (const float4*)num, den, lse_max, o_out, lse_out, rows, d / 4);
+  else
+    eq5_finalize_kernel<float><<<eq5_blocks(rows * (d / 4)), 256, 0, stream>>>((const float4*)num, den, lse_max, o_out,
+                                                                                lse_out, rows, d / 4);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* lse, float* D, float* lse2,
-                                  float* dq_acc, long long rows, int d, cudaStream_t stream) {
+                                  float* dq_acc, long long rows, int d, float scale, bool zero_dq,
+                                  cudaStream_t stream) {
   const int lanes = d / 8;   // 8 or 16
   const long long rows_per_block = 8LL * (32 / lanes) * 4;
   long long blocks = (rows + rows_per_block - 1) / rows_per_block;
   if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
   if (lanes == 8)
     bwd_preprocess_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, lse, D, lse2,
-                                                                   (float4*)dq_acc, rows);
+                                                                   (float4*)dq_acc, rows, scale, zero_dq);
   else
     bwd_preprocess_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, lse, D, lse2,
-                                                                    (float4*)dq_acc, rows);
+                                                                    (float4*)dq_acc, rows, scale, zero_dq);
   return cudaGetLastError();
 }
 

@@ -48,6 +48,16 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_chunk_fwd.restype = c_i
     L.ringx_attn_fwd_bwd_host.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_fwd_bwd_host.restype = c_i
+    L.ringx_attn_bwd_partial.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_bwd_partial.restype = c_i
+    L.ringx_attn_bwd_partial_workspace_bytes.argtypes = [c_i] * 4
+    L.ringx_attn_bwd_partial_workspace_bytes.restype = c_sz
+    L.ringx_dq_finalize.argtypes = [c_p, c_p, c_ll, c_p]
+    L.ringx_dq_finalize.restype = c_i
+    L.ringx_eq5_scale.argtypes = [c_p] * 5 + [c_ll, c_i, c_p]
+    L.ringx_eq5_scale.restype = c_i
+    L.ringx_eq5_finalize.argtypes = [c_p] * 5 + [c_ll, c_i, c_i, c_p]
+    L.ringx_eq5_finalize.restype = c_i
     for name in ("ringx_attn_fwd_workspace_bytes", "ringx_attn_bwd_workspace_bytes",
                  "ringx_attn_fwd_host_workspace_bytes", "ringx_attn_fwd_bwd_host_workspace_bytes"):
         getattr(L, name).argtypes = [c_i] * 6
@@ -238,3 +248,58 @@ def ringx_profile_read() -> dict:
 
 def ringx_version() -> int:
     return lib().ringx_version()
+
+
+def ringx_attn_bwd_partial(q, k, v, o, lse, dO, scale: float, dq_acc=None, dk=None, dv=None, workspace=None):
+    """Per-device backward step (include/ringx.h: ringx_attn_bwd_partial): q,o,dO [B,H,Nq,d], k,v [B,H,Nk,d].
+    Adds these keys' contribution to dq_acc (fp32, allocated and zeroed when None); returns (dq_acc, dk, dv)."""
+    B, H, Nq, d = q.shape
+    Nk = k.shape[2]
+    if dq_acc is None:
+        dq_acc = torch.zeros((B, H, Nq, d), dtype=torch.float32, device=q.device)
+    dk = torch.empty_like(k) if dk is None else dk
+    dv = torch.empty_like(v) if dv is None else dv
+    need = lib().ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d)
+    if workspace is None:
+        workspace = _workspace(max(need, 256), q.device)
+    st = lib().ringx_attn_bwd_partial(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                                      _dev(dO, "dO"), _dev(dq_acc, "dq_acc"), _dev(dk, "dk"), _dev(dv, "dv"),
+                                      B, H, Nq, Nk, d, scale, _DTYPES[q.dtype], workspace.data_ptr(),
+                                      workspace.numel() * workspace.element_size(), _stream())
+    _check(st, "ringx_attn_bwd_partial")
+    return dq_acc, dk, dv
+
+
+def ringx_dq_finalize(dq_acc, dq=None):
+    """bf16 cast of the fp32 dQ accumulator (include/ringx.h: ringx_dq_finalize)."""
+    if dq is None:
+        dq = torch.empty(dq_acc.shape, dtype=torch.bfloat16, device=dq_acc.device)
+    _check(lib().ringx_dq_finalize(_dev(dq_acc, "dq_acc"), _dev(dq, "dq"), dq_acc.numel(), _stream()),
+           "ringx_dq_finalize")
+    return dq
+
+
+def ringx_eq5_scale(loc_out, loc_lse, lse_max, inplace: bool = False):
+    """(num, den) of one operand of the N-operand Eq. 5 (include/ringx.h: ringx_eq5_scale)."""
+    d = loc_out.shape[-1]
+    rows = loc_out.numel() // d
+    num = loc_out if inplace else torch.empty_like(loc_out)
+    den = torch.empty_like(loc_lse)
+    _check(lib().ringx_eq5_scale(_dev(loc_out, "loc_out"), _dev(loc_lse, "loc_lse"), _dev(lse_max, "lse_max"),
+                                 _dev(num, "num"), _dev(den, "den"), rows, d, _stream()), "ringx_eq5_scale")
+    return num, den
+
+
+def ringx_eq5_finalize(num, den, lse_max, out_dtype=torch.float32):
+    """o = num/den, lse = lse_max + log(den) (include/ringx.h: ringx_eq5_finalize)."""
+    d = num.shape[-1]
+    rows = num.numel() // d
+    o = torch.empty(num.shape, dtype=out_dtype, device=num.device)
+    lse = torch.empty_like(den)
+    _check(lib().ringx_eq5_finalize(_dev(num, "num"), _dev(den, "den"), _dev(lse_max, "lse_max"), _dev(o, "o"),
+                                    _dev(lse, "lse"), rows, d, _DTYPES[out_dtype], _stream()), "ringx_eq5_finalize")
+    return o, lse
+
+
+def ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d) -> int:
+    return lib().ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d)

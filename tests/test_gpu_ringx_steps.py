@@ -1,0 +1,299 @@
+"""GPU parity of the per-device RingX steps against the fp64 oracle:
+  ringx_attn_bwd_partial / ringx_dq_finalize  (Nq != Nk, global LSE)
+  ringx_eq5_scale / ringx_eq5_finalize        (Eq. 5 with N operands)
+and of the RingX_a / RingX_b schedules of ringx_dist with the real kernels: W ranks simulated on ONE GPU (threads,
+an in-process stand-in for the collectives -- the kernels of different ranks never wait on one another), plus the
+torch.distributed/NCCL path itself at world size 1."""
+import math
+import os
+import socket
+import threading
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import attention as orc
+from paper_2507_16697_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_GRAD = 2e-2      # BASELINE.json: gradients <= 2e-2 relative Frobenius
+TOL_LSE = 1e-3
+
+
+@pytest.fixture(scope="module")
+def rx():
+    from paper_2507_16697_b200 import ringx
+    from paper_2507_16697_b200.build import build_library
+    build_library()
+    assert torch.cuda.is_available(), "GPU tests need a B200"
+    ringx.lib()
+    return ringx
+
+
+def f64(t):
+    return wl.to_f64_numpy(t)
+
+
+def relf(a, ref):
+    return np.linalg.norm(a - ref) / np.linalg.norm(ref)
+
+
+# ------------------------------------------------------------------------------------------------ bwd_partial
+@pytest.mark.parametrize("d,Nq,chunks", [(64, 512, (512, 512)), (128, 256, (384, 640)), (64, 1024, (128, 256, 128)),
+                                         (128, 384, (1024,))])
+def test_bwd_partial_steps_add_up_to_the_oracle_gradient(rx, d, Nq, chunks):
+    """Nq query rows against Nk = sum(chunks) keys, one ringx_attn_bwd_partial call per key chunk (ragged chunk
+    sizes, Nq != Nk).  dq accumulates over the calls; each call's dk, dv are complete for its keys."""
+    B, H, Nk = 1, 3, sum(chunks)
+    scale = 1.0 / math.sqrt(d)
+    q = wl.make_tensor((B, H, Nq, d), "q", seed=71, dtype="bf16")
+    do = wl.make_tensor((B, H, Nq, d), "do", seed=71, dtype="bf16")
+    k = wl.make_tensor((B, H, Nk, d), "k", seed=71, dtype="bf16")
+    v = wl.make_tensor((B, H, Nk, d), "v", seed=71, dtype="bf16")
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    bounds = np.concatenate([[0], np.cumsum(chunks)])
+    q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+    o_ref, lse_ref = orc.attention_fwd_bhnd(q64, k64, v64, scale)
+    if Nq % 256 == 0 and len(chunks) >= 2:
+        # the saved global (o, lse) of these rows from the library itself: chunk partials + Eq. 5, bf16 at the end
+        parts = [rx.ringx_attn_chunk_fwd(qd, kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous(), scale)
+                 for lo, hi in zip(bounds[:-1], bounds[1:])]
+        o_acc, lse_acc = parts[0]
+        for i, (o_p, lse_p) in enumerate(parts[1:]):
+            last = i == len(parts) - 2
+            o_acc, lse_acc = rx.ringx_lse_merge(o_acc, lse_acc, o_p, lse_p,
+                                                out_dtype=torch.bfloat16 if last else torch.float32)
+        o_dev, lse_dev = o_acc, lse_acc
+        assert np.abs(lse_dev.cpu().double().numpy() - lse_ref).max() <= 5e-5
+    else:
+        # (the bf16 forward needs 256-row query tiles: here the saved (o, lse) are the oracle's, rounded as the
+        # forward would store them)
+        o_dev = torch.from_numpy(o_ref).to(torch.bfloat16).cuda()
+        lse_dev = torch.from_numpy(lse_ref).float().cuda()
+    dq_acc = torch.zeros((B, H, Nq, d), dtype=torch.float32, device="cuda")
+    dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
+    for lo, hi in zip(bounds[:-1], bounds[1:]):
+        _, dk, dv = rx.ringx_attn_bwd_partial(qd, kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous(), o_dev,
+                                              lse_dev, dod, scale, dq_acc=dq_acc)
+        assert rx.ringx_last_launch_count() == 2           # preprocess + one chunk kernel
+        assert relf(f64(dk), dk_ref[:, :, lo:hi]) <= TOL_GRAD
+        assert relf(f64(dv), dv_ref[:, :, lo:hi]) <= TOL_GRAD
+        assert relf(f64(dk), dk_ref[:, :, lo:hi]) <= 6e-3 and relf(f64(dv), dv_ref[:, :, lo:hi]) <= 6e-3
+    dq = rx.ringx_dq_finalize(dq_acc)
+    assert dq.dtype == torch.bfloat16
+    assert relf(f64(dq), dq_ref) <= 6e-3
+    # the accumulator itself holds the true gradient (scale included), before the bf16 rounding
+    assert relf(dq_acc.cpu().double().numpy(), dq_ref) <= 6e-3
+
+
+def test_bwd_partial_equals_full_backward_when_it_sees_everything(rx):
+    """With Nq == Nk and one call, ringx_attn_bwd_partial + ringx_dq_finalize is ringx_attn_bwd (same kernels)."""
+    B, H, N, d = 1, 2, 1024, 128
+    scale = 1.0 / math.sqrt(d)
+    q, k, v, do = (t.cuda() for t in wl.make_qkv((B, H, N, d), with_do=True, seed=5, dtype="bf16"))
+    o, lse = rx.ringx_attn_fwd(q, k, v, N, scale)
+    dq, dk, dv = rx.ringx_attn_bwd(q, k, v, o, lse, do, N, scale)
+    dq_acc, dk2, dv2 = rx.ringx_attn_bwd_partial(q, k, v, o, lse, do, scale)
+    assert torch.equal(dk, dk2) and torch.equal(dv, dv2)        # atomic-free: bit-reproducible
+    dq2 = rx.ringx_dq_finalize(dq_acc)
+    assert relf(f64(dq2), f64(dq)) <= 1e-3                      # dQ: reduce-add order differs between runs
+
+
+def test_bwd_partial_rejects_bad_arguments(rx):
+    L = rx.lib()
+    t = torch.zeros(1, 1, 256, 64, dtype=torch.bfloat16, device="cuda")
+    lse = torch.zeros(1, 1, 256, device="cuda")
+    acc = torch.zeros(1, 1, 256, 64, device="cuda")
+    ws = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    p = [x.data_ptr() for x in (t, t, t, t, lse, t, acc, t, t)]
+    call = lambda Nq, Nk, d, dt, wsb: L.ringx_attn_bwd_partial(*p, 1, 1, Nq, Nk, d, 0.125, dt, ws.data_ptr(), wsb, None)
+    assert call(256, 256, 64, 1, 4096) == 0
+    assert call(200, 256, 64, 1, 4096) == 2       # BAD_SHAPE
+    assert call(256, 100, 64, 1, 4096) == 2
+    assert call(256, 256, 96, 1, 4096) == 2
+    assert call(256, 256, 64, 0, 4096) == 3       # BAD_DTYPE: bf16 only
+    assert call(256, 256, 64, 1, 16) == 5         # WORKSPACE_TOO_SMALL
+    torch.cuda.synchronize()
+
+
+# ------------------------------------------------------------------------------------------------ Eq. 5, N operands
+@pytest.mark.parametrize("rows,d,n_ops", [(1, 8, 2), (777, 64, 3), (4099, 128, 5), (130, 1024, 4)])
+def test_eq5_scale_and_finalize_match_oracle(rx, rows, d, n_ops):
+    g = torch.Generator().manual_seed(rows + d + n_ops)
+    outs = [torch.randn(rows, d, generator=g) for _ in range(n_ops)]
+    lses = [torch.randn(rows, generator=g) * 6 for _ in range(n_ops)]
+    lses[0][::7] = -math.inf                       # an empty chunk on some rows: weight 0, its loc_out ignored
+    outs[0][::7] = math.nan
+    if rows > 20:
+        for l in lses:
+            l[13] = -math.inf                      # a row with every operand empty: o = 0, lse = -inf
+    lse_max = torch.stack(lses).max(dim=0).values.cuda()         # the all-reduce(max) of the schedule
+    num = torch.zeros(rows, d, device="cuda")
+    den = torch.zeros(rows, device="cuda")
+    for o_i, l_i in zip(outs, lses):
+        n_i, d_i = rx.ringx_eq5_scale(o_i.cuda(), l_i.cuda(), lse_max)
+        num += n_i                                  # the reduce(num, den) of the schedule
+        den += d_i
+    # (the oracle multiplies by the zero weight, so the garbage behind an empty chunk is zeroed for it: reading g12)
+    o_ref, lse_ref = orc.merge_partials([np.nan_to_num(f64(o), nan=0.0) for o in outs], [f64(l) for l in lses])
+    for out_dtype, tol in ((torch.float32, 2e-6), (torch.bfloat16, 4e-3)):
+        o, lse = rx.ringx_eq5_finalize(num, den, lse_max, out_dtype=out_dtype)
+        og, lg = f64(o), f64(lse)
+        assert np.isfinite(og).all()
+        assert np.abs(og - o_ref).max() <= tol * max(1.0, np.abs(o_ref).max())
+        fin = np.isfinite(lse_ref)
+        assert (lg[~fin] == lse_ref[~fin]).all()
+        assert np.abs(lg[fin] - lse_ref[fin]).max() <= 2e-6 * max(1.0, np.abs(lse_ref[fin]).max())
+    # in place on loc_out
+    a = outs[1].cuda()
+    n_i, _ = rx.ringx_eq5_scale(a, lses[1].cuda(), lse_max, inplace=True)
+    assert n_i.data_ptr() == a.data_ptr()
+    assert rx.lib().ringx_eq5_scale(None, None, None, None, None, 0, 64, None) == 0      # rows == 0: no-op
+
+
+# ------------------------------------------------------------------------------------------------ schedules, W ranks
+class ThreadComm:
+    """In-process stand-in for ringx_dist.TorchComm: W threads = W simulated ranks sharing one GPU and one stream.
+    Every collective is "publish, barrier, combine, barrier"; combining uses plain torch copies/sums (the collectives
+    are not part of the method's arithmetic; NCCL does the same sums in the same dtypes)."""
+
+    class _Shared:
+        def __init__(self, world):
+            self.world = world
+            self.barrier = threading.Barrier(world)
+            self.slots = [None] * world
+
+    class _Done:
+        def wait(self):
+            return None
+
+    def __init__(self, shared, rank):
+        self.sh, self.rank, self.world = shared, rank, shared.world
+
+    def _exchange(self, t):
+        self.sh.slots[self.rank] = t
+        self.sh.barrier.wait()
+        return list(self.sh.slots)
+
+    def _finish(self):
+        self.sh.barrier.wait()
+        return self._Done()
+
+    def broadcast(self, t, src):
+        got = self._exchange(t)
+        if self.rank != src:
+            t.copy_(got[src])
+        return self._finish()
+
+    def all_reduce_max(self, t):
+        got = self._exchange(t.clone())
+        t.copy_(torch.stack(got).max(dim=0).values)
+        return self._finish()
+
+    def reduce_sum(self, t, dst):
+        got = self._exchange(t.clone())
+        if self.rank == dst:
+            t.copy_(torch.stack(got).float().sum(dim=0))
+        return self._finish()
+
+    def all_gather(self, stacked, t):
+        got = self._exchange(t)
+        for i, g in enumerate(got):
+            stacked[i].copy_(g)
+        return self._finish()
+
+    def reduce_scatter_sum(self, out, stacked):
+        got = self._exchange(stacked)
+        out.copy_(torch.stack([g[self.rank] for g in got]).float().sum(dim=0))
+        return self._finish()
+
+
+@pytest.mark.parametrize("variant", ["a", "b"])
+@pytest.mark.parametrize("world,d,Nl", [(2, 128, 512), (4, 64, 256)])
+def test_ringx_schedules_on_simulated_ranks(rx, variant, world, d, Nl):
+    """RingX_a / RingX_b forward + backward with the real kernels, W sequence chunks of Nl tokens, against the
+    oracle attention of the whole sequence and against the library's own single-device ringx_attn_fwd/bwd."""
+    from paper_2507_16697_b200 import ringx_dist
+    B, H, N = 1, 2, world * Nl
+    scale = 1.0 / math.sqrt(d)
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=23 + world, dtype="bf16")
+    fwd, bwd = ((ringx_dist.ringx_a_forward, ringx_dist.ringx_a_backward) if variant == "a" else
+                (ringx_dist.ringx_b_forward, ringx_dist.ringx_b_backward))
+    shared = ThreadComm._Shared(world)
+    results, errors = [None] * world, []
+
+    def rank_main(r):
+        try:
+            torch.cuda.set_device(0)
+            comm = ThreadComm(shared, r)
+            sl = slice(r * Nl, (r + 1) * Nl)
+            ql, kl, vl, dol = (t[:, :, sl].contiguous().cuda() for t in (q, k, v, do))
+            o, lse, ctx = fwd(ql, kl, vl, scale, comm=comm)
+            dq, dk, dv = bwd(ctx, dol, comm=comm)
+            torch.cuda.synchronize()
+            results[r] = [t.cpu() for t in (o, lse, dq, dk, dv)]
+        except Exception as e:                      # noqa: BLE001 -- surface it in the main thread
+            errors.append(e)
+            shared.barrier.abort()
+
+    threads = [threading.Thread(target=rank_main, args=(r,)) for r in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+    assert not errors, errors
+    q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+    o_ref, lse_ref = orc.attention_fwd_bhnd(q64, k64, v64, scale)
+    dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
+    for r in range(world):
+        sl = slice(r * Nl, (r + 1) * Nl)
+        o, lse, dq, dk, dv = results[r]
+        assert o.dtype == torch.bfloat16 and dq.dtype == torch.bfloat16
+        assert np.abs(f64(o) - o_ref[:, :, sl]).max() <= 1e-2 * np.abs(v64).max()
+        assert relf(f64(o), o_ref[:, :, sl]) <= 1e-2
+        assert np.abs(f64(lse) - lse_ref[:, :, sl]).max() <= 5e-5
+        for g, ref in ((dq, dq_ref), (dk, dk_ref), (dv, dv_ref)):
+            e = relf(f64(g), ref[:, :, sl])
+            assert e <= TOL_GRAD and e <= 8e-3, e
+
+
+def test_ringx_dist_over_nccl_world_size_one(rx):
+    """The torch.distributed path itself (backend nccl, one rank on the one GPU): both schedules reduce to the
+    single-device library calls."""
+    import torch.distributed as dist
+    from paper_2507_16697_b200 import ringx_dist
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK="0", WORLD_SIZE="1")
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        B, H, N, d = 1, 2, 512, 64
+        scale = 1.0 / math.sqrt(d)
+        q, k, v, do = (t.cuda() for t in wl.make_qkv((B, H, N, d), with_do=True, seed=9, dtype="bf16"))
+        o_ref, lse_ref = rx.ringx_attn_fwd(q, k, v, N, scale)
+        for fwd, bwd in ((ringx_dist.ringx_a_forward, ringx_dist.ringx_a_backward),
+                         (ringx_dist.ringx_b_forward, ringx_dist.ringx_b_backward)):
+            o, lse, ctx = fwd(q, k, v, scale)
+            dq, dk, dv = bwd(ctx, do)
+            assert torch.equal(o, o_ref) and torch.equal(lse, lse_ref)
+            dq_r, dk_r, dv_r = rx.ringx_attn_bwd(q, k, v, o, lse, do, N, scale)
+            assert torch.equal(dk, dk_r) and torch.equal(dv, dv_r)
+            assert relf(f64(dq), f64(dq_r)) <= 1e-3
+        # the collectives themselves, on the one rank
+        comm = ringx_dist.TorchComm()
+        t = torch.arange(8, dtype=torch.float32, device="cuda")
+        st = torch.zeros(1, 8, device="cuda")
+        comm.all_gather(st, t).wait()
+        comm.all_reduce_max(t).wait()
+        comm.reduce_sum(t, 0).wait()
+        comm.broadcast(t, 0).wait()
+        out = torch.zeros(8, device="cuda")
+        comm.reduce_scatter_sum(out, st).wait()
+        torch.cuda.synchronize()
+        assert torch.equal(out, t) and torch.equal(st[0], t)
+    finally:
+        dist.destroy_process_group()

@@ -291,6 +291,31 @@ def test_row_and_column_sampled_backward_are_exact():
     np.testing.assert_allclose(dv_c, dv[cols], atol=1e-13)
 
 
+def test_partial_backward_steps_add_up_to_the_gradient():
+    """attention_bwd_partial (one device's step of the RingX backward) against the pinned full
+    gradient: dQ shares over any partition of the keys sum to dQ; dK/dV of a key subset from a partition of the
+    query rows sum to those rows of dK/dV; and against finite differences directly (ragged 2 x 3 grid of blocks)."""
+    q, k, v, dO = rnd(7, 3), rnd(11, 3), rnd(11, 4), rnd(7, 4)
+    sc = 0.45
+    lse, D = orc.row_stats(q, k, v, dO, sc)
+    fd_q = finite_diff(lambda x: loss(x, k, v, dO, sc), q)
+    fd_k = finite_diff(lambda x: loss(q, x, v, dO, sc), k)
+    fd_v = finite_diff(lambda x: loss(q, k, x, dO, sc), v)
+    dq, dk, dv = np.zeros_like(q), np.zeros_like(k), np.zeros_like(v)
+    for r0, r1 in ((0, 3), (3, 7)):                       # two "devices" holding query rows
+        for c0, c1 in ((0, 1), (1, 6), (6, 11)):          # three key chunks (ragged)
+            a, b, c = orc.attention_bwd_partial(q[r0:r1], k[c0:c1], v[c0:c1], dO[r0:r1], lse[r0:r1], D[r0:r1], sc)
+            dq[r0:r1] += a
+            dk[c0:c1] += b
+            dv[c0:c1] += c
+    for got, fd in ((dq, fd_q), (dk, fd_k), (dv, fd_v)):
+        assert np.abs(got - fd).max() <= 1e-8 * max(1.0, np.abs(fd).max())
+    full = orc.attention_bwd(q, k, v, dO, sc)
+    for got, ref in zip((dq, dk, dv), full):
+        np.testing.assert_allclose(got, ref, atol=1e-13)
+    # a transposed operand would survive neither: shapes differ (Nq != Nk, d != dv)
+
+
 # ------------------------------------------------------------------ library second opinion
 def test_against_torch_fp64():
     q, k, v, dO = rnd(40, 16), rnd(70, 16), rnd(70, 16), rnd(40, 16)
