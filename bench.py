@@ -352,7 +352,7 @@ def main():
     # ---------------------------------------------------------------- short side measurements (not the metric)
     extra = {}
     if rank == 0 and not args.no_extra:
-        for name in ("C2", "C4"):
+        for name in ("C2", "C4", "C5"):
             if name == cfg.name:
                 continue
             extra[name] = side_measure(ringx, wl, wl.CONFIGS[name], dev)
