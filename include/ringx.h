@@ -90,6 +90,20 @@ RINGX_API int ringx_attn_bwd(const void* q, const void* k, const void* v, const 
                    int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
                    void* workspace, size_t workspace_bytes, void* stream);
 
+/* Grouped-query attention (the paper names MHA / GQA / MLA layers as compatible, l.376): `Hq` query heads share
+ * `Hkv` key/value heads, Hq % Hkv == 0, query head h attends kv head h / (Hq/Hkv).
+ *   q, o, dO, dq [B,Hq,N,d]; lse [B,Hq,N]; k, v, dk, dv [B,Hkv,N,d].  Everything else as ringx_attn_fwd /
+ *   ringx_attn_bwd, whose workspace queries (with H = Hq) size the workspace.  Hq == Hkv is exactly those calls.
+ * No extra kernels: the Hq/Hkv heads of a group are adjacent in memory, i.e. (Hq/Hkv)*N query rows against N keys;
+ * in the backward the CTA that owns a key tile walks all of them, so dk, dv are still written once, atomic-free. */
+RINGX_API int ringx_attn_fwd_gqa(const void* q, const void* k, const void* v, void* o, float* lse,
+                       int B, int Hq, int Hkv, int N, int d, int kv_chunk, float scale, int dtype,
+                       void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                       const void* dO, void* dq, void* dk, void* dv,
+                       int B, int Hq, int Hkv, int N, int d, int kv_chunk, float scale, int dtype,
+                       void* workspace, size_t workspace_bytes, void* stream);
+
 /* Two-operand Eq. 5, row by row:  m = max(lse_a,lse_b); w_a = exp(lse_a-m); w_b = exp(lse_b-m);
  * o_out = (w_a o_a + w_b o_b)/(w_a+w_b);  lse_out = m + log(w_a+w_b).
  * An operand with lse = -inf has weight 0; both -inf gives o_out = 0, lse_out = -inf; NaN propagates.

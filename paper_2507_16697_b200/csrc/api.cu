@@ -204,38 +204,23 @@ size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_ch
   return 4 * align_up(R * d * e) + align_up(R * sizeof(float)) + carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype).bytes;
 }
 
-int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* lse, int B, int H, int N, int d,
-                   int kv_chunk, float scale, int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
-  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-  if (!q || !k || !v || !o || !lse) return RINGX_ERR_NULL_PTR;
-  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false);
-  if (st != RINGX_OK) return st;
-  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse)) return RINGX_ERR_MISALIGNED;
-  const FwdWorkspace need = carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype);
-  if (need.bytes) {
-    if (!workspace) return RINGX_ERR_NULL_PTR;
-    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
-    if (workspace_bytes < need.bytes) return RINGX_ERR_WORKSPACE_TOO_SMALL;
-  }
-  if ((st = check_arch()) != RINGX_OK) return st;
-
-  tl_launches = 0;
-  const int BH = B * H;
-  const long long R = (long long)BH * N;
+// Shared forward driver.  q,o: Nq rows per (batch, kv head); k,v: N rows per (batch, kv head); Nq = G*N with G query
+// heads per kv head (G = 1: plain multi-head attention) -- the G heads that share a K,V head are adjacent in memory,
+// so they are simply G*N query rows of one [BH, Nq, d] problem.
+static int fwd_core(const void* q, const void* k, const void* v, void* o, float* lse, int BH, int Nq, int N, int d,
+                    int kv_chunk, float scale, int dtype, const FwdWorkspace& w, cudaStream_t stream) {
+  const long long R = (long long)BH * Nq;
   const int n_chunks = N / kv_chunk;
   if (n_chunks == 1) {
-    cudaError_t e = chunk_pass(q, k, v, o, lse, BH, N, N, 0, N, d, scale, dtype, true, stream);
-    if (e != cudaSuccess) return cuda_status(e);
-    tl_last_launches = tl_launches;
-    return RINGX_OK;
+    cudaError_t e = chunk_pass(q, k, v, o, lse, BH, Nq, N, 0, N, d, scale, dtype, true, stream);
+    return e == cudaSuccess ? RINGX_OK : cuda_status(e);
   }
-  const FwdWorkspace w = carve_fwd(workspace, B, H, N, d, kv_chunk, dtype);
   // running accumulator: fp32 for both dtypes (f32 accumulates straight into the caller's o/lse)
   float* o_acc = dtype == RINGX_F32 ? static_cast<float*>(o) : w.o_acc;
   float* lse_acc = dtype == RINGX_F32 ? lse : w.lse_acc;
   for (int c = 0; c < n_chunks; ++c) {
     const bool first = c == 0, last = c == n_chunks - 1;
-    cudaError_t e = chunk_pass(q, k, v, first ? o_acc : w.o_part, first ? lse_acc : w.lse_part, BH, N, N,
+    cudaError_t e = chunk_pass(q, k, v, first ? o_acc : w.o_part, first ? lse_acc : w.lse_part, BH, Nq, N,
                                c * kv_chunk, kv_chunk, d, scale, dtype, false, stream);
     if (e != cudaSuccess) return cuda_status(e);
     if (first) continue;
@@ -247,8 +232,42 @@ int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* 
     count_launch();
     if (e != cudaSuccess) return cuda_status(e);
   }
+  return RINGX_OK;
+}
+
+static int check_gqa(int Hq, int Hkv) {
+  if (Hq <= 0 || Hkv <= 0 || Hq % Hkv) return RINGX_ERR_BAD_SHAPE;
+  return RINGX_OK;
+}
+
+int ringx_attn_fwd_gqa(const void* q, const void* k, const void* v, void* o, float* lse, int B, int Hq, int Hkv, int N,
+                       int d, int kv_chunk, float scale, int dtype, void* workspace, size_t workspace_bytes,
+                       void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o || !lse) return RINGX_ERR_NULL_PTR;
+  int st = check_gqa(Hq, Hkv);
+  if (st == RINGX_OK) st = check_shape(B, Hq, N, d, kv_chunk, scale, dtype, false);
+  if (st != RINGX_OK) return st;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse)) return RINGX_ERR_MISALIGNED;
+  const FwdWorkspace need = carve_fwd(nullptr, B, Hq, N, d, kv_chunk, dtype);
+  if (need.bytes) {
+    if (!workspace) return RINGX_ERR_NULL_PTR;
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+    if (workspace_bytes < need.bytes) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  }
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  const int G = Hq / Hkv;
+  st = fwd_core(q, k, v, o, lse, B * Hkv, G * N, N, d, kv_chunk, scale, dtype,
+                carve_fwd(workspace, B, Hq, N, d, kv_chunk, dtype), stream);
+  if (st != RINGX_OK) return st;
   tl_last_launches = tl_launches;
   return RINGX_OK;
+}
+
+int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* lse, int B, int H, int N, int d,
+                   int kv_chunk, float scale, int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
+  return ringx_attn_fwd_gqa(q, k, v, o, lse, B, H, H, N, d, kv_chunk, scale, dtype, workspace, workspace_bytes, stream_);
 }
 
 int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse, int B, int H,
@@ -327,28 +346,40 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
   return RINGX_OK;
 }
 
-int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
-                   void* dq, void* dk, void* dv, int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
-                   void* workspace, size_t workspace_bytes, void* stream_) {
+int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
+                       void* dq, void* dk, void* dv, int B, int Hq, int Hkv, int N, int d, int kv_chunk, float scale,
+                       int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!q || !k || !v || !o || !lse || !dO || !dq || !dk || !dv) return RINGX_ERR_NULL_PTR;
-  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, true);
+  int st = check_gqa(Hq, Hkv);
+  if (st == RINGX_OK) st = check_shape(B, Hq, N, d, kv_chunk, scale, dtype, true);
   if (st != RINGX_OK) return st;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse) || !aligned16(dO) ||
       !aligned16(dq) || !aligned16(dk) || !aligned16(dv))
     return RINGX_ERR_MISALIGNED;
-  const BwdWorkspace need = carve_bwd(nullptr, B, H, N, d);
+  const BwdWorkspace need = carve_bwd(nullptr, B, Hq, N, d);
   if (!workspace) return RINGX_ERR_NULL_PTR;
   if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
   if (workspace_bytes < need.bytes) return RINGX_ERR_WORKSPACE_TOO_SMALL;
   if ((st = check_arch()) != RINGX_OK) return st;
 
   tl_launches = 0;
-  const BwdWorkspace w = carve_bwd(workspace, B, H, N, d);
-  st = bwd_core(q, k, v, o, lse, dO, w.D, w.lse2, w.dq_acc, true, dq, dk, dv, B * H, N, N, d, kv_chunk, scale, stream);
+  const BwdWorkspace w = carve_bwd(workspace, B, Hq, N, d);
+  // the G = Hq/Hkv query heads of a kv head are G*N adjacent query rows: the CTA that owns a key tile walks all of them,
+  // so dK, dV of the kv head are still written once, atomic-free
+  const int G = Hq / Hkv;
+  st = bwd_core(q, k, v, o, lse, dO, w.D, w.lse2, w.dq_acc, true, dq, dk, dv, B * Hkv, G * N, N, d, kv_chunk, scale,
+                stream);
   if (st != RINGX_OK) return st;
   tl_last_launches = tl_launches;
   return RINGX_OK;
+}
+
+int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
+                   void* dq, void* dk, void* dv, int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
+                   void* workspace, size_t workspace_bytes, void* stream_) {
+  return ringx_attn_bwd_gqa(q, k, v, o, lse, dO, dq, dk, dv, B, H, H, N, d, kv_chunk, scale, dtype, workspace,
+                            workspace_bytes, stream_);
 }
 
 size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d) {

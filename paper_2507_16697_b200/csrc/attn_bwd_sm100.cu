@@ -73,6 +73,11 @@ struct BwdCfg {
                                     kDsBytes + 2 * kDqPanelBytes + 256;
   static constexpr uint32_t tS = 0, tDP = 128, tDV = 256, tDK = 256 + kD, tDQ = kD == 64 ? 384 : 128;
   static constexpr bool kDqOverlaysDp = kD != 64;
+  // d = 64 leaves 64 TMEM columns: K_j and V_j (bf16, 32 columns each) are copied there once and serve as the A operands
+  // of S^T = K Q^T and dP^T = V dO^T, and dS^T (bf16) is also written over the dP^T columns as the A operand of dK +=
+  // dS^T Q.  The SM's shared memory (128 B/clk, which the SS MMAs saturate) then carries 64 KB less per step.
+  static constexpr bool kTmemOperands = kD == 64;
+  static constexpr uint32_t tK = 448, tV = 480;
   static constexpr unsigned kPolyMask = kD == 64 ? RINGX_BWD_POLY_MASK_D64 : RINGX_BWD_POLY_MASK_D128;
 };
 
@@ -108,7 +113,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   uint64_t* q_empty = q_full + Cfg::kQStages;
   uint64_t* do_full = q_empty + Cfg::kQStages;     // [kDoStages]
   uint64_t* do_empty = do_full + Cfg::kDoStages;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(do_empty + Cfg::kDoStages);
+  uint64_t* kv_tmem_full = do_empty + Cfg::kDoStages;   // compute -> MMA: K_j, V_j copied to TMEM     (256 arrivals)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(kv_tmem_full + 1);
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   const int lane = threadIdx.x & 31;
@@ -127,6 +133,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     mbar_init(dq_full, 1);
     mbar_init(dq_empty, 128);
     mbar_init(dkv_full, 1);
+    mbar_init(kv_tmem_full, 256);
     for (int i = 0; i < Cfg::kQStages; ++i) {
       mbar_init(&q_full[i], 1);
       mbar_init(&q_empty[i], 1);
@@ -224,7 +231,10 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     auto issue_st = [&](uint32_t q_addr) {
       if (leader) {
 #pragma unroll
-        for (int k = 0; k < kD / 16; ++k) mma_ss(tmem + Cfg::tS, kmajor(k_addr, k), kmajor(q_addr, k), idesc_st, k > 0);
+        for (int k = 0; k < kD / 16; ++k) {
+          if (Cfg::kTmemOperands) mma_ts(tmem + Cfg::tS, tmem + Cfg::tK + k * 8, kmajor(q_addr, k), idesc_st, k > 0);
+          else mma_ss(tmem + Cfg::tS, kmajor(k_addr, k), kmajor(q_addr, k), idesc_st, k > 0);
+        }
         mma_commit(s_full);
       }
       __syncwarp();
@@ -232,12 +242,16 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     auto issue_dpt = [&](uint32_t do_addr) {
       if (leader) {
 #pragma unroll
-        for (int k = 0; k < kD / 16; ++k) mma_ss(tmem + Cfg::tDP, kmajor(v_addr, k), kmajor(do_addr, k), idesc_st, k > 0);
+        for (int k = 0; k < kD / 16; ++k) {
+          if (Cfg::kTmemOperands) mma_ts(tmem + Cfg::tDP, tmem + Cfg::tV + k * 8, kmajor(do_addr, k), idesc_st, k > 0);
+          else mma_ss(tmem + Cfg::tDP, kmajor(v_addr, k), kmajor(do_addr, k), idesc_st, k > 0);
+        }
         mma_commit(dp_full);
       }
       __syncwarp();
     };
     mbar_wait(kv_full, 0);
+    if (Cfg::kTmemOperands) mbar_wait(kv_tmem_full, 0);
     mbar_wait(&q_full[0], 0);
     tc_fence_after();
     issue_st(q_base);
@@ -281,7 +295,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         mma_commit(dq_full);
 #pragma unroll
         for (int k = 0; k < kTile / 16; ++k)
-          mma_ss(tmem + Cfg::tDK, kmajor(ds_addr, k), mnmajor(q_addr, k), idesc_kn, i > 0 || k > 0);
+          if (Cfg::kTmemOperands)
+            mma_ts(tmem + Cfg::tDK, tmem + Cfg::tDP + (k >> 2) * 64 + (k & 3) * 8, mnmajor(q_addr, k), idesc_kn,
+                   i > 0 || k > 0);
+          else
+            mma_ss(tmem + Cfg::tDK, kmajor(ds_addr, k), mnmajor(q_addr, k), idesc_kn, i > 0 || k > 0);
         mma_commit(ds_empty);
         mma_commit(&q_empty[cur_qs]);
       }
@@ -307,6 +325,24 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     uint8_t* ds_row = sDs + half * Cfg::kPanelBytes + row * 128;
     const float2 sc2 = make_float2(scale_log2, scale_log2);
     const float2 scl2 = make_float2(scale, scale);               // dS^T carries `scale` (Dvec holds scale * D_i)
+    if (Cfg::kTmemOperands) {
+      // K_j (warps 0-3) / V_j (warps 4-7): my row of the 128B-swizzled tile -> my TMEM lane (2 bf16 per column)
+      mbar_wait(kv_full, 0);
+      const uint8_t* src = (half == 0 ? sK : sV) + row * 128;
+      uint32_t kvr[32];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        const float4 x = ld_shared_v4(src + ((c ^ (row & 7)) << 4));
+        kvr[c * 4 + 0] = __float_as_uint(x.x);
+        kvr[c * 4 + 1] = __float_as_uint(x.y);
+        kvr[c * 4 + 2] = __float_as_uint(x.z);
+        kvr[c * 4 + 3] = __float_as_uint(x.w);
+      }
+      tmem_st_x32(tmem + (half == 0 ? Cfg::tK : Cfg::tV) + lane_off, kvr);
+      tmem_wait_st();
+      tc_fence_before();
+      mbar_arrive(kv_tmem_full);
+    }
     int stage = 0, phase = 0;
     for (int i = 0; i < n_q; ++i) {
       const float4* stats = reinterpret_cast<const float4*>(sQ + stage * Cfg::kQStageBytes + Cfg::kTileBytes);
@@ -378,6 +414,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         tmem_ld_x32(tDP + 32, dp1);
         auto half_b = [&](const uint32_t (&dp)[32], int c) {
           float2 t[16];
+          uint32_t dsk[16];
 #pragma unroll
           for (int g = 0; g < 8; ++g) {
             t[g * 2] = ffma2(make_float2(__uint_as_float(dp[g * 4 + 0]), __uint_as_float(dp[g * 4 + 1])), scl2,
@@ -395,9 +432,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
             const float2 w0 = fmul2(p[c * 16 + e + 0], t[e + 0]), w1 = fmul2(p[c * 16 + e + 1], t[e + 1]);
             const float2 w2 = fmul2(p[c * 16 + e + 2], t[e + 2]), w3 = fmul2(p[c * 16 + e + 3], t[e + 3]);
             const int chunk = c * 4 + g;
-            st_shared_v4(ds_row + ((chunk ^ (row & 7)) << 4), pack_bf16x2(w0.x, w0.y), pack_bf16x2(w1.x, w1.y),
-                         pack_bf16x2(w2.x, w2.y), pack_bf16x2(w3.x, w3.y));
+            const uint32_t u0 = pack_bf16x2(w0.x, w0.y), u1 = pack_bf16x2(w1.x, w1.y);
+            const uint32_t u2 = pack_bf16x2(w2.x, w2.y), u3 = pack_bf16x2(w3.x, w3.y);
+            st_shared_v4(ds_row + ((chunk ^ (row & 7)) << 4), u0, u1, u2, u3);
+            if (Cfg::kTmemOperands) { dsk[g * 4 + 0] = u0; dsk[g * 4 + 1] = u1; dsk[g * 4 + 2] = u2; dsk[g * 4 + 3] = u3; }
           }
+          // (overlays only dP^T columns this thread has already loaded; dP^T(i+1) is issued behind dK(i))
+          if (Cfg::kTmemOperands) tmem_st_x16(tDP + c * 16, dsk);
         };
         tmem_wait_ld_x32(dp0);
         tmem_wait_ld_x32(dp1);
@@ -405,6 +446,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         half_b(dp1, 1);
       }
       fence_proxy_async_smem();
+      if (Cfg::kTmemOperands) tmem_wait_st();
       tc_fence_before();
       mbar_arrive(ds_full);
       if (threadIdx.x == 0) BTRACE(3, i);   // ds_full(i) arrived

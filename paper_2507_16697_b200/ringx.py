@@ -48,6 +48,10 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_chunk_fwd.restype = c_i
     L.ringx_attn_fwd_bwd_host.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_fwd_bwd_host.restype = c_i
+    L.ringx_attn_fwd_gqa.argtypes = [c_p] * 5 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_fwd_gqa.restype = c_i
+    L.ringx_attn_bwd_gqa.argtypes = [c_p] * 9 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_bwd_gqa.restype = c_i
     L.ringx_attn_bwd_partial.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_bwd_partial.restype = c_i
     L.ringx_attn_bwd_partial_workspace_bytes.argtypes = [c_i] * 4
@@ -303,3 +307,38 @@ def ringx_eq5_finalize(num, den, lse_max, out_dtype=torch.float32):
 
 def ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d) -> int:
     return lib().ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d)
+
+
+def ringx_attn_fwd_gqa(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, workspace=None):
+    """Grouped-query forward: q [B,Hq,N,d], k,v [B,Hkv,N,d] (include/ringx.h: ringx_attn_fwd_gqa)."""
+    B, Hq, N, d = q.shape
+    Hkv = k.shape[1]
+    dt = _DTYPES[q.dtype]
+    o = torch.empty_like(q) if o is None else o
+    lse = torch.empty((B, Hq, N), dtype=torch.float32, device=q.device) if lse is None else lse
+    need = lib().ringx_attn_fwd_workspace_bytes(B, Hq, N, d, kv_chunk, dt)
+    if workspace is None:
+        workspace = _workspace(need, q.device)
+    ws_ptr = workspace.data_ptr() if workspace is not None else None
+    ws_len = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    st = lib().ringx_attn_fwd_gqa(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                                  B, Hq, Hkv, N, d, kv_chunk, scale, dt, ws_ptr, ws_len, _stream())
+    _check(st, "ringx_attn_fwd_gqa")
+    return o, lse
+
+
+def ringx_attn_bwd_gqa(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspace=None):
+    """Grouped-query backward: dq [B,Hq,N,d], dk, dv [B,Hkv,N,d] (include/ringx.h: ringx_attn_bwd_gqa)."""
+    B, Hq, N, d = q.shape
+    Hkv = k.shape[1]
+    dt = _DTYPES[q.dtype]
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    need = lib().ringx_attn_bwd_workspace_bytes(B, Hq, N, d, kv_chunk, dt)
+    if workspace is None:
+        workspace = _workspace(max(need, 256), q.device)
+    st = lib().ringx_attn_bwd_gqa(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                                  _dev(dO, "dO"), _dev(dq, "dq"), _dev(dk, "dk"), _dev(dv, "dv"),
+                                  B, Hq, Hkv, N, d, kv_chunk, scale, dt, workspace.data_ptr(),
+                                  workspace.numel() * workspace.element_size(), _stream())
+    _check(st, "ringx_attn_bwd_gqa")
+    return dq, dk, dv

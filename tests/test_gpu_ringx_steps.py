@@ -297,3 +297,38 @@ def test_ringx_dist_over_nccl_world_size_one(rx):
         assert torch.equal(out, t) and torch.equal(st[0], t)
     finally:
         dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------ GQA (NEXT-3)
+@pytest.mark.parametrize("Hq,Hkv,N,d,chunk", [(4, 2, 512, 64, 256), (6, 2, 256, 128, 128), (8, 1, 512, 64, 512)])
+def test_gqa_forward_and_backward_match_oracle(rx, Hq, Hkv, N, d, chunk):
+    """Hq query heads share Hkv kv heads (query head h attends kv head h // (Hq/Hkv)); the oracle is the plain
+    attention of every query head against its kv head, dk/dv summed over the heads of the group."""
+    B, G = 2, Hq // Hkv
+    scale = 1.0 / math.sqrt(d)
+    q = wl.make_tensor((B, Hq, N, d), "q", seed=41, dtype="bf16")
+    do = wl.make_tensor((B, Hq, N, d), "do", seed=41, dtype="bf16")
+    k = wl.make_tensor((B, Hkv, N, d), "k", seed=41, dtype="bf16")
+    v = wl.make_tensor((B, Hkv, N, d), "v", seed=41, dtype="bf16")
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    o, lse = rx.ringx_attn_fwd_gqa(qd, kd, vd, chunk, scale)
+    dq, dk, dv = rx.ringx_attn_bwd_gqa(qd, kd, vd, o, lse, dod, chunk, scale)
+    q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+    k_rep, v_rep = np.repeat(k64, G, axis=1), np.repeat(v64, G, axis=1)      # kv head of every query head
+    o_ref, lse_ref = orc.attention_fwd_bhnd(q64, k_rep, v_rep, scale)
+    dq_ref, dk_rep, dv_rep = orc.attention_bwd_bhnd(q64, k_rep, v_rep, do64, scale)
+    dk_ref = dk_rep.reshape(B, Hkv, G, N, d).sum(axis=2)
+    dv_ref = dv_rep.reshape(B, Hkv, G, N, d).sum(axis=2)
+    assert np.abs(f64(o) - o_ref).max() <= 1e-2 * np.abs(v64).max()
+    assert relf(f64(o), o_ref) <= 1e-2
+    assert np.abs(f64(lse) - lse_ref).max() <= 5e-5
+    for g, ref in ((dq, dq_ref), (dk, dk_ref), (dv, dv_ref)):
+        e = relf(f64(g), ref)
+        assert e <= TOL_GRAD and e <= 6e-3, e
+    # Hq == Hkv is the plain multi-head call, bit for bit
+    o2, lse2 = rx.ringx_attn_fwd_gqa(qd[:, :Hkv].contiguous(), kd, vd, chunk, scale)
+    o3, lse3 = rx.ringx_attn_fwd(qd[:, :Hkv].contiguous(), kd, vd, chunk, scale)
+    assert torch.equal(o2, o3) and torch.equal(lse2, lse3)
+    L = rx.lib()
+    assert L.ringx_attn_fwd_gqa(qd.data_ptr(), kd.data_ptr(), vd.data_ptr(), o.data_ptr(), lse.data_ptr(), B, 5, 2, N, d,
+                                chunk, scale, 1, None, 0, None) == 2          # Hq % Hkv != 0: BAD_SHAPE
