@@ -306,13 +306,30 @@ def main():
     bwd_info = {"ms_per_step": bwd_ms, "tflops": cfg.bwd_flops / bwd_ms / 1e9,
                 "frac_of_sustained_peak": cfg.bwd_flops / bwd_ms / 1e9 / peaks["bf16_tflops_sustained"],
                 "frac_of_burst_peak": cfg.bwd_flops / bwd_ms / 1e9 / peaks["bf16_tflops"]} if bwd_ms > 0 else None
-    merge_ms, merge_n = prof["merge"]
+    # the Eq. 5 merge kernel (north_star subsystem 3): the bf16 forward folds Eq. 5 in the chunk kernel's epilogue, so
+    # ringx_lse_merge -- the entry RingX_a/b and the fp32 path use -- is timed on its own on this workload's [R,d] partials
     merge_info = None
-    if merge_n:
-        mbytes = 3.0 * B * H * N * (d * 4 + 4) - (B * H * N * d * 2 * args.steps / merge_n)   # last merge writes bf16
-        merge_info = {"bound": "hbm", "avg_launch_ms": merge_ms / merge_n, "launches_timed": merge_n,
-                      "achieved": mbytes / (merge_ms / merge_n * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                      "frac": mbytes / (merge_ms / merge_n * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    if rank == 0:
+        R = B * H * N
+        pa, pb = torch.randn(R, d, device=dev), torch.randn(R, d, device=dev)
+        la, lb = torch.randn(R, device=dev), torch.randn(R, device=dev)
+        for _ in range(3):
+            ringx.ringx_lse_merge(pa, la, pb, lb, inplace=True)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_merge = 10
+        e0.record()
+        for _ in range(n_merge):
+            ringx.ringx_lse_merge(pa, la, pb, lb, inplace=True)
+        e1.record()
+        torch.cuda.synchronize()
+        mms = e0.elapsed_time(e1) / n_merge
+        mbytes = 3.0 * R * (d * 4 + 4)
+        merge_info = {"bound": "hbm", "kernel": "lse_merge_kernel<float,float>", "avg_launch_ms": mms,
+                      "launches_timed": n_merge, "achieved": mbytes / (mms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                      "unit": "GB/s", "frac": mbytes / (mms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                      "note": "timed alone, back to back, in place on operand a (fp32 partials of the workload's shape)"}
+        del pa, pb, la, lb
 
     # ---------------------------------------------------------------- e2e: HOST buffers through the C ABI
     n_e2e = max(1, min(args.steps, 3))
@@ -356,6 +373,7 @@ def main():
             if name == cfg.name:
                 continue
             extra[name] = side_measure(ringx, wl, wl.CONFIGS[name], dev)
+        extra["next_rows"] = next_rows_measure(ringx, wl, dev)
 
     # ---------------------------------------------------------------- CPU baseline: the oracle, bounded sample
     cpu_baseline = None
@@ -427,6 +445,56 @@ def side_measure(ringx, wl, cfg, dev, reps=3):
             out["bwd_tflops"] = cfg.bwd_flops / ms / 1e9
         except ringx.RingxError as e:
             out["bwd"] = f"unavailable: {e}"
+    return out
+
+
+def next_rows_measure(ringx, wl, dev, reps=5):
+    """Short timings of the SURVEY.md §8(f) rows built so far (context, not the metric): grouped-query attention,
+    the per-device RingX backward step, and the N-operand Eq. 5 kernels of RingX_a."""
+    out = {}
+
+    def timeit(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    # GQA: 16 query heads on 4 kv heads, N = 32768, d = 128, 4 passes of 8192 keys
+    B, Hq, Hkv, N, d, chunk = 1, 16, 4, 32768, 128, 8192
+    scale = d ** -0.5
+    q = wl.make_tensor((B, Hq, N, d), "q", seed=77, dtype="bf16", device=dev)
+    do = wl.make_tensor((B, Hq, N, d), "do", seed=77, dtype="bf16", device=dev)
+    k = wl.make_tensor((B, Hkv, N, d), "k", seed=77, dtype="bf16", device=dev)
+    v = wl.make_tensor((B, Hkv, N, d), "v", seed=77, dtype="bf16", device=dev)
+    o, lse = ringx.ringx_attn_fwd_gqa(q, k, v, chunk, scale)
+    fl = 4.0 * B * Hq * N * N * d
+    ms = timeit(lambda: ringx.ringx_attn_fwd_gqa(q, k, v, chunk, scale, o=o, lse=lse))
+    out["gqa_16q4kv_N32768_d128"] = {"fwd_tflops": fl / ms / 1e9}
+    ms = timeit(lambda: ringx.ringx_attn_bwd_gqa(q, k, v, o, lse, do, chunk, scale))
+    out["gqa_16q4kv_N32768_d128"]["bwd_tflops"] = 2.5 * fl / ms / 1e9
+    # RingX backward step: 16384 local query rows against one 16384-key chunk of another rank (global lse)
+    ql, ol, dol = (t[:, :4, :16384].contiguous() for t in (q, o, do))
+    lsel = lse[:, :4, :16384].contiguous()
+    kc, vc = k[:, :, 16384:].contiguous(), v[:, :, 16384:].contiguous()
+    acc = torch.zeros(ql.shape, dtype=torch.float32, device=dev)
+    ms = timeit(lambda: ringx.ringx_attn_bwd_partial(ql, kc, vc, ol, lsel, dol, scale, dq_acc=acc))
+    out["bwd_partial_Nq16384_Nk16384_d128"] = {"tflops": 10.0 * B * 4 * 16384 * 16384 * d / ms / 1e9}
+    # Eq. 5 with N operands: bytes per row = d*4 read + d*4 written (+ 12 / + 12)
+    rows = 1 << 21
+    lo = torch.randn(rows, d, device=dev)
+    ll = torch.randn(rows, device=dev)
+    lm = ll + 1.0
+    ms = timeit(lambda: ringx.ringx_eq5_scale(lo, ll, lm, inplace=True))
+    out["eq5_scale_gbs"] = rows * (2 * d * 4 + 12) / ms / 1e6
+    den = torch.ones(rows, device=dev)
+    ms = timeit(lambda: ringx.ringx_eq5_finalize(lo, den, lm, out_dtype=torch.float32))
+    out["eq5_finalize_gbs"] = rows * (2 * d * 4 + 12) / ms / 1e6
     return out
 
 

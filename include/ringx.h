@@ -68,7 +68,8 @@ typedef enum { RINGX_F32 = 0, RINGX_BF16 = 1 } ringx_dtype;
 
 /* Forward (Eq. 1 via Eq. 5).  For c = 0 .. N/kv_chunk-1: one chunk pass computes
  * (loc_out_c, loc_lse_c) of every query row against keys [c*kv_chunk, (c+1)*kv_chunk); partials
- * are folded left to right with the two-operand Eq. 5 (ringx_lse_merge) in fp32.
+ * are folded left to right with the two-operand Eq. 5 in fp32 (bf16: in the chunk kernel's epilogue; f32: by
+ * ringx_lse_merge's kernel).
  *   q,k,v  [B,H,N,d] of `dtype` (in).   o [B,H,N,d] of `dtype` (out).   lse [B,H,N] float (out).
  *   dtype  RINGX_BF16: tcgen05 tensor-core path, fp32 accumulation (mixed fp32/bf16, l.286).
  *          RINGX_F32 : plain FFMA path (max abs error ~1e-6; tf32 would not meet 1e-5).
@@ -120,6 +121,19 @@ RINGX_API int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o
  *   Nq % 256 == 0 (bf16) or % 128 (f32), Nk % 128 == 0, d in {64,128}.  No workspace. */
 RINGX_API int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse,
                          int B, int H, int Nq, int Nk, int d, float scale, int dtype, void* stream);
+
+/* ringx_attn_chunk_fwd with the two-operand Eq. 5 folded into the kernel's epilogue: attends `Nq` query rows against
+ * the `Nk` keys given and folds (loc_out, loc_lse) into the running partial result (o_acc, lse_acc) of the same rows
+ * -- one step of RingX_b's local loop (l.145) without the round trip of loc_out through HBM.
+ *   q [B,H,Nq,d], k,v [B,H,Nk,d] bf16; o_acc [B,H,Nq,d] FLOAT, lse_acc [B,H,Nq] float: in/out (as written by
+ *   ringx_attn_chunk_fwd, ringx_lse_merge or an earlier fold).
+ *   o_final, lse_final: both NULL -> the fold is written back to (o_acc, lse_acc) in place;
+ *                       both given -> o_final [B,H,Nq,d] bf16 and lse_final receive the folded result (last step),
+ *                       (o_acc, lse_acc) are left untouched.
+ *   Nq % 256 == 0, Nk % 128 == 0, d in {64,128}; dtype must be RINGX_BF16.  No workspace. */
+RINGX_API int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void* v, float* o_acc, float* lse_acc,
+                              void* o_final, float* lse_final,
+                              int B, int H, int Nq, int Nk, int d, float scale, int dtype, void* stream);
 
 /* Per-device backward step of RingX_a / RingX_b (l.143, l.145): the gradient contributions that `Nq` query
  * rows and `Nk` keys of every head exchange, with P recomputed from the *global* lse of those rows (the

@@ -70,8 +70,8 @@ int check_shape(int B, int H, int N, int d, int kv_chunk, float scale, int dtype
 struct FwdWorkspace {
   float* o_acc = nullptr;      // running (merged) output, fp32 [R,d]   (bf16 only; f32 uses `o` itself)
   float* lse_acc = nullptr;    // running LSE [R]                        (bf16 only; f32 uses `lse`)
-  float* o_part = nullptr;     // loc_out of the current pass, fp32 [R,d]
-  float* lse_part = nullptr;   // loc_lse of the current pass [R]
+  float* o_part = nullptr;     // loc_out of the current pass, fp32 [R,d]   (f32 only)
+  float* lse_part = nullptr;   // loc_lse of the current pass [R]           (f32 only)
   size_t bytes = 0;
 };
 
@@ -86,12 +86,13 @@ FwdWorkspace carve_fwd(void* ws, int B, int H, int N, int d, int kv_chunk, int d
     off += align_up(n);
     return r;
   };
-  if (dtype == RINGX_BF16) {
+  if (dtype == RINGX_BF16) {   // the chunk kernel folds each pass into the running accumulator itself
     w.o_acc = reinterpret_cast<float*>(take(R * d * sizeof(float)));
     w.lse_acc = reinterpret_cast<float*>(take(R * sizeof(float)));
+  } else {                     // fp32: partials of the current pass, merged by lse_merge into the caller's o/lse
+    w.o_part = reinterpret_cast<float*>(take(R * d * sizeof(float)));
+    w.lse_part = reinterpret_cast<float*>(take(R * sizeof(float)));
   }
-  w.o_part = reinterpret_cast<float*>(take(R * d * sizeof(float)));
-  w.lse_part = reinterpret_cast<float*>(take(R * sizeof(float)));
   w.bytes = off;
   return w;
 }
@@ -168,17 +169,18 @@ bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, in
   return r == CUDA_SUCCESS;
 }
 
-// One KV-chunk pass, either dtype.  o_out: fp32 partial, or the final dtype when `final_out`.
-static cudaError_t chunk_pass(const void* q, const void* k, const void* v, void* o_out, float* lse_out, int BH, int Nq,
-                              int nk_stride, int k_off, int nk, int d, float scale, int dtype, bool final_out,
-                              cudaStream_t stream) {
+// One KV-chunk pass, either dtype.  `epilogue` (kernels.cuh, kFwdEpi*): partial / final / folded into (o_acc, lse_acc).
+// The fp32 path has the partial epilogue only.
+static cudaError_t chunk_pass(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
+                              const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride, int k_off,
+                              int nk, int d, float scale, int dtype, int epilogue, cudaStream_t stream) {
   Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
   if (dtype == RINGX_F32)
     return launch_attn_chunk_f32(static_cast<const float*>(q), static_cast<const float*>(k),
                                  static_cast<const float*>(v), static_cast<float*>(o_out), lse_out, BH, Nq, nk_stride,
                                  k_off, nk, d, scale, stream);
-  return launch_attn_chunk_fwd_sm100(q, k, v, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, d, scale,
-                                     final_out ? 1 : 0, stream);
+  return launch_attn_chunk_fwd_sm100(q, k, v, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, d, scale,
+                                     epilogue, stream);
 }
 
 }  // namespace ringx
@@ -212,23 +214,35 @@ static int fwd_core(const void* q, const void* k, const void* v, void* o, float*
   const long long R = (long long)BH * Nq;
   const int n_chunks = N / kv_chunk;
   if (n_chunks == 1) {
-    cudaError_t e = chunk_pass(q, k, v, o, lse, BH, Nq, N, 0, N, d, scale, dtype, true, stream);
+    cudaError_t e = chunk_pass(q, k, v, o, lse, nullptr, nullptr, BH, Nq, N, 0, N, d, scale, dtype, kFwdEpiFinal, stream);
     return e == cudaSuccess ? RINGX_OK : cuda_status(e);
   }
-  // running accumulator: fp32 for both dtypes (f32 accumulates straight into the caller's o/lse)
-  float* o_acc = dtype == RINGX_F32 ? static_cast<float*>(o) : w.o_acc;
-  float* lse_acc = dtype == RINGX_F32 ? lse : w.lse_acc;
   for (int c = 0; c < n_chunks; ++c) {
     const bool first = c == 0, last = c == n_chunks - 1;
-    cudaError_t e = chunk_pass(q, k, v, first ? o_acc : w.o_part, first ? lse_acc : w.lse_part, BH, Nq, N,
-                               c * kv_chunk, kv_chunk, d, scale, dtype, false, stream);
+    cudaError_t e;
+    if (dtype == RINGX_BF16) {
+      // Eq. 5, two operands, folded left to right in the chunk kernel's epilogue: the running (o_acc, lse_acc) stays
+      // fp32 in the workspace; the last pass writes the caller's bf16 o and lse
+      if (first)
+        e = chunk_pass(q, k, v, w.o_acc, w.lse_acc, nullptr, nullptr, BH, Nq, N, 0, kv_chunk, d, scale, dtype,
+                       kFwdEpiPartial, stream);
+      else if (!last)
+        e = chunk_pass(q, k, v, w.o_acc, w.lse_acc, w.o_acc, w.lse_acc, BH, Nq, N, c * kv_chunk, kv_chunk, d, scale,
+                       dtype, kFwdEpiFold, stream);
+      else
+        e = chunk_pass(q, k, v, o, lse, w.o_acc, w.lse_acc, BH, Nq, N, c * kv_chunk, kv_chunk, d, scale, dtype,
+                       kFwdEpiFoldFinal, stream);
+      if (e != cudaSuccess) return cuda_status(e);
+      continue;
+    }
+    // fp32: partials, then ringx_lse_merge's kernel, accumulating straight into the caller's o/lse
+    float* o_acc = static_cast<float*>(o);
+    e = chunk_pass(q, k, v, first ? o_acc : w.o_part, first ? lse : w.lse_part, nullptr, nullptr, BH, Nq, N,
+                   c * kv_chunk, kv_chunk, d, scale, dtype, kFwdEpiPartial, stream);
     if (e != cudaSuccess) return cuda_status(e);
     if (first) continue;
-    // Eq. 5, two operands, folded left to right; the last fold writes the caller's dtype
-    const bool to_out = last && dtype == RINGX_BF16;
     Timed timed(RINGX_PROFILE_MERGE, stream);
-    e = launch_lse_merge(o_acc, lse_acc, w.o_part, w.lse_part, to_out ? o : o_acc, to_out ? lse : lse_acc, R, d,
-                         RINGX_F32, to_out ? RINGX_BF16 : RINGX_F32, stream);
+    e = launch_lse_merge(o_acc, lse, w.o_part, w.lse_part, o_acc, lse, R, d, RINGX_F32, RINGX_F32, stream);
     count_launch();
     if (e != cudaSuccess) return cuda_status(e);
   }
@@ -285,7 +299,34 @@ int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc
   int st = check_arch();
   if (st != RINGX_OK) return st;
   tl_launches = 0;
-  cudaError_t e = chunk_pass(q, k, v, loc_out, loc_lse, B * H, Nq, Nk, 0, Nk, d, scale, dtype, false, stream);
+  cudaError_t e = chunk_pass(q, k, v, loc_out, loc_lse, nullptr, nullptr, B * H, Nq, Nk, 0, Nk, d, scale, dtype,
+                             kFwdEpiPartial, stream);
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void* v, float* o_acc, float* lse_acc, void* o_final,
+                              float* lse_final, int B, int H, int Nq, int Nk, int d, float scale, int dtype,
+                              void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o_acc || !lse_acc || (o_final == nullptr) != (lse_final == nullptr)) return RINGX_ERR_NULL_PTR;
+  if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
+  if (Nk % 128 || Nq % 256) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
+    return RINGX_ERR_BAD_SHAPE;
+  if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o_acc) || !aligned16(lse_acc) ||
+      !aligned16(o_final) || !aligned16(lse_final))
+    return RINGX_ERR_MISALIGNED;
+  int st = check_arch();
+  if (st != RINGX_OK) return st;
+  tl_launches = 0;
+  cudaError_t e = o_final ? chunk_pass(q, k, v, o_final, lse_final, o_acc, lse_acc, B * H, Nq, Nk, 0, Nk, d, scale, dtype,
+                                       kFwdEpiFoldFinal, stream)
+                          : chunk_pass(q, k, v, o_acc, lse_acc, o_acc, lse_acc, B * H, Nq, Nk, 0, Nk, d, scale, dtype,
+                                       kFwdEpiFold, stream);
   if (e != cudaSuccess) return cuda_status(e);
   tl_last_launches = tl_launches;
   return RINGX_OK;

@@ -71,11 +71,20 @@ struct FwdCfg {
   static constexpr int kSmemBytes = 1024 + 2 * kTileBytes + kStages * kTileBytes + kBarBytes;
 };
 
-template <int kD, bool kOutBf16>
+// Epilogue modes (kEpi): what happens to (loc_out, loc_lse) of this chunk
+//   kEpiPartial   written as they are, fp32                       (first pass; ringx_attn_chunk_fwd)
+//   kEpiFinal     loc_out written as bf16                         (single pass: the chunk is the whole sequence)
+//   kEpiFold      folded into the running (o_acc, lse_acc) with the two-operand Eq. 5, in place, fp32
+//   kEpiFoldFinal folded with (o_acc, lse_acc) and written to (o_out, lse_out) as bf16 (last pass)
+// Folding here instead of in a separate lse_merge launch saves the round trip of loc_out through HBM; it is the same
+// arithmetic as merge.cu's lse_merge_kernel, row by row (a thread owns a query row).
+enum { kEpiPartial = 0, kEpiFinal = 1, kEpiFold = 2, kEpiFoldFinal = 3 };
+
+template <int kD, int kEpi>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
-                      const __grid_constant__ CUtensorMap map_v, void* __restrict__ o_out,
-                      float* __restrict__ lse_out, int Nq, int nk_stride, int k_off, int n_kv, float scale_log2) {
+                      const __grid_constant__ CUtensorMap map_v, void* o_out, float* lse_out, const float* o_acc,
+                      const float* lse_acc, int Nq, int nk_stride, int k_off, int n_kv, float scale_log2) {
   using Cfg = FwdCfg<kD>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -350,33 +359,61 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     // ---- chunk epilogue: loc_out = O / l, loc_lse = m*scale + ln l  (natural log of the scaled scores)
     mbar_wait(&o_full[t], 0);
     tc_fence_after();
-    const float inv = 1.0f / l;
     const size_t row = static_cast<size_t>(q_row0) + t * kBlockM + (warp & 3) * 32 + lane;
+    constexpr bool kFold = kEpi == kEpiFold || kEpi == kEpiFoldFinal;
+    constexpr bool kOutBf16 = kEpi == kEpiFinal || kEpi == kEpiFoldFinal;
+    float lse_row = (m_sc + lg2(l)) * 0.6931471805599453f;
+    float cb = 1.0f / l, ca = 0.f;            // out = ca * o_acc + cb * O  (O = unnormalised accumulator in TMEM)
+    if (kFold) {                              // Eq. 5, two operands: (o_acc, lse_acc) and (loc_out, loc_lse)
+      const float la = lse_acc[row];
+      const float m = fmaxf(la, lse_row);
+      const float wa = ex2((la - m) * 1.4426950408889634f), wb = ex2((lse_row - m) * 1.4426950408889634f);
+      const float den = wa + wb, r = 1.0f / den;
+      ca = wa * r;
+      cb *= wb * r;
+      lse_row = m + lg2(den) * 0.6931471805599453f;
+    }
 #pragma unroll
     for (int c = 0; c < kD / 32; ++c) {
       uint32_t o[32];
       tmem_ld_x32(tO + c * 32, o);
+      float4 acc[8];
+      if (kFold) {
+        const float4* src = reinterpret_cast<const float4*>(o_acc + row * kD + c * 32);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[i] = __ldcs(src + i);
+      }
       tmem_wait_ld();
+      float r[32];
+#pragma unroll
+      for (int i = 0; i < 32; ++i) r[i] = __uint_as_float(o[i]) * cb;
+      if (kFold) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          r[i * 4 + 0] = fmaf(ca, acc[i].x, r[i * 4 + 0]);
+          r[i * 4 + 1] = fmaf(ca, acc[i].y, r[i * 4 + 1]);
+          r[i * 4 + 2] = fmaf(ca, acc[i].z, r[i * 4 + 2]);
+          r[i * 4 + 3] = fmaf(ca, acc[i].w, r[i * 4 + 3]);
+        }
+      }
       if (kOutBf16) {
         uint4* dst = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(o_out) + row * kD + c * 32);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           uint4 u;
-          u.x = pack_bf16x2(__uint_as_float(o[i * 8 + 0]) * inv, __uint_as_float(o[i * 8 + 1]) * inv);
-          u.y = pack_bf16x2(__uint_as_float(o[i * 8 + 2]) * inv, __uint_as_float(o[i * 8 + 3]) * inv);
-          u.z = pack_bf16x2(__uint_as_float(o[i * 8 + 4]) * inv, __uint_as_float(o[i * 8 + 5]) * inv);
-          u.w = pack_bf16x2(__uint_as_float(o[i * 8 + 6]) * inv, __uint_as_float(o[i * 8 + 7]) * inv);
+          u.x = pack_bf16x2(r[i * 8 + 0], r[i * 8 + 1]);
+          u.y = pack_bf16x2(r[i * 8 + 2], r[i * 8 + 3]);
+          u.z = pack_bf16x2(r[i * 8 + 4], r[i * 8 + 5]);
+          u.w = pack_bf16x2(r[i * 8 + 6], r[i * 8 + 7]);
           dst[i] = u;
         }
       } else {
         float4* dst = reinterpret_cast<float4*>(static_cast<float*>(o_out) + row * kD + c * 32);
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
-          dst[i] = make_float4(__uint_as_float(o[i * 4]) * inv, __uint_as_float(o[i * 4 + 1]) * inv,
-                               __uint_as_float(o[i * 4 + 2]) * inv, __uint_as_float(o[i * 4 + 3]) * inv);
+        for (int i = 0; i < 8; ++i) dst[i] = make_float4(r[i * 4], r[i * 4 + 1], r[i * 4 + 2], r[i * 4 + 3]);
       }
     }
-    lse_out[row] = (m_sc + lg2(l)) * 0.6931471805599453f;
+    lse_out[row] = lse_row;
   } else {
     setmaxnreg_dec<kAuxRegs>();   // warps 10-11: nothing to do but release their registers
   }
@@ -386,11 +423,12 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   if (warp == 8) tmem_dealloc<512>(tmem);
 }
 
-template <int kD, bool kOutBf16>
+template <int kD, int kEpi>
 cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, void* o_out, float* lse_out,
-                     int BH, int Nq, int nk_stride, int k_off, int nk, float scale, cudaStream_t stream) {
+                     const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride, int k_off, int nk,
+                     float scale, cudaStream_t stream) {
   using Cfg = FwdCfg<kD>;
-  auto kern = attn_chunk_fwd_kernel<kD, kOutBf16>;
+  auto kern = attn_chunk_fwd_kernel<kD, kEpi>;
   static bool configured = false;   // benign race: the attribute is idempotent
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
@@ -398,28 +436,41 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
     configured = true;
   }
   dim3 grid(Nq / (2 * kBlockM), BH);
-  kern<<<grid, kFwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, Nq, nk_stride, k_off,
+  kern<<<grid, kFwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, Nq, nk_stride, k_off,
                                                        nk / kBlockN, scale * 1.4426950408889634f);
   count_launch();
   return cudaGetLastError();
 }
 
+template <int kD>
+cudaError_t launch_d(int epi, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, void* o_out,
+                     float* lse_out, const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride, int k_off,
+                     int nk, float scale, cudaStream_t stream) {
+  switch (epi) {
+    case kEpiPartial:
+      return launch_t<kD, kEpiPartial>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+    case kEpiFinal:
+      return launch_t<kD, kEpiFinal>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+    case kEpiFold:
+      return launch_t<kD, kEpiFold>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+    default:
+      return launch_t<kD, kEpiFoldFinal>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
-                                        int BH, int Nq, int nk_stride, int k_off, int nk, int d, float scale,
-                                        int out_bf16, cudaStream_t stream) {
+                                        const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride,
+                                        int k_off, int nk, int d, float scale, int epilogue, cudaStream_t stream) {
   CUtensorMap mq, mk, mv;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   if (!make_tmap_2d(&mq, q, dt, 2, (uint64_t)BH * Nq, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mk, k, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mv, v, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64)
-    return out_bf16 ? launch_t<64, true>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream)
-                    : launch_t<64, false>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream);
-  return out_bf16 ? launch_t<128, true>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream)
-                  : launch_t<128, false>(mq, mk, mv, o_out, lse_out, BH, Nq, nk_stride, k_off, nk, scale, stream);
+  if (d == 64) return launch_d<64>(epilogue, mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+  return launch_d<128>(epilogue, mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
 }
 
 }  // namespace ringx

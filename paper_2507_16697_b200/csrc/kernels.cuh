@@ -32,11 +32,14 @@ cudaError_t launch_attn_chunk_f32(const float* q, const float* k, const float* v
                                   int Nq, int nk_stride, int k_off, int nk, int d, float scale, cudaStream_t stream);
 
 // ---- attn_fwd_sm100.cu (tcgen05 path)
-// One KV-chunk pass, bf16 in / fp32 accumulate.  out_bf16 = 0: o_out is float [BH,Nq,d] (a partial,
-// loc_out); out_bf16 = 1: o_out is bf16 (single-pass final result).
+// One KV-chunk pass, bf16 in / fp32 accumulate.  `epilogue` says what happens to (loc_out, loc_lse):
+//   0 written to (o_out, lse_out) as fp32 partials          1 loc_out written as bf16 (single-pass final result)
+//   2 folded by the two-operand Eq. 5 into the running fp32 (o_acc, lse_acc); o_out == o_acc, lse_out == lse_acc
+//   3 folded with (o_acc, lse_acc) and written to (o_out bf16, lse_out): the last pass
+enum { kFwdEpiPartial = 0, kFwdEpiFinal = 1, kFwdEpiFold = 2, kFwdEpiFoldFinal = 3 };
 cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
-                                        int BH, int Nq, int nk_stride, int k_off, int nk, int d, float scale,
-                                        int out_bf16, cudaStream_t stream);
+                                        const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride,
+                                        int k_off, int nk, int d, float scale, int epilogue, cudaStream_t stream);
 
 // ---- attn_bwd_sm100.cu (tcgen05 path)
 // One KV-chunk pass of the backward: q,dO [BH,N,d], k,v,dk,dv [BH,nk_stride,d]; writes dk,dv rows

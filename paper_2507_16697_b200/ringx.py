@@ -48,6 +48,8 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_chunk_fwd.restype = c_i
     L.ringx_attn_fwd_bwd_host.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_fwd_bwd_host.restype = c_i
+    L.ringx_attn_chunk_fwd_fold.argtypes = [c_p] * 7 + [c_i] * 5 + [c_f, c_i, c_p]
+    L.ringx_attn_chunk_fwd_fold.restype = c_i
     L.ringx_attn_fwd_gqa.argtypes = [c_p] * 5 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_fwd_gqa.restype = c_i
     L.ringx_attn_bwd_gqa.argtypes = [c_p] * 9 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
@@ -342,3 +344,21 @@ def ringx_attn_bwd_gqa(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspa
                                   workspace.numel() * workspace.element_size(), _stream())
     _check(st, "ringx_attn_bwd_gqa")
     return dq, dk, dv
+
+
+def ringx_attn_chunk_fwd_fold(q, k, v, o_acc, lse_acc, scale: float, final: bool = False):
+    """One chunk pass folded into the running fp32 (o_acc, lse_acc) by Eq. 5 inside the kernel (include/ringx.h:
+    ringx_attn_chunk_fwd_fold).  final=False: in place, returns (o_acc, lse_acc); final=True: returns the folded
+    result as (o bf16, lse), the accumulators untouched."""
+    B, H, Nq, d = q.shape
+    Nk = k.shape[2]
+    o_f = lse_f = None
+    if final:
+        o_f = torch.empty((B, H, Nq, d), dtype=q.dtype, device=q.device)
+        lse_f = torch.empty((B, H, Nq), dtype=torch.float32, device=q.device)
+    st = lib().ringx_attn_chunk_fwd_fold(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o_acc, "o_acc"),
+                                         _dev(lse_acc, "lse_acc"), _dev(o_f, "o_final") if final else None,
+                                         _dev(lse_f, "lse_final") if final else None, B, H, Nq, Nk, d, scale,
+                                         _DTYPES[q.dtype], _stream())
+    _check(st, "ringx_attn_chunk_fwd_fold")
+    return (o_f, lse_f) if final else (o_acc, lse_acc)

@@ -2,7 +2,7 @@
 attention schedules (Fig. 2), one process per GPU, NCCL over NVLink/NVSwitch.
 
 Every rank holds an equal sequence chunk `q, k, v [B,H,N/W,d]`.  All arithmetic of the method
-runs in libringx kernels (`ringx_attn_chunk_fwd`, `ringx_lse_merge`, `ringx_eq5_scale/finalize`,
+runs in libringx kernels (`ringx_attn_chunk_fwd`, `ringx_attn_chunk_fwd_fold`, `ringx_eq5_scale/finalize`,
 `ringx_attn_bwd_partial`, `ringx_dq_finalize`); this module only sequences them with the collectives the paper names:
 
   RingX_b   forward : all-gather(K,V) -> local chunk loop + running Eq. 5 merge
@@ -41,8 +41,8 @@ class CudaOps:
     def chunk_fwd(self, q, k, v, scale):                      # (loc_out fp32, loc_lse)
         return self.rx.ringx_attn_chunk_fwd(q, k, v, scale)
 
-    def lse_merge(self, o_a, lse_a, o_b, lse_b, out_dtype, inplace):   # two-operand Eq. 5
-        return self.rx.ringx_lse_merge(o_a, lse_a, o_b, lse_b, out_dtype=out_dtype, inplace=inplace)
+    def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final):   # chunk pass + two-operand Eq. 5 in one kernel
+        return self.rx.ringx_attn_chunk_fwd_fold(q, k, v, o_acc, lse_acc, scale, final=final)
 
     def eq5_scale(self, loc_out, loc_lse, lse_max):           # num, den of one operand (in place on loc_out)
         return self.rx.ringx_eq5_scale(loc_out, loc_lse, lse_max, inplace=True)
@@ -122,11 +122,10 @@ def ringx_b_forward(q, k, v, scale, comm=None, ops=None):
     o = lse = None
     for s in range(1, W):
         c = (r + s) % W                                       # ring order: every rank starts on a different chunk
-        o_p, lse_p = ops.chunk_fwd(q, kg[c], vg[c], scale)
         if s == W - 1:
-            o, lse = ops.lse_merge(o_acc, lse_acc, o_p, lse_p, q.dtype, False)
+            o, lse = ops.chunk_fwd_fold(q, kg[c], vg[c], o_acc, lse_acc, scale, True)     # last fold writes bf16
         else:
-            o_acc, lse_acc = ops.lse_merge(o_acc, lse_acc, o_p, lse_p, o_acc.dtype, True)
+            o_acc, lse_acc = ops.chunk_fwd_fold(q, kg[c], vg[c], o_acc, lse_acc, scale, False)
     return o, lse, (q, kg, vg, o, lse, scale)
 
 

@@ -38,7 +38,7 @@ def fwd_sampled_check(rx, cfg, heads, n_rows):
     o, lse = rx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale)
     torch.cuda.synchronize()
     n_c = cfg.N // cfg.kv_chunk
-    assert rx.ringx_last_launch_count() == 2 * n_c - 1
+    assert rx.ringx_last_launch_count() == n_c        # one chunk kernel per pass; Eq. 5 is folded in its epilogue
     vmax = v.float().abs().max().item()
     worst = {"o": 0.0, "relf": 0.0, "lse": 0.0}
     for (b, h) in heads:

@@ -172,7 +172,7 @@ def test_fwd_bf16_matches_oracle(rx, B, H, N, d, chunk, gain):
     scale = 1.0 / math.sqrt(d)
     o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), chunk, scale)
     n_c = N // chunk
-    assert rx.ringx_last_launch_count() == n_c + (n_c - 1)
+    assert rx.ringx_last_launch_count() == n_c        # bf16: the Eq. 5 fold runs in the chunk kernel's epilogue
     o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
     check_fwd(o, lse, o_ref, lse_ref, f64(v), "bf16")
 
@@ -409,7 +409,7 @@ def test_fwd_bwd_host_entry_matches_device_entries(rx):
     dq, dk, dv = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale)
     oh, lh, dqh, dkh, dvh = rx.ringx_attn_fwd_bwd_host(q.pin_memory(), k.pin_memory(), v.pin_memory(),
                                                        do.pin_memory(), chunk, scale)
-    assert rx.ringx_last_launch_count() == (2 * (N // chunk) - 1) + (N // chunk + 2)
+    assert rx.ringx_last_launch_count() == (N // chunk) + (N // chunk + 2)
     assert torch.equal(oh, o.cpu()) and torch.equal(lh, lse.cpu())
     assert torch.equal(dkh, dk.cpu()) and torch.equal(dvh, dv.cpu())
     assert ((dqh.float() - dq.cpu().float()).norm() / dq.float().norm()).item() <= 2e-3   # fp32 red order

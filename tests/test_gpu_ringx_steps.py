@@ -118,6 +118,49 @@ def test_bwd_partial_rejects_bad_arguments(rx):
     torch.cuda.synchronize()
 
 
+# ------------------------------------------------------------------------------------------------ fused fold
+@pytest.mark.parametrize("d,Nq,chunks,gain", [(128, 512, (256, 128, 640), 1.0), (64, 256, (512, 512), 1.0),
+                                              (128, 256, (128, 128, 128, 128), 3.0)])
+def test_chunk_fwd_fold_equals_the_running_merge(rx, d, Nq, chunks, gain):
+    """ringx_attn_chunk_fwd_fold = ringx_attn_chunk_fwd + two-operand Eq. 5 in one kernel: against the oracle's
+    running merge over ragged chunks, and against the library's own two-kernel route (fp32 rounding apart)."""
+    B, H, Nk = 2, 2, sum(chunks)
+    scale = 1.0 / math.sqrt(d)
+    q = wl.make_tensor((B, H, Nq, d), "q", seed=91, dtype="bf16", gain=gain)
+    k = wl.make_tensor((B, H, Nk, d), "k", seed=91, dtype="bf16", gain=gain)
+    v = wl.make_tensor((B, H, Nk, d), "v", seed=91, dtype="bf16")
+    qd, kd, vd = q.cuda(), k.cuda(), v.cuda()
+    bounds = np.concatenate([[0], np.cumsum(chunks)])
+    ck = [(kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous()) for lo, hi in zip(bounds[:-1], bounds[1:])]
+    o_acc, lse_acc = rx.ringx_attn_chunk_fwd(qd, *ck[0], scale)
+    o_ref2, lse_ref2 = o_acc.clone(), lse_acc.clone()
+    for kc, vc in ck[1:-1]:
+        o_acc, lse_acc = rx.ringx_attn_chunk_fwd_fold(qd, kc, vc, o_acc, lse_acc, scale)
+        assert rx.ringx_last_launch_count() == 1
+        o_p, lse_p = rx.ringx_attn_chunk_fwd(qd, kc, vc, scale)
+        o_ref2, lse_ref2 = rx.ringx_lse_merge(o_ref2, lse_ref2, o_p, lse_p)
+        assert (o_acc - o_ref2).abs().max().item() <= 2e-6 * max(1.0, o_ref2.abs().max().item())
+        assert (lse_acc - lse_ref2).abs().max().item() <= 1e-5
+    keep_o, keep_l = o_acc.clone(), lse_acc.clone()
+    o, lse = rx.ringx_attn_chunk_fwd_fold(qd, *ck[-1], o_acc, lse_acc, scale, final=True)
+    assert o.dtype == torch.bfloat16
+    assert torch.equal(keep_o, o_acc) and torch.equal(keep_l, lse_acc)          # final fold leaves the accumulators alone
+    q64, k64, v64 = f64(q), f64(k), f64(v)
+    o_ref, lse_ref = orc.attention_fwd_bhnd(q64, k64, v64, scale)
+    for b in range(B):
+        for h in range(H):
+            a, l = orc.attention_fwd_running(q64[b, h], k64[b, h], v64[b, h], scale, [int(x) for x in bounds])
+            np.testing.assert_allclose(a, o_ref[b, h], atol=1e-12)              # (oracle: running == unchunked)
+    assert np.abs(f64(o) - o_ref).max() <= 1e-2 * np.abs(v64).max()
+    assert relf(f64(o), o_ref) <= 1e-2
+    assert np.abs(f64(lse) - lse_ref).max() <= 5e-5
+    L = rx.lib()
+    assert L.ringx_attn_chunk_fwd_fold(qd.data_ptr(), kd.data_ptr(), vd.data_ptr(), o_acc.data_ptr(), lse_acc.data_ptr(),
+                                       o.data_ptr(), None, B, H, Nq, Nk, d, scale, 1, None) == 1     # one of the pair NULL
+    assert L.ringx_attn_chunk_fwd_fold(qd.data_ptr(), kd.data_ptr(), vd.data_ptr(), o_acc.data_ptr(), lse_acc.data_ptr(),
+                                       None, None, B, H, Nq, Nk, d, scale, 0, None) == 3             # bf16 only
+
+
 # ------------------------------------------------------------------------------------------------ Eq. 5, N operands
 @pytest.mark.parametrize("rows,d,n_ops", [(1, 8, 2), (777, 64, 3), (4099, 128, 5), (130, 1024, 4)])
 def test_eq5_scale_and_finalize_match_oracle(rx, rows, d, n_ops):

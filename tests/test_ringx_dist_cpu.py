@@ -46,6 +46,10 @@ class OracleOps:
             o[b, h], lse[b, h] = torch.from_numpy(a), torch.from_numpy(l)
         return o, lse
 
+    def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final):
+        o_p, lse_p = self.chunk_fwd(q, k, v, scale)
+        return self.lse_merge(o_acc, lse_acc, o_p, lse_p, o_acc.dtype, not final)
+
     def lse_merge(self, o_a, lse_a, o_b, lse_b, out_dtype, inplace):
         o, lse = orc.lse_merge(o_a.reshape(-1, o_a.shape[-1]).numpy(), lse_a.reshape(-1).numpy(),
                                o_b.reshape(-1, o_b.shape[-1]).numpy(), lse_b.reshape(-1).numpy())
