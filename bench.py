@@ -495,6 +495,24 @@ def next_rows_measure(ringx, wl, dev, reps=5):
     den = torch.ones(rows, device=dev)
     ms = timeit(lambda: ringx.ringx_eq5_finalize(lo, den, lm, out_dtype=torch.float32))
     out["eq5_finalize_gbs"] = rows * (2 * d * 4 + 12) / ms / 1e6
+    del lo, ll, lm, den, q, k, v, o, do, acc
+    # NEXT-4, the Turbulence-Transformer tokeniser: 512^3 x 4 fp32 state (2.1 GB, larger than L2),
+    # Gaussian filter k^3 with stride k.  Algorithmic bytes = 16 per input voxel + 16 (8 for bf16) per token.
+    G = 512
+    y = wl.make_field(1, G, G, G, seed=20250722, device=dev)
+    tok = {}
+    for kk, odt in ((4, torch.float32), (2, torch.bfloat16), (8, torch.float32), (1, torch.float32)):
+        size = (G, G, G) if kk > 1 else (G // 2, G, G)      # k = 1: a half-domain crop (pure copy)
+        t = ringx.ringx_fidelity_tokens(y, (0, 0, 0), size, kk, out_dtype=odt)
+        ms = timeit(lambda: ringx.ringx_fidelity_tokens(y, (0, 0, 0), size, kk, tokens=t))
+        nvox = size[0] * size[1] * size[2]
+        byt = nvox * 16 + (nvox // kk ** 3) * 4 * t.element_size()
+        tok[f"k{kk}_{'bf16' if odt == torch.bfloat16 else 'f32'}"] = {"ms": ms, "gbs": byt / ms / 1e6,
+                                                                   "tokens": nvox // kk ** 3}
+    peaks = load_peaks()
+    tok["roofline"] = {"bound": "hbm", "kernel": "fidelity_tokens_kernel (k=4, f32 tokens)", "achieved": tok["k4_f32"]["gbs"],
+                       "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": tok["k4_f32"]["gbs"] / peaks["hbm_gbs"]}
+    out["fidelity_tokens_512cube"] = tok
     return out
 
 

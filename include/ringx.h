@@ -170,6 +170,23 @@ RINGX_API int ringx_eq5_scale(const float* loc_out, const float* loc_lse, const 
 RINGX_API int ringx_eq5_finalize(const float* num, const float* den, const float* lse_max,
                        void* o_out, float* lse_out, long long rows, int d, int o_out_dtype, void* stream);
 
+/* The Turbulence-Transformer tokeniser (l.195-199): one fidelity mode F_k(C(Y)) -- a sub-domain selection C of size
+ * Dc x Hc x Wc at origin (z0,y0,x0) followed by a Gaussian filter of kernel size k^3 "via convolution", the result
+ * lying in R^{Dc/k x Hc/k x Wc/k x 4}; every filtered voxel is one token (patch size 1, l.179):
+ *   T[m,z',y',x',c] = sum_{a,b,e<k} G[a,b,e] * Y[m, z0+k z'+a, y0+k y'+b, x0+k x'+e, c]
+ * Readings (the paper is silent; DESIGN.md t1-t6): the convolution has stride k and no padding (forced by the output
+ * size); G[a,b,e] = w[a]w[b]w[e], w[a] = g[a]/sum(g), g[a] = exp(-(a-(k-1)/2)^2 / (2 sigma^2)); sigma <= 0 selects
+ * the LES Gaussian filter of width k, sigma = k/sqrt(12); the crop lies inside the domain (no periodic wrap);
+ * "centered at [x_c,y_c,z_c]" means origin = centre - size/2, computed by the caller.  k = 1 is the pure crop
+ * (high-fidelity mode); Dc = D etc. with origin 0 is the low-fidelity mode (no crop).
+ *   y       [M,D,H,W,C] float, C fastest (in); C must be 4 (V_x, V_y, V_z, P: l.176).  M = number of input states.
+ *   tokens  [M,Dc/k,Hc/k,Wc/k,C] of out_dtype (out), x' fastest: the token sequence of length L = M*Dc*Hc*Wc/k^3.
+ *   Domain  1 <= k <= 32; Dc,Hc,Wc multiples of k; Hc/k and M*Dc/k <= 65535; anything else RINGX_ERR_BAD_SHAPE.
+ *   fp32 arithmetic (k^3 fused multiply-adds per output); one launch; no workspace. */
+RINGX_API int ringx_fidelity_tokens(const float* y, void* tokens, int M, int D, int H, int W, int C,
+                          int z0, int y0, int x0, int Dc, int Hc, int Wc, int k, float sigma,
+                          int out_dtype, void* stream);
+
 /* ringx_attn_fwd with HOST buffers (the end-to-end entry): copies q,k,v host->device into the
  * workspace, runs ringx_attn_fwd, copies o and lse back, and synchronises `stream`.
  *   q_host,k_host,v_host,o_host,lse_host  HOST pointers (pinned memory recommended).
@@ -204,9 +221,9 @@ RINGX_API int ringx_last_launch_count(void);
  * ringx_profile_read synchronises on the recorded events, adds the elapsed milliseconds and launch
  * counts per kind into ms[RINGX_PROFILE_KINDS] / launches[RINGX_PROFILE_KINDS] (HOST arrays), and
  * forgets the records.  Kinds: attention forward chunk kernel, Eq. 5 merge kernel, attention
- * backward chunk kernel, backward helpers (D_i preprocess and dQ convert). */
+ * backward chunk kernel, backward helpers (D_i preprocess and dQ convert), tokeniser. */
 enum { RINGX_PROFILE_ATTN_FWD = 0, RINGX_PROFILE_MERGE = 1, RINGX_PROFILE_ATTN_BWD = 2, RINGX_PROFILE_BWD_AUX = 3,
-       RINGX_PROFILE_KINDS = 4 };
+       RINGX_PROFILE_TOKENISER = 4, RINGX_PROFILE_KINDS = 5 };
 RINGX_API int ringx_profile_enable(int on);
 RINGX_API int ringx_profile_read(double* ms, int* launches);
 

@@ -1,6 +1,8 @@
 // api.cu -- the C-ABI layer of libringx (include/ringx.h): argument validation, workspace carving,
 // TMA tensor-map creation and the KV-chunk pass loop.  No arithmetic of the method lives here; every
 // step of the path runs in the kernels this file launches.
+#include <math.h>
+
 #include <mutex>
 #include <vector>
 
@@ -605,6 +607,43 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   return RINGX_OK;
 }
 
+// ---- the Turbulence-Transformer tokeniser
+int ringx_fidelity_tokens(const float* y, void* tokens, int M, int D, int H, int W, int C, int z0, int y0, int x0,
+                          int Dc, int Hc, int Wc, int k, float sigma, int out_dtype, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (out_dtype != RINGX_F32 && out_dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (C != 4 || M <= 0 || D <= 0 || H <= 0 || W <= 0 || k < 1 || k > 32) return RINGX_ERR_BAD_SHAPE;
+  if (Dc <= 0 || Hc <= 0 || Wc <= 0 || Dc % k || Hc % k || Wc % k) return RINGX_ERR_BAD_SHAPE;
+  if (z0 < 0 || y0 < 0 || x0 < 0 || (long long)z0 + Dc > D || (long long)y0 + Hc > H || (long long)x0 + Wc > W)
+    return RINGX_ERR_BAD_SHAPE;
+  if (Hc / k > 65535 * 1 || (long long)M * (Dc / k) > 65535) return RINGX_ERR_BAD_SHAPE;
+  if (!(sigma == sigma) || sigma > 3.0e38f) return RINGX_ERR_BAD_SHAPE;
+  if (!y || !tokens) return RINGX_ERR_NULL_PTR;
+  if (!aligned16(y) || !aligned16(tokens)) return RINGX_ERR_MISALIGNED;
+  int st = check_arch();
+  if (st != RINGX_OK) return st;
+  // normalised 1-D Gaussian weights (the kernel applies w[a] w[b] w[e]); sigma <= 0 selects the LES filter width k
+  const double sg = sigma > 0.f ? (double)sigma : (double)k / sqrt(12.0);
+  double g[32], sum = 0.0;
+  for (int a = 0; a < k; ++a) {
+    const double r = a - 0.5 * (k - 1);
+    g[a] = exp(-r * r / (2.0 * sg * sg));
+    sum += g[a];
+  }
+  float w[32];
+  for (int a = 0; a < k; ++a) w[a] = (float)(g[a] / sum);
+  tl_launches = 0;
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_TOKENISER, stream);
+    e = launch_fidelity_tokens(y, tokens, M, D, H, W, z0, y0, x0, Dc, Hc, Wc, k, w, out_dtype, stream);
+  }
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
 int ringx_last_launch_count(void) { return tl_last_launches; }
 
 int ringx_profile_enable(int on) {
@@ -647,6 +686,6 @@ const char* ringx_status_string(int status) {
   }
 }
 
-int ringx_version(void) { return 110; }
+int ringx_version(void) { return 120; }
 
 }  // extern "C"

@@ -26,6 +26,11 @@ cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* ls
                                   cudaStream_t stream);
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
 
+// ---- fidelity.cu (the Turbulence-Transformer tokeniser): crop + k^3 Gaussian filter, stride k.
+// y [M,D,H,W,4] fp32 -> tokens [M,Dc/k,Hc/k,Wc/k,4] (f32 or bf16); w = k normalised 1-D weights (host array).
+cudaError_t launch_fidelity_tokens(const float* y, void* tokens, int M, int D, int H, int W, int z0, int y0, int x0,
+                                   int Dc, int Hc, int Wc, int k, const float* w, int out_dtype, cudaStream_t stream);
+
 // ---- attn_f32.cu (plain FFMA path, config C1)
 // One KV-chunk pass, fp32: q [BH,Nq,d], k/v [BH,nk_stride,d] rows [k_off, k_off+nk) -> o_out fp32, lse_out.
 cudaError_t launch_attn_chunk_f32(const float* q, const float* k, const float* v, float* o_out, float* lse_out, int BH,

@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
     L.ringx_eq5_scale.restype = c_i
     L.ringx_eq5_finalize.argtypes = [c_p] * 5 + [c_ll, c_i, c_i, c_p]
     L.ringx_eq5_finalize.restype = c_i
+    L.ringx_fidelity_tokens.argtypes = [c_p, c_p] + [c_i] * 12 + [c_f, c_i, c_p]
+    L.ringx_fidelity_tokens.restype = c_i
     for name in ("ringx_attn_fwd_workspace_bytes", "ringx_attn_bwd_workspace_bytes",
                  "ringx_attn_fwd_host_workspace_bytes", "ringx_attn_fwd_bwd_host_workspace_bytes"):
         getattr(L, name).argtypes = [c_i] * 6
@@ -237,7 +239,7 @@ def ringx_last_launch_count() -> int:
     return lib().ringx_last_launch_count()
 
 
-PROFILE_KINDS = ("attn_fwd", "merge", "attn_bwd", "bwd_aux")
+PROFILE_KINDS = ("attn_fwd", "merge", "attn_bwd", "bwd_aux", "tokeniser")
 
 
 def ringx_profile_enable(on: bool) -> None:
@@ -254,6 +256,22 @@ def ringx_profile_read() -> dict:
 
 def ringx_version() -> int:
     return lib().ringx_version()
+
+
+def ringx_fidelity_tokens(y, origin, size, k: int, sigma: float = 0.0, out_dtype=torch.float32, tokens=None):
+    """One fidelity mode F_k(C(Y)) of the Turbulence-Transformer tokeniser (include/ringx.h: ringx_fidelity_tokens).
+    y [M,D,H,W,4] fp32; origin (z0,y0,x0); size (Dc,Hc,Wc).  Returns tokens [M,Dc/k,Hc/k,Wc/k,4] of out_dtype."""
+    M, D, H, W, C = y.shape
+    if y.dtype != torch.float32:
+        raise ValueError("y must be float32")
+    (z0, y0, x0), (Dc, Hc, Wc) = origin, size
+    if tokens is None:
+        tokens = torch.empty((M, max(Dc // max(k, 1), 0), max(Hc // max(k, 1), 0), max(Wc // max(k, 1), 0), C),
+                             dtype=out_dtype, device=y.device)
+    st = lib().ringx_fidelity_tokens(_dev(y, "y"), _dev(tokens, "tokens"), M, D, H, W, C, z0, y0, x0, Dc, Hc, Wc, k,
+                                     float(sigma), _DTYPES[tokens.dtype], _stream())
+    _check(st, "ringx_fidelity_tokens")
+    return tokens
 
 
 def ringx_attn_bwd_partial(q, k, v, o, lse, dO, scale: float, dq_acc=None, dk=None, dv=None, workspace=None):

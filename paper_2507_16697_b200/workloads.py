@@ -134,3 +134,36 @@ def voxel_token_index(x: int, y: int, z: int, G: int) -> int:
     """Token order of the grid configs: x fastest.  Metadata only -- non-causal
     attention with no positional term is permutation-equivariant, which the tests use."""
     return x + G * (y + G * z)
+
+
+# ------------------------------------------------------------------------------------------------
+# Synthetic turbulence-like state for the tokeniser (PAPER.md:176: Y in R^{D x H x W x 4} = V_x, V_y, V_z, P).
+# The paper's fields (JHTDB forced HIT 1024^3, PAPER.md:81; stratified Taylor-Green, Table VI) are not available;
+# this stand-in has their *shape and layout* and a value structure with both large scales and grid-scale noise:
+# per variable, `n_modes` seeded Fourier modes with integer wave vectors |kappa| <= 8 and amplitude ~ |kappa|^(-5/6)
+# (a Kolmogorov-like E(kappa) ~ kappa^(-5/3)), plus 0.25 * iid N(0,1) from the counter-based generator.
+# No arithmetic of the method (no filtering, no cropping) happens here.
+# ------------------------------------------------------------------------------------------------
+FIELD_TENSOR_ID = 8
+
+
+def make_field(M: int, D: int, H: int, W: int, seed: int = 20250722, n_modes: int = 6, device="cpu") -> torch.Tensor:
+    """Y [M, D, H, W, 4] fp32, channels fastest; a pure function of (seed, shape)."""
+    C = 4
+    out = torch.empty((M, D, H, W, C), dtype=torch.float32, device=device)
+    par = normal_f32(M * C * n_modes * 5, seed, FIELD_TENSOR_ID + 1).view(M, C, n_modes, 5)
+    z = torch.arange(D, dtype=torch.float32, device=device).view(D, 1, 1) / D
+    y = torch.arange(H, dtype=torch.float32, device=device).view(1, H, 1) / H
+    x = torch.arange(W, dtype=torch.float32, device=device).view(1, 1, W) / W
+    for m in range(M):
+        noise = normal_f32(D * H * W * C, seed + 1 + m, FIELD_TENSOR_ID, device=device).view(D, H, W, C)
+        for c in range(C):
+            f = 0.25 * noise[..., c]
+            for j in range(n_modes):
+                kz, ky, kx = (int(round(float(v) * 3.0)) for v in par[m, c, j, :3])
+                kz, ky, kx = (max(-8, min(8, v)) for v in (kz, ky, kx))
+                kk = max(1.0, math.sqrt(kz * kz + ky * ky + kx * kx))
+                phase = float(par[m, c, j, 3]) * math.pi
+                f = f + (kk ** (-5.0 / 6.0)) * torch.sin((2.0 * math.pi) * (kz * z + ky * y + kx * x) + phase)
+            out[m, ..., c] = f
+    return out
