@@ -513,6 +513,22 @@ def next_rows_measure(ringx, wl, dev, reps=5):
     tok["roofline"] = {"bound": "hbm", "kernel": "fidelity_tokens_kernel (k=4, f32 tokens)", "achieved": tok["k4_f32"]["gbs"],
                        "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": tok["k4_f32"]["gbs"] / peaks["hbm_gbs"]}
     out["fidelity_tokens_512cube"] = tok
+    del y, t
+    # NEXT-4, Table II's projection GEMMs around the attention kernel at C3's block shape
+    # (B=1, S=262144, h=1024): 6*b*S*h^2 and 2*b*S*h^2 FLOPs; the head split / merge is fused into the TMA coordinates.
+    B, S, H, d = 1, 262144, 8, 128
+    h = H * d
+    x, wq, wo = wl.make_block_inputs(B, S, H, d, device=dev)
+    q, k, v = ringx.ringx_qkv_proj(x, wq, H)
+    ms_q = timeit(lambda: ringx.ringx_qkv_proj(x, wq, H, q=q, k=k, v=v))
+    yb = ringx.ringx_out_proj(q, wo)
+    ms_o = timeit(lambda: ringx.ringx_out_proj(q, wo, y=yb))
+    tq, to = 6.0 * B * S * h * h / ms_q / 1e9, 2.0 * B * S * h * h / ms_o / 1e9
+    out["projections_S262144_h1024"] = {
+        "qkv_ms": ms_q, "qkv_tflops": tq, "out_ms": ms_o, "out_tflops": to,
+        "roofline": {"bound": "tensor", "kernel": "proj_gemm_kernel<QKV>", "achieved": tq, "peak": peaks["bf16_tflops"],
+                     "unit": "TFLOP/s", "frac": tq / peaks["bf16_tflops"],
+                     "peak_kind": "bf16 dense, burst (kernel timed alone), measured"}}
     return out
 
 

@@ -187,6 +187,26 @@ RINGX_API int ringx_fidelity_tokens(const float* y, void* tokens, int M, int D, 
                           int z0, int y0, int x0, int Dc, int Hc, int Wc, int k, float sigma,
                           int out_dtype, void* stream);
 
+/* Table II's projection GEMMs either side of the attention kernel (l.184-190), bf16 operands, fp32 accumulation on
+ * tcgen05, bf16 results (mixed fp32/bf16, l.286):
+ *   ringx_qkv_proj  "Input to Q/K/V", (b,S,h) x (h,h) three times: [q|k|v] = x W_qkv^T, written directly in the
+ *                   head-split layout (b*a, S, h/a) that the attention entry points read.
+ *                   x [B,S,h] (in); w_qkv [3h,h] = [W_q; W_k; W_v], output-feature major (y = x W^T, in);
+ *                   q,k,v [B,H,S,d] (out), head a = features [a*d, (a+1)*d).  h = H*d.
+ *   ringx_out_proj  "Linear Projection", (bS,h) x (h,h): y = merge_heads(o) W_o^T.
+ *                   o [B,H,S,d] (in); w_o [h,h] (in); y [B,S,h] (out).
+ *   ringx_attn_block_fwd  the block: ringx_qkv_proj -> ringx_attn_fwd -> ringx_out_proj; q,k,v,o,lse live in the
+ *                   workspace (>= ringx_attn_block_fwd_workspace_bytes, 256-byte aligned).
+ * No bias, no activation (Table II counts none).  Domain: d in {64,128}; S % 128 == 0 (and the attention domain for
+ * the block); anything else RINGX_ERR_BAD_SHAPE.  Outputs must not alias inputs.  One launch per GEMM. */
+RINGX_API int ringx_qkv_proj(const void* x, const void* w_qkv, void* q, void* k, void* v,
+                   int B, int S, int H, int d, void* stream);
+RINGX_API int ringx_out_proj(const void* o, const void* w_o, void* y, int B, int S, int H, int d, void* stream);
+RINGX_API int ringx_attn_block_fwd(const void* x, const void* w_qkv, const void* w_o, void* y,
+                         int B, int S, int H, int d, int kv_chunk, float scale,
+                         void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_block_fwd_workspace_bytes(int B, int S, int H, int d, int kv_chunk);
+
 /* ringx_attn_fwd with HOST buffers (the end-to-end entry): copies q,k,v host->device into the
  * workspace, runs ringx_attn_fwd, copies o and lse back, and synchronises `stream`.
  *   q_host,k_host,v_host,o_host,lse_host  HOST pointers (pinned memory recommended).
@@ -221,9 +241,9 @@ RINGX_API int ringx_last_launch_count(void);
  * ringx_profile_read synchronises on the recorded events, adds the elapsed milliseconds and launch
  * counts per kind into ms[RINGX_PROFILE_KINDS] / launches[RINGX_PROFILE_KINDS] (HOST arrays), and
  * forgets the records.  Kinds: attention forward chunk kernel, Eq. 5 merge kernel, attention
- * backward chunk kernel, backward helpers (D_i preprocess and dQ convert), tokeniser. */
+ * backward chunk kernel, backward helpers (D_i preprocess and dQ convert), tokeniser, projection GEMMs. */
 enum { RINGX_PROFILE_ATTN_FWD = 0, RINGX_PROFILE_MERGE = 1, RINGX_PROFILE_ATTN_BWD = 2, RINGX_PROFILE_BWD_AUX = 3,
-       RINGX_PROFILE_TOKENISER = 4, RINGX_PROFILE_KINDS = 5 };
+       RINGX_PROFILE_TOKENISER = 4, RINGX_PROFILE_PROJ = 5, RINGX_PROFILE_KINDS = 6 };
 RINGX_API int ringx_profile_enable(int on);
 RINGX_API int ringx_profile_read(double* ms, int* launches);
 

@@ -644,6 +644,85 @@ int ringx_fidelity_tokens(const float* y, void* tokens, int M, int D, int H, int
   return RINGX_OK;
 }
 
+// ---- Table II's projection GEMMs and the attention block
+static int check_proj(int B, int S, int H, int d) {
+  if (B <= 0 || S <= 0 || H <= 0) return RINGX_ERR_BAD_SHAPE;
+  if (d != 64 && d != 128) return RINGX_ERR_BAD_SHAPE;
+  if (S % 128) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * S > 0x7fffffffll / 2 || (long long)B * S * H > 0x7fffffffll) return RINGX_ERR_BAD_SHAPE;
+  return RINGX_OK;
+}
+
+int ringx_qkv_proj(const void* x, const void* w_qkv, void* q, void* k, void* v, int B, int S, int H, int d,
+                   void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int st = check_proj(B, S, H, d);
+  if (st != RINGX_OK) return st;
+  if (!x || !w_qkv || !q || !k || !v) return RINGX_ERR_NULL_PTR;
+  if (!aligned16(x) || !aligned16(w_qkv) || !aligned16(q) || !aligned16(k) || !aligned16(v)) return RINGX_ERR_MISALIGNED;
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_PROJ, stream);
+    e = launch_qkv_proj(x, w_qkv, q, k, v, B, S, H, d, stream);
+  }
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_out_proj(const void* o, const void* w_o, void* y, int B, int S, int H, int d, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int st = check_proj(B, S, H, d);
+  if (st != RINGX_OK) return st;
+  if (!o || !w_o || !y) return RINGX_ERR_NULL_PTR;
+  if (!aligned16(o) || !aligned16(w_o) || !aligned16(y)) return RINGX_ERR_MISALIGNED;
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_PROJ, stream);
+    e = launch_out_proj(o, w_o, y, B, S, H, d, stream);
+  }
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+size_t ringx_attn_block_fwd_workspace_bytes(int B, int S, int H, int d, int kv_chunk) {
+  if (check_proj(B, S, H, d) != RINGX_OK) return 0;
+  const size_t R = (size_t)B * H * S;
+  return 4 * align_up(R * d * 2) + align_up(R * sizeof(float)) +
+         align_up(ringx_attn_fwd_workspace_bytes(B, H, S, d, kv_chunk, RINGX_BF16));
+}
+
+int ringx_attn_block_fwd(const void* x, const void* w_qkv, const void* w_o, void* y, int B, int S, int H, int d,
+                         int kv_chunk, float scale, void* workspace, size_t workspace_bytes, void* stream_) {
+  int st = check_proj(B, S, H, d);
+  if (st == RINGX_OK) st = check_shape(B, H, S, d, kv_chunk, scale, RINGX_BF16, false);
+  if (st != RINGX_OK) return st;
+  if (!x || !w_qkv || !w_o || !y || !workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < ringx_attn_block_fwd_workspace_bytes(B, S, H, d, kv_chunk)) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  const size_t R = (size_t)B * H * S, tba = align_up(R * d * 2);
+  char* p = static_cast<char*>(workspace);
+  void *q = p, *k = p + tba, *v = p + 2 * tba, *o = p + 3 * tba;
+  float* lse = reinterpret_cast<float*>(p + 4 * tba);
+  char* inner = p + 4 * tba + align_up(R * sizeof(float));
+  const size_t inner_bytes = workspace_bytes - (size_t)(inner - p);
+  st = ringx_qkv_proj(x, w_qkv, q, k, v, B, S, H, d, stream_);
+  if (st != RINGX_OK) return st;
+  int launches = tl_last_launches;
+  st = ringx_attn_fwd(q, k, v, o, lse, B, H, S, d, kv_chunk, scale, RINGX_BF16, inner, inner_bytes, stream_);
+  if (st != RINGX_OK) return st;
+  launches += tl_last_launches;
+  st = ringx_out_proj(o, w_o, y, B, S, H, d, stream_);
+  if (st != RINGX_OK) return st;
+  tl_last_launches += launches;
+  return RINGX_OK;
+}
+
 int ringx_last_launch_count(void) { return tl_last_launches; }
 
 int ringx_profile_enable(int on) {

@@ -31,6 +31,12 @@ cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float 
 cudaError_t launch_fidelity_tokens(const float* y, void* tokens, int M, int D, int H, int W, int z0, int y0, int x0,
                                    int Dc, int Hc, int Wc, int k, const float* w, int out_dtype, cudaStream_t stream);
 
+// ---- proj_sm100.cu (Table II's projection GEMMs; tcgen05, bf16, fp32 accumulate)
+// x [B,S,h], w_qkv [3h,h] = [W_q;W_k;W_v] (y = x W^T) -> q,k,v [B,H,S,d];  o [B,H,S,d], w_o [h,h] -> y [B,S,h].
+cudaError_t launch_qkv_proj(const void* x, const void* w_qkv, void* q, void* k, void* v, int B, int S, int H, int d,
+                            cudaStream_t stream);
+cudaError_t launch_out_proj(const void* o, const void* w_o, void* y, int B, int S, int H, int d, cudaStream_t stream);
+
 // ---- attn_f32.cu (plain FFMA path, config C1)
 // One KV-chunk pass, fp32: q [BH,Nq,d], k/v [BH,nk_stride,d] rows [k_off, k_off+nk) -> o_out fp32, lse_out.
 cudaError_t launch_attn_chunk_f32(const float* q, const float* k, const float* v, float* o_out, float* lse_out, int BH,

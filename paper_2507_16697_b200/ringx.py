@@ -66,6 +66,14 @@ def lib() -> ctypes.CDLL:
     L.ringx_eq5_finalize.restype = c_i
     L.ringx_fidelity_tokens.argtypes = [c_p, c_p] + [c_i] * 12 + [c_f, c_i, c_p]
     L.ringx_fidelity_tokens.restype = c_i
+    L.ringx_qkv_proj.argtypes = [c_p] * 5 + [c_i] * 4 + [c_p]
+    L.ringx_qkv_proj.restype = c_i
+    L.ringx_out_proj.argtypes = [c_p] * 3 + [c_i] * 4 + [c_p]
+    L.ringx_out_proj.restype = c_i
+    L.ringx_attn_block_fwd.argtypes = [c_p] * 4 + [c_i] * 5 + [c_f, c_p, c_sz, c_p]
+    L.ringx_attn_block_fwd.restype = c_i
+    L.ringx_attn_block_fwd_workspace_bytes.argtypes = [c_i] * 5
+    L.ringx_attn_block_fwd_workspace_bytes.restype = c_sz
     for name in ("ringx_attn_fwd_workspace_bytes", "ringx_attn_bwd_workspace_bytes",
                  "ringx_attn_fwd_host_workspace_bytes", "ringx_attn_fwd_bwd_host_workspace_bytes"):
         getattr(L, name).argtypes = [c_i] * 6
@@ -239,7 +247,7 @@ def ringx_last_launch_count() -> int:
     return lib().ringx_last_launch_count()
 
 
-PROFILE_KINDS = ("attn_fwd", "merge", "attn_bwd", "bwd_aux", "tokeniser")
+PROFILE_KINDS = ("attn_fwd", "merge", "attn_bwd", "bwd_aux", "tokeniser", "proj")
 
 
 def ringx_profile_enable(on: bool) -> None:
@@ -256,6 +264,50 @@ def ringx_profile_read() -> dict:
 
 def ringx_version() -> int:
     return lib().ringx_version()
+
+
+def ringx_qkv_proj(x, w_qkv, H: int, q=None, k=None, v=None):
+    """[q|k|v] = x W_qkv^T in the head-split layout (include/ringx.h: ringx_qkv_proj).  x [B,S,h], w_qkv [3h,h]."""
+    B, S, h = x.shape
+    d = h // H
+    if x.dtype != torch.bfloat16 or w_qkv.dtype != torch.bfloat16 or tuple(w_qkv.shape) != (3 * h, h) or d * H != h:
+        raise ValueError("x [B,S,h] and w_qkv [3h,h] must be bfloat16 with h = H*d")
+    q, k, v = (torch.empty((B, H, S, d), dtype=torch.bfloat16, device=x.device) if t is None else t for t in (q, k, v))
+    _check(lib().ringx_qkv_proj(_dev(x, "x"), _dev(w_qkv, "w_qkv"), _dev(q, "q"), _dev(k, "k"), _dev(v, "v"), B, S, H, d,
+                                _stream()), "ringx_qkv_proj")
+    return q, k, v
+
+
+def ringx_out_proj(o, w_o, y=None):
+    """y = merge_heads(o) W_o^T (include/ringx.h: ringx_out_proj).  o [B,H,S,d], w_o [h,h] -> y [B,S,h]."""
+    B, H, S, d = o.shape
+    h = H * d
+    if o.dtype != torch.bfloat16 or w_o.dtype != torch.bfloat16 or tuple(w_o.shape) != (h, h):
+        raise ValueError("o [B,H,S,d] and w_o [h,h] must be bfloat16")
+    y = torch.empty((B, S, h), dtype=torch.bfloat16, device=o.device) if y is None else y
+    _check(lib().ringx_out_proj(_dev(o, "o"), _dev(w_o, "w_o"), _dev(y, "y"), B, S, H, d, _stream()), "ringx_out_proj")
+    return y
+
+
+def ringx_attn_block_fwd_workspace_bytes(B, S, H, d, kv_chunk) -> int:
+    return lib().ringx_attn_block_fwd_workspace_bytes(B, S, H, d, kv_chunk)
+
+
+def ringx_attn_block_fwd(x, w_qkv, w_o, H: int, kv_chunk: int, scale: float, y=None, workspace=None):
+    """The attention block of Table II (include/ringx.h: ringx_attn_block_fwd).  x [B,S,h] -> y [B,S,h]."""
+    B, S, h = x.shape
+    d = h // H
+    if any(t.dtype != torch.bfloat16 for t in (x, w_qkv, w_o)) or tuple(w_qkv.shape) != (3 * h, h) or \
+            tuple(w_o.shape) != (h, h) or d * H != h:
+        raise ValueError("x [B,S,h], w_qkv [3h,h], w_o [h,h] must be bfloat16 with h = H*d")
+    y = torch.empty_like(x) if y is None else y
+    need = lib().ringx_attn_block_fwd_workspace_bytes(B, S, H, d, kv_chunk)
+    if workspace is None:
+        workspace = _workspace(max(need, 256), x.device)
+    st = lib().ringx_attn_block_fwd(_dev(x, "x"), _dev(w_qkv, "w_qkv"), _dev(w_o, "w_o"), _dev(y, "y"), B, S, H, d,
+                                    kv_chunk, scale, workspace.data_ptr(), workspace.numel(), _stream())
+    _check(st, "ringx_attn_block_fwd")
+    return y
 
 
 def ringx_fidelity_tokens(y, origin, size, k: int, sigma: float = 0.0, out_dtype=torch.float32, tokens=None):

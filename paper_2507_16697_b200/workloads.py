@@ -90,7 +90,17 @@ CONFIGS = {
     "C5": Config("C5", "bf16", 1, 4, 1048576, 128, 65536, qk_gain=3.0, seed=20250721, note="peaked softmax"),
 }
 
-TENSOR_IDS = {"q": 0, "k": 1, "v": 2, "do": 3}
+TENSOR_IDS = {"q": 0, "k": 1, "v": 2, "do": 3, "x": 4, "w_qkv": 5, "w_o": 6}
+
+
+def make_block_inputs(B: int, S: int, H: int, d: int, seed: int = 20250723, device="cpu"):
+    """Inputs of the attention block of Table II: x [B,S,h] ~ N(0,1); W_qkv [3h,h], W_o [h,h] ~
+    N(0, 1/h) (so that q, k, v come out ~ N(0,1), the distribution of the BASELINE.json configs); all bf16."""
+    h = H * d
+    x = make_tensor((B, S, h), "x", seed=seed, device=device)
+    w_qkv = make_tensor((3 * h, h), "w_qkv", seed=seed, gain=h ** -0.5, device=device)
+    w_o = make_tensor((h, h), "w_o", seed=seed, gain=h ** -0.5, device=device)
+    return x, w_qkv, w_o
 
 
 def make_tensor(cfg_or_shape, which: str, seed: int | None = None, dtype: str | None = None,
