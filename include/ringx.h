@@ -231,6 +231,14 @@ RINGX_API size_t ringx_attn_fwd_workspace_bytes(int B, int H, int N, int d, int 
 RINGX_API size_t ringx_attn_bwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
 RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
 
+/* Bit-reproducible dQ.  By default the per-key-tile contributions to dQ are reduce-added into the fp32
+ * accumulator in whatever order the CTAs reach them (fp32 addition is not associative: the last bits of dq may differ from run
+ * to run; dk, dv are always bit-reproducible).  With the flag set on the calling thread, ringx_attn_bwd, ringx_attn_bwd_gqa and
+ * ringx_attn_bwd_partial add the contributions to every dQ tile in key-tile order (a ticket counter per tile in the workspace):
+ * the same inputs, shapes and kv_chunk give bit-identical dq.  Costs a few per cent of backward throughput. */
+RINGX_API int ringx_set_deterministic(int on);
+RINGX_API int ringx_get_deterministic(void);
+
 /* Number of kernel launches the last successful call on this thread enqueued (bench.py's
  * `gpu_launches` claim is counted here, not guessed). */
 RINGX_API int ringx_last_launch_count(void);

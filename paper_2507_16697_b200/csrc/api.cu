@@ -103,6 +103,7 @@ struct BwdWorkspace {
   float* D = nullptr;        // D_i = dO_i . O_i, [R]
   float* lse2 = nullptr;     // LSE_i * log2(e), [R]
   float* dq_acc = nullptr;   // fp32 dQ accumulator [R,d]
+  int* dq_sem = nullptr;     // [R/128] ticket counters of the deterministic dQ order
   size_t bytes = 0;
 };
 
@@ -116,9 +117,13 @@ BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
   off += align_up(R * sizeof(float));
   w.dq_acc = reinterpret_cast<float*>(p ? p + off : nullptr);
   off += align_up(R * d * sizeof(float));
+  w.dq_sem = reinterpret_cast<int*>(p ? p + off : nullptr);
+  off += align_up(R / 128 * sizeof(int));
   w.bytes = off;
   return w;
 }
+
+thread_local bool tl_deterministic = false;
 
 // ---- optional live per-kernel timing (ringx_profile_*): CUDA events around each launch, per thread
 struct Profile {
@@ -365,9 +370,12 @@ int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const 
 // q,o,dO,lse: Nq rows per head; k,v,dk,dv: Nk rows per head.  dq_acc fp32 [BH,Nq,d] (zeroed first when zero_dq).
 static int bwd_core(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
                     float* D, float* lse2, float* dq_acc, bool zero_dq, void* dq_bf16, void* dk, void* dv, int BH,
-                    int Nq, int Nk, int d, int kv_chunk, float scale, cudaStream_t stream) {
+                    int Nq, int Nk, int d, int kv_chunk, float scale, int* dq_sem, cudaStream_t stream) {
   const long long R = (long long)BH * Nq;
   cudaError_t e;
+  if (!tl_deterministic) dq_sem = nullptr;
+  if (dq_sem && (e = cudaMemsetAsync(dq_sem, 0, (size_t)(R / 128) * sizeof(int), stream)) != cudaSuccess)
+    return cuda_status(e);
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
     e = launch_bwd_preprocess(o, dO, lse, D, lse2, dq_acc, R, d, scale, zero_dq, stream);
@@ -377,7 +385,7 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
   for (int c = 0; c < Nk / kv_chunk; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
     e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, dq_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, kv_chunk, d, scale,
-                                    stream);
+                                    dq_sem, stream);
     if (e != cudaSuccess) return cuda_status(e);
   }
   if (dq_bf16) {
@@ -412,7 +420,7 @@ int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, const void* 
   // so dK, dV of the kv head are still written once, atomic-free
   const int G = Hq / Hkv;
   st = bwd_core(q, k, v, o, lse, dO, w.D, w.lse2, w.dq_acc, true, dq, dk, dv, B * Hkv, G * N, N, d, kv_chunk, scale,
-                stream);
+                w.dq_sem, stream);
   if (st != RINGX_OK) return st;
   tl_last_launches = tl_launches;
   return RINGX_OK;
@@ -427,7 +435,8 @@ int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, c
 
 size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d) {
   if (B <= 0 || H <= 0 || Nq <= 0 || (d != 64 && d != 128)) return 0;
-  return 2 * align_up((size_t)B * H * Nq * sizeof(float));
+  const size_t R = (size_t)B * H * Nq;
+  return 2 * align_up(R * sizeof(float)) + align_up(R / 128 * sizeof(int));
 }
 
 int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const void* o, const float* lse,
@@ -452,8 +461,10 @@ int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const vo
   if (st != RINGX_OK) return st;
   tl_launches = 0;
   float* D = static_cast<float*>(workspace);
-  float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + need / 2);
-  st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, stream);
+  const size_t rb = align_up((size_t)B * H * Nq * sizeof(float));
+  float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + rb);
+  int* dq_sem = reinterpret_cast<int*>(static_cast<char*>(workspace) + 2 * rb);
+  st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, dq_sem, stream);
   if (st != RINGX_OK) return st;
   tl_last_launches = tl_launches;
   return RINGX_OK;
@@ -723,6 +734,13 @@ int ringx_attn_block_fwd(const void* x, const void* w_qkv, const void* w_o, void
   return RINGX_OK;
 }
 
+int ringx_set_deterministic(int on) {
+  tl_deterministic = on != 0;
+  return RINGX_OK;
+}
+
+int ringx_get_deterministic(void) { return tl_deterministic ? 1 : 0; }
+
 int ringx_last_launch_count(void) { return tl_last_launches; }
 
 int ringx_profile_enable(int on) {
@@ -765,6 +783,6 @@ const char* ringx_status_string(int status) {
   }
 }
 
-int ringx_version(void) { return 120; }
+int ringx_version(void) { return 130; }
 
 }  // extern "C"

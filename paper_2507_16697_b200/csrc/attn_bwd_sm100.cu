@@ -88,7 +88,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
                       const __grid_constant__ CUtensorMap map_dq, const float* __restrict__ lse2,
                       const float* __restrict__ Dvec,
                       __nv_bfloat16* __restrict__ dk, __nv_bfloat16* __restrict__ dv, int N, int nk_stride, int k_off,
-                      float scale_log2, float scale) {
+                      float scale_log2, float scale, int* __restrict__ dq_sem) {
   using Cfg = BwdCfg<kD>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -483,12 +483,19 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     const int row = (warp & 3) * 32 + lane;                      // query row of the tile = TMEM lane
     const uint32_t tDQ = tmem + Cfg::tDQ + (static_cast<uint32_t>((warp & 3) * 32) << 16);
     const bool leader = warp == 8 && elect_one();
+    // Deterministic mode (dq_sem != nullptr): the reduce-adds into one dQ tile are issued in key-tile order.  Tile
+    // (head, i) has a ticket counter; the CTA of key tile t (counted over the whole call, k_off included) waits for
+    // ticket t, issues its reduce, and once the reduce has been performed sets the ticket to t + 1.  CTAs are
+    // dispatched in block-index order, so the owner of ticket t is always resident or finished when t + 1 waits.
+    const int ticket = k_off / kTile + blockIdx.x;
+    int* sem = dq_sem ? dq_sem + bh * n_q : nullptr;
     int buf = 0;
     for (int i = 0; i < n_q; ++i) {
       const int i_ = i;
       const long long d0 = BCLK();
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
+
       const long long d1 = BCLK();
       if (threadIdx.x == 256) BTRACE(4, i);   // dq_full(i) seen
 #pragma unroll
@@ -514,15 +521,32 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           fence_proxy_async_smem();
           named_bar_sync(2, 128);
           if (leader) {
+            if (sem && rd == 0 && c == 0) {      // my turn to add into dQ tile i?
+              while (ld_acquire_gpu(sem + i) != ticket) __nanosleep(32);
+              fence_proxy_async_all();
+            }
             tma_reduce_add_2d(&map_dq, sDq + buf * Cfg::kDqPanelBytes, rd * 64 + c * 32, q_row0 + i * kTile);
             tma_commit_group();
           }
           buf ^= 1;
         }
       }
+      if (sem && leader && i > 0) {
+        // the reduce-adds of tile i-1 (every bulk group but the kD/32 just committed) have been performed: pass its
+        // ticket on.  Releasing one step late keeps the completion latency off this warp's critical path.
+        tma_wait_group<kD / 32>();
+        __threadfence();
+        st_release_gpu(sem + i - 1, ticket + 1);
+      }
       if (threadIdx.x == 256) { BADD(5, d1 - d0); BADD(6, BCLK() - d1); }
     }
-    if (leader) tma_wait_group<0>();
+    if (leader) {
+      tma_wait_group<0>();
+      if (sem) {
+        __threadfence();
+        st_release_gpu(sem + n_q - 1, ticket + 1);
+      }
+    }
     __syncwarp();
   } else {
     setmaxnreg_dec<kBwdAuxRegs>();   // warps 14-15: release their registers
@@ -536,7 +560,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 template <int kD>
 cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
                      const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int BH, int N,
-                     int nk_stride, int k_off, int nk, float scale, cudaStream_t stream) {
+                     int nk_stride, int k_off, int nk, float scale, int* dq_sem, cudaStream_t stream) {
   using Cfg = BwdCfg<kD>;
   auto kern = attn_chunk_bwd_kernel<kD>;
   static bool configured = false;
@@ -548,7 +572,8 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
   dim3 grid(nk / kTile, BH);
   kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D,
                                                        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv),
-                                                       N, nk_stride, k_off, scale * 1.4426950408889634f, scale);
+                                                       N, nk_stride, k_off, scale * 1.4426950408889634f, scale,
+                                                       dq_sem);
   count_launch();
   return cudaGetLastError();
 }
@@ -557,7 +582,8 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
 
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
-                                        int nk_stride, int k_off, int nk, int d, float scale, cudaStream_t stream) {
+                                        int nk_stride, int k_off, int nk, int d, float scale, int* dq_sem,
+                                        cudaStream_t stream) {
   CUtensorMap mq, mk, mv, mdo, mdq;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   const uint64_t rows = (uint64_t)BH * N, krows = (uint64_t)BH * nk_stride;
@@ -567,8 +593,8 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
       !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mdq, dq_acc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, rows, d, 128, 32, kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, stream);
-  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, stream);
+  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
+  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
 }
 
 }  // namespace ringx

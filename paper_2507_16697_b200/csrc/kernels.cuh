@@ -57,9 +57,12 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
 // [k_off, k_off+nk) of every head (bf16, the sum over the N query rows given), reduce-adds these keys'
 // contribution to dQ into dq_acc (fp32 [BH,N,d]).
 // lse2 = LSE * log2(e) and D = scale * rowsum(dO*O) come from launch_bwd_preprocess.
+// dq_sem: nullptr, or [BH * N/128] ticket counters (zero before the first pass of a call) that make the order of the
+// reduce-adds into every dQ tile the key-tile order (bit-reproducible dQ).
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
-                                        int nk_stride, int k_off, int nk, int d, float scale, cudaStream_t stream);
+                                        int nk_stride, int k_off, int nk, int d, float scale, int* dq_sem,
+                                        cudaStream_t stream);
 
 // ---- tensor maps (api.cu): 2-D row-major [rows, cols] view, box = {box_cols, box_rows}
 enum TmapSwizzle { kSwizzleNone = 0, kSwizzle128B = 1 };

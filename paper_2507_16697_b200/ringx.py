@@ -78,6 +78,10 @@ def lib() -> ctypes.CDLL:
                  "ringx_attn_fwd_host_workspace_bytes", "ringx_attn_fwd_bwd_host_workspace_bytes"):
         getattr(L, name).argtypes = [c_i] * 6
         getattr(L, name).restype = c_sz
+    L.ringx_set_deterministic.argtypes = [c_i]
+    L.ringx_set_deterministic.restype = c_i
+    L.ringx_get_deterministic.argtypes = []
+    L.ringx_get_deterministic.restype = c_i
     L.ringx_last_launch_count.argtypes = []
     L.ringx_last_launch_count.restype = c_i
     L.ringx_profile_enable.argtypes = [c_i]
@@ -241,6 +245,15 @@ def ringx_attn_fwd_bwd_host(q_host, k_host, v_host, dO_host, kv_chunk: int, scal
                                            workspace.data_ptr(), workspace.numel(), _stream())
     _check(st, "ringx_attn_fwd_bwd_host")
     return outs
+
+
+def ringx_set_deterministic(on: bool) -> None:
+    """Bit-reproducible dQ on the calling thread (include/ringx.h: ringx_set_deterministic)."""
+    _check(lib().ringx_set_deterministic(1 if on else 0), "ringx_set_deterministic")
+
+
+def ringx_get_deterministic() -> bool:
+    return bool(lib().ringx_get_deterministic())
 
 
 def ringx_last_launch_count() -> int:

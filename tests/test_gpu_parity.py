@@ -413,3 +413,33 @@ def test_fwd_bwd_host_entry_matches_device_entries(rx):
     assert torch.equal(oh, o.cpu()) and torch.equal(lh, lse.cpu())
     assert torch.equal(dkh, dk.cpu()) and torch.equal(dvh, dv.cpu())
     assert ((dqh.float() - dq.cpu().float()).norm() / dq.float().norm()).item() <= 2e-3   # fp32 red order
+
+
+# ------------------------------------------------------------------------------------------------ deterministic dQ
+@pytest.mark.parametrize("B,H,N,d,chunk", [(1, 2, 4096, 128, 1024), (2, 3, 2048, 64, 512)])
+def test_deterministic_mode_gives_bit_identical_dq(rx, B, H, N, d, chunk):
+    """NEXT-2: with ringx_set_deterministic(1) the contributions to every dQ tile are added in key-tile order, so
+    repeated runs agree bit for bit (dk, dv always do); the result still matches the oracle."""
+    scale = 1.0 / math.sqrt(d)
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=77, dtype="bf16")
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
+    rx.ringx_set_deterministic(True)
+    try:
+        assert rx.ringx_get_deterministic()
+        runs = [rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale) for _ in range(4)]
+        torch.cuda.synchronize()
+        acc = [rx.ringx_attn_bwd_partial(qd, kd, vd, o, lse, dod, scale)[0] for _ in range(3)]
+        torch.cuda.synchronize()
+    finally:
+        rx.ringx_set_deterministic(False)
+    assert not rx.ringx_get_deterministic()
+    for r in runs[1:]:
+        for a, b in zip(runs[0], r):
+            assert torch.equal(a, b)
+    for a in acc[1:]:
+        assert torch.equal(acc[0], a)                      # the fp32 accumulator itself is reproducible
+    q64, k64, v64, do64 = (wl.to_f64_numpy(t) for t in (q, k, v, do))
+    dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
+    for g, r in zip(runs[0], (dq_ref, dk_ref, dv_ref)):
+        assert np.linalg.norm(g.float().cpu().numpy() - r) / np.linalg.norm(r) <= 2e-2
