@@ -218,7 +218,10 @@ RINGX_API int ringx_attn_fwd_host(const void* q_host, const void* k_host, const 
 
 /* Forward + backward with HOST buffers (the end-to-end training-step entry): copies q,k,v,dO host->device
  * into the workspace, runs ringx_attn_fwd then ringx_attn_bwd, copies o, lse, dq, dk, dv back and
- * synchronises `stream`.  bf16 only.  All *_host pointers are HOST pointers (pinned recommended).
+ * synchronises `stream`.  bf16 only.  All *_host pointers are HOST pointers (pinned recommended).  The copies overlap the kernels on a
+ * side stream the library creates once per thread (a host object; still no device allocation): K,V rows go up chunk by chunk in
+ * the order the passes need them, dO goes up during the forward, o and lse come down during the backward, the dK,dV rows of a
+ * chunk come down as soon as its pass is done; only dq is copied after the last kernel.
  *   workspace  DEVICE, >= ringx_attn_fwd_bwd_host_workspace_bytes(...) bytes. */
 RINGX_API int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* v_host,
                             const void* dO_host, void* o_host, float* lse_host,

@@ -125,6 +125,22 @@ BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
 
 thread_local bool tl_deterministic = false;
 
+// side stream + events of ringx_attn_fwd_bwd_host (host objects only; no device memory)
+struct HostOverlap {
+  int device = -1;
+  cudaStream_t side = nullptr;
+  std::vector<cudaEvent_t> events;
+};
+thread_local HostOverlap tl_overlap;
+
+// Set by ringx_attn_fwd_bwd_host around its calls of the chunk loops: pass c of the forward waits for kv_ready[c] (the
+// K,V rows of chunk c have arrived from the host); the backward records pass_done[c] after pass c (its dK,dV rows are final).
+struct ChunkHooks {
+  const cudaEvent_t* kv_ready = nullptr;
+  const cudaEvent_t* pass_done = nullptr;
+};
+thread_local ChunkHooks tl_hooks;
+
 // ---- optional live per-kernel timing (ringx_profile_*): CUDA events around each launch, per thread
 struct Profile {
   bool on = false;
@@ -226,6 +242,7 @@ static int fwd_core(const void* q, const void* k, const void* v, void* o, float*
   }
   for (int c = 0; c < n_chunks; ++c) {
     const bool first = c == 0, last = c == n_chunks - 1;
+    if (tl_hooks.kv_ready && cudaStreamWaitEvent(stream, tl_hooks.kv_ready[c], 0) != cudaSuccess) return RINGX_ERR_CUDA;
     cudaError_t e;
     if (dtype == RINGX_BF16) {
       // Eq. 5, two operands, folded left to right in the chunk kernel's epilogue: the running (o_acc, lse_acc) stays
@@ -387,6 +404,7 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
     e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, dq_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, kv_chunk, d, scale,
                                     dq_sem, stream);
     if (e != cudaSuccess) return cuda_status(e);
+    if (tl_hooks.pass_done && (e = cudaEventRecord(tl_hooks.pass_done[c], stream)) != cudaSuccess) return cuda_status(e);
   }
   if (dq_bf16) {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
@@ -597,23 +615,96 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   float* dlse = reinterpret_cast<float*>(p + 8 * tba);
   char* inner = p + 8 * tba + align_up(R * sizeof(float));
   const size_t inner_bytes = workspace_bytes - (size_t)(inner - p);
-  const void* src[4] = {q_host, k_host, v_host, dO_host};
+  // Copies run on a side stream (host objects, created once per thread) so that they overlap the kernels: q and the
+  // K,V rows of chunk c go up in the order the passes need them (pass c waits for chunk c only), dO goes up while the
+  // forward runs, o and lse come down while the backward runs, and the dK,dV rows of chunk c -- final after pass c --
+  // come down while the later passes run.  Only dq is copied after the last kernel.
+  HostOverlap& ov = tl_overlap;
   cudaError_t ce;
-  for (int i = 0; i < 4; ++i)
-    if ((ce = cudaMemcpyAsync(t[i], src[i], tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+  int dev = 0;
+  if ((ce = cudaGetDevice(&dev)) != cudaSuccess) return cuda_status(ce);
+  const int n_chunks = N / kv_chunk;
+  const bool pipelined = n_chunks >= 2 && n_chunks <= 64;
+  const int n_events = 3 + (pipelined ? 2 * n_chunks : 0);
+  if (!ov.side || ov.device != dev) {      // (objects of another device are abandoned, not reused)
+    ov.device = dev;
+    ov.events.clear();
+    if ((ce = cudaStreamCreateWithFlags(&ov.side, cudaStreamNonBlocking)) != cudaSuccess) return cuda_status(ce);
+  }
+  while ((int)ov.events.size() < n_events) {
+    cudaEvent_t e;
+    if ((ce = cudaEventCreateWithFlags(&e, cudaEventDisableTiming)) != cudaSuccess) return cuda_status(ce);
+    ov.events.push_back(e);
+  }
+  cudaEvent_t ev_do_up = ov.events[0], ev_fwd_done = ov.events[1], ev_down = ov.events[2];
+  cudaEvent_t* kv_ready = ov.events.data() + 3;
+  cudaEvent_t* pass_done = kv_ready + n_chunks;
+  const int BH = B * H;
+  const size_t row_bytes = (size_t)d * 2, head_pitch = (size_t)N * row_bytes, chunk_bytes = (size_t)kv_chunk * row_bytes;
+  auto up = [&](void* dst, const void* src_, size_t bytes) {
+    return cudaMemcpyAsync(dst, src_, bytes, cudaMemcpyHostToDevice, ov.side);
+  };
+  // ---- host -> device
+  if ((ce = cudaEventRecord(ev_down, stream)) != cudaSuccess) return cuda_status(ce);          // order behind the caller's
+  if ((ce = cudaStreamWaitEvent(ov.side, ev_down, 0)) != cudaSuccess) return cuda_status(ce);  // earlier work on `stream`
+  if ((ce = up(t[0], q_host, tb)) != cudaSuccess) return cuda_status(ce);
+  if (pipelined) {
+    for (int c = 0; c < n_chunks; ++c) {
+      const size_t off = (size_t)c * chunk_bytes;
+      for (int w = 1; w <= 2; ++w) {
+        const char* src_ = static_cast<const char*>(w == 1 ? k_host : v_host) + off;
+        if ((ce = cudaMemcpy2DAsync(static_cast<char*>(t[w]) + off, head_pitch, src_, head_pitch, chunk_bytes, BH,
+                                    cudaMemcpyHostToDevice, ov.side)) != cudaSuccess)
+          return cuda_status(ce);
+      }
+      if ((ce = cudaEventRecord(kv_ready[c], ov.side)) != cudaSuccess) return cuda_status(ce);
+    }
+  } else {
+    if ((ce = up(t[1], k_host, tb)) != cudaSuccess || (ce = up(t[2], v_host, tb)) != cudaSuccess) return cuda_status(ce);
+    if ((ce = cudaEventRecord(ev_fwd_done, ov.side)) != cudaSuccess) return cuda_status(ce);
+    if ((ce = cudaStreamWaitEvent(stream, ev_fwd_done, 0)) != cudaSuccess) return cuda_status(ce);
+  }
+  if ((ce = up(t[3], dO_host, tb)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaEventRecord(ev_do_up, ov.side)) != cudaSuccess) return cuda_status(ce);
+  // ---- forward
+  if (pipelined) tl_hooks.kv_ready = kv_ready;
   st = ringx_attn_fwd(t[0], t[1], t[2], t[4], dlse, B, H, N, d, kv_chunk, scale, dtype, inner, inner_bytes, stream_);
+  tl_hooks.kv_ready = nullptr;
   if (st != RINGX_OK) return st;
   const int fwd_launches = tl_last_launches;
+  if ((ce = cudaEventRecord(ev_fwd_done, stream)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaStreamWaitEvent(ov.side, ev_fwd_done, 0)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaMemcpyAsync(o_host, t[4], tb, cudaMemcpyDeviceToHost, ov.side)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaMemcpyAsync(lse_host, dlse, R * sizeof(float), cudaMemcpyDeviceToHost, ov.side)) != cudaSuccess)
+    return cuda_status(ce);
+  // ---- backward
+  if ((ce = cudaStreamWaitEvent(stream, ev_do_up, 0)) != cudaSuccess) return cuda_status(ce);
+  if (pipelined) tl_hooks.pass_done = pass_done;
   st = ringx_attn_bwd(t[0], t[1], t[2], t[4], dlse, t[3], t[5], t[6], t[7], B, H, N, d, kv_chunk, scale, dtype, inner,
                       inner_bytes, stream_);
+  tl_hooks.pass_done = nullptr;
   if (st != RINGX_OK) return st;
   tl_last_launches += fwd_launches;
-  void* dst[4] = {o_host, dq_host, dk_host, dv_host};
-  for (int i = 0; i < 4; ++i)
-    if ((ce = cudaMemcpyAsync(dst[i], t[4 + i], tb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess)
+  // ---- device -> host (the waits are enqueued after the records they refer to)
+  if (pipelined) {
+    for (int c = 0; c < n_chunks; ++c) {
+      const size_t off = (size_t)c * chunk_bytes;
+      if ((ce = cudaStreamWaitEvent(ov.side, pass_done[c], 0)) != cudaSuccess) return cuda_status(ce);
+      for (int w = 0; w < 2; ++w) {
+        char* dst_ = static_cast<char*>(w == 0 ? dk_host : dv_host) + off;
+        if ((ce = cudaMemcpy2DAsync(dst_, head_pitch, static_cast<const char*>(t[6 + w]) + off, head_pitch, chunk_bytes,
+                                    BH, cudaMemcpyDeviceToHost, ov.side)) != cudaSuccess)
+          return cuda_status(ce);
+      }
+    }
+  } else {
+    if ((ce = cudaMemcpyAsync(dk_host, t[6], tb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(dv_host, t[7], tb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess)
       return cuda_status(ce);
-  if ((ce = cudaMemcpyAsync(lse_host, dlse, R * sizeof(float), cudaMemcpyDeviceToHost, stream)) != cudaSuccess)
-    return cuda_status(ce);
+  }
+  if ((ce = cudaMemcpyAsync(dq_host, t[5], tb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaEventRecord(ev_down, ov.side)) != cudaSuccess) return cuda_status(ce);
+  if ((ce = cudaStreamWaitEvent(stream, ev_down, 0)) != cudaSuccess) return cuda_status(ce);
   if ((ce = cudaStreamSynchronize(stream)) != cudaSuccess) return cuda_status(ce);
   return RINGX_OK;
 }
