@@ -133,6 +133,24 @@ struct HostOverlap {
 };
 thread_local HostOverlap tl_overlap;
 
+// side stream of the current device and at least n_events events (created on first use, then reused)
+int overlap_prepare(HostOverlap& ov, int n_events) {
+  cudaError_t ce;
+  int dev = 0;
+  if ((ce = cudaGetDevice(&dev)) != cudaSuccess) { cudaGetLastError(); return RINGX_ERR_CUDA; }
+  if (!ov.side || ov.device != dev) {      // (objects of another device are abandoned, not reused)
+    ov.device = dev;
+    ov.events.clear();
+    if ((ce = cudaStreamCreateWithFlags(&ov.side, cudaStreamNonBlocking)) != cudaSuccess) { cudaGetLastError(); return RINGX_ERR_CUDA; }
+  }
+  while ((int)ov.events.size() < n_events) {
+    cudaEvent_t e;
+    if ((ce = cudaEventCreateWithFlags(&e, cudaEventDisableTiming)) != cudaSuccess) { cudaGetLastError(); return RINGX_ERR_CUDA; }
+    ov.events.push_back(e);
+  }
+  return RINGX_OK;
+}
+
 // Set by ringx_attn_fwd_bwd_host around its calls of the chunk loops: pass c of the forward waits for kv_ready[c] (the
 // K,V rows of chunk c have arrived from the host); the backward records pass_done[c] after pass c (its dK,dV rows are final).
 struct ChunkHooks {
@@ -571,11 +589,36 @@ int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_ho
   float* dlse = reinterpret_cast<float*>(p + 4 * tba);
   char* inner = p + 4 * tba + align_up(R * sizeof(float));
   const size_t inner_bytes = workspace_bytes - (size_t)(inner - p);
+  // q and the K,V rows of chunk c go up on a side stream in the order the passes need them (pass c waits for chunk c
+  // only), so all but the first chunk's transfer is hidden behind the kernels.
   cudaError_t ce;
-  if ((ce = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
-  if ((ce = cudaMemcpyAsync(dk, k_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
-  if ((ce = cudaMemcpyAsync(dv, v_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+  const int n_chunks = N / kv_chunk;
+  const bool pipelined = n_chunks >= 2 && n_chunks <= 64;
+  if (pipelined) {
+    HostOverlap& ov = tl_overlap;
+    if ((st = overlap_prepare(ov, 3 + 2 * n_chunks)) != RINGX_OK) return st;
+    cudaEvent_t* kv_ready = ov.events.data() + 3;
+    const size_t head_pitch = (size_t)N * d * e, chunk_bytes = (size_t)kv_chunk * d * e;
+    if ((ce = cudaEventRecord(ov.events[2], stream)) != cudaSuccess) return cuda_status(ce);
+    if ((ce = cudaStreamWaitEvent(ov.side, ov.events[2], 0)) != cudaSuccess) return cuda_status(ce);
+    if ((ce = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, ov.side)) != cudaSuccess) return cuda_status(ce);
+    for (int c = 0; c < n_chunks; ++c) {
+      const size_t off = (size_t)c * chunk_bytes;
+      for (int w = 0; w < 2; ++w)
+        if ((ce = cudaMemcpy2DAsync(static_cast<char*>(w == 0 ? dk : dv) + off, head_pitch,
+                                    static_cast<const char*>(w == 0 ? k_host : v_host) + off, head_pitch, chunk_bytes,
+                                    (size_t)B * H, cudaMemcpyHostToDevice, ov.side)) != cudaSuccess)
+          return cuda_status(ce);
+      if ((ce = cudaEventRecord(kv_ready[c], ov.side)) != cudaSuccess) return cuda_status(ce);
+    }
+    tl_hooks.kv_ready = kv_ready;
+  } else {
+    if ((ce = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+    if ((ce = cudaMemcpyAsync(dk, k_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+    if ((ce = cudaMemcpyAsync(dv, v_host, tb, cudaMemcpyHostToDevice, stream)) != cudaSuccess) return cuda_status(ce);
+  }
   st = ringx_attn_fwd(dq, dk, dv, dob, dlse, B, H, N, d, kv_chunk, scale, dtype, inner, inner_bytes, stream_);
+  tl_hooks.kv_ready = nullptr;
   if (st != RINGX_OK) return st;
   if ((ce = cudaMemcpyAsync(o_host, dob, tb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return cuda_status(ce);
   if ((ce = cudaMemcpyAsync(lse_host, dlse, R * sizeof(float), cudaMemcpyDeviceToHost, stream)) != cudaSuccess)
@@ -621,21 +664,9 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   // come down while the later passes run.  Only dq is copied after the last kernel.
   HostOverlap& ov = tl_overlap;
   cudaError_t ce;
-  int dev = 0;
-  if ((ce = cudaGetDevice(&dev)) != cudaSuccess) return cuda_status(ce);
   const int n_chunks = N / kv_chunk;
   const bool pipelined = n_chunks >= 2 && n_chunks <= 64;
-  const int n_events = 3 + (pipelined ? 2 * n_chunks : 0);
-  if (!ov.side || ov.device != dev) {      // (objects of another device are abandoned, not reused)
-    ov.device = dev;
-    ov.events.clear();
-    if ((ce = cudaStreamCreateWithFlags(&ov.side, cudaStreamNonBlocking)) != cudaSuccess) return cuda_status(ce);
-  }
-  while ((int)ov.events.size() < n_events) {
-    cudaEvent_t e;
-    if ((ce = cudaEventCreateWithFlags(&e, cudaEventDisableTiming)) != cudaSuccess) return cuda_status(ce);
-    ov.events.push_back(e);
-  }
+  if ((st = overlap_prepare(ov, 3 + (pipelined ? 2 * n_chunks : 0))) != RINGX_OK) return st;
   cudaEvent_t ev_do_up = ov.events[0], ev_fwd_done = ov.events[1], ev_down = ov.events[2];
   cudaEvent_t* kv_ready = ov.events.data() + 3;
   cudaEvent_t* pass_done = kv_ready + n_chunks;
