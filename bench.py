@@ -485,6 +485,17 @@ def next_rows_measure(ringx, wl, dev, reps=5):
     acc = torch.zeros(ql.shape, dtype=torch.float32, device=dev)
     ms = timeit(lambda: ringx.ringx_attn_bwd_partial(ql, kc, vc, ol, lsel, dol, scale, dq_acc=acc))
     out["bwd_partial_Nq16384_Nk16384_d128"] = {"tflops": 10.0 * B * 4 * 16384 * 16384 * d / ms / 1e9}
+    # split-KV: the paper's per-device regime: 2048 local query tokens x 8 heads = 64 CTAs against a
+    # 65536-key gathered chunk; the library splits the keys over CTA groups and merges by Eq. 5 inside the pass
+    qs = q[:, :8, :2048].contiguous()
+    ks, vs = torch.cat([k, k], dim=2)[:, :, :65536].contiguous(), torch.cat([v, v], dim=2)[:, :, :65536].contiguous()
+    ks = ks.repeat(1, 2, 1, 1).contiguous()
+    vs = vs.repeat(1, 2, 1, 1).contiguous()
+    fls = 4.0 * 8 * 2048 * 65536 * d
+    ms0 = timeit(lambda: ringx.ringx_attn_chunk_fwd(qs, ks, vs, scale))
+    ms1 = timeit(lambda: ringx.ringx_attn_chunk_fwd_ex(qs, ks, vs, scale))
+    out["split_kv_Nq2048_Nk65536_H8_d128"] = {"unsplit_tflops": fls / ms0 / 1e9, "split_tflops": fls / ms1 / 1e9}
+    del qs, ks, vs
     # Eq. 5 with N operands: bytes per row = d*4 read + d*4 written (+ 12 / + 12)
     rows = 1 << 21
     lo = torch.randn(rows, d, device=dev)

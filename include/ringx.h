@@ -135,6 +135,22 @@ RINGX_API int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void
                               void* o_final, float* lse_final,
                               int B, int H, int Nq, int Nk, int d, float scale, int dtype, void* stream);
 
+/* One pass in its general form, with split-KV.  When a pass has too few query tiles to fill the 148 SMs (B*H*Nq/256 CTAs --
+ * the paper's own regime of 2K-64K query tokens per device against a long gathered key sequence, l.262-264) the library splits
+ * the Nk keys over up to 8 groups of CTAs and combines the groups' partial results with Eq. 5 -- the same merge, inside one
+ * pass -- into exactly what the unsplit pass returns (up to rounding order).  Whether it splits is the library's choice
+ * (ringx_attn_chunk_fwd_ex_workspace_bytes returns 0 when it will not); ringx_attn_fwd / ringx_attn_fwd_gqa do the same inside.
+ *   o_acc, lse_acc  NULL: (o_out, lse_out) = (loc_out, loc_lse) of these keys;  else the running fp32 accumulator this pass is
+ *                   folded with by the two-operand Eq. 5.
+ *   o_out, lse_out  result, o_out of o_out_dtype: RINGX_F32 (may be o_acc, lse_acc themselves: in-place fold) or RINGX_BF16
+ *                   (the last pass; must not alias the accumulator).
+ *   workspace       >= ringx_attn_chunk_fwd_ex_workspace_bytes(...) bytes, 256-byte aligned; may be NULL when that is 0.
+ *   bf16 inputs only; Nq % 256 == 0, Nk % 128 == 0, d in {64,128}. */
+RINGX_API int ringx_attn_chunk_fwd_ex(const void* q, const void* k, const void* v, const float* o_acc, const float* lse_acc,
+                            void* o_out, float* lse_out, int B, int H, int Nq, int Nk, int d, float scale,
+                            int dtype, int o_out_dtype, void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_chunk_fwd_ex_workspace_bytes(int B, int H, int Nq, int Nk, int d, int dtype);
+
 /* Per-device backward step of RingX_a / RingX_b (l.143, l.145): the gradient contributions that `Nq` query
  * rows and `Nk` keys of every head exchange, with P recomputed from the *global* lse of those rows (the
  * LSE over ALL keys of the sequence, not only the Nk given here; reading g8 of DESIGN.md).

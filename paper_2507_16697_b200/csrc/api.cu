@@ -69,17 +69,66 @@ int check_shape(int B, int H, int N, int d, int kv_chunk, float scale, int dtype
   return RINGX_OK;
 }
 
+// ---- split-KV: when one chunk pass has too few query tiles to fill the GPU (the paper's own regime: 2K-64K query tokens per
+// device against a long gathered key sequence), the keys of the pass are split over gridDim.z and the
+// splits' partials are combined by Eq. 5 -- the same merge, inside one pass.
+constexpr int kSmCount = 148;          // B200; a constant so that workspace sizes do not depend on a device query
+constexpr int kMaxSplits = 8;
+constexpr int kMinTilesPerSplit = 8;   // >= 1024 keys per split: below that the prologue/epilogue of a CTA dominates
+
+int choose_splits(int BH, int Nq, int nk, int dtype) {
+  if (dtype != RINGX_BF16 || Nq % 256) return 1;
+  const long long ctas = (long long)BH * (Nq / 256);
+  if (ctas >= 2 * kSmCount) return 1;
+  const int tiles = nk / 128;
+  auto eff = [](long long n) { return (double)n / (double)(((n + kSmCount - 1) / kSmCount) * kSmCount); };
+  int best = 1;
+  double best_eff = eff(ctas);
+  for (int s = 2; s <= kMaxSplits; ++s) {
+    if (tiles % s || tiles / s < kMinTilesPerSplit) continue;
+    const double e = eff(ctas * s) * (1.0 - 0.01 * s);     // every split costs one more partial to write and merge
+    if (e > best_eff * 1.05) { best = s; best_eff = e; }
+  }
+  return best;
+}
+
+struct SplitScratch {
+  int splits = 1;
+  float* parts = nullptr;     // [splits][R,d]
+  float* lses = nullptr;      // [splits][R]
+  float* lse_tmp = nullptr;   // [R]: the merged lse when the caller's lse_out aliases lse_acc
+  size_t bytes = 0;
+};
+
+SplitScratch carve_split(void* ws, size_t R, int d, int splits) {
+  SplitScratch sp;
+  sp.splits = splits;
+  if (splits <= 1) return sp;
+  char* p = static_cast<char*>(ws);
+  size_t off = 0;
+  auto take = [&](size_t n) {
+    char* r = p ? p + off : nullptr;
+    off += align_up(n);
+    return r;
+  };
+  sp.parts = reinterpret_cast<float*>(take((size_t)splits * R * d * sizeof(float)));
+  sp.lses = reinterpret_cast<float*>(take((size_t)splits * R * sizeof(float)));
+  sp.lse_tmp = reinterpret_cast<float*>(take(R * sizeof(float)));
+  sp.bytes = off;
+  return sp;
+}
+
 struct FwdWorkspace {
   float* o_acc = nullptr;      // running (merged) output, fp32 [R,d]   (bf16 only; f32 uses `o` itself)
   float* lse_acc = nullptr;    // running LSE [R]                        (bf16 only; f32 uses `lse`)
   float* o_part = nullptr;     // loc_out of the current pass, fp32 [R,d]   (f32 only)
   float* lse_part = nullptr;   // loc_lse of the current pass [R]           (f32 only)
+  SplitScratch split;          // split-KV scratch (splits == 1: none)
   size_t bytes = 0;
 };
 
 FwdWorkspace carve_fwd(void* ws, int B, int H, int N, int d, int kv_chunk, int dtype) {
   FwdWorkspace w;
-  if (kv_chunk == N) return w;   // single pass: the chunk kernel writes (o, lse) directly
   const size_t R = (size_t)B * H * N;
   char* p = static_cast<char*>(ws);
   size_t off = 0;
@@ -88,6 +137,12 @@ FwdWorkspace carve_fwd(void* ws, int B, int H, int N, int d, int kv_chunk, int d
     off += align_up(n);
     return r;
   };
+  w.split = carve_split(nullptr, R, d, choose_splits(B * H, N, kv_chunk, dtype));
+  if (w.split.splits > 1) w.split = carve_split(take(w.split.bytes), R, d, w.split.splits);
+  if (kv_chunk == N) {           // single pass: the chunk kernel writes (o, lse) directly
+    w.bytes = off;
+    return w;
+  }
   if (dtype == RINGX_BF16) {   // the chunk kernel folds each pass into the running accumulator itself
     w.o_acc = reinterpret_cast<float*>(take(R * d * sizeof(float)));
     w.lse_acc = reinterpret_cast<float*>(take(R * sizeof(float)));
@@ -214,14 +269,41 @@ bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, in
 // The fp32 path has the partial epilogue only.
 static cudaError_t chunk_pass(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
                               const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride, int k_off,
-                              int nk, int d, float scale, int dtype, int epilogue, cudaStream_t stream) {
-  Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
-  if (dtype == RINGX_F32)
+                              int nk, int d, float scale, int dtype, int epilogue, cudaStream_t stream,
+                              const SplitScratch* sp = nullptr) {
+  if (dtype == RINGX_F32) {
+    Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
     return launch_attn_chunk_f32(static_cast<const float*>(q), static_cast<const float*>(k),
                                  static_cast<const float*>(v), static_cast<float*>(o_out), lse_out, BH, Nq, nk_stride,
                                  k_off, nk, d, scale, stream);
-  return launch_attn_chunk_fwd_sm100(q, k, v, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, d, scale,
-                                     epilogue, stream);
+  }
+  if (!sp || sp->splits <= 1) {
+    Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
+    return launch_attn_chunk_fwd_sm100(q, k, v, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, d, scale,
+                                       epilogue, 1, stream);
+  }
+  // split-KV: gridDim.z splits of the keys write fp32 partials, one Eq. 5 kernel combines them (and the running
+  // accumulator, for the fold epilogues) into what the unsplit pass would have produced
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
+    e = launch_attn_chunk_fwd_sm100(q, k, v, sp->parts, sp->lses, nullptr, nullptr, BH, Nq, nk_stride, k_off, nk, d, scale,
+                                    kFwdEpiPartial, sp->splits, stream);
+  }
+  if (e != cudaSuccess) return e;
+  const bool fold = epilogue == kFwdEpiFold || epilogue == kFwdEpiFoldFinal;
+  const bool out_bf16 = epilogue == kFwdEpiFinal || epilogue == kFwdEpiFoldFinal;
+  const long long R = (long long)BH * Nq;
+  float* lse_dst = (fold && lse_out == lse_acc) ? sp->lse_tmp : lse_out;   // other threads of a row still read lse_acc
+  {
+    Timed timed(RINGX_PROFILE_MERGE, stream);
+    e = launch_split_merge(sp->parts, sp->lses, R, d, sp->splits, fold ? o_acc : nullptr, fold ? lse_acc : nullptr, o_out,
+                           lse_dst, out_bf16 ? RINGX_BF16 : RINGX_F32, stream);
+  }
+  count_launch();
+  if (e != cudaSuccess) return e;
+  if (lse_dst != lse_out) e = cudaMemcpyAsync(lse_out, lse_dst, (size_t)R * sizeof(float), cudaMemcpyDeviceToDevice, stream);
+  return e;
 }
 
 }  // namespace ringx
@@ -255,7 +337,8 @@ static int fwd_core(const void* q, const void* k, const void* v, void* o, float*
   const long long R = (long long)BH * Nq;
   const int n_chunks = N / kv_chunk;
   if (n_chunks == 1) {
-    cudaError_t e = chunk_pass(q, k, v, o, lse, nullptr, nullptr, BH, Nq, N, 0, N, d, scale, dtype, kFwdEpiFinal, stream);
+    cudaError_t e = chunk_pass(q, k, v, o, lse, nullptr, nullptr, BH, Nq, N, 0, N, d, scale, dtype, kFwdEpiFinal, stream,
+                               &w.split);
     return e == cudaSuccess ? RINGX_OK : cuda_status(e);
   }
   for (int c = 0; c < n_chunks; ++c) {
@@ -267,13 +350,13 @@ static int fwd_core(const void* q, const void* k, const void* v, void* o, float*
       // fp32 in the workspace; the last pass writes the caller's bf16 o and lse
       if (first)
         e = chunk_pass(q, k, v, w.o_acc, w.lse_acc, nullptr, nullptr, BH, Nq, N, 0, kv_chunk, d, scale, dtype,
-                       kFwdEpiPartial, stream);
+                       kFwdEpiPartial, stream, &w.split);
       else if (!last)
         e = chunk_pass(q, k, v, w.o_acc, w.lse_acc, w.o_acc, w.lse_acc, BH, Nq, N, c * kv_chunk, kv_chunk, d, scale,
-                       dtype, kFwdEpiFold, stream);
+                       dtype, kFwdEpiFold, stream, &w.split);
       else
         e = chunk_pass(q, k, v, o, lse, w.o_acc, w.lse_acc, BH, Nq, N, c * kv_chunk, kv_chunk, d, scale, dtype,
-                       kFwdEpiFoldFinal, stream);
+                       kFwdEpiFoldFinal, stream, &w.split);
       if (e != cudaSuccess) return cuda_status(e);
       continue;
     }
@@ -369,6 +452,46 @@ int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void* v, float
                                        kFwdEpiFoldFinal, stream)
                           : chunk_pass(q, k, v, o_acc, lse_acc, o_acc, lse_acc, B * H, Nq, Nk, 0, Nk, d, scale, dtype,
                                        kFwdEpiFold, stream);
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+size_t ringx_attn_chunk_fwd_ex_workspace_bytes(int B, int H, int Nq, int Nk, int d, int dtype) {
+  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128) || Nk % 128) return 0;
+  return carve_split(nullptr, (size_t)B * H * Nq, d, choose_splits(B * H, Nq, Nk, dtype)).bytes;
+}
+
+int ringx_attn_chunk_fwd_ex(const void* q, const void* k, const void* v, const float* o_acc, const float* lse_acc,
+                            void* o_out, float* lse_out, int B, int H, int Nq, int Nk, int d, float scale, int dtype,
+                            int o_out_dtype, void* workspace, size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o_out || !lse_out || (o_acc == nullptr) != (lse_acc == nullptr)) return RINGX_ERR_NULL_PTR;
+  if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (o_out_dtype != RINGX_F32 && o_out_dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
+  if (Nk % 128 || Nq % 256) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
+    return RINGX_ERR_BAD_SHAPE;
+  if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o_acc) || !aligned16(lse_acc) || !aligned16(o_out) ||
+      !aligned16(lse_out))
+    return RINGX_ERR_MISALIGNED;
+  if (o_acc && o_out_dtype == RINGX_BF16 && (o_out == static_cast<const void*>(o_acc) || lse_out == lse_acc))
+    return RINGX_ERR_BAD_SHAPE;              // a bf16 result cannot overwrite the fp32 accumulator
+  const size_t need = ringx_attn_chunk_fwd_ex_workspace_bytes(B, H, Nq, Nk, d, dtype);
+  if (need) {
+    if (!workspace) return RINGX_ERR_NULL_PTR;
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+    if (workspace_bytes < need) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  }
+  int st = check_arch();
+  if (st != RINGX_OK) return st;
+  tl_launches = 0;
+  const SplitScratch sp = carve_split(workspace, (size_t)B * H * Nq, d, choose_splits(B * H, Nq, Nk, dtype));
+  const int epi = o_acc ? (o_out_dtype == RINGX_BF16 ? kFwdEpiFoldFinal : kFwdEpiFold)
+                        : (o_out_dtype == RINGX_BF16 ? kFwdEpiFinal : kFwdEpiPartial);
+  cudaError_t e = chunk_pass(q, k, v, o_out, lse_out, o_acc, lse_acc, B * H, Nq, Nk, 0, Nk, d, scale, dtype, epi, stream, &sp);
   if (e != cudaSuccess) return cuda_status(e);
   tl_last_launches = tl_launches;
   return RINGX_OK;
@@ -905,6 +1028,6 @@ const char* ringx_status_string(int status) {
   }
 }
 
-int ringx_version(void) { return 130; }
+int ringx_version(void) { return 140; }
 
 }  // extern "C"

@@ -104,7 +104,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   const int lane = threadIdx.x & 31;
   const int bh = blockIdx.y;
   const int q_row0 = bh * Nq + blockIdx.x * (2 * kBlockM);     // row in the [BH*Nq, d] view
-  const int k_row0 = bh * nk_stride + k_off;
+  const int k_row0 = bh * nk_stride + k_off + blockIdx.z * n_kv * kBlockN;   // blockIdx.z = key split (split-KV)
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
@@ -359,7 +359,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     // ---- chunk epilogue: loc_out = O / l, loc_lse = m*scale + ln l  (natural log of the scaled scores)
     mbar_wait(&o_full[t], 0);
     tc_fence_after();
-    const size_t row = static_cast<size_t>(q_row0) + t * kBlockM + (warp & 3) * 32 + lane;
+    size_t row = static_cast<size_t>(q_row0) + t * kBlockM + (warp & 3) * 32 + lane;
+    if (kEpi == kEpiPartial) row += static_cast<size_t>(blockIdx.z) * gridDim.y * Nq;   // this split's partials
     constexpr bool kFold = kEpi == kEpiFold || kEpi == kEpiFoldFinal;
     constexpr bool kOutBf16 = kEpi == kEpiFinal || kEpi == kEpiFoldFinal;
     float lse_row = (m_sc + lg2(l)) * 0.6931471805599453f;
@@ -426,7 +427,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 template <int kD, int kEpi>
 cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, void* o_out, float* lse_out,
                      const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride, int k_off, int nk,
-                     float scale, cudaStream_t stream) {
+                     float scale, int splits, cudaStream_t stream) {
   using Cfg = FwdCfg<kD>;
   auto kern = attn_chunk_fwd_kernel<kD, kEpi>;
   static bool configured = false;   // benign race: the attribute is idempotent
@@ -435,9 +436,9 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 grid(Nq / (2 * kBlockM), BH);
+  dim3 grid(Nq / (2 * kBlockM), BH, splits);
   kern<<<grid, kFwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, Nq, nk_stride, k_off,
-                                                       nk / kBlockN, scale * 1.4426950408889634f);
+                                                       nk / kBlockN / splits, scale * 1.4426950408889634f);
   count_launch();
   return cudaGetLastError();
 }
@@ -445,16 +446,16 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
 template <int kD>
 cudaError_t launch_d(int epi, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, void* o_out,
                      float* lse_out, const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride, int k_off,
-                     int nk, float scale, cudaStream_t stream) {
+                     int nk, float scale, int splits, cudaStream_t stream) {
   switch (epi) {
     case kEpiPartial:
-      return launch_t<kD, kEpiPartial>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+      return launch_t<kD, kEpiPartial>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, splits, stream);
     case kEpiFinal:
-      return launch_t<kD, kEpiFinal>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+      return launch_t<kD, kEpiFinal>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, splits, stream);
     case kEpiFold:
-      return launch_t<kD, kEpiFold>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+      return launch_t<kD, kEpiFold>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, splits, stream);
     default:
-      return launch_t<kD, kEpiFoldFinal>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+      return launch_t<kD, kEpiFoldFinal>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, splits, stream);
   }
 }
 
@@ -462,15 +463,17 @@ cudaError_t launch_d(int epi, const CUtensorMap& mq, const CUtensorMap& mk, cons
 
 cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
                                         const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride,
-                                        int k_off, int nk, int d, float scale, int epilogue, cudaStream_t stream) {
+                                        int k_off, int nk, int d, float scale, int epilogue, int splits,
+                                        cudaStream_t stream) {
+  if (splits < 1 || (splits > 1 && epilogue != kFwdEpiPartial) || (nk / 128) % splits) return cudaErrorInvalidValue;
   CUtensorMap mq, mk, mv;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   if (!make_tmap_2d(&mq, q, dt, 2, (uint64_t)BH * Nq, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mk, k, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mv, v, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64) return launch_d<64>(epilogue, mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
-  return launch_d<128>(epilogue, mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, stream);
+  if (d == 64) return launch_d<64>(epilogue, mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, splits, stream);
+  return launch_d<128>(epilogue, mq, mk, mv, o_out, lse_out, o_acc, lse_acc, BH, Nq, nk_stride, k_off, nk, scale, splits, stream);
 }
 
 }  // namespace ringx

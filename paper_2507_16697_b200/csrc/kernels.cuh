@@ -20,6 +20,13 @@ cudaError_t launch_eq5_scale(const float* loc_out, const float* loc_lse, const f
                              long long rows, int d, cudaStream_t stream);
 cudaError_t launch_eq5_finalize(const float* num, const float* den, const float* lse_max, void* o_out, float* lse_out,
                                 long long rows, int d, int out_dtype, cudaStream_t stream);
+// Eq. 5 over the `splits` (<= 8) key splits of one chunk pass: parts [splits][rows,d], lses [splits][rows] fp32, and --
+// when o_acc != nullptr -- the running (o_acc, lse_acc) as one more operand.  o_out [rows,d] of out_dtype (may alias
+// o_acc when fp32: a thread reads its float4 before writing it), lse_out [rows] (may alias lse_acc only when d == 4...
+// it must NOT alias lse_acc: other threads of the row still read it).
+cudaError_t launch_split_merge(const float* parts, const float* lses, long long rows, int d, int splits,
+                               const float* o_acc, const float* lse_acc, void* o_out, float* lse_out, int out_dtype,
+                               cudaStream_t stream);
 // D = scale * rowsum(dO*O), lse2 = lse * log2(e); zeroes dq_acc when zero_dq.
 cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* lse, float* D, float* lse2,
                                   float* dq_acc, long long rows, int d, float scale, bool zero_dq,
@@ -48,9 +55,12 @@ cudaError_t launch_attn_chunk_f32(const float* q, const float* k, const float* v
 //   2 folded by the two-operand Eq. 5 into the running fp32 (o_acc, lse_acc); o_out == o_acc, lse_out == lse_acc
 //   3 folded with (o_acc, lse_acc) and written to (o_out bf16, lse_out): the last pass
 enum { kFwdEpiPartial = 0, kFwdEpiFinal = 1, kFwdEpiFold = 2, kFwdEpiFoldFinal = 3 };
+// splits > 1 (kFwdEpiPartial only): split z of the grid takes keys [k_off + z*nk/splits, +nk/splits) and writes its
+// partials to o_out + z*BH*Nq*d, lse_out + z*BH*Nq (launch_split_merge combines them).
 cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
                                         const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride,
-                                        int k_off, int nk, int d, float scale, int epilogue, cudaStream_t stream);
+                                        int k_off, int nk, int d, float scale, int epilogue, int splits,
+                                        cudaStream_t stream);
 
 // ---- attn_bwd_sm100.cu (tcgen05 path)
 // One KV-chunk pass of the backward: q,dO [BH,N,d], k,v,dk,dv [BH,nk_stride,d]; writes dk,dv rows

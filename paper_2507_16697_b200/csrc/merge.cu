@@ -187,6 +187,48 @@ eq5_finalize_kernel(const float4* __restrict__ num, const float* __restrict__ de
   }
 }
 
+// Eq. 5 over the s key splits of one chunk pass (split-KV), optionally with the running (o_acc, lse_acc) as one more
+// operand: parts [s][rows,d] fp32, lses [s][rows].  One thread per float4; s <= kMaxSplits so the weights sit in
+// registers.  An operand with lse = -inf has weight 0; every operand empty gives o = 0, lse = -inf.
+constexpr int kMaxSplits = 8;
+template <typename TOut>
+__global__ void __launch_bounds__(256)
+split_merge_kernel(const float4* __restrict__ parts, const float* __restrict__ lses, long long part_stride_vecs,
+                   long long rows, int s, const float4* __restrict__ o_acc, const float* __restrict__ lse_acc,
+                   void* __restrict__ o_out, float* __restrict__ lse_out, int vecs) {
+  const long long total = rows * vecs, stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
+    const long long r = i / vecs;
+    float l[kMaxSplits + 1];
+    float m = -INFINITY;
+#pragma unroll
+    for (int p = 0; p < kMaxSplits; ++p) {
+      l[p] = p < s ? lses[p * rows + r] : -INFINITY;
+      m = fmaxf(m, l[p]);
+    }
+    l[kMaxSplits] = lse_acc ? lse_acc[r] : -INFINITY;
+    m = fmaxf(m, l[kMaxSplits]);
+    const float ms = (m == -INFINITY) ? 0.f : m;
+    float den = 0.f;
+    float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int p = 0; p <= kMaxSplits; ++p) {
+      if (l[p] == -INFINITY && !(l[p] != l[p])) continue;            // empty operand: weight 0, data not read
+      const float w = __expf(l[p] - ms);
+      const float4 v = p < kMaxSplits ? __ldcs(parts + p * part_stride_vecs + i) : __ldcs(o_acc + i);
+      den += w;
+      num.x = fmaf(w, v.x, num.x); num.y = fmaf(w, v.y, num.y); num.z = fmaf(w, v.z, num.z); num.w = fmaf(w, v.w, num.w);
+    }
+    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (den != 0.f) {
+      const float inv = 1.0f / den;
+      o = make_float4(num.x * inv, num.y * inv, num.z * inv, num.w * inv);
+    }
+    Vec4<TOut>::store(o_out, (size_t)i, o);
+    if (i - r * vecs == 0) lse_out[r] = den != 0.f ? ms + logf(den) : -INFINITY;
+  }
+}
+
 // ---------------------------------------------------------------- backward helpers
 // D_i = sum_c dO_ic * O_ic (fp32), one 16-lane (d=64: 8 B/lane... ) group per row: each lane takes
 // 8 bf16 (16 B) of dO and of O; d/8 lanes per row.  Stores scale * D_i; zeroes the row of the fp32 dQ accumulator
@@ -288,6 +330,21 @@ cudaError_t launch_eq5_finalize(const float* num, const float* den, const float*
   else
     eq5_finalize_kernel<float><<<eq5_blocks(rows * (d / 4)), 256, 0, stream>>>((const float4*)num, den, lse_max, o_out,
                                                                                 lse_out, rows, d / 4);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_split_merge(const float* parts, const float* lses, long long rows, int d, int splits,
+                               const float* o_acc, const float* lse_acc, void* o_out, float* lse_out, int out_dtype,
+                               cudaStream_t stream) {
+  if (rows == 0) return cudaSuccess;
+  if (splits < 1 || splits > kMaxSplits) return cudaErrorInvalidValue;
+  const int vecs = d / 4;
+  if (out_dtype == RINGX_BF16)
+    split_merge_kernel<__nv_bfloat16><<<eq5_blocks(rows * vecs), 256, 0, stream>>>(
+        (const float4*)parts, lses, rows * vecs, rows, splits, (const float4*)o_acc, lse_acc, o_out, lse_out, vecs);
+  else
+    split_merge_kernel<float><<<eq5_blocks(rows * vecs), 256, 0, stream>>>(
+        (const float4*)parts, lses, rows * vecs, rows, splits, (const float4*)o_acc, lse_acc, o_out, lse_out, vecs);
   return cudaGetLastError();
 }
 

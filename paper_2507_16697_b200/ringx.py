@@ -50,6 +50,10 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_fwd_bwd_host.restype = c_i
     L.ringx_attn_chunk_fwd_fold.argtypes = [c_p] * 7 + [c_i] * 5 + [c_f, c_i, c_p]
     L.ringx_attn_chunk_fwd_fold.restype = c_i
+    L.ringx_attn_chunk_fwd_ex.argtypes = [c_p] * 7 + [c_i] * 5 + [c_f, c_i, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_chunk_fwd_ex.restype = c_i
+    L.ringx_attn_chunk_fwd_ex_workspace_bytes.argtypes = [c_i] * 6
+    L.ringx_attn_chunk_fwd_ex_workspace_bytes.restype = c_sz
     L.ringx_attn_fwd_gqa.argtypes = [c_p] * 5 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_fwd_gqa.restype = c_i
     L.ringx_attn_bwd_gqa.argtypes = [c_p] * 9 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
@@ -158,6 +162,40 @@ def ringx_attn_chunk_fwd(q, k, v, scale: float):
                                     _dev(loc_lse, "loc_lse"), B, H, Nq, Nk, d, scale, _DTYPES[q.dtype], _stream())
     _check(st, "ringx_attn_chunk_fwd")
     return loc_out, loc_lse
+
+
+def ringx_attn_chunk_fwd_ex_workspace_bytes(B, H, Nq, Nk, d, dtype) -> int:
+    return lib().ringx_attn_chunk_fwd_ex_workspace_bytes(B, H, Nq, Nk, d, _DTYPES[dtype])
+
+
+def ringx_attn_chunk_fwd_ex(q, k, v, scale: float, o_acc=None, lse_acc=None, final: bool = False, workspace=None):
+    """One pass in its general form, with split-KV when the pass cannot fill the GPU (include/ringx.h:
+    ringx_attn_chunk_fwd_ex).  No accumulator: returns (loc_out fp32, loc_lse), or (o bf16, lse) when final.  With
+    (o_acc, lse_acc): folds this pass in -- in place (returns them) or, when final, into a new (o bf16, lse)."""
+    B, H, Nq, d = q.shape
+    Nk = k.shape[2]
+    if (o_acc is None) != (lse_acc is None):
+        raise ValueError("o_acc and lse_acc go together")
+    if final:
+        o_out = torch.empty((B, H, Nq, d), dtype=torch.bfloat16, device=q.device)
+        lse_out = torch.empty((B, H, Nq), dtype=torch.float32, device=q.device)
+    elif o_acc is not None:
+        o_out, lse_out = o_acc, lse_acc
+    else:
+        o_out = torch.empty((B, H, Nq, d), dtype=torch.float32, device=q.device)
+        lse_out = torch.empty((B, H, Nq), dtype=torch.float32, device=q.device)
+    need = lib().ringx_attn_chunk_fwd_ex_workspace_bytes(B, H, Nq, Nk, d, _DTYPES[q.dtype])
+    if workspace is None and need:
+        workspace = _workspace(need, q.device)
+    st = lib().ringx_attn_chunk_fwd_ex(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"),
+                                       _dev(o_acc, "o_acc") if o_acc is not None else None,
+                                       _dev(lse_acc, "lse_acc") if lse_acc is not None else None,
+                                       _dev(o_out, "o_out"), _dev(lse_out, "lse_out"), B, H, Nq, Nk, d, scale,
+                                       _DTYPES[q.dtype], _DTYPES[o_out.dtype],
+                                       workspace.data_ptr() if workspace is not None else None,
+                                       workspace.numel() if workspace is not None else 0, _stream())
+    _check(st, "ringx_attn_chunk_fwd_ex")
+    return o_out, lse_out
 
 
 def ringx_lse_merge(o_a, lse_a, o_b, lse_b, out_dtype=None, inplace: bool = False):

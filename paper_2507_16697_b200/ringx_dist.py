@@ -39,10 +39,12 @@ class CudaOps:
         return self.rx.ringx_attn_fwd(q, k, v, q.shape[2], scale)
 
     def chunk_fwd(self, q, k, v, scale):                      # (loc_out fp32, loc_lse)
+        if q.dtype == torch.bfloat16:                         # split-KV when the local chunk cannot fill the GPU
+            return self.rx.ringx_attn_chunk_fwd_ex(q, k, v, scale)
         return self.rx.ringx_attn_chunk_fwd(q, k, v, scale)
 
     def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final):   # chunk pass + two-operand Eq. 5 in one kernel
-        return self.rx.ringx_attn_chunk_fwd_fold(q, k, v, o_acc, lse_acc, scale, final=final)
+        return self.rx.ringx_attn_chunk_fwd_ex(q, k, v, scale, o_acc=o_acc, lse_acc=lse_acc, final=final)
 
     def eq5_scale(self, loc_out, loc_lse, lse_max):           # num, den of one operand (in place on loc_out)
         return self.rx.ringx_eq5_scale(loc_out, loc_lse, lse_max, inplace=True)

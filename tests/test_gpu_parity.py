@@ -172,7 +172,10 @@ def test_fwd_bf16_matches_oracle(rx, B, H, N, d, chunk, gain):
     scale = 1.0 / math.sqrt(d)
     o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), chunk, scale)
     n_c = N // chunk
-    assert rx.ringx_last_launch_count() == n_c        # bf16: the Eq. 5 fold runs in the chunk kernel's epilogue
+    # bf16: the Eq. 5 fold runs in the chunk kernel's epilogue; a pass too small to fill the GPU is split over the keys
+    # (split-KV) and costs one more launch, the Eq. 5 kernel over the splits
+    split = rx.ringx_attn_chunk_fwd_ex_workspace_bytes(B, H, N, chunk, d, torch.bfloat16) > 0
+    assert rx.ringx_last_launch_count() == n_c * (2 if split else 1)
     o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
     check_fwd(o, lse, o_ref, lse_ref, f64(v), "bf16")
 

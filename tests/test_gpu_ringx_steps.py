@@ -375,3 +375,62 @@ def test_gqa_forward_and_backward_match_oracle(rx, Hq, Hkv, N, d, chunk):
     L = rx.lib()
     assert L.ringx_attn_fwd_gqa(qd.data_ptr(), kd.data_ptr(), vd.data_ptr(), o.data_ptr(), lse.data_ptr(), B, 5, 2, N, d,
                                 chunk, scale, 1, None, 0, None) == 2          # Hq % Hkv != 0: BAD_SHAPE
+
+
+# ------------------------------------------------------------------------------------------------ split-KV
+@pytest.mark.parametrize("B,H,Nq,Nk,d", [(1, 2, 256, 4096, 128), (1, 4, 512, 8192, 64), (2, 1, 256, 3072, 128),
+                                         (1, 8, 2048, 16384, 128)])
+def test_chunk_fwd_ex_split_kv_matches_the_oracle(rx, B, H, Nq, Nk, d):
+    """Few query tiles against many keys (the paper's per-device regime): the library splits the keys
+    over groups of CTAs and combines the groups by Eq. 5 inside the pass.  All four result forms against the oracle:
+    partial, final bf16, in-place fold with a running accumulator, final fold."""
+    scale = 1.0 / math.sqrt(d)
+    assert rx.ringx_attn_chunk_fwd_ex_workspace_bytes(B, H, Nq, Nk, d, torch.bfloat16) > 0      # it does split here
+    q = wl.make_tensor((B, H, Nq, d), "q", seed=5, dtype="bf16")
+    k = wl.make_tensor((B, H, Nk, d), "k", seed=5, dtype="bf16")
+    v = wl.make_tensor((B, H, Nk, d), "v", seed=5, dtype="bf16")
+    qd, kd, vd = q.cuda(), k.cuda(), v.cuda()
+    q64, k64, v64 = f64(q), f64(k), f64(v)
+    o_ref = np.empty((B, H, Nq, d))
+    l_ref = np.empty((B, H, Nq))
+    for b in range(B):
+        for h in range(H):
+            o_ref[b, h], l_ref[b, h] = orc.attention_fwd(q64[b, h], k64[b, h], v64[b, h], scale)
+    vmax = np.abs(v64).max()
+
+    def check(o, lse, what):
+        o = o.float().cpu().numpy()
+        assert np.abs(o - o_ref).max() <= 1e-2 * vmax, what
+        assert relf(o, o_ref) <= (1e-2 if o.dtype != np.float32 or what.endswith("bf16") else 5e-3), what
+        assert np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-3, what
+
+    lo, ll = rx.ringx_attn_chunk_fwd_ex(qd, kd, vd, scale)
+    assert rx.ringx_last_launch_count() == 2 and lo.dtype == torch.float32      # split chunk kernel + Eq. 5 kernel
+    check(lo, ll, "partial")
+    o, lse = rx.ringx_attn_chunk_fwd_ex(qd, kd, vd, scale, final=True)
+    check(o, lse, "final bf16")
+    # the unsplit kernel gives the same partials up to rounding (P is rounded to bf16 against a different running max)
+    lo1, ll1 = rx.ringx_attn_chunk_fwd(qd, kd, vd, scale)
+    assert (lo - lo1).abs().max().item() <= 1e-2 * lo1.abs().max().item() and (ll - ll1).abs().max().item() <= 1e-5
+    # fold: first half of the keys as the running accumulator, second half folded in with split-KV
+    half = Nk // 2
+    ka, kb, va, vb = kd[:, :, :half].contiguous(), kd[:, :, half:].contiguous(), vd[:, :, :half].contiguous(), vd[:, :, half:].contiguous()
+    acc_o, acc_l = rx.ringx_attn_chunk_fwd_ex(qd, ka, va, scale)
+    o2, l2 = rx.ringx_attn_chunk_fwd_ex(qd, kb, vb, scale, o_acc=acc_o.clone(), lse_acc=acc_l.clone(), final=True)
+    check(o2, l2, "fold final bf16")
+    o3, l3 = rx.ringx_attn_chunk_fwd_ex(qd, kb, vb, scale, o_acc=acc_o, lse_acc=acc_l)
+    assert o3.data_ptr() == acc_o.data_ptr() and l3.data_ptr() == acc_l.data_ptr()
+    check(o3, l3, "fold in place")
+
+
+def test_attn_fwd_uses_split_kv_when_the_pass_is_small(rx):
+    """ringx_attn_fwd with few query tiles: same result as the oracle through the split path (single pass and chunked)."""
+    B, H, N, d = 1, 2, 4096, 128
+    scale = 1.0 / math.sqrt(d)
+    q, k, v = wl.make_qkv((B, H, N, d), seed=9, dtype="bf16")
+    q64, k64, v64 = f64(q), f64(k), f64(v)
+    o_ref, l_ref = orc.attention_fwd_bhnd(q64, k64, v64, scale)
+    for chunk, launches in ((4096, 2), (2048, 4)):
+        o, lse = rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), chunk, scale)
+        assert rx.ringx_last_launch_count() == launches
+        assert relf(o.float().cpu().numpy(), o_ref) <= 1e-2 and np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-3
