@@ -1,0 +1,86 @@
+"""RingX attention as a drop-in for `torch.nn.functional.scaled_dot_product_attention` ("RingX is a
+standalone attention module that can be used as a drop-in replacement for the scaled_dot_product_attention in PyTorch").
+
+`ringx_sdpa(q, k, v, scale=None, kv_chunk=None, ...)` is a `torch.autograd.Function` whose forward and backward are the
+libringx entry points (`ringx_attn_fwd[_gqa]`, `ringx_attn_bwd[_gqa]`); with a `torch.distributed` group it runs the
+paper's RingX_b or RingX_a schedule (`ringx_dist`) on the local sequence chunks instead.  Argument marshalling only: no
+arithmetic of the method lives here, and there is no fallback -- non-CUDA tensors, masks, dropout and causal attention
+(none of which the paper's attention has) raise.
+"""
+from __future__ import annotations
+
+import math
+
+import torch
+
+from . import ringx, ringx_dist
+
+
+def _default_chunk(n: int) -> int:
+    """KV-chunk length when the caller names none: the largest of 32768..128 that divides N (kv_chunk doubles as the
+    L2-blocking parameter; one head's K,V chunk of 32768 x 128 bf16 is 16.8 MB of the 126 MB L2)."""
+    c = 32768
+    while c > 128 and n % c:
+        c //= 2
+    return c if n % c == 0 else n
+
+
+class _RingXAttention(torch.autograd.Function):
+    @staticmethod
+    def forward(ctx, q, k, v, scale, kv_chunk):
+        q, k, v = q.contiguous(), k.contiguous(), v.contiguous()
+        if q.shape[1] == k.shape[1]:
+            o, lse = ringx.ringx_attn_fwd(q, k, v, kv_chunk, scale)
+        else:
+            o, lse = ringx.ringx_attn_fwd_gqa(q, k, v, kv_chunk, scale)
+        ctx.save_for_backward(q, k, v, o, lse)
+        ctx.scale, ctx.kv_chunk = scale, kv_chunk
+        return o
+
+    @staticmethod
+    def backward(ctx, dO):
+        q, k, v, o, lse = ctx.saved_tensors
+        dO = dO.contiguous()
+        if q.shape[1] == k.shape[1]:
+            dq, dk, dv = ringx.ringx_attn_bwd(q, k, v, o, lse, dO, ctx.kv_chunk, ctx.scale)
+        else:
+            dq, dk, dv = ringx.ringx_attn_bwd_gqa(q, k, v, o, lse, dO, ctx.kv_chunk, ctx.scale)
+        return dq, dk, dv, None, None
+
+
+class _RingXDistAttention(torch.autograd.Function):
+    """q, k, v are this rank's sequence chunks [B,H,N/W,d]; the schedule is RingX_b (default) or RingX_a."""
+
+    @staticmethod
+    def forward(ctx, q, k, v, scale, schedule, comm, ops):
+        fwd = ringx_dist.ringx_b_forward if schedule == "b" else ringx_dist.ringx_a_forward
+        o, _lse, saved = fwd(q.contiguous(), k.contiguous(), v.contiguous(), scale, comm=comm, ops=ops)
+        ctx.saved, ctx.schedule, ctx.comm, ctx.ops = saved, schedule, comm, ops
+        return o
+
+    @staticmethod
+    def backward(ctx, dO):
+        bwd = ringx_dist.ringx_b_backward if ctx.schedule == "b" else ringx_dist.ringx_a_backward
+        dq, dk, dv = bwd(ctx.saved, dO.contiguous(), comm=ctx.comm, ops=ctx.ops)
+        return dq, dk, dv, None, None, None, None
+
+
+def ringx_sdpa(query, key, value, attn_mask=None, dropout_p: float = 0.0, is_causal: bool = False, scale=None,
+               enable_gqa: bool = False, *, kv_chunk: int | None = None, schedule: str | None = None, comm=None, ops=None):
+    """softmax(scale * Q K^T) V with the signature of torch's scaled_dot_product_attention.
+
+    query [B,Hq,N,d], key/value [B,Hkv,N,d] (Hkv divides Hq: grouped-query attention needs enable_gqa=True, as in
+    torch), bf16 or fp32 CUDA tensors, d in {64,128}.  `scale` defaults to 1/sqrt(d).  `kv_chunk`: keys per pass.
+    `schedule` = "b" or "a" runs the paper's RingX_b / RingX_a over `comm` (default: the torch.distributed world)
+    with the arguments being the local sequence chunks."""
+    if attn_mask is not None or dropout_p != 0.0 or is_causal:
+        raise NotImplementedError("RingX attention is non-causal, unmasked and has no dropout (PAPER.md:174-179)")
+    if query.shape[1] != key.shape[1] and not enable_gqa:
+        raise ValueError("query and key have different head counts: pass enable_gqa=True")
+    scale = 1.0 / math.sqrt(query.shape[-1]) if scale is None else float(scale)
+    if schedule is not None:
+        if schedule not in ("a", "b"):
+            raise ValueError("schedule must be 'a', 'b' or None")
+        return _RingXDistAttention.apply(query, key, value, scale, schedule, comm, ops)
+    kv_chunk = _default_chunk(key.shape[2]) if kv_chunk is None else kv_chunk
+    return _RingXAttention.apply(query, key, value, scale, kv_chunk)

@@ -97,16 +97,23 @@ def _worker(rank, world, port, variant, out):
         fwd, bwd = ((ringx_dist.ringx_a_forward, ringx_dist.ringx_a_backward) if variant == "a" else
                     (ringx_dist.ringx_b_forward, ringx_dist.ringx_b_backward))
         ops = OracleOps()
-        o, lse, ctx = fwd(ql, kl, vl, 0.5, ops=ops)
-        dq, dk, dv = bwd(ctx, dOl, ops=ops)
+        if variant.startswith("sdpa_"):          # the autograd drop-in over the same schedules
+            from paper_2507_16697_b200.sdpa import ringx_sdpa
+            ql, kl, vl = (t.requires_grad_() for t in (ql, kl, vl))
+            o = ringx_sdpa(ql, kl, vl, scale=0.5, schedule=variant[-1], ops=ops)
+            o.backward(dOl)
+            lse = torch.from_numpy(orc.attention_fwd_bhnd(q, k, v, 0.5)[1][:, :, sl].copy())   # (sdpa returns o only)
+            o, dq, dk, dv = o.detach(), ql.grad, kl.grad, vl.grad
+        else:
+            o, lse, ctx = fwd(ql, kl, vl, 0.5, ops=ops)
+            dq, dk, dv = bwd(ctx, dOl, ops=ops)
         out.put((rank, [t.numpy().copy() for t in (o, lse, dq, dk, dv)]))
         dist.barrier()
     finally:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("variant", ["a", "b"])
-@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("variant,world", [("a", 2), ("b", 2), ("a", 3), ("b", 3), ("sdpa_a", 2), ("sdpa_b", 2)])
 def test_ringx_schedules_equal_the_unchunked_attention(variant, world):
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
@@ -129,6 +136,22 @@ def test_ringx_schedules_equal_the_unchunked_attention(variant, world):
         np.testing.assert_allclose(lse, lse_ref[:, :, sl], atol=1e-12)
         for g, ref in zip((dq, dk, dv), grads_ref):
             np.testing.assert_allclose(g, ref[:, :, sl], atol=1e-12)
+
+
+def test_sdpa_drop_in_rejects_what_the_papers_attention_does_not_have():
+    from paper_2507_16697_b200.sdpa import ringx_sdpa, _default_chunk
+    t = torch.zeros(1, 2, 256, 64, dtype=torch.bfloat16)
+    with pytest.raises(NotImplementedError):
+        ringx_sdpa(t, t, t, is_causal=True)
+    with pytest.raises(NotImplementedError):
+        ringx_sdpa(t, t, t, attn_mask=torch.ones(256, 256, dtype=torch.bool))
+    with pytest.raises(NotImplementedError):
+        ringx_sdpa(t, t, t, dropout_p=0.1)
+    with pytest.raises(ValueError, match="enable_gqa"):
+        ringx_sdpa(t, t[:, :1], t[:, :1])
+    with pytest.raises(ValueError, match="CUDA tensor"):          # no CPU fallback
+        ringx_sdpa(t, t, t)
+    assert _default_chunk(262144) == 32768 and _default_chunk(1280) == 256 and _default_chunk(384) == 128
 
 
 def test_requires_a_process_group():
