@@ -217,11 +217,13 @@ def ringx_lse_merge(o_a, lse_a, o_b, lse_b, out_dtype=None, inplace: bool = Fals
     return o_out, lse_out
 
 
-def ringx_attn_bwd(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspace=None):
+def ringx_attn_bwd(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspace=None, dq=None, dk=None, dv=None):
     """dQ, dK, dV (bf16) from the saved (o, lse) of ringx_attn_fwd (include/ringx.h: ringx_attn_bwd)."""
     B, H, N, d = q.shape
     dt = _DTYPES[q.dtype]
-    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    dq = torch.empty_like(q) if dq is None else dq
+    dk = torch.empty_like(k) if dk is None else dk
+    dv = torch.empty_like(v) if dv is None else dv
     need = lib().ringx_attn_bwd_workspace_bytes(B, H, N, d, kv_chunk, dt)
     if workspace is None:
         workspace = _workspace(max(need, 256), q.device)
