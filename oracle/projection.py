@@ -58,3 +58,48 @@ def attention_block_fwd(x, w_qkv, w_o, H, scale):
         for a in range(H):
             o[b, a], _ = _att.attention_fwd(q[b, a], k[b, a], v[b, a], scale)
     return out_projection(o, w_o)
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# Backward of the projections and of the block: the derivative of the definitions above (the paper trains the model,
+# PAPER.md:260-264, but prints no backward formulas; reading p5: plain calculus, loss L = sum dY * Y).
+# --------------------------------------------------------------------------------------------------------------------
+def out_projection_bwd(dy, o, w_o):
+    """y = merge_heads(o) W_o^T  =>  dO = split_heads(dY W_o),  dW_o = dY^T merge_heads(o).
+    dy [B,S,h], o [B,H,S,d], w_o [h,h] -> (dO [B,H,S,d], dW_o [h,h])."""
+    dy = np.asarray(dy, dtype=np.float64)
+    o = np.asarray(o, dtype=np.float64)
+    w = np.asarray(w_o, dtype=np.float64)
+    H = o.shape[1]
+    om = merge_heads(o)                                         # [B, S, h]
+    d_o = split_heads(dy @ w, H)
+    dw = np.einsum("bsn,bsi->ni", dy, om)
+    return d_o, dw
+
+
+def qkv_projection_bwd(dq, dk, dv, x, w_qkv):
+    """[q|k|v] = x W_qkv^T  =>  dX = [dQ|dK|dV]_merged W_qkv,  dW_qkv = [dQ|dK|dV]_merged^T x.
+    dq,dk,dv [B,H,S,d], x [B,S,h], w_qkv [3h,h] -> (dX [B,S,h], dW_qkv [3h,h])."""
+    x = np.asarray(x, dtype=np.float64)
+    w = np.asarray(w_qkv, dtype=np.float64)
+    g = np.concatenate([merge_heads(np.asarray(t, dtype=np.float64)) for t in (dq, dk, dv)], axis=-1)   # [B, S, 3h]
+    dx = g @ w
+    dw = np.einsum("bsn,bsi->ni", g, x)
+    return dx, dw
+
+
+def attention_block_bwd(x, w_qkv, w_o, dy, H, scale):
+    """Gradients of L = sum dY * attention_block_fwd(x, ...): returns (dX, dW_qkv, dW_o)."""
+    q, k, v = qkv_projection(x, w_qkv, H)
+    B = q.shape[0]
+    o = np.empty_like(q)
+    for b in range(B):
+        for a in range(H):
+            o[b, a], _ = _att.attention_fwd(q[b, a], k[b, a], v[b, a], scale)
+    d_o, dw_o = out_projection_bwd(dy, o, w_o)
+    dq, dk, dv = np.empty_like(q), np.empty_like(k), np.empty_like(v)
+    for b in range(B):
+        for a in range(H):
+            dq[b, a], dk[b, a], dv[b, a] = _att.attention_bwd(q[b, a], k[b, a], v[b, a], d_o[b, a], scale)
+    dx, dw_qkv = qkv_projection_bwd(dq, dk, dv, x, w_qkv)
+    return dx, dw_qkv, dw_o

@@ -113,3 +113,65 @@ def test_linearity_and_head_independence():
     q2 = proj.qkv_projection(x1, w2, H)[0]
     np.testing.assert_array_equal(q2[:, 0], b1[0][:, 0])
     assert np.abs(q2[:, 1] - b1[0][:, 1]).max() > 0
+
+
+# ------------------------------------------------------------------------------------------------ backward (reading p5)
+def _block_loss(x, w, wo, dy, H, scale):
+    return float((dy * proj.attention_block_fwd(x, w, wo, H, scale)).sum())
+
+
+def test_block_backward_by_central_finite_differences():
+    B, S, H, d = 1, 5, 2, 3
+    h = H * d
+    scale = 0.7
+    x, w, wo, dy = (RNG.standard_normal(s) for s in ((B, S, h), (3 * h, h), (h, h), (B, S, h)))
+    w *= 0.4
+    dx, dw, dwo = proj.attention_block_bwd(x, w, wo, dy, H, scale)
+    eps = 1e-6
+    for arr, grad, idxs in ((x, dx, [(0, 0, 0), (0, 3, 4), (0, 4, 5)]), (w, dw, [(0, 0), (7, 2), (13, 5), (17, 1)]),
+                            (wo, dwo, [(0, 0), (2, 5), (5, 3)])):
+        for idx in idxs:
+            old = arr[idx]
+            arr[idx] = old + eps
+            lp = _block_loss(x, w, wo, dy, H, scale)
+            arr[idx] = old - eps
+            lm = _block_loss(x, w, wo, dy, H, scale)
+            arr[idx] = old
+            fd = (lp - lm) / (2 * eps)
+            assert abs(fd - grad[idx]) <= 1e-6 * max(1.0, abs(fd)), (idx, fd, grad[idx])
+
+
+def test_projection_backward_against_torch_autograd():
+    B, S, H, d = 2, 6, 2, 4
+    h = H * d
+    x, w, wo = RNG.standard_normal((B, S, h)), RNG.standard_normal((3 * h, h)), RNG.standard_normal((h, h))
+    dq, dk, dv, o = (RNG.standard_normal((B, H, S, d)) for _ in range(4))
+    dy = RNG.standard_normal((B, S, h))
+    xt, wt = torch.from_numpy(x).requires_grad_(), torch.from_numpy(w).requires_grad_()
+    y = torch.nn.functional.linear(xt, wt)
+    g = torch.cat([torch.from_numpy(t).permute(0, 2, 1, 3).reshape(B, S, h) for t in (dq, dk, dv)], dim=-1)
+    y.backward(g)
+    dx, dw = proj.qkv_projection_bwd(dq, dk, dv, x, w)
+    np.testing.assert_allclose(dx, xt.grad.numpy(), atol=1e-12)
+    np.testing.assert_allclose(dw, wt.grad.numpy(), atol=1e-12)
+    ot, wot = torch.from_numpy(o).requires_grad_(), torch.from_numpy(wo).requires_grad_()
+    yo = torch.nn.functional.linear(ot.permute(0, 2, 1, 3).reshape(B, S, h), wot)
+    yo.backward(torch.from_numpy(dy))
+    d_o, dwo = proj.out_projection_bwd(dy, o, wo)
+    np.testing.assert_allclose(d_o, ot.grad.numpy(), atol=1e-12)
+    np.testing.assert_allclose(dwo, wot.grad.numpy(), atol=1e-12)
+
+
+def test_projection_backward_one_hot_reads():
+    """dY one-hot at (s, n): dO row s = column... W_o[n, :] split into heads; dW_o row n = merged o row s."""
+    B, S, H, d = 1, 3, 2, 2
+    h = H * d
+    o, wo = RNG.standard_normal((B, H, S, d)), RNG.standard_normal((h, h))
+    dy = np.zeros((B, S, h))
+    dy[0, 1, 2] = 1.0
+    d_o, dwo = proj.out_projection_bwd(dy, o, wo)
+    for a in range(H):
+        for c in range(d):
+            assert d_o[0, a, 1, c] == wo[2, a * d + c] and d_o[0, a, 0, c] == 0.0
+            assert dwo[2, a * d + c] == o[0, a, 1, c]
+    assert not dwo[[0, 1, 3]].any()
