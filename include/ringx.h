@@ -223,6 +223,25 @@ RINGX_API int ringx_attn_block_fwd(const void* x, const void* w_qkv, const void*
                          void* workspace, size_t workspace_bytes, void* stream);
 RINGX_API size_t ringx_attn_block_fwd_workspace_bytes(int B, int S, int H, int d, int kv_chunk);
 
+/* Backward of the projections and of the block (the derivative of the GEMMs above; loss L = sum dY * Y):
+ *   ringx_out_proj_bwd   dO = split_heads(dY W_o) (bf16 [B,H,S,d]),  dW_o = dY^T merge_heads(o) (float [h,h]).
+ *   ringx_qkv_proj_bwd   dX = merge[dq|dk|dv] W_qkv (bf16 [B,S,h]),  dW_qkv = merge[dq|dk|dv]^T x (float [3h,h]).
+ *   ringx_attn_block_bwd ringx_out_proj_bwd -> ringx_attn_bwd -> ringx_qkv_proj_bwd.  fwd_workspace is the workspace of the
+ *                        ringx_attn_block_fwd call with the same shape arguments, left untouched since (it holds q, k, v, o, lse).
+ * Weight gradients are accumulated in fp32: the buffers are zeroed, then split-K partial sums are reduce-added by TMA (their
+ * summation order is not fixed: the last bits may differ from run to run).  Two launches per projection, each a tcgen05
+ * GEMM whose transposed operands are read MN-major straight from the row-major tensors (no transpose pass).
+ * Domain: as the forward entries, and h = H*d a multiple of 256; else RINGX_ERR_BAD_SHAPE. */
+RINGX_API int ringx_out_proj_bwd(const void* dy, const void* o, const void* w_o, void* d_o, float* dw_o,
+                       int B, int S, int H, int d, void* stream);
+RINGX_API int ringx_qkv_proj_bwd(const void* dq, const void* dk, const void* dv, const void* x, const void* w_qkv,
+                       void* dx, float* dw_qkv, int B, int S, int H, int d, void* stream);
+RINGX_API int ringx_attn_block_bwd(const void* x, const void* w_qkv, const void* w_o, const void* dy,
+                         const void* fwd_workspace, void* dx, float* dw_qkv, float* dw_o,
+                         int B, int S, int H, int d, int kv_chunk, float scale,
+                         void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_block_bwd_workspace_bytes(int B, int S, int H, int d, int kv_chunk);
+
 /* ringx_attn_fwd with HOST buffers (the end-to-end entry): copies q,k,v host->device into the
  * workspace, runs ringx_attn_fwd, copies o and lse back, and synchronises `stream`.
  *   q_host,k_host,v_host,o_host,lse_host  HOST pointers (pinned memory recommended).

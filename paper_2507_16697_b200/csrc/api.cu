@@ -863,6 +863,96 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   return RINGX_OK;
 }
 
+// ---- backward of the projections and of the block (derivative of Table II's GEMMs)
+static int check_proj(int B, int S, int H, int d);
+static int check_proj_bwd(int B, int S, int H, int d) {
+  int st = check_proj(B, S, H, d);
+  if (st != RINGX_OK) return st;
+  if ((H * d) % 256) return RINGX_ERR_BAD_SHAPE;      // the MN-major operand tiles are not ragged
+  return RINGX_OK;
+}
+
+int ringx_out_proj_bwd(const void* dy, const void* o, const void* w_o, void* d_o, float* dw_o, int B, int S, int H, int d,
+                       void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int st = check_proj_bwd(B, S, H, d);
+  if (st != RINGX_OK) return st;
+  if (!dy || !o || !w_o || !d_o || !dw_o) return RINGX_ERR_NULL_PTR;
+  if (!aligned16(dy) || !aligned16(o) || !aligned16(w_o) || !aligned16(d_o) || !aligned16(dw_o)) return RINGX_ERR_MISALIGNED;
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  const size_t h = (size_t)H * d;
+  cudaError_t e = cudaMemsetAsync(dw_o, 0, h * h * sizeof(float), stream);
+  if (e != cudaSuccess) return cuda_status(e);
+  {
+    Timed timed(RINGX_PROFILE_PROJ, stream);
+    e = launch_out_proj_bwd(dy, o, w_o, d_o, dw_o, B, S, H, d, stream);
+  }
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_qkv_proj_bwd(const void* dq, const void* dk, const void* dv, const void* x, const void* w_qkv, void* dx,
+                       float* dw_qkv, int B, int S, int H, int d, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  int st = check_proj_bwd(B, S, H, d);
+  if (st != RINGX_OK) return st;
+  if (!dq || !dk || !dv || !x || !w_qkv || !dx || !dw_qkv) return RINGX_ERR_NULL_PTR;
+  if (!aligned16(dq) || !aligned16(dk) || !aligned16(dv) || !aligned16(x) || !aligned16(w_qkv) || !aligned16(dx) ||
+      !aligned16(dw_qkv))
+    return RINGX_ERR_MISALIGNED;
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  const size_t h = (size_t)H * d;
+  cudaError_t e = cudaMemsetAsync(dw_qkv, 0, 3 * h * h * sizeof(float), stream);
+  if (e != cudaSuccess) return cuda_status(e);
+  {
+    Timed timed(RINGX_PROFILE_PROJ, stream);
+    e = launch_qkv_proj_bwd(dq, dk, dv, x, w_qkv, dx, dw_qkv, B, S, H, d, stream);
+  }
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+size_t ringx_attn_block_bwd_workspace_bytes(int B, int S, int H, int d, int kv_chunk) {
+  if (check_proj_bwd(B, S, H, d) != RINGX_OK) return 0;
+  const size_t R = (size_t)B * H * S;
+  return 4 * align_up(R * d * 2) + align_up(ringx_attn_bwd_workspace_bytes(B, H, S, d, kv_chunk, RINGX_BF16));
+}
+
+int ringx_attn_block_bwd(const void* x, const void* w_qkv, const void* w_o, const void* dy, const void* fwd_workspace,
+                         void* dx, float* dw_qkv, float* dw_o, int B, int S, int H, int d, int kv_chunk, float scale,
+                         void* workspace, size_t workspace_bytes, void* stream_) {
+  int st = check_proj_bwd(B, S, H, d);
+  if (st == RINGX_OK) st = check_shape(B, H, S, d, kv_chunk, scale, RINGX_BF16, true);
+  if (st != RINGX_OK) return st;
+  if (!x || !w_qkv || !w_o || !dy || !fwd_workspace || !dx || !dw_qkv || !dw_o || !workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign || reinterpret_cast<uintptr_t>(fwd_workspace) % kAlign)
+    return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < ringx_attn_block_bwd_workspace_bytes(B, S, H, d, kv_chunk)) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  const size_t R = (size_t)B * H * S, tba = align_up(R * d * 2);
+  // what ringx_attn_block_fwd left in its workspace: q | k | v | o | lse
+  const char* f = static_cast<const char*>(fwd_workspace);
+  const void *q = f, *k = f + tba, *v = f + 2 * tba, *o = f + 3 * tba;
+  const float* lse = reinterpret_cast<const float*>(f + 4 * tba);
+  char* p = static_cast<char*>(workspace);
+  void *d_o = p, *dq = p + tba, *dk = p + 2 * tba, *dv = p + 3 * tba;
+  char* inner = p + 4 * tba;
+  const size_t inner_bytes = workspace_bytes - 4 * tba;
+  st = ringx_out_proj_bwd(dy, o, w_o, d_o, dw_o, B, S, H, d, stream_);
+  if (st != RINGX_OK) return st;
+  int launches = tl_last_launches;
+  st = ringx_attn_bwd(q, k, v, o, lse, d_o, dq, dk, dv, B, H, S, d, kv_chunk, scale, RINGX_BF16, inner, inner_bytes, stream_);
+  if (st != RINGX_OK) return st;
+  launches += tl_last_launches;
+  st = ringx_qkv_proj_bwd(dq, dk, dv, x, w_qkv, dx, dw_qkv, B, S, H, d, stream_);
+  if (st != RINGX_OK) return st;
+  tl_last_launches += launches;
+  return RINGX_OK;
+}
+
 // ---- the Turbulence-Transformer tokeniser
 int ringx_fidelity_tokens(const float* y, void* tokens, int M, int D, int H, int W, int C, int z0, int y0, int x0,
                           int Dc, int Hc, int Wc, int k, float sigma, int out_dtype, void* stream_) {
@@ -1028,6 +1118,6 @@ const char* ringx_status_string(int status) {
   }
 }
 
-int ringx_version(void) { return 140; }
+int ringx_version(void) { return 150; }
 
 }  // extern "C"

@@ -43,6 +43,12 @@ cudaError_t launch_fidelity_tokens(const float* y, void* tokens, int M, int D, i
 cudaError_t launch_qkv_proj(const void* x, const void* w_qkv, void* q, void* k, void* v, int B, int S, int H, int d,
                             cudaStream_t stream);
 cudaError_t launch_out_proj(const void* o, const void* w_o, void* y, int B, int S, int H, int d, cudaStream_t stream);
+// Their backward (two GEMMs each: data gradient in bf16, weight gradient reduce-added in fp32 into a zeroed buffer;
+// h % 256 == 0).  dO = split(dY W_o), dW_o = dY^T merge(o);  dX = merge[dq|dk|dv] W_qkv, dW_qkv = merge[dq|dk|dv]^T x.
+cudaError_t launch_out_proj_bwd(const void* dy, const void* o, const void* w_o, void* d_o, float* dw_o, int B, int S,
+                                int H, int d, cudaStream_t stream);
+cudaError_t launch_qkv_proj_bwd(const void* dq, const void* dk, const void* dv, const void* x, const void* w_qkv,
+                                void* dx, float* dw_qkv, int B, int S, int H, int d, cudaStream_t stream);
 
 // ---- attn_f32.cu (plain FFMA path, config C1)
 // One KV-chunk pass, fp32: q [BH,Nq,d], k/v [BH,nk_stride,d] rows [k_off, k_off+nk) -> o_out fp32, lse_out.

@@ -68,6 +68,14 @@ def lib() -> ctypes.CDLL:
     L.ringx_eq5_scale.restype = c_i
     L.ringx_eq5_finalize.argtypes = [c_p] * 5 + [c_ll, c_i, c_i, c_p]
     L.ringx_eq5_finalize.restype = c_i
+    L.ringx_out_proj_bwd.argtypes = [c_p] * 5 + [c_i] * 4 + [c_p]
+    L.ringx_out_proj_bwd.restype = c_i
+    L.ringx_qkv_proj_bwd.argtypes = [c_p] * 7 + [c_i] * 4 + [c_p]
+    L.ringx_qkv_proj_bwd.restype = c_i
+    L.ringx_attn_block_bwd.argtypes = [c_p] * 8 + [c_i] * 5 + [c_f, c_p, c_sz, c_p]
+    L.ringx_attn_block_bwd.restype = c_i
+    L.ringx_attn_block_bwd_workspace_bytes.argtypes = [c_i] * 5
+    L.ringx_attn_block_bwd_workspace_bytes.restype = c_sz
     L.ringx_fidelity_tokens.argtypes = [c_p, c_p] + [c_i] * 12 + [c_f, c_i, c_p]
     L.ringx_fidelity_tokens.restype = c_i
     L.ringx_qkv_proj.argtypes = [c_p] * 5 + [c_i] * 4 + [c_p]
@@ -340,6 +348,51 @@ def ringx_out_proj(o, w_o, y=None):
     y = torch.empty((B, S, h), dtype=torch.bfloat16, device=o.device) if y is None else y
     _check(lib().ringx_out_proj(_dev(o, "o"), _dev(w_o, "w_o"), _dev(y, "y"), B, S, H, d, _stream()), "ringx_out_proj")
     return y
+
+
+def ringx_out_proj_bwd(dy, o, w_o):
+    """(dO bf16 [B,H,S,d], dW_o fp32 [h,h]) (include/ringx.h: ringx_out_proj_bwd)."""
+    B, H, S, d = o.shape
+    h = H * d
+    d_o = torch.empty_like(o)
+    dw = torch.empty((h, h), dtype=torch.float32, device=o.device)
+    _check(lib().ringx_out_proj_bwd(_dev(dy, "dy"), _dev(o, "o"), _dev(w_o, "w_o"), _dev(d_o, "d_o"), _dev(dw, "dw_o"),
+                                    B, S, H, d, _stream()), "ringx_out_proj_bwd")
+    return d_o, dw
+
+
+def ringx_qkv_proj_bwd(dq, dk, dv, x, w_qkv):
+    """(dX bf16 [B,S,h], dW_qkv fp32 [3h,h]) (include/ringx.h: ringx_qkv_proj_bwd)."""
+    B, H, S, d = dq.shape
+    h = H * d
+    dx = torch.empty_like(x)
+    dw = torch.empty((3 * h, h), dtype=torch.float32, device=x.device)
+    _check(lib().ringx_qkv_proj_bwd(_dev(dq, "dq"), _dev(dk, "dk"), _dev(dv, "dv"), _dev(x, "x"), _dev(w_qkv, "w_qkv"),
+                                    _dev(dx, "dx"), _dev(dw, "dw_qkv"), B, S, H, d, _stream()), "ringx_qkv_proj_bwd")
+    return dx, dw
+
+
+def ringx_attn_block_bwd_workspace_bytes(B, S, H, d, kv_chunk) -> int:
+    return lib().ringx_attn_block_bwd_workspace_bytes(B, S, H, d, kv_chunk)
+
+
+def ringx_attn_block_bwd(x, w_qkv, w_o, dy, fwd_workspace, H: int, kv_chunk: int, scale: float, workspace=None):
+    """(dX bf16, dW_qkv fp32, dW_o fp32) of the attention block; `fwd_workspace` is the workspace tensor the matching
+    ringx_attn_block_fwd call used (include/ringx.h: ringx_attn_block_bwd)."""
+    B, S, h = x.shape
+    d = h // H
+    dx = torch.empty_like(x)
+    dw_qkv = torch.empty((3 * h, h), dtype=torch.float32, device=x.device)
+    dw_o = torch.empty((h, h), dtype=torch.float32, device=x.device)
+    need = lib().ringx_attn_block_bwd_workspace_bytes(B, S, H, d, kv_chunk)
+    if workspace is None:
+        workspace = _workspace(max(need, 256), x.device)
+    st = lib().ringx_attn_block_bwd(_dev(x, "x"), _dev(w_qkv, "w_qkv"), _dev(w_o, "w_o"), _dev(dy, "dy"),
+                                    _dev(fwd_workspace, "fwd_workspace"), _dev(dx, "dx"), _dev(dw_qkv, "dw_qkv"),
+                                    _dev(dw_o, "dw_o"), B, S, H, d, kv_chunk, scale, workspace.data_ptr(),
+                                    workspace.numel(), _stream())
+    _check(st, "ringx_attn_block_bwd")
+    return dx, dw_qkv, dw_o
 
 
 def ringx_attn_block_fwd_workspace_bytes(B, S, H, d, kv_chunk) -> int:

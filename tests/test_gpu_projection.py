@@ -128,3 +128,74 @@ def test_error_codes(rx):
         rx.ringx_qkv_proj(x.float(), w, 2)
     with pytest.raises(ValueError):
         rx.ringx_qkv_proj(x.cpu(), w.cpu(), 2)
+
+
+# ------------------------------------------------------------------------------------------------ backward
+BWD_SHAPES = [(1, 128, 4, 64), (2, 256, 2, 128), (1, 384, 8, 64), (3, 128, 4, 128), (1, 2048, 8, 128)]
+
+
+@pytest.mark.parametrize("B,S,H,d", BWD_SHAPES)
+def test_projection_backward_matches_the_oracle(rx, B, S, H, d):
+    """Data gradients (bf16) within 2^-8 |ref| + K 2^-24 (|A||B|); weight gradients (fp32, split-K reduce-adds in any order)
+    within T 2^-24 (|A|^T |B|) with T = B*S the reduction length."""
+    h = H * d
+    x, w_qkv, w_o = wl.make_block_inputs(B, S, H, d, seed=7 + S)
+    dy = wl.make_tensor((B, S, h), "do", seed=8)
+    o = wl.make_tensor((B, H, S, d), "v", seed=9)
+    dq, dk, dv = (wl.make_tensor((B, H, S, d), w, seed=10) for w in ("q", "k", "do"))
+    T = B * S
+    # ---- output projection
+    do_ref, dwo_ref = proj.out_projection_bwd(f64(dy), f64(o), f64(w_o))
+    d_o, dwo = rx.ringx_out_proj_bwd(dy.cuda(), o.cuda(), w_o.cuda())
+    torch.cuda.synchronize()
+    assert rx.ringx_last_launch_count() == 2
+    bound = proj.split_heads(np.abs(f64(dy)) @ np.abs(f64(w_o)), H) * (h * 2.0 ** -24)
+    assert check(d_o, do_ref, bound) <= 4e-3
+    wb = np.einsum("bsn,bsi->ni", np.abs(f64(dy)), proj.merge_heads(np.abs(f64(o)))) * (T * 2.0 ** -24)
+    assert (np.abs(dwo.cpu().numpy().astype(np.float64) - dwo_ref) - wb).max() <= 0
+    assert np.linalg.norm(dwo.cpu().numpy() - dwo_ref) / np.linalg.norm(dwo_ref) <= 1e-5
+    # ---- input projections
+    dx_ref, dwq_ref = proj.qkv_projection_bwd(f64(dq), f64(dk), f64(dv), f64(x), f64(w_qkv))
+    dx, dwq = rx.ringx_qkv_proj_bwd(dq.cuda(), dk.cuda(), dv.cuda(), x.cuda(), w_qkv.cuda())
+    torch.cuda.synchronize()
+    g = np.concatenate([proj.merge_heads(np.abs(f64(t))) for t in (dq, dk, dv)], axis=-1)
+    assert check(dx, dx_ref, (g @ np.abs(f64(w_qkv))) * (3 * h * 2.0 ** -24)) <= 4e-3
+    wb = np.einsum("bsn,bsi->ni", g, np.abs(f64(x))) * (T * 2.0 ** -24)
+    assert (np.abs(dwq.cpu().numpy().astype(np.float64) - dwq_ref) - wb).max() <= 0
+    assert np.linalg.norm(dwq.cpu().numpy() - dwq_ref) / np.linalg.norm(dwq_ref) <= 1e-5
+
+
+def test_projection_backward_identity_weights_copy_bits(rx):
+    B, S, H, d = 1, 256, 4, 64
+    h = H * d
+    eye = torch.eye(h, dtype=torch.bfloat16)
+    dy = wl.make_tensor((B, S, h), "do", seed=3)
+    o = wl.make_tensor((B, H, S, d), "v", seed=3)
+    d_o, _ = rx.ringx_out_proj_bwd(dy.cuda(), o.cuda(), eye.cuda())
+    assert torch.equal(d_o.cpu(), dy.view(B, S, H, d).permute(0, 2, 1, 3))          # dO = split_heads(dY)
+
+
+@pytest.mark.parametrize("B,S,H,d,chunk", [(1, 1024, 4, 64, 256), (2, 512, 2, 128, 512)])
+def test_attention_block_backward_matches_the_oracle(rx, B, S, H, d, chunk):
+    x, w_qkv, w_o = wl.make_block_inputs(B, S, H, d, seed=31)
+    dy = wl.make_tensor((B, S, H * d), "do", seed=32)
+    scale = 1.0 / math.sqrt(d)
+    ref = proj.attention_block_bwd(f64(x), f64(w_qkv), f64(w_o), f64(dy), H, scale)
+    ws = torch.empty(rx.ringx_attn_block_fwd_workspace_bytes(B, S, H, d, chunk), dtype=torch.uint8, device="cuda")
+    xd, wq, wo, dyd = x.cuda(), w_qkv.cuda(), w_o.cuda(), dy.cuda()
+    rx.ringx_attn_block_fwd(xd, wq, wo, H, chunk, scale, workspace=ws)
+    got = rx.ringx_attn_block_bwd(xd, wq, wo, dyd, ws, H, chunk, scale)
+    torch.cuda.synchronize()
+    assert rx.ringx_last_launch_count() == 2 + (S // chunk + 2) + 2
+    for name, g, r in zip(("dx", "dw_qkv", "dw_o"), got, ref):
+        rel = np.linalg.norm(g.float().cpu().numpy() - r) / np.linalg.norm(r)
+        assert rel <= 2e-2, (name, rel)
+
+
+def test_projection_backward_rejects_h_not_multiple_of_256(rx):
+    o = torch.zeros((1, 2, 128, 64), dtype=torch.bfloat16, device="cuda")       # h = 128
+    dy = torch.zeros((1, 128, 128), dtype=torch.bfloat16, device="cuda")
+    w = torch.zeros((128, 128), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(rx.RingxError) as e:
+        rx.ringx_out_proj_bwd(dy, o, w)
+    assert e.value.status == 2
