@@ -535,8 +535,13 @@ def next_rows_measure(ringx, wl, dev, reps=5):
     yb = ringx.ringx_out_proj(q, wo)
     ms_o = timeit(lambda: ringx.ringx_out_proj(q, wo, y=yb))
     tq, to = 6.0 * B * S * h * h / ms_q / 1e9, 2.0 * B * S * h * h / ms_o / 1e9
+    dyb = wl.make_tensor((B, S, h), "do", seed=5, device=dev)
+    ms_ob = timeit(lambda: ringx.ringx_out_proj_bwd(dyb, q, wo))          # data + weight gradient: 2 x 2*b*S*h^2
+    ms_qb = timeit(lambda: ringx.ringx_qkv_proj_bwd(q, k, v, x, wq))      # 2 x 6*b*S*h^2
     out["projections_S262144_h1024"] = {
         "qkv_ms": ms_q, "qkv_tflops": tq, "out_ms": ms_o, "out_tflops": to,
+        "out_bwd_ms": ms_ob, "out_bwd_tflops": 4.0 * B * S * h * h / ms_ob / 1e9,
+        "qkv_bwd_ms": ms_qb, "qkv_bwd_tflops": 12.0 * B * S * h * h / ms_qb / 1e9,
         "roofline": {"bound": "tensor", "kernel": "proj_gemm_kernel<QKV>", "achieved": tq, "peak": peaks["bf16_tflops"],
                      "unit": "TFLOP/s", "frac": tq / peaks["bf16_tflops"],
                      "peak_kind": "bf16 dense, burst (kernel timed alone), measured"}}
