@@ -40,8 +40,12 @@ using namespace ptx;
 
 constexpr int kBlockM = 128;          // query rows per tile (= TMEM lanes)
 constexpr int kBlockN = 128;          // keys per KV tile
-constexpr int kFwdThreads = 384;
-constexpr int kSoftmaxRegs = 224, kAuxRegs = 56;   // 256*224 + 128*56 = 64512 <= 65536
+#ifndef RINGX_FWD_COLSPLIT_D64
+#define RINGX_FWD_COLSPLIT_D64 1
+#endif
+#ifndef RINGX_FWD_COLSPLIT_D128
+#define RINGX_FWD_COLSPLIT_D128 0
+#endif
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
 // d = 64 is bound by the softmax warps (one exponential per 4*64 tensor FLOPs: 2048 clk of MUFU.EX2 against 1024 clk
 // of MMA per 128-key iteration).  Of the 16 element pairs of every 32-key piece, those in this mask take 2^x from the
@@ -68,7 +72,21 @@ struct FwdCfg {
   static constexpr int kSBufs = kD == 128 ? 2 : 3;
   static constexpr uint32_t kOBase = kSBufs * 128;           // O_t at kOBase + t * kD
   static constexpr int kBarBytes = 256;
-  static constexpr int kSmemBytes = 1024 + 2 * kTileBytes + kStages * kTileBytes + kBarBytes;
+  // Column split: the 128 keys of a score tile are shared by TWO softmax warpgroups (64 keys each), i.e. four softmax
+  // warpgroups per CTA and four warps per scheduler instead of two -- the MUFU pipe then stays busy while other warps
+  // are in their TMEM-load / row-max phase or wait on a barrier.  The two halves of a row exchange their row maxima
+  // (and, in the epilogue, their row sums) through shared memory.
+  static constexpr bool kColSplit = kD == 64 ? (RINGX_FWD_COLSPLIT_D64 != 0) : (RINGX_FWD_COLSPLIT_D128 != 0);
+  static constexpr int kSoftmaxWarps = kColSplit ? 16 : 8;
+  static constexpr int kProducerWarp = kSoftmaxWarps, kMmaWarp = kSoftmaxWarps + 1;
+  static constexpr int kThreads = (kSoftmaxWarps + 4) * 32;
+  // setmaxnreg moves registers inside the CTA's own pool (threads x the launch-time count: 384 x 168 / 640 x 96), so what
+  // the softmax warpgroups gain must equal what the last warpgroup gives up: 256 x (224-168) = 128 x (168-56);
+  // 512 x (112-96) = 128 x (96-32)
+  static constexpr int kSoftmaxRegs = kColSplit ? 112 : 224;
+  static constexpr int kAuxRegs = kColSplit ? 32 : 56;
+  static constexpr int kXchBytes = kColSplit ? 2 * 2 * 2 * 128 * 4 : 0;    // [tile][parity][half][row] floats
+  static constexpr int kSmemBytes = 1024 + 2 * kTileBytes + kStages * kTileBytes + kBarBytes + kXchBytes;
 };
 
 // Epilogue modes (kEpi): what happens to (loc_out, loc_lse) of this chunk
@@ -81,7 +99,7 @@ struct FwdCfg {
 enum { kEpiPartial = 0, kEpiFinal = 1, kEpiFold = 2, kEpiFoldFinal = 3 };
 
 template <int kD, int kEpi>
-__global__ void __launch_bounds__(kFwdThreads, 1)
+__global__ void __launch_bounds__(FwdCfg<kD>::kThreads, 1)
 attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                       const __grid_constant__ CUtensorMap map_v, void* o_out, float* lse_out, const float* o_acc,
                       const float* lse_acc, int Nq, int nk_stride, int k_off, int n_kv, float scale_log2) {
@@ -99,6 +117,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   uint64_t* kv_full = bars + 13;            // [kStages]
   uint64_t* kv_empty = bars + 13 + Cfg::kStages;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 13 + 2 * Cfg::kStages);
+  float* xch = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + Cfg::kBarBytes);   // column-split exchange
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // provably warp-uniform: keeps MMA/TMA operands in uniform registers
   const int lane = threadIdx.x & 31;
@@ -121,7 +140,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     }
     fence_mbar_init();
   }
-  if (warp == 8) {
+  if (warp == Cfg::kProducerWarp) {
     if (lane == 0) {
       prefetch_tmap(&map_q);
       prefetch_tmap(&map_k);
@@ -134,8 +153,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
 
-  if (warp == 8) {
-    setmaxnreg_dec<kAuxRegs>();
+  if (warp == Cfg::kProducerWarp) {
+    setmaxnreg_dec<Cfg::kAuxRegs>();
     // ------------------------------------------------------------------ TMA producer
     // (the whole warp runs the loop so that every operand is warp-uniform; one elected lane issues)
     {
@@ -169,9 +188,9 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         if (m < n_s) push(&map_k, m >> 1);
       }
     }
-  } else if (warp == 9) {
+  } else if (warp == Cfg::kMmaWarp) {
     // ------------------------------------------------------------------ MMA issuer
-    setmaxnreg_dec<kAuxRegs>();
+    setmaxnreg_dec<Cfg::kAuxRegs>();
     {
       const bool leader = elect_one();
       constexpr uint32_t idesc_s = make_idesc_bf16(kBlockM, kBlockN, 0, 0);    // Q (K-major) x K^T (K-major)
@@ -254,107 +273,202 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         }
       }
     }
-  } else if (warp < 8) {
+  } else if (warp < Cfg::kSoftmaxWarps) {
     // ------------------------------------------------------------------ softmax warpgroups
-    setmaxnreg_inc<kSoftmaxRegs>();
-    const int t = warp >> 2;
+    setmaxnreg_inc<Cfg::kSoftmaxRegs>();
+    const int t = Cfg::kColSplit ? warp >> 3 : warp >> 2;      // query tile
+    const int hh = Cfg::kColSplit ? (warp >> 2) & 1 : 0;       // column split: which 64 keys of every score tile
     const uint32_t lane_off = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tO = tmem + Cfg::kOBase + t * kD + lane_off;
     float m_raw = -CUDART_INF_F;   // running (lazy) row max of the unscaled scores
     float m_sc = -CUDART_INF_F;    // m_raw * scale_log2
     float l = 0.f;                 // running row sum of exp2(s*scale_log2 - m_sc)
     const float2 sc2 = make_float2(scale_log2, scale_log2);
-    for (int j = 0; j < n_kv; ++j) {
-      const long long c0 = CLK();
-      const int n = 2 * j + t, buf = Cfg::kSBufs == 2 ? t : n % Cfg::kSBufs;     // this tile's scores are S number n
-      const uint32_t tS = tmem + buf * kBlockN + lane_off;
-      mbar_wait(&s_full[buf], (Cfg::kSBufs == 2 ? j : n / Cfg::kSBufs) & 1);
-      tc_fence_after();
-      const long long c1 = CLK();
-      // ---- pass 1: stream S_t(j) out of TMEM; the row max of piece c is taken while piece c+1 is in flight
-      uint32_t s[kBlockN];
-      auto piece = [&](int c) -> uint32_t(&)[32] { return *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]); };
-      auto piece_max = [&](int c, float& a, float& b) {
+    if constexpr (Cfg::kColSplit) {
+      // ---- column-split main loop: this thread owns keys [64 hh, 64 hh + 64) of its query row
+      const int row_t = (warp & 3) * 32 + lane;
+      float* xch_t = xch + t * (2 * 2 * 128);                  // [parity][half][row]
+      // the two warps that share 32 query rows (one per half) meet on their own named barrier: the rescale decision
+      // below is taken per warp, so nothing wider may be waited for
+      const int pair_bar = 1 + t * 4 + (warp & 3);
+      for (int j = 0; j < n_kv; ++j) {
+        const int n = 2 * j + t, buf = Cfg::kSBufs == 2 ? t : n % Cfg::kSBufs;
+        const uint32_t tSb = tmem + buf * kBlockN + lane_off;
+        mbar_wait(&s_full[buf], (Cfg::kSBufs == 2 ? j : n / Cfg::kSBufs) & 1);
+        tc_fence_after();
+        uint32_t s[64];
+        auto piece = [&](int c) -> uint32_t(&)[32] { return *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]); };
+        auto piece_max = [&](int c, float& a, float& b) {
 #pragma unroll
-        for (int i = 0; i < 32; i += 4) {
-          a = fmax3(a, __uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1]));
-          b = fmax3(b, __uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3]));
-        }
-      };
-      float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F, mx2 = -CUDART_INF_F, mx3 = -CUDART_INF_F;
-      tmem_ld_x32(tS, piece(0));
-      tmem_wait_ld_x32(piece(0));
-      tmem_ld_x32(tS + 32, piece(1));
-      piece_max(0, mx0, mx1);
-      tmem_wait_ld_x32(piece(1));
-      tmem_ld_x32(tS + 64, piece(2));
-      piece_max(1, mx2, mx3);
-      tmem_wait_ld_x32(piece(2));
-      tmem_ld_x32(tS + 96, piece(3));
-      piece_max(2, mx0, mx1);
-      tmem_wait_ld_x32(piece(3));
-      piece_max(3, mx2, mx3);
-      const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-      const bool grow = (mx - m_raw) * scale_log2 > kRescaleThreshold;
-      if (__any_sync(0xffffffffu, grow)) {
-        const float m_new = fmaxf(m_raw, mx);
-        const float alpha = ex2((m_raw - m_new) * scale_log2);   // 0 on the first tile (m_raw = -inf)
-        l *= alpha;
-        if (j > 0) {
-          if (Cfg::kSBufs > 2) {     // the scores ran ahead of O_t += P_t(j-1) V: wait for it before touching O_t
-            mbar_wait(&pv_done[t], (j - 1) & 1);
+          for (int i = 0; i < 32; i += 4) {
+            a = fmax3(a, __uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1]));
+            b = fmax3(b, __uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3]));
+          }
+        };
+        float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F;
+        tmem_ld_x32(tSb + hh * 64, piece(0));
+        tmem_ld_x32(tSb + hh * 64 + 32, piece(1));
+        tmem_wait_ld_x32(piece(0));
+        piece_max(0, mx0, mx1);
+        tmem_wait_ld_x32(piece(1));
+        piece_max(1, mx0, mx1);
+        // exchange the half-row maxima; the barrier also tells each half that the other has its scores in registers,
+        // so P (which overwrites the first 64 columns of the score buffer) may be written
+        float* slot = xch_t + (j & 1) * 256;
+        slot[hh * 128 + row_t] = fmaxf(mx0, mx1);
+        named_bar_sync(pair_bar, 64);
+        const float mx = fmaxf(fmaxf(mx0, mx1), slot[(hh ^ 1) * 128 + row_t]);
+        const bool grow = (mx - m_raw) * scale_log2 > kRescaleThreshold;
+        if (__any_sync(0xffffffffu, grow)) {                   // same rows, same maxima: both halves decide alike
+          const float m_new = fmaxf(m_raw, mx);
+          const float alpha = ex2((m_raw - m_new) * scale_log2);
+          l *= alpha;
+          if (j > 0) {
+            if (Cfg::kSBufs > 2) {
+              mbar_wait(&pv_done[t], (j - 1) & 1);
+              tc_fence_after();
+            }
+            uint32_t o[kD / 2];                                // my half of the O columns
+#pragma unroll
+            for (int c = 0; c < kD / 64; ++c) tmem_ld_x32(tO + hh * (kD / 2) + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&o[c * 32]));
+            tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < kD / 2; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+#pragma unroll
+            for (int c = 0; c < kD / 64; ++c) tmem_st_x32(tO + hh * (kD / 2) + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&o[c * 32]));
+            tmem_wait_st();
+            tc_fence_before();
+            named_bar_sync(pair_bar, 64);                      // these rows of O_t are rescaled in full before either half releases P
             tc_fence_after();
           }
+          m_raw = m_new;
+          m_sc = m_new * scale_log2;
+        }
+        const float2 nm2 = make_float2(-m_sc, -m_sc);
+        float2 la = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
 #pragma unroll
-          for (int c = 0; c < kD / 32; ++c) {
-            uint32_t o[32];
-            tmem_ld_x32(tO + c * 32, o);
-            tmem_wait_ld_x32(o);
+        for (int c = 0; c < 2; ++c) {
+          uint32_t pk[16];
 #pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-            tmem_st_x32(tO + c * 32, o);
+          for (int i = 0; i < 32; i += 4) {
+            const float2 x0 = ffma2(make_float2(__uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1])), sc2, nm2);
+            const float2 x1 = ffma2(make_float2(__uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3])), sc2, nm2);
+            const float2 p0 = ((Cfg::kPolyMask >> (i / 2)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x0)
+                                                                : make_float2(ex2(x0.x), ex2(x0.y));
+            const float2 p1 = ((Cfg::kPolyMask >> (i / 2 + 1)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x1)
+                                                                    : make_float2(ex2(x1.x), ex2(x1.y));
+            la = fadd2(la, p0);
+            lb = fadd2(lb, p1);
+            pk[i / 2] = pack_bf16x2(p0.x, p0.y);
+            pk[i / 2 + 1] = pack_bf16x2(p1.x, p1.y);
+          }
+          tmem_st_x16(tSb + hh * 32 + c * 16, pk);
+        }
+        tmem_wait_st();
+        tc_fence_before();
+        if (Cfg::kSBufs > 2 && j > 0) mbar_wait(&pv_done[t], (j - 1) & 1);   // (see the unsplit loop)
+        mbar_arrive(&p_full[2 * t + hh]);
+        l += (la.x + la.y) + (lb.x + lb.y);
+      }
+      // the row sum over all 128 keys of every tile = the two halves' sums (same reference max)
+      mbar_wait(&o_full[t], 0);                                // (also: every named barrier of the loop is behind us)
+      float* slot = xch_t + (n_kv & 1) * 256;
+      slot[hh * 128 + row_t] = l;
+      named_bar_sync(pair_bar, 64);
+      l += slot[(hh ^ 1) * 128 + row_t];
+    } else {
+      for (int j = 0; j < n_kv; ++j) {
+        const long long c0 = CLK();
+        const int n = 2 * j + t, buf = Cfg::kSBufs == 2 ? t : n % Cfg::kSBufs;     // this tile's scores are S number n
+        const uint32_t tS = tmem + buf * kBlockN + lane_off;
+        mbar_wait(&s_full[buf], (Cfg::kSBufs == 2 ? j : n / Cfg::kSBufs) & 1);
+        tc_fence_after();
+        const long long c1 = CLK();
+        // ---- pass 1: stream S_t(j) out of TMEM; the row max of piece c is taken while piece c+1 is in flight
+        uint32_t s[kBlockN];
+        auto piece = [&](int c) -> uint32_t(&)[32] { return *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]); };
+        auto piece_max = [&](int c, float& a, float& b) {
+#pragma unroll
+          for (int i = 0; i < 32; i += 4) {
+            a = fmax3(a, __uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1]));
+            b = fmax3(b, __uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3]));
+          }
+        };
+        float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F, mx2 = -CUDART_INF_F, mx3 = -CUDART_INF_F;
+        tmem_ld_x32(tS, piece(0));
+        tmem_wait_ld_x32(piece(0));
+        tmem_ld_x32(tS + 32, piece(1));
+        piece_max(0, mx0, mx1);
+        tmem_wait_ld_x32(piece(1));
+        tmem_ld_x32(tS + 64, piece(2));
+        piece_max(1, mx2, mx3);
+        tmem_wait_ld_x32(piece(2));
+        tmem_ld_x32(tS + 96, piece(3));
+        piece_max(2, mx0, mx1);
+        tmem_wait_ld_x32(piece(3));
+        piece_max(3, mx2, mx3);
+        const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+        const bool grow = (mx - m_raw) * scale_log2 > kRescaleThreshold;
+        if (__any_sync(0xffffffffu, grow)) {
+          const float m_new = fmaxf(m_raw, mx);
+          const float alpha = ex2((m_raw - m_new) * scale_log2);   // 0 on the first tile (m_raw = -inf)
+          l *= alpha;
+          if (j > 0) {
+            if (Cfg::kSBufs > 2) {     // the scores ran ahead of O_t += P_t(j-1) V: wait for it before touching O_t
+              mbar_wait(&pv_done[t], (j - 1) & 1);
+              tc_fence_after();
+            }
+#pragma unroll
+            for (int c = 0; c < kD / 32; ++c) {
+              uint32_t o[32];
+              tmem_ld_x32(tO + c * 32, o);
+              tmem_wait_ld_x32(o);
+#pragma unroll
+              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+              tmem_st_x32(tO + c * 32, o);
+            }
+          }
+          m_raw = m_new;
+          m_sc = m_new * scale_log2;
+        }
+        // ---- pass 2: P = exp2(s * scale_log2 - m_sc), bf16, into the first 64 columns of S_t; row sum in fp32
+        const float2 nm2 = make_float2(-m_sc, -m_sc);
+        float2 la = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int c = 0; c < kBlockN / 32; ++c) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int i = 0; i < 32; i += 4) {
+            const float2 x0 = ffma2(make_float2(__uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1])), sc2, nm2);
+            const float2 x1 = ffma2(make_float2(__uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3])), sc2, nm2);
+            const float2 p0 = ((Cfg::kPolyMask >> (i / 2)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x0)
+                                                                : make_float2(ex2(x0.x), ex2(x0.y));
+            const float2 p1 = ((Cfg::kPolyMask >> (i / 2 + 1)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x1)
+                                                                    : make_float2(ex2(x1.x), ex2(x1.y));
+            la = fadd2(la, p0);
+            lb = fadd2(lb, p1);
+            pk[i / 2] = pack_bf16x2(p0.x, p0.y);
+            pk[i / 2 + 1] = pack_bf16x2(p1.x, p1.y);
+          }
+          tmem_st_x16(tS + c * 16, pk);
+          if (c & 1) {                       // 64 keys of P are in TMEM: let the tensor core start on them
+            tmem_wait_st();
+            tc_fence_before();
+            // (with the scores running ahead, P_t(j) could otherwise complete p_full a second time before the MMA warp
+            // has seen P_t(j-1): PV_t(j-1) complete proves it has)
+            if (Cfg::kSBufs > 2 && c == 1 && j > 0) mbar_wait(&pv_done[t], (j - 1) & 1);
+            mbar_arrive(&p_full[2 * t + (c >> 1)]);
           }
         }
-        m_raw = m_new;
-        m_sc = m_new * scale_log2;
-      }
-      // ---- pass 2: P = exp2(s * scale_log2 - m_sc), bf16, into the first 64 columns of S_t; row sum in fp32
-      const float2 nm2 = make_float2(-m_sc, -m_sc);
-      float2 la = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
-#pragma unroll
-      for (int c = 0; c < kBlockN / 32; ++c) {
-        uint32_t pk[16];
-#pragma unroll
-        for (int i = 0; i < 32; i += 4) {
-          const float2 x0 = ffma2(make_float2(__uint_as_float(s[c * 32 + i]), __uint_as_float(s[c * 32 + i + 1])), sc2, nm2);
-          const float2 x1 = ffma2(make_float2(__uint_as_float(s[c * 32 + i + 2]), __uint_as_float(s[c * 32 + i + 3])), sc2, nm2);
-          const float2 p0 = ((Cfg::kPolyMask >> (i / 2)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x0)
-                                                              : make_float2(ex2(x0.x), ex2(x0.y));
-          const float2 p1 = ((Cfg::kPolyMask >> (i / 2 + 1)) & 1) ? ex2_poly2<RINGX_FWD_POLY_DEGREE>(x1)
-                                                                  : make_float2(ex2(x1.x), ex2(x1.y));
-          la = fadd2(la, p0);
-          lb = fadd2(lb, p1);
-          pk[i / 2] = pack_bf16x2(p0.x, p0.y);
-          pk[i / 2 + 1] = pack_bf16x2(p1.x, p1.y);
-        }
-        tmem_st_x16(tS + c * 16, pk);
-        if (c & 1) {                       // 64 keys of P are in TMEM: let the tensor core start on them
-          tmem_wait_st();
-          tc_fence_before();
-          // (with the scores running ahead, P_t(j) could otherwise complete p_full a second time before the MMA warp
-          // has seen P_t(j-1): PV_t(j-1) complete proves it has)
-          if (Cfg::kSBufs > 2 && c == 1 && j > 0) mbar_wait(&pv_done[t], (j - 1) & 1);
-          mbar_arrive(&p_full[2 * t + (c >> 1)]);
-        }
-      }
-      l += (la.x + la.y) + (lb.x + lb.y);
+        l += (la.x + la.y) + (lb.x + lb.y);
 #ifdef RINGX_FWD_CLOCKS
-      if (blockIdx.x == 0 && blockIdx.y == 0 && (threadIdx.x & 127) == 0 && j >= 8) {
-        atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 0], (unsigned long long)(c1 - c0));   // wait S
-        atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 1], (unsigned long long)(CLK() - c1));  // softmax
-        atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 2], 1ull);
-      }
+        if (blockIdx.x == 0 && blockIdx.y == 0 && (threadIdx.x & 127) == 0 && j >= 8) {
+          atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 0], (unsigned long long)(c1 - c0));   // wait S
+          atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 1], (unsigned long long)(CLK() - c1));  // softmax
+          atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 2], 1ull);
+        }
 #endif
+      }
     }
     // ---- chunk epilogue: loc_out = O / l, loc_lse = m*scale + ln l  (natural log of the scaled scores)
     mbar_wait(&o_full[t], 0);
@@ -376,6 +490,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     }
 #pragma unroll
     for (int c = 0; c < kD / 32; ++c) {
+      if (Cfg::kColSplit && c / (kD / 64) != hh) continue;     // column split: each half stores its half of the row
       uint32_t o[32];
       tmem_ld_x32(tO + c * 32, o);
       float4 acc[8];
@@ -414,14 +529,14 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         for (int i = 0; i < 8; ++i) dst[i] = make_float4(r[i * 4], r[i * 4 + 1], r[i * 4 + 2], r[i * 4 + 3]);
       }
     }
-    lse_out[row] = lse_row;
+    if (hh == 0) lse_out[row] = lse_row;
   } else {
-    setmaxnreg_dec<kAuxRegs>();   // warps 10-11: nothing to do but release their registers
+    setmaxnreg_dec<Cfg::kAuxRegs>();   // the two idle warps of the last warpgroup: release their registers
   }
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 8) tmem_dealloc<512>(tmem);
+  if (warp == Cfg::kProducerWarp) tmem_dealloc<512>(tmem);
 }
 
 template <int kD, int kEpi>
@@ -437,7 +552,7 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
     configured = true;
   }
   dim3 grid(Nq / (2 * kBlockM), BH, splits);
-  kern<<<grid, kFwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, Nq, nk_stride, k_off,
+  kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, Nq, nk_stride, k_off,
                                                        nk / kBlockN / splits, scale * 1.4426950408889634f);
   count_launch();
   return cudaGetLastError();
