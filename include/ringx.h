@@ -22,7 +22,9 @@
  *              caller-provided `workspace`, sized by the *_workspace_bytes queries.
  *   Streams    All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy
  *              default stream).  Calls return after enqueue; there is no host synchronisation
- *              (ringx_attn_fwd_host is the exception: it synchronises `stream` before returning).
+ *              (the *_host entries are the exception: they synchronise `stream` before returning).  Because nothing
+ *              is allocated and nothing synchronises, the device entries can be captured into a CUDA graph
+ *              (cudaStreamBeginCapture on `stream`) once their first, uncaptured call has set the kernel attributes.
  *   Errors     Return value is a ringx_status (0 = RINGX_OK).  Arguments are validated before the
  *              first launch: an error other than RINGX_ERR_CUDA means nothing was enqueued and no
  *              output was touched.  No abort, no printf, no exceptions cross this boundary.

@@ -450,3 +450,39 @@ def test_deterministic_mode_gives_bit_identical_dq(rx, B, H, N, d, chunk):
     dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
     for g, r in zip(runs[0], (dq_ref, dk_ref, dv_ref)):
         assert np.linalg.norm(g.float().cpu().numpy() - r) / np.linalg.norm(r) <= 2e-2
+
+
+# ------------------------------------------------------------------------------------------------ CUDA graphs
+def test_forward_backward_capture_into_a_cuda_graph(rx):
+    """Every entry point only enqueues work on the caller's stream (no allocation, no synchronisation), so a whole
+    forward + backward -- 4 + 6 launches here -- can be captured once into a CUDA graph and replayed on new data."""
+    B, H, N, d, chunk = 1, 2, 1024, 64, 256
+    scale = 0.125
+    q, k, v, do = (t.cuda() for t in wl.make_qkv((B, H, N, d), with_do=True, seed=71))
+    o = torch.empty_like(q)
+    lse = torch.empty((B, H, N), dtype=torch.float32, device="cuda")
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    wf = torch.empty(max(256, rx.ringx_attn_fwd_workspace_bytes(B, H, N, d, chunk, q.dtype)), dtype=torch.uint8, device="cuda")
+    wb = torch.empty(rx.ringx_attn_bwd_workspace_bytes(B, H, N, d, chunk, q.dtype), dtype=torch.uint8, device="cuda")
+
+    def step():
+        rx.ringx_attn_fwd(q, k, v, chunk, scale, o=o, lse=lse, workspace=wf)
+        rx.ringx_attn_bwd(q, k, v, o, lse, do, chunk, scale, workspace=wb, dq=dq, dk=dk, dv=dv)
+
+    step()                                   # warm-up outside the capture (function attributes are set on first use)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        step()
+    for seed in (72, 73):
+        q2, k2, v2, do2 = (t.cuda() for t in wl.make_qkv((B, H, N, d), with_do=True, seed=seed))
+        for dst, src in ((q, q2), (k, k2), (v, v2), (do, do2)):
+            dst.copy_(src)
+        g.replay()
+        torch.cuda.synchronize()
+        got = [t.clone() for t in (o, lse, dk, dv, dq)]
+        step()                               # eager, same buffers
+        torch.cuda.synchronize()
+        for a, b in zip(got[:4], (o, lse, dk, dv)):
+            assert torch.equal(a, b)
+        assert ((got[4].float() - dq.float()).norm() / dq.float().norm()).item() <= 2e-3      # fp32 reduce order
