@@ -538,6 +538,25 @@ def next_rows_measure(ringx, wl, dev, reps=5):
     dyb = wl.make_tensor((B, S, h), "do", seed=5, device=dev)
     ms_ob = timeit(lambda: ringx.ringx_out_proj_bwd(dyb, q, wo))          # data + weight gradient: 2 x 2*b*S*h^2
     ms_qb = timeit(lambda: ringx.ringx_qkv_proj_bwd(q, k, v, x, wq))      # 2 x 6*b*S*h^2
+    # the whole block of Table II as a training step: projections + attention, forward and backward
+    ws_f = torch.empty(ringx.ringx_attn_block_fwd_workspace_bytes(B, S, H, d, 32768), dtype=torch.uint8, device=dev)
+    ws_b = torch.empty(ringx.ringx_attn_block_bwd_workspace_bytes(B, S, H, d, 32768), dtype=torch.uint8, device=dev)
+
+    def block_step():
+        ringx.ringx_attn_block_fwd(x, wq, wo, H, 32768, d ** -0.5, y=yb, workspace=ws_f)
+        ringx.ringx_attn_block_bwd(x, wq, wo, dyb, ws_f, H, 32768, d ** -0.5, workspace=ws_b)
+
+    block_step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    block_step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_blk = e0.elapsed_time(e1)
+    fl_blk = 14.0 * B * H * S * S * d + 3.0 * 8.0 * B * S * h * h        # attention fwd+bwd + projections fwd+bwd
+    out["block_fwd_bwd_S262144_h1024"] = {"ms": ms_blk, "tflops": fl_blk / ms_blk / 1e9}
+    del ws_f, ws_b
     out["projections_S262144_h1024"] = {
         "qkv_ms": ms_q, "qkv_tflops": tq, "out_ms": ms_o, "out_tflops": to,
         "out_bwd_ms": ms_ob, "out_bwd_tflops": 4.0 * B * S * h * h / ms_ob / 1e9,

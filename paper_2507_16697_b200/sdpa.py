@@ -84,3 +84,34 @@ def ringx_sdpa(query, key, value, attn_mask=None, dropout_p: float = 0.0, is_cau
         return _RingXDistAttention.apply(query, key, value, scale, schedule, comm, ops)
     kv_chunk = _default_chunk(key.shape[2]) if kv_chunk is None else kv_chunk
     return _RingXAttention.apply(query, key, value, scale, kv_chunk)
+
+
+class _RingXBlock(torch.autograd.Function):
+    """The attention block of Table II as one autograd node: forward = ringx_attn_block_fwd (which keeps
+    q, k, v, o, lse in its workspace), backward = ringx_attn_block_bwd reading that workspace."""
+
+    @staticmethod
+    def forward(ctx, x, w_qkv, w_o, H, kv_chunk, scale):
+        x, w_qkv, w_o = x.contiguous(), w_qkv.contiguous(), w_o.contiguous()
+        B, S, h = x.shape
+        ws = torch.empty(max(256, ringx.ringx_attn_block_fwd_workspace_bytes(B, S, H, h // H, kv_chunk)), dtype=torch.uint8,
+                         device=x.device)
+        y = ringx.ringx_attn_block_fwd(x, w_qkv, w_o, H, kv_chunk, scale, workspace=ws)
+        ctx.save_for_backward(x, w_qkv, w_o, ws)
+        ctx.H, ctx.kv_chunk, ctx.scale = H, kv_chunk, scale
+        return y
+
+    @staticmethod
+    def backward(ctx, dy):
+        x, w_qkv, w_o, ws = ctx.saved_tensors
+        dx, dw_qkv, dw_o = ringx.ringx_attn_block_bwd(x, w_qkv, w_o, dy.contiguous(), ws, ctx.H, ctx.kv_chunk, ctx.scale)
+        return dx, dw_qkv.to(w_qkv.dtype), dw_o.to(w_o.dtype), None, None, None
+
+
+def ringx_attention_block(x, w_qkv, w_o, num_heads: int, scale=None, kv_chunk: int | None = None):
+    """y = W_o . attention(split_heads(W_qkv x)) for x [B,S,h] bf16, w_qkv [3h,h], w_o [h,h] (torch.nn.Linear layout, no
+    bias), differentiable in x, w_qkv and w_o.  h = num_heads * d with d in {64,128}; h % 256 == 0 for the backward."""
+    d = x.shape[-1] // num_heads
+    scale = 1.0 / math.sqrt(d) if scale is None else float(scale)
+    kv_chunk = _default_chunk(x.shape[1]) if kv_chunk is None else kv_chunk
+    return _RingXBlock.apply(x, w_qkv, w_o, num_heads, kv_chunk, scale)

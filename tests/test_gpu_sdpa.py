@@ -68,3 +68,20 @@ def test_sdpa_fp32_forward_only_path(sdpa):
     q.requires_grad_()
     with pytest.raises(Exception):
         sdpa(q, k, v, kv_chunk=128).sum().backward()
+
+
+def test_attention_block_autograd(sdpa):
+    """The block as one autograd node (projections + attention, forward and backward in libringx) against the oracle."""
+    from oracle import projection as proj
+    from paper_2507_16697_b200.sdpa import ringx_attention_block
+    B, S, H, d = 1, 512, 4, 64
+    x, w_qkv, w_o = (t.cuda().requires_grad_() for t in wl.make_block_inputs(B, S, H, d, seed=51))
+    dy = wl.make_tensor((B, S, H * d), "do", seed=52).cuda()
+    y = ringx_attention_block(x, w_qkv, w_o, H, kv_chunk=256)
+    y.backward(dy)
+    f = lambda t: wl.to_f64_numpy(t.detach())
+    y_ref = proj.attention_block_fwd(f(x), f(w_qkv), f(w_o), H, d ** -0.5)
+    refs = proj.attention_block_bwd(f(x), f(w_qkv), f(w_o), f(dy), H, d ** -0.5)
+    assert relf(y.detach().float().cpu().numpy(), y_ref) <= 2e-2
+    for g, r in zip((x.grad, w_qkv.grad, w_o.grad), refs):
+        assert relf(g.float().cpu().numpy(), r) <= 2e-2
