@@ -76,7 +76,8 @@ typedef enum { RINGX_F32 = 0, RINGX_BF16 = 1 } ringx_dtype;
  *   dtype  RINGX_BF16: tcgen05 tensor-core path, fp32 accumulation (mixed fp32/bf16, l.286).
  *          RINGX_F32 : plain FFMA path (max abs error ~1e-6; tf32 would not meet 1e-5).
  *   workspace  >= ringx_attn_fwd_workspace_bytes(...) bytes, 256-byte aligned; may be NULL when
- *              that query returns 0 (kv_chunk == N with bf16).  Contents are scratch. */
+ *              that query returns 0 (kv_chunk == N with bf16 and a grid large enough that the keys of the
+ *              pass are not split, see ringx_attn_chunk_fwd_ex).  Contents are scratch. */
 RINGX_API int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* lse,
                    int B, int H, int N, int d, int kv_chunk, float scale, int dtype,
                    void* workspace, size_t workspace_bytes, void* stream);
@@ -84,7 +85,7 @@ RINGX_API int ringx_attn_fwd(const void* q, const void* k, const void* v, void* 
 /* Backward of L = sum dO.O (derivative of Eq. 1; data-flow of l.143).  bf16 only, d = 64 or 128.
  * P is recomputed from the saved *global* lse; each KV-chunk pass writes that chunk's dK,dV once
  * (atomic-free: a CTA owns a 128-key tile) and adds its contribution to dQ in an fp32 accumulator
- * ("accumulated ... over N steps"); dQ summation order is not deterministic.
+ * ("accumulated ... over N steps"); the order of the dQ sums is not fixed unless ringx_set_deterministic(1).
  *   q,k,v,o,dO [B,H,N,d] bf16 (in), lse [B,H,N] float (in, as written by ringx_attn_fwd).
  *   dq,dk,dv   [B,H,N,d] bf16 (out); must not alias any input.
  *   workspace  >= ringx_attn_bwd_workspace_bytes(...) bytes, 256-byte aligned. */
