@@ -3,6 +3,7 @@
 // step of the path runs in the kernels this file launches.
 #include <math.h>
 
+#include <atomic>
 #include <mutex>
 #include <vector>
 
@@ -44,15 +45,15 @@ int check_arch() {
     return RINGX_ERR_CUDA;
   }
   static std::mutex mu;
-  static int cached[64];   // 0 = unknown, 1 = ok, 2 = unsupported
+  static int cached[kMaxDevices];   // 0 = unknown, 1 = ok, 2 = unsupported
   std::lock_guard<std::mutex> g(mu);
-  if (dev >= 0 && dev < 64 && cached[dev]) return cached[dev] == 1 ? RINGX_OK : RINGX_ERR_UNSUPPORTED_ARCH;
+  if (dev >= 0 && dev < kMaxDevices && cached[dev]) return cached[dev] == 1 ? RINGX_OK : RINGX_ERR_UNSUPPORTED_ARCH;
   int major = 0;
   if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
     cudaGetLastError();
     return RINGX_ERR_CUDA;
   }
-  if (dev >= 0 && dev < 64) cached[dev] = (major == 10) ? 1 : 2;
+  if (dev >= 0 && dev < kMaxDevices) cached[dev] = (major == 10) ? 1 : 2;
   return major == 10 ? RINGX_OK : RINGX_ERR_UNSUPPORTED_ARCH;
 }
 
@@ -72,16 +73,16 @@ int check_shape(int B, int H, int N, int d, int kv_chunk, float scale, int dtype
 // ---- split-KV: when one chunk pass has too few query tiles to fill the GPU (the paper's own regime: 2K-64K query tokens per
 // device against a long gathered key sequence), the keys of the pass are split over gridDim.z and the
 // splits' partials are combined by Eq. 5 -- the same merge, inside one pass.
-constexpr int kSmCount = 148;          // B200; a constant so that workspace sizes do not depend on a device query
 constexpr int kMaxSplits = 8;
 constexpr int kMinTilesPerSplit = 8;   // >= 1024 keys per split: below that the prologue/epilogue of a CTA dominates
 
 int choose_splits(int BH, int Nq, int nk, int dtype) {
   if (dtype != RINGX_BF16 || Nq % 256) return 1;
   const long long ctas = (long long)BH * (Nq / 256);
+  const int kSmCount = sm_count();       // of the current device: the same value sizes the workspace and picks the grid
   if (ctas >= 2 * kSmCount) return 1;
   const int tiles = nk / 128;
-  auto eff = [](long long n) { return (double)n / (double)(((n + kSmCount - 1) / kSmCount) * kSmCount); };
+  auto eff = [kSmCount](long long n) { return (double)n / (double)(((n + kSmCount - 1) / kSmCount) * kSmCount); };
   int best = 1;
   double best_eff = eff(ctas);
   for (int s = 2; s <= kMaxSplits; ++s) {
@@ -178,7 +179,9 @@ BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
   return w;
 }
 
-thread_local bool tl_deterministic = false;
+// process-wide, not per thread: a backward launched by an autograd worker thread must see the flag the user set on
+// the main thread (torch runs `backward` of an autograd.Function on its own device thread)
+std::atomic<int> g_deterministic{0};
 
 // side stream + events of ringx_attn_fwd_bwd_host (host objects only; no device memory)
 struct HostOverlap {
@@ -250,6 +253,23 @@ int cuda_status(cudaError_t e) {
 }  // namespace
 
 void count_launch(int n) { tl_launches += n; }
+
+int sm_count() {
+  static int cached[kMaxDevices];   // 0 = unknown (benign race: every writer stores the same value)
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return 148;
+  }
+  if (dev >= 0 && dev < kMaxDevices && cached[dev]) return cached[dev];
+  int n = 0;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+    cudaGetLastError();
+    return 148;
+  }
+  if (dev >= 0 && dev < kMaxDevices) cached[dev] = n;
+  return n;
+}
 
 bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t rows,
                   uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz) {
@@ -531,7 +551,7 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
                     int Nq, int Nk, int d, int kv_chunk, float scale, int* dq_sem, cudaStream_t stream) {
   const long long R = (long long)BH * Nq;
   cudaError_t e;
-  if (!tl_deterministic) dq_sem = nullptr;
+  if (!g_deterministic.load(std::memory_order_relaxed)) dq_sem = nullptr;
   if (dq_sem && (e = cudaMemsetAsync(dq_sem, 0, (size_t)(R / 128) * sizeof(int), stream)) != cudaSuccess)
     return cuda_status(e);
   {
@@ -1070,11 +1090,11 @@ int ringx_attn_block_fwd(const void* x, const void* w_qkv, const void* w_o, void
 }
 
 int ringx_set_deterministic(int on) {
-  tl_deterministic = on != 0;
+  g_deterministic.store(on != 0 ? 1 : 0, std::memory_order_relaxed);
   return RINGX_OK;
 }
 
-int ringx_get_deterministic(void) { return tl_deterministic ? 1 : 0; }
+int ringx_get_deterministic(void) { return g_deterministic.load(std::memory_order_relaxed); }
 
 int ringx_last_launch_count(void) { return tl_last_launches; }
 

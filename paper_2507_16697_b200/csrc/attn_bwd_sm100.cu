@@ -25,24 +25,11 @@
 #include "kernels.cuh"
 
 namespace ringx {
-#ifdef RINGX_BWD_CLOCKS
-__device__ long long g_bwd_clocks[16];
-#define BCLK() clock64()
-#define BADD(i, v) do { if (blockIdx.x == 0 && blockIdx.y == 0 && i_ >= 8) atomicAdd((unsigned long long*)&g_bwd_clocks[i], (unsigned long long)(v)); } while (0)
-#else
-#define BCLK() 0ll
-#define BADD(i, v) do { } while (0)
-#endif
-#ifdef RINGX_BWD_TRACE
-// debug timeline: clock64 of event `ev` of step i (16 <= i < 24) of CTA (0,0), one writer thread per event
-__device__ long long g_bwd_trace[8 * 16];
-#define BTRACE(ev, step) do { if (blockIdx.x == 0 && blockIdx.y == 0 && (step) >= 16 && (step) < 24) g_bwd_trace[((step) - 16) * 16 + (ev)] = clock64(); } while (0)
-#else
-#define BTRACE(ev, step) do { } while (0)
-#endif
 namespace {
 
 using namespace ptx;
+
+__device__ unsigned g_bwd_smem_probe;   // written by the alignment probe launch (module memory: nothing is allocated)
 
 constexpr int kTile = 128;
 constexpr int kBwdThreads = 512;                 // 4 warpgroups; registers re-split with setmaxnreg
@@ -88,11 +75,17 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
                       const __grid_constant__ CUtensorMap map_dq, const float* __restrict__ lse2,
                       const float* __restrict__ Dvec,
                       __nv_bfloat16* __restrict__ dk, __nv_bfloat16* __restrict__ dv, int N, int nk_stride, int k_off,
-                      float scale_log2, float scale, int* __restrict__ dq_sem) {
+                      float scale_log2, float scale, int* __restrict__ dq_sem, unsigned* __restrict__ smem_probe) {
   using Cfg = BwdCfg<kD>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
+  // d = 128 uses every byte of the 227 KB, so it cannot round the base up: the launcher proves the alignment of this
+  // kernel's dynamic shared memory once per device with a probe launch (smem_probe != nullptr: report and return) and
+  // refuses to launch (RINGX_ERR_CUDA) if the base is not 1 KB aligned -- no trap, no abort.
+  if (smem_probe) {
+    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0) *smem_probe = smem_u32(smem_raw) & 1023u;
+    return;
+  }
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  if (Cfg::kAlignSlack == 0 && smem != smem_raw) __trap();
   uint8_t* sK = smem;
   uint8_t* sV = smem + Cfg::kTileBytes;
   uint8_t* sQ = smem + 2 * Cfg::kTileBytes;                    // [kQStages] Q_i | lse2_i | D_i
@@ -268,7 +261,6 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       // ---- behind phase A: dV += P^T(i) dO_i, then S^T(i+1)
       mbar_wait(p_full, i & 1);
       tc_fence_after();
-      if (leader) BTRACE(8, i);      // MMA warp saw p_full(i)
       if (leader) {
 #pragma unroll
         for (int k = 0; k < kTile / 16; ++k)
@@ -280,14 +272,12 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       if (more) {
         mbar_wait(&q_full[qs], qph);
         tc_fence_after();
-        if (leader) BTRACE(9, i);    // Q(i+1) there, S^T(i+1) issued
         issue_st(q_base + qs * Cfg::kQStageBytes);
       }
       // ---- behind phase B: dQ(i) = dS(i) K_j (drained under the next MMA), dK += dS^T(i) Q_i, then dP^T(i+1)
       mbar_wait(ds_full, i & 1);
       if (!Cfg::kDqOverlaysDp && i > 0) mbar_wait(dq_empty, (i - 1) & 1);
       tc_fence_after();
-      if (leader) BTRACE(10, i);     // MMA warp saw ds_full(i)
       if (leader) {
 #pragma unroll
         for (int k = 0; k < kTile / 16; ++k)
@@ -306,10 +296,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       __syncwarp();
       if (more) {
         mbar_wait(&do_full[ds], dph);
-        if (leader) BTRACE(11, i);   // dO(i+1) there
         if (Cfg::kDqOverlaysDp) mbar_wait(dq_empty, i & 1);   // dQ(i) sits in the dP^T columns until drained
         tc_fence_after();
-        if (leader) BTRACE(12, i);   // dq_empty(i) seen, dP^T(i+1) issued
         issue_dpt(do_base + ds * Cfg::kTileBytes);
       }
     }
@@ -353,15 +341,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       // ---- phase A: P^T = exp2(scale_log2 * S^T - lse2)
       // (lse2 / D are read from shared memory eight 16-byte loads at a time, ahead of the arithmetic that uses
       // them, so that their latency is paid once per half and mostly behind the mbarrier wait)
-      const int i_ = i;
-      const long long b0 = BCLK();
       float4 aux[8];
 #pragma unroll
       for (int g = 0; g < 8; ++g) aux[g] = ld_shared_v4(lse4 + g);
       mbar_wait(s_full, i & 1);
       tc_fence_after();
-      const long long b1 = BCLK();
-      if (threadIdx.x == 0) BTRACE(0, i);   // s_full(i) seen
       float2 p[32];
       {
         uint32_t s0[32], s1[32];
@@ -400,14 +384,10 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       tmem_wait_st();
       tc_fence_before();
       mbar_arrive(p_full);
-      const long long b2 = BCLK();
-      if (threadIdx.x == 0) BTRACE(1, i);   // p_full(i) arrived
       // ---- phase B: dS^T = P^T o (dP^T - D), bf16, to shared memory [keys][queries] (128B-swizzled rows)
       mbar_wait(dp_full, i & 1);
       if (i > 0) mbar_wait(ds_empty, (i - 1) & 1);
       tc_fence_after();
-      const long long b3 = BCLK();
-      if (threadIdx.x == 0) BTRACE(2, i);   // dp_full(i) (and ds_empty(i-1)) seen
       {
         uint32_t dp0[32], dp1[32];
         tmem_ld_x32(tDP, dp0);
@@ -449,8 +429,6 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       if (Cfg::kTmemOperands) tmem_wait_st();
       tc_fence_before();
       mbar_arrive(ds_full);
-      if (threadIdx.x == 0) BTRACE(3, i);   // ds_full(i) arrived
-      if (threadIdx.x == 0) { BADD(0, b1 - b0); BADD(1, b2 - b1); BADD(2, b3 - b2); BADD(3, BCLK() - b3); BADD(4, 1); }
     }
     // ---- epilogue: dV_j (warps 0-3) and dK_j (warps 4-7), bf16, written once
     mbar_wait(dkv_full, 0);
@@ -491,13 +469,9 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     int* sem = dq_sem ? dq_sem + bh * n_q : nullptr;
     int buf = 0;
     for (int i = 0; i < n_q; ++i) {
-      const int i_ = i;
-      const long long d0 = BCLK();
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
 
-      const long long d1 = BCLK();
-      if (threadIdx.x == 256) BTRACE(4, i);   // dq_full(i) seen
 #pragma unroll
       for (int rd = 0; rd < kD / 64; ++rd) {     // 64 columns per round keep the drain warps under 100 registers
         uint32_t r[2][32];
@@ -508,7 +482,6 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         if (rd == kD / 64 - 1) {
           tc_fence_before();
           mbar_arrive(dq_empty);             // the whole dQ(i) row has left TMEM: hand the columns back
-          if (threadIdx.x == 256) BTRACE(5, i);
         }
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
@@ -538,7 +511,6 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         __threadfence();
         st_release_gpu(sem + i - 1, ticket + 1);
       }
-      if (threadIdx.x == 256) { BADD(5, d1 - d0); BADD(6, BCLK() - d1); }
     }
     if (leader) {
       tma_wait_group<0>();
@@ -563,17 +535,35 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
                      int nk_stride, int k_off, int nk, float scale, int* dq_sem, cudaStream_t stream) {
   using Cfg = BwdCfg<kD>;
   auto kern = attn_chunk_bwd_kernel<kD>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
+  static unsigned char configured[kMaxDevices];
+  if (cudaError_t e = set_max_dyn_smem_once(kern, Cfg::kSmemBytes, configured); e != cudaSuccess) return e;
+  if (Cfg::kAlignSlack == 0) {
+    // first use on this device: prove that the dynamic shared memory of this kernel starts 1 KB aligned (see the kernel)
+    static unsigned char probed[kMaxDevices];    // 0 = not yet, 1 = aligned, 2 = misaligned
+    int dev = 0;
+    if (cudaError_t e = cudaGetDevice(&dev); e != cudaSuccess) return e;
+    const bool cacheable = dev >= 0 && dev < kMaxDevices;
+    if (!cacheable || !probed[dev]) {
+      unsigned* flag = nullptr;
+      unsigned h = 0xffffffffu;
+      cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&flag), g_bwd_smem_probe);
+      if (e != cudaSuccess) return e;
+      kern<<<1, 32, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0.f, 0.f,
+                                               nullptr, flag);
+      if ((e = cudaGetLastError()) != cudaSuccess) return e;
+      if ((e = cudaMemcpyAsync(&h, flag, sizeof(h), cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return e;
+      if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return e;
+      if (cacheable) probed[dev] = h == 0 ? 1 : 2;
+      if (h != 0) return cudaErrorInvalidConfiguration;
+    } else if (probed[dev] == 2) {
+      return cudaErrorInvalidConfiguration;
+    }
   }
   dim3 grid(nk / kTile, BH);
   kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D,
                                                        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv),
                                                        N, nk_stride, k_off, scale * 1.4426950408889634f, scale,
-                                                       dq_sem);
+                                                       dq_sem, nullptr);
   count_launch();
   return cudaGetLastError();
 }
@@ -599,19 +589,3 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
 
 }  // namespace ringx
 
-#ifdef RINGX_BWD_TRACE
-extern "C" __attribute__((visibility("default"))) int ringx_debug_bwd_trace(long long* out) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, ringx::g_bwd_trace, sizeof(long long) * 128);
-  return 0;
-}
-#endif
-#ifdef RINGX_BWD_CLOCKS
-extern "C" __attribute__((visibility("default"))) int ringx_debug_bwd_clocks(long long* out) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, ringx::g_bwd_clocks, sizeof(long long) * 16);
-  long long z[16] = {0};
-  cudaMemcpyToSymbol(ringx::g_bwd_clocks, z, sizeof(z));
-  return 0;
-}
-#endif

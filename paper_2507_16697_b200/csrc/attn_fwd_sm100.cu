@@ -28,12 +28,6 @@
 #include "kernels.cuh"
 
 namespace ringx {
-#ifdef RINGX_FWD_CLOCKS
-__device__ long long g_fwd_clocks[16];
-#define CLK() clock64()
-#else
-#define CLK() 0ll
-#endif
 namespace {
 
 using namespace ptx;
@@ -256,12 +250,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         for (int t = 0; t < 2; ++t) {
           const int n = 2 * j + t;
           if (t == 0) v_slot = acquire();
-          const long long m0 = CLK();
           mbar_wait(&p_full[2 * t], j & 1);
           tc_fence_after();
-#ifdef RINGX_FWD_CLOCKS
-          if (blockIdx.x == 0 && blockIdx.y == 0 && leader && j >= 8) atomicAdd((unsigned long long*)&g_fwd_clocks[8 + t], (unsigned long long)(CLK() - m0));
-#endif
           issue_o(n, t, v_slot, 0, j > 0);
           mbar_wait(&p_full[2 * t + 1], j & 1);
           tc_fence_after();
@@ -280,6 +270,11 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     const int hh = Cfg::kColSplit ? (warp >> 2) & 1 : 0;       // column split: which 64 keys of every score tile
     const uint32_t lane_off = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tO = tmem + Cfg::kOBase + t * kD + lane_off;
+    constexpr bool kFold = kEpi == kEpiFold || kEpi == kEpiFoldFinal;
+    constexpr bool kOutBf16 = kEpi == kEpiFinal || kEpi == kEpiFoldFinal;
+    size_t row = static_cast<size_t>(q_row0) + t * kBlockM + (warp & 3) * 32 + lane;   // my query row in the [BH*Nq] views
+    if (kEpi == kEpiPartial) row += static_cast<size_t>(blockIdx.z) * gridDim.y * Nq;    // this split's partials
+    float lse_prev = 0.f;          // lse_acc[row], the running LSE this pass is folded with (kFold)
     float m_raw = -CUDART_INF_F;   // running (lazy) row max of the unscaled scores
     float m_sc = -CUDART_INF_F;    // m_raw * scale_log2
     float l = 0.f;                 // running row sum of exp2(s*scale_log2 - m_sc)
@@ -374,16 +369,17 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_wait(&o_full[t], 0);                                // (also: every named barrier of the loop is behind us)
       float* slot = xch_t + (n_kv & 1) * 256;
       slot[hh * 128 + row_t] = l;
+      // Both halves of a row read the running lse, and half 0 overwrites it when the fold is in place (lse_out == lse_acc):
+      // the read sits BEFORE the pair barrier, the write after it, so the partner's read cannot see the merged value.
+      if (kFold) lse_prev = lse_acc[row];
       named_bar_sync(pair_bar, 64);
       l += slot[(hh ^ 1) * 128 + row_t];
     } else {
       for (int j = 0; j < n_kv; ++j) {
-        const long long c0 = CLK();
         const int n = 2 * j + t, buf = Cfg::kSBufs == 2 ? t : n % Cfg::kSBufs;     // this tile's scores are S number n
         const uint32_t tS = tmem + buf * kBlockN + lane_off;
         mbar_wait(&s_full[buf], (Cfg::kSBufs == 2 ? j : n / Cfg::kSBufs) & 1);
         tc_fence_after();
-        const long long c1 = CLK();
         // ---- pass 1: stream S_t(j) out of TMEM; the row max of piece c is taken while piece c+1 is in flight
         uint32_t s[kBlockN];
         auto piece = [&](int c) -> uint32_t(&)[32] { return *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]); };
@@ -461,26 +457,15 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           }
         }
         l += (la.x + la.y) + (lb.x + lb.y);
-#ifdef RINGX_FWD_CLOCKS
-        if (blockIdx.x == 0 && blockIdx.y == 0 && (threadIdx.x & 127) == 0 && j >= 8) {
-          atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 0], (unsigned long long)(c1 - c0));   // wait S
-          atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 1], (unsigned long long)(CLK() - c1));  // softmax
-          atomicAdd((unsigned long long*)&g_fwd_clocks[t * 4 + 2], 1ull);
-        }
-#endif
       }
     }
     // ---- chunk epilogue: loc_out = O / l, loc_lse = m*scale + ln l  (natural log of the scaled scores)
     mbar_wait(&o_full[t], 0);
     tc_fence_after();
-    size_t row = static_cast<size_t>(q_row0) + t * kBlockM + (warp & 3) * 32 + lane;
-    if (kEpi == kEpiPartial) row += static_cast<size_t>(blockIdx.z) * gridDim.y * Nq;   // this split's partials
-    constexpr bool kFold = kEpi == kEpiFold || kEpi == kEpiFoldFinal;
-    constexpr bool kOutBf16 = kEpi == kEpiFinal || kEpi == kEpiFoldFinal;
     float lse_row = (m_sc + lg2(l)) * 0.6931471805599453f;
     float cb = 1.0f / l, ca = 0.f;            // out = ca * o_acc + cb * O  (O = unnormalised accumulator in TMEM)
     if (kFold) {                              // Eq. 5, two operands: (o_acc, lse_acc) and (loc_out, loc_lse)
-      const float la = lse_acc[row];
+      const float la = Cfg::kColSplit ? lse_prev : lse_acc[row];
       const float m = fmaxf(la, lse_row);
       const float wa = ex2((la - m) * 1.4426950408889634f), wb = ex2((lse_row - m) * 1.4426950408889634f);
       const float den = wa + wb, r = 1.0f / den;
@@ -545,12 +530,8 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
                      float scale, int splits, cudaStream_t stream) {
   using Cfg = FwdCfg<kD>;
   auto kern = attn_chunk_fwd_kernel<kD, kEpi>;
-  static bool configured = false;   // benign race: the attribute is idempotent
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static unsigned char configured[kMaxDevices];
+  if (cudaError_t e = set_max_dyn_smem_once(kern, Cfg::kSmemBytes, configured); e != cudaSuccess) return e;
   dim3 grid(Nq / (2 * kBlockM), BH, splits);
   kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, Nq, nk_stride, k_off,
                                                        nk / kBlockN / splits, scale * 1.4426950408889634f);
@@ -593,12 +574,3 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
 
 }  // namespace ringx
 
-#ifdef RINGX_FWD_CLOCKS
-extern "C" __attribute__((visibility("default"))) int ringx_debug_clocks(long long* out) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, ringx::g_fwd_clocks, sizeof(long long) * 16);
-  long long z[16] = {0};
-  cudaMemcpyToSymbol(ringx::g_fwd_clocks, z, sizeof(z));
-  return 0;
-}
-#endif

@@ -87,4 +87,25 @@ bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, in
 
 void count_launch(int n = 1);
 
+// ---- per-device state (api.cu).  The C ABI promises that anything cached is cached per DEVICE, not per process
+// (SURVEY.md §8(b)): one process may call on several GPUs.
+constexpr int kMaxDevices = 64;
+// multiprocessors of the current device, cached per device (148 on B200); 148 when no device can be queried
+// (the workspace-size queries also run on boxes without a GPU)
+int sm_count();
+// cudaFuncAttributeMaxDynamicSharedMemorySize, once per (kernel, device): `done` is the call site's own static array.
+// The attribute is idempotent, so the unsynchronised flag is a benign race.
+template <typename Kern>
+inline cudaError_t set_max_dyn_smem_once(Kern kern, int bytes, unsigned char (&done)[kMaxDevices]) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const bool cacheable = dev >= 0 && dev < kMaxDevices;
+  if (cacheable && done[dev]) return cudaSuccess;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return e;
+  if (cacheable) done[dev] = 1;
+  return cudaSuccess;
+}
+
 }  // namespace ringx

@@ -123,7 +123,7 @@ cudaError_t launch_merge_t(const void* o_a, const float* lse_a, const void* o_b,
   if (vecs < 32 && (vecs & (vecs - 1)) == 0) lanes = vecs;
   const long long rows_per_block = (long long)(kMergeThreads / 32) * (32 / lanes) * kRowUnroll;
   long long blocks = (rows + rows_per_block - 1) / rows_per_block;
-  const long long max_blocks = 148LL * 8 * 4;   // 8 CTAs of 256 threads per SM, 4 waves
+  const long long max_blocks = (long long)sm_count() * 8 * 4;   // 8 CTAs of 256 threads per SM, 4 waves
   if (blocks > max_blocks) blocks = max_blocks;
   if (blocks < 1) blocks = 1;
 #define RINGX_MERGE_CASE(L)                                                                                     \
@@ -149,8 +149,8 @@ cudaError_t launch_merge_t(const void* o_a, const float* lse_a, const void* o_b,
 // lse_max is the all-reduce(max) of loc_lse over the devices; an operand with loc_lse = -inf (or a row whose
 // lse_max is -inf) contributes 0 and its loc_out is not read into the result.  One thread per float4.
 __global__ void __launch_bounds__(256)
-eq5_scale_kernel(const float4* __restrict__ loc_out, const float* __restrict__ loc_lse,
-                 const float* __restrict__ lse_max, float4* __restrict__ num, float* __restrict__ den, long long rows,
+eq5_scale_kernel(const float4* loc_out, const float* __restrict__ loc_lse,     // num may alias loc_out (in place):
+                 const float* __restrict__ lse_max, float4* num, float* __restrict__ den, long long rows,   // no restrict
                  int vecs) {
   const long long total = rows * vecs, stride = (long long)gridDim.x * blockDim.x;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
@@ -170,8 +170,8 @@ eq5_scale_kernel(const float4* __restrict__ loc_out, const float* __restrict__ l
 // After the sums: o = num / den, lse = lse_max + ln(den); den = 0 (every operand empty) gives o = 0, lse = -inf.
 template <typename TOut>
 __global__ void __launch_bounds__(256)
-eq5_finalize_kernel(const float4* __restrict__ num, const float* __restrict__ den, const float* __restrict__ lse_max,
-                    void* __restrict__ o_out, float* __restrict__ lse_out, long long rows, int vecs) {
+eq5_finalize_kernel(const float4* num, const float* __restrict__ den, const float* lse_max,   // o_out may alias num and
+                    void* o_out, float* lse_out, long long rows, int vecs) {                  // lse_out lse_max: no restrict
   const long long total = rows * vecs, stride = (long long)gridDim.x * blockDim.x;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
     const long long r = i / vecs;
@@ -194,8 +194,8 @@ constexpr int kMaxSplits = 8;
 template <typename TOut>
 __global__ void __launch_bounds__(256)
 split_merge_kernel(const float4* __restrict__ parts, const float* __restrict__ lses, long long part_stride_vecs,
-                   long long rows, int s, const float4* __restrict__ o_acc, const float* __restrict__ lse_acc,
-                   void* __restrict__ o_out, float* __restrict__ lse_out, int vecs) {
+                   long long rows, int s, const float4* o_acc, const float* __restrict__ lse_acc,   // o_out may alias
+                   void* o_out, float* __restrict__ lse_out, int vecs) {                           // o_acc: no restrict
   const long long total = rows * vecs, stride = (long long)gridDim.x * blockDim.x;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
     const long long r = i / vecs;
@@ -309,7 +309,7 @@ cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_
 
 static unsigned eq5_blocks(long long total) {
   long long blocks = (total + 255) / 256;
-  if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
+  if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
   return (unsigned)(blocks < 1 ? 1 : blocks);
 }
 
@@ -354,7 +354,7 @@ cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* ls
   const int lanes = d / 8;   // 8 or 16
   const long long rows_per_block = 8LL * (32 / lanes) * 4;
   long long blocks = (rows + rows_per_block - 1) / rows_per_block;
-  if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
+  if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
   if (lanes == 8)
     bwd_preprocess_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, lse, D, lse2,
                                                                    (float4*)dq_acc, rows, scale, zero_dq);
@@ -367,7 +367,7 @@ cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* ls
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream) {
   const long long n4 = n / 4;
   long long blocks = (n4 + 255) / 256;
-  if (blocks > 148LL * 8 * 4) blocks = 148LL * 8 * 4;
+  if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
   dq_convert_kernel<<<(unsigned)blocks, 256, 0, stream>>>((const float4*)dq_acc, (uint2*)dq, n4, scale);
   return cudaGetLastError();
 }

@@ -295,27 +295,13 @@ proj_gemm_kernel(const __grid_constant__ CUtensorMap map_a0, const __grid_consta
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
-int sm_count() {
-  static int n = 0;
-  if (!n) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-  }
-  return n;
-}
-
 template <int kMode>
 cudaError_t launch_mode(const CUtensorMap& a0, const CUtensorMap& a1, const CUtensorMap& a2, const CUtensorMap& mb,
                         const CUtensorMap& c0, const CUtensorMap& c1, const CUtensorMap& c2, const ProjParams& p,
                         cudaStream_t stream) {
   auto kern = proj_gemm_kernel<kMode>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kProjSmem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static unsigned char configured[kMaxDevices];
+  if (cudaError_t e = set_max_dyn_smem_once(kern, kProjSmem, configured); e != cudaSuccess) return e;
   const int items = p.m_tiles * p.n_tiles * p.splits;
   const int grid = items < sm_count() ? items : sm_count();
   kern<<<grid, kProjThreads, kProjSmem, stream>>>(a0, a1, a2, mb, c0, c1, c2, p);

@@ -296,7 +296,7 @@ def ringx_attn_fwd_bwd_host(q_host, k_host, v_host, dO_host, kv_chunk: int, scal
 
 
 def ringx_set_deterministic(on: bool) -> None:
-    """Bit-reproducible dQ on the calling thread (include/ringx.h: ringx_set_deterministic)."""
+    """Bit-reproducible dQ, process-wide (include/ringx.h: ringx_set_deterministic)."""
     _check(lib().ringx_set_deterministic(1 if on else 0), "ringx_set_deterministic")
 
 
