@@ -10,6 +10,7 @@ import numpy as np
 import pytest
 import torch
 
+import grad_bounds as gb
 from oracle import attention as orc
 from paper_2507_16697_b200 import workloads as wl
 
@@ -75,23 +76,22 @@ def test_C2_full_size(rx):
     assert ((o1.float() - o.float()).norm() / o.float().norm()).item() <= 4e-3
 
 
-def elementwise_excess(gn, ref):
-    """max_e |g_e - ref_e| / (2^-7 |ref_e| + 8 * 2^-8 * rms(ref)); see tests/test_gpu_parity.py::elementwise_excess."""
-    rms = np.sqrt(np.mean(ref * ref))
-    return float((np.abs(gn - ref) / (2.0 ** -7 * np.abs(ref) + 8.0 * 2.0 ** -8 * rms)).max())
-
-
-def check_grad_np(name, gn, ref, tol=2e-2):
-    assert np.isfinite(gn).all(), name
-    e = np.linalg.norm(gn - ref) / np.linalg.norm(ref)
-    assert e <= tol, (name, e)
-    x = elementwise_excess(gn, ref)
-    assert x <= 1.0, (name, "element-wise bound exceeded", x)
-    return e
-
-
 def np64(t):
     return t.float().cpu().double().numpy()
+
+
+def all_row_stats(q64, k64, v64, do64, scale, block=2048):
+    """(LSE_i, D_i, E_i) of EVERY query row of a head from the oracle's forward (one full 4 N^2 d fp64 pass): what a
+    key-column check of dK/dV needs.  D_i = dO_i . O_i (oracle.row_stats); E_i = 2^-9 sum_c |dO_ic| |O_ic| bounds the
+    error of the kernel's D_i, which is formed from the saved bf16 O (tests/grad_bounds.py)."""
+    N = q64.shape[0]
+    lse, D, E = np.empty(N), np.empty(N), np.empty(N)
+    for r0 in range(0, N, block):
+        sl = slice(r0, r0 + block)
+        o, lse[sl] = orc.attention_fwd(q64[sl], k64, v64, scale)
+        D[sl] = (do64[sl] * o).sum(axis=1)
+        E[sl] = gb.U_BF16 * (np.abs(do64[sl]) * np.abs(o)).sum(axis=1)
+    return lse, D, E
 
 
 def test_C3_full_size(rx):
@@ -133,7 +133,7 @@ def test_C3_full_size_forward_and_backward(rx):
         assert np.abs(og - o_ref).max() <= 1e-2 * np.abs(v64).max()
         assert np.linalg.norm(og - o_ref) / np.linalg.norm(o_ref) <= 1e-2
         assert np.abs(lse[b, h][rows].cpu().double().numpy() - lse_ref).max() <= 1e-3
-        check_grad_np("dq", np64(dq[b, h][rows]), dq_ref)
+        gb.check_grad("dq", np64(dq[b, h][rows]), dq_ref, gb.dq_dterm(q64, k64, v64, do64, cfg.scale))
     sum_dv, sum_do = dv.float().sum(dim=2), do.float().sum(dim=2)
     assert ((sum_dv - sum_do).norm() / sum_do.norm()).item() <= 1e-2
     assert (dk.float().sum(dim=2).norm() / dk.float().abs().sum(dim=2).norm()).item() <= 1e-2
@@ -153,9 +153,11 @@ def test_C3_full_size_forward_and_backward(rx):
         k64, v64 = wl.to_f64_numpy(k[b, h]), wl.to_f64_numpy(v[b, h])
         q64, do64 = wl.to_f64_numpy(q[b, h][rows]), wl.to_f64_numpy(do[b, h][rows])
         dq_ref, dk_ref, dv_ref = orc.attention_bwd(q64, k64, v64, do64, cfg.scale)
-        check_grad_np("dq(sparse)", np64(dq[b, h][rows]), dq_ref)
-        check_grad_np("dk(all keys)", np64(dk[b, h]), dk_ref)
-        check_grad_np("dv(all keys)", np64(dv[b, h]), dv_ref)
+        E = gb.d_error_rows(q64, k64, v64, do64, cfg.scale)
+        _, lse_rows = orc.attention_fwd(q64, k64, v64, cfg.scale)
+        gb.check_grad("dq(sparse)", np64(dq[b, h][rows]), dq_ref, gb.dq_dterm(q64, k64, v64, do64, cfg.scale))
+        gb.check_grad("dk(all keys)", np64(dk[b, h]), dk_ref, gb.dk_dterm(q64, k64, lse_rows, E, cfg.scale))
+        gb.check_grad("dv(all keys)", np64(dv[b, h]), dv_ref)
 
 
 def test_C5_full_size_peaked(rx):
@@ -204,15 +206,11 @@ def test_C4_full_size_forward_and_backward(rx):
         assert np.abs(og - o_ref).max() <= 1e-2 * np.abs(v64).max()
         assert np.linalg.norm(og - o_ref) / np.linalg.norm(o_ref) <= 1e-2
         assert np.abs(lse[b, h][rows].cpu().double().numpy() - lse_ref).max() <= 1e-3
-        check_grad_np("dq", np64(dq[b, h][rows]), dq_ref)
+        gb.check_grad("dq", np64(dq[b, h][rows]), dq_ref, gb.dq_dterm(q64, k64, v64, do64, cfg.scale))
     # ---- sampled key columns of one head: dK, dV (tile / chunk boundaries + random)
     b, h = 1, 3
     q64, k64, v64, do64 = (wl.to_f64_numpy(t[b, h]) for t in (q, k, v, do))
-    lse_all = np.empty(cfg.N)
-    D_all = np.empty(cfg.N)
-    for r0 in range(0, cfg.N, 2048):
-        lse_all[r0:r0 + 2048], D_all[r0:r0 + 2048] = orc.row_stats(q64[r0:r0 + 2048], k64, v64, do64[r0:r0 + 2048],
-                                                                   cfg.scale)
+    lse_all, D_all, E_all = all_row_stats(q64, k64, v64, do64, cfg.scale)
     assert np.abs(lse[b, h].cpu().double().numpy() - lse_all).max() <= 1e-3       # every row of the head
     C = cfg.kv_chunk
     cols = sorted(set([0, 127, 128, C - 1, C, C + 127, 3 * C - 1, 3 * C, cfg.N - 128, cfg.N - 1])
@@ -221,8 +219,8 @@ def test_C4_full_size_forward_and_backward(rx):
     dk_ref, dv_ref = orc.attention_bwd_cols(q64, k64[cols], v64[cols], do64, lse_all, D_all, cfg.scale)
     dkg = dk[b, h][cols].float().cpu().double().numpy()
     dvg = dv[b, h][cols].float().cpu().double().numpy()
-    check_grad_np("dk(cols)", dkg, dk_ref)
-    check_grad_np("dv(cols)", dvg, dv_ref)
+    gb.check_grad("dk(cols)", dkg, dk_ref, gb.dk_dterm(q64, k64[cols], lse_all, E_all, cfg.scale))
+    gb.check_grad("dv(cols)", dvg, dv_ref)
     # ---- invariants on the full output (every head)
     sum_dv, sum_do = dv.float().sum(dim=2), do.float().sum(dim=2)
     assert ((sum_dv - sum_do).norm() / sum_do.norm()).item() <= 1e-2
@@ -239,7 +237,8 @@ def test_C3_shape_backward_d128_sampled(rx):
     rows = sample_rows(N, 48, seed=5)
     k64, v64 = wl.to_f64_numpy(k[0, 1]), wl.to_f64_numpy(v[0, 1])
     dq_ref, _, _ = orc.attention_bwd(wl.to_f64_numpy(q[0, 1][rows]), k64, v64, wl.to_f64_numpy(do[0, 1][rows]), scale)
-    check_grad_np("dq", np64(dq[0, 1][rows]), dq_ref)
+    gb.check_grad("dq", np64(dq[0, 1][rows]), dq_ref,
+                  gb.dq_dterm(wl.to_f64_numpy(q[0, 1][rows]), k64, v64, wl.to_f64_numpy(do[0, 1][rows]), scale))
     sum_dv, sum_do = dv.float().sum(dim=2), do.float().sum(dim=2)
     assert ((sum_dv - sum_do).norm() / sum_do.norm()).item() <= 1e-2
     assert (dk.float().sum(dim=2).norm() / dk.float().abs().sum(dim=2).norm()).item() <= 1e-2
@@ -248,13 +247,11 @@ def test_C3_shape_backward_d128_sampled(rx):
     # key-tile and chunk boundaries plus random ones.
     b, h = 0, 0
     q64, k64, v64, do64 = (wl.to_f64_numpy(t[b, h]) for t in (q, k, v, do))
-    lse_all, D_all = np.empty(N), np.empty(N)
-    for r0 in range(0, N, 2048):
-        lse_all[r0:r0 + 2048], D_all[r0:r0 + 2048] = orc.row_stats(q64[r0:r0 + 2048], k64, v64, do64[r0:r0 + 2048], scale)
+    lse_all, D_all, E_all = all_row_stats(q64, k64, v64, do64, scale)
     assert np.abs(lse[b, h].cpu().double().numpy() - lse_all).max() <= 1e-3       # every row of the head
     cols = sorted(set([0, 1, 127, 128, 129, chunk - 1, chunk, chunk + 127, 2 * chunk - 1, 2 * chunk, 3 * chunk + 64,
                        N - 129, N - 128, N - 1]) | set(np.random.default_rng(73).integers(0, N, 82).tolist()))
     cols = np.array(cols)
     dk_ref, dv_ref = orc.attention_bwd_cols(q64, k64[cols], v64[cols], do64, lse_all, D_all, scale)
-    check_grad_np("dk(cols)", np64(dk[b, h][cols]), dk_ref)
-    check_grad_np("dv(cols)", np64(dv[b, h][cols]), dv_ref)
+    gb.check_grad("dk(cols)", np64(dk[b, h][cols]), dk_ref, gb.dk_dterm(q64, k64[cols], lse_all, E_all, scale))
+    gb.check_grad("dv(cols)", np64(dv[b, h][cols]), dv_ref)
