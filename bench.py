@@ -369,10 +369,11 @@ def main():
     # ---------------------------------------------------------------- short side measurements (not the metric)
     extra = {}
     if rank == 0 and not args.no_extra:
+        extra["C1"] = c1_measure(ringx, wl, dev)
         for name in ("C2", "C4", "C5"):
             if name == cfg.name:
                 continue
-            extra[name] = side_measure(ringx, wl, wl.CONFIGS[name], dev)
+            extra[name] = side_measure(ringx, wl, wl.CONFIGS[name], dev, oracle_seconds=args.cpu_baseline_seconds / 5.0)
         extra["next_rows"] = next_rows_measure(ringx, wl, dev)
 
     # ---------------------------------------------------------------- CPU baseline: the oracle, bounded sample
@@ -388,7 +389,12 @@ def main():
                         "seconds": dt,
                         "sample": f"first {n_rows} query rows of head (0,0) against all {N} keys "
                                   f"(oracle.attention_fwd" + (" + attention_bwd" if do_bwd else "") +
-                                  ", fp64 numpy, blocks of 256 rows)"}
+                                  ", fp64 numpy, blocks of 256 rows)",
+                        "full_config_seconds_extrapolated": flops_step / (fl / dt),
+                        "extrapolation": "linear in query rows x heads",
+                        # the other BASELINE.json configs: measured sample + labelled extrapolation each
+                        "per_config": {name: extra[name]["cpu_baseline"] for name in extra
+                                       if isinstance(extra[name], dict) and "cpu_baseline" in extra[name]}}
 
     if rank == 0:
         line = {
@@ -409,8 +415,55 @@ def main():
         dist.destroy_process_group()
 
 
-def side_measure(ringx, wl, cfg, dev, reps=3):
-    """A short forward (and backward) timing of another BASELINE.json config; context, not the metric."""
+def timed_loop(fn, min_seconds=0.5, min_reps=5, max_reps=400):
+    """Per-call CUDA-event timings of `fn` after a warm loop of >= min_seconds (so that clocks and power have settled
+    where they will sit under this kernel), collected for >= min_seconds and >= min_reps calls.  Returns the list of ms."""
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    n_warm = 0
+    while n_warm < 3 or time.perf_counter() - t0 < min_seconds:
+        fn()
+        torch.cuda.synchronize()
+        n_warm += 1
+    per_call = max((time.perf_counter() - t0) / n_warm, 1e-5)
+    reps = int(min(max_reps, max(min_reps if per_call < 0.5 else 3, math.ceil(min_seconds / per_call))))
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    for a, b in evs:
+        a.record()
+        fn()
+        b.record()
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in evs]
+
+
+def summarise(ms_list, flops):
+    med, best = float(np.median(ms_list)), float(min(ms_list))
+    return {"ms_median": med, "ms_best": best, "reps": len(ms_list), "tflops_median": flops / med / 1e9,
+            "tflops_best": flops / best / 1e9}
+
+
+def oracle_extrapolated(cfg, q, k, v, do, seconds):
+    """cpu_baseline of a config: the oracle as it stands on a sample of query rows of head (0,0) against all keys, sized
+    for ~`seconds` of CPU work; the time for the whole config is a LINEAR EXTRAPOLATION (rows are independent), labelled so."""
+    from paper_2507_16697_b200 import workloads as wl
+    k64, v64 = wl.to_f64_numpy(k[0, 0]), wl.to_f64_numpy(v[0, 0])
+    cap = min(cfg.N, 4096)
+    q64 = wl.to_f64_numpy(q[0, 0, :cap])
+    do64 = wl.to_f64_numpy(do[0, 0, :cap]) if do is not None else None
+    n0 = min(32, cap)
+    dt0, _ = oracle_sample(cfg, k64, v64, q64[:n0], do64[:n0] if do64 is not None else None, block=64)
+    n_rows = int(min(cap, max(n0, seconds / (dt0 / n0) // 32 * 32)))
+    dt, fl = oracle_sample(cfg, k64, v64, q64[:n_rows], do64[:n_rows] if do64 is not None else None, block=64)
+    full = cfg.fwd_flops + (cfg.bwd_flops if do is not None else 0.0)
+    return {"value": fl / dt / 1e12, "unit": UNIT, "cores": host_cores(), "kind": "oracle", "seconds": dt,
+            "sample": f"first {n_rows} query rows of head (0,0) against all {cfg.N} keys (oracle.attention_fwd"
+                      + (" + attention_bwd" if do is not None else "") + ", fp64 numpy)",
+            "full_config_seconds_extrapolated": full / (fl / dt), "extrapolation": "linear in query rows x heads"}
+
+
+def side_measure(ringx, wl, cfg, dev, oracle_seconds=0.0):
+    """Forward (and backward) timing of another BASELINE.json config; context, not the metric.  Each call is timed on its
+    own with CUDA events for >= 0.5 s after a >= 0.5 s warm loop; median and best are both reported."""
     tensors = wl.make_qkv(cfg, with_do=cfg.backward, device=dev)
     q, k, v = tensors[:3]
     B, H, N, d = q.shape
@@ -419,33 +472,36 @@ def side_measure(ringx, wl, cfg, dev, reps=3):
     ws = torch.empty(max(256, ringx.ringx_attn_fwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
                      dtype=torch.uint8, device=dev)
     out = {}
-
-    def timeit(fn):
-        for _ in range(3):
-            fn()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(reps):
-            fn()
-        e1.record()
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / reps
-
-    ms = timeit(lambda: ringx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale, o=o, lse=lse, workspace=ws))
-    out["fwd_ms"] = ms
-    out["fwd_tflops"] = cfg.fwd_flops / ms / 1e9
+    r = summarise(timed_loop(lambda: ringx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale, o=o, lse=lse, workspace=ws)),
+                  cfg.fwd_flops)
+    out["fwd"] = r
+    out["fwd_ms"], out["fwd_tflops"] = r["ms_median"], r["tflops_median"]
     if cfg.backward:
         wsb = torch.empty(max(256, ringx.ringx_attn_bwd_workspace_bytes(B, H, N, d, cfg.kv_chunk, q.dtype)),
                           dtype=torch.uint8, device=dev)
-        try:
-            ms = timeit(lambda: ringx.ringx_attn_bwd(q, k, v, o, lse, tensors[3], cfg.kv_chunk, cfg.scale,
-                                                     workspace=wsb))
-            out["bwd_ms"] = ms
-            out["bwd_tflops"] = cfg.bwd_flops / ms / 1e9
-        except ringx.RingxError as e:
-            out["bwd"] = f"unavailable: {e}"
+        dq, dk, dv = torch.empty_like(q), torch.empty_like(q), torch.empty_like(q)
+        r = summarise(timed_loop(lambda: ringx.ringx_attn_bwd(q, k, v, o, lse, tensors[3], cfg.kv_chunk, cfg.scale,
+                                                              workspace=wsb, dq=dq, dk=dk, dv=dv)), cfg.bwd_flops)
+        out["bwd"] = r
+        out["bwd_ms"], out["bwd_tflops"] = r["ms_median"], r["tflops_median"]
+    if oracle_seconds > 0:
+        out["cpu_baseline"] = oracle_extrapolated(cfg, q, k, v, tensors[3] if cfg.backward else None, oracle_seconds)
     return out
+
+
+def c1_measure(ringx, wl, dev):
+    """BASELINE.json configs[0] (fp32, N = 1024, 4 chunks): the FFMA path's time and the oracle's, both on the whole config."""
+    from oracle import attention as orc
+    cfg = wl.CONFIGS["C1"]
+    q, k, v = wl.make_qkv(cfg, device=dev)
+    r = summarise(timed_loop(lambda: ringx.ringx_attn_fwd(q, k, v, cfg.kv_chunk, cfg.scale), min_seconds=0.2), cfg.fwd_flops)
+    q64, k64, v64 = (wl.to_f64_numpy(t[0, 0]) for t in (q, k, v))
+    t0 = time.perf_counter()
+    orc.attention_fwd_chunked(q64, k64, v64, cfg.scale, list(range(0, cfg.N + 1, cfg.kv_chunk)))
+    dt = time.perf_counter() - t0
+    return {"fwd": r, "cpu_baseline": {"value": cfg.fwd_flops / dt / 1e12, "unit": UNIT, "cores": host_cores(),
+                                       "kind": "oracle", "seconds": dt,
+                                       "sample": "the whole config (oracle.attention_fwd_chunked, 4 chunks of 256)"}}
 
 
 def next_rows_measure(ringx, wl, dev, reps=5):
