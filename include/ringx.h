@@ -275,7 +275,7 @@ RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d,
 /* Bit-reproducible dQ.  By default the per-key-tile contributions to dQ are reduce-added into the fp32
  * accumulator in whatever order the CTAs reach them (fp32 addition is not associative: the last bits of dq may differ from run
  * to run; dk, dv are always bit-reproducible).  With the flag set -- it is process-wide, so that a backward issued from another
- * thread (PyTorch's autograd worker) sees it -- ringx_attn_bwd, ringx_attn_bwd_gqa and ringx_attn_bwd_partial add the
+ * thread (a framework's autograd worker thread) sees it -- ringx_attn_bwd, ringx_attn_bwd_gqa and ringx_attn_bwd_partial add the
  * contributions to every dQ tile in key-tile order (a ticket counter per tile in the workspace): the same inputs, shapes and
  * kv_chunk give bit-identical dq.  Costs about a third of the backward throughput (the CTAs proceed as a convoy).  The weight
  * gradients of ringx_*_proj_bwd are not covered (split-K partial sums are reduce-added in arbitrary order). */

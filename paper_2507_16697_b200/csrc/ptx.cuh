@@ -87,6 +87,10 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const void* tmap, ui
       ::"r"(smem_u32(smem_dst)), "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "l"(policy)
       : "memory");
 }
+// L2 prefetch of a 2-D tile (no shared-memory destination, no completion to wait for)
+__device__ __forceinline__ void tma_prefetch_2d(const void* tmap, int c0, int c1) {
+  asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(tmap), "r"(c0), "r"(c1) : "memory");
+}
 // 1-D bulk copy global -> shared (bytes % 16 == 0, both addresses 16-byte aligned), completion on an mbarrier
 __device__ __forceinline__ void bulk_load_1d(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -127,6 +131,35 @@ __device__ __forceinline__ uint64_t policy_evict_normal() {
   uint64_t p;
   asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
   return p;
+}
+
+// ---------------------------------------------------------------- cluster launch control (hardware work stealing)
+// A running CTA asks the hardware to CANCEL the launch of a CTA of the same grid that has not started yet and takes over
+// its block index: a persistent kernel whose work items are handed out by the block scheduler itself (dynamic, in
+// launch order, no global counter).  The 16-byte response lands in shared memory asynchronously (mbarrier tx bytes).
+// Once a request has FAILED (no CTA left to cancel) the CTA must not issue another one.
+__device__ __forceinline__ void clc_try_cancel(void* smem_response16, uint64_t* bar) {
+  asm volatile("clusterlaunchcontrol.try_cancel.async.shared::cta.mbarrier::complete_tx::bytes.b128 [%0], [%1];"
+               ::"r"(smem_u32(smem_response16)), "r"(smem_u32(bar))
+               : "memory");
+}
+// decode a response: returns true and the cancelled CTA's blockIdx (x, y, z) when the request succeeded
+__device__ __forceinline__ bool clc_query(const void* smem_response16, int& x, int& y, int& z) {
+  uint32_t ok, cx, cy, cz;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b128 r;\n\t"
+      "ld.shared.b128 r, [%4];\n\t"
+      "clusterlaunchcontrol.query_cancel.is_canceled.pred.b128 p, r;\n\t"
+      "selp.u32 %3, 1, 0, p;\n\t"
+      "mov.u32 %0, 0;\n\tmov.u32 %1, 0;\n\tmov.u32 %2, 0;\n\t"
+      "@p clusterlaunchcontrol.query_cancel.get_first_ctaid.v4.b32.b128 {%0, %1, %2, _}, r;\n\t}"
+      : "=r"(cx), "=r"(cy), "=r"(cz), "=r"(ok)
+      : "r"(smem_u32(smem_response16))
+      : "memory");
+  x = static_cast<int>(cx);
+  y = static_cast<int>(cy);
+  z = static_cast<int>(cz);
+  return ok != 0;
 }
 
 // ---------------------------------------------------------------- tcgen05: TMEM management
