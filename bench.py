@@ -190,6 +190,10 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=256, help="query rows per step of the reference arm")
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0)
     ap.add_argument("--no-extra", action="store_true", help="skip the short C2/C4 side measurements")
+    ap.add_argument("--schedule", default="replicas", choices=["replicas", "ringx_b", "ringx_a"],
+                    help="replicas (default: the single-GPU hot path, one seeded batch per rank) or one of the paper's "
+                         "sequence-parallel schedules over the ranks (PAPER.md:137-147): the config's sequence is sharded "
+                         "over the W ranks and every step is one RingX forward + backward")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -217,6 +221,9 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
         dist.barrier()
     ringx.lib()
+    if args.schedule != "replicas":
+        run_schedule(args, cfg, rank, world, dev, dist)
+        return
 
     def barrier():
         if dist is not None:
@@ -413,6 +420,80 @@ def main():
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def run_schedule(args, cfg, rank, world, dev, dist):
+    """--schedule ringx_b | ringx_a: the paper's schedules (paper_2507_16697_b200/ringx_dist.py) over the W ranks of the
+    launch.  Every rank holds N/W tokens of every head; a step is one forward + one backward of the WHOLE sequence
+    (strong scaling: the work per step is fixed, `value` = its FLOPs over the slowest rank's time).  No multi-GPU box
+    has been available to this project: at W = 1 this is the single-device path behind the same interface."""
+    from paper_2507_16697_b200 import multirank, ringx, ringx_dist, workloads as wl
+    if dist is None:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+    B, H, N, d = cfg.B, cfg.H, cfg.N, cfg.d
+    Nl = N // world
+    if N % world or Nl % 256:
+        raise SystemExit(f"--schedule needs N / W to be a multiple of 256 (N = {N}, W = {world})")
+    fwd, bwd = ((ringx_dist.ringx_b_forward, ringx_dist.ringx_b_backward) if args.schedule == "ringx_b" else
+                (ringx_dist.ringx_a_forward, ringx_dist.ringx_a_backward))
+
+    def local(which):          # this rank's sequence chunk of the config's seeded tensor (same bits as the single-GPU run)
+        full = wl.make_tensor(cfg, which, device=dev)
+        return full[:, :, rank * Nl:(rank + 1) * Nl].contiguous()
+
+    q, k, v, dO = local("q"), local("k"), local("v"), local("do")
+    comm = ringx_dist.TorchComm()
+
+    def step():
+        o, lse, ctx = fwd(q, k, v, cfg.scale, comm=comm)
+        return (o, lse) + tuple(bwd(ctx, dO, comm=comm))
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index or 0) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    ms_step = multirank.max_over_ranks(e0.elapsed_time(e1), dist if world > 1 else None, dev) / args.steps
+    flops = cfg.fwd_flops + cfg.bwd_flops
+    # end to end: pinned host chunks up, the schedule step, the local results down
+    host = [t.cpu().pin_memory() for t in (q, k, v, dO)]
+    t0 = time.perf_counter()
+    dq_, dk_, dv_, do_ = (h.to(dev, non_blocking=True) for h in host)
+    o, lse, ctx = fwd(dq_, dk_, dv_, cfg.scale, comm=comm)
+    outs = [t.cpu() for t in (o, lse) + tuple(bwd(ctx, do_, comm=comm))]
+    torch.cuda.synchronize()
+    dt = multirank.max_over_ranks(time.perf_counter() - t0, dist if world > 1 else None, dev)
+    tb = q.numel() * q.element_size()
+    if rank == 0:
+        peaks = load_peaks()
+        value = flops / ms_step / 1e9
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "bf16",
+                "data": "synthetic", "config": dict(workload_config(cfg, "fwd+bwd"), schedule=args.schedule,
+                                                    tokens_per_rank=Nl),
+                "clocks": clocks,
+                "e2e": {"value": flops / dt / 1e12, "unit": UNIT, "ms_per_step": dt * 1e3, "steps": 1,
+                        "h2d_bytes_per_step": 4 * tb * world, "d2h_bytes_per_step": (4 * tb + lse.numel() * 4) * world,
+                        "entry": f"ringx_dist {args.schedule} forward + backward on pinned host chunks"},
+                "gpu_launches": None, "roofline": None, "cpu_baseline": None,
+                "frac_of_bf16_peak": {"sustained": value / world / peaks["bf16_tflops_sustained"], "source": peaks["source"]}}
+        print(json.dumps(line), flush=True)
+    dist.barrier()
+    dist.destroy_process_group()
 
 
 def timed_loop(fn, min_seconds=0.5, min_reps=5, max_reps=400):

@@ -171,6 +171,21 @@ RINGX_API int ringx_attn_bwd_partial(const void* q, const void* k, const void* v
                            void* workspace, size_t workspace_bytes, void* stream);
 RINGX_API size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d);
 
+/* ringx_attn_bwd_partial in its general form, as the RingX_a / RingX_b schedules call it once per step (l.143, l.145):
+ *   dkv_dtype  RINGX_BF16: dk, dv [B,H,Nk,d] bf16 (as ringx_attn_bwd_partial).
+ *              RINGX_F32 : dk, dv [B,H,Nk,d] FLOAT -- the fp32 accumulators written unrounded.  A device's dK,dV of a step are
+ *              only its SHARE of a sum over devices (reduce / reduce-scatter, l.143, l.145): reducing fp32 shares and
+ *              rounding once keeps the single-device accuracy, where bf16 shares would be rounded W times and then summed
+ *              in bf16.
+ *   prepared   0: the call first forms D_i = dO_i.O_i and the exp2-domain lse of the Nq rows in the workspace.
+ *              1: the workspace still holds them from an earlier call with the same (o, lse, dO, scale, shape) -- every
+ *              step of one backward after the first: the preprocess runs once per backward, not once per step.
+ * Everything else as ringx_attn_bwd_partial. */
+RINGX_API int ringx_attn_bwd_partial_ex(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                              const void* dO, float* dq_acc, void* dk, void* dv,
+                              int B, int H, int Nq, int Nk, int d, float scale, int dtype, int dkv_dtype, int prepared,
+                              void* workspace, size_t workspace_bytes, void* stream);
+
 /* dq = bf16(dq_acc), n elements (n % 4 == 0), round to nearest even: closes the accumulation over steps. */
 RINGX_API int ringx_dq_finalize(const float* dq_acc, void* dq, long long n, void* stream);
 

@@ -546,24 +546,29 @@ int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const 
 
 // Shared backward driver: D/lse2 preprocess, one kernel pass per KV chunk of the nk keys, optional bf16 cast of dQ.
 // q,o,dO,lse: Nq rows per head; k,v,dk,dv: Nk rows per head.  dq_acc fp32 [BH,Nq,d] (zeroed first when zero_dq).
+// `prepared`: D and lse2 already hold this (o, lse, dO)'s values (an earlier step of the same RingX backward wrote them).
+// dkv_dtype: dtype of dk, dv (bf16, or fp32 for one device's share of a cross-device sum).
 static int bwd_core(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
                     float* D, float* lse2, float* dq_acc, bool zero_dq, void* dq_bf16, void* dk, void* dv, int BH,
-                    int Nq, int Nk, int d, int kv_chunk, float scale, int* dq_sem, cudaStream_t stream) {
+                    int Nq, int Nk, int d, int kv_chunk, float scale, int* dq_sem, cudaStream_t stream,
+                    int dkv_dtype = RINGX_BF16, bool prepared = false) {
   const long long R = (long long)BH * Nq;
   cudaError_t e;
   if (!g_deterministic.load(std::memory_order_relaxed)) dq_sem = nullptr;
   if (dq_sem && (e = cudaMemsetAsync(dq_sem, 0, (size_t)(R / 128) * sizeof(int), stream)) != cudaSuccess)
     return cuda_status(e);
-  {
-    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-    e = launch_bwd_preprocess(o, dO, lse, D, lse2, dq_acc, R, d, scale, zero_dq, stream);
+  if (!prepared) {
+    {
+      Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+      e = launch_bwd_preprocess(o, dO, lse, D, lse2, dq_acc, R, d, scale, zero_dq, stream);
+    }
+    count_launch();
+    if (e != cudaSuccess) return cuda_status(e);
   }
-  count_launch();
-  if (e != cudaSuccess) return cuda_status(e);
   for (int c = 0; c < Nk / kv_chunk; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
     e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, dq_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, kv_chunk, d, scale,
-                                    dq_sem, stream);
+                                    dq_sem, dkv_dtype, stream);
     if (e != cudaSuccess) return cuda_status(e);
     if (tl_hooks.pass_done && (e = cudaEventRecord(tl_hooks.pass_done[c], stream)) != cudaSuccess) return cuda_status(e);
   }
@@ -618,12 +623,14 @@ size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d) {
   return 2 * align_up(R * sizeof(float)) + align_up(R / 128 * sizeof(int));
 }
 
-int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const void* o, const float* lse,
-                           const void* dO, float* dq_acc, void* dk, void* dv, int B, int H, int Nq, int Nk, int d,
-                           float scale, int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
+int ringx_attn_bwd_partial_ex(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                              const void* dO, float* dq_acc, void* dk, void* dv, int B, int H, int Nq, int Nk, int d,
+                              float scale, int dtype, int dkv_dtype, int prepared, void* workspace,
+                              size_t workspace_bytes, void* stream_) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!q || !k || !v || !o || !lse || !dO || !dq_acc || !dk || !dv) return RINGX_ERR_NULL_PTR;
   if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (dkv_dtype != RINGX_BF16 && dkv_dtype != RINGX_F32) return RINGX_ERR_BAD_DTYPE;
   if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
   if (Nq % 128 || Nk % 128) return RINGX_ERR_BAD_SHAPE;
   if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
@@ -643,10 +650,18 @@ int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const vo
   const size_t rb = align_up((size_t)B * H * Nq * sizeof(float));
   float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + rb);
   int* dq_sem = reinterpret_cast<int*>(static_cast<char*>(workspace) + 2 * rb);
-  st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, dq_sem, stream);
+  st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, dq_sem, stream,
+                dkv_dtype, prepared != 0);
   if (st != RINGX_OK) return st;
   tl_last_launches = tl_launches;
   return RINGX_OK;
+}
+
+int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                           const void* dO, float* dq_acc, void* dk, void* dv, int B, int H, int Nq, int Nk, int d,
+                           float scale, int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
+  return ringx_attn_bwd_partial_ex(q, k, v, o, lse, dO, dq_acc, dk, dv, B, H, Nq, Nk, d, scale, dtype, RINGX_BF16, 0,
+                                   workspace, workspace_bytes, stream_);
 }
 
 int ringx_dq_finalize(const float* dq_acc, void* dq, long long n, void* stream_) {

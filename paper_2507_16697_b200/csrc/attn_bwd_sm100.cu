@@ -74,7 +74,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
                       const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_do,
                       const __grid_constant__ CUtensorMap map_dq, const float* __restrict__ lse2,
                       const float* __restrict__ Dvec,
-                      __nv_bfloat16* __restrict__ dk, __nv_bfloat16* __restrict__ dv, int N, int nk_stride, int k_off,
+                      void* __restrict__ dk, void* __restrict__ dv, int dkv_f32, int N, int nk_stride, int k_off,
                       float scale_log2, float scale, int* __restrict__ dq_sem, unsigned* __restrict__ smem_probe) {
   using Cfg = BwdCfg<kD>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -434,21 +434,31 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     mbar_wait(dkv_full, 0);
     tc_fence_after();
     const uint32_t tSrc = tmem + (half == 0 ? Cfg::tDV : Cfg::tDK) + lane_off;
-    __nv_bfloat16* dst_base = (half == 0 ? dv : dk) + (static_cast<size_t>(k_row0) + row) * kD;
+    const size_t out_off = (static_cast<size_t>(k_row0) + row) * kD;
+    // bf16 (the single-device result), or fp32 (one device's share of a cross-device sum: RingX_a/b reduce the shares
+    // in fp32 and round once, instead of rounding every share to bf16 first)
 #pragma unroll
     for (int c = 0; c < kD / 32; ++c) {
       uint32_t r[32];
       tmem_ld_x32(tSrc + c * 32, r);
       tmem_wait_ld();
-      uint4* dst = reinterpret_cast<uint4*>(dst_base + c * 32);
+      if (dkv_f32) {
+        float4* dst = reinterpret_cast<float4*>(static_cast<float*>(half == 0 ? dv : dk) + out_off + c * 32);
 #pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        uint4 u;
-        u.x = pack_bf16x2(__uint_as_float(r[g * 8 + 0]), __uint_as_float(r[g * 8 + 1]));
-        u.y = pack_bf16x2(__uint_as_float(r[g * 8 + 2]), __uint_as_float(r[g * 8 + 3]));
-        u.z = pack_bf16x2(__uint_as_float(r[g * 8 + 4]), __uint_as_float(r[g * 8 + 5]));
-        u.w = pack_bf16x2(__uint_as_float(r[g * 8 + 6]), __uint_as_float(r[g * 8 + 7]));
-        dst[g] = u;
+        for (int g = 0; g < 8; ++g)
+          dst[g] = make_float4(__uint_as_float(r[g * 4]), __uint_as_float(r[g * 4 + 1]), __uint_as_float(r[g * 4 + 2]),
+                               __uint_as_float(r[g * 4 + 3]));
+      } else {
+        uint4* dst = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(half == 0 ? dv : dk) + out_off + c * 32);
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          uint4 u;
+          u.x = pack_bf16x2(__uint_as_float(r[g * 8 + 0]), __uint_as_float(r[g * 8 + 1]));
+          u.y = pack_bf16x2(__uint_as_float(r[g * 8 + 2]), __uint_as_float(r[g * 8 + 3]));
+          u.z = pack_bf16x2(__uint_as_float(r[g * 8 + 4]), __uint_as_float(r[g * 8 + 5]));
+          u.w = pack_bf16x2(__uint_as_float(r[g * 8 + 6]), __uint_as_float(r[g * 8 + 7]));
+          dst[g] = u;
+        }
       }
     }
   } else if (warp < 12) {
@@ -531,8 +541,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 
 template <int kD>
 cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
-                     const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int BH, int N,
-                     int nk_stride, int k_off, int nk, float scale, int* dq_sem, cudaStream_t stream) {
+                     const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int dkv_f32, int BH,
+                     int N, int nk_stride, int k_off, int nk, float scale, int* dq_sem, cudaStream_t stream) {
   using Cfg = BwdCfg<kD>;
   auto kern = attn_chunk_bwd_kernel<kD>;
   static unsigned char configured[kMaxDevices];
@@ -548,8 +558,8 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
       unsigned h = 0xffffffffu;
       cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&flag), g_bwd_smem_probe);
       if (e != cudaSuccess) return e;
-      kern<<<1, 32, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0.f, 0.f,
-                                               nullptr, flag);
+      kern<<<1, 32, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0, 0.f,
+                                               0.f, nullptr, flag);
       if ((e = cudaGetLastError()) != cudaSuccess) return e;
       if ((e = cudaMemcpyAsync(&h, flag, sizeof(h), cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return e;
       if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return e;
@@ -560,10 +570,8 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
     }
   }
   dim3 grid(nk / kTile, BH);
-  kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D,
-                                                       static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv),
-                                                       N, nk_stride, k_off, scale * 1.4426950408889634f, scale,
-                                                       dq_sem, nullptr);
+  kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, N, nk_stride, k_off,
+                                                       scale * 1.4426950408889634f, scale, dq_sem, nullptr);
   count_launch();
   return cudaGetLastError();
 }
@@ -573,8 +581,9 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
                                         int nk_stride, int k_off, int nk, int d, float scale, int* dq_sem,
-                                        cudaStream_t stream) {
+                                        int dkv_dtype, cudaStream_t stream) {
   CUtensorMap mq, mk, mv, mdo, mdq;
+  const int dkv_f32 = dkv_dtype == RINGX_F32;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   const uint64_t rows = (uint64_t)BH * N, krows = (uint64_t)BH * nk_stride;
   if (!make_tmap_2d(&mq, q, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
@@ -583,8 +592,8 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
       !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mdq, dq_acc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, rows, d, 128, 32, kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
-  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
+  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
+  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
 }
 
 }  // namespace ringx

@@ -75,10 +75,11 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
 // lse2 = LSE * log2(e) and D = scale * rowsum(dO*O) come from launch_bwd_preprocess.
 // dq_sem: nullptr, or [BH * N/128] ticket counters (zero before the first pass of a call) that make the order of the
 // reduce-adds into every dQ tile the key-tile order (bit-reproducible dQ).
+// dkv_dtype: RINGX_BF16 (dk, dv bf16) or RINGX_F32 (fp32: one device's share of a cross-device sum).
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
                                         int nk_stride, int k_off, int nk, int d, float scale, int* dq_sem,
-                                        cudaStream_t stream);
+                                        int dkv_dtype, cudaStream_t stream);
 
 // ---- tensor maps (api.cu): 2-D row-major [rows, cols] view, box = {box_cols, box_rows}
 enum TmapSwizzle { kSwizzleNone = 0, kSwizzle128B = 1 };

@@ -60,6 +60,8 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_bwd_gqa.restype = c_i
     L.ringx_attn_bwd_partial.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_bwd_partial.restype = c_i
+    L.ringx_attn_bwd_partial_ex.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_i, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_bwd_partial_ex.restype = c_i
     L.ringx_attn_bwd_partial_workspace_bytes.argtypes = [c_i] * 4
     L.ringx_attn_bwd_partial_workspace_bytes.restype = c_sz
     L.ringx_dq_finalize.argtypes = [c_p, c_p, c_ll, c_p]
@@ -449,6 +451,22 @@ def ringx_attn_bwd_partial(q, k, v, o, lse, dO, scale: float, dq_acc=None, dk=No
                                       B, H, Nq, Nk, d, scale, _DTYPES[q.dtype], workspace.data_ptr(),
                                       workspace.numel() * workspace.element_size(), _stream())
     _check(st, "ringx_attn_bwd_partial")
+    return dq_acc, dk, dv
+
+
+def ringx_attn_bwd_partial_ex(q, k, v, o, lse, dO, scale: float, dq_acc, dk, dv, workspace, prepared: bool = False):
+    """The per-device backward step in its general form (include/ringx.h: ringx_attn_bwd_partial_ex): dk, dv may be
+    float32 (this device's unrounded share of a cross-device sum); `prepared` reuses the D / lse2 that an earlier step of the
+    same backward left in `workspace`.  Every buffer is the caller's; returns (dq_acc, dk, dv)."""
+    B, H, Nq, d = q.shape
+    Nk = k.shape[2]
+    if dk.dtype != dv.dtype:
+        raise ValueError("dk and dv must have the same dtype")
+    st = lib().ringx_attn_bwd_partial_ex(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                                         _dev(dO, "dO"), _dev(dq_acc, "dq_acc"), _dev(dk, "dk"), _dev(dv, "dv"),
+                                         B, H, Nq, Nk, d, scale, _DTYPES[q.dtype], _DTYPES[dk.dtype], 1 if prepared else 0,
+                                         workspace.data_ptr(), workspace.numel() * workspace.element_size(), _stream())
+    _check(st, "ringx_attn_bwd_partial_ex")
     return dq_acc, dk, dv
 
 

@@ -17,6 +17,12 @@ before the kernels of step t are enqueued, into the other of two ping-pong buffe
 already owns while the all-gather is in flight.  On NVSwitch every peer is one hop away at full bandwidth, so the
 all-gather form (RingX_b) is the natural default; RingX_a keeps per-rank memory at O(N/W).
 
+Gradient shares cross the collectives in fp32: a device's dK,dV of a step are only its SHARE of a sum over devices
+(PAPER.md:143, 145), so `ringx_attn_bwd_partial_ex` writes them unrounded, the reduce / reduce-scatter sums fp32, and
+the owner rounds once to bf16 -- the accuracy of the single-device path, independent of the world size (bf16 shares
+would be rounded W times and then added in bf16).  Scratch buffers are allocated once per schedule call, and
+D_i = dO_i.O_i is formed once per backward, not once per step.
+
 `ops` is the per-device kernel set; the default drives the CUDA library and has no CPU fallback.  `comm` is the
 set of collectives (default: torch.distributed, NCCL on GPUs).  The CPU/gloo tests substitute an fp64 `ops` to check
 the schedules themselves (which chunk meets which, what is reduced where) without a GPU; the one-GPU tests run the
@@ -38,13 +44,20 @@ class CudaOps:
     def attn_fwd(self, q, k, v, scale):                       # single device, single pass
         return self.rx.ringx_attn_fwd(q, k, v, q.shape[2], scale)
 
-    def chunk_fwd(self, q, k, v, scale):                      # (loc_out fp32, loc_lse)
+    def fwd_scratch(self, q, k):                              # split-KV workspace of one chunk pass (None: not needed)
+        if q.dtype != torch.bfloat16:
+            return None
+        B, H, Nq, d = q.shape
+        n = self.rx.ringx_attn_chunk_fwd_ex_workspace_bytes(B, H, Nq, k.shape[2], d, q.dtype)
+        return torch.empty(n, dtype=torch.uint8, device=q.device) if n else None
+
+    def chunk_fwd(self, q, k, v, scale, scratch=None):        # (loc_out fp32, loc_lse)
         if q.dtype == torch.bfloat16:                         # split-KV when the local chunk cannot fill the GPU
-            return self.rx.ringx_attn_chunk_fwd_ex(q, k, v, scale)
+            return self.rx.ringx_attn_chunk_fwd_ex(q, k, v, scale, workspace=scratch)
         return self.rx.ringx_attn_chunk_fwd(q, k, v, scale)
 
-    def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final):   # chunk pass + two-operand Eq. 5 in one kernel
-        return self.rx.ringx_attn_chunk_fwd_ex(q, k, v, scale, o_acc=o_acc, lse_acc=lse_acc, final=final)
+    def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final, scratch=None):   # chunk pass + two-operand Eq. 5
+        return self.rx.ringx_attn_chunk_fwd_ex(q, k, v, scale, o_acc=o_acc, lse_acc=lse_acc, final=final, workspace=scratch)
 
     def eq5_scale(self, loc_out, loc_lse, lse_max):           # num, den of one operand (in place on loc_out)
         return self.rx.ringx_eq5_scale(loc_out, loc_lse, lse_max, inplace=True)
@@ -52,13 +65,23 @@ class CudaOps:
     def eq5_finalize(self, num, den, lse_max, out_dtype):
         return self.rx.ringx_eq5_finalize(num, den, lse_max, out_dtype=out_dtype)
 
-    def bwd_partial(self, q, k, v, o, lse, dO, scale, dq_acc, dk, dv):
-        return self.rx.ringx_attn_bwd_partial(q, k, v, o, lse, dO, scale, dq_acc=dq_acc, dk=dk, dv=dv)
+    def bwd_scratch(self, q):                                 # D, lse2 (+ tickets) of one backward: allocated once
+        B, H, Nq, d = q.shape
+        n = max(256, self.rx.ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d))
+        return torch.empty(n, dtype=torch.uint8, device=q.device)
+
+    def bwd_partial(self, q, k, v, o, lse, dO, scale, dq_acc, dk, dv, scratch, prepared):
+        """dq_acc += these keys' contribution; (dk, dv) = this device's share for these keys, in dk's dtype.  `prepared`:
+        `scratch` holds D, lse2 of (o, lse, dO) from an earlier step of this backward."""
+        return self.rx.ringx_attn_bwd_partial_ex(q, k, v, o, lse, dO, scale, dq_acc, dk, dv, scratch, prepared=prepared)
 
     def dq_finalize(self, dq_acc, like):
         return self.rx.ringx_dq_finalize(dq_acc)
 
-    def acc_dtype(self, q):                                   # dtype of partials / accumulators
+    def round_share(self, acc, like):                         # the one rounding of a reduced fp32 gradient (same kernel)
+        return self.rx.ringx_dq_finalize(acc)
+
+    def acc_dtype(self, q):                                   # dtype of partials, accumulators and gradient shares
         return torch.float32
 
 
@@ -118,16 +141,17 @@ def ringx_b_forward(q, k, v, scale, comm=None, ops=None):
     kg = torch.empty((W,) + tuple(k.shape), dtype=k.dtype, device=k.device)
     vg = torch.empty((W,) + tuple(v.shape), dtype=v.dtype, device=v.device)
     works = [comm.all_gather(kg, k), comm.all_gather(vg, v)]
-    o_acc, lse_acc = ops.chunk_fwd(q, k, v, scale)            # the chunk already here overlaps the gather
+    scratch = ops.fwd_scratch(q, k)                           # one allocation for all W chunk passes
+    o_acc, lse_acc = ops.chunk_fwd(q, k, v, scale, scratch)   # the chunk already here overlaps the gather
     for w in works:
         w.wait()
     o = lse = None
     for s in range(1, W):
         c = (r + s) % W                                       # ring order: every rank starts on a different chunk
         if s == W - 1:
-            o, lse = ops.chunk_fwd_fold(q, kg[c], vg[c], o_acc, lse_acc, scale, True)     # last fold writes bf16
+            o, lse = ops.chunk_fwd_fold(q, kg[c], vg[c], o_acc, lse_acc, scale, True, scratch)     # last fold writes bf16
         else:
-            o_acc, lse_acc = ops.chunk_fwd_fold(q, kg[c], vg[c], o_acc, lse_acc, scale, False)
+            o_acc, lse_acc = ops.chunk_fwd_fold(q, kg[c], vg[c], o_acc, lse_acc, scale, False, scratch)
     return o, lse, (q, kg, vg, o, lse, scale)
 
 
@@ -139,18 +163,23 @@ def ringx_b_backward(ctx, dO, comm=None, ops=None):
     comm = comm or TorchComm()
     W, r = comm.world, comm.rank
     dq_acc = torch.zeros(q.shape, dtype=ops.acc_dtype(q), device=q.device)
-    dkg, dvg = torch.empty_like(kg), torch.empty_like(vg)
+    scratch = ops.bwd_scratch(q)
+    if W == 1:
+        dk, dv = torch.empty_like(kg[0]), torch.empty_like(vg[0])
+        ops.bwd_partial(q, kg[0], vg[0], o, lse, dO, scale, dq_acc, dk, dv, scratch, False)
+        return ops.dq_finalize(dq_acc, q), dk, dv
+    share = ops.acc_dtype(q)                                  # the shares cross the reduce-scatter unrounded
+    dkg = torch.empty(kg.shape, dtype=share, device=kg.device)
+    dvg = torch.empty(vg.shape, dtype=share, device=vg.device)
     for s in range(W):
         c = (r + s) % W
-        ops.bwd_partial(q, kg[c], vg[c], o, lse, dO, scale, dq_acc, dkg[c], dvg[c])
+        ops.bwd_partial(q, kg[c], vg[c], o, lse, dO, scale, dq_acc, dkg[c], dvg[c], scratch, s > 0)
     dq = ops.dq_finalize(dq_acc, q)
-    if W == 1:
-        return dq, dkg[0], dvg[0]
-    dk, dv = torch.empty_like(kg[0]), torch.empty_like(vg[0])
+    dk, dv = torch.empty_like(dkg[0]), torch.empty_like(dvg[0])
     works = [comm.reduce_scatter_sum(dk, dkg), comm.reduce_scatter_sum(dv, dvg)]
     for w in works:
         w.wait()
-    return dq, dk, dv
+    return dq, ops.round_share(dk, kg[0]), ops.round_share(dv, vg[0])
 
 
 # ---------------------------------------------------------------------------------------------- RingX_a
@@ -171,13 +200,14 @@ def ringx_a_forward(q, k, v, scale, comm=None, ops=None):
         return buf, comm.broadcast(buf, t)
 
     nxt = start_bcast(0)
+    scratch = ops.fwd_scratch(q, k)                           # one allocation for all W steps
     o = lse = None
     for t in range(W):
         q_t, work = nxt
         if t + 1 < W:
             nxt = start_bcast(t + 1)
         work.wait()
-        loc_out, loc_lse = ops.chunk_fwd(q_t, k, v, scale)
+        loc_out, loc_lse = ops.chunk_fwd(q_t, k, v, scale, scratch)
         lse_max = loc_lse.clone()
         comm.all_reduce_max(lse_max).wait()
         num, den = ops.eq5_scale(loc_out, loc_lse, lse_max)
@@ -197,10 +227,14 @@ def ringx_a_backward(ctx, dO, comm=None, ops=None):
     comm = comm or TorchComm()
     W, r = comm.world, comm.rank
     dq_acc = torch.zeros(q.shape, dtype=ops.acc_dtype(q), device=q.device)
+    scratch = ops.bwd_scratch(q)
     if W == 1:
         dk, dv = torch.empty_like(k), torch.empty_like(v)
-        ops.bwd_partial(q, k, v, o, lse, dO, scale, dq_acc, dk, dv)
+        ops.bwd_partial(q, k, v, o, lse, dO, scale, dq_acc, dk, dv, scratch, False)
         return ops.dq_finalize(dq_acc, q), dk, dv
+    share = ops.acc_dtype(q)
+    dkb = [torch.empty(k.shape, dtype=share, device=k.device) for _ in range(2)]     # ping-pong: step t's reduce may still
+    dvb = [torch.empty(v.shape, dtype=share, device=v.device) for _ in range(2)]     # read one pair while t+1 writes the other
     kb = [torch.empty_like(k), torch.empty_like(k)]
     vb = [torch.empty_like(v), torch.empty_like(v)]
 
@@ -216,11 +250,11 @@ def ringx_a_backward(ctx, dO, comm=None, ops=None):
             nxt = start_bcast(t + 1)
         for w in works:
             w.wait()
-        dk_t, dv_t = torch.empty_like(k_t), torch.empty_like(v_t)
-        ops.bwd_partial(q, k_t, v_t, o, lse, dO, scale, dq_acc, dk_t, dv_t)
+        dk_t, dv_t = dkb[t & 1], dvb[t & 1]
+        ops.bwd_partial(q, k_t, v_t, o, lse, dO, scale, dq_acc, dk_t, dv_t, scratch, t > 0)
         works = [comm.reduce_sum(dk_t, t), comm.reduce_sum(dv_t, t)]
         for w in works:
             w.wait()
-        if t == r:
-            dk, dv = dk_t, dv_t
+        if t == r:                                            # the fp32 sums over all ranks: round once
+            dk, dv = ops.round_share(dk_t, k), ops.round_share(dv_t, v)
     return ops.dq_finalize(dq_acc, q), dk, dv

@@ -199,8 +199,8 @@ def test_eq5_scale_and_finalize_match_oracle(rx, rows, d, n_ops):
 # ------------------------------------------------------------------------------------------------ schedules, W ranks
 class ThreadComm:
     """In-process stand-in for ringx_dist.TorchComm: W threads = W simulated ranks sharing one GPU and one stream.
-    Every collective is "publish, barrier, combine, barrier"; combining uses plain torch copies/sums (the collectives
-    are not part of the method's arithmetic; NCCL does the same sums in the same dtypes)."""
+    Every collective is "publish, barrier, combine, barrier"; combining uses plain torch copies and sums IN THE
+    TENSOR'S OWN DTYPE, as NCCL does (the schedules hand it fp32 gradient shares, so that is an fp32 sum)."""
 
     class _Shared:
         def __init__(self, world):
@@ -238,7 +238,7 @@ class ThreadComm:
     def reduce_sum(self, t, dst):
         got = self._exchange(t.clone())
         if self.rank == dst:
-            t.copy_(torch.stack(got).float().sum(dim=0))
+            t.copy_(torch.stack(got).sum(dim=0))
         return self._finish()
 
     def all_gather(self, stacked, t):
@@ -249,7 +249,7 @@ class ThreadComm:
 
     def reduce_scatter_sum(self, out, stacked):
         got = self._exchange(stacked)
-        out.copy_(torch.stack([g[self.rank] for g in got]).float().sum(dim=0))
+        out.copy_(torch.stack([g[self.rank] for g in got]).sum(dim=0))
         return self._finish()
 
 
@@ -300,6 +300,155 @@ def test_ringx_schedules_on_simulated_ranks(rx, variant, world, d, Nl):
         for g, ref in ((dq, dq_ref), (dk, dk_ref), (dv, dv_ref)):
             e = relf(f64(g), ref[:, :, sl])
             assert e <= TOL_GRAD and e <= 8e-3, e
+
+
+def run_simulated(rx, variant, world, B, H, Nl, d, seed):
+    """Both directions of one schedule on `world` simulated ranks; returns the per-rank results and the whole-sequence inputs."""
+    from paper_2507_16697_b200 import ringx_dist
+    N = world * Nl
+    scale = 1.0 / math.sqrt(d)
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=seed, dtype="bf16")
+    fwd, bwd = ((ringx_dist.ringx_a_forward, ringx_dist.ringx_a_backward) if variant == "a" else
+                (ringx_dist.ringx_b_forward, ringx_dist.ringx_b_backward))
+    shared = ThreadComm._Shared(world)
+    results, errors = [None] * world, []
+
+    def rank_main(r):
+        try:
+            torch.cuda.set_device(0)
+            comm = ThreadComm(shared, r)
+            sl = slice(r * Nl, (r + 1) * Nl)
+            ql, kl, vl, dol = (t[:, :, sl].contiguous().cuda() for t in (q, k, v, do))
+            o, lse, ctx = fwd(ql, kl, vl, scale, comm=comm)
+            dq, dk, dv = bwd(ctx, dol, comm=comm)
+            torch.cuda.synchronize()
+            results[r] = [t.cpu() for t in (o, lse, dq, dk, dv)]
+        except Exception as e:                      # noqa: BLE001 -- surface it in the main thread
+            errors.append(e)
+            shared.barrier.abort()
+
+    threads = [threading.Thread(target=rank_main, args=(r,)) for r in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=600)
+    assert not errors, errors
+    return results, (q, k, v, do), scale
+
+
+def test_gradient_error_does_not_grow_with_the_world_size(rx):
+    """The gradient shares cross the collectives in fp32 and are rounded once (ringx_attn_bwd_partial_ex): the error of
+    dK, dV against the oracle at W = 2, 4, 8, 16 ranks (same whole sequence, N = 4096) stays at the single-device level
+    -- with bf16 shares it would grow with W (W roundings, then a bf16 sum)."""
+    import grad_bounds as gb
+    B, H, N, d = 1, 1, 4096, 64
+    errs = {}
+    for variant in ("b", "a"):
+        for world in (2, 4, 8, 16):
+            results, (q, k, v, do), scale = run_simulated(rx, variant, world, B, H, N // world, d, seed=31)
+            q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+            if "ref" not in errs:
+                errs["ref"] = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
+                qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+                o1, l1 = rx.ringx_attn_fwd(qd, kd, vd, N, scale)
+                errs["single"] = [relf(f64(g), r) for g, r in zip(rx.ringx_attn_bwd(qd, kd, vd, o1, l1, dod, N, scale), errs["ref"])]
+            got = [torch.cat([results[r][i] for r in range(world)], dim=2) for i in (2, 3, 4)]     # dq, dk, dv, whole sequence
+            e = [relf(f64(g), r) for g, r in zip(got, errs["ref"])]
+            errs[(variant, world)] = e
+            for name, g, r in zip(("dq", "dk", "dv"), got, errs["ref"]):
+                assert g.dtype == torch.bfloat16
+                gb.check_grad(f"{name} RingX_{variant} W={world}", f64(g)[0, 0], r[0, 0])
+    print("relative Frobenius error of (dq, dk, dv) vs W:", {k_: [f"{x:.2e}" for x in v_] for k_, v_ in errs.items() if k_ != "ref"})
+    for key, e in errs.items():
+        if key in ("ref", "single"):
+            continue
+        for x, x1 in zip(e, errs["single"]):
+            assert x <= 1.5 * x1 + 5e-4, (key, e, errs["single"])       # no growth with W
+
+
+def test_bwd_partial_ex_fp32_shares_and_prepared_workspace(rx):
+    """ringx_attn_bwd_partial_ex: fp32 dk, dv are the accumulators the bf16 form rounds (so rounding them gives the bf16
+    result bit for bit), and `prepared` reuses D / lse2 left in the workspace by the first step of the backward."""
+    B, H, Nq, Nk, d = 1, 2, 512, 384, 128
+    scale = 1.0 / math.sqrt(d)
+    q = wl.make_tensor((B, H, Nq, d), "q", seed=61, dtype="bf16").cuda()
+    do = wl.make_tensor((B, H, Nq, d), "do", seed=61, dtype="bf16").cuda()
+    k = wl.make_tensor((B, H, 2 * Nk, d), "k", seed=61, dtype="bf16").cuda()
+    v = wl.make_tensor((B, H, 2 * Nk, d), "v", seed=61, dtype="bf16").cuda()
+    o, lse = rx.ringx_attn_fwd(q[:, :, :512].contiguous(), k[:, :, :512].contiguous(), v[:, :, :512].contiguous(), 512, scale)
+    ws = torch.empty(rx.ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d), dtype=torch.uint8, device="cuda")
+    ka, va = k[:, :, :Nk].contiguous(), v[:, :, :Nk].contiguous()
+    kb, vb = k[:, :, Nk:].contiguous(), v[:, :, Nk:].contiguous()
+    acc = torch.zeros(B, H, Nq, d, device="cuda")
+    dk16, dv16 = torch.empty_like(ka), torch.empty_like(va)
+    rx.ringx_attn_bwd_partial_ex(q, ka, va, o, lse, do, scale, acc, dk16, dv16, ws)
+    assert rx.ringx_last_launch_count() == 2                     # preprocess + one backward pass
+    acc2 = torch.zeros_like(acc)
+    dk32 = torch.empty(ka.shape, device="cuda")
+    dv32 = torch.empty(va.shape, device="cuda")
+    rx.ringx_attn_bwd_partial_ex(q, ka, va, o, lse, do, scale, acc2, dk32, dv32, ws, prepared=True)
+    assert rx.ringx_last_launch_count() == 1                     # the pass alone: D, lse2 reused
+    assert torch.equal(dk32.to(torch.bfloat16), dk16) and torch.equal(dv32.to(torch.bfloat16), dv16)
+    assert torch.equal(rx.ringx_dq_finalize(dk32), dk16)         # the library's own rounding kernel: the same bits
+    # a second step on other keys with the prepared workspace, against the un-prepared call
+    rx.ringx_attn_bwd_partial_ex(q, kb, vb, o, lse, do, scale, acc2, dk32, dv32, ws, prepared=True)
+    ref = torch.zeros_like(acc)
+    dkr, dvr = torch.empty_like(dk32), torch.empty_like(dv32)
+    rx.ringx_attn_bwd_partial_ex(q, kb, vb, o, lse, do, scale, ref, dkr, dvr, ws, prepared=False)
+    assert torch.equal(dkr, dk32) and torch.equal(dvr, dv32)
+    L = rx.lib()
+    p = [x.data_ptr() for x in (q, kb, vb, o, lse, do, ref, dkr, dvr)]
+    assert L.ringx_attn_bwd_partial_ex(*p, B, H, Nq, Nk, d, scale, 1, 2, 0, ws.data_ptr(), ws.numel(), None) == 3   # dkv dtype
+    torch.cuda.synchronize()
+
+
+_NCCL_W2 = r"""
+import math, os, sys, torch, torch.distributed as dist
+sys.path.insert(0, {root!r})
+from paper_2507_16697_b200 import ringx, ringx_dist, workloads as wl
+rank = int(os.environ["RANK"]); world = int(os.environ["WORLD_SIZE"])
+torch.cuda.set_device(rank)
+dist.init_process_group("nccl", device_id=torch.device("cuda", rank))
+B, H, Nl, d = 1, 2, 512, 128
+N = world * Nl
+scale = 1.0 / math.sqrt(d)
+q, k, v, do = (t.cuda() for t in wl.make_qkv((B, H, N, d), with_do=True, seed=47, dtype="bf16"))
+o1, l1 = ringx.ringx_attn_fwd(q, k, v, N, scale)
+g1 = ringx.ringx_attn_bwd(q, k, v, o1, l1, do, N, scale)
+sl = slice(rank * Nl, (rank + 1) * Nl)
+ql, kl, vl, dol = (t[:, :, sl].contiguous() for t in (q, k, v, do))
+for fwd, bwd in ((ringx_dist.ringx_b_forward, ringx_dist.ringx_b_backward), (ringx_dist.ringx_a_forward, ringx_dist.ringx_a_backward)):
+    o, lse, ctx = fwd(ql, kl, vl, scale)
+    dq, dk, dv = bwd(ctx, dol)
+    torch.cuda.synchronize()
+    rel = lambda a, b: ((a.float() - b.float()).norm() / b.float().norm()).item()
+    assert rel(o, o1[:, :, sl]) <= 5e-3 and (lse - l1[:, :, sl]).abs().max().item() <= 5e-5
+    for g, r in zip((dq, dk, dv), g1):
+        assert rel(g, r[:, :, sl]) <= 5e-3, rel(g, r[:, :, sl])
+dist.barrier()
+dist.destroy_process_group()
+if rank == 0:
+    print("NCCL_W2_OK")
+"""
+
+
+def test_ringx_schedules_over_nccl_two_gpus(rx, tmp_path):
+    """RingX_a and RingX_b across two real devices over NCCL (one process per GPU), against the single-device library
+    result of the whole sequence.  Skipped on a box with one GPU (every box of this project so far: no multi-GPU run of
+    the schedules exists, and none is claimed)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "nccl_w2.py"
+    script.write_text(_NCCL_W2.format(root=root))
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr",
+                        "127.0.0.1", "--master-port", str(port), str(script)], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "NCCL_W2_OK" in r.stdout, (r.stdout[-2000:], r.stderr[-2000:])
 
 
 def test_ringx_dist_over_nccl_world_size_one(rx):

@@ -38,7 +38,16 @@ class OracleOps:
     def attn_fwd(self, q, k, v, scale):
         return self.chunk_fwd(q, k, v, scale)
 
-    def chunk_fwd(self, q, k, v, scale):
+    def fwd_scratch(self, q, k):
+        return None
+
+    def bwd_scratch(self, q):
+        return {"prepared_for": None}          # stands in for the D / lse2 workspace: records what it was prepared for
+
+    def round_share(self, acc, like):
+        return acc.clone()
+
+    def chunk_fwd(self, q, k, v, scale, scratch=None):
         o = torch.empty(q.shape[:3] + (v.shape[3],), dtype=torch.float64)
         lse = torch.empty(q.shape[:3], dtype=torch.float64)
         for (b, h), (qq, kk, vv) in self._heads(q, k, v):
@@ -46,7 +55,7 @@ class OracleOps:
             o[b, h], lse[b, h] = torch.from_numpy(a), torch.from_numpy(l)
         return o, lse
 
-    def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final):
+    def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final, scratch=None):
         o_p, lse_p = self.chunk_fwd(q, k, v, scale)
         return self.lse_merge(o_acc, lse_acc, o_p, lse_p, o_acc.dtype, not final)
 
@@ -68,7 +77,12 @@ class OracleOps:
     def eq5_finalize(self, num, den, lse_max, out_dtype):
         return num / den.unsqueeze(-1), lse_max + torch.log(den)
 
-    def bwd_partial(self, q, k, v, o, lse, dO, scale, dq_acc, dk, dv):
+    def bwd_partial(self, q, k, v, o, lse, dO, scale, dq_acc, dk, dv, scratch, prepared):
+        # the schedule must prepare (D, lse2) exactly once per backward, on its first step, and say so afterwards
+        key = (o.data_ptr(), dO.data_ptr())
+        assert prepared == (scratch["prepared_for"] == key), "D/lse2 preprocess: once per backward, first step only"
+        scratch["prepared_for"] = key
+        assert dk.dtype == self.acc_dtype(q) and dv.dtype == self.acc_dtype(q) or not prepared and dk.dtype == k.dtype
         for (b, h), (qq, kk, vv, oo, ll, dd) in self._heads(q, k, v, o, lse, dO):
             D = (dd * oo).sum(axis=1)
             a, bk, bv = orc.attention_bwd_partial(qq, kk, vv, dd, ll, D, scale)
