@@ -108,6 +108,19 @@ RINGX_API int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, co
                        int B, int Hq, int Hkv, int N, int d, int kv_chunk, float scale, int dtype,
                        void* workspace, size_t workspace_bytes, void* stream);
 
+/* Multi-head latent attention shapes (l.376 names MHA / GQA / MLA as the layer designs RingX is compatible with).  In its
+ * materialised form an MLA layer attends with a score contraction wider than the values: d_qk = 192 (128 + 64 rotary
+ * dimensions) and d_v = 128.  The path is the one of ringx_attn_fwd -- Eq. 1 per KV chunk, partials folded left to right by
+ * the two-operand Eq. 5 in the chunk kernel's epilogue -- on a kernel laid out for these widths.  Forward only (the backward
+ * of these shapes is not built: its accumulators, 128 + 192 columns beside S^T and dP^T, exceed the 512 TMEM columns).
+ *   q, k [B,H,N,d_qk] bf16 (in); v [B,H,N,d_v] bf16 (in); o [B,H,N,d_v] bf16 (out); lse [B,H,N] float (out).
+ *   Domain: d_qk == 192, d_v == 128, dtype RINGX_BF16, N % 256 == 0, kv_chunk % 128 == 0, N % kv_chunk == 0.
+ *   workspace  >= ringx_attn_fwd_mla_workspace_bytes(...) bytes (0 when kv_chunk == N), 256-byte aligned. */
+RINGX_API int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, float* lse,
+                       int B, int H, int N, int d_qk, int d_v, int kv_chunk, float scale, int dtype,
+                       void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_fwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk);
+
 /* Two-operand Eq. 5, row by row:  m = max(lse_a,lse_b); w_a = exp(lse_a-m); w_b = exp(lse_b-m);
  * o_out = (w_a o_a + w_b o_b)/(w_a+w_b);  lse_out = m + log(w_a+w_b).
  * An operand with lse = -inf has weight 0; both -inf gives o_out = 0, lse_out = -inf; NaN propagates.

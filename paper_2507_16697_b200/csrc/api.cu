@@ -429,6 +429,53 @@ int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* 
   return ringx_attn_fwd_gqa(q, k, v, o, lse, B, H, H, N, d, kv_chunk, scale, dtype, workspace, workspace_bytes, stream_);
 }
 
+// ---- multi-head latent attention shapes (d_qk = 192, d_v = 128): the same chunk loop on the MLA kernel
+size_t ringx_attn_fwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk) {
+  if (d_qk != 192 || d_v != 128 || check_shape(B, H, N, d_v, kv_chunk, 1.f, RINGX_BF16, false) != RINGX_OK) return 0;
+  if (kv_chunk == N) return 0;
+  const size_t R = (size_t)B * H * N;
+  return align_up(R * d_v * sizeof(float)) + align_up(R * sizeof(float));
+}
+
+int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, float* lse, int B, int H, int N, int d_qk,
+                       int d_v, int kv_chunk, float scale, int dtype, void* workspace, size_t workspace_bytes,
+                       void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o || !lse) return RINGX_ERR_NULL_PTR;
+  if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (d_qk != 192 || d_v != 128) return RINGX_ERR_BAD_SHAPE;
+  int st = check_shape(B, H, N, d_v, kv_chunk, scale, dtype, false);
+  if (st != RINGX_OK) return st;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse)) return RINGX_ERR_MISALIGNED;
+  const size_t need = ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk);
+  if (need) {
+    if (!workspace) return RINGX_ERR_NULL_PTR;
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+    if (workspace_bytes < need) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  }
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  const int BH = B * H, n_chunks = N / kv_chunk;
+  const size_t R = (size_t)BH * N;
+  float* o_acc = static_cast<float*>(workspace);
+  float* lse_acc = need ? reinterpret_cast<float*>(static_cast<char*>(workspace) + align_up(R * d_v * sizeof(float))) : nullptr;
+  for (int c = 0; c < n_chunks; ++c) {
+    const bool first = c == 0, last = c == n_chunks - 1;
+    const int epi = n_chunks == 1 ? kFwdEpiFinal : first ? kFwdEpiPartial : last ? kFwdEpiFoldFinal : kFwdEpiFold;
+    void* o_dst = (epi == kFwdEpiFinal || epi == kFwdEpiFoldFinal) ? o : static_cast<void*>(o_acc);
+    float* l_dst = (epi == kFwdEpiFinal || epi == kFwdEpiFoldFinal) ? lse : lse_acc;
+    cudaError_t e;
+    {
+      Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
+      e = launch_attn_chunk_fwd_mla_sm100(q, k, v, o_dst, l_dst, o_acc, lse_acc, BH, N, N, c * kv_chunk, kv_chunk, scale, epi,
+                                          stream);
+    }
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
 int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse, int B, int H,
                          int Nq, int Nk, int d, float scale, int dtype, void* stream_) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);

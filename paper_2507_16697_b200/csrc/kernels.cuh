@@ -68,6 +68,13 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
                                         int k_off, int nk, int d, float scale, int epilogue, int splits,
                                         cudaStream_t stream);
 
+// ---- attn_fwd_mla_sm100.cu (tcgen05 path, d_qk = 192, d_v = 128: multi-head latent attention in its materialised form)
+// One KV-chunk pass: q [BH,Nq,192], k [BH,nk_stride,192], v [BH,nk_stride,128]; epilogues as launch_attn_chunk_fwd_sm100
+// (o_out / o_acc are [BH,Nq,128]).
+cudaError_t launch_attn_chunk_fwd_mla_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
+                                            const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride,
+                                            int k_off, int nk, float scale, int epilogue, cudaStream_t stream);
+
 // ---- attn_bwd_sm100.cu (tcgen05 path)
 // One KV-chunk pass of the backward: q,dO [BH,N,d], k,v,dk,dv [BH,nk_stride,d]; writes dk,dv rows
 // [k_off, k_off+nk) of every head (bf16, the sum over the N query rows given), reduce-adds these keys'

@@ -42,6 +42,10 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_fwd_host.restype = c_i
     L.ringx_attn_bwd.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_bwd.restype = c_i
+    L.ringx_attn_fwd_mla.argtypes = [c_p] * 5 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_fwd_mla.restype = c_i
+    L.ringx_attn_fwd_mla_workspace_bytes.argtypes = [c_i] * 6
+    L.ringx_attn_fwd_mla_workspace_bytes.restype = c_sz
     L.ringx_lse_merge.argtypes = [c_p] * 6 + [c_ll, c_i, c_i, c_i, c_p]
     L.ringx_lse_merge.restype = c_i
     L.ringx_attn_chunk_fwd.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p]
@@ -159,6 +163,29 @@ def ringx_attn_fwd(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, works
     st = lib().ringx_attn_fwd(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
                               B, H, N, d, kv_chunk, scale, dt, ws_ptr, ws_len, _stream())
     _check(st, "ringx_attn_fwd")
+    return o, lse
+
+
+def ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk) -> int:
+    return lib().ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
+
+
+def ringx_attn_fwd_mla(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, workspace=None):
+    """O, LSE for multi-head latent attention shapes: q, k [B,H,N,192], v [B,H,N,128] bf16 (include/ringx.h:
+    ringx_attn_fwd_mla)."""
+    B, H, N, d_qk = q.shape
+    d_v = v.shape[3]
+    if o is None:
+        o = torch.empty((B, H, N, d_v), dtype=q.dtype, device=q.device)
+    if lse is None:
+        lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    need = lib().ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
+    if workspace is None:
+        workspace = _workspace(need, q.device)
+    st = lib().ringx_attn_fwd_mla(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"), B, H, N, d_qk, d_v,
+                                  kv_chunk, scale, _DTYPES[q.dtype], workspace.data_ptr() if workspace is not None else None,
+                                  workspace.numel() if workspace is not None else 0, _stream())
+    _check(st, "ringx_attn_fwd_mla")
     return o, lse
 
 
