@@ -571,7 +571,7 @@ def side_measure(ringx, wl, cfg, dev, oracle_seconds=0.0):
 
 
 def c1_measure(ringx, wl, dev):
-    """BASELINE.json configs[0] (fp32, N = 1024, 4 chunks): the FFMA path's time and the oracle's, both on the whole config."""
+    """BASELINE.json configs[0] (fp32, N = 1024, 4 chunks): the fp32 (3-term bf16 split, tensor-core) path's time and the oracle's, both on the whole config."""
     from oracle import attention as orc
     cfg = wl.CONFIGS["C1"]
     q, k, v = wl.make_qkv(cfg, device=dev)

@@ -74,7 +74,9 @@ typedef enum { RINGX_F32 = 0, RINGX_BF16 = 1 } ringx_dtype;
  * ringx_lse_merge's kernel).
  *   q,k,v  [B,H,N,d] of `dtype` (in).   o [B,H,N,d] of `dtype` (out).   lse [B,H,N] float (out).
  *   dtype  RINGX_BF16: tcgen05 tensor-core path, fp32 accumulation (mixed fp32/bf16, l.286).
- *          RINGX_F32 : plain FFMA path (max abs error ~1e-6; tf32 would not meet 1e-5).
+ *          RINGX_F32 : fp32 accuracy on the bf16 tensor cores: every fp32 operand is split exactly into three bf16 terms
+ *                      and the six leading cross products are accumulated in fp32 (max abs error ~1e-6 on O;
+ *                      kind::tf32, 10 mantissa bits, would not meet 1e-5).
  *   workspace  >= ringx_attn_fwd_workspace_bytes(...) bytes, 256-byte aligned; may be NULL when
  *              that query returns 0 (kv_chunk == N with bf16 and a grid large enough that the keys of the
  *              pass are not split, see ringx_attn_chunk_fwd_ex).  Contents are scratch. */

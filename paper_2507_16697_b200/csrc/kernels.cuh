@@ -50,7 +50,7 @@ cudaError_t launch_out_proj_bwd(const void* dy, const void* o, const void* w_o, 
 cudaError_t launch_qkv_proj_bwd(const void* dq, const void* dk, const void* dv, const void* x, const void* w_qkv,
                                 void* dx, float* dw_qkv, int B, int S, int H, int d, cudaStream_t stream);
 
-// ---- attn_f32.cu (plain FFMA path, config C1)
+// ---- attn_f32_split_sm100.cu (fp32 accuracy on the bf16 tensor cores by a 3-term operand split; config C1)
 // One KV-chunk pass, fp32: q [BH,Nq,d], k/v [BH,nk_stride,d] rows [k_off, k_off+nk) -> o_out fp32, lse_out.
 cudaError_t launch_attn_chunk_f32(const float* q, const float* k, const float* v, float* o_out, float* lse_out, int BH,
                                   int Nq, int nk_stride, int k_off, int nk, int d, float scale, cudaStream_t stream);

@@ -60,7 +60,7 @@ def test_sdpa_forward_and_gradients(sdpa, B, Hq, Hkv, N, d, chunk):
 
 
 def test_sdpa_fp32_forward_only_path(sdpa):
-    """fp32 tensors take the FFMA path (config C1); it has no backward, which must fail loudly, not fall back."""
+    """fp32 tensors take the tensor-core split path (config C1); it has no backward, which must fail loudly, not fall back."""
     q, k, v = (wl.make_tensor((1, 1, 512, 64), w, seed=2, dtype="f32").cuda() for w in "qkv")
     o = sdpa(q, k, v, kv_chunk=128)
     o_ref, _ = orc.attention_fwd(*(wl.to_f64_numpy(t[0, 0]) for t in (q, k, v)), 0.125)
