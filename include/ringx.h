@@ -113,8 +113,7 @@ RINGX_API int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, co
 /* Multi-head latent attention shapes (l.376 names MHA / GQA / MLA as the layer designs RingX is compatible with).  In its
  * materialised form an MLA layer attends with a score contraction wider than the values: d_qk = 192 (128 + 64 rotary
  * dimensions) and d_v = 128.  The path is the one of ringx_attn_fwd -- Eq. 1 per KV chunk, partials folded left to right by
- * the two-operand Eq. 5 in the chunk kernel's epilogue -- on a kernel laid out for these widths.  Forward only (the backward
- * of these shapes is not built: its accumulators, 128 + 192 columns beside S^T and dP^T, exceed the 512 TMEM columns).
+ * the two-operand Eq. 5 in the chunk kernel's epilogue -- on a kernel laid out for these widths.
  *   q, k [B,H,N,d_qk] bf16 (in); v [B,H,N,d_v] bf16 (in); o [B,H,N,d_v] bf16 (out); lse [B,H,N] float (out).
  *   Domain: d_qk == 192, d_v == 128, dtype RINGX_BF16, N % 256 == 0, kv_chunk % 128 == 0, N % kv_chunk == 0.
  *   workspace  >= ringx_attn_fwd_mla_workspace_bytes(...) bytes (0 when kv_chunk == N), 256-byte aligned. */
@@ -122,6 +121,19 @@ RINGX_API int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, vo
                        int B, int H, int N, int d_qk, int d_v, int kv_chunk, float scale, int dtype,
                        void* workspace, size_t workspace_bytes, void* stream);
 RINGX_API size_t ringx_attn_fwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk);
+
+/* Backward of the same shapes (the derivative of Eq. 1, P recomputed from the saved LSE; data flow of l.143 as for
+ * ringx_attn_bwd): per KV chunk dk, dv of the chunk's keys are complete and written once (atomic-free), dq accumulates in
+ * fp32 over the chunk passes (order of the sums not fixed) and is rounded to bf16 once at the end.
+ *   q, k, dq, dk [B,H,N,d_qk] bf16; v, o, dO, dv [B,H,N,d_v] bf16; lse [B,H,N] float (from ringx_attn_fwd_mla).
+ *   Outputs must not alias inputs.  Domain: d_qk == 192, d_v == 128, RINGX_BF16, N % 128 == 0, kv_chunk % 128 == 0,
+ *   N % kv_chunk == 0.  workspace >= ringx_attn_bwd_mla_workspace_bytes(...) bytes, 256-byte aligned (D, LSE*log2e and
+ *   the fp32 dq accumulator, which the kernel keeps transposed, [B,H,d_qk,N]).  ringx_set_deterministic has no effect here. */
+RINGX_API int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                       const void* dO, void* dq, void* dk, void* dv,
+                       int B, int H, int N, int d_qk, int d_v, int kv_chunk, float scale, int dtype,
+                       void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_bwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk);
 
 /* Two-operand Eq. 5, row by row:  m = max(lse_a,lse_b); w_a = exp(lse_a-m); w_b = exp(lse_b-m);
  * o_out = (w_a o_a + w_b o_b)/(w_a+w_b);  lse_out = m + log(w_a+w_b).

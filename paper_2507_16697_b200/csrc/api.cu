@@ -476,6 +476,62 @@ int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, flo
   return RINGX_OK;
 }
 
+// backward of the same shapes: D / lse2 preprocess (d_v = 128 wide), one pass of the MLA backward kernel per KV chunk into
+// the transposed fp32 dQ accumulator, transpose + bf16 cast of dQ
+size_t ringx_attn_bwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk) {
+  if (d_qk != 192 || d_v != 128 || check_shape(B, H, N, d_v, kv_chunk, 1.f, RINGX_BF16, true) != RINGX_OK) return 0;
+  const size_t R = (size_t)B * H * N;
+  return 2 * align_up(R * sizeof(float)) + align_up(R * d_qk * sizeof(float));
+}
+
+int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
+                       void* dq, void* dk, void* dv, int B, int H, int N, int d_qk, int d_v, int kv_chunk, float scale,
+                       int dtype, void* workspace, size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o || !lse || !dO || !dq || !dk || !dv) return RINGX_ERR_NULL_PTR;
+  if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (d_qk != 192 || d_v != 128) return RINGX_ERR_BAD_SHAPE;
+  int st = check_shape(B, H, N, d_v, kv_chunk, scale, dtype, true);
+  if (st != RINGX_OK) return st;
+  if ((long long)B * H * d_qk > 0x7FFFFFFFLL) return RINGX_ERR_BAD_SHAPE;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse) || !aligned16(dO) ||
+      !aligned16(dq) || !aligned16(dk) || !aligned16(dv))
+    return RINGX_ERR_MISALIGNED;
+  const size_t need = ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk);
+  if (!workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < need) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  const int BH = B * H;
+  const size_t R = (size_t)BH * N;
+  float* D = static_cast<float*>(workspace);
+  float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + align_up(R * sizeof(float)));
+  float* dq_acc_t = reinterpret_cast<float*>(static_cast<char*>(workspace) + 2 * align_up(R * sizeof(float)));
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = cudaMemsetAsync(dq_acc_t, 0, R * d_qk * sizeof(float), stream);
+    if (e == cudaSuccess) e = launch_bwd_preprocess(o, dO, lse, D, lse2, nullptr, (long long)R, d_v, scale, false, stream);
+  }
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  for (int c = 0; c < N / kv_chunk; ++c) {
+    Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
+    e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, BH, N, N, c * kv_chunk, kv_chunk, scale,
+                                        stream);
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = launch_dq_transpose_convert_mla(dq_acc_t, dq, BH, N, stream);
+  }
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
 int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse, int B, int H,
                          int Nq, int Nk, int d, float scale, int dtype, void* stream_) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);

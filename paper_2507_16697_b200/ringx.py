@@ -46,6 +46,10 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_fwd_mla.restype = c_i
     L.ringx_attn_fwd_mla_workspace_bytes.argtypes = [c_i] * 6
     L.ringx_attn_fwd_mla_workspace_bytes.restype = c_sz
+    L.ringx_attn_bwd_mla.argtypes = [c_p] * 9 + [c_i] * 6 + [c_f, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_bwd_mla.restype = c_i
+    L.ringx_attn_bwd_mla_workspace_bytes.argtypes = [c_i] * 6
+    L.ringx_attn_bwd_mla_workspace_bytes.restype = c_sz
     L.ringx_lse_merge.argtypes = [c_p] * 6 + [c_ll, c_i, c_i, c_i, c_p]
     L.ringx_lse_merge.restype = c_i
     L.ringx_attn_chunk_fwd.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p]
@@ -187,6 +191,26 @@ def ringx_attn_fwd_mla(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, w
                                   workspace.numel() if workspace is not None else 0, _stream())
     _check(st, "ringx_attn_fwd_mla")
     return o, lse
+
+
+def ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk) -> int:
+    return lib().ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
+
+
+def ringx_attn_bwd_mla(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspace=None):
+    """(dq, dk, dv) for multi-head latent attention shapes: q, k [B,H,N,192], v, o, dO [B,H,N,128] bf16 (include/ringx.h:
+    ringx_attn_bwd_mla)."""
+    B, H, N, d_qk = q.shape
+    d_v = v.shape[3]
+    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    need = lib().ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
+    if workspace is None:
+        workspace = _workspace(max(need, 256), q.device)
+    st = lib().ringx_attn_bwd_mla(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"), _dev(dO, "dO"),
+                                  _dev(dq, "dq"), _dev(dk, "dk"), _dev(dv, "dv"), B, H, N, d_qk, d_v, kv_chunk, scale,
+                                  _DTYPES[q.dtype], workspace.data_ptr(), workspace.numel(), _stream())
+    _check(st, "ringx_attn_bwd_mla")
+    return dq, dk, dv
 
 
 def ringx_attn_chunk_fwd(q, k, v, scale: float):

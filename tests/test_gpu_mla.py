@@ -1,12 +1,14 @@
 """Multi-head latent attention shapes (PAPER.md:376 names MLA among the layer designs RingX is
-compatible with): d_qk = 192, d_v = 128, forward.  The oracle is the same definition (oracle.attention takes d != dv;
-pinned by tests/test_oracle_pins.py::test_brute_force_forward_nonsquare); tolerances are the bf16 forward's."""
+compatible with): d_qk = 192, d_v = 128, forward and backward.  The oracle is the same definition (oracle.attention takes
+d != dv; pinned by tests/test_oracle_pins.py::test_brute_force_forward_nonsquare and, for the gradients, by
+test_gradients_match_finite_differences, which runs with d = 3, dv = 4); tolerances are those of the bf16 d = 64 / 128 paths."""
 import math
 
 import numpy as np
 import pytest
 import torch
 
+import grad_bounds as gb
 from oracle import attention as orc
 from paper_2507_16697_b200 import workloads as wl
 
@@ -109,4 +111,124 @@ def test_mla_errors(rx):
     assert call(192, 128, 256, 256, 0) == 3       # bf16 only
     assert call(192, 128, 256, 128, 1) == 1       # two passes need a workspace: NULL_PTR
     assert call(192, 128, 384, 384, 1) == 2       # N % 256
+    torch.cuda.synchronize()
+
+
+# ------------------------------------------------------------------------------------------------ backward
+def make_do(B, H, N, seed, device="cpu"):
+    return wl.make_tensor((B, H, N, DV), "do", seed=seed, dtype="bf16", device=device)
+
+
+def check_grads(dq, dk, dv, q64, k64, v64, do64, scale):
+    """stated Frobenius tolerance (2e-2) and the element-wise bounds of tests/grad_bounds.py, head by head"""
+    worst = 0.0
+    for b in range(q64.shape[0]):
+        for h in range(q64.shape[1]):
+            q_, k_, v_, do_ = q64[b, h], k64[b, h], v64[b, h], do64[b, h]
+            dq_ref, dk_ref, dv_ref = orc.attention_bwd(q_, k_, v_, do_, scale)
+            E = gb.d_error_rows(q_, k_, v_, do_, scale)
+            _, lse = orc.attention_fwd(q_, k_, v_, scale)
+            worst = max(worst, gb.check_grad("dq", f64(dq[b, h]), dq_ref, gb.dq_dterm(q_, k_, v_, do_, scale)),
+                        gb.check_grad("dk", f64(dk[b, h]), dk_ref, gb.dk_dterm(q_, k_, lse, E, scale)),
+                        gb.check_grad("dv", f64(dv[b, h]), dv_ref, None))
+    return worst
+
+
+@pytest.mark.parametrize("B,H,N,chunk,gain", [(1, 1, 128, 128, 1.0), (1, 2, 512, 128, 1.0), (2, 3, 1280, 256, 1.0),
+                                              (1, 2, 2304, 768, 1.0), (1, 1, 2048, 2048, 3.0), (1, 4, 1024, 512, 0.05)])
+def test_mla_backward_matches_oracle(rx, B, H, N, chunk, gain):
+    """dq, dk [.,192], dv [.,128] against the derivative of the definition: several 64-query sub-tiles and key tiles,
+    1-4 passes, peaked and near-uniform softmax; element by element."""
+    q, k, v = make(B, H, N, seed=131, gain=gain)
+    do = make_do(B, H, N, seed=131)
+    scale = 1.0 / math.sqrt(DQK)
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    if N % 256 == 0:
+        o, lse = rx.ringx_attn_fwd_mla(qd, kd, vd, chunk if N % chunk == 0 else N, scale)
+    else:                                   # the backward takes N % 128 == 0; feed it the oracle's forward there
+        o64, l64 = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+        o, lse = torch.from_numpy(o64).to(torch.bfloat16).cuda(), torch.from_numpy(l64).float().cuda()
+    dq, dk, dv = rx.ringx_attn_bwd_mla(qd, kd, vd, o, lse, dod, chunk, scale)
+    assert rx.ringx_last_launch_count() == N // chunk + 2
+    assert dq.shape == (B, H, N, DQK) and dk.shape == (B, H, N, DQK) and dv.shape == (B, H, N, DV)
+    check_grads(dq, dk, dv, f64(q), f64(k), f64(v), f64(do), scale)
+
+
+def test_mla_backward_every_panel_matters_and_chunk_independent(rx):
+    """Zeroing one 64-column panel of q (k, v, dO) in the ORACLE must break the agreement with the kernel's result: the
+    kernel contracts over all three panels of q, k and both of v, dO.  dk, dv of a key tile are written once by one CTA
+    whatever the chunking: bit-identical; dq is an fp32 reduce-add in arbitrary order: equal within rounding."""
+    B, H, N = 1, 1, 512
+    q, k, v = make(B, H, N, seed=137)
+    do = make_do(B, H, N, seed=137)
+    scale = 0.2
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    o, lse = rx.ringx_attn_fwd_mla(qd, kd, vd, N, scale)
+    dq, dk, dv = rx.ringx_attn_bwd_mla(qd, kd, vd, o, lse, dod, N, scale)
+    q64, k64, v64, do64 = (f64(t[0, 0]) for t in (q, k, v, do))
+    full = orc.attention_bwd(q64, k64, v64, do64, scale)
+    err = lambda g, r: np.linalg.norm(f64(g[0, 0]) - r) / np.linalg.norm(r)
+    assert max(err(dq, full[0]), err(dk, full[1]), err(dv, full[2])) <= 2e-2
+    for name, width in (("q", DQK), ("k", DQK), ("v", DV), ("do", DV)):
+        for p in range(width // 64):
+            args = {"q": q64.copy(), "k": k64.copy(), "v": v64.copy(), "do": do64.copy()}
+            args[name][:, 64 * p:64 * p + 64] = 0.0
+            cut = orc.attention_bwd(args["q"], args["k"], args["v"], args["do"], scale)
+            assert max(err(dq, cut[0]), err(dk, cut[1]), err(dv, cut[2])) > 0.1, (name, p)
+    for chunk in (128, 256):
+        dq2, dk2, dv2 = rx.ringx_attn_bwd_mla(qd, kd, vd, o, lse, dod, chunk, scale)
+        assert torch.equal(dk2, dk) and torch.equal(dv2, dv)
+        assert ((dq2.float() - dq.float()).norm() / dq.float().norm()).item() <= 2e-3
+
+
+def test_mla_backward_long_sequence_sampled(rx):
+    """N = 16384, two passes: dq on sampled query rows (sub-tile, tile and chunk boundaries) against all keys; dk, dv on
+    sampled key columns with the oracle's LSE and D of all rows of the head; sum_j dV_j = sum_i P^T dO invariants."""
+    B, H, N, chunk = 1, 2, 16384, 8192
+    q, k, v = make(B, H, N, seed=139, device="cuda")
+    do = make_do(B, H, N, seed=139, device="cuda")
+    scale = 1.0 / math.sqrt(DQK)
+    o, lse = rx.ringx_attn_fwd_mla(q, k, v, chunk, scale)
+    dq, dk, dv = rx.ringx_attn_bwd_mla(q, k, v, o, lse, do, chunk, scale)
+    for t in (dq, dk, dv):
+        assert torch.isfinite(t.float()).all()
+    rng = np.random.default_rng(5)
+    rows = np.array(sorted({0, 1, 63, 64, 65, 127, 128, 8191, 8192, N - 65, N - 64, N - 1} | set(rng.integers(0, N, 40).tolist())))
+    cols = np.array(sorted({0, 1, 127, 128, 129, 8191, 8192, 8193, N - 129, N - 128, N - 1} | set(rng.integers(0, N, 40).tolist())))
+    h = 1
+    q64, k64, v64, do64 = (f64(t[0, h]) for t in (q, k, v, do))
+    dq_ref, _, _ = orc.attention_bwd(q64[rows], k64, v64, do64[rows], scale)
+    gb.check_grad("dq", f64(dq[0, h][rows]), dq_ref, gb.dq_dterm(q64[rows], k64, v64, do64[rows], scale))
+    lse_all = np.empty(N)
+    D_all = np.empty(N)
+    for r0 in range(0, N, 2048):
+        lse_all[r0:r0 + 2048], D_all[r0:r0 + 2048] = orc.row_stats(q64[r0:r0 + 2048], k64, v64, do64[r0:r0 + 2048], scale)
+    dk_ref, dv_ref = orc.attention_bwd_cols(q64, k64[cols], v64[cols], do64, lse_all, D_all, scale)
+    o_all = np.concatenate([orc.attention_fwd(q64[r0:r0 + 2048], k64, v64, scale)[0] for r0 in range(0, N, 2048)])
+    E = gb.U_BF16 * (np.abs(do64) * np.abs(o_all)).sum(axis=1)
+    gb.check_grad("dk", f64(dk[0, h][cols]), dk_ref, gb.dk_dterm(q64, k64[cols], lse_all, E, scale))
+    gb.check_grad("dv", f64(dv[0, h][cols]), dv_ref, None)
+    # sum_j dV_j = sum_i dO_i (rows of P sum to 1) and sum_j dK_j = 0 on every head, from the full outputs
+    for hh in range(H):
+        sv, sdo = f64(dv[0, hh]).sum(axis=0), f64(do[0, hh]).sum(axis=0)
+        assert np.abs(sv - sdo).max() <= 2e-2 * np.abs(sdo).max() + 0.5
+        assert np.abs(f64(dk[0, hh]).sum(axis=0)).max() <= 1.0
+
+
+def test_mla_backward_errors(rx):
+    L = rx.lib()
+    t = torch.zeros(1, 1, 256, 192, dtype=torch.bfloat16, device="cuda")
+    v = torch.zeros(1, 1, 256, 128, dtype=torch.bfloat16, device="cuda")
+    lse = torch.zeros(1, 1, 256, device="cuda")
+    ws = torch.empty(rx.ringx_attn_bwd_mla_workspace_bytes(1, 1, 256, 192, 128, 256), dtype=torch.uint8, device="cuda")
+    call = lambda dqk, dv_, N, chunk, dt, w, wb: L.ringx_attn_bwd_mla(
+        t.data_ptr(), t.data_ptr(), v.data_ptr(), v.data_ptr(), lse.data_ptr(), v.data_ptr(), t.data_ptr(), t.data_ptr(),
+        v.data_ptr(), 1, 1, N, dqk, dv_, chunk, 0.1, dt, w, wb, None)
+    assert rx.ringx_attn_bwd_mla_workspace_bytes(1, 1, 256, 128, 128, 256) == 0
+    assert call(192, 128, 256, 256, 1, ws.data_ptr(), ws.numel()) == 0
+    assert call(128, 128, 256, 256, 1, ws.data_ptr(), ws.numel()) == 2      # only the 192 / 128 pair: BAD_SHAPE
+    assert call(192, 128, 256, 256, 0, ws.data_ptr(), ws.numel()) == 3      # bf16 only
+    assert call(192, 128, 256, 256, 1, None, 0) == 1                        # NULL_PTR
+    assert call(192, 128, 256, 256, 1, ws.data_ptr(), 1024) == 5            # WORKSPACE_TOO_SMALL
+    assert call(192, 128, 192, 192, 1, ws.data_ptr(), ws.numel()) == 2      # N % 128
     torch.cuda.synchronize()
