@@ -615,6 +615,17 @@ def next_rows_measure(ringx, wl, dev, reps=5):
     out["gqa_16q4kv_N32768_d128"] = {"fwd_tflops": fl / ms / 1e9}
     ms = timeit(lambda: ringx.ringx_attn_bwd_gqa(q, k, v, o, lse, do, chunk, scale))
     out["gqa_16q4kv_N32768_d128"]["bwd_tflops"] = 2.5 * fl / ms / 1e9
+    # MLA shapes (d_qk = 192, d_v = 128): 8 heads, N = 65536, 4 passes of 16384 keys; FLOPs 2 N^2 (192 + 128) forward,
+    # 2 N^2 (192 + 128 + 128 + 192 + 192) backward per head
+    Hm, Nm, cm = 8, 65536, 16384
+    qm, km = (wl.make_tensor((1, Hm, Nm, 192), w, seed=78, dtype="bf16", device=dev) for w in "qk")
+    vm, dom = (wl.make_tensor((1, Hm, Nm, 128), w, seed=78, dtype="bf16", device=dev) for w in ("v", "do"))
+    om, lm_ = ringx.ringx_attn_fwd_mla(qm, km, vm, cm, 192 ** -0.5)
+    ms = timeit(lambda: ringx.ringx_attn_fwd_mla(qm, km, vm, cm, 192 ** -0.5, o=om, lse=lm_))
+    out["mla_dqk192_dv128_H8_N65536"] = {"fwd_tflops": 2.0 * Hm * Nm * Nm * 320 / ms / 1e9}
+    ms = timeit(lambda: ringx.ringx_attn_bwd_mla(qm, km, vm, om, lm_, dom, cm, 192 ** -0.5))
+    out["mla_dqk192_dv128_H8_N65536"]["bwd_tflops"] = 2.0 * Hm * Nm * Nm * 832 / ms / 1e9
+    del qm, km, vm, dom, om, lm_
     # RingX backward step: 16384 local query rows against one 16384-key chunk of another rank (global lse)
     ql, ol, dol = (t[:, :4, :16384].contiguous() for t in (q, o, do))
     lsel = lse[:, :4, :16384].contiguous()

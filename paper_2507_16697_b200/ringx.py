@@ -197,12 +197,14 @@ def ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk) -> int:
     return lib().ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
 
 
-def ringx_attn_bwd_mla(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspace=None):
+def ringx_attn_bwd_mla(q, k, v, o, lse, dO, kv_chunk: int, scale: float, dq=None, dk=None, dv=None, workspace=None):
     """(dq, dk, dv) for multi-head latent attention shapes: q, k [B,H,N,192], v, o, dO [B,H,N,128] bf16 (include/ringx.h:
     ringx_attn_bwd_mla)."""
     B, H, N, d_qk = q.shape
     d_v = v.shape[3]
-    dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    dq = torch.empty_like(q) if dq is None else dq
+    dk = torch.empty_like(k) if dk is None else dk
+    dv = torch.empty_like(v) if dv is None else dv
     need = lib().ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
     if workspace is None:
         workspace = _workspace(max(need, 256), q.device)

@@ -29,7 +29,9 @@ class _RingXAttention(torch.autograd.Function):
     @staticmethod
     def forward(ctx, q, k, v, scale, kv_chunk):
         q, k, v = q.contiguous(), k.contiguous(), v.contiguous()
-        if q.shape[1] == k.shape[1]:
+        if q.shape[-1] != v.shape[-1]:        # multi-head latent attention shapes (d_qk = 192, d_v = 128)
+            o, lse = ringx.ringx_attn_fwd_mla(q, k, v, kv_chunk, scale)
+        elif q.shape[1] == k.shape[1]:
             o, lse = ringx.ringx_attn_fwd(q, k, v, kv_chunk, scale)
         else:
             o, lse = ringx.ringx_attn_fwd_gqa(q, k, v, kv_chunk, scale)
@@ -41,7 +43,9 @@ class _RingXAttention(torch.autograd.Function):
     def backward(ctx, dO):
         q, k, v, o, lse = ctx.saved_tensors
         dO = dO.contiguous()
-        if q.shape[1] == k.shape[1]:
+        if q.shape[-1] != v.shape[-1]:
+            dq, dk, dv = ringx.ringx_attn_bwd_mla(q, k, v, o, lse, dO, ctx.kv_chunk, ctx.scale)
+        elif q.shape[1] == k.shape[1]:
             dq, dk, dv = ringx.ringx_attn_bwd(q, k, v, o, lse, dO, ctx.kv_chunk, ctx.scale)
         else:
             dq, dk, dv = ringx.ringx_attn_bwd_gqa(q, k, v, o, lse, dO, ctx.kv_chunk, ctx.scale)
@@ -70,7 +74,8 @@ def ringx_sdpa(query, key, value, attn_mask=None, dropout_p: float = 0.0, is_cau
     """softmax(scale * Q K^T) V with the signature of torch's scaled_dot_product_attention.
 
     query [B,Hq,N,d], key/value [B,Hkv,N,d] (Hkv divides Hq: grouped-query attention needs enable_gqa=True, as in
-    torch), bf16 or fp32 CUDA tensors, d in {64,128}.  `scale` defaults to 1/sqrt(d).  `kv_chunk`: keys per pass.
+    torch), bf16 or fp32 CUDA tensors, d in {64,128} -- or the multi-head-latent-attention widths query/key [.,192],
+    value [.,128] (bf16, Hkv == Hq).  `scale` defaults to 1/sqrt(d).  `kv_chunk`: keys per pass.
     `schedule` = "b" or "a" runs the paper's RingX_b / RingX_a over `comm` (default: the torch.distributed world)
     with the arguments being the local sequence chunks."""
     if attn_mask is not None or dropout_p != 0.0 or is_causal:

@@ -53,6 +53,23 @@ def test_attention_forward_backward_guards(rx):
         assert bool(torch.isfinite(dq.float()).all())
 
 
+def test_mla_forward_backward_guards(rx):
+    for (B, H, N, chunk) in ((1, 1, 256, 128), (2, 3, 768, 256)):
+        g = Guarded()
+        q, k = (wl.make_tensor((B, H, N, 192), w, seed=5).cuda() for w in "qk")
+        v, do = (wl.make_tensor((B, H, N, 128), w, seed=5).cuda() for w in ("v", "do"))
+        scale = 192 ** -0.5
+        o, lse = g.make((B, H, N, 128), torch.bfloat16), g.make((B, H, N), torch.float32)
+        ws = g.make((max(256, rx.ringx_attn_fwd_mla_workspace_bytes(B, H, N, 192, 128, chunk)),), torch.uint8)
+        rx.ringx_attn_fwd_mla(q, k, v, chunk, scale, o=o, lse=lse, workspace=ws)
+        dq, dk = (g.make((B, H, N, 192), torch.bfloat16) for _ in range(2))
+        dv = g.make((B, H, N, 128), torch.bfloat16)
+        wsb = g.make((rx.ringx_attn_bwd_mla_workspace_bytes(B, H, N, 192, 128, chunk),), torch.uint8)
+        rx.ringx_attn_bwd_mla(q, k, v, o, lse, do, chunk, scale, dq=dq, dk=dk, dv=dv, workspace=wsb)
+        g.check()
+        assert bool(torch.isfinite(dq.float()).all())
+
+
 def test_split_kv_guards(rx):
     B, H, Nq, Nk, d = 1, 3, 256, 3072, 128
     g = Guarded()

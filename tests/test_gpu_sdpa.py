@@ -59,6 +59,31 @@ def test_sdpa_forward_and_gradients(sdpa, B, Hq, Hkv, N, d, chunk):
     assert relf(k.grad.float().cpu().numpy(), kt.grad.cpu().numpy()) <= 2e-2
 
 
+def test_sdpa_mla_shapes(sdpa):
+    """query/key of width 192, value of width 128 (multi-head latent attention) through the same drop-in:
+    forward and gradients against the oracle and against torch's SDPA (which takes E != Ev as well)."""
+    B, H, N = 1, 2, 512
+    q = wl.make_tensor((B, H, N, 192), "q", seed=43).cuda().requires_grad_()
+    k = wl.make_tensor((B, H, N, 192), "k", seed=43).cuda().requires_grad_()
+    v = wl.make_tensor((B, H, N, 128), "v", seed=43).cuda().requires_grad_()
+    do = wl.make_tensor((B, H, N, 128), "do", seed=43).cuda()
+    o = sdpa(q, k, v, kv_chunk=256)
+    o.backward(do)
+    scale = 1.0 / math.sqrt(192)
+    q64, k64, v64, do64 = (wl.to_f64_numpy(t.detach()) for t in (q, k, v, do))
+    for h in range(H):
+        o_ref, _ = orc.attention_fwd(q64[0, h], k64[0, h], v64[0, h], scale)
+        refs = orc.attention_bwd(q64[0, h], k64[0, h], v64[0, h], do64[0, h], scale)
+        assert relf(o[0, h].detach().float().cpu().numpy(), o_ref) <= 1e-2
+        for g, r in zip((q.grad, k.grad, v.grad), refs):
+            assert relf(g[0, h].float().cpu().numpy(), r) <= 2e-2
+    qt, kt, vt = (t.detach().float().requires_grad_() for t in (q, k, v))
+    ot = torch.nn.functional.scaled_dot_product_attention(qt, kt, vt)
+    ot.backward(do.float())
+    assert relf(o.detach().float().cpu().numpy(), ot.detach().cpu().numpy()) <= 1e-2
+    assert relf(k.grad.float().cpu().numpy(), kt.grad.cpu().numpy()) <= 2e-2
+
+
 def test_sdpa_fp32_forward_only_path(sdpa):
     """fp32 tensors take the tensor-core split path (config C1); it has no backward, which must fail loudly, not fall back."""
     q, k, v = (wl.make_tensor((1, 1, 512, 64), w, seed=2, dtype="f32").cuda() for w in "qkv")
