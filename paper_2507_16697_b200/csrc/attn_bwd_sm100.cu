@@ -38,12 +38,7 @@ constexpr int kBwdComputeRegs = 176, kBwdDrainRegs = 96, kBwdAuxRegs = 40;   // 
 // instead of MUFU.EX2.  At d = 64 phase A's 16 ex2 per clock are the co-limiter (5 MMAs of half the length per
 // exponential): every fourth pair on the FMA pipe measured +4 % (C4 backward 897 -> 935 TFLOP/s); at d = 128 the
 // tensor chain hides phase A and any share measured -1 %, so it stays on the MUFU.
-#ifndef RINGX_BWD_POLY_MASK_D64
-#define RINGX_BWD_POLY_MASK_D64 0x8888
-#endif
-#ifndef RINGX_BWD_POLY_MASK_D128
-#define RINGX_BWD_POLY_MASK_D128 0x0000
-#endif
+constexpr unsigned kBwdPolyMaskD64 = 0x8888, kBwdPolyMaskD128 = 0x0000;
 
 template <int kD>
 struct BwdCfg {
@@ -65,7 +60,7 @@ struct BwdCfg {
   // dS^T Q.  The SM's shared memory (128 B/clk, which the SS MMAs saturate) then carries 64 KB less per step.
   static constexpr bool kTmemOperands = kD == 64;
   static constexpr uint32_t tK = 448, tV = 480;
-  static constexpr unsigned kPolyMask = kD == 64 ? RINGX_BWD_POLY_MASK_D64 : RINGX_BWD_POLY_MASK_D128;
+  static constexpr unsigned kPolyMask = kD == 64 ? kBwdPolyMaskD64 : kBwdPolyMaskD128;
 };
 
 template <int kD>

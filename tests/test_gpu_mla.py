@@ -183,8 +183,9 @@ def test_mla_backward_every_panel_matters_and_chunk_independent(rx):
 
 def test_mla_backward_long_sequence_sampled(rx):
     """N = 16384, two passes: dq on sampled query rows (sub-tile, tile and chunk boundaries) against all keys; dk, dv on
-    sampled key columns with the oracle's LSE and D of all rows of the head; sum_j dV_j = sum_i P^T dO invariants."""
-    B, H, N, chunk = 1, 2, 16384, 8192
+    sampled key columns with the oracle's LSE and D of all rows of the head; sum_j dV_j = sum_i P^T dO invariants.
+    192 CTAs per pass: more than one wave of the 148 SMs."""
+    B, H, N, chunk = 1, 3, 16384, 8192
     q, k, v = make(B, H, N, seed=139, device="cuda")
     do = make_do(B, H, N, seed=139, device="cuda")
     scale = 1.0 / math.sqrt(DQK)
@@ -195,7 +196,7 @@ def test_mla_backward_long_sequence_sampled(rx):
     rng = np.random.default_rng(5)
     rows = np.array(sorted({0, 1, 63, 64, 65, 127, 128, 8191, 8192, N - 65, N - 64, N - 1} | set(rng.integers(0, N, 40).tolist())))
     cols = np.array(sorted({0, 1, 127, 128, 129, 8191, 8192, 8193, N - 129, N - 128, N - 1} | set(rng.integers(0, N, 40).tolist())))
-    h = 1
+    h = 2
     q64, k64, v64, do64 = (f64(t[0, h]) for t in (q, k, v, do))
     dq_ref, _, _ = orc.attention_bwd(q64[rows], k64, v64, do64[rows], scale)
     gb.check_grad("dq", f64(dq[0, h][rows]), dq_ref, gb.dq_dterm(q64[rows], k64, v64, do64[rows], scale))
