@@ -135,6 +135,24 @@ RINGX_API int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, co
                        void* workspace, size_t workspace_bytes, void* stream);
 RINGX_API size_t ringx_attn_bwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk);
 
+/* The per-device RingX steps (l.137-147) for the same widths -- `Nq` local query rows against the `Nk` keys given:
+ * ringx_attn_chunk_fwd_mla is ringx_attn_chunk_fwd_ex (one pass in general form: partials, in-place fold, or last fold to
+ * bf16; o_acc / o_out are [B,H,Nq,d_v]; no split-KV, no workspace), Nq % 256 == 0, Nk % 128 == 0;
+ * ringx_attn_bwd_partial_mla is ringx_attn_bwd_partial_ex with the fp32 dQ accumulator kept TRANSPOSED, dq_acc_t
+ * [B,H,d_qk,Nq] (zeroed by the caller before the first step; reduce-added in arbitrary order), dk [B,H,Nk,d_qk] and dv
+ * [B,H,Nk,d_v] of dkv_dtype (bf16, or fp32 shares of a cross-device sum), `prepared` != 0 when the workspace already holds
+ * D and LSE*log2e of this (o, lse, dO) from an earlier step; workspace >= ringx_attn_bwd_partial_mla_workspace_bytes(B,H,Nq),
+ * Nq % 128 == 0;  ringx_dq_finalize_mla writes dq [B,H,Nq,d_qk] bf16 = transpose(dq_acc_t) after the last step. */
+RINGX_API int ringx_attn_chunk_fwd_mla(const void* q, const void* k, const void* v, const float* o_acc, const float* lse_acc,
+                             void* o_out, float* lse_out, int B, int H, int Nq, int Nk, int d_qk, int d_v, float scale,
+                             int dtype, int o_out_dtype, void* stream);
+RINGX_API int ringx_attn_bwd_partial_mla(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                               const void* dO, float* dq_acc_t, void* dk, void* dv,
+                               int B, int H, int Nq, int Nk, int d_qk, int d_v, float scale, int dtype, int dkv_dtype,
+                               int prepared, void* workspace, size_t workspace_bytes, void* stream);
+RINGX_API size_t ringx_attn_bwd_partial_mla_workspace_bytes(int B, int H, int Nq);
+RINGX_API int ringx_dq_finalize_mla(const float* dq_acc_t, void* dq, int B, int H, int Nq, int d_qk, void* stream);
+
 /* Two-operand Eq. 5, row by row:  m = max(lse_a,lse_b); w_a = exp(lse_a-m); w_b = exp(lse_b-m);
  * o_out = (w_a o_a + w_b o_b)/(w_a+w_b);  lse_out = m + log(w_a+w_b).
  * An operand with lse = -inf has weight 0; both -inf gives o_out = 0, lse_out = -inf; NaN propagates.

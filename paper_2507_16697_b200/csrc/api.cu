@@ -519,12 +519,114 @@ int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* 
   for (int c = 0; c < N / kv_chunk; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
     e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, BH, N, N, c * kv_chunk, kv_chunk, scale,
-                                        stream);
+                                        RINGX_BF16, stream);
     if (e != cudaSuccess) return cuda_status(e);
   }
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
     e = launch_dq_transpose_convert_mla(dq_acc_t, dq, BH, N, stream);
+  }
+  count_launch();
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+// ---- the per-device RingX steps for the MLA widths (Nq != Nk; PAPER.md:137-147 with the layer design of PAPER.md:376)
+static int check_mla_step(int B, int H, int Nq, int Nk, int d_qk, int d_v, float scale, int dtype, int nq_mult) {
+  if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  if (d_qk != 192 || d_v != 128) return RINGX_ERR_BAD_SHAPE;
+  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || Nk % 128 || Nq % nq_mult) return RINGX_ERR_BAD_SHAPE;
+  if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
+    return RINGX_ERR_BAD_SHAPE;
+  if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
+  return RINGX_OK;
+}
+
+int ringx_attn_chunk_fwd_mla(const void* q, const void* k, const void* v, const float* o_acc, const float* lse_acc,
+                             void* o_out, float* lse_out, int B, int H, int Nq, int Nk, int d_qk, int d_v, float scale,
+                             int dtype, int o_out_dtype, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o_out || !lse_out || (o_acc == nullptr) != (lse_acc == nullptr)) return RINGX_ERR_NULL_PTR;
+  if (o_out_dtype != RINGX_F32 && o_out_dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
+  int st = check_mla_step(B, H, Nq, Nk, d_qk, d_v, scale, dtype, 256);
+  if (st != RINGX_OK) return st;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o_acc) || !aligned16(lse_acc) || !aligned16(o_out) ||
+      !aligned16(lse_out))
+    return RINGX_ERR_MISALIGNED;
+  if (o_acc && o_out_dtype == RINGX_BF16 && (o_out == static_cast<const void*>(o_acc) || lse_out == lse_acc))
+    return RINGX_ERR_BAD_SHAPE;              // a bf16 result cannot overwrite the fp32 accumulator
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  const int epi = o_acc ? (o_out_dtype == RINGX_BF16 ? kFwdEpiFoldFinal : kFwdEpiFold)
+                        : (o_out_dtype == RINGX_BF16 ? kFwdEpiFinal : kFwdEpiPartial);
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
+    e = launch_attn_chunk_fwd_mla_sm100(q, k, v, o_out, lse_out, o_acc, lse_acc, B * H, Nq, Nk, 0, Nk, scale, epi, stream);
+  }
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+size_t ringx_attn_bwd_partial_mla_workspace_bytes(int B, int H, int Nq) {
+  if (B <= 0 || H <= 0 || Nq <= 0) return 0;
+  return 2 * align_up((size_t)B * H * Nq * sizeof(float));
+}
+
+int ringx_attn_bwd_partial_mla(const void* q, const void* k, const void* v, const void* o, const float* lse,
+                               const void* dO, float* dq_acc_t, void* dk, void* dv, int B, int H, int Nq, int Nk, int d_qk,
+                               int d_v, float scale, int dtype, int dkv_dtype, int prepared, void* workspace,
+                               size_t workspace_bytes, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!q || !k || !v || !o || !lse || !dO || !dq_acc_t || !dk || !dv) return RINGX_ERR_NULL_PTR;
+  if (dkv_dtype != RINGX_BF16 && dkv_dtype != RINGX_F32) return RINGX_ERR_BAD_DTYPE;
+  int st = check_mla_step(B, H, Nq, Nk, d_qk, d_v, scale, dtype, 128);
+  if (st != RINGX_OK) return st;
+  if ((long long)B * H * d_qk > 0x7FFFFFFFLL) return RINGX_ERR_BAD_SHAPE;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse) || !aligned16(dO) ||
+      !aligned16(dq_acc_t) || !aligned16(dk) || !aligned16(dv))
+    return RINGX_ERR_MISALIGNED;
+  const size_t need = ringx_attn_bwd_partial_mla_workspace_bytes(B, H, Nq);
+  if (!workspace) return RINGX_ERR_NULL_PTR;
+  if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return RINGX_ERR_MISALIGNED;
+  if (workspace_bytes < need) return RINGX_ERR_WORKSPACE_TOO_SMALL;
+  if ((st = check_arch()) != RINGX_OK) return st;
+  tl_launches = 0;
+  const size_t R = (size_t)B * H * Nq;
+  float* D = static_cast<float*>(workspace);
+  float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + align_up(R * sizeof(float)));
+  cudaError_t e;
+  if (!prepared) {
+    {
+      Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+      e = launch_bwd_preprocess(o, dO, lse, D, lse2, nullptr, (long long)R, d_v, scale, false, stream);
+    }
+    count_launch();
+    if (e != cudaSuccess) return cuda_status(e);
+  }
+  {
+    Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
+    e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, B * H, Nq, Nk, 0, Nk, scale, dkv_dtype, stream);
+  }
+  if (e != cudaSuccess) return cuda_status(e);
+  tl_last_launches = tl_launches;
+  return RINGX_OK;
+}
+
+int ringx_dq_finalize_mla(const float* dq_acc_t, void* dq, int B, int H, int Nq, int d_qk, void* stream_) {
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  if (!dq_acc_t || !dq) return RINGX_ERR_NULL_PTR;
+  if (d_qk != 192 || B <= 0 || H <= 0 || Nq <= 0 || Nq % 64 || (long long)B * H > 65535) return RINGX_ERR_BAD_SHAPE;
+  if (!aligned16(dq_acc_t) || !aligned16(dq)) return RINGX_ERR_MISALIGNED;
+  int st = check_arch();
+  if (st != RINGX_OK) return st;
+  tl_launches = 0;
+  cudaError_t e;
+  {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = launch_dq_transpose_convert_mla(dq_acc_t, dq, B * H, Nq, stream);
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);

@@ -52,7 +52,8 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
                           const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_do,
                           const __grid_constant__ CUtensorMap map_dq_a, const __grid_constant__ CUtensorMap map_dq_b,
                           const float* __restrict__ lse2, const float* __restrict__ Dvec, void* __restrict__ dk,
-                          void* __restrict__ dv, int N, int nk_stride, int k_off, float scale_log2, float scale) {
+                          void* __restrict__ dv, int dkv_f32, int N, int nk_stride, int k_off, float scale_log2,
+                          float scale) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sK = smem;
@@ -345,20 +346,30 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     tc_fence_after();
     const int width = half == 0 ? kDv : kDqk;
     const uint32_t tSrc = tmem + (half == 0 ? tDV : tDK) + lane_off;
-    __nv_bfloat16* out = static_cast<__nv_bfloat16*>(half == 0 ? dv : dk) + (static_cast<size_t>(k_row0) + row) * width;
+    const size_t out_off = (static_cast<size_t>(k_row0) + row) * width;
+    // bf16 (the single-device result), or fp32 (one device's share of a cross-device sum: RingX_a/b reduce the shares
+    // in fp32 and round once)
     for (int c = 0; c < width / 32; ++c) {
       uint32_t r[32];
       tmem_ld_x32(tSrc + c * 32, r);
       tmem_wait_ld();
-      uint4* dst = reinterpret_cast<uint4*>(out + c * 32);
+      if (dkv_f32) {
+        float4* dst = reinterpret_cast<float4*>(static_cast<float*>(half == 0 ? dv : dk) + out_off + c * 32);
 #pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        uint4 u;
-        u.x = pack_bf16x2(__uint_as_float(r[g * 8 + 0]), __uint_as_float(r[g * 8 + 1]));
-        u.y = pack_bf16x2(__uint_as_float(r[g * 8 + 2]), __uint_as_float(r[g * 8 + 3]));
-        u.z = pack_bf16x2(__uint_as_float(r[g * 8 + 4]), __uint_as_float(r[g * 8 + 5]));
-        u.w = pack_bf16x2(__uint_as_float(r[g * 8 + 6]), __uint_as_float(r[g * 8 + 7]));
-        dst[g] = u;
+        for (int g = 0; g < 8; ++g)
+          dst[g] = make_float4(__uint_as_float(r[g * 4]), __uint_as_float(r[g * 4 + 1]), __uint_as_float(r[g * 4 + 2]),
+                               __uint_as_float(r[g * 4 + 3]));
+      } else {
+        uint4* dst = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(half == 0 ? dv : dk) + out_off + c * 32);
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          uint4 u;
+          u.x = pack_bf16x2(__uint_as_float(r[g * 8 + 0]), __uint_as_float(r[g * 8 + 1]));
+          u.y = pack_bf16x2(__uint_as_float(r[g * 8 + 2]), __uint_as_float(r[g * 8 + 3]));
+          u.z = pack_bf16x2(__uint_as_float(r[g * 8 + 4]), __uint_as_float(r[g * 8 + 5]));
+          u.w = pack_bf16x2(__uint_as_float(r[g * 8 + 6]), __uint_as_float(r[g * 8 + 7]));
+          dst[g] = u;
+        }
       }
     }
   } else if (warp < 12) {
@@ -440,7 +451,7 @@ dq_transpose_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __rest
 cudaError_t launch_attn_chunk_bwd_mla_sm100(const void* q, const void* k, const void* v, const void* dO,
                                             const float* lse2, const float* D, float* dq_acc_t, void* dk, void* dv,
                                             int BH, int N, int nk_stride, int k_off, int nk, float scale,
-                                            cudaStream_t stream) {
+                                            int dkv_dtype, cudaStream_t stream) {
   CUtensorMap mq, mk, mv, mdo, mdqa, mdqb;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   const uint64_t rows = (uint64_t)BH * N, krows = (uint64_t)BH * nk_stride;
@@ -455,8 +466,8 @@ cudaError_t launch_attn_chunk_bwd_mla_sm100(const void* q, const void* k, const 
   static unsigned char configured[kMaxDevices];
   if (cudaError_t e = set_max_dyn_smem_once(kern, kSmemBytes, configured); e != cudaSuccess) return e;
   dim3 grid(nk / kKeys, BH);
-  kern<<<grid, kThreads, kSmemBytes, stream>>>(mq, mk, mv, mdo, mdqa, mdqb, lse2, D, dk, dv, N, nk_stride, k_off,
-                                               scale * 1.4426950408889634f, scale);
+  kern<<<grid, kThreads, kSmemBytes, stream>>>(mq, mk, mv, mdo, mdqa, mdqb, lse2, D, dk, dv, dkv_dtype == RINGX_F32, N, nk_stride,
+                                               k_off, scale * 1.4426950408889634f, scale);
   count_launch();
   return cudaGetLastError();
 }

@@ -79,11 +79,11 @@ cudaError_t launch_attn_chunk_fwd_mla_sm100(const void* q, const void* k, const 
 // One KV-chunk pass of the backward: q [BH,N,192], dO [BH,N,128], k,dk [BH,nk_stride,192], v,dv [BH,nk_stride,128];
 // writes dk,dv rows [k_off, k_off+nk) of every head (bf16), reduce-adds these keys' contribution to dQ into the
 // TRANSPOSED fp32 accumulator dq_acc_t [BH,192,N] (zeroed by the caller before the first pass).  N % 64 == 0.
-// lse2, D as for launch_attn_chunk_bwd_sm100 (launch_bwd_preprocess with d = 128).
+// lse2, D as for launch_attn_chunk_bwd_sm100 (launch_bwd_preprocess with d = 128).  dkv_dtype: RINGX_BF16 or RINGX_F32.
 cudaError_t launch_attn_chunk_bwd_mla_sm100(const void* q, const void* k, const void* v, const void* dO,
                                             const float* lse2, const float* D, float* dq_acc_t, void* dk, void* dv,
                                             int BH, int N, int nk_stride, int k_off, int nk, float scale,
-                                            cudaStream_t stream);
+                                            int dkv_dtype, cudaStream_t stream);
 // dq [BH,N,192] bf16 = transpose(dq_acc_t [BH,192,N] fp32)
 cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int BH, int N, cudaStream_t stream);
 

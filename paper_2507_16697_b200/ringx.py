@@ -50,6 +50,14 @@ def lib() -> ctypes.CDLL:
     L.ringx_attn_bwd_mla.restype = c_i
     L.ringx_attn_bwd_mla_workspace_bytes.argtypes = [c_i] * 6
     L.ringx_attn_bwd_mla_workspace_bytes.restype = c_sz
+    L.ringx_attn_chunk_fwd_mla.argtypes = [c_p] * 7 + [c_i] * 6 + [c_f, c_i, c_i, c_p]
+    L.ringx_attn_chunk_fwd_mla.restype = c_i
+    L.ringx_attn_bwd_partial_mla.argtypes = [c_p] * 9 + [c_i] * 6 + [c_f, c_i, c_i, c_i, c_p, c_sz, c_p]
+    L.ringx_attn_bwd_partial_mla.restype = c_i
+    L.ringx_attn_bwd_partial_mla_workspace_bytes.argtypes = [c_i] * 3
+    L.ringx_attn_bwd_partial_mla_workspace_bytes.restype = c_sz
+    L.ringx_dq_finalize_mla.argtypes = [c_p, c_p, c_i, c_i, c_i, c_i, c_p]
+    L.ringx_dq_finalize_mla.restype = c_i
     L.ringx_lse_merge.argtypes = [c_p] * 6 + [c_ll, c_i, c_i, c_i, c_p]
     L.ringx_lse_merge.restype = c_i
     L.ringx_attn_chunk_fwd.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p]
@@ -213,6 +221,63 @@ def ringx_attn_bwd_mla(q, k, v, o, lse, dO, kv_chunk: int, scale: float, dq=None
                                   _DTYPES[q.dtype], workspace.data_ptr(), workspace.numel(), _stream())
     _check(st, "ringx_attn_bwd_mla")
     return dq, dk, dv
+
+
+def ringx_attn_chunk_fwd_mla(q, k, v, scale: float, o_acc=None, lse_acc=None, final: bool = False):
+    """One pass of the MLA widths in general form (include/ringx.h: ringx_attn_chunk_fwd_mla): q [B,H,Nq,192] against
+    k [B,H,Nk,192], v [B,H,Nk,128].  No accumulator: (loc_out fp32, loc_lse), or (o bf16, lse) when final.  With
+    (o_acc, lse_acc): folds this pass in -- in place, or, when final, into a new (o bf16, lse)."""
+    B, H, Nq, d_qk = q.shape
+    Nk, d_v = k.shape[2], v.shape[3]
+    if (o_acc is None) != (lse_acc is None):
+        raise ValueError("o_acc and lse_acc go together")
+    if final:
+        o_out = torch.empty((B, H, Nq, d_v), dtype=torch.bfloat16, device=q.device)
+        lse_out = torch.empty((B, H, Nq), dtype=torch.float32, device=q.device)
+    elif o_acc is not None:
+        o_out, lse_out = o_acc, lse_acc
+    else:
+        o_out = torch.empty((B, H, Nq, d_v), dtype=torch.float32, device=q.device)
+        lse_out = torch.empty((B, H, Nq), dtype=torch.float32, device=q.device)
+    st = lib().ringx_attn_chunk_fwd_mla(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"),
+                                        _dev(o_acc, "o_acc") if o_acc is not None else None,
+                                        _dev(lse_acc, "lse_acc") if lse_acc is not None else None,
+                                        _dev(o_out, "o_out"), _dev(lse_out, "lse_out"), B, H, Nq, Nk, d_qk, d_v, scale,
+                                        _DTYPES[q.dtype], _DTYPES[o_out.dtype], _stream())
+    _check(st, "ringx_attn_chunk_fwd_mla")
+    return o_out, lse_out
+
+
+def ringx_attn_bwd_partial_mla_workspace_bytes(B, H, Nq) -> int:
+    return lib().ringx_attn_bwd_partial_mla_workspace_bytes(B, H, Nq)
+
+
+def ringx_attn_bwd_partial_mla(q, k, v, o, lse, dO, scale: float, dq_acc_t, dk, dv, workspace, prepared: bool = False):
+    """The per-device backward step for the MLA widths (include/ringx.h: ringx_attn_bwd_partial_mla).  dq_acc_t holds the
+    fp32 dQ accumulator TRANSPOSED, [B,H,192,Nq] (any tensor of B*H*Nq*192 floats: it is opaque until
+    ringx_dq_finalize_mla); dk, dv bf16 or float32 shares.  Every buffer is the caller's; returns (dq_acc_t, dk, dv)."""
+    B, H, Nq, d_qk = q.shape
+    Nk, d_v = k.shape[2], v.shape[3]
+    if dk.dtype != dv.dtype:
+        raise ValueError("dk and dv must have the same dtype")
+    if dq_acc_t.dtype != torch.float32 or dq_acc_t.numel() != q.numel():
+        raise ValueError("dq_acc_t must hold B*H*Nq*d_qk floats")
+    st = lib().ringx_attn_bwd_partial_mla(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                                          _dev(dO, "dO"), _dev(dq_acc_t, "dq_acc_t"), _dev(dk, "dk"), _dev(dv, "dv"),
+                                          B, H, Nq, Nk, d_qk, d_v, scale, _DTYPES[q.dtype], _DTYPES[dk.dtype],
+                                          1 if prepared else 0, workspace.data_ptr(),
+                                          workspace.numel() * workspace.element_size(), _stream())
+    _check(st, "ringx_attn_bwd_partial_mla")
+    return dq_acc_t, dk, dv
+
+
+def ringx_dq_finalize_mla(dq_acc_t, B, H, Nq, d_qk=192, dq=None):
+    """dq [B,H,Nq,192] bf16 from the transposed fp32 accumulator (include/ringx.h: ringx_dq_finalize_mla)."""
+    if dq is None:
+        dq = torch.empty((B, H, Nq, d_qk), dtype=torch.bfloat16, device=dq_acc_t.device)
+    _check(lib().ringx_dq_finalize_mla(_dev(dq_acc_t, "dq_acc_t"), _dev(dq, "dq"), B, H, Nq, d_qk, _stream()),
+           "ringx_dq_finalize_mla")
+    return dq
 
 
 def ringx_attn_chunk_fwd(q, k, v, scale: float):

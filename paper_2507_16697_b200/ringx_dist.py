@@ -85,6 +85,41 @@ class CudaOps:
         return torch.float32
 
 
+class MlaCudaOps(CudaOps):
+    """The same steps for multi-head latent attention widths (q, k [.,192]; v, o, dO [.,128]): the MLA
+    kernels of libringx.  The fp32 dQ accumulator is kept transposed by the kernel; the schedules only create, pass on and
+    finalize it, so it stays a tensor of q's shape whose layout is the kernel's business."""
+
+    def attn_fwd(self, q, k, v, scale):
+        return self.rx.ringx_attn_fwd_mla(q, k, v, q.shape[2], scale)
+
+    def fwd_scratch(self, q, k):
+        return None
+
+    def chunk_fwd(self, q, k, v, scale, scratch=None):
+        return self.rx.ringx_attn_chunk_fwd_mla(q, k, v, scale)
+
+    def chunk_fwd_fold(self, q, k, v, o_acc, lse_acc, scale, final, scratch=None):
+        return self.rx.ringx_attn_chunk_fwd_mla(q, k, v, scale, o_acc=o_acc, lse_acc=lse_acc, final=final)
+
+    def bwd_scratch(self, q):
+        B, H, Nq, _ = q.shape
+        n = max(256, self.rx.ringx_attn_bwd_partial_mla_workspace_bytes(B, H, Nq))
+        return torch.empty(n, dtype=torch.uint8, device=q.device)
+
+    def bwd_partial(self, q, k, v, o, lse, dO, scale, dq_acc, dk, dv, scratch, prepared):
+        return self.rx.ringx_attn_bwd_partial_mla(q, k, v, o, lse, dO, scale, dq_acc, dk, dv, scratch, prepared=prepared)
+
+    def dq_finalize(self, dq_acc, like):
+        B, H, Nq, d_qk = like.shape
+        return self.rx.ringx_dq_finalize_mla(dq_acc, B, H, Nq, d_qk)
+
+
+def default_ops(q, v):
+    """The CUDA kernel set for these widths: MHA / GQA-free d in {64,128}, or the MLA widths (d_qk != d_v)."""
+    return MlaCudaOps() if q.shape[-1] != v.shape[-1] else CudaOps()
+
+
 class _Done:
     def wait(self):
         return None
@@ -132,7 +167,7 @@ class TorchComm:
 def ringx_b_forward(q, k, v, scale, comm=None, ops=None):
     """All-gather(K,V), then the local chunk loop with the running Eq. 5 merge.
     Returns (o, lse, ctx); ctx keeps the gathered K,V for the backward."""
-    ops = ops or CudaOps()
+    ops = ops or default_ops(q, v)
     comm = comm or TorchComm()
     W, r = comm.world, comm.rank
     if W == 1:
@@ -158,8 +193,8 @@ def ringx_b_forward(q, k, v, scale, comm=None, ops=None):
 def ringx_b_backward(ctx, dO, comm=None, ops=None):
     """Local loop over the gathered chunks (dK_c, dV_c shares; dQ accumulates), then reduce-scatter(dK,dV)
     (PAPER.md:145).  Returns (dq, dk, dv) for the local sequence chunk."""
-    ops = ops or CudaOps()
     q, kg, vg, o, lse, scale = ctx
+    ops = ops or default_ops(q, vg)
     comm = comm or TorchComm()
     W, r = comm.world, comm.rank
     dq_acc = torch.zeros(q.shape, dtype=ops.acc_dtype(q), device=q.device)
@@ -187,7 +222,7 @@ def ringx_a_forward(q, k, v, scale, comm=None, ops=None):
     """Step t: broadcast(Q_t), every rank attends it against its own (K,V) chunk, all-reduce(max) of loc_lse,
     reduce(num, den) to rank t, which forms num/den.  The broadcast for step t+1 is issued
     before step t computes, into the other ping-pong buffer.  Returns (o, lse, ctx)."""
-    ops = ops or CudaOps()
+    ops = ops or default_ops(q, v)
     comm = comm or TorchComm()
     W, r = comm.world, comm.rank
     if W == 1:
@@ -222,8 +257,8 @@ def ringx_a_forward(q, k, v, scale, comm=None, ops=None):
 def ringx_a_backward(ctx, dO, comm=None, ops=None):
     """Step t: broadcast(K_t, V_t); every rank computes its share of dK_t, dV_t from its local Q, dO (reduced to
     rank t) and adds these keys' contribution to its dQ accumulator.  Returns (dq, dk, dv)."""
-    ops = ops or CudaOps()
     q, k, v, o, lse, scale = ctx
+    ops = ops or default_ops(q, v)
     comm = comm or TorchComm()
     W, r = comm.world, comm.rank
     dq_acc = torch.zeros(q.shape, dtype=ops.acc_dtype(q), device=q.device)

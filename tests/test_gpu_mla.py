@@ -233,3 +233,120 @@ def test_mla_backward_errors(rx):
     assert call(192, 128, 256, 256, 1, ws.data_ptr(), 1024) == 5            # WORKSPACE_TOO_SMALL
     assert call(192, 128, 192, 192, 1, ws.data_ptr(), ws.numel()) == 2      # N % 128
     torch.cuda.synchronize()
+
+
+# ------------------------------------------------------------------------------------------------ per-device RingX steps
+def test_mla_chunk_steps_are_the_papers_partials_and_fold(rx):
+    """ringx_attn_chunk_fwd_mla with Nq != Nk: (loc_out, loc_lse) of a key chunk = the oracle's partials of that chunk
+    (PAPER.md:135); folding chunk after chunk (in place, last fold to bf16) = the unchunked attention (Eq. 5)."""
+    B, H, Nq, Nk = 1, 2, 256, 1024
+    q = wl.make_tensor((B, H, Nq, DQK), "q", seed=151, dtype="bf16")
+    k = wl.make_tensor((B, H, Nk, DQK), "k", seed=151, dtype="bf16")
+    v = wl.make_tensor((B, H, Nk, DV), "v", seed=151, dtype="bf16")
+    scale = 1.0 / math.sqrt(DQK)
+    qd, kd, vd = q.cuda(), k.cuda(), v.cuda()
+    bounds = [0, 384, 512, 1024]
+    acc = None
+    for i, (lo, hi) in enumerate(zip(bounds[:-1], bounds[1:])):
+        kc, vc = kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous()
+        if acc is None:
+            acc = rx.ringx_attn_chunk_fwd_mla(qd, kc, vc, scale)
+            for h in range(H):
+                o_ref, l_ref = orc.attention_fwd(f64(q[0, h]), f64(k[0, h, lo:hi]), f64(v[0, h, lo:hi]), scale)
+                assert np.abs(f64(acc[0][0, h]) - o_ref).max() <= 2e-2 * np.abs(o_ref).max()
+                assert np.abs(f64(acc[1][0, h]) - l_ref).max() <= 5e-5
+        elif i < len(bounds) - 2:
+            got = rx.ringx_attn_chunk_fwd_mla(qd, kc, vc, scale, o_acc=acc[0], lse_acc=acc[1])
+            assert got[0].data_ptr() == acc[0].data_ptr()
+        else:
+            keep_o, keep_l = acc[0].clone(), acc[1].clone()
+            o, lse = rx.ringx_attn_chunk_fwd_mla(qd, kc, vc, scale, o_acc=acc[0], lse_acc=acc[1], final=True)
+            assert torch.equal(keep_o, acc[0]) and torch.equal(keep_l, acc[1])
+    assert o.dtype == torch.bfloat16
+    o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+    assert np.linalg.norm(f64(o) - o_ref) / np.linalg.norm(o_ref) <= 1e-2
+    assert np.abs(f64(lse) - lse_ref).max() <= 5e-5
+
+
+def test_mla_bwd_partial_steps_add_up_to_the_gradient(rx):
+    """Two key chunks through ringx_attn_bwd_partial_mla (global LSE; dQ accumulates across the steps in the transposed
+    fp32 accumulator, finalized once): dq = the oracle's, the chunks' dk, dv = the oracle's rows; fp32 shares round to the
+    bf16 result bit for bit; `prepared` reuses D / lse2."""
+    B, H, Nq, Nk = 1, 2, 384, 768
+    q = wl.make_tensor((B, H, Nq, DQK), "q", seed=157, dtype="bf16")
+    k = wl.make_tensor((B, H, Nk, DQK), "k", seed=157, dtype="bf16")
+    v = wl.make_tensor((B, H, Nk, DV), "v", seed=157, dtype="bf16")
+    do = wl.make_tensor((B, H, Nq, DV), "do", seed=157, dtype="bf16")
+    scale = 1.0 / math.sqrt(DQK)
+    q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+    o64, lse64 = orc.attention_fwd_bhnd(q64, k64, v64, scale)
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    o, lse = torch.from_numpy(o64).to(torch.bfloat16).cuda(), torch.from_numpy(lse64).float().cuda()
+    ws = torch.empty(rx.ringx_attn_bwd_partial_mla_workspace_bytes(B, H, Nq), dtype=torch.uint8, device="cuda")
+    acc = torch.zeros((B, H, DQK, Nq), dtype=torch.float32, device="cuda")
+    dk16, dv16 = torch.empty_like(kd), torch.empty_like(vd)
+    dk32 = torch.empty(kd.shape, dtype=torch.float32, device="cuda")
+    dv32 = torch.empty(vd.shape, dtype=torch.float32, device="cuda")
+    for step, (lo, hi) in enumerate(((0, 256), (256, 768))):
+        kc, vc = kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous()
+        a, b = torch.empty_like(kc), torch.empty_like(vc)
+        rx.ringx_attn_bwd_partial_mla(qd, kc, vc, o, lse, dod, scale, acc, a, b, ws, prepared=step > 0)
+        dk16[:, :, lo:hi], dv16[:, :, lo:hi] = a, b
+        a32 = torch.empty(kc.shape, dtype=torch.float32, device="cuda")
+        b32 = torch.empty(vc.shape, dtype=torch.float32, device="cuda")
+        scratch_acc = torch.zeros_like(acc)
+        rx.ringx_attn_bwd_partial_mla(qd, kc, vc, o, lse, dod, scale, scratch_acc, a32, b32, ws, prepared=True)
+        dk32[:, :, lo:hi], dv32[:, :, lo:hi] = a32, b32
+    dq = rx.ringx_dq_finalize_mla(acc, B, H, Nq)
+    assert torch.equal(dk32.to(torch.bfloat16), dk16) and torch.equal(dv32.to(torch.bfloat16), dv16)
+    check_grads(dq, dk16, dv16, q64, k64, v64, do64, scale)
+
+
+@pytest.mark.parametrize("variant", ["a", "b"])
+def test_mla_ringx_schedules_on_simulated_ranks(rx, variant):
+    """RingX_a / RingX_b with the MLA kernels on W = 2 simulated ranks of 256 tokens, forward and
+    backward, against the oracle attention of the whole sequence."""
+    import threading
+    from paper_2507_16697_b200 import ringx_dist
+    from test_gpu_ringx_steps import ThreadComm
+    world, Nl, B, H = 2, 256, 1, 2
+    N = world * Nl
+    scale = 1.0 / math.sqrt(DQK)
+    q, k, v = make(B, H, N, seed=163)
+    do = make_do(B, H, N, seed=163)
+    fwd, bwd = ((ringx_dist.ringx_a_forward, ringx_dist.ringx_a_backward) if variant == "a" else
+                (ringx_dist.ringx_b_forward, ringx_dist.ringx_b_backward))
+    shared = ThreadComm._Shared(world)
+    results, errors = [None] * world, []
+
+    def rank_main(r):
+        try:
+            torch.cuda.set_device(0)
+            comm = ThreadComm(shared, r)
+            sl = slice(r * Nl, (r + 1) * Nl)
+            ql, kl, vl, dol = (t[:, :, sl].contiguous().cuda() for t in (q, k, v, do))
+            o, lse, ctx = fwd(ql, kl, vl, scale, comm=comm)
+            dq, dk, dv = bwd(ctx, dol, comm=comm)
+            torch.cuda.synchronize()
+            results[r] = [t.cpu() for t in (o, lse, dq, dk, dv)]
+        except Exception as e:                      # noqa: BLE001 -- surface it in the main thread
+            errors.append(e)
+            shared.barrier.abort()
+
+    threads = [threading.Thread(target=rank_main, args=(r,)) for r in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+    assert not errors, errors
+    q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+    o_ref, lse_ref = orc.attention_fwd_bhnd(q64, k64, v64, scale)
+    dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
+    rel = lambda a, r: np.linalg.norm(a - r) / np.linalg.norm(r)
+    for r in range(world):
+        sl = slice(r * Nl, (r + 1) * Nl)
+        o, lse, dq, dk, dv = results[r]
+        assert o.shape == (B, H, Nl, DV) and dq.shape == (B, H, Nl, DQK) and dq.dtype == torch.bfloat16
+        assert rel(f64(o), o_ref[:, :, sl]) <= 1e-2 and np.abs(f64(lse) - lse_ref[:, :, sl]).max() <= 5e-5
+        for g, ref in ((dq, dq_ref), (dk, dk_ref), (dv, dv_ref)):
+            assert rel(f64(g), ref[:, :, sl]) <= 8e-3
