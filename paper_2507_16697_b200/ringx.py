@@ -139,6 +139,15 @@ def _dev(t: torch.Tensor, name: str) -> int:
     return t.data_ptr()
 
 
+def _expect(t: torch.Tensor, shape, name: str, dtype=None):
+    """The C ABI takes ONE set of sizes for all its tensors: a tensor of another shape would be read or written out of
+    bounds, so the binding refuses it (argument marshalling, no arithmetic)."""
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name} has shape {tuple(t.shape)}, expected {tuple(shape)}")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"{name} has dtype {t.dtype}, expected {dtype}")
+
+
 def _stream() -> int:
     return torch.cuda.current_stream().cuda_stream
 
@@ -167,6 +176,9 @@ def ringx_attn_fwd(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, works
         o = torch.empty_like(q)
     if lse is None:
         lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    for t, nm in ((k, "k"), (v, "v"), (o, "o")):
+        _expect(t, q.shape, nm, q.dtype)
+    _expect(lse, (B, H, N), "lse", torch.float32)
     need = lib().ringx_attn_fwd_workspace_bytes(B, H, N, d, kv_chunk, dt)
     if workspace is None:
         workspace = _workspace(need, q.device)
@@ -178,6 +190,13 @@ def ringx_attn_fwd(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, works
     return o, lse
 
 
+def _check_mla_shapes(q, k, v, same_len=True):
+    """q [B,H,Nq,192], k [B,H,Nk,192], v [B,H,Nk,128]: the C ABI takes one (B, H) for all three, so they must agree."""
+    if q.dim() != 4 or k.dim() != 4 or v.dim() != 4 or q.shape[:2] != k.shape[:2] or k.shape[:3] != v.shape[:3] \
+            or q.shape[3] != k.shape[3] or (same_len and q.shape[2] != k.shape[2]):
+        raise ValueError(f"MLA shapes do not match: q {tuple(q.shape)}, k {tuple(k.shape)}, v {tuple(v.shape)}")
+
+
 def ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk) -> int:
     return lib().ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
 
@@ -185,12 +204,15 @@ def ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk) -> int:
 def ringx_attn_fwd_mla(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, workspace=None):
     """O, LSE for multi-head latent attention shapes: q, k [B,H,N,192], v [B,H,N,128] bf16 (include/ringx.h:
     ringx_attn_fwd_mla)."""
+    _check_mla_shapes(q, k, v)
     B, H, N, d_qk = q.shape
     d_v = v.shape[3]
     if o is None:
         o = torch.empty((B, H, N, d_v), dtype=q.dtype, device=q.device)
     if lse is None:
         lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    _expect(o, (B, H, N, d_v), "o", q.dtype)
+    _expect(lse, (B, H, N), "lse", torch.float32)
     need = lib().ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
     if workspace is None:
         workspace = _workspace(need, q.device)
@@ -208,11 +230,17 @@ def ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk) -> int:
 def ringx_attn_bwd_mla(q, k, v, o, lse, dO, kv_chunk: int, scale: float, dq=None, dk=None, dv=None, workspace=None):
     """(dq, dk, dv) for multi-head latent attention shapes: q, k [B,H,N,192], v, o, dO [B,H,N,128] bf16 (include/ringx.h:
     ringx_attn_bwd_mla)."""
+    _check_mla_shapes(q, k, v)
     B, H, N, d_qk = q.shape
     d_v = v.shape[3]
     dq = torch.empty_like(q) if dq is None else dq
     dk = torch.empty_like(k) if dk is None else dk
     dv = torch.empty_like(v) if dv is None else dv
+    for t, nm in ((o, "o"), (dO, "dO"), (dv, "dv")):
+        _expect(t, v.shape, nm, q.dtype)
+    for t, nm in ((dq, "dq"), (dk, "dk")):
+        _expect(t, q.shape, nm, q.dtype)
+    _expect(lse, (B, H, N), "lse", torch.float32)
     need = lib().ringx_attn_bwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk)
     if workspace is None:
         workspace = _workspace(max(need, 256), q.device)
@@ -227,6 +255,7 @@ def ringx_attn_chunk_fwd_mla(q, k, v, scale: float, o_acc=None, lse_acc=None, fi
     """One pass of the MLA widths in general form (include/ringx.h: ringx_attn_chunk_fwd_mla): q [B,H,Nq,192] against
     k [B,H,Nk,192], v [B,H,Nk,128].  No accumulator: (loc_out fp32, loc_lse), or (o bf16, lse) when final.  With
     (o_acc, lse_acc): folds this pass in -- in place, or, when final, into a new (o bf16, lse)."""
+    _check_mla_shapes(q, k, v, same_len=False)
     B, H, Nq, d_qk = q.shape
     Nk, d_v = k.shape[2], v.shape[3]
     if (o_acc is None) != (lse_acc is None):
@@ -256,6 +285,7 @@ def ringx_attn_bwd_partial_mla(q, k, v, o, lse, dO, scale: float, dq_acc_t, dk, 
     """The per-device backward step for the MLA widths (include/ringx.h: ringx_attn_bwd_partial_mla).  dq_acc_t holds the
     fp32 dQ accumulator TRANSPOSED, [B,H,192,Nq] (any tensor of B*H*Nq*192 floats: it is opaque until
     ringx_dq_finalize_mla); dk, dv bf16 or float32 shares.  Every buffer is the caller's; returns (dq_acc_t, dk, dv)."""
+    _check_mla_shapes(q, k, v, same_len=False)
     B, H, Nq, d_qk = q.shape
     Nk, d_v = k.shape[2], v.shape[3]
     if dk.dtype != dv.dtype:
@@ -352,6 +382,9 @@ def ringx_attn_bwd(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspace=N
     dq = torch.empty_like(q) if dq is None else dq
     dk = torch.empty_like(k) if dk is None else dk
     dv = torch.empty_like(v) if dv is None else dv
+    for t, nm in ((k, "k"), (v, "v"), (o, "o"), (dO, "dO"), (dq, "dq"), (dk, "dk"), (dv, "dv")):
+        _expect(t, q.shape, nm, q.dtype)
+    _expect(lse, (B, H, N), "lse", torch.float32)
     need = lib().ringx_attn_bwd_workspace_bytes(B, H, N, d, kv_chunk, dt)
     if workspace is None:
         workspace = _workspace(max(need, 256), q.device)
@@ -630,6 +663,10 @@ def ringx_attn_fwd_gqa(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, w
     dt = _DTYPES[q.dtype]
     o = torch.empty_like(q) if o is None else o
     lse = torch.empty((B, Hq, N), dtype=torch.float32, device=q.device) if lse is None else lse
+    _expect(k, (B, Hkv, N, d), "k", q.dtype)
+    _expect(v, (B, Hkv, N, d), "v", q.dtype)
+    _expect(o, q.shape, "o", q.dtype)
+    _expect(lse, (B, Hq, N), "lse", torch.float32)
     need = lib().ringx_attn_fwd_workspace_bytes(B, Hq, N, d, kv_chunk, dt)
     if workspace is None:
         workspace = _workspace(need, q.device)
@@ -647,6 +684,11 @@ def ringx_attn_bwd_gqa(q, k, v, o, lse, dO, kv_chunk: int, scale: float, workspa
     Hkv = k.shape[1]
     dt = _DTYPES[q.dtype]
     dq, dk, dv = torch.empty_like(q), torch.empty_like(k), torch.empty_like(v)
+    _expect(k, (B, Hkv, N, d), "k", q.dtype)
+    _expect(v, (B, Hkv, N, d), "v", q.dtype)
+    for t, nm in ((o, "o"), (dO, "dO")):
+        _expect(t, q.shape, nm, q.dtype)
+    _expect(lse, (B, Hq, N), "lse", torch.float32)
     need = lib().ringx_attn_bwd_workspace_bytes(B, Hq, N, d, kv_chunk, dt)
     if workspace is None:
         workspace = _workspace(max(need, 256), q.device)

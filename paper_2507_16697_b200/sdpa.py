@@ -82,6 +82,8 @@ def ringx_sdpa(query, key, value, attn_mask=None, dropout_p: float = 0.0, is_cau
         raise NotImplementedError("RingX attention is non-causal, unmasked and has no dropout (PAPER.md:174-179)")
     if query.shape[1] != key.shape[1] and not enable_gqa:
         raise ValueError("query and key have different head counts: pass enable_gqa=True")
+    if query.shape[-1] != value.shape[-1] and query.shape[1] != key.shape[1]:
+        raise NotImplementedError("the MLA widths (d_qk != d_v) are built for Hkv == Hq only")
     scale = 1.0 / math.sqrt(query.shape[-1]) if scale is None else float(scale)
     if schedule is not None:
         if schedule not in ("a", "b"):

@@ -132,3 +132,21 @@ def test_product_does_not_import_the_oracle():
         if f.endswith(".py"):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_2507_16697_b200" not in re.sub(r'"""[\s\S]*?"""', "", text), f
+
+
+def test_binding_refuses_tensors_whose_shapes_disagree():
+    """The C ABI takes one set of sizes for all tensors of a call; the binding must refuse a tensor of another shape or
+    dtype BEFORE the call (it would be read or written out of bounds).  Needs no GPU: the check precedes the device check."""
+    import pytest
+    import torch
+    from paper_2507_16697_b200 import ringx
+    q = torch.zeros(1, 2, 256, 64, dtype=torch.bfloat16)
+    with pytest.raises(ValueError, match="k has shape"):
+        ringx.ringx_attn_fwd(q, q[:, :1], q, 256, 0.125)
+    with pytest.raises(ValueError, match="dO has shape"):
+        ringx.ringx_attn_bwd(q, q, q, q, torch.zeros(1, 2, 256), q[:, :, :128], 256, 0.125)
+    with pytest.raises(ValueError, match="lse has dtype"):
+        ringx.ringx_attn_bwd(q, q, q, q, torch.zeros(1, 2, 256, dtype=torch.float64), q, 256, 0.125)
+    qm, vm = torch.zeros(1, 2, 256, 192, dtype=torch.bfloat16), torch.zeros(1, 1, 256, 128, dtype=torch.bfloat16)
+    with pytest.raises(ValueError, match="MLA shapes"):
+        ringx.ringx_attn_fwd_mla(qm, qm, vm, 256, 0.1)
