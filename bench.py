@@ -382,6 +382,15 @@ def main():
                 continue
             extra[name] = side_measure(ringx, wl, wl.CONFIGS[name], dev, oracle_seconds=args.cpu_baseline_seconds / 5.0)
         extra["next_rows"] = next_rows_measure(ringx, wl, dev)
+        if do_bwd:
+            # the workload's backward with ringx_set_deterministic (int32 fixed-point dQ accumulator): context, not the metric
+            ringx.ringx_set_deterministic(True)
+            try:
+                det_ms = timed_loop(lambda: ringx.ringx_attn_bwd(q, k, v, o, lse, dO, cfg.kv_chunk, cfg.scale,
+                                                                 workspace=ws_b), min_seconds=2.0, min_reps=3)
+            finally:
+                ringx.ringx_set_deterministic(False)
+            extra["deterministic_bwd"] = summarise(det_ms, cfg.bwd_flops)
 
     # ---------------------------------------------------------------- CPU baseline: the oracle, bounded sample
     cpu_baseline = None

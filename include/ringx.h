@@ -205,7 +205,7 @@ RINGX_API size_t ringx_attn_chunk_fwd_ex_workspace_bytes(int B, int H, int Nq, i
  *   q, o, dO [B,H,Nq,d] bf16 (in); lse [B,H,Nq] float (in); k, v [B,H,Nk,d] bf16 (in).
  *   dq_acc [B,H,Nq,d] FLOAT, in/out: += sum over the Nk keys of dS_ij K_j (scale included) -- "the gradient
  *          for Q is accumulated ... over N steps"; the caller zeroes it before the first step and casts it
- *          with ringx_dq_finalize after the last.  Summation order is not deterministic.
+ *          with ringx_dq_finalize after the last.  Summation order is not fixed unless ringx_set_deterministic(1).
  *   dk, dv [B,H,Nk,d] bf16 (out): the sums over the Nq query rows given (complete when the caller holds
  *          every query of the head, otherwise one device's share to be reduced across devices).
  *   Nq % 128 == 0, Nk % 128 == 0, d in {64,128}; dtype must be RINGX_BF16.
@@ -335,10 +335,19 @@ RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d,
 /* Bit-reproducible dQ.  By default the per-key-tile contributions to dQ are reduce-added into the fp32
  * accumulator in whatever order the CTAs reach them (fp32 addition is not associative: the last bits of dq may differ from run
  * to run; dk, dv are always bit-reproducible).  With the flag set -- it is process-wide, so that a backward issued from another
- * thread (a framework's autograd worker thread) sees it -- ringx_attn_bwd, ringx_attn_bwd_gqa and ringx_attn_bwd_partial add the
- * contributions to every dQ tile in key-tile order (a ticket counter per tile in the workspace): the same inputs, shapes and
- * kv_chunk give bit-identical dq.  Costs about a third of the backward throughput (the CTAs proceed as a convoy).  The weight
- * gradients of ringx_*_proj_bwd are not covered (split-K partial sums are reduce-added in arbitrary order). */
+ * thread (a framework's autograd worker thread) sees it -- ringx_attn_bwd, ringx_attn_bwd_gqa and ringx_attn_bwd_partial[_ex]
+ * accumulate dQ as int32 FIXED POINT: query row i gets the scale 1.5e9 / (2.03 scale ||dO_i|| max_j||V_j|| max_jc|K_jc|), a
+ * bound on |dQ_ic| that follows from sum_j P_ij = 1 (two extra launches read K, V and dO once), every fp32 tile contribution
+ * is scaled and rounded to an integer, and the reduce-adds are integer adds -- associative, so the same inputs give
+ * bit-identical dq in any arrival order, on any grid, with no ordering between CTAs (about 5 % of the backward throughput at
+ * d = 128, 10 % at d = 64).  Resolution: 2^-30.5 of that bound per contribution; for diffuse attention over very long
+ * sequences, where |dQ| is far below the bound, this is comparable to the final bf16 rounding (measured at B=1 H=8
+ * N=262144 d=128 with iid inputs: rel. Frobenius difference to the fp32 accumulator 1.3e-3), otherwise far below it.
+ * ringx_attn_bwd_partial[_ex] keeps the caller's fp32 dq_acc: the step's contribution is accumulated in an int32 scratch
+ * inside the workspace and added to dq_acc by one element-wise kernel, so a fixed sequence of steps is reproducible; its
+ * workspace query returns the larger size while the flag is set (a call with a workspace sized before the flag was set
+ * returns RINGX_ERR_WORKSPACE_TOO_SMALL).  Not covered: the MLA entries, and the weight gradients of ringx_*_proj_bwd
+ * (split-K partial sums are reduce-added in arbitrary order). */
 RINGX_API int ringx_set_deterministic(int on);
 RINGX_API int ringx_get_deterministic(void);
 

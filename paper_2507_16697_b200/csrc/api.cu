@@ -159,7 +159,8 @@ struct BwdWorkspace {
   float* D = nullptr;        // D_i = dO_i . O_i, [R]
   float* lse2 = nullptr;     // LSE_i * log2(e), [R]
   float* dq_acc = nullptr;   // fp32 dQ accumulator [R,d]
-  int* dq_sem = nullptr;     // [R/128] ticket counters of the deterministic dQ order
+  float* dq_qs = nullptr;    // [R] per-row scales of the fixed-point dQ accumulator (deterministic mode)
+  float* kvmax = nullptr;    // [2*B*H] scratch of launch_dq_fixed_scale
   size_t bytes = 0;
 };
 
@@ -173,8 +174,10 @@ BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
   off += align_up(R * sizeof(float));
   w.dq_acc = reinterpret_cast<float*>(p ? p + off : nullptr);
   off += align_up(R * d * sizeof(float));
-  w.dq_sem = reinterpret_cast<int*>(p ? p + off : nullptr);
-  off += align_up(R / 128 * sizeof(int));
+  w.dq_qs = reinterpret_cast<float*>(p ? p + off : nullptr);
+  off += align_up(R * sizeof(float));
+  w.kvmax = reinterpret_cast<float*>(p ? p + off : nullptr);
+  off += align_up((size_t)B * H * 2 * sizeof(float));
   w.bytes = off;
   return w;
 }
@@ -753,15 +756,23 @@ int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const 
 // q,o,dO,lse: Nq rows per head; k,v,dk,dv: Nk rows per head.  dq_acc fp32 [BH,Nq,d] (zeroed first when zero_dq).
 // `prepared`: D and lse2 already hold this (o, lse, dO)'s values (an earlier step of the same RingX backward wrote them).
 // dkv_dtype: dtype of dk, dv (bf16, or fp32 for one device's share of a cross-device sum).
+// Deterministic mode (ringx_set_deterministic): det.qs != nullptr.  The passes accumulate dQ as int32 fixed point with
+// the per-row scales det.qs (integer reduce-adds: order-independent) into det.fix -- dq_acc itself when the library owns
+// the accumulator (dq_bf16 != nullptr), else a zeroed scratch that is added to the caller's fp32 dq_acc afterwards.
+struct DetScratch {
+  float* qs = nullptr;      // [BH*Nq]
+  float* kvmax = nullptr;   // [2*BH]
+  int* fix = nullptr;       // [BH*Nq*d] int32 (only when the caller owns dq_acc)
+};
+
 static int bwd_core(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
                     float* D, float* lse2, float* dq_acc, bool zero_dq, void* dq_bf16, void* dk, void* dv, int BH,
-                    int Nq, int Nk, int d, int kv_chunk, float scale, int* dq_sem, cudaStream_t stream,
+                    int Nq, int Nk, int d, int kv_chunk, float scale, DetScratch det, cudaStream_t stream,
                     int dkv_dtype = RINGX_BF16, bool prepared = false) {
   const long long R = (long long)BH * Nq;
   cudaError_t e;
-  if (!g_deterministic.load(std::memory_order_relaxed)) dq_sem = nullptr;
-  if (dq_sem && (e = cudaMemsetAsync(dq_sem, 0, (size_t)(R / 128) * sizeof(int), stream)) != cudaSuccess)
-    return cuda_status(e);
+  const bool fixed = g_deterministic.load(std::memory_order_relaxed) != 0;
+  if (fixed && (!det.qs || !det.kvmax || (!dq_bf16 && !det.fix))) return RINGX_ERR_WORKSPACE_TOO_SMALL;
   if (!prepared) {
     {
       Timed timed(RINGX_PROFILE_BWD_AUX, stream);
@@ -770,14 +781,30 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
     count_launch();
     if (e != cudaSuccess) return cuda_status(e);
   }
+  float* pass_acc = dq_acc;
+  if (fixed) {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    if (!dq_bf16) {
+      pass_acc = reinterpret_cast<float*>(det.fix);
+      if ((e = cudaMemsetAsync(det.fix, 0, (size_t)R * d * sizeof(int), stream)) != cudaSuccess) return cuda_status(e);
+    }
+    e = launch_dq_fixed_scale(k, v, dO, det.kvmax, det.qs, BH, Nq, Nk, 0, Nk, d, scale, stream);
+    count_launch(2);
+    if (e != cudaSuccess) return cuda_status(e);
+  }
   for (int c = 0; c < Nk / kv_chunk; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
-    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, dq_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, kv_chunk, d, scale,
-                                    dq_sem, dkv_dtype, stream);
+    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, pass_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, kv_chunk, d, scale,
+                                    fixed ? det.qs : nullptr, dkv_dtype, stream);
     if (e != cudaSuccess) return cuda_status(e);
     if (tl_hooks.pass_done && (e = cudaEventRecord(tl_hooks.pass_done[c], stream)) != cudaSuccess) return cuda_status(e);
   }
-  if (dq_bf16) {
+  if (fixed) {
+    Timed timed(RINGX_PROFILE_BWD_AUX, stream);
+    e = launch_dq_fixed_finish(reinterpret_cast<const int*>(pass_acc), det.qs, dq_bf16, dq_acc, R, d, stream);
+    count_launch();
+    if (e != cudaSuccess) return cuda_status(e);
+  } else if (dq_bf16) {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
     e = launch_dq_convert(dq_acc, dq_bf16, R * d, 1.0f, stream);
     count_launch();
@@ -808,8 +835,11 @@ int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, const void* 
   // the G = Hq/Hkv query heads of a kv head are G*N adjacent query rows: the CTA that owns a key tile walks all of them,
   // so dK, dV of the kv head are still written once, atomic-free
   const int G = Hq / Hkv;
+  DetScratch det;
+  det.qs = w.dq_qs;
+  det.kvmax = w.kvmax;
   st = bwd_core(q, k, v, o, lse, dO, w.D, w.lse2, w.dq_acc, true, dq, dk, dv, B * Hkv, G * N, N, d, kv_chunk, scale,
-                w.dq_sem, stream);
+                det, stream);
   if (st != RINGX_OK) return st;
   tl_last_launches = tl_launches;
   return RINGX_OK;
@@ -825,7 +855,11 @@ int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, c
 size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d) {
   if (B <= 0 || H <= 0 || Nq <= 0 || (d != 64 && d != 128)) return 0;
   const size_t R = (size_t)B * H * Nq;
-  return 2 * align_up(R * sizeof(float)) + align_up(R / 128 * sizeof(int));
+  size_t bytes = 2 * align_up(R * sizeof(float));
+  // deterministic mode: per-row scales, the K/V maxima and an int32 fixed-point image of this step's dQ contribution
+  if (g_deterministic.load(std::memory_order_relaxed))
+    bytes += align_up(R * sizeof(float)) + align_up((size_t)B * H * 2 * sizeof(float)) + align_up(R * d * sizeof(int));
+  return bytes;
 }
 
 int ringx_attn_bwd_partial_ex(const void* q, const void* k, const void* v, const void* o, const float* lse,
@@ -854,8 +888,14 @@ int ringx_attn_bwd_partial_ex(const void* q, const void* k, const void* v, const
   float* D = static_cast<float*>(workspace);
   const size_t rb = align_up((size_t)B * H * Nq * sizeof(float));
   float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + rb);
-  int* dq_sem = reinterpret_cast<int*>(static_cast<char*>(workspace) + 2 * rb);
-  st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, dq_sem, stream,
+  DetScratch det;
+  if (need > 2 * rb) {      // the workspace was sized in deterministic mode
+    char* p = static_cast<char*>(workspace) + 2 * rb;
+    det.qs = reinterpret_cast<float*>(p);
+    det.kvmax = reinterpret_cast<float*>(p + rb);
+    det.fix = reinterpret_cast<int*>(p + rb + align_up((size_t)B * H * 2 * sizeof(float)));
+  }
+  st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, det, stream,
                 dkv_dtype, prepared != 0);
   if (st != RINGX_OK) return st;
   tl_last_launches = tl_launches;

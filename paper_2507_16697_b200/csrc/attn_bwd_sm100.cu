@@ -70,7 +70,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
                       const __grid_constant__ CUtensorMap map_dq, const float* __restrict__ lse2,
                       const float* __restrict__ Dvec,
                       void* __restrict__ dk, void* __restrict__ dv, int dkv_f32, int N, int nk_stride, int k_off,
-                      float scale_log2, float scale, int* __restrict__ dq_sem, unsigned* __restrict__ smem_probe) {
+                      float scale_log2, float scale, const float* __restrict__ dq_qs, unsigned* __restrict__ smem_probe) {
   using Cfg = BwdCfg<kD>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   // d = 128 uses every byte of the 227 KB, so it cannot round the base up: the launcher proves the alignment of this
@@ -466,14 +466,17 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     const int row = (warp & 3) * 32 + lane;                      // query row of the tile = TMEM lane
     const uint32_t tDQ = tmem + Cfg::tDQ + (static_cast<uint32_t>((warp & 3) * 32) << 16);
     const bool leader = warp == 8 && elect_one();
-    // Deterministic mode (dq_sem != nullptr): the reduce-adds into one dQ tile are issued in key-tile order.  Tile
-    // (head, i) has a ticket counter; the CTA of key tile t (counted over the whole call, k_off included) waits for
-    // ticket t, issues its reduce, and once the reduce has been performed sets the ticket to t + 1.  CTAs are
-    // dispatched in block-index order, so the owner of ticket t is always resident or finished when t + 1 waits.
-    const int ticket = k_off / kTile + blockIdx.x;
-    int* sem = dq_sem ? dq_sem + bh * n_q : nullptr;
+    // Deterministic mode (dq_qs != nullptr): dq_acc is an int32 fixed-point accumulator.  Row r of the head carries a
+    // scale dq_qs[r] chosen from a bound on |dQ_r| (launch_dq_fixed_scale), every fp32 partial is scaled and rounded
+    // to an integer here, and the TMA reduce-adds are integer adds: associative, so the sum does
+    // not depend on the order in which the CTAs' adds arrive -- bit-reproducible dQ with no ordering between CTAs.
+    const bool fixed = dq_qs != nullptr;
+    const float* qs_row = fixed ? dq_qs + q_row0 + row : nullptr;
+    float qs_next = fixed ? __ldg(qs_row) : 1.f;
     int buf = 0;
     for (int i = 0; i < n_q; ++i) {
+      const float qs = qs_next;
+      if (fixed && i + 1 < n_q) qs_next = __ldg(qs_row + (i + 1) * kTile);   // ahead of the wait: latency hidden
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
 
@@ -488,6 +491,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           tc_fence_before();
           mbar_arrive(dq_empty);             // the whole dQ(i) row has left TMEM: hand the columns back
         }
+        if (fixed) {
+#pragma unroll
+          for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int e = 0; e < 32; ++e)
+              r[c][e] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][e]) * qs));
+        }
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
           if (leader) tma_wait_group_read<1>();      // the reduce that last read this panel has finished reading
@@ -499,31 +509,14 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           fence_proxy_async_smem();
           named_bar_sync(2, 128);
           if (leader) {
-            if (sem && rd == 0 && c == 0) {      // my turn to add into dQ tile i?
-              while (ld_acquire_gpu(sem + i) != ticket) __nanosleep(32);
-              fence_proxy_async_all();
-            }
             tma_reduce_add_2d(&map_dq, sDq + buf * Cfg::kDqPanelBytes, rd * 64 + c * 32, q_row0 + i * kTile);
             tma_commit_group();
           }
           buf ^= 1;
         }
       }
-      if (sem && leader && i > 0) {
-        // the reduce-adds of tile i-1 (every bulk group but the kD/32 just committed) have been performed: pass its
-        // ticket on.  Releasing one step late keeps the completion latency off this warp's critical path.
-        tma_wait_group<kD / 32>();
-        __threadfence();
-        st_release_gpu(sem + i - 1, ticket + 1);
-      }
     }
-    if (leader) {
-      tma_wait_group<0>();
-      if (sem) {
-        __threadfence();
-        st_release_gpu(sem + n_q - 1, ticket + 1);
-      }
-    }
+    if (leader) tma_wait_group<0>();
     __syncwarp();
   } else {
     setmaxnreg_dec<kBwdAuxRegs>();   // warps 14-15: release their registers
@@ -537,7 +530,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
 template <int kD>
 cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
                      const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int dkv_f32, int BH,
-                     int N, int nk_stride, int k_off, int nk, float scale, int* dq_sem, cudaStream_t stream) {
+                     int N, int nk_stride, int k_off, int nk, float scale, const float* dq_qs, cudaStream_t stream) {
   using Cfg = BwdCfg<kD>;
   auto kern = attn_chunk_bwd_kernel<kD>;
   static unsigned char configured[kMaxDevices];
@@ -566,7 +559,7 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
   }
   dim3 grid(nk / kTile, BH);
   kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, N, nk_stride, k_off,
-                                                       scale * 1.4426950408889634f, scale, dq_sem, nullptr);
+                                                       scale * 1.4426950408889634f, scale, dq_qs, nullptr);
   count_launch();
   return cudaGetLastError();
 }
@@ -575,7 +568,7 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
 
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
-                                        int nk_stride, int k_off, int nk, int d, float scale, int* dq_sem,
+                                        int nk_stride, int k_off, int nk, int d, float scale, const float* dq_qs,
                                         int dkv_dtype, cudaStream_t stream) {
   CUtensorMap mq, mk, mv, mdo, mdq;
   const int dkv_f32 = dkv_dtype == RINGX_F32;
@@ -585,10 +578,11 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
       !make_tmap_2d(&mk, k, dt, 2, krows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mv, v, dt, 2, krows, d, 128, 64, kSwizzle128B) ||
       !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mdq, dq_acc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, rows, d, 128, 32, kSwizzle128B))
+      !make_tmap_2d(&mdq, dq_acc, dq_qs ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, rows, d, 128, 32,
+                    kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
-  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_sem, stream);
+  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_qs, stream);
+  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_qs, stream);
 }
 
 }  // namespace ringx

@@ -32,6 +32,15 @@ cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* ls
                                   float* dq_acc, long long rows, int d, float scale, bool zero_dq,
                                   cudaStream_t stream);
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
+// Deterministic dQ (int32 fixed-point accumulator, merge.cu).  launch_dq_fixed_scale: kvmax [2*BH] (scratch) and the
+// per-row scales qs [BH*rows_per_head] from k, v rows [k_off, k_off+nk) of every head and dO
+// (2 launches + a memset).  launch_dq_fixed_finish: dq_bf16 = dq_fix / qs (dq_bf16 != nullptr), else dq_acc += dq_fix / qs
+// (1 launch).
+cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, float* kvmax, float* qs, int BH,
+                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d, float scale,
+                                  cudaStream_t stream);
+cudaError_t launch_dq_fixed_finish(const int* dq_fix, const float* qs, void* dq_bf16, float* dq_acc, long long rows, int d,
+                                   cudaStream_t stream);
 
 // ---- fidelity.cu (the Turbulence-Transformer tokeniser): crop + k^3 Gaussian filter, stride k.
 // y [M,D,H,W,4] fp32 -> tokens [M,Dc/k,Hc/k,Wc/k,4] (f32 or bf16); w = k normalised 1-D weights (host array).
@@ -92,12 +101,12 @@ cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int
 // [k_off, k_off+nk) of every head (bf16, the sum over the N query rows given), reduce-adds these keys'
 // contribution to dQ into dq_acc (fp32 [BH,N,d]).
 // lse2 = LSE * log2(e) and D = scale * rowsum(dO*O) come from launch_bwd_preprocess.
-// dq_sem: nullptr, or [BH * N/128] ticket counters (zero before the first pass of a call) that make the order of the
-// reduce-adds into every dQ tile the key-tile order (bit-reproducible dQ).
+// dq_qs: nullptr, or [BH * N] per-row scales (launch_dq_fixed_scale): dq_acc is then an int32 fixed-point
+// accumulator and the reduce-adds are integer adds -- bit-reproducible dQ in any arrival order.
 // dkv_dtype: RINGX_BF16 (dk, dv bf16) or RINGX_F32 (fp32: one device's share of a cross-device sum).
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
-                                        int nk_stride, int k_off, int nk, int d, float scale, int* dq_sem,
+                                        int nk_stride, int k_off, int nk, int d, float scale, const float* dq_qs,
                                         int dkv_dtype, cudaStream_t stream);
 
 // ---- tensor maps (api.cu): 2-D row-major [rows, cols] view, box = {box_cols, box_rows}

@@ -292,6 +292,119 @@ dq_convert_kernel(const float4* __restrict__ dq_acc, uint2* __restrict__ dq, lon
   }
 }
 
+// ---------------------------------------------------------------- deterministic dQ: int32 fixed-point accumulator
+// (ringx_set_deterministic).  Integer adds are associative, so TMA reduce-adds of integers give the same sum in any
+// arrival order.  Row r gets a scale qs[r] with |dQ_rc| * qs[r] <= 1.5e9 < 2^31 guaranteed by
+//   |dQ_rc| = scale |sum_j P_rj (dP_rj - D_r) K_jc| <= scale * 2 max_j|dO_r.V_j| * max_j|K_jc|      (sum_j P_rj = 1,
+//                                                 <= 2 scale ||dO_r|| max_j||V_j|| max_jc|K_jc|      D_r in the hull of dP_rj)
+// (the partial sums may wrap: two's-complement adds are exact modulo 2^32, only the final value has to fit).
+
+// kvmax[2h] = max_j ||V_j||^2, kvmax[2h+1] = max_jc |K_jc| over the nk key rows [k_off, k_off+nk) of kv head h
+// (atomicMax on the bit patterns of non-negative floats: order-independent).  grid = (blocks, BH); kvmax zeroed before.
+template <int kLanes>
+__global__ void __launch_bounds__(256)
+kv_absmax_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v, unsigned* __restrict__ kvmax, int nk_stride,
+                 int k_off, int nk) {
+  constexpr int kRowsPerWarp = 32 / kLanes;
+  const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
+  const int bh = blockIdx.y;
+  const long long head0 = (long long)bh * nk_stride + k_off;
+  float vmax2 = 0.f, kmax = 0.f;
+  for (int base = (blockIdx.x * 8 + (threadIdx.x >> 5)) * kRowsPerWarp; base < nk; base += gridDim.x * 8 * kRowsPerWarp) {
+    const int r = base + sub;      // nk % 128 == 0: every lane has a row
+    const uint4 a = __ldg(k + (head0 + r) * kLanes + l);
+    const uint4 b = __ldg(v + (head0 + r) * kLanes + l);
+    const uint32_t* pa = reinterpret_cast<const uint32_t*>(&a);
+    const uint32_t* pb = reinterpret_cast<const uint32_t*>(&b);
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float v0 = __uint_as_float(pb[i] << 16), v1 = __uint_as_float(pb[i] & 0xFFFF0000u);
+      s = fmaf(v0, v0, s);
+      s = fmaf(v1, v1, s);
+      kmax = fmaxf(kmax, fmaxf(fabsf(__uint_as_float(pa[i] << 16)), fabsf(__uint_as_float(pa[i] & 0xFFFF0000u))));
+    }
+#pragma unroll
+    for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    vmax2 = fmaxf(vmax2, s);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    vmax2 = fmaxf(vmax2, __shfl_xor_sync(0xffffffffu, vmax2, off));
+    kmax = fmaxf(kmax, __shfl_xor_sync(0xffffffffu, kmax, off));
+  }
+  if (lane == 0) {
+    atomicMax(kvmax + 2 * bh, __float_as_uint(vmax2));
+    atomicMax(kvmax + 2 * bh + 1, __float_as_uint(kmax));
+  }
+}
+
+// qs[r] = 1.5e9 / bound_r (clamped to [2^-100, 2^100]), bound_r = 2.03125 * scale * ||dO_r|| * sqrt(kvmax[2h]) * kvmax[2h+1],
+// h = r / rows_per_head.  The 2.03125 covers the bf16 roundings of O (in D_r) and of dS and a row sum of P up to 1.001;
+// 1.5e9 + one rounding of 1/2 per key tile stays below 2^31.
+template <int kLanes>
+__global__ void __launch_bounds__(256)
+dq_fixed_scale_kernel(const uint4* __restrict__ dO, const float* __restrict__ kvmax, float* __restrict__ qs,
+                      long long rows, long long rows_per_head, float scale) {
+  constexpr int kRowsPerWarp = 32 / kLanes;
+  const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
+  const long long warp_global = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const long long warp_count = (long long)gridDim.x * 8;
+  for (long long base = warp_global * kRowsPerWarp; base < rows; base += warp_count * kRowsPerWarp) {
+    const long long r = base + sub;
+    float s = 0.f;
+    if (r < rows) {
+      const uint4 b = __ldg(dO + r * kLanes + l);
+      const uint32_t* pb = reinterpret_cast<const uint32_t*>(&b);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float v0 = __uint_as_float(pb[i] << 16), v1 = __uint_as_float(pb[i] & 0xFFFF0000u);
+        s = fmaf(v0, v0, s);
+        s = fmaf(v1, v1, s);
+      }
+    }
+#pragma unroll
+    for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    if (r < rows && l == 0) {
+      const long long h = r / rows_per_head;
+      const float bound = 2.03125f * scale * sqrtf(s) * sqrtf(kvmax[2 * h]) * kvmax[2 * h + 1];
+      qs[r] = fminf(fmaxf(1.5e9f / fmaxf(bound, 1e-37f), 7.8886e-31f), 1.2676506e30f);
+    }
+  }
+}
+
+// dq (bf16) = dq_fix / qs[row], vecs = d / 4 int4 per row
+__global__ void __launch_bounds__(256)
+dq_fixed_convert_kernel(const int4* __restrict__ dq_fix, const float* __restrict__ qs, uint2* __restrict__ dq,
+                        long long n4, int vecs) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+    const int4 v = __ldcs(dq_fix + i);
+    const float inv = 1.0f / __ldg(qs + i / vecs);
+    uint2 u;
+    u.x = ptx::pack_bf16x2(static_cast<float>(v.x) * inv, static_cast<float>(v.y) * inv);
+    u.y = ptx::pack_bf16x2(static_cast<float>(v.z) * inv, static_cast<float>(v.w) * inv);
+    dq[i] = u;
+  }
+}
+
+// dq_acc (fp32, the caller's accumulator across the steps of a RingX backward) += dq_fix / qs[row]
+__global__ void __launch_bounds__(256)
+dq_fixed_accumulate_kernel(const int4* __restrict__ dq_fix, const float* __restrict__ qs, float4* __restrict__ dq_acc,
+                           long long n4, int vecs) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+    const int4 v = __ldcs(dq_fix + i);
+    const float inv = 1.0f / __ldg(qs + i / vecs);
+    float4 a = dq_acc[i];
+    a.x += static_cast<float>(v.x) * inv;
+    a.y += static_cast<float>(v.y) * inv;
+    a.z += static_cast<float>(v.z) * inv;
+    a.w += static_cast<float>(v.w) * inv;
+    dq_acc[i] = a;
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_lse_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b, void* o_out,
@@ -369,6 +482,42 @@ cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float 
   long long blocks = (n4 + 255) / 256;
   if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
   dq_convert_kernel<<<(unsigned)blocks, 256, 0, stream>>>((const float4*)dq_acc, (uint2*)dq, n4, scale);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, float* kvmax, float* qs, int BH,
+                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d, float scale,
+                                  cudaStream_t stream) {
+  cudaError_t e = cudaMemsetAsync(kvmax, 0, (size_t)BH * 2 * sizeof(float), stream);
+  if (e != cudaSuccess) return e;
+  const int lanes = d / 8;   // 8 or 16
+  const int rows_per_block = 8 * (32 / lanes);
+  int bx = (nk + rows_per_block - 1) / rows_per_block;
+  const int cap = (sm_count() * 8 + BH - 1) / BH;
+  if (bx > cap) bx = cap;
+  const dim3 grid((unsigned)bx, (unsigned)BH);
+  const long long rows = (long long)BH * rows_per_head;
+  long long blocks = (rows + rows_per_block - 1) / rows_per_block;
+  if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
+  if (lanes == 8) {
+    kv_absmax_kernel<8><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk);
+    dq_fixed_scale_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, qs, rows, rows_per_head, scale);
+  } else {
+    kv_absmax_kernel<16><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk);
+    dq_fixed_scale_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, qs, rows, rows_per_head, scale);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_dq_fixed_finish(const int* dq_fix, const float* qs, void* dq_bf16, float* dq_acc, long long rows, int d,
+                                   cudaStream_t stream) {
+  const long long n4 = rows * d / 4;
+  long long blocks = (n4 + 255) / 256;
+  if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
+  if (dq_bf16)
+    dq_fixed_convert_kernel<<<(unsigned)blocks, 256, 0, stream>>>((const int4*)dq_fix, qs, (uint2*)dq_bf16, n4, d / 4);
+  else
+    dq_fixed_accumulate_kernel<<<(unsigned)blocks, 256, 0, stream>>>((const int4*)dq_fix, qs, (float4*)dq_acc, n4, d / 4);
   return cudaGetLastError();
 }
 

@@ -65,7 +65,7 @@ class CudaOps:
     def eq5_finalize(self, num, den, lse_max, out_dtype):
         return self.rx.ringx_eq5_finalize(num, den, lse_max, out_dtype=out_dtype)
 
-    def bwd_scratch(self, q):                                 # D, lse2 (+ tickets) of one backward: allocated once
+    def bwd_scratch(self, q):                                 # D, lse2 (+ fixed-point scratch in deterministic mode): allocated once
         B, H, Nq, d = q.shape
         n = max(256, self.rx.ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d))
         return torch.empty(n, dtype=torch.uint8, device=q.device)

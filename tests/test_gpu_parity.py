@@ -494,8 +494,9 @@ def test_fwd_bwd_host_entry_matches_device_entries(rx, B, H, N, d, chunk):
 # ------------------------------------------------------------------------------------------------ deterministic dQ
 @pytest.mark.parametrize("B,H,N,d,chunk", [(1, 2, 4096, 128, 1024), (2, 3, 2048, 64, 512)])
 def test_deterministic_mode_gives_bit_identical_dq(rx, B, H, N, d, chunk):
-    """NEXT-2: with ringx_set_deterministic(1) the contributions to every dQ tile are added in key-tile order, so
-    repeated runs agree bit for bit (dk, dv always do); the result still matches the oracle."""
+    """NEXT-2: with ringx_set_deterministic(1) dQ is accumulated as int32 fixed point (integer adds are associative), so
+    repeated runs agree bit for bit whatever order the CTAs' reduce-adds arrive in (dk, dv always do); the result still
+    matches the oracle."""
     scale = 1.0 / math.sqrt(d)
     q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=77, dtype="bf16")
     qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
@@ -545,9 +546,10 @@ print("MULTIWAVE_DET_OK", B * H * (chunk // 128), "CTAs per pass")
 
 @pytest.mark.parametrize("shape", [(1, 8, 16384, 128, 16384), (2, 8, 8192, 64, 4096), (1, 8, 16384, 128, 4096)])
 def test_deterministic_mode_multi_wave_grid(rx, shape):
-    """The ticket protocol's no-deadlock argument is "CTAs are dispatched in block-index order" -- it only matters when
-    the grid exceeds the 148 resident CTAs.  1024 / 512 / 256 CTAs per pass (7 / 3.5 / 1.7 waves), three runs,
-    bit-identical dq; run in a child process with a timeout so that a deadlock FAILS instead of hanging the suite."""
+    """Deterministic mode on grids of several waves -- 1024 / 512 / 256 CTAs per pass (7 / 3.5 / 1.7 waves of the 148
+    resident CTAs), where the arrival order of the reduce-adds into a dQ tile differs from run to run: three runs,
+    bit-identical dq, dk/dv identical to the default mode's.  (Run in a child process with a timeout: the first
+    implementation ordered the adds with tickets and could have deadlocked; the fixed-point accumulator cannot.)"""
     import os
     import subprocess
     import sys
@@ -556,8 +558,42 @@ def test_deterministic_mode_multi_wave_grid(rx, shape):
     try:
         r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300)
     except subprocess.TimeoutExpired:
-        pytest.fail("deterministic-dQ backward did not finish in 300 s on a multi-wave grid (ticket deadlock?)")
+        pytest.fail("deterministic-dQ backward did not finish in 300 s on a multi-wave grid")
     assert r.returncode == 0 and "MULTIWAVE_DET_OK" in r.stdout, (r.stdout[-2000:], r.stderr[-2000:])
+
+
+def test_deterministic_mode_at_half_of_its_overflow_bound(rx):
+    """The fixed-point scale of row i comes from |dQ_ic| <= 2 scale ||dO_i|| max_j||V_j|| max_jc|K_jc|.  Inputs that reach
+    HALF of that bound (the factor 2 is |dP_ij - D_i| <= 2 max|dP|; with D_i = 0 one of the two is left): Q = 0, so P is
+    uniform; keys are +kvec / -kvec with values +vvec / -vvec, so dP_ij = +-(dO_i . vvec), D_i = 0 and
+    dQ_i = scale (dO_i . vvec) kvec; dO_i parallel to vvec makes Cauchy-Schwarz tight.  The int32 accumulator must hold
+    2^29.5 without wrapping and the result must match the oracle to bf16 accuracy."""
+    B, H, N, d, chunk = 1, 2, 2048, 128, 512
+    scale = 1.0 / math.sqrt(d)
+    g = torch.Generator().manual_seed(5)
+    kvec = torch.randn(d, generator=g).to(torch.bfloat16)
+    vvec = torch.randn(d, generator=g).to(torch.bfloat16)
+    sign = torch.where(torch.arange(N) % 2 == 0, 1.0, -1.0).view(1, 1, N, 1)
+    k = (sign * kvec.float()).expand(B, H, N, d).to(torch.bfloat16).contiguous()
+    v = (sign * vvec.float()).expand(B, H, N, d).to(torch.bfloat16).contiguous()
+    q = torch.zeros(B, H, N, d, dtype=torch.bfloat16)
+    amp = torch.linspace(0.25, 4.0, N).view(1, 1, N, 1)           # rows of very different ||dO_i||
+    do = (amp * vvec.float()).expand(B, H, N, d).to(torch.bfloat16).contiguous()
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
+    rx.ringx_set_deterministic(True)
+    try:
+        dq, dk, dv = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale)
+        torch.cuda.synchronize()
+    finally:
+        rx.ringx_set_deterministic(False)
+    q64, k64, v64, do64 = (wl.to_f64_numpy(t) for t in (q, k, v, do))
+    dq_ref, _, _ = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
+    bound = 2 * scale * np.linalg.norm(do64, axis=-1, keepdims=True) * np.linalg.norm(v64[0, 0, 0]) * np.abs(k64).max()
+    assert (np.abs(dq_ref) / bound).max() >= 0.45                 # the inputs do reach half of the bound
+    got = dq.float().cpu().numpy()
+    assert np.abs(got - dq_ref).max() <= 2.0 ** -7 * np.abs(dq_ref).max()
+    assert np.linalg.norm(got - dq_ref) / np.linalg.norm(dq_ref) <= 5e-3
 
 
 # ------------------------------------------------------------------------------------------------ CUDA graphs

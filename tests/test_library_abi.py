@@ -78,7 +78,9 @@ def test_workspace_queries_are_host_only(lib):
     assert f(1, 1, 1024, 64, 384, 1) == 0                         # N % kv_chunk != 0
     assert f(1, 1, 384, 64, 128, 1) == 0                          # bf16 needs N % 256 == 0
     b = lib.ringx_attn_bwd_workspace_bytes
-    assert b(2, 4, 1024, 64, 256, 1) == 2 * R * 4 + R * 64 * 4 + 256   # D, lse2, fp32 dQ accumulator, R/128 dQ tickets
+    # D, lse2, the dQ accumulator (fp32, or int32 fixed point in deterministic mode), the per-row fixed-point scales
+    # and the two K/V maxima per head
+    assert b(2, 4, 1024, 64, 256, 1) == 3 * R * 4 + R * 64 * 4 + 256
     assert b(2, 4, 1024, 64, 256, 0) == 0                         # backward is bf16 only
     h = lib.ringx_attn_fwd_host_workspace_bytes
     assert h(2, 4, 1024, d, 256, 1) == 4 * R * d * 2 + R * 4 + f(2, 4, 1024, d, 256, 1)
