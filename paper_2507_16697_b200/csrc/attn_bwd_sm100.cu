@@ -91,11 +91,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   uint64_t* kv_full = bars;          // TMA -> MMA: K_j, V_j
   uint64_t* s_full = bars + 1;       // MMA -> compute: S^T(i)
   uint64_t* dp_full = bars + 2;      // MMA -> compute: dP^T(i)
-  uint64_t* p_full = bars + 3;       // compute -> MMA: P^T(i) in TMEM, S^T(i) consumed            (256 arrivals)
-  uint64_t* ds_full = bars + 4;      // compute -> MMA: dS^T(i) in smem, dP^T(i) consumed          (256 arrivals)
+  uint64_t* p_full = bars + 3;       // compute -> MMA: P^T(i) in TMEM, S^T(i) consumed            (8 arrivals: one per warp)
+  uint64_t* ds_full = bars + 4;      // compute -> MMA: dS^T(i) in smem, dP^T(i) consumed          (8 arrivals)
   uint64_t* ds_empty = bars + 5;     // MMA -> compute: dK(i), dQ(i) have read dS^T(i)
   uint64_t* dq_full = bars + 6;      // MMA -> drain: dQ(i) in TMEM
-  uint64_t* dq_empty = bars + 7;     // drain -> MMA: dQ(i) in registers                            (128 arrivals)
+  uint64_t* dq_empty = bars + 7;     // drain -> MMA: dQ(i) in registers                            (4 arrivals)
   uint64_t* dkv_full = bars + 8;     // MMA -> compute: dK_j, dV_j complete
   uint64_t* q_full = bars + 9;       // [kQStages] TMA -> MMA, compute
   uint64_t* q_empty = q_full + Cfg::kQStages;
@@ -115,11 +115,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     mbar_init(kv_full, 1);
     mbar_init(s_full, 1);
     mbar_init(dp_full, 1);
-    mbar_init(p_full, 256);
-    mbar_init(ds_full, 256);
+    mbar_init(p_full, 8);
+    mbar_init(ds_full, 8);
     mbar_init(ds_empty, 1);
     mbar_init(dq_full, 1);
-    mbar_init(dq_empty, 128);
+    mbar_init(dq_empty, 4);
     mbar_init(dkv_full, 1);
     mbar_init(kv_tmem_full, 256);
     for (int i = 0; i < Cfg::kQStages; ++i) {
@@ -378,7 +378,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       }
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(p_full);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(p_full);          // one arrival per warp (8): 256 separate arrivals are 256 shared-memory atomics
       // ---- phase B: dS^T = P^T o (dP^T - D), bf16, to shared memory [keys][queries] (128B-swizzled rows)
       mbar_wait(dp_full, i & 1);
       if (i > 0) mbar_wait(ds_empty, (i - 1) & 1);
@@ -423,7 +424,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       fence_proxy_async_smem();
       if (Cfg::kTmemOperands) tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(ds_full);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ds_full);
     }
     // ---- epilogue: dV_j (warps 0-3) and dK_j (warps 4-7), bf16, written once
     mbar_wait(dkv_full, 0);
@@ -489,7 +491,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         for (int c = 0; c < 2; ++c) tmem_wait_ld_x32(r[c]);
         if (rd == kD / 64 - 1) {
           tc_fence_before();
-          mbar_arrive(dq_empty);             // the whole dQ(i) row has left TMEM: hand the columns back
+          __syncwarp();
+          if (lane == 0) mbar_arrive(dq_empty);   // the whole dQ(i) tile has left TMEM: hand the columns back
         }
         if (fixed) {
 #pragma unroll
