@@ -128,7 +128,8 @@ RINGX_API size_t ringx_attn_fwd_mla_workspace_bytes(int B, int H, int N, int d_q
  *   q, k, dq, dk [B,H,N,d_qk] bf16; v, o, dO, dv [B,H,N,d_v] bf16; lse [B,H,N] float (from ringx_attn_fwd_mla).
  *   Outputs must not alias inputs.  Domain: d_qk == 192, d_v == 128, RINGX_BF16, N % 128 == 0, kv_chunk % 128 == 0,
  *   N % kv_chunk == 0.  workspace >= ringx_attn_bwd_mla_workspace_bytes(...) bytes, 256-byte aligned (D, LSE*log2e and
- *   the fp32 dq accumulator, which the kernel keeps transposed, [B,H,d_qk,N]).  ringx_set_deterministic has no effect here. */
+ *   the fp32 dq accumulator, which the kernel keeps transposed, [B,H,d_qk,N]; + the fixed-point scales of
+ *   ringx_set_deterministic, which applies here as it does to ringx_attn_bwd). */
 RINGX_API int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* o, const float* lse,
                        const void* dO, void* dq, void* dk, void* dv,
                        int B, int H, int N, int d_qk, int d_v, int kv_chunk, float scale, int dtype,
@@ -346,7 +347,8 @@ RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d,
  * ringx_attn_bwd_partial[_ex] keeps the caller's fp32 dq_acc: the step's contribution is accumulated in an int32 scratch
  * inside the workspace and added to dq_acc by one element-wise kernel, so a fixed sequence of steps is reproducible; its
  * workspace query returns the larger size while the flag is set (a call with a workspace sized before the flag was set
- * returns RINGX_ERR_WORKSPACE_TOO_SMALL).  Not covered: the MLA entries, and the weight gradients of ringx_*_proj_bwd
+ * returns RINGX_ERR_WORKSPACE_TOO_SMALL).  ringx_attn_bwd_mla is covered in the same way (per-query scales on the transposed
+ * accumulator).  Not covered: ringx_attn_bwd_partial_mla, and the weight gradients of ringx_*_proj_bwd
  * (split-K partial sums are reduce-added in arbitrary order). */
 RINGX_API int ringx_set_deterministic(int on);
 RINGX_API int ringx_get_deterministic(void);

@@ -484,7 +484,8 @@ int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, flo
 size_t ringx_attn_bwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk) {
   if (d_qk != 192 || d_v != 128 || check_shape(B, H, N, d_v, kv_chunk, 1.f, RINGX_BF16, true) != RINGX_OK) return 0;
   const size_t R = (size_t)B * H * N;
-  return 2 * align_up(R * sizeof(float)) + align_up(R * d_qk * sizeof(float));
+  // D, lse2, the transposed dQ accumulator, and for deterministic mode the per-query fixed-point scales + K/V maxima
+  return 3 * align_up(R * sizeof(float)) + align_up(R * d_qk * sizeof(float)) + align_up((size_t)B * H * 2 * sizeof(float));
 }
 
 int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
@@ -510,24 +511,33 @@ int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* 
   const size_t R = (size_t)BH * N;
   float* D = static_cast<float*>(workspace);
   float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + align_up(R * sizeof(float)));
-  float* dq_acc_t = reinterpret_cast<float*>(static_cast<char*>(workspace) + 2 * align_up(R * sizeof(float)));
+  char* wp = static_cast<char*>(workspace) + 2 * align_up(R * sizeof(float));
+  float* dq_acc_t = reinterpret_cast<float*>(wp);
+  wp += align_up(R * d_qk * sizeof(float));
+  float* qs = reinterpret_cast<float*>(wp);
+  float* kvmax = reinterpret_cast<float*>(wp + align_up(R * sizeof(float)));
+  const bool fixed = g_deterministic.load(std::memory_order_relaxed) != 0;     // int32 fixed-point dQ (see bwd_core)
   cudaError_t e;
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
     e = cudaMemsetAsync(dq_acc_t, 0, R * d_qk * sizeof(float), stream);
     if (e == cudaSuccess) e = launch_bwd_preprocess(o, dO, lse, D, lse2, nullptr, (long long)R, d_v, scale, false, stream);
+    if (e == cudaSuccess && fixed) {
+      e = launch_dq_fixed_scale(k, v, dO, kvmax, qs, BH, N, N, 0, N, d_qk, d_v, scale, stream);
+      count_launch(2);
+    }
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
   for (int c = 0; c < N / kv_chunk; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
     e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, BH, N, N, c * kv_chunk, kv_chunk, scale,
-                                        RINGX_BF16, stream);
+                                        fixed ? qs : nullptr, RINGX_BF16, stream);
     if (e != cudaSuccess) return cuda_status(e);
   }
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-    e = launch_dq_transpose_convert_mla(dq_acc_t, dq, BH, N, stream);
+    e = launch_dq_transpose_convert_mla(dq_acc_t, dq, BH, N, fixed ? qs : nullptr, stream);
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
@@ -611,7 +621,8 @@ int ringx_attn_bwd_partial_mla(const void* q, const void* k, const void* v, cons
   }
   {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
-    e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, B * H, Nq, Nk, 0, Nk, scale, dkv_dtype, stream);
+    e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, B * H, Nq, Nk, 0, Nk, scale, nullptr, dkv_dtype,
+                                        stream);
   }
   if (e != cudaSuccess) return cuda_status(e);
   tl_last_launches = tl_launches;
@@ -629,7 +640,7 @@ int ringx_dq_finalize_mla(const float* dq_acc_t, void* dq, int B, int H, int Nq,
   cudaError_t e;
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-    e = launch_dq_transpose_convert_mla(dq_acc_t, dq, B * H, Nq, stream);
+    e = launch_dq_transpose_convert_mla(dq_acc_t, dq, B * H, Nq, nullptr, stream);
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
@@ -788,7 +799,7 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
       pass_acc = reinterpret_cast<float*>(det.fix);
       if ((e = cudaMemsetAsync(det.fix, 0, (size_t)R * d * sizeof(int), stream)) != cudaSuccess) return cuda_status(e);
     }
-    e = launch_dq_fixed_scale(k, v, dO, det.kvmax, det.qs, BH, Nq, Nk, 0, Nk, d, scale, stream);
+    e = launch_dq_fixed_scale(k, v, dO, det.kvmax, det.qs, BH, Nq, Nk, 0, Nk, d, d, scale, stream);
     count_launch(2);
     if (e != cudaSuccess) return cuda_status(e);
   }

@@ -53,7 +53,7 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
                           const __grid_constant__ CUtensorMap map_dq_a, const __grid_constant__ CUtensorMap map_dq_b,
                           const float* __restrict__ lse2, const float* __restrict__ Dvec, void* __restrict__ dk,
                           void* __restrict__ dv, int dkv_f32, int N, int nk_stride, int k_off, float scale_log2,
-                          float scale) {
+                          float scale, const float* __restrict__ dq_qs) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sK = smem;
@@ -396,6 +396,21 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
           tc_fence_before();
           mbar_arrive(dq_empty);             // both pieces of dQ^T(s) have left TMEM: hand the columns back
         }
+        if (dq_qs) {
+          // deterministic mode (attn_bwd_sm100.cu): int32 fixed point; here a thread is a feature row and its 64
+          // registers are the 64 queries of the sub-tile, each with its own scale (warp-uniform 16-byte loads)
+          const float4* qs4 = reinterpret_cast<const float4*>(dq_qs + static_cast<size_t>(bh) * N + s * kSub);
+#pragma unroll
+          for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int g = 0; g < 8; ++g) {
+              const float4 f = __ldg(qs4 + c * 8 + g);
+              r[c][g * 4 + 0] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 0]) * f.x));
+              r[c][g * 4 + 1] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 1]) * f.y));
+              r[c][g * 4 + 2] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 2]) * f.z));
+              r[c][g * 4 + 3] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 3]) * f.w));
+            }
+        }
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
           if (leader) tma_wait_group_read<1>();      // the reduce that last read this panel has finished reading
@@ -431,15 +446,21 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
 }
 
 // dq_acc^T [BH, 192, N] fp32 -> dq [BH, N, 192] bf16 (RN-even): 64 x 64 tiles through shared memory, reads coalesced
-// along the queries, writes coalesced along the features.
+// along the queries, writes coalesced along the features.  qs != nullptr: the accumulator is int32 fixed point and query n
+// of head bh carries the scale qs[bh * N + n] (deterministic mode).
 __global__ void __launch_bounds__(256)
-dq_transpose_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dq, int N) {
+dq_transpose_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dq, int N,
+                            const float* __restrict__ qs) {
   __shared__ float tile[64][65];
   const int bh = blockIdx.z, f0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
   const int tx = threadIdx.x & 63, ty = threadIdx.x >> 6;          // 64 x 4
   const float* src = acc + (static_cast<size_t>(bh) * kDqk + f0) * N + n0;
+  const float inv = qs ? 1.0f / __ldg(qs + static_cast<size_t>(bh) * N + n0 + tx) : 1.0f;
 #pragma unroll
-  for (int r = ty; r < 64; r += 4) tile[r][tx] = __ldcs(src + static_cast<size_t>(r) * N + tx);   // [feature][query]
+  for (int r = ty; r < 64; r += 4) {                               // [feature][query]
+    const float x = __ldcs(src + static_cast<size_t>(r) * N + tx);
+    tile[r][tx] = qs ? static_cast<float>(__float_as_int(x)) * inv : x;
+  }
   __syncthreads();
   __nv_bfloat16* dst = dq + (static_cast<size_t>(bh) * N + n0) * kDqk + f0;
 #pragma unroll
@@ -451,30 +472,32 @@ dq_transpose_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __rest
 cudaError_t launch_attn_chunk_bwd_mla_sm100(const void* q, const void* k, const void* v, const void* dO,
                                             const float* lse2, const float* D, float* dq_acc_t, void* dk, void* dv,
                                             int BH, int N, int nk_stride, int k_off, int nk, float scale,
-                                            int dkv_dtype, cudaStream_t stream) {
+                                            const float* dq_qs, int dkv_dtype, cudaStream_t stream) {
   CUtensorMap mq, mk, mv, mdo, mdqa, mdqb;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+  const CUtensorMapDataType dqt = dq_qs ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
   const uint64_t rows = (uint64_t)BH * N, krows = (uint64_t)BH * nk_stride;
   if (!make_tmap_2d(&mq, q, dt, 2, rows, kDqk, kSub, 64, kSwizzle128B) ||
       !make_tmap_2d(&mk, k, dt, 2, krows, kDqk, kKeys, 64, kSwizzle128B) ||
       !make_tmap_2d(&mv, v, dt, 2, krows, kDv, kKeys, 64, kSwizzle128B) ||
       !make_tmap_2d(&mdo, dO, dt, 2, rows, kDv, kSub, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mdqa, dq_acc_t, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (uint64_t)BH * kDqk, N, 128, 32, kSwizzle128B) ||
-      !make_tmap_2d(&mdqb, dq_acc_t, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (uint64_t)BH * kDqk, N, 64, 32, kSwizzle128B))
+      !make_tmap_2d(&mdqa, dq_acc_t, dqt, 4, (uint64_t)BH * kDqk, N, 128, 32, kSwizzle128B) ||
+      !make_tmap_2d(&mdqb, dq_acc_t, dqt, 4, (uint64_t)BH * kDqk, N, 64, 32, kSwizzle128B))
     return cudaErrorInvalidValue;
   auto kern = attn_chunk_bwd_mla_kernel;
   static unsigned char configured[kMaxDevices];
   if (cudaError_t e = set_max_dyn_smem_once(kern, kSmemBytes, configured); e != cudaSuccess) return e;
   dim3 grid(nk / kKeys, BH);
   kern<<<grid, kThreads, kSmemBytes, stream>>>(mq, mk, mv, mdo, mdqa, mdqb, lse2, D, dk, dv, dkv_dtype == RINGX_F32, N, nk_stride,
-                                               k_off, scale * 1.4426950408889634f, scale);
+                                               k_off, scale * 1.4426950408889634f, scale, dq_qs);
   count_launch();
   return cudaGetLastError();
 }
 
-cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int BH, int N, cudaStream_t stream) {
+cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int BH, int N, const float* dq_qs,
+                                            cudaStream_t stream) {
   dim3 grid(N / 64, kDqk / 64, BH);
-  dq_transpose_convert_kernel<<<grid, 256, 0, stream>>>(dq_acc_t, static_cast<__nv_bfloat16*>(dq), N);
+  dq_transpose_convert_kernel<<<grid, 256, 0, stream>>>(dq_acc_t, static_cast<__nv_bfloat16*>(dq), N, dq_qs);
   return cudaGetLastError();
 }
 

@@ -33,11 +33,11 @@ cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* ls
                                   cudaStream_t stream);
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
 // Deterministic dQ (int32 fixed-point accumulator, merge.cu).  launch_dq_fixed_scale: kvmax [2*BH] (scratch) and the
-// per-row scales qs [BH*rows_per_head] from k, v rows [k_off, k_off+nk) of every head and dO
-// (2 launches + a memset).  launch_dq_fixed_finish: dq_bf16 = dq_fix / qs (dq_bf16 != nullptr), else dq_acc += dq_fix / qs
+// per-row scales qs [BH*rows_per_head] from k (rows d_k wide), v (d_v wide) rows [k_off, k_off+nk) of every head and dO
+// (d_v wide) (2 launches + a memset).  launch_dq_fixed_finish: dq_bf16 = dq_fix / qs (dq_bf16 != nullptr), else dq_acc += dq_fix / qs
 // (1 launch).
 cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, float* kvmax, float* qs, int BH,
-                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d, float scale,
+                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d_k, int d_v, float scale,
                                   cudaStream_t stream);
 cudaError_t launch_dq_fixed_finish(const int* dq_fix, const float* qs, void* dq_bf16, float* dq_acc, long long rows, int d,
                                    cudaStream_t stream);
@@ -89,12 +89,14 @@ cudaError_t launch_attn_chunk_fwd_mla_sm100(const void* q, const void* k, const 
 // writes dk,dv rows [k_off, k_off+nk) of every head (bf16), reduce-adds these keys' contribution to dQ into the
 // TRANSPOSED fp32 accumulator dq_acc_t [BH,192,N] (zeroed by the caller before the first pass).  N % 64 == 0.
 // lse2, D as for launch_attn_chunk_bwd_sm100 (launch_bwd_preprocess with d = 128).  dkv_dtype: RINGX_BF16 or RINGX_F32.
+// dq_qs: nullptr, or [BH * N] per-query scales (launch_dq_fixed_scale): dq_acc_t is then an int32 fixed-point accumulator.
 cudaError_t launch_attn_chunk_bwd_mla_sm100(const void* q, const void* k, const void* v, const void* dO,
                                             const float* lse2, const float* D, float* dq_acc_t, void* dk, void* dv,
                                             int BH, int N, int nk_stride, int k_off, int nk, float scale,
-                                            int dkv_dtype, cudaStream_t stream);
-// dq [BH,N,192] bf16 = transpose(dq_acc_t [BH,192,N] fp32)
-cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int BH, int N, cudaStream_t stream);
+                                            const float* dq_qs, int dkv_dtype, cudaStream_t stream);
+// dq [BH,N,192] bf16 = transpose(dq_acc_t [BH,192,N] fp32), or of the int32 fixed-point accumulator / dq_qs[query]
+cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int BH, int N, const float* dq_qs,
+                                            cudaStream_t stream);
 
 // ---- attn_bwd_sm100.cu (tcgen05 path)
 // One KV-chunk pass of the backward: q,dO [BH,N,d], k,v,dk,dv [BH,nk_stride,d]; writes dk,dv rows

@@ -301,20 +301,19 @@ dq_convert_kernel(const float4* __restrict__ dq_acc, uint2* __restrict__ dq, lon
 
 // kvmax[2h] = max_j ||V_j||^2, kvmax[2h+1] = max_jc |K_jc| over the nk key rows [k_off, k_off+nk) of kv head h
 // (atomicMax on the bit patterns of non-negative floats: order-independent).  grid = (blocks, BH); kvmax zeroed before.
-template <int kLanes>
+// V rows are kLanesV uint4 wide (d_v = 8 kLanesV), K rows k_vecs uint4 wide (any width: only max |.| is needed).
+template <int kLanesV>
 __global__ void __launch_bounds__(256)
 kv_absmax_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v, unsigned* __restrict__ kvmax, int nk_stride,
-                 int k_off, int nk) {
-  constexpr int kRowsPerWarp = 32 / kLanes;
-  const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
+                 int k_off, int nk, int k_vecs) {
+  constexpr int kRowsPerWarp = 32 / kLanesV;
+  const int lane = threadIdx.x & 31, sub = lane / kLanesV, l = lane % kLanesV;
   const int bh = blockIdx.y;
   const long long head0 = (long long)bh * nk_stride + k_off;
   float vmax2 = 0.f, kmax = 0.f;
   for (int base = (blockIdx.x * 8 + (threadIdx.x >> 5)) * kRowsPerWarp; base < nk; base += gridDim.x * 8 * kRowsPerWarp) {
     const int r = base + sub;      // nk % 128 == 0: every lane has a row
-    const uint4 a = __ldg(k + (head0 + r) * kLanes + l);
-    const uint4 b = __ldg(v + (head0 + r) * kLanes + l);
-    const uint32_t* pa = reinterpret_cast<const uint32_t*>(&a);
+    const uint4 b = __ldg(v + (head0 + r) * kLanesV + l);
     const uint32_t* pb = reinterpret_cast<const uint32_t*>(&b);
     float s = 0.f;
 #pragma unroll
@@ -322,11 +321,18 @@ kv_absmax_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v, unsig
       const float v0 = __uint_as_float(pb[i] << 16), v1 = __uint_as_float(pb[i] & 0xFFFF0000u);
       s = fmaf(v0, v0, s);
       s = fmaf(v1, v1, s);
-      kmax = fmaxf(kmax, fmaxf(fabsf(__uint_as_float(pa[i] << 16)), fabsf(__uint_as_float(pa[i] & 0xFFFF0000u))));
     }
 #pragma unroll
-    for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    for (int off = kLanesV / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
     vmax2 = fmaxf(vmax2, s);
+  }
+  const uint4* kh = k + head0 * k_vecs;
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < (long long)nk * k_vecs; i += (long long)gridDim.x * 256) {
+    const uint4 a = __ldg(kh + i);
+    const uint32_t* pa = reinterpret_cast<const uint32_t*>(&a);
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      kmax = fmaxf(kmax, fmaxf(fabsf(__uint_as_float(pa[j] << 16)), fabsf(__uint_as_float(pa[j] & 0xFFFF0000u))));
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
@@ -486,11 +492,11 @@ cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float 
 }
 
 cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, float* kvmax, float* qs, int BH,
-                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d, float scale,
+                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d_k, int d_v, float scale,
                                   cudaStream_t stream) {
   cudaError_t e = cudaMemsetAsync(kvmax, 0, (size_t)BH * 2 * sizeof(float), stream);
   if (e != cudaSuccess) return e;
-  const int lanes = d / 8;   // 8 or 16
+  const int lanes = d_v / 8;   // 8 or 16: V rows and dO rows
   const int rows_per_block = 8 * (32 / lanes);
   int bx = (nk + rows_per_block - 1) / rows_per_block;
   const int cap = (sm_count() * 8 + BH - 1) / BH;
@@ -500,10 +506,10 @@ cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, 
   long long blocks = (rows + rows_per_block - 1) / rows_per_block;
   if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
   if (lanes == 8) {
-    kv_absmax_kernel<8><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk);
+    kv_absmax_kernel<8><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk, d_k / 8);
     dq_fixed_scale_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, qs, rows, rows_per_head, scale);
   } else {
-    kv_absmax_kernel<16><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk);
+    kv_absmax_kernel<16><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk, d_k / 8);
     dq_fixed_scale_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, qs, rows, rows_per_head, scale);
   }
   return cudaGetLastError();

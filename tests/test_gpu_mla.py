@@ -154,6 +154,34 @@ def test_mla_backward_matches_oracle(rx, B, H, N, chunk, gain):
     check_grads(dq, dk, dv, f64(q), f64(k), f64(v), f64(do), scale)
 
 
+@pytest.mark.parametrize("B,H,N,chunk,gain", [(2, 3, 1280, 256, 1.0), (1, 8, 8192, 2048, 1.0), (1, 2, 2048, 512, 3.0)])
+def test_mla_backward_deterministic_mode(rx, B, H, N, chunk, gain):
+    """ringx_set_deterministic with the MLA widths: the transposed dQ accumulator becomes int32 fixed point (per-query
+    scales; integer reduce-adds are associative), so repeated runs agree bit for bit -- (1, 8, 8192, 2048) is 512 CTAs per
+    pass, 3.5 waves, where the arrival order of the adds varies -- dk, dv are the default mode's, and the result still
+    matches the oracle element by element."""
+    q, k, v = make(B, H, N, seed=139, gain=gain)
+    do = make_do(B, H, N, seed=139)
+    scale = 1.0 / math.sqrt(DQK)
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    o, lse = rx.ringx_attn_fwd_mla(qd, kd, vd, chunk, scale)
+    loose = rx.ringx_attn_bwd_mla(qd, kd, vd, o, lse, dod, chunk, scale)
+    rx.ringx_set_deterministic(True)
+    try:
+        runs = [rx.ringx_attn_bwd_mla(qd, kd, vd, o, lse, dod, chunk, scale) for _ in range(3)]
+        assert rx.ringx_last_launch_count() == N // chunk + 4
+        torch.cuda.synchronize()
+    finally:
+        rx.ringx_set_deterministic(False)
+    for r in runs[1:]:
+        for a, b in zip(runs[0], r):
+            assert torch.equal(a, b)
+    assert torch.equal(runs[0][1], loose[1]) and torch.equal(runs[0][2], loose[2])
+    assert ((runs[0][0].float() - loose[0].float()).norm() / loose[0].float().norm()).item() <= 2e-3
+    if N <= 2048:
+        check_grads(*runs[0], f64(q), f64(k), f64(v), f64(do), scale)
+
+
 def test_mla_backward_every_panel_matters_and_chunk_independent(rx):
     """Zeroing one 64-column panel of q (k, v, dO) in the ORACLE must break the agreement with the kernel's result: the
     kernel contracts over all three panels of q, k and both of v, dO.  dk, dv of a key tile are written once by one CTA
