@@ -28,9 +28,14 @@
  *   Errors     Return value is a ringx_status (0 = RINGX_OK).  Arguments are validated before the
  *              first launch: an error other than RINGX_ERR_CUDA means nothing was enqueued and no
  *              output was touched.  No abort, no printf, no exceptions cross this boundary.
- *   Domain     d in {64, 128}; N % 128 == 0; kv_chunk % 128 == 0; 0 < kv_chunk <= N;
- *              N % kv_chunk == 0 (every device holds an equal chunk S/N, l.128).  bf16 kernels also
- *              need N % 256 == 0 (one CTA owns two 128-row query tiles).  Anything else returns
+ *   Domain     d in {64, 128}; kv_chunk % 128 == 0.  ringx_attn_fwd / ringx_attn_bwd and their GQA forms
+ *              with RINGX_BF16 take ANY sequence length N >= 1 and any kv_chunk <= N rounded up to 128:
+ *              there are ceil(N / kv_chunk) passes, the last one over the keys that are left; tiles
+ *              that run past the end of a head read zeros (3-D tensor maps), keys past the end are
+ *              masked, rows past the end are never written.  Every other entry (fp32, the per-chunk /
+ *              per-device steps, the *_host, MLA and block entries) needs N % 128 == 0 (N % 256 == 0 for a
+ *              bf16 forward: one CTA owns two 128-row query tiles), 0 < kv_chunk <= N and N % kv_chunk == 0
+ *              (every device holds an equal chunk S/N, l.128).  Anything else returns
  *              RINGX_ERR_BAD_SHAPE -- never a silently wrong answer.  A device that is not
  *              compute capability 10.x returns RINGX_ERR_UNSUPPORTED_ARCH.
  *   Semantics  Non-causal, no mask, no dropout, no bias.  `scale` multiplies Q.K^T before the

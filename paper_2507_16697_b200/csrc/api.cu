@@ -57,13 +57,20 @@ int check_arch() {
   return major == 10 ? RINGX_OK : RINGX_ERR_UNSUPPORTED_ARCH;
 }
 
-int check_shape(int B, int H, int N, int d, int kv_chunk, float scale, int dtype, bool backward) {
+// `ragged_ok`: the entry point takes any sequence length (bf16 ringx_attn_fwd / ringx_attn_bwd and their GQA forms): the
+// kernels zero-fill and mask what lies past the end of a head, and the last KV chunk may be shorter than kv_chunk.
+int check_shape(int B, int H, int N, int d, int kv_chunk, float scale, int dtype, bool backward, bool ragged_ok = false) {
   if (dtype != RINGX_F32 && dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (backward && dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (B <= 0 || H <= 0 || N <= 0 || kv_chunk <= 0) return RINGX_ERR_BAD_SHAPE;
   if (d != 64 && d != 128) return RINGX_ERR_BAD_SHAPE;
-  if (N % 128 || kv_chunk % 128 || kv_chunk > N || N % kv_chunk) return RINGX_ERR_BAD_SHAPE;
-  if (dtype == RINGX_BF16 && !backward && N % 256) return RINGX_ERR_BAD_SHAPE;
+  if (kv_chunk % 128) return RINGX_ERR_BAD_SHAPE;
+  if (ragged_ok && dtype == RINGX_BF16) {
+    if (kv_chunk > (N + 127) / 128 * 128) return RINGX_ERR_BAD_SHAPE;
+  } else {
+    if (N % 128 || kv_chunk > N || N % kv_chunk) return RINGX_ERR_BAD_SHAPE;
+    if (dtype == RINGX_BF16 && !backward && N % 256) return RINGX_ERR_BAD_SHAPE;
+  }
   if ((long long)B * H > 65535) return RINGX_ERR_BAD_SHAPE;
   if ((long long)B * H * N > 0x7FFFFFFFLL) return RINGX_ERR_BAD_SHAPE;   // TMA row coordinate is int32
   if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
@@ -77,7 +84,7 @@ constexpr int kMaxSplits = 8;
 constexpr int kMinTilesPerSplit = 8;   // >= 1024 keys per split: below that the prologue/epilogue of a CTA dominates
 
 int choose_splits(int BH, int Nq, int nk, int dtype) {
-  if (dtype != RINGX_BF16 || Nq % 256) return 1;
+  if (dtype != RINGX_BF16 || Nq % 256 || nk % 128) return 1;
   const long long ctas = (long long)BH * (Nq / 256);
   const int kSmCount = sm_count();       // of the current device: the same value sizes the workspace and picks the grid
   if (ctas >= 2 * kSmCount) return 1;
@@ -138,9 +145,10 @@ FwdWorkspace carve_fwd(void* ws, int B, int H, int N, int d, int kv_chunk, int d
     off += align_up(n);
     return r;
   };
-  w.split = carve_split(nullptr, R, d, choose_splits(B * H, N, kv_chunk, dtype));
+  // (a ragged sequence or a short last chunk: no split-KV -- the passes would not all split alike)
+  w.split = carve_split(nullptr, R, d, (N % 128 || N % kv_chunk) ? 1 : choose_splits(B * H, N, kv_chunk, dtype));
   if (w.split.splits > 1) w.split = carve_split(take(w.split.bytes), R, d, w.split.splits);
-  if (kv_chunk == N) {           // single pass: the chunk kernel writes (o, lse) directly
+  if (kv_chunk >= N) {           // single pass: the chunk kernel writes (o, lse) directly
     w.bytes = off;
     return w;
   }
@@ -167,11 +175,12 @@ struct BwdWorkspace {
 BwdWorkspace carve_bwd(void* ws, int B, int H, int N, int d) {
   BwdWorkspace w;
   const size_t R = (size_t)B * H * N;
+  const size_t R_stat = (size_t)B * H * ((N + 127) / 128 * 128);   // D, lse2: every head padded to the 128-row tile
   char* p = static_cast<char*>(ws);
   w.D = reinterpret_cast<float*>(p);
-  size_t off = align_up(R * sizeof(float));
+  size_t off = align_up(R_stat * sizeof(float));
   w.lse2 = reinterpret_cast<float*>(p ? p + off : nullptr);
-  off += align_up(R * sizeof(float));
+  off += align_up(R_stat * sizeof(float));
   w.dq_acc = reinterpret_cast<float*>(p ? p + off : nullptr);
   off += align_up(R * d * sizeof(float));
   w.dq_qs = reinterpret_cast<float*>(p ? p + off : nullptr);
@@ -288,6 +297,22 @@ bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, in
   return r == CUDA_SUCCESS;
 }
 
+// 3-D view [heads][rows][cols] (row-major, contiguous), box = {box_cols, box_rows, 1}: a box that runs past the last row
+// of a head is zero-filled on load and clipped on store / reduce (ragged sequence lengths)
+bool make_tmap_3d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t heads, uint64_t rows,
+                  uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz) {
+  EncodeFn enc = encode_fn();
+  if (!enc) return false;
+  cuuint64_t dims[3] = {cols, rows, heads};
+  cuuint64_t strides[2] = {cols * (uint64_t)elem_bytes, rows * cols * (uint64_t)elem_bytes};
+  cuuint32_t box[3] = {box_cols, box_rows, 1};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = enc(out, dt, 3, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   swz == kSwizzle128B ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
 // One KV-chunk pass, either dtype.  `epilogue` (kernels.cuh, kFwdEpi*): partial / final / folded into (o_acc, lse_acc).
 // The fp32 path has the partial epilogue only.
 static cudaError_t chunk_pass(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
@@ -336,12 +361,12 @@ using namespace ringx;
 extern "C" {
 
 size_t ringx_attn_fwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
-  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false) != RINGX_OK) return 0;
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false, true) != RINGX_OK) return 0;
   return carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype).bytes;
 }
 
 size_t ringx_attn_bwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
-  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, true) != RINGX_OK) return 0;
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, true, true) != RINGX_OK) return 0;
   return carve_bwd(nullptr, B, H, N, d).bytes;
 }
 
@@ -358,7 +383,8 @@ size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_ch
 static int fwd_core(const void* q, const void* k, const void* v, void* o, float* lse, int BH, int Nq, int N, int d,
                     int kv_chunk, float scale, int dtype, const FwdWorkspace& w, cudaStream_t stream) {
   const long long R = (long long)BH * Nq;
-  const int n_chunks = N / kv_chunk;
+  const int n_chunks = (N + kv_chunk - 1) / kv_chunk;      // the last chunk may be short (and its last key tile ragged)
+  const int nk_last = N - (n_chunks - 1) * kv_chunk;
   if (n_chunks == 1) {
     cudaError_t e = chunk_pass(q, k, v, o, lse, nullptr, nullptr, BH, Nq, N, 0, N, d, scale, dtype, kFwdEpiFinal, stream,
                                &w.split);
@@ -378,7 +404,7 @@ static int fwd_core(const void* q, const void* k, const void* v, void* o, float*
         e = chunk_pass(q, k, v, w.o_acc, w.lse_acc, w.o_acc, w.lse_acc, BH, Nq, N, c * kv_chunk, kv_chunk, d, scale,
                        dtype, kFwdEpiFold, stream, &w.split);
       else
-        e = chunk_pass(q, k, v, o, lse, w.o_acc, w.lse_acc, BH, Nq, N, c * kv_chunk, kv_chunk, d, scale, dtype,
+        e = chunk_pass(q, k, v, o, lse, w.o_acc, w.lse_acc, BH, Nq, N, c * kv_chunk, nk_last, d, scale, dtype,
                        kFwdEpiFoldFinal, stream, &w.split);
       if (e != cudaSuccess) return cuda_status(e);
       continue;
@@ -408,7 +434,7 @@ int ringx_attn_fwd_gqa(const void* q, const void* k, const void* v, void* o, flo
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!q || !k || !v || !o || !lse) return RINGX_ERR_NULL_PTR;
   int st = check_gqa(Hq, Hkv);
-  if (st == RINGX_OK) st = check_shape(B, Hq, N, d, kv_chunk, scale, dtype, false);
+  if (st == RINGX_OK) st = check_shape(B, Hq, N, d, kv_chunk, scale, dtype, false, true);
   if (st != RINGX_OK) return st;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse)) return RINGX_ERR_MISALIGNED;
   const FwdWorkspace need = carve_fwd(nullptr, B, Hq, N, d, kv_chunk, dtype);
@@ -787,9 +813,9 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
   if (!prepared) {
     {
       Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-      e = launch_bwd_preprocess(o, dO, lse, D, lse2, dq_acc, R, d, scale, zero_dq, stream);
+      e = launch_bwd_preprocess(o, dO, lse, D, lse2, dq_acc, R, d, scale, zero_dq, stream, Nq);
     }
-    count_launch();
+    count_launch(Nq % 128 ? 2 : 1);
     if (e != cudaSuccess) return cuda_status(e);
   }
   float* pass_acc = dq_acc;
@@ -803,9 +829,11 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
     count_launch(2);
     if (e != cudaSuccess) return cuda_status(e);
   }
-  for (int c = 0; c < Nk / kv_chunk; ++c) {
+  const int n_chunks = (Nk + kv_chunk - 1) / kv_chunk;       // the last chunk may be short (and its last key tile ragged)
+  for (int c = 0; c < n_chunks; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
-    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, pass_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, kv_chunk, d, scale,
+    const int nk_c = c + 1 < n_chunks ? kv_chunk : Nk - c * kv_chunk;
+    e = launch_attn_chunk_bwd_sm100(q, k, v, dO, lse2, D, pass_acc, dk, dv, BH, Nq, Nk, c * kv_chunk, nk_c, d, scale,
                                     fixed ? det.qs : nullptr, dkv_dtype, stream);
     if (e != cudaSuccess) return cuda_status(e);
     if (tl_hooks.pass_done && (e = cudaEventRecord(tl_hooks.pass_done[c], stream)) != cudaSuccess) return cuda_status(e);
@@ -830,7 +858,7 @@ int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, const void* 
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!q || !k || !v || !o || !lse || !dO || !dq || !dk || !dv) return RINGX_ERR_NULL_PTR;
   int st = check_gqa(Hq, Hkv);
-  if (st == RINGX_OK) st = check_shape(B, Hq, N, d, kv_chunk, scale, dtype, true);
+  if (st == RINGX_OK) st = check_shape(B, Hq, N, d, kv_chunk, scale, dtype, true, true);
   if (st != RINGX_OK) return st;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse) || !aligned16(dO) ||
       !aligned16(dq) || !aligned16(dk) || !aligned16(dv))

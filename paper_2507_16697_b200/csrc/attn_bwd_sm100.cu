@@ -63,13 +63,18 @@ struct BwdCfg {
   static constexpr unsigned kPolyMask = kD == 64 ? kBwdPolyMaskD64 : kBwdPolyMaskD128;
 };
 
-template <int kD>
+// Ragged sequences (N no multiple of 128).  Q_i, dO_i, K_j, V_j come through [BH][rows][d] tensor maps: rows past the end
+// of a head read as zero, and the dQ reduce-add skips them.  lse2 / D are [BH][n_stat] with n_stat = N rounded up to 128
+// and lse2 = +inf in the padding, so P = 0 for query rows that do not exist.  kTail: the launch contains the key tile
+// that runs past the end of the head; its missing keys (K row zero: score 0) get P = 0 by a select in phase A and their
+// dK, dV rows are not stored.  A separate instantiation: launches over full tiles carry none of it.
+template <int kD, bool kTail>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                       const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_do,
                       const __grid_constant__ CUtensorMap map_dq, const float* __restrict__ lse2,
                       const float* __restrict__ Dvec,
-                      void* __restrict__ dk, void* __restrict__ dv, int dkv_f32, int N, int nk_stride, int k_off,
+                      void* __restrict__ dk, void* __restrict__ dv, int dkv_f32, int N, int n_stat, int nk_stride, int k_off,
                       float scale_log2, float scale, const float* __restrict__ dq_qs, unsigned* __restrict__ smem_probe) {
   using Cfg = BwdCfg<kD>;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -107,9 +112,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   const int lane = threadIdx.x & 31;
   const int bh = blockIdx.y;
-  const int n_q = N / kTile;
-  const int q_row0 = bh * N;                                  // rows of this head in the [BH*N, d] views
-  const int k_row0 = bh * nk_stride + k_off + blockIdx.x * kTile;   // rows in the [BH*nk_stride, d] views of K, V, dK, dV
+  const int n_q = (N + kTile - 1) / kTile;
+  const int q_row0 = bh * N;                                  // rows of this head in the flat [BH*N] arrays (dq_qs)
+  const int s_row0 = bh * n_stat;                             // ... in lse2, D
+  const int k_in = k_off + blockIdx.x * kTile;                // first key row of my tile within the head
+  const int k_row0 = bh * nk_stride + k_in;                   // ... in the flat [BH*nk_stride, d] arrays dK, dV
 
   if (threadIdx.x == 0) {
     mbar_init(kv_full, 1);
@@ -157,21 +164,20 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       mbar_arrive_expect_tx(kv_full, 2 * Cfg::kTileBytes);
 #pragma unroll
       for (int p = 0; p < Cfg::kPanels; ++p) {
-        tma_load_2d(sK + p * Cfg::kPanelBytes, &map_k, kv_full, p * 64, k_row0, pol_kv);
-        tma_load_2d(sV + p * Cfg::kPanelBytes, &map_v, kv_full, p * 64, k_row0, pol_kv);
+        tma_load_3d(sK + p * Cfg::kPanelBytes, &map_k, kv_full, p * 64, k_in, bh, pol_kv);
+        tma_load_3d(sV + p * Cfg::kPanelBytes, &map_v, kv_full, p * 64, k_in, bh, pol_kv);
       }
     }
     __syncwarp();
     auto load_q = [&](int i, int st) {
       if (leader) {
         uint8_t* dst = sQ + st * Cfg::kQStageBytes;
-        const int row = q_row0 + i * kTile;
         mbar_arrive_expect_tx(&q_full[st], Cfg::kQStageBytes);
 #pragma unroll
         for (int p = 0; p < Cfg::kPanels; ++p)
-          tma_load_2d(dst + p * Cfg::kPanelBytes, &map_q, &q_full[st], p * 64, row, pol_q);
-        bulk_load_1d(dst + Cfg::kTileBytes, lse2 + row, 512, &q_full[st]);
-        bulk_load_1d(dst + Cfg::kTileBytes + 512, Dvec + row, 512, &q_full[st]);
+          tma_load_3d(dst + p * Cfg::kPanelBytes, &map_q, &q_full[st], p * 64, i * kTile, bh, pol_q);
+        bulk_load_1d(dst + Cfg::kTileBytes, lse2 + s_row0 + i * kTile, 512, &q_full[st]);
+        bulk_load_1d(dst + Cfg::kTileBytes + 512, Dvec + s_row0 + i * kTile, 512, &q_full[st]);
       }
       __syncwarp();
     };
@@ -184,8 +190,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         mbar_arrive_expect_tx(&do_full[ds], Cfg::kTileBytes);
 #pragma unroll
         for (int p = 0; p < Cfg::kPanels; ++p)
-          tma_load_2d(sDo + ds * Cfg::kTileBytes + p * Cfg::kPanelBytes, &map_do, &do_full[ds], p * 64,
-                      q_row0 + i * kTile, pol_q);
+          tma_load_3d(sDo + ds * Cfg::kTileBytes + p * Cfg::kPanelBytes, &map_do, &do_full[ds], p * 64, i * kTile, bh,
+                      pol_q);
       }
       __syncwarp();
       if (++ds == Cfg::kDoStages) { ds = 0; dph ^= 1; }
@@ -308,6 +314,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     uint8_t* ds_row = sDs + half * Cfg::kPanelBytes + row * 128;
     const float2 sc2 = make_float2(scale_log2, scale_log2);
     const float2 scl2 = make_float2(scale, scale);               // dS^T carries `scale` (Dvec holds scale * D_i)
+    const bool key_valid = !kTail || k_in + row < nk_stride;
     if (Cfg::kTmemOperands) {
       // K_j (warps 0-3) / V_j (warps 4-7): my row of the 128B-swizzled tile -> my TMEM lane (2 bf16 per column)
       mbar_wait(kv_full, 0);
@@ -365,7 +372,8 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           uint32_t pk[16];
 #pragma unroll
           for (int e = 0; e < 16; ++e) {
-            const float2 pe = ((Cfg::kPolyMask >> e) & 1) ? ex2_poly2(x[e]) : make_float2(ex2(x[e].x), ex2(x[e].y));
+            float2 pe = ((Cfg::kPolyMask >> e) & 1) ? ex2_poly2(x[e]) : make_float2(ex2(x[e].x), ex2(x[e].y));
+            if (kTail && !key_valid) pe = make_float2(0.f, 0.f);       // a key past the end of the head
             p[c * 16 + e] = pe;
             pk[e] = pack_bf16x2(pe.x, pe.y);
           }
@@ -439,6 +447,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       uint32_t r[32];
       tmem_ld_x32(tSrc + c * 32, r);
       tmem_wait_ld();
+      if (!key_valid) continue;              // (after the warp-wide TMEM load) a key row past the end of the head
       if (dkv_f32) {
         float4* dst = reinterpret_cast<float4*>(static_cast<float*>(half == 0 ? dv : dk) + out_off + c * 32);
 #pragma unroll
@@ -474,11 +483,11 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     // not depend on the order in which the CTAs' adds arrive -- bit-reproducible dQ with no ordering between CTAs.
     const bool fixed = dq_qs != nullptr;
     const float* qs_row = fixed ? dq_qs + q_row0 + row : nullptr;
-    float qs_next = fixed ? __ldg(qs_row) : 1.f;
+    float qs_next = fixed && row < N ? __ldg(qs_row) : 1.f;
     int buf = 0;
     for (int i = 0; i < n_q; ++i) {
       const float qs = qs_next;
-      if (fixed && i + 1 < n_q) qs_next = __ldg(qs_row + (i + 1) * kTile);   // ahead of the wait: latency hidden
+      if (fixed && (i + 1) * kTile + row < N) qs_next = __ldg(qs_row + (i + 1) * kTile);   // ahead of the wait: latency hidden
       mbar_wait(dq_full, i & 1);
       tc_fence_after();
 
@@ -512,7 +521,7 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           fence_proxy_async_smem();
           named_bar_sync(2, 128);
           if (leader) {
-            tma_reduce_add_2d(&map_dq, sDq + buf * Cfg::kDqPanelBytes, rd * 64 + c * 32, q_row0 + i * kTile);
+            tma_reduce_add_3d(&map_dq, sDq + buf * Cfg::kDqPanelBytes, rd * 64 + c * 32, i * kTile, bh);
             tma_commit_group();
           }
           buf ^= 1;
@@ -530,12 +539,13 @@ attn_chunk_bwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   if (warp == 12) tmem_dealloc<512>(tmem);
 }
 
-template <int kD>
-cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
-                     const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int dkv_f32, int BH,
-                     int N, int nk_stride, int k_off, int nk, float scale, const float* dq_qs, cudaStream_t stream) {
+template <int kD, bool kTail>
+cudaError_t launch_tt(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
+                      const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int dkv_f32, int BH,
+                      int N, int n_stat, int nk_stride, int k_off, int nk, float scale, const float* dq_qs,
+                      cudaStream_t stream) {
   using Cfg = BwdCfg<kD>;
-  auto kern = attn_chunk_bwd_kernel<kD>;
+  auto kern = attn_chunk_bwd_kernel<kD, kTail>;
   static unsigned char configured[kMaxDevices];
   if (cudaError_t e = set_max_dyn_smem_once(kern, Cfg::kSmemBytes, configured); e != cudaSuccess) return e;
   if (Cfg::kAlignSlack == 0) {
@@ -549,7 +559,7 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
       unsigned h = 0xffffffffu;
       cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&flag), g_bwd_smem_probe);
       if (e != cudaSuccess) return e;
-      kern<<<1, 32, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0, 0.f,
+      kern<<<1, 32, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0, 0, 0.f,
                                                0.f, nullptr, flag);
       if ((e = cudaGetLastError()) != cudaSuccess) return e;
       if ((e = cudaMemcpyAsync(&h, flag, sizeof(h), cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return e;
@@ -560,11 +570,23 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
       return cudaErrorInvalidConfiguration;
     }
   }
-  dim3 grid(nk / kTile, BH);
-  kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, N, nk_stride, k_off,
-                                                       scale * 1.4426950408889634f, scale, dq_qs, nullptr);
+  dim3 grid((nk + kTile - 1) / kTile, BH);
+  kern<<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, N, n_stat, nk_stride,
+                                                       k_off, scale * 1.4426950408889634f, scale, dq_qs, nullptr);
   count_launch();
   return cudaGetLastError();
+}
+
+template <int kD>
+cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mdo,
+                     const CUtensorMap& mdq, const float* lse2, const float* D, void* dk, void* dv, int dkv_f32, int BH,
+                     int N, int n_stat, int nk_stride, int k_off, int nk, float scale, const float* dq_qs,
+                     cudaStream_t stream) {
+  if (nk % kTile)
+    return launch_tt<kD, true>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, n_stat, nk_stride, k_off, nk, scale, dq_qs,
+                               stream);
+  return launch_tt<kD, false>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, n_stat, nk_stride, k_off, nk, scale, dq_qs,
+                              stream);
 }
 
 }  // namespace
@@ -573,20 +595,22 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
                                         int nk_stride, int k_off, int nk, int d, float scale, const float* dq_qs,
                                         int dkv_dtype, cudaStream_t stream) {
+  if (nk % kTile && k_off + nk != nk_stride) return cudaErrorInvalidValue;   // only the head's last key tile may be ragged
   CUtensorMap mq, mk, mv, mdo, mdq;
   const int dkv_f32 = dkv_dtype == RINGX_F32;
+  const int n_stat = (N + kTile - 1) / kTile * kTile;      // row stride of lse2, D (launch_bwd_preprocess)
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
-  const uint64_t rows = (uint64_t)BH * N, krows = (uint64_t)BH * nk_stride;
-  if (!make_tmap_2d(&mq, q, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mk, k, dt, 2, krows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mv, v, dt, 2, krows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mdo, dO, dt, 2, rows, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mdq, dq_acc, dq_qs ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, rows, d, 128, 32,
+  // [BH][rows][d] views: tiles that run past the end of a head read zeros there, and the dQ reduce-add skips those rows
+  if (!make_tmap_3d(&mq, q, dt, 2, BH, N, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mk, k, dt, 2, BH, nk_stride, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mv, v, dt, 2, BH, nk_stride, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mdo, dO, dt, 2, BH, N, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mdq, dq_acc, dq_qs ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, BH, N, d, 128, 32,
                     kSwizzle128B))
     return cudaErrorInvalidValue;
-  if (d == 64) return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_qs, stream);
-  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, nk_stride, k_off, nk, scale, dq_qs, stream);
+  if (d == 64)
+    return launch_t<64>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, n_stat, nk_stride, k_off, nk, scale, dq_qs, stream);
+  return launch_t<128>(mq, mk, mv, mdo, mdq, lse2, D, dk, dv, dkv_f32, BH, N, n_stat, nk_stride, k_off, nk, scale, dq_qs, stream);
 }
 
 }  // namespace ringx
-

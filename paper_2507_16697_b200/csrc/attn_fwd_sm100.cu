@@ -112,6 +112,7 @@ struct FwdParams {
   const float* o_acc;
   const float* lse_acc;
   int Nq, nk_stride, k_off, n_kv;      // n_kv = key tiles per item
+  int k_tail;                          // keys of the pass's last key tile that exist (0: all 128) -- a ragged sequence
   float scale_log2;
 };
 
@@ -121,20 +122,27 @@ struct ItemId {
   bool valid;
 };
 struct ItemRows {
-  int q_row0;        // first query row in the [BH*Nq, d] view
-  int k_row0;        // first key row in the [BH*nk_stride, d] view
+  int bh;            // head: the third TMA coordinate of the [BH][rows][d] views
+  int q_in;          // first query row of the item within its head (rows >= Nq do not exist: loaded as zero, never stored)
+  int k_in;          // first key row within the head
+  int q_row0;        // first query row in the flat [BH*Nq, d] view (global-memory addressing of o_acc, lse_acc)
   size_t out_row0;   // first row of (o_out, lse_out): q_row0, plus the split's offset for partials
 };
 template <int kEpi>
 __device__ __forceinline__ ItemRows item_rows(const FwdParams& p, const ItemId& id) {
   ItemRows r;
-  r.q_row0 = id.bh * p.Nq + id.qt * (2 * kBlockM);
-  r.k_row0 = id.bh * p.nk_stride + p.k_off + id.z * p.n_kv * kBlockN;     // z = key split (split-KV; partials only)
+  r.bh = id.bh;
+  r.q_in = id.qt * (2 * kBlockM);
+  r.k_in = p.k_off + id.z * p.n_kv * kBlockN;                             // z = key split (split-KV; partials only)
+  r.q_row0 = id.bh * p.Nq + r.q_in;
   r.out_row0 = static_cast<size_t>(r.q_row0) + (kEpi == kEpiPartial ? static_cast<size_t>(id.z) * gridDim.y * p.Nq : 0);
   return r;
 }
 
-template <int kD, int kEpi>
+// kTail: the pass ends in a key tile with fewer than 128 keys (a ragged sequence; prm.k_tail of them exist).  A separate
+// instantiation, so that the mask costs the full-tile kernels neither an instruction nor a register (the d = 64 softmax
+// warps have none to spare: with the mask compiled in they spill inside the loop, -2 % on C2 / C4).
+template <int kD, int kEpi, bool kTail>
 __global__ void __launch_bounds__(FwdCfg<kD>::kThreads, 1)
 attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                       const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_oacc,
@@ -230,37 +238,40 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     // The K cursor runs kKLead tiles ahead of the V cursor, possibly into later items: it is the one that asks the
     // scheduler for items; their first key rows wait in a 3-deep register FIFO for the V cursor.
     int stage = 0, phase = 0;
-    auto push = [&](const CUtensorMap* map, int row) {
+    auto push = [&](const CUtensorMap* map, int row, int head) {
       mbar_wait_relaxed(&kv_empty[stage], phase ^ 1);
       if (leader) {
         uint8_t* dst = sKV + stage * Cfg::kTileBytes;
         mbar_arrive_expect_tx(&kv_full[stage], Cfg::kTileBytes);
 #pragma unroll
-        for (int p = 0; p < Cfg::kPanels; ++p) tma_load_2d(dst + p * Cfg::kPanelBytes, map, &kv_full[stage], p * 64, row, pol_kv);
+        for (int p = 0; p < Cfg::kPanels; ++p)
+          tma_load_3d(dst + p * Cfg::kPanelBytes, map, &kv_full[stage], p * 64, row, head, pol_kv);
       }
       __syncwarp();
       if (++stage == Cfg::kStages) { stage = 0; phase ^= 1; }
     };
-    int f0 = item_rows<kEpi>(prm, own).k_row0, f1 = 0, f2 = 0, fn = 1;    // FIFO of k_row0: f0 = the V cursor's item
-    int k_row = f0, kj = 0, vj = 0, req = 0;
+    // FIFO of (first key row in the head, head): f0 = the V cursor's item
+    int f0 = item_rows<kEpi>(prm, own).k_in, f1 = 0, f2 = 0, h0 = own.bh, h1 = 0, h2 = 0, fn = 1;
+    int k_row = f0, k_head = h0, kj = 0, vj = 0, req = 0;
     bool k_more = true;                     // the K cursor stands in a valid item
     auto push_k = [&]() {
-      push(&map_k, k_row + kj * kBlockN);
+      push(&map_k, k_row + kj * kBlockN, k_head);
       if (++kj == n_kv) {
         kj = 0;
         const ItemId id = next_item(req++);
         k_more = id.valid;
         if (k_more) {
-          k_row = item_rows<kEpi>(prm, id).k_row0;
-          if (fn == 1) f1 = k_row; else f2 = k_row;          // (fn <= 2 here: the K cursor is at most 2 items ahead)
+          k_row = item_rows<kEpi>(prm, id).k_in;
+          k_head = id.bh;
+          if (fn == 1) { f1 = k_row; h1 = k_head; } else { f2 = k_row; h2 = k_head; }   // (fn <= 2 here: at most 2 items ahead)
           ++fn;
         }
       }
     };
     for (int i = 0; i < Cfg::kKLead && k_more; ++i) push_k();
     while (fn > 0) {
-      push(&map_v, f0 + vj * kBlockN);
-      if (++vj == n_kv) { vj = 0; f0 = f1; f1 = f2; --fn; }
+      push(&map_v, f0 + vj * kBlockN, h0);
+      if (++vj == n_kv) { vj = 0; f0 = f1; f1 = f2; h0 = h1; h1 = h2; --fn; }
       if (k_more) push_k();
     }
   } else if (warp == Cfg::kAuxWarp) {
@@ -288,8 +299,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           mbar_arrive_expect_tx(&q_full[t], Cfg::kTileBytes);
 #pragma unroll
           for (int p = 0; p < Cfg::kPanels; ++p)
-            tma_load_2d(sQ + t * Cfg::kTileBytes + p * Cfg::kPanelBytes, &map_q, &q_full[t], p * 64,
-                        it.q_row0 + t * kBlockM, pol_q);
+            tma_load_3d(sQ + t * Cfg::kTileBytes + p * Cfg::kPanelBytes, &map_q, &q_full[t], p * 64,
+                        it.q_in + t * kBlockM, it.bh, pol_q);
         }
         __syncwarp();
       }
@@ -299,8 +310,8 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           mbar_arrive_expect_tx(oacc_full, Cfg::kOaccBytes);
 #pragma unroll
           for (int p = 0; p < 4; ++p)           // panel p = (query tile p >> 1, columns [32 (p & 1), +32))
-            tma_load_2d(sOacc + p * Cfg::kPanelBytes, &map_oacc, oacc_full, (p & 1) * 32, it.q_row0 + (p >> 1) * kBlockM,
-                        pol_q);
+            tma_load_3d(sOacc + p * Cfg::kPanelBytes, &map_oacc, oacc_full, (p & 1) * 32, it.q_in + (p >> 1) * kBlockM,
+                        it.bh, pol_q);
         }
         __syncwarp();
       }
@@ -309,11 +320,11 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
       cur.valid = clc_query(sched_resp + 16 * sl, cur.qt, cur.bh, cur.z);
       if (!cur.valid) break;
       if (leader) {                             // its Q: into L2 now, so that the load at the item boundary is an L2 hit
-        const int nq0 = item_rows<kEpi>(prm, cur).q_row0;
+        const int nq0 = item_rows<kEpi>(prm, cur).q_in;
 #pragma unroll
         for (int t = 0; t < 2; ++t)
 #pragma unroll
-          for (int p = 0; p < Cfg::kPanels; ++p) tma_prefetch_2d(&map_q, p * 64, nq0 + t * kBlockM);
+          for (int p = 0; p < Cfg::kPanels; ++p) tma_prefetch_3d(&map_q, p * 64, nq0 + t * kBlockM, cur.bh);
       }
       __syncwarp();
     }
@@ -441,9 +452,16 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
     for (int li = 0; cur.valid; ++li) {
       const ItemRows it = item_rows<kEpi>(prm, cur);
       const size_t row = it.out_row0 + t * kBlockM + row_t;     // my row in (o_out, lse_out)
-      const size_t acc_row = static_cast<size_t>(it.q_row0) + t * kBlockM + row_t;   // ... in (o_acc, lse_acc)
+      // ... in (o_acc, lse_acc); -1 for a row past the end of the head (a ragged sequence): such rows were loaded as
+      // zeros, are computed like any other and never stored.  (A sentinel instead of a flag: the d = 64 softmax warps
+      // have no register to spare.)
+      const long long acc_row = it.q_in + t * kBlockM + row_t < prm.Nq ? static_cast<long long>(it.q_row0) + t * kBlockM + row_t : -1;
+      auto row_valid = [&]() { return acc_row >= 0; };
+      // the keys past the end of the head in the pass's last key tile (zero rows of K: score 0) are masked to -inf
+      // (kTail launches have no key splits)
+      auto tail_tile = [&](int j) { return kTail && j == n_kv - 1; };
       float lse_prev = 0.f;                                     // lse_acc of my row: the running LSE this pass is folded with
-      if (kFold) lse_prev = prm.lse_acc[acc_row];               // (read at the item's start: long since there at its end)
+      if (kFold && row_valid()) lse_prev = prm.lse_acc[acc_row];   // (read at the item's start: long since there at its end)
       float m_raw = -CUDART_INF_F;   // running (lazy) row max of the unscaled scores
       float m_sc = -CUDART_INF_F;    // m_raw * scale_log2
       float l = 0.f;                 // running row sum of exp2(s*scale_log2 - m_sc)
@@ -470,6 +488,14 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           piece_max(0, mx0, mx1);
           tmem_wait_ld_x32(piece(1));
           piece_max(1, mx0, mx1);
+          if (tail_tile(j)) {                                    // warp-uniform, last key tile of a ragged pass only
+#pragma unroll
+            for (int c = 0; c < 64; ++c)
+              if (hh * 64 + c >= prm.k_tail) s[c] = 0xff800000u;   // -inf
+            mx0 = mx1 = -CUDART_INF_F;
+            piece_max(0, mx0, mx1);
+            piece_max(1, mx0, mx1);
+          }
           // exchange the half-row maxima; the barrier also tells each half that the other has its scores in registers,
           // so P (which overwrites the first 64 columns of the score buffer) may be written
           float* slot = xch_t + (j & 1) * 256;
@@ -567,6 +593,16 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
           piece_max(2, mx0, mx1);
           tmem_wait_ld_x32(piece(3));
           piece_max(3, mx2, mx3);
+          if (tail_tile(j)) {                                    // warp-uniform, last key tile of a ragged pass only
+#pragma unroll
+            for (int c = 0; c < kBlockN; ++c)
+              if (c >= prm.k_tail) s[c] = 0xff800000u;           // -inf
+            mx0 = mx1 = mx2 = mx3 = -CUDART_INF_F;
+            piece_max(0, mx0, mx1);
+            piece_max(1, mx2, mx3);
+            piece_max(2, mx0, mx1);
+            piece_max(3, mx2, mx3);
+          }
           const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
           const bool grow = (mx - m_raw) * scale_log2 > kRescaleThreshold;
           if (__any_sync(0xffffffffu, grow)) {
@@ -653,7 +689,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         } else if (kFold) {
           const float4* src = reinterpret_cast<const float4*>(prm.o_acc + acc_row * kD + c * 32);
 #pragma unroll
-          for (int i = 0; i < 8; ++i) acc[i] = __ldcs(src + i);
+          for (int i = 0; i < 8; ++i) acc[i] = row_valid() ? __ldcs(src + i) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
         tmem_wait_ld();
         float r[32];
@@ -668,6 +704,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
             r[i * 4 + 3] = fmaf(ca, acc[i].w, r[i * 4 + 3]);
           }
         }
+        if (!row_valid()) continue;
         if (kOutBf16) {
           uint4* dst = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(prm.o_out) + row * kD + c * 32);
 #pragma unroll
@@ -686,7 +723,7 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
         }
       }
       if (kOaccSmem) mbar_arrive(oacc_empty);        // my part of the o_acc tile is in registers / consumed
-      if (hh == 0) prm.lse_out[row] = lse_row;
+      if (hh == 0 && row_valid()) prm.lse_out[row] = lse_row;
       tc_fence_before();                             // my reads of O_t are ordered before the P I will signal next
       cur = next_item(li);
     }
@@ -699,16 +736,23 @@ attn_chunk_fwd_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_co
   if (warp == Cfg::kProducerWarp) tmem_dealloc<512>(tmem);
 }
 
-template <int kD, int kEpi>
-cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& moacc,
-                     const FwdParams& prm, dim3 grid, cudaStream_t stream) {
+template <int kD, int kEpi, bool kTail>
+cudaError_t launch_tt(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& moacc,
+                      const FwdParams& prm, dim3 grid, cudaStream_t stream) {
   using Cfg = FwdCfg<kD>;
-  auto kern = attn_chunk_fwd_kernel<kD, kEpi>;
+  auto kern = attn_chunk_fwd_kernel<kD, kEpi, kTail>;
   static unsigned char configured[kMaxDevices];
   if (cudaError_t e = set_max_dyn_smem_once(kern, Cfg::kSmemBytes, configured); e != cudaSuccess) return e;
   kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(mq, mk, mv, moacc, prm);
   count_launch();
   return cudaGetLastError();
+}
+
+template <int kD, int kEpi>
+cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& moacc,
+                     const FwdParams& prm, dim3 grid, cudaStream_t stream) {
+  if (prm.k_tail) return launch_tt<kD, kEpi, true>(mq, mk, mv, moacc, prm, grid, stream);
+  return launch_tt<kD, kEpi, false>(mq, mk, mv, moacc, prm, grid, stream);
 }
 
 template <int kD>
@@ -732,17 +776,20 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
                                         const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride,
                                         int k_off, int nk, int d, float scale, int epilogue, int splits,
                                         cudaStream_t stream) {
-  if (splits < 1 || (splits > 1 && epilogue != kFwdEpiPartial) || (nk / 128) % splits) return cudaErrorInvalidValue;
+  const int n_tiles = (nk + kBlockN - 1) / kBlockN;      // the last one may be ragged (then k_off + nk == nk_stride)
+  if (splits < 1 || (splits > 1 && (epilogue != kFwdEpiPartial || nk % kBlockN)) || n_tiles % splits) return cudaErrorInvalidValue;
+  if (nk % kBlockN && k_off + nk != nk_stride) return cudaErrorInvalidValue;
   CUtensorMap mq, mk, mv, moacc;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
-  if (!make_tmap_2d(&mq, q, dt, 2, (uint64_t)BH * Nq, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mk, k, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mv, v, dt, 2, (uint64_t)BH * nk_stride, d, 128, 64, kSwizzle128B))
+  // [BH][rows][d] views: a tile that runs past the end of a head reads zeros there, not the next head's rows
+  if (!make_tmap_3d(&mq, q, dt, 2, BH, Nq, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mk, k, dt, 2, BH, nk_stride, d, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mv, v, dt, 2, BH, nk_stride, d, 128, 64, kSwizzle128B))
     return cudaErrorInvalidValue;
   const bool fold = epilogue == kFwdEpiFold || epilogue == kFwdEpiFoldFinal;
   moacc = mq;                                  // (unused unless d = 64 and the epilogue folds)
   if (fold && d == 64 &&
-      !make_tmap_2d(&moacc, o_acc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (uint64_t)BH * Nq, d, 128, 32, kSwizzle128B))
+      !make_tmap_3d(&moacc, o_acc, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, BH, Nq, d, 128, 32, kSwizzle128B))
     return cudaErrorInvalidValue;
   FwdParams prm;
   prm.o_out = o_out;
@@ -752,9 +799,10 @@ cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void
   prm.Nq = Nq;
   prm.nk_stride = nk_stride;
   prm.k_off = k_off;
-  prm.n_kv = nk / kBlockN / splits;
+  prm.n_kv = n_tiles / splits;
+  prm.k_tail = nk % kBlockN;
   prm.scale_log2 = scale * 1.4426950408889634f;
-  const dim3 grid(Nq / (2 * kBlockM), BH, splits);      // one CTA per item; most are cancelled and taken over (see the top)
+  const dim3 grid((Nq + 2 * kBlockM - 1) / (2 * kBlockM), BH, splits);      // one CTA per item; most are cancelled and taken over (see the top)
   if (d == 64) return launch_d<64>(epilogue, mq, mk, mv, moacc, prm, grid, stream);
   return launch_d<128>(epilogue, mq, mk, mv, moacc, prm, grid, stream);
 }

@@ -27,10 +27,12 @@ cudaError_t launch_eq5_finalize(const float* num, const float* den, const float*
 cudaError_t launch_split_merge(const float* parts, const float* lses, long long rows, int d, int splits,
                                const float* o_acc, const float* lse_acc, void* o_out, float* lse_out, int out_dtype,
                                cudaStream_t stream);
-// D = scale * rowsum(dO*O), lse2 = lse * log2(e); zeroes dq_acc when zero_dq.
+// D = scale * rowsum(dO*O), lse2 = lse * log2(e); zeroes dq_acc when zero_dq.  rows_per_head > 0: D, lse2 are laid out
+// [rows / rows_per_head][rows_per_head rounded up to 128] with lse2 = +inf, D = 0 in the padding (ragged sequences: what
+// launch_attn_chunk_bwd_sm100 reads); 0: flat [rows].
 cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* lse, float* D, float* lse2,
                                   float* dq_acc, long long rows, int d, float scale, bool zero_dq,
-                                  cudaStream_t stream);
+                                  cudaStream_t stream, long long rows_per_head = 0);
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
 // Deterministic dQ (int32 fixed-point accumulator, merge.cu).  launch_dq_fixed_scale: kvmax [2*BH] (scratch) and the
 // per-row scales qs [BH*rows_per_head] from k (rows d_k wide), v (d_v wide) rows [k_off, k_off+nk) of every head and dO
@@ -114,6 +116,9 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
 // ---- tensor maps (api.cu): 2-D row-major [rows, cols] view, box = {box_cols, box_rows}
 enum TmapSwizzle { kSwizzleNone = 0, kSwizzle128B = 1 };
 bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t rows,
+                  uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz);
+// 3-D view [heads][rows][cols], box = {box_cols, box_rows, 1}: rows past the end of a head read as zero and are not written
+bool make_tmap_3d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t heads, uint64_t rows,
                   uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz);
 
 void count_launch(int n = 1);

@@ -237,7 +237,7 @@ template <int kLanes>
 __global__ void __launch_bounds__(256)
 bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO, const float* __restrict__ lse,
                       float* __restrict__ D, float* __restrict__ lse2, float4* __restrict__ dq_acc, long long rows,
-                      float scale, bool zero_dq) {
+                      float scale, bool zero_dq, long long rows_per_head, long long n_stat) {
   constexpr int kRowsPerWarp = 32 / kLanes;
   const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
   const long long warp_global = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -273,10 +273,23 @@ bwd_preprocess_kernel(const uint4* __restrict__ o, const uint4* __restrict__ dO,
 #pragma unroll
       for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
       if (r < rows && l == 0) {
-        D[r] = s * scale;                          // phase B of the backward forms scale*dP - scale*D
-        lse2[r] = lse[r] * 1.4426950408889634f;   // the backward kernel works in the exp2 domain
+        // D, lse2 are [heads][n_stat]: n_stat = rows_per_head rounded up to the 128-row tile (equal unless the sequence
+        // is ragged), so that the backward kernel's 128-entry loads of a head's last tile stay inside the head
+        const long long rs = n_stat == rows_per_head ? r : (r / rows_per_head) * n_stat + r % rows_per_head;
+        D[rs] = s * scale;                         // phase B of the backward forms scale*dP - scale*D
+        lse2[rs] = lse[r] * 1.4426950408889634f;  // the backward kernel works in the exp2 domain
       }
     }
+  }
+}
+
+// the padding of a ragged head in D, lse2: lse2 = +inf makes P = exp2(x - lse2) = 0 for query rows that do not exist
+__global__ void __launch_bounds__(128)
+bwd_stat_pad_kernel(float* __restrict__ D, float* __restrict__ lse2, int rows_per_head, int n_stat) {
+  const int n = rows_per_head + threadIdx.x;
+  if (n < n_stat) {
+    D[(long long)blockIdx.x * n_stat + n] = 0.f;
+    lse2[(long long)blockIdx.x * n_stat + n] = CUDART_INF_F;
   }
 }
 
@@ -312,8 +325,9 @@ kv_absmax_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v, unsig
   const long long head0 = (long long)bh * nk_stride + k_off;
   float vmax2 = 0.f, kmax = 0.f;
   for (int base = (blockIdx.x * 8 + (threadIdx.x >> 5)) * kRowsPerWarp; base < nk; base += gridDim.x * 8 * kRowsPerWarp) {
-    const int r = base + sub;      // nk % 128 == 0: every lane has a row
-    const uint4 b = __ldg(v + (head0 + r) * kLanesV + l);
+    const int r = base + sub;
+    uint4 b = make_uint4(0u, 0u, 0u, 0u);
+    if (r < nk) b = __ldg(v + (head0 + r) * kLanesV + l);
     const uint32_t* pb = reinterpret_cast<const uint32_t*>(&b);
     float s = 0.f;
 #pragma unroll
@@ -469,17 +483,21 @@ cudaError_t launch_split_merge(const float* parts, const float* lses, long long 
 
 cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* lse, float* D, float* lse2,
                                   float* dq_acc, long long rows, int d, float scale, bool zero_dq,
-                                  cudaStream_t stream) {
+                                  cudaStream_t stream, long long rows_per_head) {
+  const long long n_stat = rows_per_head <= 0 ? rows : (rows_per_head + 127) / 128 * 128;
+  if (rows_per_head <= 0) rows_per_head = rows;
+  if (n_stat != rows_per_head)
+    bwd_stat_pad_kernel<<<(unsigned)(rows / rows_per_head), 128, 0, stream>>>(D, lse2, (int)rows_per_head, (int)n_stat);
   const int lanes = d / 8;   // 8 or 16
   const long long rows_per_block = 8LL * (32 / lanes) * 4;
   long long blocks = (rows + rows_per_block - 1) / rows_per_block;
   if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
   if (lanes == 8)
     bwd_preprocess_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, lse, D, lse2,
-                                                                   (float4*)dq_acc, rows, scale, zero_dq);
+                                                                   (float4*)dq_acc, rows, scale, zero_dq, rows_per_head, n_stat);
   else
     bwd_preprocess_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)o, (const uint4*)dO, lse, D, lse2,
-                                                                    (float4*)dq_acc, rows, scale, zero_dq);
+                                                                    (float4*)dq_acc, rows, scale, zero_dq, rows_per_head, n_stat);
   return cudaGetLastError();
 }
 

@@ -22,7 +22,10 @@ def _default_chunk(n: int) -> int:
     c = 32768
     while c > 128 and n % c:
         c //= 2
-    return c if n % c == 0 else n
+    if n % c == 0:
+        return c
+    # a ragged length (bf16 entries take any N): passes of 32768 keys, the last one shorter
+    return min(32768, (n + 127) // 128 * 128)
 
 
 class _RingXAttention(torch.autograd.Function):

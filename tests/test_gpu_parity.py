@@ -181,6 +181,39 @@ def test_fwd_bf16_matches_oracle(rx, B, H, N, d, chunk, gain):
     check_fwd(o, lse, o_ref, lse_ref, f64(v), "bf16")
 
 
+RAGGED_SHAPES = [
+    # B, H, N, d, kv_chunk, qk_gain: sequence lengths that are no multiple of the 128-key / 256-row tiles
+    (1, 1, 1, 64, 128, 1.0),               # one token: O = V, LSE = scale q.k
+    (1, 2, 100, 128, 128, 1.0),            # less than one tile
+    (1, 1, 257, 64, 128, 1.0),             # one row and one key past two tiles, 3 passes (the last of one key)
+    (2, 3, 1000, 64, 256, 1.0),            # 4 passes, the last one 232 keys (one full and one ragged tile)
+    (1, 2, 1337, 128, 512, 3.0),           # peaked softmax; last pass 313 keys
+    (1, 2, 640, 128, 256, 1.0),            # N % 128 == 0 but not % 256: the second query tile of the last item is empty
+    (1, 2, 2049, 64, 2176, 1.0),           # single pass of 17 key tiles, the last with one key
+    (1, 1, 3000, 128, 3072, 0.05),         # single pass, nearly uniform softmax
+]
+
+
+@pytest.mark.parametrize("B,H,N,d,chunk,gain", RAGGED_SHAPES)
+def test_fwd_bf16_ragged_lengths_match_oracle(rx, B, H, N, d, chunk, gain):
+    """Any sequence length: tiles that run past the end of a head read zeros (3-D tensor maps), the keys past the end
+    are masked to -inf in the pass's last key tile, rows past the end are never stored.  The tensors sit in the middle
+    of a sentinel-filled buffer so that a store past the end of a head (into the next head or past the tensor) shows."""
+    q, k, v = (wl.make_tensor((B, H, N, d), w, seed=19, dtype="bf16", gain=(gain if w != "v" else 1.0)) for w in "qkv")
+    scale = 1.0 / math.sqrt(d)
+    guard_o = torch.full((B * H * N * d + 4096,), 555.0, dtype=torch.bfloat16, device="cuda")
+    o = guard_o[2048:2048 + B * H * N * d].view(B, H, N, d)
+    guard_l = torch.full((B * H * N + 2048,), 555.0, dtype=torch.float32, device="cuda")
+    lse = guard_l[1024:1024 + B * H * N].view(B, H, N)
+    rx.ringx_attn_fwd(q.cuda(), k.cuda(), v.cuda(), chunk, scale, o=o, lse=lse)
+    torch.cuda.synchronize()
+    assert rx.ringx_last_launch_count() == -(-N // chunk)
+    assert (guard_o[:2048] == 555.0).all() and (guard_o[2048 + B * H * N * d:] == 555.0).all()
+    assert (guard_l[:1024] == 555.0).all() and (guard_l[1024 + B * H * N:] == 555.0).all()
+    o_ref, lse_ref = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
+    check_fwd(o, lse, o_ref, lse_ref, f64(v), "bf16")
+
+
 def test_fwd_bf16_chunk_partials_and_merge_are_the_papers_quantities(rx):
     """ringx_attn_chunk_fwd returns (loc_out_i, loc_lse_i) of PAPER.md:135 with Nq != Nk; merging them with
     ringx_lse_merge reproduces the oracle's Eq. 5 result."""
@@ -304,7 +337,10 @@ def test_fwd_host_entry_matches_device_entry(rx):
 def test_errors_on_the_gpu_box(rx):
     q = torch.zeros(1, 1, 512, 64, dtype=torch.bfloat16, device="cuda")
     with pytest.raises(rx.RingxError) as e:
-        rx.ringx_attn_fwd(q, q, q, 384, 0.125)
+        rx.ringx_attn_fwd(q, q, q, 200, 0.125)            # kv_chunk must be a multiple of the 128-key tile
+    assert e.value.status == 2
+    with pytest.raises(rx.RingxError) as e:
+        rx.ringx_attn_fwd(q, q, q, 640, 0.125)            # ... and no longer than the sequence rounded up to a tile
     assert e.value.status == 2
     with pytest.raises(rx.RingxError) as e:
         rx.ringx_attn_fwd(q, q, q, 256, 0.125, workspace=torch.empty(256, dtype=torch.uint8, device="cuda"))
@@ -362,15 +398,56 @@ def test_bwd_bf16_matches_oracle(rx, B, H, N, d, chunk, gain):
                    for w in ("q", "k", "v", "do"))
     scale = 1.0 / math.sqrt(d)
     qd, kd, vd, dod = q.cuda(), k.cuda(), v.cuda(), do.cuda()
-    if N % 256 == 0:
-        o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
-    else:   # the bf16 forward needs N % 256 == 0: take (o, lse) of this shape from the oracle instead
-        o64, lse64 = orc.attention_fwd_bhnd(f64(q), f64(k), f64(v), scale)
-        o, lse = torch.from_numpy(o64).to(torch.bfloat16).cuda(), torch.from_numpy(lse64).float().cuda()
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
     dq, dk, dv = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale)
     assert rx.ringx_last_launch_count() == N // chunk + 2
     worst = check_grads_full(dq, dk, dv, f64(q), f64(k), f64(v), f64(do), scale)
     assert max(worst.values()) <= 8e-3, worst        # expected ~2.4e-3 (bf16 P, dS and outputs); 5e-3 when peaked
+
+
+BWD_RAGGED_SHAPES = [
+    # B, H, N, d, kv_chunk, qk_gain: sequence lengths that are no multiple of the 128-row tile
+    (1, 1, 1, 64, 128, 1.0),               # one token: dq = dk = 0, dv = dO
+    (1, 2, 100, 128, 128, 1.0),            # less than one tile
+    (1, 1, 257, 64, 128, 1.0),             # one row and one key past two tiles; the last pass has one key
+    (2, 3, 1000, 64, 256, 1.0),            # 4 passes, the last one 232 keys
+    (1, 2, 1337, 128, 512, 3.0),           # peaked softmax
+    (1, 2, 2049, 128, 2176, 1.0),          # single pass of 17 key tiles, the last with one key
+]
+
+
+@pytest.mark.parametrize("B,H,N,d,chunk,gain", BWD_RAGGED_SHAPES)
+def test_bwd_bf16_ragged_lengths_match_oracle(rx, B, H, N, d, chunk, gain):
+    """Forward + backward of any sequence length: query rows and keys past the end of a head are read as zeros, get
+    P = 0 (lse2 = +inf in the padding of the per-head statistics; a select on the key rows of the ragged key tile) and
+    are neither stored nor reduce-added.  Gradients sit in sentinel-guarded buffers; the default and the deterministic
+    mode (fixed-point dQ) are both checked element by element."""
+    q, k, v, do = (wl.make_tensor((B, H, N, d), w, seed=59, dtype="bf16", gain=(gain if w in "qk" else 1.0))
+                   for w in ("q", "k", "v", "do"))
+    scale = 1.0 / math.sqrt(d)
+    qd, kd, vd, dod = q.cuda(), k.cuda(), v.cuda(), do.cuda()
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, chunk, scale)
+    n = B * H * N * d
+    refs = orc.attention_bwd_bhnd(f64(q), f64(k), f64(v), f64(do), scale)
+    for det in (False, True):
+        guards = [torch.full((n + 4096,), 555.0, dtype=torch.bfloat16, device="cuda") for _ in range(3)]
+        dq, dk, dv = (g[2048:2048 + n].view(B, H, N, d) for g in guards)
+        rx.ringx_set_deterministic(det)
+        try:
+            rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale, dq=dq, dk=dk, dv=dv)
+            torch.cuda.synchronize()
+            assert rx.ringx_last_launch_count() == -(-N // chunk) + 2 + (1 if N % 128 else 0) + (2 if det else 0)
+            if det:
+                dq2, _, _ = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, chunk, scale)
+                assert torch.equal(dq2, dq)
+        finally:
+            rx.ringx_set_deterministic(False)
+        for g in guards:
+            assert (g[:2048] == 555.0).all() and (g[2048 + n:] == 555.0).all()
+        if N == 1:
+            assert not dq.float().any() and not dk.float().any() and torch.equal(dv, dod)
+        else:
+            check_grads_full(dq, dk, dv, f64(q), f64(k), f64(v), f64(do), scale, refs=refs)
 
 
 @pytest.mark.parametrize("d", [64, 128])

@@ -492,7 +492,8 @@ def test_ringx_dist_over_nccl_world_size_one(rx):
 
 
 # ------------------------------------------------------------------------------------------------ GQA (NEXT-3)
-@pytest.mark.parametrize("Hq,Hkv,N,d,chunk", [(4, 2, 512, 64, 256), (6, 2, 256, 128, 128), (8, 1, 512, 64, 512)])
+@pytest.mark.parametrize("Hq,Hkv,N,d,chunk", [(4, 2, 512, 64, 256), (6, 2, 256, 128, 128), (8, 1, 512, 64, 512),
+                                              (4, 2, 333, 128, 128), (6, 3, 700, 64, 384)])   # the last two: ragged lengths
 def test_gqa_forward_and_backward_match_oracle(rx, Hq, Hkv, N, d, chunk):
     """Hq query heads share Hkv kv heads (query head h attends kv head h // (Hq/Hkv)); the oracle is the plain
     attention of every query head against its kv head, dk/dv summed over the heads of the group."""

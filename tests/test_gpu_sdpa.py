@@ -26,7 +26,8 @@ def relf(a, ref):
     return np.linalg.norm(a - ref) / np.linalg.norm(ref)
 
 
-@pytest.mark.parametrize("B,Hq,Hkv,N,d,chunk", [(1, 2, 2, 1024, 64, 256), (2, 4, 2, 512, 128, None), (1, 6, 2, 768, 64, 768)])
+@pytest.mark.parametrize("B,Hq,Hkv,N,d,chunk", [(1, 2, 2, 1024, 64, 256), (2, 4, 2, 512, 128, None), (1, 6, 2, 768, 64, 768),
+                                                (2, 2, 2, 777, 128, None), (1, 4, 2, 1500, 64, 512)])   # ragged lengths
 def test_sdpa_forward_and_gradients(sdpa, B, Hq, Hkv, N, d, chunk):
     q = wl.make_tensor((B, Hq, N, d), "q", seed=41).cuda().requires_grad_()
     k = wl.make_tensor((B, Hkv, N, d), "k", seed=41).cuda().requires_grad_()

@@ -65,6 +65,7 @@ def test_version_and_status_strings(lib):
 
 
 def test_workspace_queries_are_host_only(lib):
+    align = lambda n: (n + 255) // 256 * 256
     f = lib.ringx_attn_fwd_workspace_bytes
     # single pass needs no workspace; multi-pass bf16 needs the running fp32 accumulator [R,d] + [R]
     # (Eq. 5 is folded in the chunk kernel's epilogue: no separate partial buffer)
@@ -75,8 +76,12 @@ def test_workspace_queries_are_host_only(lib):
     # unsupported shapes report 0 (and the compute entry points reject them)
     assert f(1, 1, 1000, 64, 250, 1) == 0
     assert f(1, 1, 1024, 96, 256, 1) == 0
-    assert f(1, 1, 1024, 64, 384, 1) == 0                         # N % kv_chunk != 0
-    assert f(1, 1, 384, 64, 128, 1) == 0                          # bf16 needs N % 256 == 0
+    assert f(1, 1, 1024, 64, 1152, 1) == 0                        # kv_chunk longer than the sequence rounded up to a tile
+    assert f(1, 1, 1024, 64, 384, 0) == 0                         # fp32: N % kv_chunk != 0
+    # bf16 takes any sequence length and a short last chunk: the running accumulator for the rows that exist
+    assert f(1, 1, 1024, 64, 384, 1) == 1024 * 64 * 4 + 1024 * 4
+    assert f(1, 1, 1000, 64, 256, 1) == 1000 * 64 * 4 + align(1000 * 4)
+    assert f(1, 1, 100, 128, 128, 1) == 0                         # one (ragged) pass
     b = lib.ringx_attn_bwd_workspace_bytes
     # D, lse2, the dQ accumulator (fp32, or int32 fixed point in deterministic mode), the per-row fixed-point scales
     # and the two K/V maxima per head
