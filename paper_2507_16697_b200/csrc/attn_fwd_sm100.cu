@@ -3,6 +3,8 @@
 // For every query row of a [128 x 2]-row work item and the keys [k_off, k_off + nk) of its head:
 //   loc_out = softmax(scale q K_c^T) V_c,  loc_lse = log sum_j exp(scale q.k_j)      (Eq. 1/3/4)
 // bf16 operands, fp32 accumulation ("mixed float32-bfloat16").
+// Any sequence length: Q, K, V are addressed through [BH][rows][d] tensor maps, so rows and keys past the end of a head
+// read as zeros; such rows are computed like any other and never stored, such keys get a score of -inf (kTail).
 //
 // PERSISTENT kernel with hardware work stealing (cluster launch control).  The grid is one CTA per work item (item =
 // 256 query rows of one head [x one key split]; blockIdx.x = query tile, so the CTAs running at any time share one

@@ -74,6 +74,9 @@ cudaError_t launch_attn_chunk_f32(const float* q, const float* k, const float* v
 enum { kFwdEpiPartial = 0, kFwdEpiFinal = 1, kFwdEpiFold = 2, kFwdEpiFoldFinal = 3 };
 // splits > 1 (kFwdEpiPartial only): split z of the grid takes keys [k_off + z*nk/splits, +nk/splits) and writes its
 // partials to o_out + z*BH*Nq*d, lse_out + z*BH*Nq (launch_split_merge combines them).
+// Any Nq >= 1; nk % 128 != 0 only for the head's last keys (k_off + nk == nk_stride) and with splits == 1: rows and keys
+// past the end of a head are read as zeros through [BH][rows][d] tensor maps, the missing keys are masked (kTail
+// instantiation), rows past the end are not written.
 cudaError_t launch_attn_chunk_fwd_sm100(const void* q, const void* k, const void* v, void* o_out, float* lse_out,
                                         const float* o_acc, const float* lse_acc, int BH, int Nq, int nk_stride,
                                         int k_off, int nk, int d, float scale, int epilogue, int splits,
@@ -108,6 +111,7 @@ cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int
 // dq_qs: nullptr, or [BH * N] per-row scales (launch_dq_fixed_scale): dq_acc is then an int32 fixed-point
 // accumulator and the reduce-adds are integer adds -- bit-reproducible dQ in any arrival order.
 // dkv_dtype: RINGX_BF16 (dk, dv bf16) or RINGX_F32 (fp32: one device's share of a cross-device sum).
+// Any N >= 1 (lse2, D then in launch_bwd_preprocess's per-head padded layout); nk % 128 != 0 only for the head's last keys.
 cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void* v, const void* dO, const float* lse2,
                                         const float* D, float* dq_acc, void* dk, void* dv, int BH, int N,
                                         int nk_stride, int k_off, int nk, int d, float scale, const float* dq_qs,
