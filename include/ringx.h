@@ -32,8 +32,8 @@
  *              with RINGX_BF16 take ANY sequence length N >= 1 and any kv_chunk <= N rounded up to 128:
  *              there are ceil(N / kv_chunk) passes, the last one over the keys that are left; tiles
  *              that run past the end of a head read zeros (3-D tensor maps), keys past the end are
- *              masked, rows past the end are never written.  Every other entry (fp32, the per-chunk /
- *              per-device steps, the *_host, MLA and block entries) needs N % 128 == 0 (N % 256 == 0 for a
+ *              masked, rows past the end are never written (the *_host entries likewise).  Every other entry
+ *              (fp32, the per-chunk / per-device steps, MLA and block entries) needs N % 128 == 0 (N % 256 == 0 for a
  *              bf16 forward: one CTA owns two 128-row query tiles), 0 < kv_chunk <= N and N % kv_chunk == 0
  *              (every device holds an equal chunk S/N, l.128).  Anything else returns
  *              RINGX_ERR_BAD_SHAPE -- never a silently wrong answer.  A device that is not

@@ -371,7 +371,7 @@ size_t ringx_attn_bwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, 
 }
 
 size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
-  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false) != RINGX_OK) return 0;
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false, true) != RINGX_OK) return 0;
   const size_t e = dtype == RINGX_F32 ? 4 : 2;
   const size_t R = (size_t)B * H * N;
   return 4 * align_up(R * d * e) + align_up(R * sizeof(float)) + carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype).bytes;
@@ -1017,7 +1017,7 @@ int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_ho
                         size_t workspace_bytes, void* stream_) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!q_host || !k_host || !v_host || !o_host || !lse_host) return RINGX_ERR_NULL_PTR;
-  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false);
+  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false, true);
   if (st != RINGX_OK) return st;
   const size_t need = ringx_attn_fwd_host_workspace_bytes(B, H, N, d, kv_chunk, dtype);
   if (!workspace) return RINGX_ERR_NULL_PTR;
@@ -1034,7 +1034,7 @@ int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_ho
   // q and the K,V rows of chunk c go up on a side stream in the order the passes need them (pass c waits for chunk c
   // only), so all but the first chunk's transfer is hidden behind the kernels.
   cudaError_t ce;
-  const int n_chunks = N / kv_chunk;
+  const int n_chunks = (N + kv_chunk - 1) / kv_chunk;      // the last chunk may be short (ragged lengths)
   const bool pipelined = n_chunks >= 2 && n_chunks <= 64;
   if (pipelined) {
     HostOverlap& ov = tl_overlap;
@@ -1045,10 +1045,10 @@ int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_ho
     if ((ce = cudaStreamWaitEvent(ov.side, ov.events[2], 0)) != cudaSuccess) return cuda_status(ce);
     if ((ce = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, ov.side)) != cudaSuccess) return cuda_status(ce);
     for (int c = 0; c < n_chunks; ++c) {
-      const size_t off = (size_t)c * chunk_bytes;
+      const size_t off = (size_t)c * chunk_bytes, this_bytes = c + 1 < n_chunks ? chunk_bytes : head_pitch - off;
       for (int w = 0; w < 2; ++w)
         if ((ce = cudaMemcpy2DAsync(static_cast<char*>(w == 0 ? dk : dv) + off, head_pitch,
-                                    static_cast<const char*>(w == 0 ? k_host : v_host) + off, head_pitch, chunk_bytes,
+                                    static_cast<const char*>(w == 0 ? k_host : v_host) + off, head_pitch, this_bytes,
                                     (size_t)B * H, cudaMemcpyHostToDevice, ov.side)) != cudaSuccess)
           return cuda_status(ce);
       if ((ce = cudaEventRecord(kv_ready[c], ov.side)) != cudaSuccess) return cuda_status(ce);
@@ -1070,8 +1070,8 @@ int ringx_attn_fwd_host(const void* q_host, const void* k_host, const void* v_ho
 }
 
 size_t ringx_attn_fwd_bwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype) {
-  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, true) != RINGX_OK ||
-      check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false) != RINGX_OK)
+  if (check_shape(B, H, N, d, kv_chunk, 1.f, dtype, true, true) != RINGX_OK ||
+      check_shape(B, H, N, d, kv_chunk, 1.f, dtype, false, true) != RINGX_OK)
     return 0;
   const size_t R = (size_t)B * H * N;
   const size_t fw = carve_fwd(nullptr, B, H, N, d, kv_chunk, dtype).bytes, bw = carve_bwd(nullptr, B, H, N, d).bytes;
@@ -1085,8 +1085,8 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!q_host || !k_host || !v_host || !dO_host || !o_host || !lse_host || !dq_host || !dk_host || !dv_host)
     return RINGX_ERR_NULL_PTR;
-  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, true);
-  if (st == RINGX_OK) st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false);
+  int st = check_shape(B, H, N, d, kv_chunk, scale, dtype, true, true);
+  if (st == RINGX_OK) st = check_shape(B, H, N, d, kv_chunk, scale, dtype, false, true);
   if (st != RINGX_OK) return st;
   const size_t need = ringx_attn_fwd_bwd_host_workspace_bytes(B, H, N, d, kv_chunk, dtype);
   if (!workspace) return RINGX_ERR_NULL_PTR;
@@ -1106,7 +1106,7 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   // come down while the later passes run.  Only dq is copied after the last kernel.
   HostOverlap& ov = tl_overlap;
   cudaError_t ce;
-  const int n_chunks = N / kv_chunk;
+  const int n_chunks = (N + kv_chunk - 1) / kv_chunk;      // the last chunk may be short (ragged lengths)
   const bool pipelined = n_chunks >= 2 && n_chunks <= 64;
   if ((st = overlap_prepare(ov, 3 + (pipelined ? 2 * n_chunks : 0))) != RINGX_OK) return st;
   cudaEvent_t ev_do_up = ov.events[0], ev_fwd_done = ov.events[1], ev_down = ov.events[2];
@@ -1123,10 +1123,10 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   if ((ce = up(t[0], q_host, tb)) != cudaSuccess) return cuda_status(ce);
   if (pipelined) {
     for (int c = 0; c < n_chunks; ++c) {
-      const size_t off = (size_t)c * chunk_bytes;
+      const size_t off = (size_t)c * chunk_bytes, this_bytes = c + 1 < n_chunks ? chunk_bytes : head_pitch - off;
       for (int w = 1; w <= 2; ++w) {
         const char* src_ = static_cast<const char*>(w == 1 ? k_host : v_host) + off;
-        if ((ce = cudaMemcpy2DAsync(static_cast<char*>(t[w]) + off, head_pitch, src_, head_pitch, chunk_bytes, BH,
+        if ((ce = cudaMemcpy2DAsync(static_cast<char*>(t[w]) + off, head_pitch, src_, head_pitch, this_bytes, BH,
                                     cudaMemcpyHostToDevice, ov.side)) != cudaSuccess)
           return cuda_status(ce);
       }
@@ -1161,11 +1161,11 @@ int ringx_attn_fwd_bwd_host(const void* q_host, const void* k_host, const void* 
   // ---- device -> host (the waits are enqueued after the records they refer to)
   if (pipelined) {
     for (int c = 0; c < n_chunks; ++c) {
-      const size_t off = (size_t)c * chunk_bytes;
+      const size_t off = (size_t)c * chunk_bytes, this_bytes = c + 1 < n_chunks ? chunk_bytes : head_pitch - off;
       if ((ce = cudaStreamWaitEvent(ov.side, pass_done[c], 0)) != cudaSuccess) return cuda_status(ce);
       for (int w = 0; w < 2; ++w) {
         char* dst_ = static_cast<char*>(w == 0 ? dk_host : dv_host) + off;
-        if ((ce = cudaMemcpy2DAsync(dst_, head_pitch, static_cast<const char*>(t[6 + w]) + off, head_pitch, chunk_bytes,
+        if ((ce = cudaMemcpy2DAsync(dst_, head_pitch, static_cast<const char*>(t[6 + w]) + off, head_pitch, this_bytes,
                                     BH, cudaMemcpyDeviceToHost, ov.side)) != cudaSuccess)
           return cuda_status(ce);
       }
