@@ -32,8 +32,9 @@
  *              with RINGX_BF16 take ANY sequence length N >= 1 and any kv_chunk <= N rounded up to 128:
  *              there are ceil(N / kv_chunk) passes, the last one over the keys that are left; tiles
  *              that run past the end of a head read zeros (3-D tensor maps), keys past the end are
- *              masked, rows past the end are never written (the *_host entries likewise).  Every other entry
- *              (fp32, the per-chunk / per-device steps, MLA and block entries) needs N % 128 == 0 (N % 256 == 0 for a
+ *              masked, rows past the end are never written (the *_host entries and the bf16 per-device
+ *              steps ringx_attn_chunk_fwd*, ringx_attn_bwd_partial* likewise).  Every other entry
+ *              (fp32, MLA and block entries) needs N % 128 == 0 (N % 256 == 0 for a
  *              bf16 forward: one CTA owns two 128-row query tiles), 0 < kv_chunk <= N and N % kv_chunk == 0
  *              (every device holds an equal chunk S/N, l.128).  Anything else returns
  *              RINGX_ERR_BAD_SHAPE -- never a silently wrong answer.  A device that is not
@@ -172,7 +173,8 @@ RINGX_API int ringx_lse_merge(const void* o_a, const float* lse_a, const void* o
 /* One KV-chunk pass on its own: (loc_out, loc_lse) of `Nq` query rows per head against `Nk` keys
  * (l.135) -- the per-device step of RingX_a/RingX_b with Nq != Nk allowed.
  *   q [B,H,Nq,d], k,v [B,H,Nk,d] of `dtype`; loc_out [B,H,Nq,d] FLOAT; loc_lse [B,H,Nq] float.
- *   Nq % 256 == 0 (bf16) or % 128 (f32), Nk % 128 == 0, d in {64,128}.  No workspace. */
+ *   bf16: any Nq, Nk >= 1 (ragged tiles are zero-filled, masked and never stored); f32: Nq % 128 == 0, Nk % 128 == 0;
+ *   d in {64,128}.  No workspace. */
 RINGX_API int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc_out, float* loc_lse,
                          int B, int H, int Nq, int Nk, int d, float scale, int dtype, void* stream);
 
@@ -184,7 +186,7 @@ RINGX_API int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, 
  *   o_final, lse_final: both NULL -> the fold is written back to (o_acc, lse_acc) in place;
  *                       both given -> o_final [B,H,Nq,d] bf16 and lse_final receive the folded result (last step),
  *                       (o_acc, lse_acc) are left untouched.
- *   Nq % 256 == 0, Nk % 128 == 0, d in {64,128}; dtype must be RINGX_BF16.  No workspace. */
+ *   Any Nq, Nk >= 1, d in {64,128}; dtype must be RINGX_BF16.  No workspace. */
 RINGX_API int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void* v, float* o_acc, float* lse_acc,
                               void* o_final, float* lse_final,
                               int B, int H, int Nq, int Nk, int d, float scale, int dtype, void* stream);
@@ -199,7 +201,8 @@ RINGX_API int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void
  *   o_out, lse_out  result, o_out of o_out_dtype: RINGX_F32 (may be o_acc, lse_acc themselves: in-place fold) or RINGX_BF16
  *                   (the last pass; must not alias the accumulator).
  *   workspace       >= ringx_attn_chunk_fwd_ex_workspace_bytes(...) bytes, 256-byte aligned; may be NULL when that is 0.
- *   bf16 inputs only; Nq % 256 == 0, Nk % 128 == 0, d in {64,128}. */
+ *   bf16 inputs only; any Nq, Nk >= 1 (split-KV needs Nq % 256 == 0 and Nk % 128 == 0, else the pass is not split),
+ *   d in {64,128}. */
 RINGX_API int ringx_attn_chunk_fwd_ex(const void* q, const void* k, const void* v, const float* o_acc, const float* lse_acc,
                             void* o_out, float* lse_out, int B, int H, int Nq, int Nk, int d, float scale,
                             int dtype, int o_out_dtype, void* workspace, size_t workspace_bytes, void* stream);
@@ -214,7 +217,7 @@ RINGX_API size_t ringx_attn_chunk_fwd_ex_workspace_bytes(int B, int H, int Nq, i
  *          with ringx_dq_finalize after the last.  Summation order is not fixed unless ringx_set_deterministic(1).
  *   dk, dv [B,H,Nk,d] bf16 (out): the sums over the Nq query rows given (complete when the caller holds
  *          every query of the head, otherwise one device's share to be reduced across devices).
- *   Nq % 128 == 0, Nk % 128 == 0, d in {64,128}; dtype must be RINGX_BF16.
+ *   Any Nq, Nk >= 1, d in {64,128}; dtype must be RINGX_BF16.
  *   workspace  >= ringx_attn_bwd_partial_workspace_bytes(B,H,Nq,d) bytes, 256-byte aligned. */
 RINGX_API int ringx_attn_bwd_partial(const void* q, const void* k, const void* v, const void* o, const float* lse,
                            const void* dO, float* dq_acc, void* dk, void* dv,

@@ -680,7 +680,7 @@ int ringx_attn_chunk_fwd(const void* q, const void* k, const void* v, float* loc
   if (!q || !k || !v || !loc_out || !loc_lse) return RINGX_ERR_NULL_PTR;
   if (dtype != RINGX_F32 && dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
-  if (Nk % 128 || Nq % (dtype == RINGX_BF16 ? 256 : 128)) return RINGX_ERR_BAD_SHAPE;
+  if (dtype != RINGX_BF16 && (Nk % 128 || Nq % 128)) return RINGX_ERR_BAD_SHAPE;   // bf16: any Nq, Nk (ragged tiles)
   if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
     return RINGX_ERR_BAD_SHAPE;
   if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
@@ -703,7 +703,6 @@ int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void* v, float
   if (!q || !k || !v || !o_acc || !lse_acc || (o_final == nullptr) != (lse_final == nullptr)) return RINGX_ERR_NULL_PTR;
   if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
-  if (Nk % 128 || Nq % 256) return RINGX_ERR_BAD_SHAPE;
   if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
     return RINGX_ERR_BAD_SHAPE;
   if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
@@ -723,7 +722,7 @@ int ringx_attn_chunk_fwd_fold(const void* q, const void* k, const void* v, float
 }
 
 size_t ringx_attn_chunk_fwd_ex_workspace_bytes(int B, int H, int Nq, int Nk, int d, int dtype) {
-  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128) || Nk % 128) return 0;
+  if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return 0;
   return carve_split(nullptr, (size_t)B * H * Nq, d, choose_splits(B * H, Nq, Nk, dtype)).bytes;
 }
 
@@ -735,7 +734,6 @@ int ringx_attn_chunk_fwd_ex(const void* q, const void* k, const void* v, const f
   if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (o_out_dtype != RINGX_F32 && o_out_dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
-  if (Nk % 128 || Nq % 256) return RINGX_ERR_BAD_SHAPE;
   if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
     return RINGX_ERR_BAD_SHAPE;
   if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
@@ -894,7 +892,7 @@ int ringx_attn_bwd(const void* q, const void* k, const void* v, const void* o, c
 size_t ringx_attn_bwd_partial_workspace_bytes(int B, int H, int Nq, int d) {
   if (B <= 0 || H <= 0 || Nq <= 0 || (d != 64 && d != 128)) return 0;
   const size_t R = (size_t)B * H * Nq;
-  size_t bytes = 2 * align_up(R * sizeof(float));
+  size_t bytes = 2 * align_up((size_t)B * H * ((Nq + 127) / 128 * 128) * sizeof(float));   // D, lse2: heads padded to 128 rows
   // deterministic mode: per-row scales, the K/V maxima and an int32 fixed-point image of this step's dQ contribution
   if (g_deterministic.load(std::memory_order_relaxed))
     bytes += align_up(R * sizeof(float)) + align_up((size_t)B * H * 2 * sizeof(float)) + align_up(R * d * sizeof(int));
@@ -910,7 +908,6 @@ int ringx_attn_bwd_partial_ex(const void* q, const void* k, const void* v, const
   if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (dkv_dtype != RINGX_BF16 && dkv_dtype != RINGX_F32) return RINGX_ERR_BAD_DTYPE;
   if (B <= 0 || H <= 0 || Nq <= 0 || Nk <= 0 || (d != 64 && d != 128)) return RINGX_ERR_BAD_SHAPE;
-  if (Nq % 128 || Nk % 128) return RINGX_ERR_BAD_SHAPE;
   if ((long long)B * H > 65535 || (long long)B * H * Nq > 0x7FFFFFFFLL || (long long)B * H * Nk > 0x7FFFFFFFLL)
     return RINGX_ERR_BAD_SHAPE;
   if (!(scale > 0.f) || !(scale < 3.0e38f)) return RINGX_ERR_BAD_SHAPE;
@@ -925,14 +922,15 @@ int ringx_attn_bwd_partial_ex(const void* q, const void* k, const void* v, const
   if (st != RINGX_OK) return st;
   tl_launches = 0;
   float* D = static_cast<float*>(workspace);
-  const size_t rb = align_up((size_t)B * H * Nq * sizeof(float));
+  const size_t rb = align_up((size_t)B * H * ((Nq + 127) / 128 * 128) * sizeof(float));
   float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + rb);
   DetScratch det;
   if (need > 2 * rb) {      // the workspace was sized in deterministic mode
     char* p = static_cast<char*>(workspace) + 2 * rb;
+    const size_t qb = align_up((size_t)B * H * Nq * sizeof(float));
     det.qs = reinterpret_cast<float*>(p);
-    det.kvmax = reinterpret_cast<float*>(p + rb);
-    det.fix = reinterpret_cast<int*>(p + rb + align_up((size_t)B * H * 2 * sizeof(float)));
+    det.kvmax = reinterpret_cast<float*>(p + qb);
+    det.fix = reinterpret_cast<int*>(p + qb + align_up((size_t)B * H * 2 * sizeof(float)));
   }
   st = bwd_core(q, k, v, o, lse, dO, D, lse2, dq_acc, false, nullptr, dk, dv, B * H, Nq, Nk, d, Nk, scale, det, stream,
                 dkv_dtype, prepared != 0);

@@ -42,7 +42,8 @@ def relf(a, ref):
 
 # ------------------------------------------------------------------------------------------------ bwd_partial
 @pytest.mark.parametrize("d,Nq,chunks", [(64, 512, (512, 512)), (128, 256, (384, 640)), (64, 1024, (128, 256, 128)),
-                                         (128, 384, (1024,))])
+                                         (128, 384, (1024,)), (128, 300, (200, 333)), (64, 77, (1000,)),
+                                         (64, 129, (1, 127, 130))])       # the last three: ragged Nq and Nk
 def test_bwd_partial_steps_add_up_to_the_oracle_gradient(rx, d, Nq, chunks):
     """Nq query rows against Nk = sum(chunks) keys, one ringx_attn_bwd_partial call per key chunk (ragged chunk
     sizes, Nq != Nk).  dq accumulates over the calls; each call's dk, dv are complete for its keys."""
@@ -56,28 +57,23 @@ def test_bwd_partial_steps_add_up_to_the_oracle_gradient(rx, d, Nq, chunks):
     bounds = np.concatenate([[0], np.cumsum(chunks)])
     q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
     o_ref, lse_ref = orc.attention_fwd_bhnd(q64, k64, v64, scale)
-    if Nq % 256 == 0 and len(chunks) >= 2:
-        # the saved global (o, lse) of these rows from the library itself: chunk partials + Eq. 5, bf16 at the end
-        parts = [rx.ringx_attn_chunk_fwd(qd, kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous(), scale)
-                 for lo, hi in zip(bounds[:-1], bounds[1:])]
-        o_acc, lse_acc = parts[0]
-        for i, (o_p, lse_p) in enumerate(parts[1:]):
-            last = i == len(parts) - 2
-            o_acc, lse_acc = rx.ringx_lse_merge(o_acc, lse_acc, o_p, lse_p,
-                                                out_dtype=torch.bfloat16 if last else torch.float32)
-        o_dev, lse_dev = o_acc, lse_acc
-        assert np.abs(lse_dev.cpu().double().numpy() - lse_ref).max() <= 5e-5
-    else:
-        # (the bf16 forward needs 256-row query tiles: here the saved (o, lse) are the oracle's, rounded as the
-        # forward would store them)
-        o_dev = torch.from_numpy(o_ref).to(torch.bfloat16).cuda()
-        lse_dev = torch.from_numpy(lse_ref).float().cuda()
+    # the saved global (o, lse) of these rows from the library itself: chunk partials + Eq. 5, bf16 at the end
+    parts = [rx.ringx_attn_chunk_fwd(qd, kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous(), scale)
+             for lo, hi in zip(bounds[:-1], bounds[1:])]
+    o_acc, lse_acc = parts[0]
+    for i, (o_p, lse_p) in enumerate(parts[1:]):
+        last = i == len(parts) - 2
+        o_acc, lse_acc = rx.ringx_lse_merge(o_acc, lse_acc, o_p, lse_p,
+                                            out_dtype=torch.bfloat16 if last else torch.float32)
+    o_dev, lse_dev = o_acc.to(torch.bfloat16), lse_acc
+    assert np.abs(lse_dev.cpu().double().numpy() - lse_ref).max() <= 5e-5
+    assert relf(f64(o_dev), o_ref) <= 1e-2
     dq_acc = torch.zeros((B, H, Nq, d), dtype=torch.float32, device="cuda")
     dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
     for lo, hi in zip(bounds[:-1], bounds[1:]):
         _, dk, dv = rx.ringx_attn_bwd_partial(qd, kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous(), o_dev,
                                               lse_dev, dod, scale, dq_acc=dq_acc)
-        assert rx.ringx_last_launch_count() == 2           # preprocess + one chunk kernel
+        assert rx.ringx_last_launch_count() == 2 + (1 if Nq % 128 else 0)   # preprocess (+ pad of a ragged head) + chunk kernel
         assert relf(f64(dk), dk_ref[:, :, lo:hi]) <= TOL_GRAD
         assert relf(f64(dv), dv_ref[:, :, lo:hi]) <= TOL_GRAD
         assert relf(f64(dk), dk_ref[:, :, lo:hi]) <= 6e-3 and relf(f64(dv), dv_ref[:, :, lo:hi]) <= 6e-3
@@ -110,8 +106,9 @@ def test_bwd_partial_rejects_bad_arguments(rx):
     p = [x.data_ptr() for x in (t, t, t, t, lse, t, acc, t, t)]
     call = lambda Nq, Nk, d, dt, wsb: L.ringx_attn_bwd_partial(*p, 1, 1, Nq, Nk, d, 0.125, dt, ws.data_ptr(), wsb, None)
     assert call(256, 256, 64, 1, 4096) == 0
-    assert call(200, 256, 64, 1, 4096) == 2       # BAD_SHAPE
-    assert call(256, 100, 64, 1, 4096) == 2
+    assert call(200, 100, 64, 1, 4096) == 0       # any Nq, Nk (ragged tiles)
+    assert call(0, 256, 64, 1, 4096) == 2         # BAD_SHAPE
+    assert call(256, 0, 64, 1, 4096) == 2
     assert call(256, 256, 96, 1, 4096) == 2
     assert call(256, 256, 64, 0, 4096) == 3       # BAD_DTYPE: bf16 only
     assert call(256, 256, 64, 1, 16) == 5         # WORKSPACE_TOO_SMALL
@@ -120,7 +117,8 @@ def test_bwd_partial_rejects_bad_arguments(rx):
 
 # ------------------------------------------------------------------------------------------------ fused fold
 @pytest.mark.parametrize("d,Nq,chunks,gain", [(128, 512, (256, 128, 640), 1.0), (64, 256, (512, 512), 1.0),
-                                              (128, 256, (128, 128, 128, 128), 3.0)])
+                                              (128, 256, (128, 128, 128, 128), 3.0), (128, 300, (200, 333, 1), 1.0),
+                                              (64, 1000, (77, 500), 1.0)])      # the last two: ragged Nq and Nk
 def test_chunk_fwd_fold_equals_the_running_merge(rx, d, Nq, chunks, gain):
     """ringx_attn_chunk_fwd_fold = ringx_attn_chunk_fwd + two-operand Eq. 5 in one kernel: against the oracle's
     running merge over ragged chunks, and against the library's own two-kernel route (fp32 rounding apart)."""

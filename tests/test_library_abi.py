@@ -109,7 +109,8 @@ def test_argument_validation_happens_before_any_cuda_call(lib):
     assert lib.ringx_lse_merge(p, p, p, p, p, p, 8, 64, 0, 5, None) == 3
     assert lib.ringx_lse_merge(None, None, None, None, None, None, 0, 64, 0, 0, None) == 0             # rows=0 no-op
     assert lib.ringx_attn_bwd(p, p, p, p, p, p, p, p, p, 1, 1, 256, 64, 256, 0.125, 0, p, 1 << 20, None) == 3
-    assert lib.ringx_attn_chunk_fwd(p, p, p, p, p, 1, 1, 256, 100, 64, 0.125, 1, None) == 2
+    assert lib.ringx_attn_chunk_fwd(p, p, p, p, p, 1, 1, 256, 100, 64, 0.125, 0, None) == 2   # fp32: Nk % 128
+    assert lib.ringx_attn_chunk_fwd(p, p, p, p, p, 1, 1, 256, 0, 64, 0.125, 1, None) == 2
 
 
 def test_product_fails_loudly_without_the_library(monkeypatch, tmp_path):
