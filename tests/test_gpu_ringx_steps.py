@@ -252,7 +252,7 @@ class ThreadComm:
 
 
 @pytest.mark.parametrize("variant", ["a", "b"])
-@pytest.mark.parametrize("world,d,Nl", [(2, 128, 512), (4, 64, 256)])
+@pytest.mark.parametrize("world,d,Nl", [(2, 128, 512), (4, 64, 256), (3, 128, 300)])   # the last: ragged per-rank chunks
 def test_ringx_schedules_on_simulated_ranks(rx, variant, world, d, Nl):
     """RingX_a / RingX_b forward + backward with the real kernels, W sequence chunks of Nl tokens, against the
     oracle attention of the whole sequence and against the library's own single-device ringx_attn_fwd/bwd."""
