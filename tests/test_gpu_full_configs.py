@@ -271,3 +271,49 @@ def test_C3_shape_backward_d128_sampled(rx):
     dk_ref, dv_ref = orc.attention_bwd_cols(q64, k64[cols], v64[cols], do64, lse_all, D_all, scale)
     gb.check_grad("dk(cols)", np64(dk[b, h][cols]), dk_ref, gb.dk_dterm(q64, k64[cols], lse_all, E_all, scale))
     gb.check_grad("dv(cols)", np64(dv[b, h][cols]), dv_ref)
+
+
+def test_C3_minus_one_token_ragged_full_size(rx):
+    """C3's shape with one token fewer (N = 262143: every head ends one key short of a tile, the last of the 8 passes
+    has 32767 keys).  Forward + backward at full size through the kTail instantiations: O, LSE, dQ on sampled rows
+    (incl. the last rows of the ragged tile) against the oracle over all keys; the sum invariants on every head; then,
+    with dO non-zero on the sampled rows only, dK and dV of every key of a head element by element."""
+    cfg = wl.CONFIGS["C3"]
+    B, H, N, d, C = cfg.B, cfg.H, cfg.N - 1, cfg.d, cfg.kv_chunk
+    q, k, v, do = (wl.make_tensor((B, H, N, d), w, seed=cfg.seed + 3, dtype="bf16", device="cuda") for w in ("q", "k", "v", "do"))
+    o, lse = rx.ringx_attn_fwd(q, k, v, C, cfg.scale)
+    assert rx.ringx_last_launch_count() == 8
+    dq, dk, dv = rx.ringx_attn_bwd(q, k, v, o, lse, do, C, cfg.scale)
+    torch.cuda.synchronize()
+    assert rx.ringx_last_launch_count() == 8 + 3
+    for t in (o, dq, dk, dv):
+        assert torch.isfinite(t.float()).all()
+    b, h = 0, 6
+    rows = sample_rows(N, 180, seed=cfg.seed + 11)
+    k64, v64 = wl.to_f64_numpy(k[b, h]), wl.to_f64_numpy(v[b, h])
+    q64, do64 = wl.to_f64_numpy(q[b, h][rows]), wl.to_f64_numpy(do[b, h][rows])
+    o_ref, lse_ref = orc.attention_fwd(q64, k64, v64, cfg.scale)
+    dq_ref, _, _ = orc.attention_bwd(q64, k64, v64, do64, cfg.scale)
+    og = np64(o[b, h][rows])
+    assert np.linalg.norm(og - o_ref) / np.linalg.norm(o_ref) <= 1e-2
+    assert np.abs(lse[b, h][rows].cpu().double().numpy() - lse_ref).max() <= 1e-3
+    gb.check_grad("dq", np64(dq[b, h][rows]), dq_ref, gb.dq_dterm(q64, k64, v64, do64, cfg.scale))
+    sum_dv, sum_do = dv.float().sum(dim=2), do.float().sum(dim=2)
+    assert ((sum_dv - sum_do).norm() / sum_do.norm()).item() <= 1e-2
+    assert (dk.float().sum(dim=2).norm() / dk.float().abs().sum(dim=2).norm()).item() <= 1e-2
+    del dq, dk, dv
+    # sparse dO (as in test_C3_full_size_forward_and_backward): dO is non-zero on the sampled rows only, so dK, dV of EVERY key
+    # are sums over those rows, which the oracle computes exactly -- all 2048 key tiles incl. the ragged one, element by element
+    idx = torch.from_numpy(rows).cuda()
+    do_s = torch.zeros_like(do)
+    do_s[:, :, idx] = do[:, :, idx]
+    dq, dk, dv = rx.ringx_attn_bwd(q, k, v, o, lse, do_s, C, cfg.scale)
+    torch.cuda.synchronize()
+    mask = torch.ones(N, dtype=torch.bool, device="cuda")
+    mask[idx] = False
+    assert not dq[:, :, mask].float().any()
+    dq_ref, dk_ref, dv_ref = orc.attention_bwd(q64, k64, v64, do64, cfg.scale)
+    E = gb.d_error_rows(q64, k64, v64, do64, cfg.scale)
+    gb.check_grad("dq(sparse)", np64(dq[b, h][rows]), dq_ref, gb.dq_dterm(q64, k64, v64, do64, cfg.scale))
+    gb.check_grad("dk(all keys)", np64(dk[b, h]), dk_ref, gb.dk_dterm(q64, k64, lse_ref, E, cfg.scale))
+    gb.check_grad("dv(all keys)", np64(dv[b, h]), dv_ref)
