@@ -82,6 +82,22 @@ def test_bwd_partial_steps_add_up_to_the_oracle_gradient(rx, d, Nq, chunks):
     assert relf(f64(dq), dq_ref) <= 6e-3
     # the accumulator itself holds the true gradient (scale included), before the bf16 rounding
     assert relf(dq_acc.cpu().double().numpy(), dq_ref) <= 6e-3
+    if Nq % 128:
+        # the same steps with ringx_set_deterministic (int32 scratch per step, added to the fp32 accumulator): reproducible
+        accs = []
+        rx.ringx_set_deterministic(True)
+        try:
+            for _ in range(2):
+                acc = torch.zeros((B, H, Nq, d), dtype=torch.float32, device="cuda")
+                for lo, hi in zip(bounds[:-1], bounds[1:]):
+                    rx.ringx_attn_bwd_partial(qd, kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous(), o_dev, lse_dev,
+                                              dod, scale, dq_acc=acc)
+                accs.append(acc)
+            torch.cuda.synchronize()
+        finally:
+            rx.ringx_set_deterministic(False)
+        assert torch.equal(accs[0], accs[1])
+        assert relf(accs[0].cpu().double().numpy(), dq_ref) <= 6e-3
 
 
 def test_bwd_partial_equals_full_backward_when_it_sees_everything(rx):
