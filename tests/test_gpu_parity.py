@@ -708,3 +708,49 @@ def test_forward_backward_capture_into_a_cuda_graph(rx):
         for a, b in zip(got[:4], (o, lse, dk, dv)):
             assert torch.equal(a, b)
         assert ((got[4].float() - dq.float()).norm() / dq.float().norm()).item() <= 2e-3      # fp32 reduce order
+
+
+# ------------------------------------------------------------------------------------------------ seeded random shapes
+def _random_shapes(n, seed=20250716):
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(n):
+        N = int(rng.choice([rng.integers(1, 300), rng.integers(300, 1800), 128 * rng.integers(1, 12)]))
+        chunk = 128 * int(rng.integers(1, (N + 127) // 128 + 1))
+        out.append((int(rng.choice([1, 2])), int(rng.choice([1, 2, 3])), int(rng.choice([1, 1, 2, 4])), N,
+                    int(rng.choice([64, 128])), chunk, float(rng.choice([1.0, 1.0, 3.0, 0.05])), bool(rng.random() < 0.3)))
+    return out
+
+
+@pytest.mark.parametrize("B,Hkv,G,N,d,chunk,gain,det", _random_shapes(12))
+def test_seeded_random_shapes_match_oracle(rx, B, Hkv, G, N, d, chunk, gain, det):
+    """Twelve shapes drawn from a seeded generator -- any length, any chunk that is a multiple of 128, MHA and GQA,
+    diffuse and peaked softmax, default and deterministic mode -- forward and backward against the oracle (query head h
+    attends kv head h // G; dk, dv summed over the heads of a group)."""
+    Hq = Hkv * G
+    scale = 1.0 / math.sqrt(d)
+    q = wl.make_tensor((B, Hq, N, d), "q", seed=N, dtype="bf16", gain=gain)
+    do = wl.make_tensor((B, Hq, N, d), "do", seed=N, dtype="bf16")
+    k = wl.make_tensor((B, Hkv, N, d), "k", seed=N, dtype="bf16", gain=gain)
+    v = wl.make_tensor((B, Hkv, N, d), "v", seed=N, dtype="bf16")
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    rx.ringx_set_deterministic(det)
+    try:
+        o, lse = rx.ringx_attn_fwd_gqa(qd, kd, vd, chunk, scale)
+        dq, dk, dv = rx.ringx_attn_bwd_gqa(qd, kd, vd, o, lse, dod, chunk, scale)
+        torch.cuda.synchronize()
+    finally:
+        rx.ringx_set_deterministic(False)
+    q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+    k_rep, v_rep = np.repeat(k64, G, axis=1), np.repeat(v64, G, axis=1)
+    o_ref, lse_ref = orc.attention_fwd_bhnd(q64, k_rep, v_rep, scale)
+    check_fwd(o, lse, o_ref, lse_ref, v64, "bf16")
+    dq_ref, dk_rep, dv_rep = orc.attention_bwd_bhnd(q64, k_rep, v_rep, do64, scale)
+    dk_ref = dk_rep.reshape(B, Hkv, G, N, d).sum(axis=2)
+    dv_ref = dv_rep.reshape(B, Hkv, G, N, d).sum(axis=2)
+    for name, g, ref in (("dq", dq, dq_ref), ("dk", dk, dk_ref), ("dv", dv, dv_ref)):
+        nr = np.linalg.norm(ref)
+        if nr == 0.0:                      # N = 1: dq = dk = 0 exactly
+            assert not g.float().any(), name
+        else:
+            assert np.linalg.norm(to64(g) - ref) / nr <= TOL_GRAD, name
