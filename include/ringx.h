@@ -33,8 +33,9 @@
  *              there are ceil(N / kv_chunk) passes, the last one over the keys that are left; tiles
  *              that run past the end of a head read zeros (3-D tensor maps), keys past the end are
  *              masked, rows past the end are never written (the *_host entries and the bf16 per-device
- *              steps ringx_attn_chunk_fwd*, ringx_attn_bwd_partial* likewise).  Every other entry
- *              (fp32, MLA and block entries) needs N % 128 == 0 (N % 256 == 0 for a
+ *              steps ringx_attn_chunk_fwd*, ringx_attn_bwd_partial*, and ringx_attn_fwd_mla /
+ *              ringx_attn_bwd_mla likewise).  Every other entry (fp32, the MLA per-device steps, the block
+ *              entries) needs N % 128 == 0 (N % 256 == 0 for a
  *              bf16 forward: one CTA owns two 128-row query tiles), 0 < kv_chunk <= N and N % kv_chunk == 0
  *              (every device holds an equal chunk S/N, l.128).  Anything else returns
  *              RINGX_ERR_BAD_SHAPE -- never a silently wrong answer.  A device that is not
@@ -121,7 +122,7 @@ RINGX_API int ringx_attn_bwd_gqa(const void* q, const void* k, const void* v, co
  * dimensions) and d_v = 128.  The path is the one of ringx_attn_fwd -- Eq. 1 per KV chunk, partials folded left to right by
  * the two-operand Eq. 5 in the chunk kernel's epilogue -- on a kernel laid out for these widths.
  *   q, k [B,H,N,d_qk] bf16 (in); v [B,H,N,d_v] bf16 (in); o [B,H,N,d_v] bf16 (out); lse [B,H,N] float (out).
- *   Domain: d_qk == 192, d_v == 128, dtype RINGX_BF16, N % 256 == 0, kv_chunk % 128 == 0, N % kv_chunk == 0.
+ *   Domain: d_qk == 192, d_v == 128, dtype RINGX_BF16, any N >= 1, kv_chunk % 128 == 0 (as ringx_attn_fwd).
  *   workspace  >= ringx_attn_fwd_mla_workspace_bytes(...) bytes (0 when kv_chunk == N), 256-byte aligned. */
 RINGX_API int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, float* lse,
                        int B, int H, int N, int d_qk, int d_v, int kv_chunk, float scale, int dtype,
@@ -132,8 +133,8 @@ RINGX_API size_t ringx_attn_fwd_mla_workspace_bytes(int B, int H, int N, int d_q
  * ringx_attn_bwd): per KV chunk dk, dv of the chunk's keys are complete and written once (atomic-free), dq accumulates in
  * fp32 over the chunk passes (order of the sums not fixed) and is rounded to bf16 once at the end.
  *   q, k, dq, dk [B,H,N,d_qk] bf16; v, o, dO, dv [B,H,N,d_v] bf16; lse [B,H,N] float (from ringx_attn_fwd_mla).
- *   Outputs must not alias inputs.  Domain: d_qk == 192, d_v == 128, RINGX_BF16, N % 128 == 0, kv_chunk % 128 == 0,
- *   N % kv_chunk == 0.  workspace >= ringx_attn_bwd_mla_workspace_bytes(...) bytes, 256-byte aligned (D, LSE*log2e and
+ *   Outputs must not alias inputs.  Domain: d_qk == 192, d_v == 128, RINGX_BF16, any N >= 1, kv_chunk % 128 == 0.
+ *   workspace >= ringx_attn_bwd_mla_workspace_bytes(...) bytes, 256-byte aligned (D, LSE*log2e and
  *   the fp32 dq accumulator, which the kernel keeps transposed, [B,H,d_qk,N]; + the fixed-point scales of
  *   ringx_set_deterministic, which applies here as it does to ringx_attn_bwd). */
 RINGX_API int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* o, const float* lse,

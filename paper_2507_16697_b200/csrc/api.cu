@@ -297,6 +297,22 @@ bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, in
   return r == CUDA_SUCCESS;
 }
 
+// 2-D view with a row pitch of `pitch_cols` elements (>= cols): columns >= cols are out of bounds (zero on load, skipped on
+// store / reduce)
+bool make_tmap_2d_pitched(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t rows,
+                          uint64_t cols, uint64_t pitch_cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz) {
+  EncodeFn enc = encode_fn();
+  if (!enc) return false;
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {pitch_cols * (uint64_t)elem_bytes};
+  cuuint32_t box[2] = {box_cols, box_rows};
+  cuuint32_t es[2] = {1, 1};
+  CUresult r = enc(out, dt, 2, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   swz == kSwizzle128B ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
 // 3-D view [heads][rows][cols] (row-major, contiguous), box = {box_cols, box_rows, 1}: a box that runs past the last row
 // of a head is zero-filled on load and clipped on store / reduce (ragged sequence lengths)
 bool make_tmap_3d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t heads, uint64_t rows,
@@ -460,8 +476,8 @@ int ringx_attn_fwd(const void* q, const void* k, const void* v, void* o, float* 
 
 // ---- multi-head latent attention shapes (d_qk = 192, d_v = 128): the same chunk loop on the MLA kernel
 size_t ringx_attn_fwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk) {
-  if (d_qk != 192 || d_v != 128 || check_shape(B, H, N, d_v, kv_chunk, 1.f, RINGX_BF16, false) != RINGX_OK) return 0;
-  if (kv_chunk == N) return 0;
+  if (d_qk != 192 || d_v != 128 || check_shape(B, H, N, d_v, kv_chunk, 1.f, RINGX_BF16, false, true) != RINGX_OK) return 0;
+  if (kv_chunk >= N) return 0;
   const size_t R = (size_t)B * H * N;
   return align_up(R * d_v * sizeof(float)) + align_up(R * sizeof(float));
 }
@@ -473,7 +489,7 @@ int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, flo
   if (!q || !k || !v || !o || !lse) return RINGX_ERR_NULL_PTR;
   if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (d_qk != 192 || d_v != 128) return RINGX_ERR_BAD_SHAPE;
-  int st = check_shape(B, H, N, d_v, kv_chunk, scale, dtype, false);
+  int st = check_shape(B, H, N, d_v, kv_chunk, scale, dtype, false, true);
   if (st != RINGX_OK) return st;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse)) return RINGX_ERR_MISALIGNED;
   const size_t need = ringx_attn_fwd_mla_workspace_bytes(B, H, N, d_qk, d_v, kv_chunk);
@@ -484,7 +500,7 @@ int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, flo
   }
   if ((st = check_arch()) != RINGX_OK) return st;
   tl_launches = 0;
-  const int BH = B * H, n_chunks = N / kv_chunk;
+  const int BH = B * H, n_chunks = (N + kv_chunk - 1) / kv_chunk;      // the last chunk may be short (ragged lengths)
   const size_t R = (size_t)BH * N;
   float* o_acc = static_cast<float*>(workspace);
   float* lse_acc = need ? reinterpret_cast<float*>(static_cast<char*>(workspace) + align_up(R * d_v * sizeof(float))) : nullptr;
@@ -496,8 +512,8 @@ int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, flo
     cudaError_t e;
     {
       Timed timed(RINGX_PROFILE_ATTN_FWD, stream);
-      e = launch_attn_chunk_fwd_mla_sm100(q, k, v, o_dst, l_dst, o_acc, lse_acc, BH, N, N, c * kv_chunk, kv_chunk, scale, epi,
-                                          stream);
+      e = launch_attn_chunk_fwd_mla_sm100(q, k, v, o_dst, l_dst, o_acc, lse_acc, BH, N, N, c * kv_chunk,
+                                          last ? N - c * kv_chunk : kv_chunk, scale, epi, stream);
     }
     if (e != cudaSuccess) return cuda_status(e);
   }
@@ -508,10 +524,12 @@ int ringx_attn_fwd_mla(const void* q, const void* k, const void* v, void* o, flo
 // backward of the same shapes: D / lse2 preprocess (d_v = 128 wide), one pass of the MLA backward kernel per KV chunk into
 // the transposed fp32 dQ accumulator, transpose + bf16 cast of dQ
 size_t ringx_attn_bwd_mla_workspace_bytes(int B, int H, int N, int d_qk, int d_v, int kv_chunk) {
-  if (d_qk != 192 || d_v != 128 || check_shape(B, H, N, d_v, kv_chunk, 1.f, RINGX_BF16, true) != RINGX_OK) return 0;
-  const size_t R = (size_t)B * H * N;
-  // D, lse2, the transposed dQ accumulator, and for deterministic mode the per-query fixed-point scales + K/V maxima
-  return 3 * align_up(R * sizeof(float)) + align_up(R * d_qk * sizeof(float)) + align_up((size_t)B * H * 2 * sizeof(float));
+  if (d_qk != 192 || d_v != 128 || check_shape(B, H, N, d_v, kv_chunk, 1.f, RINGX_BF16, true, true) != RINGX_OK) return 0;
+  const size_t R = (size_t)B * H * N, Rp = (size_t)B * H * ((N + 127) / 128 * 128);    // Rp: every head padded to 128 rows
+  // D, lse2 (padded), the transposed dQ accumulator (rows of padded length), and for deterministic mode the per-query
+  // fixed-point scales + K/V maxima
+  return 2 * align_up(Rp * sizeof(float)) + align_up(R * sizeof(float)) + align_up(Rp * d_qk * sizeof(float)) +
+         align_up((size_t)B * H * 2 * sizeof(float));
 }
 
 int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* o, const float* lse, const void* dO,
@@ -521,7 +539,7 @@ int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* 
   if (!q || !k || !v || !o || !lse || !dO || !dq || !dk || !dv) return RINGX_ERR_NULL_PTR;
   if (dtype != RINGX_BF16) return RINGX_ERR_BAD_DTYPE;
   if (d_qk != 192 || d_v != 128) return RINGX_ERR_BAD_SHAPE;
-  int st = check_shape(B, H, N, d_v, kv_chunk, scale, dtype, true);
+  int st = check_shape(B, H, N, d_v, kv_chunk, scale, dtype, true, true);
   if (st != RINGX_OK) return st;
   if ((long long)B * H * d_qk > 0x7FFFFFFFLL) return RINGX_ERR_BAD_SHAPE;
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(lse) || !aligned16(dO) ||
@@ -534,20 +552,21 @@ int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* 
   if ((st = check_arch()) != RINGX_OK) return st;
   tl_launches = 0;
   const int BH = B * H;
-  const size_t R = (size_t)BH * N;
+  const size_t R = (size_t)BH * N, Rp = (size_t)BH * ((N + 127) / 128 * 128);
   float* D = static_cast<float*>(workspace);
-  float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + align_up(R * sizeof(float)));
-  char* wp = static_cast<char*>(workspace) + 2 * align_up(R * sizeof(float));
-  float* dq_acc_t = reinterpret_cast<float*>(wp);
-  wp += align_up(R * d_qk * sizeof(float));
+  float* lse2 = reinterpret_cast<float*>(static_cast<char*>(workspace) + align_up(Rp * sizeof(float)));
+  char* wp = static_cast<char*>(workspace) + 2 * align_up(Rp * sizeof(float));
+  float* dq_acc_t = reinterpret_cast<float*>(wp);               // [BH*192][N rounded up to 128]
+  wp += align_up(Rp * d_qk * sizeof(float));
   float* qs = reinterpret_cast<float*>(wp);
   float* kvmax = reinterpret_cast<float*>(wp + align_up(R * sizeof(float)));
   const bool fixed = g_deterministic.load(std::memory_order_relaxed) != 0;     // int32 fixed-point dQ (see bwd_core)
   cudaError_t e;
   {
     Timed timed(RINGX_PROFILE_BWD_AUX, stream);
-    e = cudaMemsetAsync(dq_acc_t, 0, R * d_qk * sizeof(float), stream);
-    if (e == cudaSuccess) e = launch_bwd_preprocess(o, dO, lse, D, lse2, nullptr, (long long)R, d_v, scale, false, stream);
+    e = cudaMemsetAsync(dq_acc_t, 0, Rp * d_qk * sizeof(float), stream);
+    if (e == cudaSuccess) e = launch_bwd_preprocess(o, dO, lse, D, lse2, nullptr, (long long)R, d_v, scale, false, stream, N);
+    if (N % 128) count_launch();
     if (e == cudaSuccess && fixed) {
       e = launch_dq_fixed_scale(k, v, dO, kvmax, qs, BH, N, N, 0, N, d_qk, d_v, scale, stream);
       count_launch(2);
@@ -555,9 +574,11 @@ int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* 
   }
   count_launch();
   if (e != cudaSuccess) return cuda_status(e);
-  for (int c = 0; c < N / kv_chunk; ++c) {
+  const int n_chunks = (N + kv_chunk - 1) / kv_chunk;
+  for (int c = 0; c < n_chunks; ++c) {
     Timed timed(RINGX_PROFILE_ATTN_BWD, stream);
-    e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, BH, N, N, c * kv_chunk, kv_chunk, scale,
+    e = launch_attn_chunk_bwd_mla_sm100(q, k, v, dO, lse2, D, dq_acc_t, dk, dv, BH, N, N, c * kv_chunk,
+                                        c + 1 < n_chunks ? kv_chunk : N - c * kv_chunk, scale,
                                         fixed ? qs : nullptr, RINGX_BF16, stream);
     if (e != cudaSuccess) return cuda_status(e);
   }

@@ -52,8 +52,8 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
                           const __grid_constant__ CUtensorMap map_v, const __grid_constant__ CUtensorMap map_do,
                           const __grid_constant__ CUtensorMap map_dq_a, const __grid_constant__ CUtensorMap map_dq_b,
                           const float* __restrict__ lse2, const float* __restrict__ Dvec, void* __restrict__ dk,
-                          void* __restrict__ dv, int dkv_f32, int N, int nk_stride, int k_off, float scale_log2,
-                          float scale, const float* __restrict__ dq_qs) {
+                          void* __restrict__ dv, int dkv_f32, int N, int n_stat, int nk_stride, int k_off,
+                          float scale_log2, float scale, const float* __restrict__ dq_qs) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sK = smem;
@@ -81,9 +81,14 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   const int lane = threadIdx.x & 31;
   const int bh = blockIdx.y;
-  const int n_s = N / kSub;
-  const int q_row0 = bh * N;                                        // rows of this head in the [BH*N, .] views
-  const int k_row0 = bh * nk_stride + k_off + blockIdx.x * kKeys;   // rows in the [BH*nk_stride, .] views of K, V, dK, dV
+  // Any sequence length (as attn_bwd_sm100.cu): q, dO, k, v are [BH][rows][.] tensor maps (rows past the end of a head read
+  // as zeros), lse2 / D are [BH][n_stat] with lse2 = +inf in the padding (P = 0 for query rows that do not exist), keys past
+  // the end get P = 0 by a select and their dK, dV rows are not stored, the dQ^T reduce-add skips the missing queries.
+  const int n_s = (N + kSub - 1) / kSub;
+  const int q_row0 = bh * N;                                        // rows of this head in the flat [BH*N] array dq_qs
+  const int s_row0 = bh * n_stat;                                   // ... in lse2, D
+  const int k_in = k_off + blockIdx.x * kKeys;                      // first key row of my tile within the head
+  const int k_row0 = bh * nk_stride + k_in;                         // ... in the flat [BH*nk_stride, .] arrays dK, dV
 
   if (threadIdx.x == 0) {
     mbar_init(kv_full, 1);
@@ -130,20 +135,19 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     if (leader) {
       mbar_arrive_expect_tx(kv_full, kKBytes + kVBytes);
 #pragma unroll
-      for (int p = 0; p < kDqk / 64; ++p) tma_load_2d(sK + p * kKPanel, &map_k, kv_full, p * 64, k_row0, pol_kv);
+      for (int p = 0; p < kDqk / 64; ++p) tma_load_3d(sK + p * kKPanel, &map_k, kv_full, p * 64, k_in, bh, pol_kv);
 #pragma unroll
-      for (int p = 0; p < kDv / 64; ++p) tma_load_2d(sV + p * kKPanel, &map_v, kv_full, p * 64, k_row0, pol_kv);
+      for (int p = 0; p < kDv / 64; ++p) tma_load_3d(sV + p * kKPanel, &map_v, kv_full, p * 64, k_in, bh, pol_kv);
     }
     __syncwarp();
     auto load_q = [&](int s, int st) {
       if (leader) {
         uint8_t* dst = sQ + st * kQStageBytes;
-        const int row = q_row0 + s * kSub;
         mbar_arrive_expect_tx(&q_full[st], kQBytes + 512);
 #pragma unroll
-        for (int p = 0; p < kDqk / 64; ++p) tma_load_2d(dst + p * kQPanel, &map_q, &q_full[st], p * 64, row, pol_q);
-        bulk_load_1d(dst + kQBytes, lse2 + row, 256, &q_full[st]);
-        bulk_load_1d(dst + kQBytes + 256, Dvec + row, 256, &q_full[st]);
+        for (int p = 0; p < kDqk / 64; ++p) tma_load_3d(dst + p * kQPanel, &map_q, &q_full[st], p * 64, s * kSub, bh, pol_q);
+        bulk_load_1d(dst + kQBytes, lse2 + s_row0 + s * kSub, 256, &q_full[st]);
+        bulk_load_1d(dst + kQBytes + 256, Dvec + s_row0 + s * kSub, 256, &q_full[st]);
       }
       __syncwarp();
     };
@@ -156,7 +160,7 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         mbar_arrive_expect_tx(&do_full[ds], kDoBytes);
 #pragma unroll
         for (int p = 0; p < kDv / 64; ++p)
-          tma_load_2d(sDo + ds * kDoBytes + p * kQPanel, &map_do, &do_full[ds], p * 64, q_row0 + s * kSub, pol_q);
+          tma_load_3d(sDo + ds * kDoBytes + p * kQPanel, &map_do, &do_full[ds], p * 64, s * kSub, bh, pol_q);
       }
       __syncwarp();
       if (++ds == kDoStages) { ds = 0; dph ^= 1; }
@@ -275,6 +279,7 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     uint8_t* ds_row = sDs + row * 128;
     const float2 sc2 = make_float2(scale_log2, scale_log2);
     const float2 scl2 = make_float2(scale, scale);               // dS^T carries `scale` (Dvec holds scale * D_i)
+    const bool key_valid = k_in + row < nk_stride;
     int stage = 0, phase = 0;
     for (int s = 0; s < n_s; ++s) {
       const float4* stats = reinterpret_cast<const float4*>(sQ + stage * kQStageBytes + kQBytes);
@@ -299,8 +304,8 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
                                   make_float2(-aux[g].x, -aux[g].y));
           const float2 x1 = ffma2(make_float2(__uint_as_float(sv[g * 4 + 2]), __uint_as_float(sv[g * 4 + 3])), sc2,
                                   make_float2(-aux[g].z, -aux[g].w));
-          p[g * 2] = make_float2(ex2(x0.x), ex2(x0.y));
-          p[g * 2 + 1] = make_float2(ex2(x1.x), ex2(x1.y));
+          p[g * 2] = key_valid ? make_float2(ex2(x0.x), ex2(x0.y)) : make_float2(0.f, 0.f);     // (a key past the end of the head)
+          p[g * 2 + 1] = key_valid ? make_float2(ex2(x1.x), ex2(x1.y)) : make_float2(0.f, 0.f);
           pk[g * 2] = pack_bf16x2(p[g * 2].x, p[g * 2].y);
           pk[g * 2 + 1] = pack_bf16x2(p[g * 2 + 1].x, p[g * 2 + 1].y);
         }
@@ -353,6 +358,7 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       uint32_t r[32];
       tmem_ld_x32(tSrc + c * 32, r);
       tmem_wait_ld();
+      if (!key_valid) continue;              // (after the warp-wide TMEM load)
       if (dkv_f32) {
         float4* dst = reinterpret_cast<float4*>(static_cast<float*>(half == 0 ? dv : dk) + out_off + c * 32);
 #pragma unroll
@@ -399,16 +405,13 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         if (dq_qs) {
           // deterministic mode (attn_bwd_sm100.cu): int32 fixed point; here a thread is a feature row and its 64
           // registers are the 64 queries of the sub-tile, each with its own scale (warp-uniform 16-byte loads)
-          const float4* qs4 = reinterpret_cast<const float4*>(dq_qs + static_cast<size_t>(bh) * N + s * kSub);
+          const float* qs1 = dq_qs + q_row0 + s * kSub;       // (scalar loads: a ragged head is not 16-byte aligned)
 #pragma unroll
           for (int c = 0; c < 2; ++c)
 #pragma unroll
-            for (int g = 0; g < 8; ++g) {
-              const float4 f = __ldg(qs4 + c * 8 + g);
-              r[c][g * 4 + 0] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 0]) * f.x));
-              r[c][g * 4 + 1] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 1]) * f.y));
-              r[c][g * 4 + 2] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 2]) * f.z));
-              r[c][g * 4 + 3] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][g * 4 + 3]) * f.w));
+            for (int e = 0; e < 32; ++e) {
+              const float f = s * kSub + c * 32 + e < N ? __ldg(qs1 + c * 32 + e) : 0.f;
+              r[c][e] = static_cast<uint32_t>(__float2int_rn(__uint_as_float(r[c][e]) * f));
             }
         }
 #pragma unroll
@@ -449,22 +452,25 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
 // along the queries, writes coalesced along the features.  qs != nullptr: the accumulator is int32 fixed point and query n
 // of head bh carries the scale qs[bh * N + n] (deterministic mode).
 __global__ void __launch_bounds__(256)
-dq_transpose_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dq, int N,
+dq_transpose_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dq, int N, int n_pitch,
                             const float* __restrict__ qs) {
+  // (acc rows are n_pitch floats apart: N rounded up to 128, so that a ragged N keeps the rows 16-byte aligned for TMA)
   __shared__ float tile[64][65];
   const int bh = blockIdx.z, f0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
   const int tx = threadIdx.x & 63, ty = threadIdx.x >> 6;          // 64 x 4
-  const float* src = acc + (static_cast<size_t>(bh) * kDqk + f0) * N + n0;
-  const float inv = qs ? 1.0f / __ldg(qs + static_cast<size_t>(bh) * N + n0 + tx) : 1.0f;
+  const float* src = acc + (static_cast<size_t>(bh) * kDqk + f0) * n_pitch + n0;
+  const bool q_valid = n0 + tx < N;
+  const float inv = qs && q_valid ? 1.0f / __ldg(qs + static_cast<size_t>(bh) * N + n0 + tx) : 1.0f;
 #pragma unroll
   for (int r = ty; r < 64; r += 4) {                               // [feature][query]
-    const float x = __ldcs(src + static_cast<size_t>(r) * N + tx);
+    const float x = q_valid ? __ldcs(src + static_cast<size_t>(r) * n_pitch + tx) : 0.f;
     tile[r][tx] = qs ? static_cast<float>(__float_as_int(x)) * inv : x;
   }
   __syncthreads();
   __nv_bfloat16* dst = dq + (static_cast<size_t>(bh) * N + n0) * kDqk + f0;
 #pragma unroll
-  for (int r = ty; r < 64; r += 4) dst[static_cast<size_t>(r) * kDqk + tx] = __float2bfloat16_rn(tile[tx][r]);   // [query][feature]
+  for (int r = ty; r < 64; r += 4)                                 // [query][feature]
+    if (n0 + r < N) dst[static_cast<size_t>(r) * kDqk + tx] = __float2bfloat16_rn(tile[tx][r]);
 }
 
 }  // namespace
@@ -476,28 +482,30 @@ cudaError_t launch_attn_chunk_bwd_mla_sm100(const void* q, const void* k, const 
   CUtensorMap mq, mk, mv, mdo, mdqa, mdqb;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   const CUtensorMapDataType dqt = dq_qs ? CU_TENSOR_MAP_DATA_TYPE_INT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-  const uint64_t rows = (uint64_t)BH * N, krows = (uint64_t)BH * nk_stride;
-  if (!make_tmap_2d(&mq, q, dt, 2, rows, kDqk, kSub, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mk, k, dt, 2, krows, kDqk, kKeys, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mv, v, dt, 2, krows, kDv, kKeys, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mdo, dO, dt, 2, rows, kDv, kSub, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mdqa, dq_acc_t, dqt, 4, (uint64_t)BH * kDqk, N, 128, 32, kSwizzle128B) ||
-      !make_tmap_2d(&mdqb, dq_acc_t, dqt, 4, (uint64_t)BH * kDqk, N, 64, 32, kSwizzle128B))
+  const int n_stat = (N + 127) / 128 * 128;      // row stride of lse2, D and of the transposed dQ accumulator
+  if (nk % kKeys && k_off + nk != nk_stride) return cudaErrorInvalidValue;   // only the head's last key tile may be ragged
+  // dq_acc_t is [BH*192][n_stat] with N valid columns: the reduce-add clips the queries past the end
+  if (!make_tmap_3d(&mq, q, dt, 2, BH, N, kDqk, kSub, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mk, k, dt, 2, BH, nk_stride, kDqk, kKeys, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mv, v, dt, 2, BH, nk_stride, kDv, kKeys, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mdo, dO, dt, 2, BH, N, kDv, kSub, 64, kSwizzle128B) ||
+      !make_tmap_2d_pitched(&mdqa, dq_acc_t, dqt, 4, (uint64_t)BH * kDqk, N, n_stat, 128, 32, kSwizzle128B) ||
+      !make_tmap_2d_pitched(&mdqb, dq_acc_t, dqt, 4, (uint64_t)BH * kDqk, N, n_stat, 64, 32, kSwizzle128B))
     return cudaErrorInvalidValue;
   auto kern = attn_chunk_bwd_mla_kernel;
   static unsigned char configured[kMaxDevices];
   if (cudaError_t e = set_max_dyn_smem_once(kern, kSmemBytes, configured); e != cudaSuccess) return e;
-  dim3 grid(nk / kKeys, BH);
-  kern<<<grid, kThreads, kSmemBytes, stream>>>(mq, mk, mv, mdo, mdqa, mdqb, lse2, D, dk, dv, dkv_dtype == RINGX_F32, N, nk_stride,
-                                               k_off, scale * 1.4426950408889634f, scale, dq_qs);
+  dim3 grid((nk + kKeys - 1) / kKeys, BH);
+  kern<<<grid, kThreads, kSmemBytes, stream>>>(mq, mk, mv, mdo, mdqa, mdqb, lse2, D, dk, dv, dkv_dtype == RINGX_F32, N, n_stat,
+                                               nk_stride, k_off, scale * 1.4426950408889634f, scale, dq_qs);
   count_launch();
   return cudaGetLastError();
 }
 
 cudaError_t launch_dq_transpose_convert_mla(const float* dq_acc_t, void* dq, int BH, int N, const float* dq_qs,
                                             cudaStream_t stream) {
-  dim3 grid(N / 64, kDqk / 64, BH);
-  dq_transpose_convert_kernel<<<grid, 256, 0, stream>>>(dq_acc_t, static_cast<__nv_bfloat16*>(dq), N, dq_qs);
+  dim3 grid((N + 63) / 64, kDqk / 64, BH);
+  dq_transpose_convert_kernel<<<grid, 256, 0, stream>>>(dq_acc_t, static_cast<__nv_bfloat16*>(dq), N, (N + 127) / 128 * 128, dq_qs);
   return cudaGetLastError();
 }
 

@@ -44,7 +44,8 @@ template <int kEpi>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __grid_constant__ CUtensorMap map_k,
                           const __grid_constant__ CUtensorMap map_v, void* o_out, float* lse_out, const float* o_acc,
-                          const float* lse_acc, int Nq, int nk_stride, int k_off, int n_kv, float scale_log2) {
+                          const float* lse_acc, int Nq, int nk_stride, int k_off, int n_kv, int k_tail,
+                          float scale_log2) {
   constexpr bool kFold = kEpi == kEpiFold || kEpi == kEpiFoldFinal;
   constexpr bool kOutBf16 = kEpi == kEpiFinal || kEpi == kEpiFoldFinal;
   extern __shared__ uint8_t smem_raw[];
@@ -66,8 +67,10 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   const int lane = threadIdx.x & 31;
   const int bh = blockIdx.y;
-  const int q_row0 = bh * Nq + blockIdx.x * (2 * kBlockM);
-  const int k_row0 = bh * nk_stride + k_off;
+  // Any sequence length (as attn_fwd_sm100.cu): q, k, v are [BH][rows][.] tensor maps, so tiles that run past the end of a
+  // head read zeros; such query rows are computed and never stored, such keys (k_tail of the last key tile exist) are masked.
+  const int q_in = blockIdx.x * (2 * kBlockM);              // first query row of the CTA within its head
+  const int q_row0 = bh * Nq + q_in;                        // ... in the flat [BH*Nq] arrays
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
@@ -108,18 +111,18 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       if (leader) {
         mbar_arrive_expect_tx(bar, kQkTileBytes);
 #pragma unroll
-        for (int p = 0; p < kDqk / 64; ++p) tma_load_2d(dst + p * kPanelBytes, map, bar, p * 64, row, pol);
+        for (int p = 0; p < kDqk / 64; ++p) tma_load_3d(dst + p * kPanelBytes, map, bar, p * 64, row, bh, pol);
       }
       __syncwarp();
     };
     auto push_k = [&](int j) {
       const int st = j % kKStages;
       mbar_wait_relaxed(&k_empty[st], ((j / kKStages) & 1) ^ 1);
-      load_qk(sK + st * kQkTileBytes, &map_k, &k_full[st], k_row0 + j * kBlockN, pol_kv);
+      load_qk(sK + st * kQkTileBytes, &map_k, &k_full[st], k_off + j * kBlockN, pol_kv);
     };
-    load_qk(sQ, &map_q, &q_full[0], q_row0, pol_q);
+    load_qk(sQ, &map_q, &q_full[0], q_in, pol_q);
     push_k(0);
-    load_qk(sQ + kQkTileBytes, &map_q, &q_full[1], q_row0 + kBlockM, pol_q);
+    load_qk(sQ + kQkTileBytes, &map_q, &q_full[1], q_in + kBlockM, pol_q);
     for (int j = 0; j < n_kv; ++j) {
       if (j + 1 < n_kv) push_k(j + 1);
 #pragma unroll
@@ -129,8 +132,8 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
           mbar_arrive_expect_tx(&v_full[h], kVHalfBytes);
 #pragma unroll
           for (int p = 0; p < kDv / 64; ++p)       // map_v's box is 64 keys x 64 columns
-            tma_load_2d(sV + h * kVHalfBytes + p * kVHalfPanelBytes, &map_v, &v_full[h], p * 64,
-                        k_row0 + j * kBlockN + h * 64, pol_kv);
+            tma_load_3d(sV + h * kVHalfBytes + p * kVHalfPanelBytes, &map_v, &v_full[h], p * 64,
+                        k_off + j * kBlockN + h * 64, bh, pol_kv);
         }
         __syncwarp();
       }
@@ -211,8 +214,9 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     const uint32_t tO = tmem + kOBase + t * kDv + lane_off;
     const float2 sc2 = make_float2(scale_log2, scale_log2);
     const size_t row = static_cast<size_t>(q_row0) + t * kBlockM + row_t;
+    const bool row_valid = q_in + t * kBlockM + row_t < Nq;
     float lse_prev = 0.f;
-    if (kFold) lse_prev = lse_acc[row];
+    if (kFold && row_valid) lse_prev = lse_acc[row];
     float m_raw = -CUDART_INF_F, m_sc = -CUDART_INF_F, l = 0.f;
     for (int j = 0; j < n_kv; ++j) {
       mbar_wait(&s_full[t], j & 1);
@@ -239,6 +243,16 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       piece_max(2, mx0, mx1);
       tmem_wait_ld_x32(piece(3));
       piece_max(3, mx2, mx3);
+      if (k_tail != 0 && j == n_kv - 1) {                    // warp-uniform: the last key tile of a ragged head
+#pragma unroll
+        for (int c = 0; c < kBlockN; ++c)
+          if (c >= k_tail) s[c] = 0xff800000u;               // -inf
+        mx0 = mx1 = mx2 = mx3 = -CUDART_INF_F;
+        piece_max(0, mx0, mx1);
+        piece_max(1, mx2, mx3);
+        piece_max(2, mx0, mx1);
+        piece_max(3, mx2, mx3);
+      }
       const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
       const bool grow = (mx - m_raw) * scale_log2 > kRescaleThreshold;
       if (__any_sync(0xffffffffu, grow)) {
@@ -305,7 +319,7 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       if (kFold) {
         const float4* src = reinterpret_cast<const float4*>(o_acc + row * kDv + c * 32);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) acc[i] = __ldcs(src + i);
+        for (int i = 0; i < 8; ++i) acc[i] = row_valid ? __ldcs(src + i) : make_float4(0.f, 0.f, 0.f, 0.f);
       }
       tmem_wait_ld();
       float r[32];
@@ -320,6 +334,7 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
           r[i * 4 + 3] = fmaf(ca, acc[i].w, r[i * 4 + 3]);
         }
       }
+      if (!row_valid) continue;
       if (kOutBf16) {
         uint4* dst = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(o_out) + row * kDv + c * 32);
 #pragma unroll
@@ -337,7 +352,7 @@ attn_chunk_fwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         for (int i = 0; i < 8; ++i) dst[i] = make_float4(r[i * 4], r[i * 4 + 1], r[i * 4 + 2], r[i * 4 + 3]);
       }
     }
-    lse_out[row] = lse_row;
+    if (row_valid) lse_out[row] = lse_row;
   } else {
     setmaxnreg_dec<kAuxRegs>();
   }
@@ -354,9 +369,9 @@ cudaError_t launch_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
   auto kern = attn_chunk_fwd_mla_kernel<kEpi>;
   static unsigned char configured[kMaxDevices];
   if (cudaError_t e = set_max_dyn_smem_once(kern, kSmemBytes, configured); e != cudaSuccess) return e;
-  dim3 grid(Nq / (2 * kBlockM), BH);
+  dim3 grid((Nq + 2 * kBlockM - 1) / (2 * kBlockM), BH);
   kern<<<grid, kThreads, kSmemBytes, stream>>>(mq, mk, mv, o_out, lse_out, o_acc, lse_acc, Nq, nk_stride, k_off,
-                                               nk / kBlockN, scale * 1.4426950408889634f);
+                                               (nk + kBlockN - 1) / kBlockN, nk % kBlockN, scale * 1.4426950408889634f);
   count_launch();
   return cudaGetLastError();
 }
@@ -368,9 +383,10 @@ cudaError_t launch_attn_chunk_fwd_mla_sm100(const void* q, const void* k, const 
                                             int k_off, int nk, float scale, int epilogue, cudaStream_t stream) {
   CUtensorMap mq, mk, mv;
   const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
-  if (!make_tmap_2d(&mq, q, dt, 2, (uint64_t)BH * Nq, kDqk, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mk, k, dt, 2, (uint64_t)BH * nk_stride, kDqk, 128, 64, kSwizzle128B) ||
-      !make_tmap_2d(&mv, v, dt, 2, (uint64_t)BH * nk_stride, kDv, 64, 64, kSwizzle128B))      // half tiles: 64 keys
+  if (nk % kBlockN && k_off + nk != nk_stride) return cudaErrorInvalidValue;   // only the head's last key tile may be ragged
+  if (!make_tmap_3d(&mq, q, dt, 2, BH, Nq, kDqk, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mk, k, dt, 2, BH, nk_stride, kDqk, 128, 64, kSwizzle128B) ||
+      !make_tmap_3d(&mv, v, dt, 2, BH, nk_stride, kDv, 64, 64, kSwizzle128B))      // half tiles: 64 keys
     return cudaErrorInvalidValue;
   switch (epilogue) {
     case kFwdEpiPartial:

@@ -121,6 +121,9 @@ cudaError_t launch_attn_chunk_bwd_sm100(const void* q, const void* k, const void
 enum TmapSwizzle { kSwizzleNone = 0, kSwizzle128B = 1 };
 bool make_tmap_2d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t rows,
                   uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz);
+// 2-D view whose rows are pitch_cols (>= cols) elements apart: columns >= cols read as zero and are not written
+bool make_tmap_2d_pitched(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t rows,
+                          uint64_t cols, uint64_t pitch_cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz);
 // 3-D view [heads][rows][cols], box = {box_cols, box_rows, 1}: rows past the end of a head read as zero and are not written
 bool make_tmap_3d(CUtensorMap* out, const void* base, CUtensorMapDataType dt, int elem_bytes, uint64_t heads, uint64_t rows,
                   uint64_t cols, uint32_t box_rows, uint32_t box_cols, TmapSwizzle swz);

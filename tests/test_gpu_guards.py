@@ -39,7 +39,8 @@ class Guarded:
 
 
 def test_attention_forward_backward_guards(rx):
-    for (B, H, N, d, chunk) in ((1, 1, 256, 64, 128), (2, 3, 768, 128, 256), (1, 2, 4096, 128, 2048)):
+    for (B, H, N, d, chunk) in ((1, 1, 256, 64, 128), (2, 3, 768, 128, 256), (1, 2, 4096, 128, 2048),
+                                (2, 3, 1000, 128, 384), (1, 2, 77, 64, 128), (1, 2, 1337, 64, 512)):     # the last three: ragged lengths
         g = Guarded()
         q, k, v, do = (t.cuda() for t in wl.make_qkv((B, H, N, d), with_do=True, seed=3))
         scale = d ** -0.5
@@ -54,7 +55,7 @@ def test_attention_forward_backward_guards(rx):
 
 
 def test_mla_forward_backward_guards(rx):
-    for (B, H, N, chunk) in ((1, 1, 256, 128), (2, 3, 768, 256)):
+    for (B, H, N, chunk) in ((1, 1, 256, 128), (2, 3, 768, 256), (2, 2, 1000, 384), (1, 1, 77, 128)):   # the last two: ragged
         g = Guarded()
         q, k = (wl.make_tensor((B, H, N, 192), w, seed=5).cuda() for w in "qk")
         v, do = (wl.make_tensor((B, H, N, 128), w, seed=5).cuda() for w in ("v", "do"))
