@@ -19,7 +19,8 @@
  *   Pointers   Unless a parameter says HOST, every pointer is a DEVICE pointer, 16-byte aligned.
  *   Ownership  The caller owns every buffer.  The library never allocates or frees device
  *              memory and keeps no pointer after a call returns.  Scratch space is the
- *              caller-provided `workspace`, sized by the *_workspace_bytes queries.
+ *              caller-provided `workspace`, sized by the *_workspace_bytes queries (the one exception:
+ *              ringx_attn_fwd_static, whose scratch is a fixed array inside the library image).
  *   Streams    All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy
  *              default stream).  Calls return after enqueue; there is no host synchronisation
  *              (the *_host entries are the exception: they synchronise `stream` before returning).  Because nothing
@@ -341,6 +342,39 @@ RINGX_API size_t ringx_attn_fwd_bwd_host_workspace_bytes(int B, int H, int N, in
 RINGX_API size_t ringx_attn_fwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
 RINGX_API size_t ringx_attn_bwd_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
 RINGX_API size_t ringx_attn_fwd_host_workspace_bytes(int B, int H, int N, int d, int kv_chunk, int dtype);
+
+/* ringx_attn_fwd without a workspace argument, for callers that have no device memory to lend and no way to get any.
+ * Every other entry point expects the caller to bring the scratch space; some callers cannot:
+ *   - a plug-in or operator that runs inside a host process whose own allocator has already claimed the whole GPU
+ *     (inference servers and training frameworks reserve HBM up front), where a cudaMalloc simply fails;
+ *   - a host thread that must issue work while another thread of the process is capturing a CUDA graph in global capture
+ *     mode, during which cudaMalloc is a prohibited call;
+ *   - a latency-bound loop (in-situ analysis inside a solver's time step) that cannot take the device-wide synchronisation
+ *     cudaMalloc and cudaFree imply;
+ *   - a small C or Fortran driver on this ABI that has inputs and outputs but no workspace management of its own.
+ * For them the scratch of the multi-pass forward -- the running fp32 (o_acc, lse_acc) that the chunk kernel folds each
+ * KV-chunk pass into by the two-operand Eq. 5 (l.130-133), plus the per-split partials when a pass is split over its keys --
+ * lives in a fixed array inside the library's device image.  This call, and everything below it, makes no cudaMalloc,
+ * cudaFree or other allocating call.
+ *   q, k, v, o, lse, shapes, dtype, scale, stream: exactly as ringx_attn_fwd; the results are those of ringx_attn_fwd (same
+ *   kernels, same launch configuration, same passes).  Inputs and outputs are still the caller's buffers.
+ *   Limit     ringx_attn_fwd_workspace_bytes(B,H,N,d,kv_chunk,dtype) must not exceed RINGX_STATIC_SCRATCH_BYTES (32 MiB:
+ *             e.g. B*H*N*d <= 8 Mi elements of fp32 accumulator less the [B,H,N] lse, when no pass is split).  A larger
+ *             problem returns RINGX_ERR_WORKSPACE_TOO_SMALL before anything is enqueued -- use ringx_attn_fwd with your
+ *             own workspace for those.  A single-pass call (kv_chunk >= N, no split) needs no scratch and always fits.
+ *   Cost      the array is part of the library image: every GPU on which the process uses libringx holds those 32 MiB from
+ *             module load until the process exits, whether or not this entry is ever called.
+ *   Set-up    the first call on each device that needs the scratch looks up the array's device address
+ *             (cudaGetSymbolAddress, with that device current; the result is cached per device under a mutex).  Make that
+ *             first call outside any stream capture.  A failed look-up returns RINGX_ERR_CUDA.
+ *   Sharing   there is ONE array per device and every call uses it.  It keeps whatever the previous call wrote; the forward
+ *             needs none of it to start at zero (the first pass overwrites what later passes read), so nothing is cleared.
+ *             Two calls whose kernels can overlap on the same GPU -- different streams, or different host threads on different
+ *             streams -- race on the array and corrupt each other's results: serialise them (one stream, or an event between
+ *             them).  Calls on different GPUs do not interact. */
+#define RINGX_STATIC_SCRATCH_BYTES ((size_t)32 << 20)
+RINGX_API int ringx_attn_fwd_static(const void* q, const void* k, const void* v, void* o, float* lse,
+                          int B, int H, int N, int d, int kv_chunk, float scale, int dtype, void* stream);
 
 /* Bit-reproducible dQ.  By default the per-key-tile contributions to dQ are reduce-added into the fp32
  * accumulator in whatever order the CTAs reach them (fp32 addition is not associative: the last bits of dq may differ from run

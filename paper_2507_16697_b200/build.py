@@ -15,7 +15,7 @@ import sys
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libringx.so")
-SOURCES = ["api.cu", "merge.cu", "attn_f32_split_sm100.cu", "attn_fwd_sm100.cu", "attn_fwd_mla_sm100.cu", "attn_bwd_sm100.cu", "attn_bwd_mla_sm100.cu", "fidelity.cu", "proj_sm100.cu"]
+SOURCES = ["api.cu", "merge.cu", "attn_f32_split_sm100.cu", "attn_fwd_sm100.cu", "attn_fwd_mla_sm100.cu", "attn_bwd_sm100.cu", "attn_bwd_mla_sm100.cu", "fidelity.cu", "proj_sm100.cu", "static_scratch.cu"]
 HEADERS = ["kernels.cuh", "ptx.cuh", os.path.join("..", "..", "include", "ringx.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

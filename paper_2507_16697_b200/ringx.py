@@ -38,6 +38,8 @@ def lib() -> ctypes.CDLL:
     c_p, c_i, c_f, c_sz, c_ll = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t, ctypes.c_longlong
     L.ringx_attn_fwd.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_fwd.restype = c_i
+    L.ringx_attn_fwd_static.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p]
+    L.ringx_attn_fwd_static.restype = c_i
     L.ringx_attn_fwd_host.argtypes = [c_p] * 5 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
     L.ringx_attn_fwd_host.restype = c_i
     L.ringx_attn_bwd.argtypes = [c_p] * 9 + [c_i] * 5 + [c_f, c_i, c_p, c_sz, c_p]
@@ -187,6 +189,29 @@ def ringx_attn_fwd(q, k, v, kv_chunk: int, scale: float, o=None, lse=None, works
     st = lib().ringx_attn_fwd(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
                               B, H, N, d, kv_chunk, scale, dt, ws_ptr, ws_len, _stream())
     _check(st, "ringx_attn_fwd")
+    return o, lse
+
+
+RINGX_STATIC_SCRATCH_BYTES = 32 << 20     # include/ringx.h
+
+
+def ringx_attn_fwd_static(q, k, v, kv_chunk: int, scale: float, o=None, lse=None):
+    """ringx_attn_fwd for callers that cannot supply a device workspace (include/ringx.h: ringx_attn_fwd_static): the
+    scratch of the chunk passes is a fixed 32 MiB array inside libringx, so the call allocates no device memory -- pass
+    `o` and `lse` and this wrapper allocates nothing either (without them it creates the two outputs, nothing else).
+    Problems whose ringx_attn_fwd workspace would exceed RINGX_STATIC_SCRATCH_BYTES raise RingxError
+    (RINGX_ERR_WORKSPACE_TOO_SMALL).  All calls on one GPU share the array: do not let two of them overlap."""
+    B, H, N, d = q.shape
+    if o is None:
+        o = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    for t, nm in ((k, "k"), (v, "v"), (o, "o")):
+        _expect(t, q.shape, nm, q.dtype)
+    _expect(lse, (B, H, N), "lse", torch.float32)
+    st = lib().ringx_attn_fwd_static(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
+                                     B, H, N, d, kv_chunk, scale, _DTYPES[q.dtype], _stream())
+    _check(st, "ringx_attn_fwd_static")
     return o, lse
 
 
