@@ -26,6 +26,12 @@
  *              (the *_host entries are the exception: they synchronise `stream` before returning).  Because nothing
  *              is allocated and nothing synchronises, the device entries can be captured into a CUDA graph
  *              (cudaStreamBeginCapture on `stream`) once their first, uncaptured call has set the kernel attributes.
+ *              One-time set-up: the first d = 128 backward on each device checks the alignment of the kernel's shared
+ *              memory with a one-warp launch on a short-lived stream of the library's own and waits for that launch
+ *              (microseconds; `stream` itself is neither used for it nor synchronised).  If `stream` is being captured
+ *              at that moment the call returns RINGX_ERR_CUDA before the attention kernel is enqueued (the capture stays
+ *              valid; the call's helper launches may already be in it): make the first backward on a device outside a
+ *              capture.
  *   Errors     Return value is a ringx_status (0 = RINGX_OK).  Arguments are validated before the
  *              first launch: an error other than RINGX_ERR_CUDA means nothing was enqueued and no
  *              output was touched.  No abort, no printf, no exceptions cross this boundary.
@@ -151,7 +157,8 @@ RINGX_API size_t ringx_attn_bwd_mla_workspace_bytes(int B, int H, int N, int d_q
  * [B,H,d_qk,Nq] (zeroed by the caller before the first step; reduce-added in arbitrary order), dk [B,H,Nk,d_qk] and dv
  * [B,H,Nk,d_v] of dkv_dtype (bf16, or fp32 shares of a cross-device sum), `prepared` != 0 when the workspace already holds
  * D and LSE*log2e of this (o, lse, dO) from an earlier step; workspace >= ringx_attn_bwd_partial_mla_workspace_bytes(B,H,Nq),
- * Nq % 128 == 0;  ringx_dq_finalize_mla writes dq [B,H,Nq,d_qk] bf16 = transpose(dq_acc_t) after the last step. */
+ * Nq % 128 == 0;  ringx_dq_finalize_mla writes dq [B,H,Nq,d_qk] bf16 = transpose(dq_acc_t) after the last step (Nq % 128 == 0
+ * like the step that fills dq_acc_t; anything else RINGX_ERR_BAD_SHAPE). */
 RINGX_API int ringx_attn_chunk_fwd_mla(const void* q, const void* k, const void* v, const float* o_acc, const float* lse_acc,
                              void* o_out, float* lse_out, int B, int H, int Nq, int Nk, int d_qk, int d_v, float scale,
                              int dtype, int o_out_dtype, void* stream);
@@ -380,8 +387,10 @@ RINGX_API int ringx_attn_fwd_static(const void* q, const void* k, const void* v,
  * accumulator in whatever order the CTAs reach them (fp32 addition is not associative: the last bits of dq may differ from run
  * to run; dk, dv are always bit-reproducible).  With the flag set -- it is process-wide, so that a backward issued from another
  * thread (a framework's autograd worker thread) sees it -- ringx_attn_bwd, ringx_attn_bwd_gqa and ringx_attn_bwd_partial[_ex]
- * accumulate dQ as int32 FIXED POINT: query row i gets the scale 1.5e9 / (2.03 scale ||dO_i|| max_j||V_j|| max_jc|K_jc|), a
- * bound on |dQ_ic| that follows from sum_j P_ij = 1 (two extra launches read K, V and dO once), every fp32 tile contribution
+ * accumulate dQ as int32 FIXED POINT: query row i gets the scale
+ * 1.5e9 / (1.016 scale (||dO_i|| max_j||V_j|| + |dO_i.O_i|) max_jc|K_jc|), maxima over the keys of the call -- a bound on its
+ * |dQ_ic| that follows from sum_j P_ij <= 1 and holds for a per-device step too, where O comes from the keys of all devices
+ * and the step's own V may be small or zero (two extra launches read K, V and dO once), every fp32 tile contribution
  * is scaled and rounded to an integer, and the reduce-adds are integer adds -- associative, so the same inputs give
  * bit-identical dq in any arrival order, on any grid, with no ordering between CTAs (about 5 % of the backward throughput at
  * d = 128, 10 % at d = 64).  Resolution: 2^-30.5 of that bound per contribution; for diffuse attention over very long
@@ -391,7 +400,9 @@ RINGX_API int ringx_attn_fwd_static(const void* q, const void* k, const void* v,
  * inside the workspace and added to dq_acc by one element-wise kernel, so a fixed sequence of steps is reproducible; its
  * workspace query returns the larger size while the flag is set (a call with a workspace sized before the flag was set
  * returns RINGX_ERR_WORKSPACE_TOO_SMALL).  ringx_attn_bwd_mla is covered in the same way (per-query scales on the transposed
- * accumulator).  Not covered: ringx_attn_bwd_partial_mla, and the weight gradients of ringx_*_proj_bwd
+ * accumulator).  Non-finite inputs: a NaN or Inf in dO_i, O_i, or in the K, V of the call makes row i of dq NaN (as the fp32
+ * accumulator would); a non-finite q or lse is NOT detected in this mode (the integer conversion turns NaN into 0).
+ * Not covered: ringx_attn_bwd_partial_mla, and the weight gradients of ringx_*_proj_bwd
  * (split-K partial sums are reduce-added in arbitrary order). */
 RINGX_API int ringx_set_deterministic(int on);
 RINGX_API int ringx_get_deterministic(void);

@@ -568,7 +568,7 @@ int ringx_attn_bwd_mla(const void* q, const void* k, const void* v, const void* 
     if (e == cudaSuccess) e = launch_bwd_preprocess(o, dO, lse, D, lse2, nullptr, (long long)R, d_v, scale, false, stream, N);
     if (N % 128) count_launch();
     if (e == cudaSuccess && fixed) {
-      e = launch_dq_fixed_scale(k, v, dO, kvmax, qs, BH, N, N, 0, N, d_qk, d_v, scale, stream);
+      e = launch_dq_fixed_scale(k, v, dO, D, kvmax, qs, BH, N, N, 0, N, d_qk, d_v, scale, stream);
       count_launch(2);
     }
   }
@@ -679,7 +679,9 @@ int ringx_attn_bwd_partial_mla(const void* q, const void* k, const void* v, cons
 int ringx_dq_finalize_mla(const float* dq_acc_t, void* dq, int B, int H, int Nq, int d_qk, void* stream_) {
   cudaStream_t stream = static_cast<cudaStream_t>(stream_);
   if (!dq_acc_t || !dq) return RINGX_ERR_NULL_PTR;
-  if (d_qk != 192 || B <= 0 || H <= 0 || Nq <= 0 || Nq % 64 || (long long)B * H > 65535) return RINGX_ERR_BAD_SHAPE;
+  // Nq % 128 as ringx_attn_bwd_partial_mla, the only producer of dq_acc_t [B,H,d_qk,Nq]: the transpose reads it with a row
+  // pitch of Nq rounded up to 128, which is the documented layout only when that is Nq itself
+  if (d_qk != 192 || B <= 0 || H <= 0 || Nq <= 0 || Nq % 128 || (long long)B * H > 65535) return RINGX_ERR_BAD_SHAPE;
   if (!aligned16(dq_acc_t) || !aligned16(dq)) return RINGX_ERR_MISALIGNED;
   int st = check_arch();
   if (st != RINGX_OK) return st;
@@ -844,7 +846,7 @@ static int bwd_core(const void* q, const void* k, const void* v, const void* o, 
       pass_acc = reinterpret_cast<float*>(det.fix);
       if ((e = cudaMemsetAsync(det.fix, 0, (size_t)R * d * sizeof(int), stream)) != cudaSuccess) return cuda_status(e);
     }
-    e = launch_dq_fixed_scale(k, v, dO, det.kvmax, det.qs, BH, Nq, Nk, 0, Nk, d, d, scale, stream);
+    e = launch_dq_fixed_scale(k, v, dO, D, det.kvmax, det.qs, BH, Nq, Nk, 0, Nk, d, d, scale, stream);
     count_launch(2);
     if (e != cudaSuccess) return cuda_status(e);
   }

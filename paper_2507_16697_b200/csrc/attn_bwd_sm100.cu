@@ -22,6 +22,8 @@
 // Pipeline: the compute warps alternate phase A (S^T -> P^T) and phase B (dP^T -> dS^T) while the tensor core runs
 // {dV(i), S^T(i+1)} behind phase A and {dQ(i), dK(i), dP^T(i+1)} behind phase B (dQ first, so that its drain runs
 // under the dK MMA); in-order MMA execution makes the P^T / S^T overlay safe.
+#include <mutex>
+
 #include "kernels.cuh"
 
 namespace ringx {
@@ -547,23 +549,46 @@ cudaError_t launch_tt(const CUtensorMap& mq, const CUtensorMap& mk, const CUtens
   using Cfg = BwdCfg<kD>;
   auto kern = attn_chunk_bwd_kernel<kD, kTail>;
   static unsigned char configured[kMaxDevices];
-  if (cudaError_t e = set_max_dyn_smem_once(kern, Cfg::kSmemBytes, configured); e != cudaSuccess) return e;
+  // First use on a device (kernels without alignment slack, d = 128): prove that the dynamic shared memory of this kernel
+  // starts 1 KB aligned (see the kernel).  The probe runs on a stream of its own that exists only for this check (a host
+  // object, no device memory) and the host waits for THAT stream: the caller's stream is neither used nor synchronised.
+  // A caller's stream that is being captured is refused before this launcher touches anything (the first backward on a
+  // device belongs outside a capture).
+  static unsigned char probed[kMaxDevices];    // 0 = not yet, 1 = aligned, 2 = misaligned; guarded by probe_mu
+  static std::mutex probe_mu;
+  int dev = 0;
+  bool need_probe = false, cacheable = false;
   if (Cfg::kAlignSlack == 0) {
-    // first use on this device: prove that the dynamic shared memory of this kernel starts 1 KB aligned (see the kernel)
-    static unsigned char probed[kMaxDevices];    // 0 = not yet, 1 = aligned, 2 = misaligned
-    int dev = 0;
     if (cudaError_t e = cudaGetDevice(&dev); e != cudaSuccess) return e;
-    const bool cacheable = dev >= 0 && dev < kMaxDevices;
-    if (!cacheable || !probed[dev]) {
+    cacheable = dev >= 0 && dev < kMaxDevices;
+    {
+      std::lock_guard<std::mutex> guard(probe_mu);
+      if (cacheable && probed[dev] == 2) return cudaErrorInvalidConfiguration;
+      need_probe = !cacheable || !probed[dev];
+    }
+    if (need_probe) {
+      cudaStreamCaptureStatus capturing = cudaStreamCaptureStatusNone;
+      if (cudaError_t e = cudaStreamIsCapturing(stream, &capturing); e != cudaSuccess) return e;
+      if (capturing != cudaStreamCaptureStatusNone) return cudaErrorStreamCaptureUnsupported;
+    }
+  }
+  if (cudaError_t e = set_max_dyn_smem_once(kern, Cfg::kSmemBytes, configured); e != cudaSuccess) return e;
+  if (need_probe) {
+    std::lock_guard<std::mutex> guard(probe_mu);
+    if (!cacheable || !probed[dev]) {          // (another thread may have probed this device in the meantime)
       unsigned* flag = nullptr;
       unsigned h = 0xffffffffu;
       cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&flag), g_bwd_smem_probe);
       if (e != cudaSuccess) return e;
-      kern<<<1, 32, Cfg::kSmemBytes, stream>>>(mq, mk, mv, mdo, mdq, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0, 0, 0.f,
-                                               0.f, nullptr, flag);
-      if ((e = cudaGetLastError()) != cudaSuccess) return e;
-      if ((e = cudaMemcpyAsync(&h, flag, sizeof(h), cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return e;
-      if ((e = cudaStreamSynchronize(stream)) != cudaSuccess) return e;
+      cudaStream_t probe_stream = nullptr;
+      if ((e = cudaStreamCreateWithFlags(&probe_stream, cudaStreamNonBlocking)) != cudaSuccess) return e;
+      kern<<<1, 32, Cfg::kSmemBytes, probe_stream>>>(mq, mk, mv, mdo, mdq, nullptr, nullptr, nullptr, nullptr, 0, 0, 0, 0, 0,
+                                                     0.f, 0.f, nullptr, flag);
+      e = cudaGetLastError();
+      if (e == cudaSuccess) e = cudaMemcpyAsync(&h, flag, sizeof(h), cudaMemcpyDeviceToHost, probe_stream);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(probe_stream);
+      cudaStreamDestroy(probe_stream);
+      if (e != cudaSuccess) return e;
       if (cacheable) probed[dev] = h == 0 ? 1 : 2;
       if (h != 0) return cudaErrorInvalidConfiguration;
     } else if (probed[dev] == 2) {

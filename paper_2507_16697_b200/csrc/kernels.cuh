@@ -35,12 +35,13 @@ cudaError_t launch_bwd_preprocess(const void* o, const void* dO, const float* ls
                                   cudaStream_t stream, long long rows_per_head = 0);
 cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float scale, cudaStream_t stream);
 // Deterministic dQ (int32 fixed-point accumulator, merge.cu).  launch_dq_fixed_scale: kvmax [2*BH] (scratch) and the
-// per-row scales qs [BH*rows_per_head] from k (rows d_k wide), v (d_v wide) rows [k_off, k_off+nk) of every head and dO
-// (d_v wide) (2 launches + a memset).  launch_dq_fixed_finish: dq_bf16 = dq_fix / qs (dq_bf16 != nullptr), else dq_acc += dq_fix / qs
+// per-row scales qs [BH*rows_per_head] from k (rows d_k wide), v (d_v wide) rows [k_off, k_off+nk) of every head, dO
+// (d_v wide) and Ds = launch_bwd_preprocess's D buffer of the same rows (rows_per_head given there too: per-head padded
+// layout) (2 launches + a memset).  launch_dq_fixed_finish: dq_bf16 = dq_fix / qs (dq_bf16 != nullptr), else dq_acc += dq_fix / qs
 // (1 launch).
-cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, float* kvmax, float* qs, int BH,
-                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d_k, int d_v, float scale,
-                                  cudaStream_t stream);
+cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, const float* Ds, float* kvmax, float* qs,
+                                  int BH, long long rows_per_head, int nk_stride, int k_off, int nk, int d_k, int d_v,
+                                  float scale, cudaStream_t stream);
 cudaError_t launch_dq_fixed_finish(const int* dq_fix, const float* qs, void* dq_bf16, float* dq_acc, long long rows, int d,
                                    cudaStream_t stream);
 

@@ -65,8 +65,9 @@ __device__ __forceinline__ void merge_weights(float la, float lb, float& wa, flo
 // row all come from one warp: running in place on operand a is race-free.
 template <typename TIn, typename TOut, int kLanes>
 __global__ void __launch_bounds__(kMergeThreads)
-lse_merge_kernel(const void* __restrict__ o_a, const float* lse_a, const void* __restrict__ o_b,
+lse_merge_kernel(const void* o_a, const float* lse_a, const void* __restrict__ o_b,
                  const float* __restrict__ lse_b, void* o_out, float* lse_out, long long rows, int d) {
+  // o_a / lse_a carry no __restrict__: the header lets o_out alias o_a and lse_out alias lse_a (in-place merge)
   constexpr int kRowsPerWarp = 32 / kLanes;
   const int lane = threadIdx.x & 31;
   const int sub = lane / kLanes, l = lane % kLanes;
@@ -308,9 +309,16 @@ dq_convert_kernel(const float4* __restrict__ dq_acc, uint2* __restrict__ dq, lon
 // ---------------------------------------------------------------- deterministic dQ: int32 fixed-point accumulator
 // (ringx_set_deterministic).  Integer adds are associative, so TMA reduce-adds of integers give the same sum in any
 // arrival order.  Row r gets a scale qs[r] with |dQ_rc| * qs[r] <= 1.5e9 < 2^31 guaranteed by
-//   |dQ_rc| = scale |sum_j P_rj (dP_rj - D_r) K_jc| <= scale * 2 max_j|dO_r.V_j| * max_j|K_jc|      (sum_j P_rj = 1,
-//                                                 <= 2 scale ||dO_r|| max_j||V_j|| max_jc|K_jc|      D_r in the hull of dP_rj)
+//   |dQ_rc| = scale |sum_j P_rj (dP_rj - D_r) K_jc| <= scale (sum_j P_rj) (max_j|dO_r.V_j| + |D_r|) max_j|K_jc|
+//                                                 <= scale (||dO_r|| max_j||V_j|| + |D_r|) max_jc|K_jc|
+// over the keys j of THIS call, with sum_j P_rj <= 1 because P is formed from the LSE over all keys of the sequence.
+// |D_r| is read from the preprocess buffer, not bounded by ||dO_r|| max||V||: in a per-device step (ringx_attn_bwd_partial)
+// O, and with it D_r = dO_r.O_r, comes from the keys of ALL devices, whose values may be far larger than this step's (or
+// this step's V may be all zeros) -- D_r then lies outside the hull of the local dP_rj.
 // (the partial sums may wrap: two's-complement adds are exact modulo 2^32, only the final value has to fit).
+// Non-finite inputs: a NaN/Inf in dO_r or O_r (through D_r) or in the K, V of the call makes the bound non-finite; qs[r] is
+// then NaN and the row of dq comes out NaN, as the fp32 accumulator would give (a non-finite Q or lse is NOT detected: the
+// kernel's fp32 contribution is NaN and rounds to integer 0).
 
 // kvmax[2h] = max_j ||V_j||^2, kvmax[2h+1] = max_jc |K_jc| over the nk key rows [k_off, k_off+nk) of kv head h
 // (atomicMax on the bit patterns of non-negative floats: order-independent).  grid = (blocks, BH); kvmax zeroed before.
@@ -338,15 +346,17 @@ kv_absmax_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v, unsig
     }
 #pragma unroll
     for (int off = kLanesV / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
-    vmax2 = fmaxf(vmax2, s);
+    vmax2 = s != s ? CUDART_INF_F : fmaxf(vmax2, s);      // fmaxf drops a NaN: keep it as +inf (the bound turns non-finite)
   }
   const uint4* kh = k + head0 * k_vecs;
   for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < (long long)nk * k_vecs; i += (long long)gridDim.x * 256) {
     const uint4 a = __ldg(kh + i);
     const uint32_t* pa = reinterpret_cast<const uint32_t*>(&a);
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
-      kmax = fmaxf(kmax, fmaxf(fabsf(__uint_as_float(pa[j] << 16)), fabsf(__uint_as_float(pa[j] & 0xFFFF0000u))));
+    for (int j = 0; j < 4; ++j) {
+      const float k0 = fabsf(__uint_as_float(pa[j] << 16)), k1 = fabsf(__uint_as_float(pa[j] & 0xFFFF0000u));
+      kmax = (k0 != k0 || k1 != k1) ? CUDART_INF_F : fmaxf(kmax, fmaxf(k0, k1));
+    }
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
@@ -359,13 +369,15 @@ kv_absmax_kernel(const uint4* __restrict__ k, const uint4* __restrict__ v, unsig
   }
 }
 
-// qs[r] = 1.5e9 / bound_r (clamped to [2^-100, 2^100]), bound_r = 2.03125 * scale * ||dO_r|| * sqrt(kvmax[2h]) * kvmax[2h+1],
-// h = r / rows_per_head.  The 2.03125 covers the bf16 roundings of O (in D_r) and of dS and a row sum of P up to 1.001;
-// 1.5e9 + one rounding of 1/2 per key tile stays below 2^31.
+// qs[r] = 1.5e9 / bound_r (clamped to [2^-100, 2^100]; NaN when bound_r is not finite),
+// bound_r = 1.015625 * (scale * ||dO_r|| * sqrt(kvmax[2h]) + |Ds_r|) * kvmax[2h+1], h = r / rows_per_head, where
+// Ds = scale * D is launch_bwd_preprocess's buffer ([heads][n_stat] layout) -- the very values the backward kernel subtracts.
+// The 1.015625 covers the bf16 rounding of dS and a row sum of P up to 1.001; 1.5e9 + one rounding of 1/2 per key tile
+// stays below 2^31.
 template <int kLanes>
 __global__ void __launch_bounds__(256)
-dq_fixed_scale_kernel(const uint4* __restrict__ dO, const float* __restrict__ kvmax, float* __restrict__ qs,
-                      long long rows, long long rows_per_head, float scale) {
+dq_fixed_scale_kernel(const uint4* __restrict__ dO, const float* __restrict__ kvmax, const float* __restrict__ Ds,
+                      float* __restrict__ qs, long long rows, long long rows_per_head, long long n_stat, float scale) {
   constexpr int kRowsPerWarp = 32 / kLanes;
   const int lane = threadIdx.x & 31, sub = lane / kLanes, l = lane % kLanes;
   const long long warp_global = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -387,8 +399,10 @@ dq_fixed_scale_kernel(const uint4* __restrict__ dO, const float* __restrict__ kv
     for (int off = kLanes / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
     if (r < rows && l == 0) {
       const long long h = r / rows_per_head;
-      const float bound = 2.03125f * scale * sqrtf(s) * sqrtf(kvmax[2 * h]) * kvmax[2 * h + 1];
-      qs[r] = fminf(fmaxf(1.5e9f / fmaxf(bound, 1e-37f), 7.8886e-31f), 1.2676506e30f);
+      const float ds = fabsf(__ldg(Ds + h * n_stat + (r - h * rows_per_head)));
+      const float bound = 1.015625f * (scale * sqrtf(s) * sqrtf(kvmax[2 * h]) + ds) * kvmax[2 * h + 1];
+      const float q = fminf(fmaxf(1.5e9f / fmaxf(bound, 1e-37f), 7.8886e-31f), 1.2676506e30f);
+      qs[r] = bound <= 3.0e38f ? q : CUDART_NAN_F;          // NaN or Inf bound: the row of dq is NaN, not silently finite
     }
   }
 }
@@ -509,9 +523,9 @@ cudaError_t launch_dq_convert(const float* dq_acc, void* dq, long long n, float 
   return cudaGetLastError();
 }
 
-cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, float* kvmax, float* qs, int BH,
-                                  long long rows_per_head, int nk_stride, int k_off, int nk, int d_k, int d_v, float scale,
-                                  cudaStream_t stream) {
+cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, const float* Ds, float* kvmax, float* qs,
+                                  int BH, long long rows_per_head, int nk_stride, int k_off, int nk, int d_k, int d_v,
+                                  float scale, cudaStream_t stream) {
   cudaError_t e = cudaMemsetAsync(kvmax, 0, (size_t)BH * 2 * sizeof(float), stream);
   if (e != cudaSuccess) return e;
   const int lanes = d_v / 8;   // 8 or 16: V rows and dO rows
@@ -521,14 +535,15 @@ cudaError_t launch_dq_fixed_scale(const void* k, const void* v, const void* dO, 
   if (bx > cap) bx = cap;
   const dim3 grid((unsigned)bx, (unsigned)BH);
   const long long rows = (long long)BH * rows_per_head;
+  const long long n_stat = (rows_per_head + 127) / 128 * 128;      // launch_bwd_preprocess's per-head pitch of D
   long long blocks = (rows + rows_per_block - 1) / rows_per_block;
   if (blocks > (long long)sm_count() * 8 * 4) blocks = (long long)sm_count() * 8 * 4;
   if (lanes == 8) {
     kv_absmax_kernel<8><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk, d_k / 8);
-    dq_fixed_scale_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, qs, rows, rows_per_head, scale);
+    dq_fixed_scale_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, Ds, qs, rows, rows_per_head, n_stat, scale);
   } else {
     kv_absmax_kernel<16><<<grid, 256, 0, stream>>>((const uint4*)k, (const uint4*)v, (unsigned*)kvmax, nk_stride, k_off, nk, d_k / 8);
-    dq_fixed_scale_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, qs, rows, rows_per_head, scale);
+    dq_fixed_scale_kernel<16><<<(unsigned)blocks, 256, 0, stream>>>((const uint4*)dO, kvmax, Ds, qs, rows, rows_per_head, n_stat, scale);
   }
   return cudaGetLastError();
 }

@@ -100,6 +100,75 @@ def test_bwd_partial_steps_add_up_to_the_oracle_gradient(rx, d, Nq, chunks):
         assert relf(accs[0].cpu().double().numpy(), dq_ref) <= 6e-3
 
 
+@pytest.mark.parametrize("d", [64, 128])
+@pytest.mark.parametrize("case", ["zero_local_v", "other_chunk_16x"])
+def test_deterministic_partial_step_with_zero_and_small_local_v(rx, d, case):
+    """Deterministic (int32 fixed-point) dQ in a per-device step whose own V says nothing about D_i = dO_i.O_i: O comes from
+    the keys of ALL steps, so with this step's V all zero (padding) or another step's V 16x larger, |D_i| is far above
+    ||dO_i|| max_local||V||.  A scale taken from the local V alone overflows the int32 (the advisor's finding on r02);
+    the bound now carries |D_i| itself.  Two steps of 512 keys; dq must match the oracle, and the fp32 mode's result."""
+    B, H, Nq, Nk = 1, 2, 384, 1024
+    scale = 1.0 / math.sqrt(d)
+    q = wl.make_tensor((B, H, Nq, d), "q", seed=73, dtype="bf16")
+    do = wl.make_tensor((B, H, Nq, d), "do", seed=73, dtype="bf16")
+    k = wl.make_tensor((B, H, Nk, d), "k", seed=73, dtype="bf16")
+    v = wl.make_tensor((B, H, Nk, d), "v", seed=73, dtype="bf16").clone()
+    if case == "zero_local_v":
+        v[:, :, :512] = 0
+    else:
+        v[:, :, 512:] = (v[:, :, 512:].float() * 16).to(torch.bfloat16)
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    q64, k64, v64, do64 = (f64(t) for t in (q, k, v, do))
+    o_dev, lse_dev = rx.ringx_attn_chunk_fwd_ex(qd, kd, vd, scale, final=True)
+    dq_ref, dk_ref, dv_ref = orc.attention_bwd_bhnd(q64, k64, v64, do64, scale)
+    results = {}
+    for det in (False, True):
+        rx.ringx_set_deterministic(det)
+        try:
+            acc = torch.zeros((B, H, Nq, d), dtype=torch.float32, device="cuda")
+            for lo, hi in ((0, 512), (512, 1024)):
+                _, dk, dv = rx.ringx_attn_bwd_partial(qd, kd[:, :, lo:hi].contiguous(), vd[:, :, lo:hi].contiguous(), o_dev,
+                                                      lse_dev, dod, scale, dq_acc=acc)
+                assert relf(f64(dk), dk_ref[:, :, lo:hi]) <= TOL_GRAD
+            torch.cuda.synchronize()
+        finally:
+            rx.ringx_set_deterministic(False)
+        results[det] = acc.cpu().double().numpy()
+    assert relf(results[False], dq_ref) <= 6e-3
+    assert relf(results[True], dq_ref) <= 6e-3                     # r02: saturated integers, garbage
+    assert np.abs(results[True] - results[False]).max() <= 1e-4 * np.abs(dq_ref).max()
+
+
+def test_deterministic_mode_propagates_non_finite_gradients(rx):
+    """The fp32 accumulator turns a NaN or Inf upstream gradient into a NaN row of dq; the integer accumulator would round it
+    to 0 (float -> int of NaN is 0).  The per-row scale is NaN when its bound is not finite, so the row comes out NaN in
+    deterministic mode too, and the other rows are untouched."""
+    B, H, N, d = 1, 2, 512, 128
+    scale = 1.0 / math.sqrt(d)
+    q, k, v, do = wl.make_qkv((B, H, N, d), with_do=True, seed=83, dtype="bf16")
+    do = do.clone()
+    do[0, 0, 5, 3] = float("nan")
+    do[0, 1, 300, 0] = float("inf")
+    qd, kd, vd, dod = (t.cuda() for t in (q, k, v, do))
+    o, lse = rx.ringx_attn_fwd(qd, kd, vd, N, scale)
+    rx.ringx_set_deterministic(True)
+    try:
+        dq, _, _ = rx.ringx_attn_bwd(qd, kd, vd, o, lse, dod, N, scale)
+        torch.cuda.synchronize()
+    finally:
+        rx.ringx_set_deterministic(False)
+    dq = dq.float().cpu()
+    assert torch.isnan(dq[0, 0, 5]).all() and torch.isnan(dq[0, 1, 300]).all()
+    finite = torch.ones(B, H, N, dtype=torch.bool)
+    finite[0, 0, 5] = finite[0, 1, 300] = False
+    assert torch.isfinite(dq[finite]).all()
+    do_clean = do.clone()
+    do_clean[0, 0, 5] = 0
+    do_clean[0, 1, 300] = 0
+    dq_ref, _, _ = orc.attention_bwd_bhnd(f64(q), f64(k), f64(v), f64(do_clean), scale)
+    assert relf(dq[finite].double().numpy(), dq_ref[finite.numpy()]) <= 6e-3
+
+
 def test_bwd_partial_equals_full_backward_when_it_sees_everything(rx):
     """With Nq == Nk and one call, ringx_attn_bwd_partial + ringx_dq_finalize is ringx_attn_bwd (same kernels)."""
     B, H, N, d = 1, 2, 1024, 128
