@@ -150,6 +150,12 @@ def _expect(t: torch.Tensor, shape, name: str, dtype=None):
         raise ValueError(f"{name} has dtype {t.dtype}, expected {dtype}")
 
 
+def _expect_workspace(workspace: torch.Tensor, need: int, name: str):
+    if workspace.numel() * workspace.element_size() < need:
+        raise ValueError(f"{name}: workspace holds {workspace.numel() * workspace.element_size()} bytes, "
+                         f"the size query asks for {need}")
+
+
 def _stream() -> int:
     return torch.cuda.current_stream().cuda_stream
 
@@ -317,6 +323,12 @@ def ringx_attn_bwd_partial_mla(q, k, v, o, lse, dO, scale: float, dq_acc_t, dk, 
         raise ValueError("dk and dv must have the same dtype")
     if dq_acc_t.dtype != torch.float32 or dq_acc_t.numel() != q.numel():
         raise ValueError("dq_acc_t must hold B*H*Nq*d_qk floats")
+    _expect(o, (B, H, Nq, d_v), "o", q.dtype)
+    _expect(dO, (B, H, Nq, d_v), "dO", q.dtype)
+    _expect(lse, (B, H, Nq), "lse", torch.float32)
+    _expect(dk, (B, H, Nk, d_qk), "dk")
+    _expect(dv, (B, H, Nk, d_v), "dv")
+    _expect_workspace(workspace, lib().ringx_attn_bwd_partial_mla_workspace_bytes(B, H, Nq), "ringx_attn_bwd_partial_mla")
     st = lib().ringx_attn_bwd_partial_mla(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
                                           _dev(dO, "dO"), _dev(dq_acc_t, "dq_acc_t"), _dev(dk, "dk"), _dev(dv, "dv"),
                                           B, H, Nq, Nk, d_qk, d_v, scale, _DTYPES[q.dtype], _DTYPES[dk.dtype],
@@ -610,6 +622,22 @@ def ringx_fidelity_tokens(y, origin, size, k: int, sigma: float = 0.0, out_dtype
     return tokens
 
 
+def _expect_bwd_partial(q, k, v, o, lse, dO, dq_acc, dk, dv):
+    """Shapes of one per-device backward step: q, o, dO [B,H,Nq,d]; k, v, dk, dv [B,H,Nk,d]; lse [B,H,Nq]; dq_acc B*H*Nq*d
+    floats.  The kernel writes dk, dv with the sizes of k: a slice of another length would be written out of bounds."""
+    B, H, Nq, d = q.shape
+    Nk = k.shape[2]
+    _expect(k, (B, H, Nk, d), "k", q.dtype)
+    _expect(v, (B, H, Nk, d), "v", q.dtype)
+    _expect(o, q.shape, "o", q.dtype)
+    _expect(dO, q.shape, "dO", q.dtype)
+    _expect(lse, (B, H, Nq), "lse", torch.float32)
+    _expect(dk, (B, H, Nk, d), "dk")
+    _expect(dv, (B, H, Nk, d), "dv", dk.dtype)
+    if dq_acc.dtype != torch.float32 or dq_acc.numel() != q.numel():
+        raise ValueError(f"dq_acc must hold B*H*Nq*d = {q.numel()} floats, got {dq_acc.numel()} of {dq_acc.dtype}")
+
+
 def ringx_attn_bwd_partial(q, k, v, o, lse, dO, scale: float, dq_acc=None, dk=None, dv=None, workspace=None):
     """Per-device backward step (include/ringx.h: ringx_attn_bwd_partial): q,o,dO [B,H,Nq,d], k,v [B,H,Nk,d].
     Adds these keys' contribution to dq_acc (fp32, allocated and zeroed when None); returns (dq_acc, dk, dv)."""
@@ -619,9 +647,11 @@ def ringx_attn_bwd_partial(q, k, v, o, lse, dO, scale: float, dq_acc=None, dk=No
         dq_acc = torch.zeros((B, H, Nq, d), dtype=torch.float32, device=q.device)
     dk = torch.empty_like(k) if dk is None else dk
     dv = torch.empty_like(v) if dv is None else dv
+    _expect_bwd_partial(q, k, v, o, lse, dO, dq_acc, dk, dv)
     need = lib().ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d)
     if workspace is None:
         workspace = _workspace(max(need, 256), q.device)
+    _expect_workspace(workspace, need, "ringx_attn_bwd_partial")
     st = lib().ringx_attn_bwd_partial(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
                                       _dev(dO, "dO"), _dev(dq_acc, "dq_acc"), _dev(dk, "dk"), _dev(dv, "dv"),
                                       B, H, Nq, Nk, d, scale, _DTYPES[q.dtype], workspace.data_ptr(),
@@ -638,6 +668,8 @@ def ringx_attn_bwd_partial_ex(q, k, v, o, lse, dO, scale: float, dq_acc, dk, dv,
     Nk = k.shape[2]
     if dk.dtype != dv.dtype:
         raise ValueError("dk and dv must have the same dtype")
+    _expect_bwd_partial(q, k, v, o, lse, dO, dq_acc, dk, dv)
+    _expect_workspace(workspace, lib().ringx_attn_bwd_partial_workspace_bytes(B, H, Nq, d), "ringx_attn_bwd_partial_ex")
     st = lib().ringx_attn_bwd_partial_ex(_dev(q, "q"), _dev(k, "k"), _dev(v, "v"), _dev(o, "o"), _dev(lse, "lse"),
                                          _dev(dO, "dO"), _dev(dq_acc, "dq_acc"), _dev(dk, "dk"), _dev(dv, "dv"),
                                          B, H, Nq, Nk, d, scale, _DTYPES[q.dtype], _DTYPES[dk.dtype], 1 if prepared else 0,

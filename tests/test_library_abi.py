@@ -111,6 +111,10 @@ def test_argument_validation_happens_before_any_cuda_call(lib):
     assert lib.ringx_attn_bwd(p, p, p, p, p, p, p, p, p, 1, 1, 256, 64, 256, 0.125, 0, p, 1 << 20, None) == 3
     assert lib.ringx_attn_chunk_fwd(p, p, p, p, p, 1, 1, 256, 100, 64, 0.125, 0, None) == 2   # fp32: Nk % 128
     assert lib.ringx_attn_chunk_fwd(p, p, p, p, p, 1, 1, 256, 0, 64, 0.125, 1, None) == 2
+    # the MLA dQ finalize takes what ringx_attn_bwd_partial_mla can have produced: Nq % 128 == 0 (not 64)
+    assert lib.ringx_dq_finalize_mla(p, p, 1, 1, 192, 192, None) == 2
+    assert lib.ringx_dq_finalize_mla(p, p, 1, 1, 64, 192, None) == 2
+    assert lib.ringx_dq_finalize_mla(p, p, 1, 1, 256, 128, None) == 2
 
 
 def test_product_fails_loudly_without_the_library(monkeypatch, tmp_path):
@@ -158,3 +162,28 @@ def test_binding_refuses_tensors_whose_shapes_disagree():
     qm, vm = torch.zeros(1, 2, 256, 192, dtype=torch.bfloat16), torch.zeros(1, 1, 256, 128, dtype=torch.bfloat16)
     with pytest.raises(ValueError, match="MLA shapes"):
         ringx.ringx_attn_fwd_mla(qm, qm, vm, 256, 0.1)
+    # the per-device backward steps (what ringx_dist hands slices to): keys of another length than dk / dv, a gradient
+    # accumulator of another size, a workspace smaller than the size query
+    kk = torch.zeros(1, 2, 384, 64, dtype=torch.bfloat16)
+    lse = torch.zeros(1, 2, 256)
+    acc = torch.zeros(1, 2, 256, 64)
+    ws = torch.zeros(1 << 16, dtype=torch.uint8)
+    with pytest.raises(ValueError, match="dk has shape"):
+        ringx.ringx_attn_bwd_partial_ex(q, kk, kk, q, lse, q, 0.125, acc, kk[:, :, :256], kk, ws)
+    with pytest.raises(ValueError, match="v has shape"):
+        ringx.ringx_attn_bwd_partial_ex(q, kk, kk[:, :, :128], q, lse, q, 0.125, acc, kk, kk, ws)
+    with pytest.raises(ValueError, match="dq_acc"):
+        ringx.ringx_attn_bwd_partial_ex(q, kk, kk, q, lse, q, 0.125, acc[:, :1], kk, kk, ws)
+    with pytest.raises(ValueError, match="lse has shape"):
+        ringx.ringx_attn_bwd_partial(q, kk, kk, q, lse[:, :, :128], q, 0.125, dq_acc=acc)
+    with pytest.raises(ValueError, match="workspace"):
+        ringx.ringx_attn_bwd_partial_ex(q, kk, kk, q, lse, q, 0.125, acc, kk, kk, ws[:64])
+    km, vv = torch.zeros(1, 2, 384, 192, dtype=torch.bfloat16), torch.zeros(1, 2, 384, 128, dtype=torch.bfloat16)
+    om = torch.zeros(1, 2, 256, 128, dtype=torch.bfloat16)
+    acc_t = torch.zeros(1, 2, 192, 256)
+    with pytest.raises(ValueError, match="dv has shape"):
+        ringx.ringx_attn_bwd_partial_mla(qm, km, vv, om, lse, om, 0.1, acc_t, km, vv[:, :, :256], ws)
+    with pytest.raises(ValueError, match="o has shape"):
+        ringx.ringx_attn_bwd_partial_mla(qm, km, vv, om[:, :, :128], lse, om, 0.1, acc_t, km, vv, ws)
+    with pytest.raises(ValueError, match="workspace"):
+        ringx.ringx_attn_bwd_partial_mla(qm, km, vv, om, lse, om, 0.1, acc_t, km, vv, ws[:64])
