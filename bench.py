@@ -425,6 +425,32 @@ def main():
                                   "burst": value / world / peaks["bf16_tflops"], "nominal_2250": value / world / 2250.0,
                                   "source": peaks["source"]},
         }
+        # LAST key, < 1 KB: the side figures in one place, so that a reader who keeps only the tail of the line still has the
+        # d = 64 configs, the merge kernel, the MLA widths and the deterministic backward (TFLOP/s unless named _gbs)
+        def _get(*path):
+            node = extra
+            for key in path:
+                if not isinstance(node, dict) or key not in node:
+                    return None
+                node = node[key]
+            return round(float(node), 1)
+        line["summary"] = {
+            "fwd_tflops": round(fwd_info["tflops"], 1) if fwd_info else None,
+            "bwd_tflops": round(bwd_info["tflops"], 1) if bwd_info else None,
+            "C2_fwd": _get("C2", "fwd_tflops"), "C4_fwd": _get("C4", "fwd_tflops"), "C4_bwd": _get("C4", "bwd_tflops"),
+            "C5_fwd": _get("C5", "fwd_tflops"),
+            "merge_gbs": round(merge_info["achieved"], 1) if merge_info else None,
+            "mla_fwd": _get("next_rows", "mla_dqk192_dv128_H8_N65536", "fwd_tflops"),
+            "mla_bwd": _get("next_rows", "mla_dqk192_dv128_H8_N65536", "bwd_tflops"),
+            "gqa_fwd": _get("next_rows", "gqa_16q4kv_N32768_d128", "fwd_tflops"),
+            "gqa_bwd": _get("next_rows", "gqa_16q4kv_N32768_d128", "bwd_tflops"),
+            "split_kv": _get("next_rows", "split_kv_Nq2048_Nk65536_H8_d128", "split_tflops"),
+            "bwd_partial": _get("next_rows", "bwd_partial_Nq16384_Nk16384_d128", "tflops"),
+            "det_bwd": _get("deterministic_bwd", "tflops_median"),
+            "tokeniser_gbs": _get("next_rows", "fidelity_tokens_512cube", "k4_f32", "gbs"),
+            "qkv_proj": _get("next_rows", "projections_S262144_h1024", "qkv_tflops"),
+            "block_fwd_bwd": _get("next_rows", "block_fwd_bwd_S262144_h1024", "tflops"),
+        }
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
@@ -600,16 +626,9 @@ def next_rows_measure(ringx, wl, dev, reps=5):
     out = {}
 
     def timeit(fn):
-        for _ in range(3):
-            fn()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(reps):
-            fn()
-        e1.record()
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / reps
+        # the same loop as side_measure: >= 0.5 s warm, then >= 0.5 s and >= `reps` calls timed one by one; the median, so that
+        # every figure of the line is a sustained one and reads the same way in every run
+        return float(np.median(timed_loop(fn, min_seconds=0.5, min_reps=reps)))
 
     # GQA: 16 query heads on 4 kv heads, N = 32768, d = 128, 4 passes of 8192 keys
     B, Hq, Hkv, N, d, chunk = 1, 16, 4, 32768, 128, 8192

@@ -66,11 +66,11 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
   uint64_t* kv_full = bars;          // TMA -> MMA: K_j, V_j
   uint64_t* s_full = bars + 1;       // MMA -> compute: S^T(s)
   uint64_t* dp_full = bars + 2;      // MMA -> compute: dP^T(s)
-  uint64_t* p_full = bars + 3;       // compute -> MMA: P^T(s) in TMEM, S^T(s) consumed            (256 arrivals)
-  uint64_t* ds_full = bars + 4;      // compute -> MMA: dS^T(s) in smem, dP^T(s) consumed          (256 arrivals)
+  uint64_t* p_full = bars + 3;       // compute -> MMA: P^T(s) in TMEM, S^T(s) consumed            (8 arrivals: one per warp)
+  uint64_t* ds_full = bars + 4;      // compute -> MMA: dS^T(s) in smem, dP^T(s) consumed          (8 arrivals)
   uint64_t* ds_empty = bars + 5;     // MMA -> compute: dK(s), dQ^T(s) have read dS^T(s)
   uint64_t* dq_full = bars + 6;      // MMA -> drain: both pieces of dQ^T(s) in TMEM
-  uint64_t* dq_empty = bars + 7;     // drain -> MMA: dQ^T(s) in registers                          (128 arrivals)
+  uint64_t* dq_empty = bars + 7;     // drain -> MMA: dQ^T(s) in registers                          (4 arrivals)
   uint64_t* dkv_full = bars + 8;     // MMA -> compute: dK_j, dV_j complete
   uint64_t* q_full = bars + 9;       // [kQStages]
   uint64_t* q_empty = q_full + kQStages;
@@ -94,11 +94,11 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
     mbar_init(kv_full, 1);
     mbar_init(s_full, 1);
     mbar_init(dp_full, 1);
-    mbar_init(p_full, 256);
-    mbar_init(ds_full, 256);
+    mbar_init(p_full, 8);
+    mbar_init(ds_full, 8);
     mbar_init(ds_empty, 1);
     mbar_init(dq_full, 1);
-    mbar_init(dq_empty, 128);
+    mbar_init(dq_empty, 4);
     mbar_init(dkv_full, 1);
     for (int i = 0; i < kQStages; ++i) {
       mbar_init(&q_full[i], 1);
@@ -315,7 +315,8 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       }
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive(p_full);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(p_full);          // one arrival per warp (8), as in attn_bwd_sm100.cu: 256 separate arrivals are 256 shared-memory atomics
       // ---- phase B: dS^T = P^T o (scale dP^T - scale D), bf16, to shared memory [keys][queries] (128B-swizzled rows)
       mbar_wait(dp_full, s & 1);
       if (s > 0) mbar_wait(ds_empty, (s - 1) & 1);
@@ -344,7 +345,8 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
       }
       fence_proxy_async_smem();
       tc_fence_before();
-      mbar_arrive(ds_full);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ds_full);
     }
     // ---- epilogue: dV_j (warps 0-3, 128 columns) and dK_j (warps 4-7, 192 columns), bf16, written once
     mbar_wait(dkv_full, 0);
@@ -400,7 +402,8 @@ attn_chunk_bwd_mla_kernel(const __grid_constant__ CUtensorMap map_q, const __gri
         for (int c = 0; c < 2; ++c) tmem_wait_ld_x32(r[c]);
         if (piece == 1) {
           tc_fence_before();
-          mbar_arrive(dq_empty);             // both pieces of dQ^T(s) have left TMEM: hand the columns back
+          __syncwarp();
+          if (lane == 0) mbar_arrive(dq_empty);   // both pieces of dQ^T(s) have left TMEM: hand the columns back
         }
         if (dq_qs) {
           // deterministic mode (attn_bwd_sm100.cu): int32 fixed point; here a thread is a feature row and its 64
